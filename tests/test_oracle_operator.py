@@ -1,0 +1,155 @@
+"""Operator-level pins of the CPU oracle: invariants the paper states (exact conservation, L17;
+species-uncoupled Jacobian, L75; N = Ne*Nq, Table I) and those the mathematics fixes."""
+import math
+import os
+
+import numpy as np
+import pytest
+
+from paper_2104_10000_b200 import inputs
+
+GOLD = os.path.join(os.path.dirname(__file__), "golden")
+
+
+def _rows(name):
+    return [ln.split("#")[0].split() for ln in open(os.path.join(GOLD, name)) if ln.split("#")[0].split()]
+
+
+@pytest.fixture(scope="module")
+def built(oracle):
+    """cfg0 (refined Q2, hanging nodes, 2 species) and a refined Q3 3-species case, built once."""
+    out = {}
+    wl = inputs.config(0)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z)
+    out["q2"] = (wl, sp, f) + tuple(oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0)[1:])
+    mesh = inputs.mesh_quadtree(0.0, 4.0, -4.0, 4.0, 2, 4, 1.0, 2, 2.0, 1)
+    spc = inputs._sp([(1, -1, 1, 1), (3670, 1, 0.5, 1), (7344, 2, 0.25, 1)])
+    comps = [[inputs.Component(0, 1, 1), inputs.Component(0, 0.05, 2.0, 0.7), inputs.Component(1, 0.5, 400.0),
+              inputs.Component(2, 0.25, 900.0, -0.2)]]
+    wl3 = inputs.Workload("q3-3sp", 3, mesh, spc, comps, 1e-3, 99)
+    sp3 = oracle.build_space(mesh, 3)
+    f3 = inputs.nodal_f(wl3, sp3.dof_r, sp3.dof_z)
+    out["q3"] = (wl3, sp3, f3) + tuple(oracle.build_all(mesh, 3, spc, f3, 1.0)[1:])
+    return out
+
+
+@pytest.mark.parametrize("key", ["q2", "q3"])
+def test_discrete_conservation_of_density_momentum_energy(built, key):
+    """the discretisation conserves density, momentum and energy exactly:
+    1^T C_a = 0 for every a;  sum_a m_a z^T C_a = 0;  sum_a m_a (v^2/2)^T C_a = 0
+    (nodal interpolants of 1, z, r^2+z^2 lie in Q2/Q3 and survive the constraints)."""
+    wl, sp, f, vals, Cf, mv = built[key]
+    m = wl.species.mass
+    S = wl.species.S
+    for a in range(S):
+        assert abs(Cf[a].sum()) <= 1e-13 * np.abs(Cf[a]).sum()
+    for psi in (sp.dof_z, 0.5 * (sp.dof_r ** 2 + sp.dof_z ** 2)):
+        num = abs(sum(m[a] * (psi @ Cf[a]) for a in range(S)))
+        den = sum(m[a] * np.abs(psi * Cf[a]).sum() for a in range(S))
+        assert num <= 1e-13 * den
+    # a single species alone does NOT conserve momentum/energy when others are present: the pin bites
+    assert abs(sp.dof_z @ Cf[0]) > 1e-6 * np.abs(sp.dof_z * Cf[0]).sum()
+
+
+@pytest.mark.parametrize("key", ["q2", "q3"])
+def test_jacobian_column_sums_vanish_and_Jf_equals_Cf(built, oracle, key):
+    wl, sp, f, vals, Cf, mv = built[key]
+    rows = np.repeat(np.arange(sp.n), np.diff(sp.rowptr))
+    for a in range(wl.species.S):
+        colsum = np.zeros(sp.n)
+        np.add.at(colsum, sp.colidx, vals[a])
+        assert np.abs(colsum).max() <= 1e-12 * np.abs(vals[a]).max()      # sum_a grad psi_a = 0
+        Jf = np.zeros(sp.n)
+        np.add.at(Jf, rows, vals[a] * f[a, sp.colidx])
+        # frozen-coefficient Jacobian applied to f reproduces C(f) (computed independently)
+        assert np.abs(Jf - Cf[a]).max() <= 1e-11 * np.abs(Cf[a]).max()
+
+
+def test_mass_matrix(built, oracle):
+    wl, sp, f, vals, Cf, mv = built["q3"]
+    # sum of all entries = shift * 2 pi int r dr dz = shift * pi R^2 Lz
+    assert abs(mv.sum() - math.pi * 4.0 ** 2 * 8.0) < 1e-12 * mv.sum()
+    assert abs(oracle.mass(sp, 2.5).sum() - 2.5 * mv.sum()) < 1e-12 * mv.sum()
+    rows = np.repeat(np.arange(sp.n), np.diff(sp.rowptr))
+    M = np.zeros((sp.n, sp.n)); M[rows, sp.colidx] = mv
+    assert np.abs(M - M.T).max() < 1e-14 * np.abs(M).max()
+    # 1^T M f = density of the interpolated Maxwellian (electrons: n = 1.05), to discretisation error
+    assert abs(np.ones(sp.n) @ M @ f[0] - 1.05) < 2e-2
+    wl1 = inputs.config(1)
+    sp1 = oracle.build_space(wl1.mesh, 2)
+    assert abs(oracle.mass(sp1, 1.0).sum() - 785.3981633974483) < 1e-10   # pi * 25 * 10
+
+
+@pytest.mark.parametrize("p", [2, 3])
+def test_constraints_reproduce_polynomials(oracle, p):
+    """A global polynomial of degree <= p in each variable set on the free DOFs is reproduced
+    exactly at every integration point (including through chained hanging nodes)."""
+    mesh = inputs.mesh_config3("A") if p == 3 else inputs.config(0).mesh
+    sp = oracle.build_space(mesh, p)
+    assert sp.n_constrained > 0
+    poly = lambda r, z: 1 + 0.3 * r - 0.7 * z + 0.2 * r ** p * z ** p - 0.11 * r ** (p - 1) * z + 0.05 * z ** p
+    dpr = lambda r, z: 0.3 + 0.2 * p * r ** (p - 1) * z ** p - 0.11 * (p - 1) * r ** (p - 2) * z
+    dpz = lambda r, z: -0.7 + 0.2 * p * r ** p * z ** (p - 1) - 0.11 * r ** (p - 1) + 0.05 * p * z ** (p - 1)
+    fq, dfr, dfz = oracle.fields_at_points(sp, poly(sp.dof_r, sp.dof_z)[None, :])
+    sc = np.abs(fq).max()
+    assert np.abs(fq[0] - poly(sp.r, sp.z)).max() < 1e-12 * sc
+    assert np.abs(dfr[0] - dpr(sp.r, sp.z)).max() < 1e-11 * sc
+    assert np.abs(dfz[0] - dpz(sp.r, sp.z)).max() < 1e-11 * sc
+
+
+def test_hanging_weights_golden(oracle):
+    for row in _rows("hanging_weights.txt"):
+        p, xi, w = int(row[0]), float(row[1]), np.array(row[2:], dtype=float)
+        val, _ = oracle.lagrange_1d(p, [xi])
+        assert np.allclose(val[0], w, atol=1e-15)
+
+
+def test_sizes_and_patterns(oracle):
+    """n = prod(p n_d + 1), nnz(A1) = prod[2(p+1) + (n_d-1)(2p+1) + n_d (p-1)(p+1)] on uniform
+    tensor meshes (1-D Lagrange connectivity counted by hand); N = Ne*Nq (Table I)."""
+    for k, n, nnz, N in ((1, 231, 3321, 450), (2, 1225, 29161, 2048)):
+        wl = inputs.config(k)
+        sp = oracle.build_space(wl.mesh, wl.order)
+        assert (sp.n, sp.nnz, sp.N) == (n, nnz, N)
+        assert sp.n_constrained == 0
+        assert np.all(np.diff(sp.dof_z) >= 0)
+    for grids, cells, Npaper in _rows("table1_counts.txt"):
+        assert int(grids) * int(cells) * 16 == int(Npaper)
+    sp = oracle.build_space(inputs.mesh_config3("B"), 3)
+    assert (sp.Ne, sp.N) == (308, 4928)
+    for i in range(sp.n):   # columns ascending, diagonal present
+        cols = sp.colidx[sp.rowptr[i]:sp.rowptr[i + 1]]
+        assert np.all(np.diff(cols) > 0) and i in cols
+
+
+def test_linearity_scaling_and_species_permutation(oracle):
+    wl = inputs.config(0)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z)
+    spc = wl.species
+    v1 = oracle.jacobian(sp, spc, f)
+    # J is linear in f (frozen coefficients are linear functionals of f)
+    v2 = oracle.jacobian(sp, spc, 3.0 * f)
+    assert np.abs(v2 - 3.0 * v1).max() <= 1e-13 * np.abs(v2).max()
+    # J scales with nu
+    spn = inputs.Species(spc.mass, spc.charge, spc.density, spc.temperature, spc.m0, 2.0)
+    assert np.abs(oracle.jacobian(sp, spn, f) - 2.0 * v1).max() <= 1e-13 * np.abs(v1).max()
+    # permuting species permutes the diagonal blocks
+    spp = inputs.Species(spc.mass[::-1].copy(), spc.charge[::-1].copy(), spc.density[::-1].copy(), spc.temperature[::-1].copy())
+    vp = oracle.jacobian(sp, spp, f[::-1].copy())
+    for a in range(2):
+        assert np.abs(vp[1 - a] - v1[a]).max() <= 1e-13 * np.abs(v1[a]).max()
+    # m0 is arbitrary (L42) only up to the overall nu normalisation: doubling m0 scales K by 2*2, D by 4
+    # -> J scales by 4 (nu_ab carries 1/m0^2 in physical units; here nu is held fixed)
+    sp2 = inputs.Species(spc.mass, spc.charge, spc.density, spc.temperature, 2.0, 1.0)
+    assert np.abs(oracle.jacobian(sp, sp2, f) - 4.0 * v1).max() <= 1e-13 * 4 * np.abs(v1).max()
+
+
+def test_double_and_long_double_instantiations_agree(oracle):
+    wl = inputs.config(1)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z)
+    a = oracle.jacobian(sp, wl.species, f, "ld")
+    b = oracle.jacobian(sp, wl.species, f, "d")
+    assert np.abs(a - b).max() <= 1e-12 * np.abs(a).max()
