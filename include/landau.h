@@ -1,0 +1,138 @@
+/*
+ * landau.h -- C ABI of the B200-native Landau Jacobian hot path (arxiv 2104.10000).
+ *
+ * PAPER.md = the paper's text.  The library builds, on ONE sm_100a GPU and in fp64, the
+ * frozen-coefficient Jacobian of the conservative finite-element Landau collision
+ * operator (Eq. 2, weak form Eqs. 4-8) on a 2-D axisymmetric (r,z) velocity mesh with
+ * S species, following Algorithm 1 (L109-131):
+ *
+ *   a1  f_b(q), grad f_b(q) at all N integration points                          (L101)
+ *   a2  T_D(j) = sum_b e_b^2 f_b(j),  T_K(j) = sum_b e_b^2 (m0/m_b) grad f_b(j)  (lines 5-8, Eq. 10)
+ *   a3  G_D(i) = sum_{j!=i} w_j T_D(j) U^D(i,j),  G_K(i) = sum_{j!=i} w_j U^K(i,j).T_K(j)
+ *                                                                                 (lines 3-12)
+ *   a4  K_a = nu e_a^2 (m0/m_a) G_K,  D_a = -nu e_a^2 (m0/m_a)^2 G_D;
+ *       KK = J^-1 K_a w,  DD = J^-1 D_a J^-T w                                    (lines 13-20)
+ *   a5  C_e[a][b] = sum_q ( Ehat_qa.DD_q.Ehat_qb + Ehat_qa.KK_q B_qb )           (line 23)
+ *   a6  vals_a[k] = sum over (e,a,b) of P_e[a,row k] P_e[b,col k] C_e[a][b], fixed order
+ *                                                                                 (L101, L165-167, L297)
+ *   a7  C(f)_a[i] = sum_q w grad psi_i.(K_a f_a + D_a grad f_a)   (right side of Eq. 4, = J_a f_a)
+ *   a8  mass: M[a][b] = shift sum_q w psi_a psi_b                                 (L280)
+ *
+ * U^D, U^K are Eq. 3 (L44) integrated over the azimuth (complete elliptic integrals K, E);
+ * DESIGN.md "Readings" Q1 gives the formulas, Q2 the weights: w_in = omega detJ r in a3,
+ * w = 2 pi omega detJ r in a4-a8.
+ *
+ * Discretisation conventions (part of the problem statement; the CPU oracle follows the same):
+ *   - mesh: leaves of a quadtree forest on [rmin,rmax]x[zmin,zmax], nbr x nbz level-0 cells,
+ *     2:1 FACE balanced, rmin >= 0.  Leaf (level l, ir, iz) covers
+ *     r in rmin + hr0/2^l [ir,ir+1], z in zmin + hz0/2^l [iz,iz+1].
+ *   - order p in {2,3}: tensor Lagrange elements on EQUISPACED nodes, (p+1)^2 Gauss-Legendre
+ *     points; local basis a = az (p+1) + ar; point gi = e Nq + qz (p+1) + qr (abscissae ascending).
+ *   - hanging nodes: nodes of a fine edge whose face neighbour is one level coarser and that do
+ *     not coincide with a coarse node take the coarse edge's 1-D Lagrange interpolant; chains are
+ *     closed.  Natural boundary conditions everywhere (nothing imposed at r = 0).
+ *   - unknowns: per species, the n unconstrained nodes numbered by ascending (z, r) node
+ *     coordinate; f, Cf are [S][n] species-major.
+ *   - matrix: block diagonal I_S (x) A1 (L75); one CSR pattern A1 (rows in DOF order, columns
+ *     ascending) and vals[S][nnz].
+ *
+ * General rules: every function returns 0 (LANDAU_OK) or a negative LANDAU_E* code and never
+ * throws.  "dev" pointers are CUDA device pointers, "host" pointers plain host memory.  Device
+ * entry points enqueue work on `stream` (a cudaStream_t passed as void*, NULL = default
+ * stream) and do NOT synchronise; inputs are never modified; the CALLER owns f/vals/Cf/mvals,
+ * the ctx owns pattern, gather lists, point arrays and scratch.  A ctx must not be used from two
+ * streams at once (it owns one scratch arena).  There is no CPU fallback: without a CUDA device
+ * landau_create fails with LANDAU_ECUDA.
+ */
+#ifndef LANDAU_H
+#define LANDAU_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define LANDAU_OK 0
+#define LANDAU_EINVAL (-1) /* bad argument: order, S < 1, mass <= 0, rmin < 0, mesh not a 2:1 tiling, nb > max_batch */
+#define LANDAU_ENOMEM (-2) /* host or device allocation failed */
+#define LANDAU_ECUDA (-3)  /* CUDA runtime error; text via landau_last_cuda_error() */
+
+typedef struct landau_ctx landau_ctx; /* opaque; owns all device + host state */
+
+/* Quadtree-forest leaves (host memory, borrowed for the call). */
+typedef struct {
+    double rmin, rmax, zmin, zmax;
+    int32_t nbr, nbz;       /* level-0 cells in r and z */
+    int32_t ncells;         /* number of leaves */
+    const int32_t *level;   /* [ncells] */
+    const int32_t *ir, *iz; /* [ncells] integer coordinates at the leaf's own level */
+} landau_mesh;
+
+/* Species table (host, borrowed).  The operator uses mass, charge, m0, nu (Alg. 1 lines 5-16;
+ * nu_ab = nu e_a^2 e_b^2, L83; Appendix A: nu = 1, m0 = m_e).  density/temperature are carried for
+ * the harness's Maxwellian generator only and may be NULL. */
+typedef struct {
+    int32_t S;
+    const double *mass, *charge, *density, *temperature; /* [S] */
+    double m0, nu;
+} landau_species;
+
+/* Set-up, once per mesh: DOF numbering, constraint closure, CSR pattern, gather
+ * lists, point arrays, tabulations; uploads them.  max_batch >= 1 sizes the scratch arena for
+ * landau_jacobian_batched.  On failure *out is NULL. */
+int landau_create(const landau_mesh *mesh, int order, const landau_species *species, int max_batch,
+                  landau_ctx **out);
+int landau_destroy(landau_ctx *ctx);
+
+/* Host-only part of landau_create (no CUDA device needed): runs the same set-up and returns the
+ * sizes and, where the pointer is not NULL, the CSR pattern of A1 (rowptr[n+1], colidx[nnz]) and
+ * the unknowns' node coordinates ([n] each).  Call once with NULL arrays to get the sizes. */
+int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *nnz, int64_t *N,
+                      int32_t *rowptr_host, int32_t *colidx_host, double *dof_r_host, double *dof_z_host);
+
+/* Sizes: S species, n unknowns per species, nnz of A1, N integration points, Ne cells. */
+int landau_sizes(const landau_ctx *ctx, int32_t *S, int64_t *n, int64_t *nnz, int64_t *N, int64_t *Ne);
+/* Device pointers (owned by ctx) to the CSR pattern of A1: rowptr[n+1], colidx[nnz], int32. */
+int landau_csr_pattern(const landau_ctx *ctx, const int32_t **rowptr_dev, const int32_t **colidx_dev);
+/* Host copies of the pattern (rowptr_host[n+1], colidx_host[nnz]); either may be NULL. */
+int landau_csr_pattern_host(const landau_ctx *ctx, int32_t *rowptr_host, int32_t *colidx_host);
+/* Coordinates of the unknowns' nodes (host, [n] each) -- to build nodal f. */
+int landau_dof_coords(const landau_ctx *ctx, double *r_host, double *z_host);
+/* Integration points (host, [N] each; any may be NULL): r, z, inner weight omega detJ r. */
+int landau_points(const landau_ctx *ctx, double *r_host, double *z_host, double *w_host);
+
+/* Steps a1-a3 only: G[nb][5][N] = (G_D rr, G_D rz, G_D zz, G_K r, G_K z) for nb problems.
+ * f_dev [nb][S][n].  Exposed so the O(N^2) kernel can be checked and timed alone. */
+int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *G_dev, void *stream);
+
+/* Steps a1-a7 for one problem: f_dev [S][n] -> vals_dev [S][nnz], Cf_dev [S][n].
+ * vals_dev or Cf_dev may be NULL to skip that output. */
+int landau_jacobian(landau_ctx *ctx, const double *f_dev, double *vals_dev, double *Cf_dev, void *stream);
+/* The same for nb <= max_batch independent problems on the same mesh and species (PAPER.md L244,
+ * L377): f_dev [nb][S][n] -> vals_dev [nb][S][nnz], Cf_dev [nb][S][n].  Bitwise equal to nb
+ * single calls. */
+int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double *vals_dev,
+                            double *Cf_dev, void *stream);
+/* Step a8: mvals_dev [nnz] = shift * mass matrix on the pattern A1 (same for every species). */
+int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream);
+
+/* End-to-end variant with HOST buffers (pageable or pinned): copies f to the device, runs
+ * landau_jacobian_batched on the ctx's own stream, copies vals/Cf back, and synchronises. */
+int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *vals_host, double *Cf_host);
+
+/* Number of kernel launches the ctx has enqueued since creation (for bench.py's gpu_launches). */
+int landau_launch_count(const landau_ctx *ctx, int64_t *count);
+
+/* Measurement aid, not part of the operator: runs a register-resident chain of dependent-free
+ * DFMA on every SM for `iters` iterations and returns the achieved FP64 rate in flop/s (the
+ * "alu" roofline denominator).  Synchronises. */
+int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_est);
+
+const char *landau_strerror(int code);
+const char *landau_last_cuda_error(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* LANDAU_H */

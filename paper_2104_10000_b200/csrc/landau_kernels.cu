@@ -1,0 +1,371 @@
+// Device kernels of the Landau Jacobian hot path for sm_100a (fp64).  Steps a1-a8 of
+// include/landau.h; Algorithm 1 (L109-131).  See DESIGN.md "Kernels" for the layout
+// and the roofline of each.
+//
+//   k_fields_beta   a1+a2  f -> w_in*T_D, w_in*T_K at every integration point (beta sum hoisted
+//                          out of the pair loop: it does not depend on i)
+//   k_pair          a3     all-pairs inner integral, thread owns i, j streamed through smem
+//   k_element       a4+a5  scale, transform, element matrix C_e and element vector C_e u
+//   k_gather        a6/a7  deterministic gather of element entries into CSR values / C(f)
+//   k_mass_element  a8     shift * element mass matrices (gathered by k_gather)
+//   k_dfma_probe           FP64 peak probe (measurement aid)
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+#include "landau_kernels.h"
+
+namespace landau {
+
+// ------------------------------------------------------------------------------------------------
+// fast fp64 reciprocal / rsqrt: MUFU seed (rel. err ~2^-22) + two Newton steps on the DFMA pipe.
+// Not IEEE-rounded (<= ~1 ulp), no special-case handling: arguments here are finite and > 0.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ double rcp_fast(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, e, y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
+// returns sqrt(x); *half_rsqrt = 1/(2 sqrt(x))
+__device__ __forceinline__ double sqrt_fast(double x, double *half_rsqrt) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double g = x * y, h = 0.5 * y;
+    double r = fma(-h, g, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    r = fma(-h, g, 0.5);
+    g = fma(g, r, g);
+    h = fma(h, r, h);
+    *half_rsqrt = h;
+    return g;
+}
+
+// ------------------------------------------------------------------------------------------------
+// a3: pair kernel.  PAPER.md Alg. 1 lines 3-12 (L114-121), Eqs. 7-8 (L65-67).
+//
+// Azimuth-integrated Landau tensor through the scaled AGM (DESIGN.md "Elliptic integrals on the
+// device"): with a0 = sqrt(s), b0 = sqrt(d2), q = 4 r rb = s - d2,
+//     a_{k+1} = (a_k+b_k)/2, b_{k+1} = sqrt(a_k b_k), c_{k+1} = (a_k-b_k)/2,  A = lim a_k
+//     Kt = K(m)/sqrt(s) = pi/(2A)
+//     W  = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(8 a_1^2) + (sum_{k>=2} 2^k c_k^2)/q^2     (c_1 = q/(4 a_1))
+//     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2)
+// every sum has positive terms except the last bracket (E/K, bounded cancellation ~ K/E).
+// ------------------------------------------------------------------------------------------------
+struct PairAcc { double drr, drz, dzz, kr, kz; };
+
+__device__ __forceinline__ void pair_accumulate(double ri, double zi, double inv4ri, double rj, double zj,
+                                                double invrj, double tD, double tKr, double tKz, PairAcc &acc) {
+    const double dz = zi - zj, dr = ri - rj, sr = ri + rj;
+    const double dz2 = dz * dz;
+    double d2 = fma(dr, dr, dz2);
+    const double s = fma(sr, sr, dz2);
+    const bool self = !(d2 > 0.0);   // coincident pair (j == i): contributes nothing (reading Q3)
+    if (self) d2 = 1.0;
+    const double q = 4.0 * ri * rj;
+    const double invq = inv4ri * invrj;
+
+    double h;
+    double a = sqrt_fast(s, &h);
+    double b = sqrt_fast(d2, &h);
+    // step 1
+    double an = 0.5 * (a + b);
+    b = sqrt_fast(a * b, &h);
+    a = an;
+    const double inva1 = rcp_fast(a);
+    double wsum = 0.0, pw = 4.0;
+#pragma unroll 1
+    for (int it = 0; it < 8; ++it) {
+        const double c = 0.5 * (a - b);
+        an = 0.5 * (a + b);
+        wsum = fma(pw * c, c, wsum);
+        pw += pw;
+        const bool done = c <= 1.0e-8 * a;
+        if (__all_sync(0xffffffffu, done)) { a = an; break; }
+        b = sqrt_fast(a * b, &h);
+        a = an;
+    }
+    const double Kt = 1.5707963267948966 * rcp_fast(a);
+    const double W = fma(0.125 * inva1, inva1, wsum * invq * invq);
+    const double invs = rcp_fast(s);
+    const double invd2 = rcp_fast(d2);
+    double Pss = 16.0 * Kt * W;
+    double Pc = 4.0 * Kt * fma(q, W, 1.0) * invs;
+    double P0 = 2.0 * Kt * (s + d2 - q * q * W) * invs * invd2;
+    if (self) { Pss = 0.0; Pc = 0.0; P0 = 0.0; }
+
+    const double rirj = ri * rj;
+    const double UDrr = fma(rj * rj, Pss, dz2 * P0);
+    const double UDrz = -dz * fma(dr, P0, rj * Pc);
+    const double UDzz = fma(dr * dr, P0, 2.0 * rirj * Pc);
+    const double UKrr = fma(dz2, P0 - Pc, rirj * Pss);
+    const double UKzr = dz * fma(-dr, P0, ri * Pc);
+    acc.drr = fma(tD, UDrr, acc.drr);
+    acc.drz = fma(tD, UDrz, acc.drz);
+    acc.dzz = fma(tD, UDzz, acc.dzz);
+    acc.kr = fma(UKrr, tKr, fma(UDrz, tKz, acc.kr));
+    acc.kz = fma(UKzr, tKr, fma(UDzz, tKz, acc.kz));
+}
+
+// Deterministic summation order: the j range is cut into chunks of
+// PAIR_CHUNK points from j = 0; each chunk's partial sum starts from zero and the chunk partials
+// are added in chunk order.  Both launch shapes below follow that order, so a batched build is
+// bitwise equal to single builds.
+//
+// SPLIT = false (batch fills the GPU): grid = (ceil(N/PAIR_THREADS), 1, nb); each thread owns one
+//   i, streams ALL j through shared memory in tiles of PAIR_TILE and writes G[b][5][N].
+// SPLIT = true (few problems): grid = (ceil(N/PAIR_THREADS), nchunks, nb); each block does one
+//   chunk and writes its partial to Gpart[b][chunk][5][N]; k_element / k_sum_partials add them.
+// r,z,invr [N] are shared by the batch; T[b][3][N] = w_in * (T_D, T_Kr, T_Kz).
+template <bool SPLIT>
+__global__ void __launch_bounds__(PAIR_THREADS)
+k_pair(int N, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
+       const double *__restrict__ T, double *__restrict__ Gout) {
+    constexpr int TILE = SPLIT ? PAIR_CHUNK : PAIR_TILE;
+    __shared__ double s_r[TILE], s_z[TILE], s_ir[TILE], s_td[TILE], s_tr[TILE], s_tz[TILE];
+    const int b = blockIdx.z;
+    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
+    const int ic = i < N ? i : N - 1;
+    const double ri = r[ic], zi = z[ic];
+    const double inv4ri = 0.25 * invr[ic];
+    const double *Tb = T + (size_t)b * 3 * N;
+    PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
+    const int j0 = SPLIT ? blockIdx.y * PAIR_CHUNK : 0;
+    const int j1 = SPLIT ? min(N, j0 + PAIR_CHUNK) : N;
+    for (int jt = j0; jt < j1; jt += TILE) {
+        const int cnt = min(TILE, j1 - jt);
+        __syncthreads();
+        for (int t = threadIdx.x; t < cnt; t += PAIR_THREADS) {
+            s_r[t] = r[jt + t]; s_z[t] = z[jt + t]; s_ir[t] = invr[jt + t];
+            s_td[t] = Tb[jt + t]; s_tr[t] = Tb[N + jt + t]; s_tz[t] = Tb[2 * N + jt + t];
+        }
+        __syncthreads();
+        for (int c0 = 0; c0 < cnt; c0 += PAIR_CHUNK) {
+            PairAcc part = {0.0, 0.0, 0.0, 0.0, 0.0};
+            const int c1 = min(cnt, c0 + PAIR_CHUNK);
+            for (int t = c0; t < c1; ++t)
+                pair_accumulate(ri, zi, inv4ri, s_r[t], s_z[t], s_ir[t], s_td[t], s_tr[t], s_tz[t], part);
+            acc.drr += part.drr; acc.drz += part.drz; acc.dzz += part.dzz; acc.kr += part.kr; acc.kz += part.kz;
+        }
+    }
+    if (i < N) {
+        double *G = Gout + (SPLIT ? ((size_t)b * gridDim.y + blockIdx.y) : (size_t)b) * 5 * N;
+        G[i] = acc.drr; G[N + i] = acc.drz; G[2 * N + i] = acc.dzz; G[3 * N + i] = acc.kr; G[4 * N + i] = acc.kz;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a1 + a2: field values at the integration points and the beta sums (L101, Alg. 1 lines 5-8,
+// Eq. 10).  grid = (ceil(Ne/EPB), nb), block = (Nq, EPB).  Thread (q, e): local node a = q
+// gathers u_a = sum P_e[a,d] f_b[d]; then f = B u, grad f = J^-T (E u).
+// Output T[b][3][N] = w_in * (T_D, T_Kr, T_Kz): the weight of the inner sum is folded in here.
+// ------------------------------------------------------------------------------------------------
+constexpr int FIELD_EPB = 8;
+
+__global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, double *__restrict__ T) {
+    __shared__ double s_u[FIELD_EPB][16];
+    const int b = blockIdx.y;
+    const int e = blockIdx.x * FIELD_EPB + threadIdx.y;
+    const int q = threadIdx.x;
+    const bool valid = e < ds.Ne;
+    const int Nb = ds.Nb;
+    const double *fb = f + (size_t)b * ds.S * ds.n;
+    double tD = 0.0, tKr = 0.0, tKz = 0.0;
+    double ijr = 0.0, ijz = 0.0;
+    if (valid) { ijr = ds.invJ[2 * e]; ijz = ds.invJ[2 * e + 1]; }
+    for (int sp = 0; sp < ds.S; ++sp) {
+        if (valid) {
+            double u = 0.0;
+            const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
+            for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
+            s_u[threadIdx.y][q] = u;
+        }
+        __syncthreads();
+        if (valid) {
+            double fq = 0.0, g0 = 0.0, g1 = 0.0;
+            for (int a = 0; a < Nb; ++a) {
+                const double u = s_u[threadIdx.y][a];
+                fq = fma(ds.B[q * Nb + a], u, fq);
+                g0 = fma(ds.E0[q * Nb + a], u, g0);
+                g1 = fma(ds.E1[q * Nb + a], u, g1);
+            }
+            const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
+            tD = fma(e2, fq, tD);
+            tKr = fma(em, ijr * g0, tKr);
+            tKz = fma(em, ijz * g1, tKz);
+        }
+        __syncthreads();
+    }
+    if (valid) {
+        const int gi = e * ds.Nq + q;
+        const double w = ds.w_in[gi];
+        double *Tb = T + (size_t)b * 3 * ds.N;
+        Tb[gi] = w * tD; Tb[ds.N + gi] = w * tKr; Tb[2 * ds.N + gi] = w * tKz;
+    }
+}
+
+// ------------------------------------------------------------------------------------------------
+// a4 + a5 (+ element part of a7): Alg. 1 lines 13-23 (L122-131).  grid = (Ne, S, nb),
+// block = Nb*Nb threads, thread (a,b) owns C_e[a][b].  Partial G over the j splits are summed
+// here in fixed order.  Also writes ce = C_e u (u = P_e f_alpha), the element vector of C(f).
+// ------------------------------------------------------------------------------------------------
+__global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gpart,
+                          double *__restrict__ Ce, double *__restrict__ ce) {
+    __shared__ double s_c[16][5];
+    __shared__ double s_B[256], s_E0[256], s_E1[256], s_Ce[256], s_u[16];
+    const int e = blockIdx.x, sp = blockIdx.y, b = blockIdx.z;
+    const int Nb = ds.Nb, Nq = ds.Nq, N = ds.N;
+    const int tid = threadIdx.x;
+    s_B[tid] = ds.B[tid]; s_E0[tid] = ds.E0[tid]; s_E1[tid] = ds.E1[tid];
+    if (tid < Nq) {
+        const int gi = e * Nq + tid;
+        double g[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        for (int js = 0; js < jsplit; ++js) {
+            const double *G = Gpart + ((size_t)b * jsplit + js) * 5 * N;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) g[c] += G[c * N + gi];
+        }
+        const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1], w = ds.w_out[gi];
+        const double kf = ds.kfac[sp] * w, df = ds.dfac[sp] * w;
+        s_c[tid][0] = ir * ir * df * g[0];
+        s_c[tid][1] = ir * iz * df * g[1];
+        s_c[tid][2] = iz * iz * df * g[2];
+        s_c[tid][3] = ir * kf * g[3];
+        s_c[tid][4] = iz * kf * g[4];
+    } else if (tid < Nq + Nb) {
+        const int a = tid - Nq;
+        const double *fa = f + ((size_t)b * ds.S + sp) * ds.n;
+        double u = 0.0;
+        for (int t = ds.lptr[e * Nb + a]; t < ds.lptr[e * Nb + a + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
+        s_u[a] = u;
+    }
+    __syncthreads();
+    const int a = tid / Nb, bb = tid % Nb;
+    double acc = 0.0;
+    for (int q = 0; q < Nq; ++q) {
+        const double e0a = s_E0[q * Nb + a], e1a = s_E1[q * Nb + a];
+        const double e0b = s_E0[q * Nb + bb], e1b = s_E1[q * Nb + bb], bq = s_B[q * Nb + bb];
+        const double t0 = fma(s_c[q][0], e0b, s_c[q][1] * e1b);
+        const double t1 = fma(s_c[q][1], e0b, s_c[q][2] * e1b);
+        const double tk = fma(e0a, s_c[q][3], e1a * s_c[q][4]);
+        acc += fma(e0a, t0, fma(e1a, t1, tk * bq));
+    }
+    const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
+    Ce[mat * Nb * Nb + tid] = acc;
+    s_Ce[tid] = acc;
+    __syncthreads();
+    if (tid < Nb) {
+        double v = 0.0;
+        for (int c = 0; c < Nb; ++c) v = fma(s_Ce[tid * Nb + c], s_u[c], v);
+        ce[mat * Nb + tid] = v;
+    }
+}
+
+// a8: element mass matrices, M_e[a][b] = shift sum_q w_out B_qa B_qb (L280).  grid = Ne.
+__global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict__ Ce) {
+    const int e = blockIdx.x, Nb = ds.Nb, tid = threadIdx.x;
+    const int a = tid / Nb, b = tid % Nb;
+    double acc = 0.0;
+    for (int q = 0; q < ds.Nq; ++q) acc = fma(ds.w_out[e * ds.Nq + q] * ds.B[q * Nb + a], ds.B[q * Nb + b], acc);
+    Ce[(size_t)e * Nb * Nb + tid] = shift * acc;
+}
+
+// a6 / a7: out[m][k] = sum_{t in [ptr[k], ptr[k+1])} w[t] * src[m*stride + idx[t]], fixed order
+// (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), nmat).
+__global__ void k_gather(int K, size_t stride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+                         const double *__restrict__ w, const double *__restrict__ src, double *__restrict__ out) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= K) return;
+    const double *s = src + (size_t)blockIdx.y * stride;
+    double acc = 0.0;
+    for (int t = ptr[k]; t < ptr[k + 1]; ++t) acc = fma(w[t], s[idx[t]], acc);
+    out[(size_t)blockIdx.y * K + k] = acc;
+}
+
+// Sums the j-split partials (used by landau_inner_integral when jsplit > 1).  grid over 5N x nb.
+__global__ void k_sum_partials(int n5, int jsplit, const double *__restrict__ Gpart, double *__restrict__ G) {
+    const int t = blockIdx.x * blockDim.x + threadIdx.x;
+    if (t >= n5) return;
+    const size_t b = blockIdx.y;
+    double acc = 0.0;
+    for (int js = 0; js < jsplit; ++js) acc += Gpart[(b * jsplit + js) * n5 + t];
+    G[b * n5 + t] = acc;
+}
+
+// FP64 peak probe: 8 independent DFMA chains per thread, all operands in registers.
+__global__ void k_dfma_probe(int iters, double *out) {
+    double x0 = threadIdx.x * 1e-9, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
+    const double a = 0.999999999, c = 1e-12;
+    for (int i = 0; i < iters; ++i) {
+        x0 = fma(x0, a, c); x1 = fma(x1, a, c); x2 = fma(x2, a, c); x3 = fma(x3, a, c);
+        x4 = fma(x4, a, c); x5 = fma(x5, a, c); x6 = fma(x6, a, c); x7 = fma(x7, a, c);
+    }
+    const double s = x0 + x1 + x2 + x3 + x4 + x5 + x6 + x7;
+    if (s == 12345.678) out[0] = s;  // keep the chains alive
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+int pair_chunks(int N) { return (N + PAIR_CHUNK - 1) / PAIR_CHUNK; }
+
+// Split the j range over blocks when the batch alone cannot give every SM four 128-thread blocks.
+bool pair_use_split(int N, int nb, int num_sms) {
+    const long long itiles = (N + PAIR_THREADS - 1) / PAIR_THREADS;
+    return itiles * nb < 4LL * num_sms;
+}
+
+int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
+    dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
+    k_fields_beta<<<grid, block, 0, st>>>(ds, f, T);
+    return 1;
+}
+
+int launch_pair(const DeviceSpace &ds, int nb, bool split, const double *T, double *G, cudaStream_t st) {
+    dim3 grid((ds.N + PAIR_THREADS - 1) / PAIR_THREADS, split ? pair_chunks(ds.N) : 1, nb);
+    if (split) k_pair<true><<<grid, PAIR_THREADS, 0, st>>>(ds.N, ds.r, ds.z, ds.invr, T, G);
+    else k_pair<false><<<grid, PAIR_THREADS, 0, st>>>(ds.N, ds.r, ds.z, ds.invr, T, G);
+    return 1;
+}
+
+int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
+                   cudaStream_t st) {
+    dim3 grid(ds.Ne, ds.S, nb);
+    k_element<<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce);
+    return 1;
+}
+
+int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st) {
+    dim3 grid((ds.nnz + 255) / 256, nmat);
+    k_gather<<<grid, 256, 0, st>>>(ds.nnz, (size_t)ds.Ne * ds.Nb * ds.Nb, ds.gptr, ds.gidx, ds.gw, Ce, vals);
+    return 1;
+}
+
+int launch_gather_cf(const DeviceSpace &ds, int nvec, const double *ce, double *Cf, cudaStream_t st) {
+    dim3 grid((ds.n + 255) / 256, nvec);
+    k_gather<<<grid, 256, 0, st>>>(ds.n, (size_t)ds.Ne * ds.Nb, ds.cptr, ds.cidx, ds.cw, ce, Cf);
+    return 1;
+}
+
+int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st) {
+    k_mass_element<<<ds.Ne, ds.Nb * ds.Nb, 0, st>>>(ds, shift, Ce);
+    return 1;
+}
+
+int launch_sum_partials(const DeviceSpace &ds, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
+    const int n5 = 5 * ds.N;
+    dim3 grid((n5 + 255) / 256, nb);
+    k_sum_partials<<<grid, 256, 0, st>>>(n5, jsplit, Gpart, G);
+    return 1;
+}
+
+int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st) {
+    k_dfma_probe<<<blocks, threads, 0, st>>>(iters, out);
+    return 1;
+}
+
+}  // namespace landau

@@ -1,0 +1,54 @@
+// Launchers of the device kernels (landau_kernels.cu); called by the C-ABI layer only.
+#pragma once
+#include <cuda_runtime.h>
+
+#include <cstdint>
+
+namespace landau {
+
+constexpr int PAIR_THREADS = 128;  // i points per block of the pair kernel
+constexpr int PAIR_TILE = 256;     // j points staged in shared memory per tile (batch shape)
+constexpr int PAIR_CHUNK = 64;     // summation granule: chunk partials are added in chunk order
+constexpr int MAX_SPECIES = 16;
+
+// Device-resident description of one mesh/order/species set (all pointers device memory,
+// shared by every problem of a batch).
+struct DeviceSpace {
+    int p, Nq, Nb, S;
+    int N, Ne, n, nnz;
+    const double *r, *z, *invr, *w_in, *w_out;  // [N]
+    const double *invJ;                          // [Ne][2]
+    const double *B, *E0, *E1;                   // [Nq][Nb]
+    const int32_t *lptr, *ldof; const double *lw;
+    const int32_t *rowptr, *colidx;
+    const int32_t *gptr, *gidx; const double *gw;
+    const int32_t *cptr, *cidx; const double *cw;
+    double e2[MAX_SPECIES];    // e_b^2
+    double m0m[MAX_SPECIES];   // m0/m_b
+    double kfac[MAX_SPECIES];  // nu e_a^2 (m0/m_a)
+    double dfac[MAX_SPECIES];  // -nu e_a^2 (m0/m_a)^2
+};
+
+// Scratch for up to max_batch problems.
+struct Scratch {
+    double *T;      // [nb][3][N]
+    double *G;      // [nb][5][N] (batch shape) or [nb][nchunks][5][N] (split shape)
+    double *Ce;     // [nb][S][Ne][Nb*Nb]
+    double *ce;     // [nb][S][Ne][Nb]
+};
+
+// each returns the number of kernels launched
+int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
+int launch_pair(const DeviceSpace &ds, int nb, bool split, const double *T, double *G, cudaStream_t st);
+int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce,
+                   double *ce, cudaStream_t st);
+int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st);
+int launch_gather_cf(const DeviceSpace &ds, int nvec, const double *ce, double *Cf, cudaStream_t st);
+int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
+int launch_sum_partials(const DeviceSpace &ds, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
+int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
+
+int pair_chunks(int N);
+bool pair_use_split(int N, int nb, int num_sms);
+
+}  // namespace landau
