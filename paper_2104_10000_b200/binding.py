@@ -1,0 +1,219 @@
+"""Thin ctypes binding of include/landau.h -- argument marshalling only.
+
+Every step of the path runs in the CUDA kernels behind the C ABI; torch is used here only for
+device memory and streams.  There is no fallback: if the shared library is missing or fails to
+load, importing names from it raises.
+"""
+from __future__ import annotations
+
+import ctypes
+import os
+from ctypes import POINTER, c_double, c_int, c_int32, c_int64, c_void_p
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(_HERE, "liblandau_b200.so")
+
+LANDAU_OK, LANDAU_EINVAL, LANDAU_ENOMEM, LANDAU_ECUDA = 0, -1, -2, -3
+
+
+class landau_mesh(ctypes.Structure):
+    _fields_ = [("rmin", c_double), ("rmax", c_double), ("zmin", c_double), ("zmax", c_double),
+                ("nbr", c_int32), ("nbz", c_int32), ("ncells", c_int32),
+                ("level", POINTER(c_int32)), ("ir", POINTER(c_int32)), ("iz", POINTER(c_int32))]
+
+
+class landau_species(ctypes.Structure):
+    _fields_ = [("S", c_int32), ("mass", POINTER(c_double)), ("charge", POINTER(c_double)),
+                ("density", POINTER(c_double)), ("temperature", POINTER(c_double)),
+                ("m0", c_double), ("nu", c_double)]
+
+
+_lib = None
+
+# every symbol include/landau.h declares: name -> (restype, argtypes)
+SIGNATURES = {
+    "landau_create": (c_int, [POINTER(landau_mesh), c_int, POINTER(landau_species), c_int, POINTER(c_void_p)]),
+    "landau_destroy": (c_int, [c_void_p]),
+    "landau_setup_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64),
+                                  POINTER(c_int32), POINTER(c_int32), POINTER(c_double), POINTER(c_double)]),
+    "landau_sizes": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]),
+    "landau_csr_pattern": (c_int, [c_void_p, POINTER(c_void_p), POINTER(c_void_p)]),
+    "landau_csr_pattern_host": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_int32)]),
+    "landau_dof_coords": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double)]),
+    "landau_points": (c_int, [c_void_p, POINTER(c_double), POINTER(c_double), POINTER(c_double)]),
+    "landau_inner_integral": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
+    "landau_jacobian": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "landau_jacobian_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
+    "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
+    "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
+    "landau_fp64_peak_probe": (c_int, [c_int, POINTER(c_double), POINTER(c_double)]),
+    "landau_strerror": (ctypes.c_char_p, [c_int]),
+    "landau_last_cuda_error": (ctypes.c_char_p, []),
+}
+
+
+def lib():
+    """Loads liblandau_b200.so (built in-tree by paper_2104_10000_b200.build); raises if absent."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2104_10000_b200.build` "
+                               "(there is no CPU fallback)")
+        L = ctypes.CDLL(LIB_PATH)
+        for name, (res, args) in SIGNATURES.items():
+            fn = getattr(L, name)
+            fn.restype, fn.argtypes = res, args
+        _lib = L
+    return _lib
+
+
+class LandauError(RuntimeError):
+    def __init__(self, code: int):
+        L = lib()
+        msg = L.landau_strerror(code).decode()
+        detail = L.landau_last_cuda_error().decode()
+        super().__init__(f"landau error {code}: {msg}" + (f" ({detail})" if detail else ""))
+        self.code = code
+
+
+def _check(code: int) -> None:
+    if code != LANDAU_OK:
+        raise LandauError(code)
+
+
+def _i32(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def _f64(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _mesh_struct(mesh):
+    lev, ir, iz = _i32(mesh.level), _i32(mesh.ir), _i32(mesh.iz)
+    m = landau_mesh(float(mesh.rmin), float(mesh.rmax), float(mesh.zmin), float(mesh.zmax), int(mesh.nbr), int(mesh.nbz),
+                    int(lev.shape[0]), lev.ctypes.data_as(POINTER(c_int32)), ir.ctypes.data_as(POINTER(c_int32)),
+                    iz.ctypes.data_as(POINTER(c_int32)))
+    return m, (lev, ir, iz)
+
+
+def _dp(a):
+    return a.ctypes.data_as(POINTER(c_double))
+
+
+def landau_setup_host(mesh, order: int):
+    """Host-only set-up: returns dict(n, nnz, N, rowptr, colidx, dof_r, dof_z).  No GPU needed."""
+    L = lib()
+    m, keep = _mesh_struct(mesh)
+    n, nnz, N = c_int64(), c_int64(), c_int64()
+    _check(L.landau_setup_host(ctypes.byref(m), order, ctypes.byref(n), ctypes.byref(nnz), ctypes.byref(N), None, None, None, None))
+    rowptr, colidx = np.zeros(n.value + 1, np.int32), np.zeros(nnz.value, np.int32)
+    dr, dz = np.zeros(n.value), np.zeros(n.value)
+    _check(L.landau_setup_host(ctypes.byref(m), order, None, None, None, rowptr.ctypes.data_as(POINTER(c_int32)),
+                               colidx.ctypes.data_as(POINTER(c_int32)), _dp(dr), _dp(dz)))
+    return dict(n=n.value, nnz=nnz.value, N=N.value, rowptr=rowptr, colidx=colidx, dof_r=dr, dof_z=dz)
+
+
+def landau_fp64_peak_probe(iters: int = 1 << 16):
+    L = lib()
+    fl, mhz = c_double(), c_double()
+    _check(L.landau_fp64_peak_probe(iters, ctypes.byref(fl), ctypes.byref(mhz)))
+    return fl.value, mhz.value
+
+
+def _stream_ptr(stream):
+    import torch
+    s = torch.cuda.current_stream() if stream is None else stream
+    return c_void_p(s.cuda_stream)
+
+
+class LandauContext:
+    """Owns a landau_ctx.  Methods mirror the C entry points one to one (same names without the
+    prefix); tensors are torch CUDA float64, contiguous."""
+
+    def __init__(self, mesh, order: int, species, max_batch: int = 1):
+        L = lib()
+        m, keep = _mesh_struct(mesh)
+        mass, charge = _f64(species.mass), _f64(species.charge)
+        dens, temp = _f64(species.density), _f64(species.temperature)
+        sp = landau_species(int(mass.shape[0]), _dp(mass), _dp(charge), _dp(dens), _dp(temp), float(species.m0), float(species.nu))
+        h = c_void_p()
+        _check(L.landau_create(ctypes.byref(m), order, ctypes.byref(sp), int(max_batch), ctypes.byref(h)))
+        self._h = h
+        S, n, nnz, N, Ne = c_int32(), c_int64(), c_int64(), c_int64(), c_int64()
+        _check(L.landau_sizes(h, ctypes.byref(S), ctypes.byref(n), ctypes.byref(nnz), ctypes.byref(N), ctypes.byref(Ne)))
+        self.S, self.n, self.nnz, self.N, self.Ne = S.value, n.value, nnz.value, N.value, Ne.value
+        self.max_batch = int(max_batch)
+
+    def destroy(self):
+        if getattr(self, "_h", None):
+            lib().landau_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.destroy()
+        except Exception:
+            pass
+
+    def csr_pattern_host(self):
+        rowptr, colidx = np.zeros(self.n + 1, np.int32), np.zeros(self.nnz, np.int32)
+        _check(lib().landau_csr_pattern_host(self._h, rowptr.ctypes.data_as(POINTER(c_int32)), colidx.ctypes.data_as(POINTER(c_int32))))
+        return rowptr, colidx
+
+    def csr_pattern(self):
+        """Device pointers (ints) of rowptr/colidx owned by the ctx."""
+        a, b = c_void_p(), c_void_p()
+        _check(lib().landau_csr_pattern(self._h, ctypes.byref(a), ctypes.byref(b)))
+        return a.value, b.value
+
+    def dof_coords(self):
+        r, z = np.zeros(self.n), np.zeros(self.n)
+        _check(lib().landau_dof_coords(self._h, _dp(r), _dp(z)))
+        return r, z
+
+    def points(self):
+        r, z, w = np.zeros(self.N), np.zeros(self.N), np.zeros(self.N)
+        _check(lib().landau_points(self._h, _dp(r), _dp(z), _dp(w)))
+        return r, z, w
+
+    @staticmethod
+    def _ptr(t, shape):
+        import torch
+        assert t.is_cuda and t.dtype == torch.float64 and t.is_contiguous() and tuple(t.shape) == tuple(shape), (t.shape, shape)
+        return c_void_p(t.data_ptr())
+
+    def inner_integral(self, f, G, stream=None):
+        nb = f.shape[0]
+        _check(lib().landau_inner_integral(self._h, nb, self._ptr(f, (nb, self.S, self.n)), self._ptr(G, (nb, 5, self.N)), _stream_ptr(stream)))
+
+    def jacobian(self, f, vals=None, Cf=None, stream=None):
+        pv = self._ptr(vals, (self.S, self.nnz)) if vals is not None else None
+        pc = self._ptr(Cf, (self.S, self.n)) if Cf is not None else None
+        _check(lib().landau_jacobian(self._h, self._ptr(f, (self.S, self.n)), pv, pc, _stream_ptr(stream)))
+
+    def jacobian_batched(self, f, vals=None, Cf=None, stream=None):
+        nb = f.shape[0]
+        pv = self._ptr(vals, (nb, self.S, self.nnz)) if vals is not None else None
+        pc = self._ptr(Cf, (nb, self.S, self.n)) if Cf is not None else None
+        _check(lib().landau_jacobian_batched(self._h, nb, self._ptr(f, (nb, self.S, self.n)), pv, pc, _stream_ptr(stream)))
+
+    def mass(self, shift, mvals, stream=None):
+        _check(lib().landau_mass(self._h, float(shift), self._ptr(mvals, (self.nnz,)), _stream_ptr(stream)))
+
+    def jacobian_host(self, f_host, vals_host=None, Cf_host=None):
+        """Host buffers: numpy arrays or pinned CPU torch tensors (float64, contiguous)."""
+        def hp(a):
+            if a is None:
+                return None
+            return c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
+        nb = f_host.shape[0]
+        _check(lib().landau_jacobian_host(self._h, nb, hp(f_host), hp(vals_host), hp(Cf_host)))
+
+    def launch_count(self) -> int:
+        c = c_int64()
+        _check(lib().landau_launch_count(self._h, ctypes.byref(c)))
+        return c.value

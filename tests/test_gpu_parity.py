@@ -1,0 +1,187 @@
+"""GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
+the same seeded inputs.  Tolerance (BASELINE.json north_star; reading R): per species
+block max|x_gpu - x_ref| / max|x_ref| <= 1e-10 for Jacobian values and C(f); conservation
+residuals of the GPU's C(f) < 1e-12 relative; integer work (pattern) bit-exact."""
+import numpy as np
+import pytest
+
+from paper_2104_10000_b200 import inputs
+
+pytestmark = pytest.mark.gpu
+TOL = 1e-10
+
+
+@pytest.fixture(scope="module")
+def gpu():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.skip("no CUDA device")
+    from paper_2104_10000_b200 import binding
+    binding.lib()   # raises if the extension is missing: no silent fallback
+    return binding
+
+
+def block_err(x, ref):
+    return np.abs(x - ref).max() / np.abs(ref).max()
+
+
+def entry_err(x, ref):
+    big = np.abs(ref) > 1e-8 * np.abs(ref).max()
+    return (np.abs(x - ref)[big] / np.abs(ref)[big]).max()
+
+
+def conservation_residuals(dof_r, dof_z, mass, Cf):
+    S = Cf.shape[0]
+    out = [abs(Cf[a].sum()) / np.abs(Cf[a]).sum() for a in range(S)]
+    for psi in (dof_z, 0.5 * (dof_r ** 2 + dof_z ** 2)):
+        num = abs(sum(mass[a] * (psi @ Cf[a]) for a in range(S)))
+        den = sum(mass[a] * np.abs(psi * Cf[a]).sum() for a in range(S))
+        out.append(num / den)
+    return max(out)
+
+
+def run_gpu(gpu, wl, problems, max_batch=None, batched=True):
+    import torch
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, max_batch or len(problems))
+    r, z = ctx.dof_coords()
+    f = np.stack([inputs.nodal_f(wl, r, z, b) for b in problems])
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.full((len(problems), ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+    Cf = torch.full((len(problems), ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+    if batched:
+        ctx.jacobian_batched(fd, vals, Cf)
+    else:
+        for k in range(len(problems)):
+            ctx.jacobian(fd[k], vals[k], Cf[k])
+    mv = torch.zeros(ctx.nnz, dtype=torch.float64, device="cuda")
+    ctx.mass(1.7, mv)
+    torch.cuda.synchronize()
+    return ctx, f, vals.cpu().numpy(), Cf.cpu().numpy(), mv.cpu().numpy()
+
+
+def check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, problems):
+    sp = oracle.build_space(wl.mesh, wl.order)
+    rowptr, colidx = ctx.csr_pattern_host()
+    assert np.array_equal(rowptr, sp.rowptr) and np.array_equal(colidx, sp.colidx)
+    r, z = ctx.dof_coords()
+    assert np.abs(r - sp.dof_r).max() < 1e-14 and np.abs(z - sp.dof_z).max() < 1e-14
+    worst = 0.0
+    for k in range(len(problems)):
+        _, ovals, oCf, omv = oracle.build_all(wl.mesh, wl.order, wl.species, f[k], 1.7)
+        for a in range(wl.species.S):
+            ev, ec = block_err(vals[k, a], ovals[a]), block_err(Cf[k, a], oCf[a])
+            assert ev <= TOL and ec <= TOL, (wl.name, k, a, ev, ec)
+            assert entry_err(vals[k, a], ovals[a]) <= 1e-7
+            worst = max(worst, ev, ec)
+        assert block_err(mv, omv) <= 1e-13
+        assert conservation_residuals(sp.dof_r, sp.dof_z, wl.species.mass, Cf[k]) < 1e-12
+    return worst
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2])
+def test_small_configs_full_parity(gpu, oracle, cfg):
+    wl = inputs.config(cfg)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    print(f"{wl.name}: worst block error {worst:.2e}")
+
+
+@pytest.mark.parametrize("cfg,variant", [(3, "A"), (3, "B"), (4, "B")])
+def test_refined_configs_full_parity(gpu, oracle, cfg, variant):
+    wl = inputs.config(cfg, variant=variant)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    print(f"{wl.name}: worst block error {worst:.2e}")
+
+
+def test_inner_integral_parity(gpu, oracle):
+    """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
+    import torch
+    wl = inputs.config(2)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 1)
+    r, z = ctx.dof_coords()
+    f = inputs.nodal_f(wl, r, z)
+    G = torch.zeros((1, 5, ctx.N), dtype=torch.float64, device="cuda")
+    ctx.inner_integral(torch.from_numpy(f[None]).cuda(), G)
+    G = G.cpu().numpy()[0]
+    sp = oracle.build_space(wl.mesh, wl.order)
+    pr, pz, pw = ctx.points()
+    assert np.abs(pr - sp.r).max() < 1e-14 and np.abs(pz - sp.z).max() < 1e-14 and np.abs(pw - sp.w_in).max() < 1e-15
+    _, _, (GD, GK) = oracle.coefficients(sp, wl.species, f)
+    ref = np.concatenate([GD.T, GK.T])
+    for c in range(5):
+        assert block_err(G[c], ref[c]) <= 1e-12, c
+
+
+def test_config5_batched_full_size(gpu, oracle):
+    """BASELINE config 5 at full size (512 problems, the launch shape bench.py times): sampled
+    problems against the oracle one by one; conservation (holds at any size) on all 512."""
+    wl = inputs.config(5)
+    problems = list(range(wl.nbatch))
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, problems)
+    assert np.isfinite(vals).all() and np.isfinite(Cf).all()
+    sp = oracle.build_space(wl.mesh, wl.order)
+    for k in problems:
+        assert conservation_residuals(sp.dof_r, sp.dof_z, wl.species.mass, Cf[k]) < 1e-12, k
+    # extremes of bulk temperature + first/last
+    Tb = [wl.components[b][0].T for b in problems]
+    sample = sorted({0, wl.nbatch - 1, int(np.argmin(Tb)), int(np.argmax(Tb))})
+    for k in sample:
+        _, ovals, oCf, _ = oracle.build_all(wl.mesh, wl.order, wl.species, f[k], 1.0)
+        for a in range(2):
+            assert block_err(vals[k, a], ovals[a]) <= TOL, (k, a)
+            assert block_err(Cf[k, a], oCf[a]) <= TOL, (k, a)
+
+
+def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu):
+    wl = inputs.config(5, nbatch=24, variant="A")
+    problems = list(range(24))
+    _, _, v1, c1, _ = run_gpu(gpu, wl, problems, batched=True)
+    _, _, v2, c2, _ = run_gpu(gpu, wl, problems, batched=True)
+    _, _, v3, c3, _ = run_gpu(gpu, wl, problems, batched=False)
+    assert np.array_equal(v1, v2) and np.array_equal(c1, c2)      # run-to-run determinism
+    assert np.array_equal(v1, v3) and np.array_equal(c1, c3)      # batch shape == split shape, bitwise
+
+
+def test_host_entry_point_equals_device_entry_point(gpu):
+    import torch
+    wl = inputs.config(5, nbatch=3, variant="A")
+    ctx, f, vals, Cf, _ = run_gpu(gpu, wl, [0, 1, 2])
+    fh = torch.from_numpy(f).pin_memory()
+    vh = torch.zeros((3, ctx.S, ctx.nnz), dtype=torch.float64).pin_memory()
+    ch = torch.zeros((3, ctx.S, ctx.n), dtype=torch.float64).pin_memory()
+    ctx.jacobian_host(fh, vh, ch)
+    assert np.array_equal(vh.numpy(), vals) and np.array_equal(ch.numpy(), Cf)
+    v2 = np.zeros_like(vals)
+    ctx.jacobian_host(f, v2, None)                                  # pageable numpy buffers
+    assert np.array_equal(v2, vals)
+
+
+def test_edge_cases(gpu, oracle):
+    import torch
+    # single cell, Q2: 9 points, one ragged tile
+    mesh = inputs.mesh_uniform(0.0, 2.0, -1.0, 1.0, 1, 1)
+    spc = inputs._sp([(1, -1, 1, 1)])
+    wl = inputs.Workload("one-cell", 2, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 5)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    # f = 0 -> J = 0, C = 0 exactly
+    z = torch.zeros((1, ctx.n), dtype=torch.float64, device="cuda")
+    v = torch.ones((1, ctx.nnz), dtype=torch.float64, device="cuda")
+    c = torch.ones((1, ctx.n), dtype=torch.float64, device="cuda")
+    ctx.jacobian(z, v, c)
+    assert float(v.abs().max()) == 0.0 and float(c.abs().max()) == 0.0
+    # nb > max_batch is refused; NULL outputs are skipped
+    with pytest.raises(gpu.LandauError):
+        ctx.jacobian_batched(torch.zeros((2, 1, ctx.n), dtype=torch.float64, device="cuda"), None, None)
+    ctx.jacobian(z, None, None)
+    torch.cuda.synchronize()
+    # maximum species count (16) on a refined mesh
+    m16 = inputs.config(0).mesh
+    rows = [(1.0 + 3.0 * s, (-1) ** s * (1 + s % 3), 1.0, 1.0) for s in range(16)]
+    sp16 = inputs._sp(rows)
+    wl16 = inputs.Workload("16sp", 2, m16, sp16, [[inputs.Component(s, 1.0, 1.0 + 0.1 * s, 0.05 * s) for s in range(16)]], 1e-3, 6)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl16, [0])
+    check_against_oracle(oracle, wl16, ctx, f, vals, Cf, mv, [0])
+    with pytest.raises(gpu.LandauError):
+        gpu.LandauContext(m16, 2, inputs._sp(rows + [(2.0, 1, 1, 1)]))   # S = 17 > 16

@@ -1,0 +1,86 @@
+"""CPU-only checks of the C-ABI library: it loads, exports every symbol include/landau.h
+declares, its host set-up agrees BIT-EXACTLY with the oracle's independent DOF numbering and CSR
+pattern, and its error paths return codes instead of crashing.  No compute calls (no GPU)."""
+import os
+import re
+
+import numpy as np
+import pytest
+
+from paper_2104_10000_b200 import inputs
+
+
+@pytest.fixture(scope="module")
+def binding():
+    from paper_2104_10000_b200 import build
+    build.build()
+    from paper_2104_10000_b200 import binding as b
+    b.lib()
+    return b
+
+
+def test_exports_every_declared_symbol(binding):
+    hdr = open(os.path.join(os.path.dirname(__file__), "..", "include", "landau.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    declared = set(re.findall(r"\b(landau_[a-z0-9_]+)\s*\(", hdr))
+    assert declared == set(binding.SIGNATURES), declared ^ set(binding.SIGNATURES)
+    L = binding.lib()
+    for name in declared:
+        assert hasattr(L, name)
+
+
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, "3A"])
+def test_setup_matches_oracle_numbering_and_pattern(binding, oracle, cfg):
+    if cfg == "3A":
+        wl = inputs.config(3, variant="A")
+    else:
+        wl = inputs.config(cfg)
+    hs = binding.landau_setup_host(wl.mesh, wl.order)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    assert (hs["n"], hs["nnz"], hs["N"]) == (sp.n, sp.nnz, sp.N)
+    assert np.array_equal(hs["rowptr"], sp.rowptr)          # integer work: bit-exact
+    assert np.array_equal(hs["colidx"], sp.colidx)
+    assert np.abs(hs["dof_r"] - sp.dof_r).max() < 1e-14 and np.abs(hs["dof_z"] - sp.dof_z).max() < 1e-14
+
+
+def test_setup_rejects_bad_meshes(binding):
+    m = inputs.mesh_uniform(0.0, 1.0, -1.0, 1.0, 2, 2)
+    L = binding.lib()
+
+    def code(mesh, order=3):
+        try:
+            binding.landau_setup_host(mesh, order)
+            return 0
+        except binding.LandauError as e:
+            return e.code
+    assert code(m) == 0
+    assert code(m, order=4) == binding.LANDAU_EINVAL
+    bad = inputs.Mesh(-1.0, 1.0, -1.0, 1.0, 2, 2, m.level, m.ir, m.iz)           # rmin < 0
+    assert code(bad) == binding.LANDAU_EINVAL
+    hole = inputs.Mesh(0.0, 1.0, -1.0, 1.0, 2, 2, m.level[:3], m.ir[:3], m.iz[:3])  # does not tile
+    assert code(hole) == binding.LANDAU_EINVAL
+    dup = inputs.Mesh(0.0, 1.0, -1.0, 1.0, 2, 2, m.level, np.array([0, 0, 0, 1], np.int32), m.iz)
+    assert code(dup) == binding.LANDAU_EINVAL
+    # not 2:1 balanced: one level-0 cell next to level-2 cells
+    lev, ir, iz = [0], [1], [0]
+    for cj in range(2):
+        for ci in range(2):
+            if (ci, cj) == (1, 0):
+                for dj in range(2):
+                    for di in range(2):
+                        lev.append(2); ir.append(2 + di); iz.append(0 + dj)
+            else:
+                lev.append(1); ir.append(ci); iz.append(cj)
+    unb = inputs.Mesh(0.0, 2.0, 0.0, 1.0, 2, 1, np.array(lev, np.int32), np.array(ir, np.int32), np.array(iz, np.int32))
+    assert code(unb) == binding.LANDAU_EINVAL
+    assert L.landau_strerror(binding.LANDAU_EINVAL).decode() == "invalid argument"
+
+
+def test_create_without_gpu_fails_loudly(binding):
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    wl = inputs.config(1)
+    with pytest.raises(binding.LandauError) as ei:
+        binding.LandauContext(wl.mesh, wl.order, wl.species)
+    assert ei.value.code == binding.LANDAU_ECUDA
