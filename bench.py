@@ -1,0 +1,282 @@
+#!/usr/bin/env python
+"""bench.py -- Landau Jacobian builds/s and GPair-evals/s (fp64) on B200.
+
+One "step" = one pass of the whole hot path (a1-a7: fields, beta sums, all-pairs inner integral,
+element matrices, CSR gather, C(f)) over BASELINE.json config 5: 512 independent velocity-space
+problems on the refined Q3 mesh "3B" (308 cells, 4,928 points, 2 species), one
+landau_jacobian_batched call.  value = ordered point pairs N(N-1) x problems / time, whole job.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+
+N > 1: launched by torchrun, one rank per GPU; the problems are independent (weak scaling: every
+rank builds its own 512 problems, no data-path collective).
+--impl reference: times the CPU oracle (double instantiation) on the host cores on a bounded
+sample of the same workload.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import subprocess
+import sys
+import threading
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+import numpy as np
+
+METRIC = "landau_jacobian_gpair_evals_per_s"
+UNIT = "GPair/s"
+WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
+# FP64 flop per ordered pair executed by k_pair (DFMA x 2 + DMUL + DADD, ncu-counted,
+# profiles/r01_pair_kernel.md).
+FLOP_PER_PAIR = 271.0
+FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
+
+
+class ClockSampler(threading.Thread):
+    """nvidia-smi clocks / throttle reasons during the timed region (B200_PROFILING.md)."""
+
+    def __init__(self, index: int):
+        super().__init__(daemon=True)
+        self.index, self.rows, self._stop_evt = index, [], threading.Event()
+
+    def run(self):
+        q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+             "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+        while not self._stop_evt.is_set():
+            try:
+                out = subprocess.run(["nvidia-smi", f"--query-gpu={q}", "--format=csv,noheader,nounits", "-i", str(self.index)],
+                                     capture_output=True, text=True, timeout=5).stdout.strip()
+                if out:
+                    self.rows.append([c.strip() for c in out.split(",")])
+            except Exception:
+                pass
+            self._stop_evt.wait(0.2)
+
+    def stop(self):
+        self._stop_evt.set()
+        self.join(timeout=6)
+        sm = [float(r[0]) for r in self.rows if r[0].replace(".", "").isdigit()]
+        mx = [float(r[1]) for r in self.rows if r[1].replace(".", "").isdigit()]
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        reasons = sorted({names[k] for r in self.rows for k in range(4) if len(r) >= 7 and r[3 + k].lower() == "active"})
+        return {"sm_mhz": float(np.median(sm)) if sm else None, "sm_max_mhz": max(mx) if mx else None,
+                "reasons": reasons, "samples": len(self.rows)}
+
+
+def cpu_baseline_sample(wl, inputs):
+    """The oracle as it stands (double instantiation), one problem of the workload."""
+    from oracle import landau_oracle as oracle
+    oracle.build()
+    sp = oracle.build_space(wl.mesh, wl.order)
+    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z, 0)
+    t0 = time.perf_counter()
+    oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
+    dt = time.perf_counter() - t0
+    pairs = sp.N * (sp.N - 1)
+    return pairs / dt * 1e-9, dt, os.cpu_count()
+
+
+def run_reference(args):
+    """--impl reference: the CPU oracle on the host cores, each step one problem of config 5."""
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return
+    from paper_2104_10000_b200 import inputs
+    from oracle import landau_oracle as oracle
+    oracle.build()
+    wl = inputs.config(5, nbatch=max(1, args.steps + args.warmup))
+    sp = oracle.build_space(wl.mesh, wl.order)
+    pairs = sp.N * (sp.N - 1)
+    times = []
+    for k in range(args.warmup + args.steps):
+        f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z, k)
+        t0 = time.perf_counter()
+        oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
+        if k >= args.warmup:
+            times.append(time.perf_counter() - t0)
+    ms = 1e3 * float(np.mean(times))
+    val = pairs / (ms * 1e-3) * 1e-9
+    sample = "1 of the 512 problems per step (full N=4928 mesh, a1-a8), double-precision oracle, OpenMP over i"
+    print(json.dumps({
+        "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f64", "data": "synthetic", "config": {"workload": WORKLOAD, "sample": sample},
+        "builds_per_s": 1e3 / ms,
+        "cpu_baseline": {"value": val, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle", "sample": sample},
+        "e2e": {"value": val, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+    }))
+
+
+def time_single_config(binding, inputs, torch, k, variant="B", reps=20):
+    """Single-problem build (split launch shape) of configs 1-4: device time per build."""
+    wl = inputs.config(k, variant=variant)
+    ctx = binding.LandauContext(wl.mesh, wl.order, wl.species, 1)
+    r, z = ctx.dof_coords()
+    f = torch.from_numpy(inputs.nodal_f(wl, r, z)).cuda()
+    vals = torch.zeros((ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    Cf = torch.zeros((ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    for _ in range(3):
+        ctx.jacobian(f, vals, Cf)
+    torch.cuda.synchronize()
+    ctx.profile_enable(True)
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record()
+    for _ in range(reps):
+        ctx.jacobian(f, vals, Cf)
+    e1.record()
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / reps
+    pair_ms, cnt = ctx.profile_read()
+    pairs = ctx.N * (ctx.N - 1)
+    out = {"config": wl.name, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz, "ms_per_build": ms,
+           "builds_per_s": 1e3 / ms, "gpair_per_s": pairs / (ms * 1e-3) * 1e-9,
+           "pair_kernel_ms": pair_ms / max(cnt, 1), "pair_kernel_gpair_per_s": pairs / (pair_ms / max(cnt, 1) * 1e-3) * 1e-9}
+    ctx.destroy()
+    return out
+
+
+def run_ours(args):
+    import torch
+    from paper_2104_10000_b200 import binding, inputs
+
+    rank = int(os.environ.get("RANK", "0"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device (no CPU fallback); use --impl reference for the CPU oracle")
+    binding.lib()
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    wl = inputs.config(5)
+    nb = wl.nbatch
+    ctx = binding.LandauContext(wl.mesh, wl.order, wl.species, nb)
+    r, z = ctx.dof_coords()
+    # every rank builds its own 512 problems (weak scaling); problem seeds are offset by rank
+    f_host = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in range(nb)])).pin_memory()
+    if rank:
+        f_host.mul_(1.0 + 1e-3 * rank)
+    f = f_host.cuda()
+    vals = torch.zeros((nb, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    Cf = torch.zeros((nb, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    flush = torch.zeros(256 * 1024 * 1024 // 8, dtype=torch.float64, device="cuda")   # 256 MiB > 126 MB L2
+    pairs_per_step = nb * ctx.N * (ctx.N - 1)
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        ctx.jacobian_batched(f, vals, Cf)
+    barrier()
+
+    # ---- device-resident timing: K steps, CUDA events per step on the launching stream ----------
+    sampler = ClockSampler(local_rank)
+    sampler.start()
+    ctx.profile_enable(True)
+    ctx.profile_read()
+    l0 = ctx.launch_count()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
+    barrier()
+    t_wall = time.perf_counter()
+    for k in range(args.steps):
+        flush.add_(1.0)                      # L2 flush between timed iterations (outside the events)
+        evs[k][0].record()
+        ctx.jacobian_batched(f, vals, Cf)
+        evs[k][1].record()
+    barrier()
+    t_wall = time.perf_counter() - t_wall
+    launches = ctx.launch_count() - l0
+    step_ms = [a.elapsed_time(b) for a, b in evs]
+    total_ms = float(sum(step_ms))
+    pair_ms, pair_cnt = ctx.profile_read()
+    ctx.profile_enable(False)
+    clocks = sampler.stop()
+
+    # ---- end to end through the host entry point: pinned host buffers, H2D + D2H inside -----------
+    vals_host = torch.zeros((nb, ctx.S, ctx.nnz), dtype=torch.float64).pin_memory()
+    Cf_host = torch.zeros((nb, ctx.S, ctx.n), dtype=torch.float64).pin_memory()
+    ctx.jacobian_host(f_host, vals_host, Cf_host)        # warm-up (allocates staging)
+    barrier()
+    e2e_steps = max(1, min(args.steps, 5))
+    t0 = time.perf_counter()
+    for _ in range(e2e_steps):
+        ctx.jacobian_host(f_host, vals_host, Cf_host)    # synchronises
+    barrier()
+    e2e_ms = (time.perf_counter() - t0) * 1e3
+    assert torch.equal(vals_host[-1], vals[-1].cpu())
+
+    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    total_ms, e2e_ms = float(t[0]), float(t[1])
+    ms_per_step = total_ms / args.steps
+    value = world * pairs_per_step / (ms_per_step * 1e-3) * 1e-9
+    e2e_value = world * pairs_per_step / (e2e_ms / e2e_steps * 1e-3) * 1e-9
+
+    if rank == 0:
+        peak_flops, _ = binding.landau_fp64_peak_probe(1 << 16)
+        sm_max = clocks["sm_max_mhz"] or 1965.0
+        sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
+        nominal_peak = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
+        pair_launch_ms = pair_ms / max(pair_cnt, 1)
+        achieved = FLOP_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) * 1e-12
+        roof = {"bound": "alu", "kernel": "k_pair<false>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
+                "frac": achieved / nominal_peak, "traffic": None,
+                "peak_source": "derived: SMs x 64 DFMA lanes x 2 x clocks.max.sm (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
+                "peak_probe_measured": peak_flops * 1e-12, "frac_of_probe": achieved / (peak_flops * 1e-12),
+                "flop_per_pair": FLOP_PER_PAIR, "kernel_ms_per_launch": pair_launch_ms,
+                "kernel_share_of_step": pair_ms / total_ms if world == 1 else None,
+                "kernel_gpair_per_s": pairs_per_step / (pair_launch_ms * 1e-3) * 1e-9}
+        cpu_val, cpu_dt, cores = cpu_baseline_sample(wl, inputs)
+        detail = [time_single_config(binding, inputs, torch, k) for k in (1, 2, 3, 4)]
+        detail.append(time_single_config(binding, inputs, torch, 3, variant="A"))
+        h2d = nb * ctx.S * ctx.n * 8
+        d2h = nb * ctx.S * (ctx.nnz + ctx.n) * 8
+        print(json.dumps({
+            "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "data": "synthetic",
+            "config": {"workload": WORKLOAD, "problems_per_gpu": nb, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz,
+                       "pairs_per_step_per_gpu": pairs_per_step, "l2": "256 MiB flush write between timed steps; outputs 0.7 GB > L2"},
+            "builds_per_s": world * nb / (ms_per_step * 1e-3),
+            "wall_ms_per_step_incl_flush": t_wall * 1e3 / args.steps,
+            "clocks": clocks, "gpu_launches": launches,
+            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps, "api": "landau_jacobian_host (pinned host buffers)"},
+            "roofline": roof,
+            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
+                             "sample": f"1 of the 512 problems (N=4928, a1-a8), double-precision oracle, {cpu_dt:.2f} s"},
+            "per_config": detail,
+        }))
+    ctx.destroy()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=10)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    args = ap.parse_args()
+    if args.impl == "reference":
+        run_reference(args)
+    else:
+        args.warmup = max(args.warmup, 3)
+        run_ours(args)
+
+
+if __name__ == "__main__":
+    main()

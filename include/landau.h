@@ -124,6 +124,12 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
 /* Number of kernel launches the ctx has enqueued since creation (for bench.py's gpu_launches). */
 int landau_launch_count(const landau_ctx *ctx, int64_t *count);
 
+/* Measurement aid: when enabled, every pair-kernel launch (step a3) is bracketed by CUDA events on
+ * its own stream.  landau_profile_read synchronises those events, returns the summed device time
+ * (ms) and the number of bracketed launches since the last read, and resets both. */
+int landau_profile_enable(landau_ctx *ctx, int on);
+int landau_profile_read(landau_ctx *ctx, double *pair_ms_total, int64_t *pair_launches);
+
 /* Measurement aid, not part of the operator: runs a register-resident chain of dependent-free
  * DFMA on every SM for `iters` iterations and returns the achieved FP64 rate in flop/s (the
  * "alu" roofline denominator).  Synchronises. */

@@ -49,6 +49,8 @@ SIGNATURES = {
     "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
+    "landau_profile_enable": (c_int, [c_void_p, c_int]),
+    "landau_profile_read": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
     "landau_fp64_peak_probe": (c_int, [c_int, POINTER(c_double), POINTER(c_double)]),
     "landau_strerror": (ctypes.c_char_p, [c_int]),
     "landau_last_cuda_error": (ctypes.c_char_p, []),
@@ -212,6 +214,15 @@ class LandauContext:
             return c_void_p(a.ctypes.data if isinstance(a, np.ndarray) else a.data_ptr())
         nb = f_host.shape[0]
         _check(lib().landau_jacobian_host(self._h, nb, hp(f_host), hp(vals_host), hp(Cf_host)))
+
+    def profile_enable(self, on: bool = True):
+        _check(lib().landau_profile_enable(self._h, int(bool(on))))
+
+    def profile_read(self):
+        """(summed pair-kernel device time in ms, number of launches) since the last read."""
+        ms, cnt = c_double(), c_int64()
+        _check(lib().landau_profile_read(self._h, ctypes.byref(ms), ctypes.byref(cnt)))
+        return ms.value, cnt.value
 
     def launch_count(self) -> int:
         c = c_int64()

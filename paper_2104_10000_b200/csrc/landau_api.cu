@@ -53,7 +53,25 @@ struct landau_ctx {
     cudaStream_t own_stream = nullptr;
     double *h2d_f = nullptr, *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
     int host_nb = 0;
+    bool profiling = false;
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;  // recorded, not yet read
+    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pool;    // free
 };
+
+namespace {
+// launch_pair bracketed by events when profiling is on
+int timed_pair(landau_ctx *ctx, int nb, bool split, double *G, cudaStream_t st) {
+    if (!ctx->profiling) return launch_pair(ctx->ds, nb, split, ctx->sc.T, G, st);
+    std::pair<cudaEvent_t, cudaEvent_t> ev;
+    if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
+    else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
+    cudaEventRecord(ev.first, st);
+    int k = launch_pair(ctx->ds, nb, split, ctx->sc.T, G, st);
+    cudaEventRecord(ev.second, st);
+    ctx->prof_events.push_back(ev);
+    return k;
+}
+}  // namespace
 
 extern "C" {
 
@@ -76,6 +94,8 @@ int landau_destroy(landau_ctx *ctx) {
     if (ctx->d_vals) cudaFree(ctx->d_vals);
     if (ctx->d_Cf) cudaFree(ctx->d_Cf);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    for (auto &ev : ctx->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    for (auto &ev : ctx->prof_pool) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     delete ctx;
     return LANDAU_OK;
 }
@@ -224,9 +244,9 @@ int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *
     const bool split = pair_use_split(ctx->ds.N, nb, ctx->num_sms);
     ctx->launches += launch_fields_beta(ctx->ds, nb, f_dev, ctx->sc.T, st);
     if (!split) {
-        ctx->launches += launch_pair(ctx->ds, nb, false, ctx->sc.T, G_dev, st);
+        ctx->launches += timed_pair(ctx, nb, false, G_dev, st);
     } else {
-        ctx->launches += launch_pair(ctx->ds, nb, true, ctx->sc.T, ctx->sc.G, st);
+        ctx->launches += timed_pair(ctx, nb, true, ctx->sc.G, st);
         ctx->launches += launch_sum_partials(ctx->ds, nb, pair_chunks(ctx->ds.N), ctx->sc.G, G_dev, st);
     }
     CK(cudaGetLastError());
@@ -240,7 +260,7 @@ int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double
     const bool split = pair_use_split(ds.N, nb, ctx->num_sms);
     const int js = split ? pair_chunks(ds.N) : 1;
     ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
-    ctx->launches += launch_pair(ds, nb, split, ctx->sc.T, ctx->sc.G, st);
+    ctx->launches += timed_pair(ctx, nb, split, ctx->sc.G, st);
     ctx->launches += launch_element(ds, nb, js, f_dev, ctx->sc.G, ctx->sc.Ce, ctx->sc.ce, st);
     if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
     if (Cf_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, Cf_dev, st);
@@ -286,6 +306,28 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
 int landau_launch_count(const landau_ctx *ctx, int64_t *count) {
     if (!ctx || !count) return LANDAU_EINVAL;
     *count = ctx->launches;
+    return LANDAU_OK;
+}
+
+int landau_profile_enable(landau_ctx *ctx, int on) {
+    if (!ctx) return LANDAU_EINVAL;
+    ctx->profiling = on != 0;
+    return LANDAU_OK;
+}
+
+int landau_profile_read(landau_ctx *ctx, double *pair_ms_total, int64_t *pair_launches) {
+    if (!ctx || !pair_ms_total || !pair_launches) return LANDAU_EINVAL;
+    double total = 0.0;
+    for (auto &ev : ctx->prof_events) {
+        CK(cudaEventSynchronize(ev.second));
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, ev.first, ev.second));
+        total += ms;
+        ctx->prof_pool.push_back(ev);
+    }
+    *pair_ms_total = total;
+    *pair_launches = int64_t(ctx->prof_events.size());
+    ctx->prof_events.clear();
     return LANDAU_OK;
 }
 
