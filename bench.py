@@ -33,8 +33,8 @@ METRIC = "landau_jacobian_gpair_evals_per_s"
 UNIT = "GPair/s"
 WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
 # FP64 flop per ordered pair executed by k_pair (DFMA x 2 + DMUL + DADD, ncu-counted,
-# profiles/r01_pair_kernel.md).
-FLOP_PER_PAIR = 271.0
+# profiles/r01a_pair_kernel.md).
+FLOP_PER_PAIR = 196.0
 FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
 
 
