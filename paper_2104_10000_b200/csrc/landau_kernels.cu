@@ -18,97 +18,122 @@
 namespace landau {
 
 // ------------------------------------------------------------------------------------------------
-// fast fp64 reciprocal / rsqrt: MUFU seed (rel. err ~2^-22) + two Newton steps on the DFMA pipe.
-// Not IEEE-rounded (<= ~1 ulp), no special-case handling: arguments here are finite and > 0.
+// fast fp64 reciprocal / square roots: MUFU seed (relative error < 2^-19 including the truncation
+// of the operand to its high word) + ONE cubic correction on the DFMA pipe (error ~ seed^3 < 1e-17).
+// Not IEEE-rounded (~1 ulp), no special cases: arguments here are finite and > 0.
 // ------------------------------------------------------------------------------------------------
 __device__ __forceinline__ double rcp_fast(double x) {
     double y;
     asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double e = fma(-x, y, 1.0);
-    y = fma(y, e, y);
-    e = fma(-x, y, 1.0);
-    return fma(y, e, y);
+    const double e = fma(-x, y, 1.0);
+    const double p = fma(e, e, e);      // e + e^2
+    return fma(y, p, y);                // y (1 + e + e^2)
 }
 
-// returns sqrt(x); *half_rsqrt = 1/(2 sqrt(x))
-__device__ __forceinline__ double sqrt_fast(double x, double *half_rsqrt) {
+// g = sqrt(x), yy = 1/sqrt(x)
+__device__ __forceinline__ void sqrt_rsqrt_fast(double x, double &g, double &yy) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    double g = x * y, h = 0.5 * y;
-    double r = fma(-h, g, 0.5);
-    g = fma(g, r, g);
-    h = fma(h, r, h);
-    r = fma(-h, g, 0.5);
-    g = fma(g, r, g);
-    h = fma(h, r, h);
-    *half_rsqrt = h;
-    return g;
+    const double t = x * y;
+    const double r = fma(-t, y, 1.0);   // 1 - x y^2
+    double p = fma(0.375, r, 0.5);
+    p = p * r;                          // r/2 + 3 r^2/8
+    g = fma(t, p, t);
+    yy = fma(y, p, y);
+}
+
+// 2 sqrt(x): the factor 2 is put into the seed's exponent (integer add on the high word), so the
+// scaled AGM below needs no multiplication by 1/2 or 2 on the FP64 pipe.
+__device__ __forceinline__ double sqrt_times2_fast(double x) {
+    double y;
+    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    const double y2 = __hiloint2double(__double2hiint(y) + 0x00100000, __double2loint(y));
+    const double t = x * y2;            // ~ 2 sqrt(x)
+    const double r2 = fma(-t, y, 2.0);  // 2 (1 - x y^2)
+    double p = fma(0.09375, r2, 0.25);
+    p = p * r2;                         // r/2 + 3 r^2/8
+    return fma(t, p, t);
 }
 
 // ------------------------------------------------------------------------------------------------
 // a3: pair kernel.  PAPER.md Alg. 1 lines 3-12 (L114-121), Eqs. 7-8 (L65-67).
 //
-// Azimuth-integrated Landau tensor through the scaled AGM (DESIGN.md "Elliptic integrals on the
-// device"): with a0 = sqrt(s), b0 = sqrt(d2), q = 4 r rb = s - d2,
-//     a_{k+1} = (a_k+b_k)/2, b_{k+1} = sqrt(a_k b_k), c_{k+1} = (a_k-b_k)/2,  A = lim a_k
-//     Kt = K(m)/sqrt(s) = pi/(2A)
-//     W  = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(8 a_1^2) + (sum_{k>=2} 2^k c_k^2)/q^2     (c_1 = q/(4 a_1))
-//     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2)
-// every sum has positive terms except the last bracket (E/K, bounded cancellation ~ K/E).
+// Azimuth-integrated Landau tensor through a SCALED arithmetic-geometric mean (DESIGN.md "Elliptic
+// integrals on the device").  With a0 = sqrt(s), b0 = sqrt(d2), q = 4 r rb = s - d2 and
+// A_k = 2^k a_k, B_k = 2^k b_k:
+//     A_{k+1} = A_k + B_k,  B_{k+1} = 2 sqrt(A_k B_k),  C_{k+1} = A_k - B_k = 2^{k+1} c_{k+1}
+//     K(m)/sqrt(s) = pi/(2 lim a_k) = pi 2^k / A_{k+1}
+//     W = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(2 A_1^2) + (sum_{k>=2} C_k^2 / 2^k)/q^2   (c_1 = q/(4 a_1))
+//     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2),  Kt = K/sqrt(s)
+// every sum has positive terms except the bracket of P0 (= 2 s E/K: bounded cancellation ~ K/E).
+// The iteration stops for the whole warp once every lane has c_{k+1} < 2^-26 a_k (the neglected
+// c_{k+2} ~ c_{k+1}^2/(4a) is then < 6e-17 a).  The test compares exponents with integer ops.
 // ------------------------------------------------------------------------------------------------
 struct PairAcc { double drr, drz, dzz, kr, kz; };
+struct __align__(16) JPoint { double r, z, invr, tD, tKr, tKz; };
 
-__device__ __forceinline__ void pair_accumulate(double ri, double zi, double inv4ri, double rj, double zj,
-                                                double invrj, double tD, double tKr, double tKz, PairAcc &acc) {
-    const double dz = zi - zj, dr = ri - rj, sr = ri + rj;
-    const double dz2 = dz * dz;
-    double d2 = fma(dr, dr, dz2);
+constexpr int AGM_MAX_STEPS = 8;
+
+template <bool CHECK_SELF>
+__device__ __forceinline__ void pair_accumulate(double ri, double zi, double ri4, double inv4ri, const JPoint &pj,
+                                                PairAcc &acc) {
+    const double rj = pj.r;
+    const double dz = zi - pj.z, dr = ri - rj, sr = ri + rj;
+    const double dz2 = dz * dz, dr2 = dr * dr;
+    double d2 = dr2 + dz2;
     const double s = fma(sr, sr, dz2);
-    const bool self = !(d2 > 0.0);   // coincident pair (j == i): contributes nothing (reading Q3)
-    if (self) d2 = 1.0;
-    const double q = 4.0 * ri * rj;
-    const double invq = inv4ri * invrj;
-
-    double h;
-    double a = sqrt_fast(s, &h);
-    double b = sqrt_fast(d2, &h);
-    // step 1
-    double an = 0.5 * (a + b);
-    b = sqrt_fast(a * b, &h);
-    a = an;
-    const double inva1 = rcp_fast(a);
-    double wsum = 0.0, pw = 4.0;
-#pragma unroll 1
-    for (int it = 0; it < 8; ++it) {
-        const double c = 0.5 * (a - b);
-        an = 0.5 * (a + b);
-        wsum = fma(pw * c, c, wsum);
-        pw += pw;
-        const bool done = c <= 1.0e-8 * a;
-        if (__all_sync(0xffffffffu, done)) { a = an; break; }
-        b = sqrt_fast(a * b, &h);
-        a = an;
+    bool self = false;
+    if (CHECK_SELF) {                 // coincident pair (j == i): contributes nothing (reading Q3)
+        self = !(d2 > 0.0);
+        if (self) d2 = 1.0;
     }
-    const double Kt = 1.5707963267948966 * rcp_fast(a);
-    const double W = fma(0.125 * inva1, inva1, wsum * invq * invq);
-    const double invs = rcp_fast(s);
-    const double invd2 = rcp_fast(d2);
-    double Pss = 16.0 * Kt * W;
-    double Pc = 4.0 * Kt * fma(q, W, 1.0) * invs;
-    double P0 = 2.0 * Kt * (s + d2 - q * q * W) * invs * invd2;
-    if (self) { Pss = 0.0; Pc = 0.0; P0 = 0.0; }
+    double a0, b0, ys, yd;
+    sqrt_rsqrt_fast(s, a0, ys);
+    sqrt_rsqrt_fast(d2, b0, yd);
+    double A = a0 + b0;               // 2 a_1
+    double B = sqrt_times2_fast(a0 * b0);
+    const double iA1 = rcp_fast(A);
+    double wsum = 0.0, kscale = 6.283185307179586476925286766559;   // 2 Kt = kscale / A_final
+#pragma unroll
+    for (int k = 1; k <= AGM_MAX_STEPS; ++k) {
+        const double C = A - B;
+        const double An = A + B;
+        wsum = fma(C * (1.0 / double(1 << (k + 1))), C, wsum);
+        kscale = 6.283185307179586476925286766559 * double(1 << k);
+        const bool conv = __double2hiint(C) + (27 << 20) <= __double2hiint(A);
+        if (k == AGM_MAX_STEPS || __all_sync(0xffffffffu, conv)) { A = An; break; }
+        B = sqrt_times2_fast(A * B);
+        A = An;
+    }
+    const double KP2 = kscale * rcp_fast(A);          // 2 K/sqrt(s)
+    const double rho = ri * rj, q = ri4 * rj;
+    const double invq = inv4ri * pj.invr;
+    const double W = fma(0.5 * iA1, iA1, wsum * (invq * invq));
+    const double Ks = KP2 * (ys * ys);
+    const double x = q * W;
+    double Pc = Ks * fma(2.0, x, 2.0);
+    double P0 = Ks * (yd * yd) * fma(-q, x, s + d2);
+    double Pss = 8.0 * (KP2 * W);
+    if (CHECK_SELF && self) { Pss = 0.0; Pc = 0.0; P0 = 0.0; }
 
-    const double rirj = ri * rj;
     const double UDrr = fma(rj * rj, Pss, dz2 * P0);
-    const double UDrz = -dz * fma(dr, P0, rj * Pc);
-    const double UDzz = fma(dr * dr, P0, 2.0 * rirj * Pc);
-    const double UKrr = fma(dz2, P0 - Pc, rirj * Pss);
+    const double nUDrz = dz * fma(dr, P0, rj * Pc);         // -U^D_rz
+    const double UDzz = fma(2.0, rho * Pc, dr2 * P0);
+    const double UKrr = fma(dz2, P0 - Pc, rho * Pss);
     const double UKzr = dz * fma(-dr, P0, ri * Pc);
-    acc.drr = fma(tD, UDrr, acc.drr);
-    acc.drz = fma(tD, UDrz, acc.drz);
-    acc.dzz = fma(tD, UDzz, acc.dzz);
-    acc.kr = fma(UKrr, tKr, fma(UDrz, tKz, acc.kr));
-    acc.kz = fma(UKzr, tKr, fma(UDzz, tKz, acc.kz));
+    acc.drr = fma(pj.tD, UDrr, acc.drr);
+    acc.drz = fma(-pj.tD, nUDrz, acc.drz);
+    acc.dzz = fma(pj.tD, UDzz, acc.dzz);
+    acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
+    acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
+}
+
+template <bool CHECK_SELF>
+__device__ __forceinline__ void pair_chunk(double ri, double zi, double ri4, double inv4ri, const JPoint *__restrict__ sj,
+                                           int cnt, PairAcc &acc) {
+    PairAcc part = {0.0, 0.0, 0.0, 0.0, 0.0};
+    for (int t = 0; t < cnt; ++t) pair_accumulate<CHECK_SELF>(ri, zi, ri4, inv4ri, sj[t], part);
+    acc.drr += part.drr; acc.drz += part.drz; acc.dzz += part.dzz; acc.kr += part.kr; acc.kz += part.kz;
 }
 
 // Deterministic summation order: the j range is cut into chunks of
@@ -121,17 +146,19 @@ __device__ __forceinline__ void pair_accumulate(double ri, double zi, double inv
 // SPLIT = true (few problems): grid = (ceil(N/PAIR_THREADS), nchunks, nb); each block does one
 //   chunk and writes its partial to Gpart[b][chunk][5][N]; k_element / k_sum_partials add them.
 // r,z,invr [N] are shared by the batch; T[b][3][N] = w_in * (T_D, T_Kr, T_Kz).
+// The coincident pair is tested only in chunks that overlap the block's own i range.
 template <bool SPLIT>
-__global__ void __launch_bounds__(PAIR_THREADS)
+__global__ void __launch_bounds__(PAIR_THREADS, 6)
 k_pair(int N, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
        const double *__restrict__ T, double *__restrict__ Gout) {
     constexpr int TILE = SPLIT ? PAIR_CHUNK : PAIR_TILE;
-    __shared__ double s_r[TILE], s_z[TILE], s_ir[TILE], s_td[TILE], s_tr[TILE], s_tz[TILE];
+    __shared__ JPoint sj[TILE];
     const int b = blockIdx.z;
-    const int i = blockIdx.x * PAIR_THREADS + threadIdx.x;
+    const int ibase = blockIdx.x * PAIR_THREADS;
+    const int i = ibase + threadIdx.x;
     const int ic = i < N ? i : N - 1;
     const double ri = r[ic], zi = z[ic];
-    const double inv4ri = 0.25 * invr[ic];
+    const double ri4 = 4.0 * ri, inv4ri = 0.25 * invr[ic];
     const double *Tb = T + (size_t)b * 3 * N;
     PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
     const int j0 = SPLIT ? blockIdx.y * PAIR_CHUNK : 0;
@@ -140,16 +167,18 @@ k_pair(int N, const double *__restrict__ r, const double *__restrict__ z, const 
         const int cnt = min(TILE, j1 - jt);
         __syncthreads();
         for (int t = threadIdx.x; t < cnt; t += PAIR_THREADS) {
-            s_r[t] = r[jt + t]; s_z[t] = z[jt + t]; s_ir[t] = invr[jt + t];
-            s_td[t] = Tb[jt + t]; s_tr[t] = Tb[N + jt + t]; s_tz[t] = Tb[2 * N + jt + t];
+            JPoint pj;
+            pj.r = r[jt + t]; pj.z = z[jt + t]; pj.invr = invr[jt + t];
+            pj.tD = Tb[jt + t]; pj.tKr = Tb[N + jt + t]; pj.tKz = Tb[2 * N + jt + t];
+            sj[t] = pj;
         }
         __syncthreads();
         for (int c0 = 0; c0 < cnt; c0 += PAIR_CHUNK) {
-            PairAcc part = {0.0, 0.0, 0.0, 0.0, 0.0};
-            const int c1 = min(cnt, c0 + PAIR_CHUNK);
-            for (int t = c0; t < c1; ++t)
-                pair_accumulate(ri, zi, inv4ri, s_r[t], s_z[t], s_ir[t], s_td[t], s_tr[t], s_tz[t], part);
-            acc.drr += part.drr; acc.drz += part.drz; acc.dzz += part.dzz; acc.kr += part.kr; acc.kz += part.kz;
+            const int clen = min(PAIR_CHUNK, cnt - c0);
+            const int jg = jt + c0;                                   // global j of the chunk start
+            const bool overlap = jg < ibase + PAIR_THREADS && jg + clen > ibase;   // block-uniform
+            if (overlap) pair_chunk<true>(ri, zi, ri4, inv4ri, sj + c0, clen, acc);
+            else pair_chunk<false>(ri, zi, ri4, inv4ri, sj + c0, clen, acc);
         }
     }
     if (i < N) {
