@@ -48,7 +48,6 @@ struct landau_ctx {
     std::vector<void *> owned;   // device allocations
     int max_batch = 1;
     int num_sms = 148;
-    int split_nb_max = 1;   // largest nb that uses the split launch shape
     int64_t launches = 0;
     cudaStream_t own_stream = nullptr;
     double *h2d_f = nullptr, *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
@@ -60,13 +59,13 @@ struct landau_ctx {
 
 namespace {
 // launch_pair bracketed by events when profiling is on
-int timed_pair(landau_ctx *ctx, int nb, bool split, double *G, cudaStream_t st) {
-    if (!ctx->profiling) return launch_pair(ctx->ds, nb, split, ctx->sc.T, G, st);
+int timed_pair(landau_ctx *ctx, int nb, double *G, cudaStream_t st) {
+    if (!ctx->profiling) return launch_pair(ctx->ds, nb, ctx->sc.T, G, st);
     std::pair<cudaEvent_t, cudaEvent_t> ev;
     if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
     else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
     cudaEventRecord(ev.first, st);
-    int k = launch_pair(ctx->ds, nb, split, ctx->sc.T, G, st);
+    int k = launch_pair(ctx->ds, nb, ctx->sc.T, G, st);
     cudaEventRecord(ev.second, st);
     ctx->prof_events.push_back(ev);
     return k;
@@ -142,7 +141,6 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev);
     ctx->max_batch = max_batch;
-    while (ctx->split_nb_max < max_batch && pair_use_split(ds.N, ctx->split_nb_max + 1, ctx->num_sms)) ctx->split_nb_max++;
 
 #define UP(field, vec)                                                   \
     if ((rc = upload(vec, &ds.field, ctx->owned)) != LANDAU_OK) { landau_destroy(ctx); return rc; }
@@ -155,10 +153,11 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
 #undef UP
     // scratch arena
     const size_t nbm = size_t(max_batch);
-    const size_t gsz = std::max(nbm, size_t(ctx->split_nb_max) * pair_chunks(ds.N)) * 5 * hs.N;
+    const size_t gsz = nbm * pair_tiles(ds.N) * 5 * hs.N;
     struct { double **p; size_t n; } allocs[] = {
         {&ctx->sc.T, nbm * 3 * hs.N},
         {&ctx->sc.G, gsz},
+        {&ctx->sc.Gsum, nbm * 5 * hs.N},
         {&ctx->sc.Ce, nbm * ds.S * hs.Ne * hs.Nb * hs.Nb},
         {&ctx->sc.ce, nbm * ds.S * hs.Ne * hs.Nb},
     };
@@ -241,14 +240,9 @@ int landau_points(const landau_ctx *ctx, double *r_host, double *z_host, double 
 int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *G_dev, void *stream) {
     if (!ctx || !f_dev || !G_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool split = pair_use_split(ctx->ds.N, nb, ctx->num_sms);
     ctx->launches += launch_fields_beta(ctx->ds, nb, f_dev, ctx->sc.T, st);
-    if (!split) {
-        ctx->launches += timed_pair(ctx, nb, false, G_dev, st);
-    } else {
-        ctx->launches += timed_pair(ctx, nb, true, ctx->sc.G, st);
-        ctx->launches += launch_sum_partials(ctx->ds, nb, pair_chunks(ctx->ds.N), ctx->sc.G, G_dev, st);
-    }
+    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
+    ctx->launches += launch_sum_partials(ctx->ds, nb, pair_tiles(ctx->ds.N), ctx->sc.G, G_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
@@ -257,11 +251,10 @@ int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double
     if (!ctx || !f_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     const DeviceSpace &ds = ctx->ds;
-    const bool split = pair_use_split(ds.N, nb, ctx->num_sms);
-    const int js = split ? pair_chunks(ds.N) : 1;
     ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
-    ctx->launches += timed_pair(ctx, nb, split, ctx->sc.G, st);
-    ctx->launches += launch_element(ds, nb, js, f_dev, ctx->sc.G, ctx->sc.Ce, ctx->sc.ce, st);
+    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
+    ctx->launches += launch_sum_partials(ds, nb, pair_tiles(ds.N), ctx->sc.G, ctx->sc.Gsum, st);
+    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, st);
     if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
     if (Cf_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, Cf_dev, st);
     CK(cudaGetLastError());

@@ -4,7 +4,8 @@
 //
 //   k_fields_beta   a1+a2  f -> w_in*T_D, w_in*T_K at every integration point (beta sum hoisted
 //                          out of the pair loop: it does not depend on i)
-//   k_pair          a3     all-pairs inner integral, thread owns i, j streamed through smem
+//   k_pair_sym      a3     all-pairs inner integral over tile pairs, one tensor evaluation per
+//                          unordered pair, thread owns i, j broadcast from shared memory
 //   k_element       a4+a5  scale, transform, element matrix C_e and element vector C_e u
 //   k_gather        a6/a7  deterministic gather of element entries into CSR values / C(f)
 //   k_mass_element  a8     shift * element mass matrices (gathered by k_gather)
@@ -74,14 +75,18 @@ struct __align__(16) JPoint { double r, z, invr, tD, tKr, tKz; };
 
 constexpr int AGM_MAX_STEPS = 8;
 
+// P0, Pc, Pss of one pair (header above) plus the geometry the tensor entries need.
+struct PairParts { double P0, Pc, Pss, dz, dr, dz2, dr2, rho; };
+
 template <bool CHECK_SELF>
-__device__ __forceinline__ void pair_accumulate(double ri, double zi, double ri4, double inv4ri, const JPoint &pj,
-                                                PairAcc &acc) {
+__device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4, double inv4ri, const JPoint &pj) {
+    PairParts pp;
     const double rj = pj.r;
-    const double dz = zi - pj.z, dr = ri - rj, sr = ri + rj;
-    const double dz2 = dz * dz, dr2 = dr * dr;
-    double d2 = dr2 + dz2;
-    const double s = fma(sr, sr, dz2);
+    const double sr = ri + rj;
+    pp.dz = zi - pj.z; pp.dr = ri - rj;
+    pp.dz2 = pp.dz * pp.dz; pp.dr2 = pp.dr * pp.dr;
+    double d2 = pp.dr2 + pp.dz2;
+    const double s = fma(sr, sr, pp.dz2);
     bool self = false;
     if (CHECK_SELF) {                 // coincident pair (j == i): contributes nothing (reading Q3)
         self = !(d2 > 0.0);
@@ -106,84 +111,135 @@ __device__ __forceinline__ void pair_accumulate(double ri, double zi, double ri4
         A = An;
     }
     const double KP2 = kscale * rcp_fast(A);          // 2 K/sqrt(s)
-    const double rho = ri * rj, q = ri4 * rj;
+    const double q = ri4 * rj;
+    pp.rho = ri * rj;
     const double invq = inv4ri * pj.invr;
     const double W = fma(0.5 * iA1, iA1, wsum * (invq * invq));
     const double Ks = KP2 * (ys * ys);
     const double x = q * W;
-    double Pc = Ks * fma(2.0, x, 2.0);
-    double P0 = Ks * (yd * yd) * fma(-q, x, s + d2);
-    double Pss = 8.0 * (KP2 * W);
-    if (CHECK_SELF && self) { Pss = 0.0; Pc = 0.0; P0 = 0.0; }
-
-    const double UDrr = fma(rj * rj, Pss, dz2 * P0);
-    const double nUDrz = dz * fma(dr, P0, rj * Pc);         // -U^D_rz
-    const double UDzz = fma(2.0, rho * Pc, dr2 * P0);
-    const double UKrr = fma(dz2, P0 - Pc, rho * Pss);
-    const double UKzr = dz * fma(-dr, P0, ri * Pc);
-    acc.drr = fma(pj.tD, UDrr, acc.drr);
-    acc.drz = fma(-pj.tD, nUDrz, acc.drz);
-    acc.dzz = fma(pj.tD, UDzz, acc.dzz);
-    acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
-    acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
+    pp.Pc = Ks * fma(2.0, x, 2.0);
+    pp.P0 = Ks * (yd * yd) * fma(-q, x, s + d2);
+    pp.Pss = 8.0 * (KP2 * W);
+    if (CHECK_SELF && self) { pp.Pss = 0.0; pp.Pc = 0.0; pp.P0 = 0.0; }
+    return pp;
 }
 
-template <bool CHECK_SELF>
-__device__ __forceinline__ void pair_chunk(double ri, double zi, double ri4, double inv4ri, const JPoint *__restrict__ sj,
-                                           int cnt, PairAcc &acc) {
-    PairAcc part = {0.0, 0.0, 0.0, 0.0, 0.0};
-    for (int t = 0; t < cnt; ++t) pair_accumulate<CHECK_SELF>(ri, zi, ri4, inv4ri, sj[t], part);
-    acc.drr += part.drr; acc.drz += part.drz; acc.dzz += part.dzz; acc.kr += part.kr; acc.kz += part.kz;
-}
-
-// Deterministic summation order: the j range is cut into chunks of
-// PAIR_CHUNK points from j = 0; each chunk's partial sum starts from zero and the chunk partials
-// are added in chunk order.  Both launch shapes below follow that order, so a batched build is
-// bitwise equal to single builds.
+// ------------------------------------------------------------------------------------------------
+// Symmetric tile-pair kernel.  P0, Pc, Pss are exchange-symmetric and
+//   U^D_rr(j,i) = ri^2 Pss + dz^2 P0,  U^D_rz(j,i) = U^K_zr(i,j),  U^D_zz(j,i) = U^D_zz(i,j),
+//   U^K_rr(j,i) = U^K_rr(i,j),  U^K_zr(j,i) = U^D_rz(i,j)
+// so one elliptic evaluation serves the ordered pairs (i,j) and (j,i) (the paper notes the
+// symmetry, L193, and does not exploit it).
 //
-// SPLIT = false (batch fills the GPU): grid = (ceil(N/PAIR_THREADS), 1, nb); each thread owns one
-//   i, streams ALL j through shared memory in tiles of PAIR_TILE and writes G[b][5][N].
-// SPLIT = true (few problems): grid = (ceil(N/PAIR_THREADS), nchunks, nb); each block does one
-//   chunk and writes its partial to Gpart[b][chunk][5][N]; k_element / k_sum_partials add them.
-// r,z,invr [N] are shared by the batch; T[b][3][N] = w_in * (T_D, T_Kr, T_Kz).
-// The coincident pair is tested only in chunks that overlap the block's own i range.
-template <bool SPLIT>
-__global__ void __launch_bounds__(PAIR_THREADS, 6)
-k_pair(int N, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
-       const double *__restrict__ T, double *__restrict__ Gout) {
-    constexpr int TILE = SPLIT ? PAIR_CHUNK : PAIR_TILE;
-    __shared__ JPoint sj[TILE];
-    const int b = blockIdx.z;
-    const int ibase = blockIdx.x * PAIR_THREADS;
-    const int i = ibase + threadIdx.x;
-    const int ic = i < N ? i : N - 1;
-    const double ri = r[ic], zi = z[ic];
-    const double ri4 = 4.0 * ri, inv4ri = 0.25 * invr[ic];
+// Points are cut into tiles of TS; block (I <= J, problem b), TS threads, thread t owns
+// i = I*TS + t and walks the j of tile J through shared memory (broadcast reads).  It keeps the
+// i-side sums in registers; the j-side terms are butterfly-reduced over the warp and parked in
+// shared memory per warp, then added over the warps in warp order.  Diagonal blocks (I == J) do
+// all ordered pairs of the tile with the coincident-pair test.
+//
+// Deterministic order: Gpart[b][src tile][5][N] holds, for every target
+// point, the partial sum over the points of one source tile; each slot is written by exactly one
+// block, and k_element / k_sum_partials add the slabs in tile order.  TS depends on N only, so a
+// batched build is bitwise equal to single builds.
+// ------------------------------------------------------------------------------------------------
+template <int TS>
+__global__ void __launch_bounds__(TS)
+k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
+           const double *__restrict__ T, double *__restrict__ Gpart) {
+    constexpr int NW = TS / 32;
+    __shared__ JPoint sj[TS];
+    __shared__ double sacc[NW][5][TS];
+    const int b = blockIdx.y;
+    // linear tile-pair index p = J (J+1)/2 + I, I <= J
+    const int p = blockIdx.x;
+    int J = int((sqrt(8.0 * double(p) + 1.0) - 1.0) * 0.5);
+    while ((J + 1) * (J + 2) / 2 <= p) ++J;
+    while (J * (J + 1) / 2 > p) --J;
+    const int I = p - J * (J + 1) / 2;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double *Tb = T + (size_t)b * 3 * N;
+    const int i = I * TS + tid;
+    const bool valid = i < N;
+    const int ic = valid ? i : N - 1;
+    const double ri = r[ic], zi = z[ic];
+    const double ri4 = 4.0 * ri, inv4ri = 0.25 * invr[ic], ri2 = ri * ri;
+    const double tDi = valid ? Tb[ic] : 0.0, tKri = valid ? Tb[N + ic] : 0.0, tKzi = valid ? Tb[2 * N + ic] : 0.0;
+    const int jbase = J * TS;
+    const int cnt = min(TS, N - jbase);
+    if (tid < cnt) {
+        JPoint pj;
+        const int j = jbase + tid;
+        pj.r = r[j]; pj.z = z[j]; pj.invr = invr[j];
+        pj.tD = Tb[j]; pj.tKr = Tb[N + j]; pj.tKz = Tb[2 * N + j];
+        sj[tid] = pj;
+    }
+    __syncthreads();
     PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
-    const int j0 = SPLIT ? blockIdx.y * PAIR_CHUNK : 0;
-    const int j1 = SPLIT ? min(N, j0 + PAIR_CHUNK) : N;
-    for (int jt = j0; jt < j1; jt += TILE) {
-        const int cnt = min(TILE, j1 - jt);
-        __syncthreads();
-        for (int t = threadIdx.x; t < cnt; t += PAIR_THREADS) {
-            JPoint pj;
-            pj.r = r[jt + t]; pj.z = z[jt + t]; pj.invr = invr[jt + t];
-            pj.tD = Tb[jt + t]; pj.tKr = Tb[N + jt + t]; pj.tKz = Tb[2 * N + jt + t];
-            sj[t] = pj;
+    if (I == J) {
+        for (int t = 0; t < cnt; ++t) {
+            const JPoint pj = sj[t];
+            const PairParts pp = pair_parts<true>(ri, zi, ri4, inv4ri, pj);
+            const double UDrr = fma(pj.r * pj.r, pp.Pss, pp.dz2 * pp.P0);
+            const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
+            const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
+            const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
+            const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);
+            acc.drr = fma(pj.tD, UDrr, acc.drr);
+            acc.drz = fma(-pj.tD, nUDrz, acc.drz);
+            acc.dzz = fma(pj.tD, UDzz, acc.dzz);
+            acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
+            acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
         }
-        __syncthreads();
-        for (int c0 = 0; c0 < cnt; c0 += PAIR_CHUNK) {
-            const int clen = min(PAIR_CHUNK, cnt - c0);
-            const int jg = jt + c0;                                   // global j of the chunk start
-            const bool overlap = jg < ibase + PAIR_THREADS && jg + clen > ibase;   // block-uniform
-            if (overlap) pair_chunk<true>(ri, zi, ri4, inv4ri, sj + c0, clen, acc);
-            else pair_chunk<false>(ri, zi, ri4, inv4ri, sj + c0, clen, acc);
+    } else {
+        for (int t = 0; t < cnt; ++t) {
+            const JPoint pj = sj[t];
+            const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
+            const double dzP0 = pp.dz2 * pp.P0;
+            const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
+            const double UDrrT = fma(ri2, pp.Pss, dzP0);                          // U^D_rr(j,i)
+            const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
+            const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
+            const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
+            const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);           // = U^D_rz(j,i)
+            acc.drr = fma(pj.tD, UDrr, acc.drr);
+            acc.drz = fma(-pj.tD, nUDrz, acc.drz);
+            acc.dzz = fma(pj.tD, UDzz, acc.dzz);
+            acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
+            acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
+            // terms of target j from source i
+            double v0 = tDi * UDrrT, v1 = tDi * UKzr, v2 = tDi * UDzz;
+            double v3 = fma(UKrr, tKri, UKzr * tKzi);
+            double v4 = fma(-nUDrz, tKri, UDzz * tKzi);
+#pragma unroll
+            for (int o = 16; o > 0; o >>= 1) {
+                v0 += __shfl_xor_sync(0xffffffffu, v0, o);
+                v1 += __shfl_xor_sync(0xffffffffu, v1, o);
+                v2 += __shfl_xor_sync(0xffffffffu, v2, o);
+                v3 += __shfl_xor_sync(0xffffffffu, v3, o);
+                v4 += __shfl_xor_sync(0xffffffffu, v4, o);
+            }
+            if (lane == 0) {
+                sacc[warp][0][t] = v0; sacc[warp][1][t] = v1; sacc[warp][2][t] = v2;
+                sacc[warp][3][t] = v3; sacc[warp][4][t] = v4;
+            }
         }
     }
-    if (i < N) {
-        double *G = Gout + (SPLIT ? ((size_t)b * gridDim.y + blockIdx.y) : (size_t)b) * 5 * N;
+    if (valid) {
+        double *G = Gpart + ((size_t)b * ntiles + J) * 5 * N;
         G[i] = acc.drr; G[N + i] = acc.drz; G[2 * N + i] = acc.dzz; G[3 * N + i] = acc.kr; G[4 * N + i] = acc.kz;
+    }
+    if (I != J) {
+        __syncthreads();
+        if (tid < cnt) {
+            double *G = Gpart + ((size_t)b * ntiles + I) * 5 * N + jbase + tid;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                double sum = sacc[0][c][tid];
+#pragma unroll
+                for (int w = 1; w < NW; ++w) sum += sacc[w][c][tid];
+                G[(size_t)c * N] = sum;
+            }
+        }
     }
 }
 
@@ -340,13 +396,9 @@ __global__ void k_dfma_probe(int iters, double *out) {
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-int pair_chunks(int N) { return (N + PAIR_CHUNK - 1) / PAIR_CHUNK; }
-
-// Split the j range over blocks when the batch alone cannot give every SM four 128-thread blocks.
-bool pair_use_split(int N, int nb, int num_sms) {
-    const long long itiles = (N + PAIR_THREADS - 1) / PAIR_THREADS;
-    return itiles * nb < 4LL * num_sms;
-}
+// Tile size of the pair kernel: a function of N ONLY (it fixes the summation order).
+int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 1024 ? 64 : 32); }
+int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / ts; }
 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
     dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
@@ -354,10 +406,12 @@ int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T
     return 1;
 }
 
-int launch_pair(const DeviceSpace &ds, int nb, bool split, const double *T, double *G, cudaStream_t st) {
-    dim3 grid((ds.N + PAIR_THREADS - 1) / PAIR_THREADS, split ? pair_chunks(ds.N) : 1, nb);
-    if (split) k_pair<true><<<grid, PAIR_THREADS, 0, st>>>(ds.N, ds.r, ds.z, ds.invr, T, G);
-    else k_pair<false><<<grid, PAIR_THREADS, 0, st>>>(ds.N, ds.r, ds.z, ds.invr, T, G);
+int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st) {
+    const int ts = pair_tile_size(ds.N), nt = pair_tiles(ds.N);
+    dim3 grid(nt * (nt + 1) / 2, nb);
+    if (ts == 128) k_pair_sym<128><<<grid, 128, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    else if (ts == 64) k_pair_sym<64><<<grid, 64, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    else k_pair_sym<32><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
     return 1;
 }
 

@@ -6,9 +6,6 @@
 
 namespace landau {
 
-constexpr int PAIR_THREADS = 128;  // i points per block of the pair kernel
-constexpr int PAIR_TILE = 256;     // j points staged in shared memory per tile (batch shape)
-constexpr int PAIR_CHUNK = 64;     // summation granule: chunk partials are added in chunk order
 constexpr int MAX_SPECIES = 16;
 
 // Device-resident description of one mesh/order/species set (all pointers device memory,
@@ -32,14 +29,15 @@ struct DeviceSpace {
 // Scratch for up to max_batch problems.
 struct Scratch {
     double *T;      // [nb][3][N]
-    double *G;      // [nb][5][N] (batch shape) or [nb][nchunks][5][N] (split shape)
+    double *G;      // [nb][ntiles][5][N]: per source tile partial sums of G_D, G_K
+    double *Gsum;   // [nb][5][N]: G_D (rr,rz,zz), G_K (r,z) after the tile-order sum
     double *Ce;     // [nb][S][Ne][Nb*Nb]
     double *ce;     // [nb][S][Ne][Nb]
 };
 
 // each returns the number of kernels launched
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
-int launch_pair(const DeviceSpace &ds, int nb, bool split, const double *T, double *G, cudaStream_t st);
+int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st);
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce,
                    double *ce, cudaStream_t st);
 int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st);
@@ -48,7 +46,7 @@ int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStr
 int launch_sum_partials(const DeviceSpace &ds, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
 
-int pair_chunks(int N);
-bool pair_use_split(int N, int nb, int num_sms);
+int pair_tile_size(int N);
+int pair_tiles(int N);
 
 }  // namespace landau
