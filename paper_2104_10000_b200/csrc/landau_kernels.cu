@@ -132,9 +132,9 @@ __device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4
 // symmetry, L193, and does not exploit it).
 //
 // Points are cut into tiles of TS; block (I <= J, problem b), TS threads, thread t owns
-// i = I*TS + t and walks the j of tile J through shared memory (broadcast reads).  It keeps the
-// i-side sums in registers; the j-side terms are butterfly-reduced over the warp and parked in
-// shared memory per warp, then added over the warps in warp order.  Diagonal blocks (I == J) do
+// i = I*TS + t and walks the j of tile J held in shared memory.  It keeps the i-side sums in
+// registers; the j-side sums rotate around the warp's lanes together with their j (see below) and
+// are parked in shared memory per warp, then added over the warps in warp order.  Diagonal blocks (I == J) do
 // all ordered pairs of the tile with the coincident-pair test.
 //
 // Deterministic order: Gpart[b][src tile][5][N] holds, for every target
@@ -172,6 +172,11 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
         pj.r = r[j]; pj.z = z[j]; pj.invr = invr[j];
         pj.tD = Tb[j]; pj.tKr = Tb[N + j]; pj.tKz = Tb[2 * N + j];
         sj[tid] = pj;
+    } else {
+        // padding of a ragged tile: a far-away point with zero weight (finite tensor, no effect)
+        JPoint pj;
+        pj.r = 1.0; pj.z = 1.0e6; pj.invr = 1.0; pj.tD = 0.0; pj.tKr = 0.0; pj.tKz = 0.0;
+        sj[tid] = pj;
     }
     __syncthreads();
     PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
@@ -191,37 +196,44 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
             acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
         }
     } else {
-        for (int t = 0; t < cnt; ++t) {
-            const JPoint pj = sj[t];
-            const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
-            const double dzP0 = pp.dz2 * pp.P0;
-            const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
-            const double UDrrT = fma(ri2, pp.Pss, dzP0);                          // U^D_rr(j,i)
-            const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
-            const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
-            const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
-            const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);           // = U^D_rz(j,i)
-            acc.drr = fma(pj.tD, UDrr, acc.drr);
-            acc.drz = fma(-pj.tD, nUDrz, acc.drz);
-            acc.dzz = fma(pj.tD, UDzz, acc.dzz);
-            acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
-            acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
-            // terms of target j from source i
-            double v0 = tDi * UDrrT, v1 = tDi * UKzr, v2 = tDi * UDzz;
-            double v3 = fma(UKrr, tKri, UKzr * tKzi);
-            double v4 = fma(-nUDrz, tKri, UDzz * tKzi);
-#pragma unroll
-            for (int o = 16; o > 0; o >>= 1) {
-                v0 += __shfl_xor_sync(0xffffffffu, v0, o);
-                v1 += __shfl_xor_sync(0xffffffffu, v1, o);
-                v2 += __shfl_xor_sync(0xffffffffu, v2, o);
-                v3 += __shfl_xor_sync(0xffffffffu, v3, o);
-                v4 += __shfl_xor_sync(0xffffffffu, v4, o);
+        // Lane t walks the 32 j of a sub-tile in rotated order, j = (t + k) mod 32, so that the warp
+        // touches 32 different j per step; the j-side sums travel around the lanes with their j
+        // (one shuffle per value per step) and need no cross-lane reduction.
+        const int nsub = (cnt + 31) >> 5;
+        for (int sub = 0; sub < nsub; ++sub) {
+            double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
+#pragma unroll 1
+            for (int k = 0; k < 32; ++k) {
+                const JPoint pj = sj[sub * 32 + ((lane + k) & 31)];
+                const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
+                const double dzP0 = pp.dz2 * pp.P0;
+                const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
+                const double UDrrT = fma(ri2, pp.Pss, dzP0);                          // U^D_rr(j,i)
+                const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
+                const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
+                const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
+                const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);           // = U^D_rz(j,i)
+                acc.drr = fma(pj.tD, UDrr, acc.drr);
+                acc.drz = fma(-pj.tD, nUDrz, acc.drz);
+                acc.dzz = fma(pj.tD, UDzz, acc.dzz);
+                acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
+                acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
+                // terms of target j from source i, then pass the sums on with their j
+                v0 = fma(tDi, UDrrT, v0);
+                v1 = fma(tDi, UKzr, v1);
+                v2 = fma(tDi, UDzz, v2);
+                v3 = fma(UKrr, tKri, fma(UKzr, tKzi, v3));
+                v4 = fma(-nUDrz, tKri, fma(UDzz, tKzi, v4));
+                const int src = (lane + 1) & 31;
+                v0 = __shfl_sync(0xffffffffu, v0, src);
+                v1 = __shfl_sync(0xffffffffu, v1, src);
+                v2 = __shfl_sync(0xffffffffu, v2, src);
+                v3 = __shfl_sync(0xffffffffu, v3, src);
+                v4 = __shfl_sync(0xffffffffu, v4, src);
             }
-            if (lane == 0) {
-                sacc[warp][0][t] = v0; sacc[warp][1][t] = v1; sacc[warp][2][t] = v2;
-                sacc[warp][3][t] = v3; sacc[warp][4][t] = v4;
-            }
+            const int jl = sub * 32 + lane;
+            sacc[warp][0][jl] = v0; sacc[warp][1][jl] = v1; sacc[warp][2][jl] = v2;
+            sacc[warp][3][jl] = v3; sacc[warp][4][jl] = v4;
         }
     }
     if (valid) {
