@@ -27,6 +27,7 @@ def build(force: bool = False, verbose: bool = False) -> str:
            "-Xcompiler", "-fPIC", "-shared", "-I", os.path.join(ROOT, "include"), "-I", os.path.join(HERE, "csrc")]
     if verbose:
         cmd += ["-Xptxas", "-v"]
+    cmd += os.environ.get("LANDAU_NVCC_FLAGS", "").split()   # e.g. -DPAIR_MIN_BLOCKS=6 for tuning sweeps
     cmd += [os.path.join(HERE, "csrc", s) for s in SOURCES] + ["-o", LIB]
     subprocess.check_call(cmd)
     return LIB
