@@ -32,9 +32,10 @@ import numpy as np
 METRIC = "landau_jacobian_gpair_evals_per_s"
 UNIT = "GPair/s"
 WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
-# FP64 flop per ordered pair executed by k_pair (DFMA x 2 + DMUL + DADD, ncu-counted,
-# profiles/r01a_pair_kernel.md).
-FLOP_PER_PAIR = 196.0
+# FP64 flop (2 DFMA + DMUL + DADD) and FP64-pipe instructions the pair kernel executes per ORDERED
+# pair on this workload, ncu-counted (profiles/r01_pair_kernel.md).
+FLOP_PER_PAIR = 82.8
+FP64_INST_PER_PAIR = 56.65
 FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
 
 
@@ -231,11 +232,13 @@ def run_ours(args):
         nominal_peak = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
         pair_launch_ms = pair_ms / max(pair_cnt, 1)
         achieved = FLOP_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) * 1e-12
-        roof = {"bound": "alu", "kernel": "k_pair<false>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
+        roof = {"bound": "alu", "kernel": "k_pair_sym<128>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
                 "frac": achieved / nominal_peak, "traffic": None,
                 "peak_source": "derived: SMs x 64 DFMA lanes x 2 x clocks.max.sm (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
                 "peak_probe_measured": peak_flops * 1e-12, "frac_of_probe": achieved / (peak_flops * 1e-12),
-                "flop_per_pair": FLOP_PER_PAIR, "kernel_ms_per_launch": pair_launch_ms,
+                "flop_per_pair": FLOP_PER_PAIR,
+                "fp64_pipe_frac": FP64_INST_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) / (nominal_peak * 0.5e12),
+                "kernel_ms_per_launch": pair_launch_ms,
                 "kernel_share_of_step": pair_ms / total_ms if world == 1 else None,
                 "kernel_gpair_per_s": pairs_per_step / (pair_launch_ms * 1e-3) * 1e-9}
         cpu_val, cpu_dt, cores = cpu_baseline_sample(wl, inputs)
