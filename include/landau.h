@@ -118,7 +118,8 @@ int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double
 int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream);
 
 /* End-to-end variant with HOST buffers (pageable or pinned): copies f to the device, runs
- * landau_jacobian_batched on the ctx's own stream, copies vals/Cf back, and synchronises. */
+ * landau_jacobian_batched on the ctx's own stream in sub-batches whose device-to-host copies overlap
+ * the next sub-batch's build, and synchronises.  Values are bitwise those of the device entry point. */
 int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *vals_host, double *Cf_host);
 
 /* Number of kernel launches the ctx has enqueued since creation (for bench.py's gpu_launches). */

@@ -49,7 +49,8 @@ struct landau_ctx {
     int max_batch = 1;
     int num_sms = 148;
     int64_t launches = 0;
-    cudaStream_t own_stream = nullptr;
+    cudaStream_t own_stream = nullptr, copy_stream = nullptr;
+    cudaEvent_t chunk_done = nullptr;
     double *h2d_f = nullptr, *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
     int host_nb = 0;
     bool profiling = false;
@@ -93,6 +94,8 @@ int landau_destroy(landau_ctx *ctx) {
     if (ctx->d_vals) cudaFree(ctx->d_vals);
     if (ctx->d_Cf) cudaFree(ctx->d_Cf);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
+    if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
+    if (ctx->chunk_done) cudaEventDestroy(ctx->chunk_done);
     for (auto &ev : ctx->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     for (auto &ev : ctx->prof_pool) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
     delete ctx;
@@ -277,7 +280,11 @@ int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream) 
 int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *vals_host, double *Cf_host) {
     if (!ctx || !f_host || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     const DeviceSpace &ds = ctx->ds;
-    if (!ctx->own_stream) CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+    if (!ctx->own_stream) {
+        CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
+        CK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
+        CK(cudaEventCreateWithFlags(&ctx->chunk_done, cudaEventDisableTiming));
+    }
     if (ctx->host_nb < nb) {
         if (ctx->d_f) { cudaFree(ctx->d_f); cudaFree(ctx->d_vals); cudaFree(ctx->d_Cf); ctx->d_f = ctx->d_vals = ctx->d_Cf = nullptr; }
         cudaError_t e = cudaMalloc((void **)&ctx->d_f, size_t(nb) * ds.S * ds.n * sizeof(double));
@@ -286,13 +293,26 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
         if (e != cudaSuccess) { ctx->host_nb = 0; return cuda_fail(e, "cudaMalloc(host staging)"); }
         ctx->host_nb = nb;
     }
-    cudaStream_t st = ctx->own_stream;
-    CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * ds.S * ds.n * sizeof(double), cudaMemcpyHostToDevice, st));
-    int rc = landau_jacobian_batched(ctx, nb, ctx->d_f, vals_host ? ctx->d_vals : nullptr, Cf_host ? ctx->d_Cf : nullptr, st);
-    if (rc != LANDAU_OK) return rc;
-    if (vals_host) CK(cudaMemcpyAsync(vals_host, ctx->d_vals, size_t(nb) * ds.S * ds.nnz * sizeof(double), cudaMemcpyDeviceToHost, st));
-    if (Cf_host) CK(cudaMemcpyAsync(Cf_host, ctx->d_Cf, size_t(nb) * ds.S * ds.n * sizeof(double), cudaMemcpyDeviceToHost, st));
+    // Pipeline over sub-batches: the device-to-host copy of chunk c overlaps the build of chunk
+    // c+1 (the scratch arena is reused in stream order; problems are independent, so the values
+    // are bitwise those of one batched call).
+    cudaStream_t st = ctx->own_stream, cp = ctx->copy_stream;
+    const size_t fsz = size_t(ds.S) * ds.n, vsz = size_t(ds.S) * ds.nnz;
+    CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
+    const int nchunks = nb >= 8 ? 4 : 1;
+    const int cb = (nb + nchunks - 1) / nchunks;
+    for (int b0 = 0; b0 < nb; b0 += cb) {
+        const int nbc = std::min(cb, nb - b0);
+        int rc = landau_jacobian_batched(ctx, nbc, ctx->d_f + b0 * fsz, vals_host ? ctx->d_vals + b0 * vsz : nullptr,
+                                         Cf_host ? ctx->d_Cf + b0 * fsz : nullptr, st);
+        if (rc != LANDAU_OK) return rc;
+        CK(cudaEventRecord(ctx->chunk_done, st));
+        CK(cudaStreamWaitEvent(cp, ctx->chunk_done, 0));
+        if (vals_host) CK(cudaMemcpyAsync(vals_host + b0 * vsz, ctx->d_vals + b0 * vsz, size_t(nbc) * vsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
+        if (Cf_host) CK(cudaMemcpyAsync(Cf_host + b0 * fsz, ctx->d_Cf + b0 * fsz, size_t(nbc) * fsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
+    }
     CK(cudaStreamSynchronize(st));
+    CK(cudaStreamSynchronize(cp));
     return LANDAU_OK;
 }
 

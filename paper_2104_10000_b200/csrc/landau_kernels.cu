@@ -43,17 +43,21 @@ __device__ __forceinline__ void sqrt_rsqrt_fast(double x, double &g, double &yy)
     yy = fma(y, p, y);
 }
 
-// 2 sqrt(x): the factor 2 is put into the seed's exponent (integer add on the high word), so the
-// scaled AGM below needs no multiplication by 1/2 or 2 on the FP64 pipe.
+// 2 sqrt(x) = t (2 + r + 3 r^2/4), t = x y, r = 1 - x y^2: the factor 2 sits in the correction
+// polynomial, so the scaled AGM below needs no multiplication by 1/2 or 2 and no integer fix-up.
 __device__ __forceinline__ double sqrt_times2_fast(double x) {
     double y;
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double y2 = __hiloint2double(__double2hiint(y) + 0x00100000, __double2loint(y));
-    const double t = x * y2;            // ~ 2 sqrt(x)
-    const double r2 = fma(-t, y, 2.0);  // 2 (1 - x y^2)
-    double p = fma(0.09375, r2, 0.25);
-    p = p * r2;                         // r/2 + 3 r^2/8
-    return fma(t, p, t);
+    const double t = x * y;
+    const double r = fma(-t, y, 1.0);
+    const double p = fma(0.75, r, 1.0);
+    const double q = fma(p, r, 2.0);
+    return t * q;
+}
+
+// x * 2^e for a normal positive x that stays normal (integer add on the exponent field)
+__device__ __forceinline__ double scale_pow2(double x, int e) {
+    return __hiloint2double(__double2hiint(x) + (e << 20), __double2loint(x));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -63,12 +67,13 @@ __device__ __forceinline__ double sqrt_times2_fast(double x) {
 // integrals on the device").  With a0 = sqrt(s), b0 = sqrt(d2), q = 4 r rb = s - d2 and
 // A_k = 2^k a_k, B_k = 2^k b_k:
 //     A_{k+1} = A_k + B_k,  B_{k+1} = 2 sqrt(A_k B_k),  C_{k+1} = A_k - B_k = 2^{k+1} c_{k+1}
+//     (powers of two are applied at the end by integer adds on the exponent field)
 //     K(m)/sqrt(s) = pi/(2 lim a_k) = pi 2^k / A_{k+1}
 //     W = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(2 A_1^2) + (sum_{k>=2} C_k^2 / 2^k)/q^2   (c_1 = q/(4 a_1))
 //     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2),  Kt = K/sqrt(s)
 // every sum has positive terms except the bracket of P0 (= 2 s E/K: bounded cancellation ~ K/E).
-// The iteration stops for the whole warp once every lane has c_{k+1} < 2^-26 a_k (the neglected
-// c_{k+2} ~ c_{k+1}^2/(4a) is then < 6e-17 a).  The test compares exponents with integer ops.
+// The iteration stops for the whole warp once every lane's next c would be < 2^-27 a (the then
+// neglected term is < 6e-17 a).  The test compares exponents with integer ops, one pass ahead.
 // ------------------------------------------------------------------------------------------------
 struct PairAcc { double drr, drz, dzz, kr, kz; };
 struct __align__(16) JPoint { double r, z, invr, tD, tKr, tKz; };
@@ -95,26 +100,35 @@ __device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4
     double a0, b0, ys, yd;
     sqrt_rsqrt_fast(s, a0, ys);
     sqrt_rsqrt_fast(d2, b0, yd);
-    double A = a0 + b0;               // 2 a_1
+    double A = a0 + b0;               // A_1 = 2 a_1
     double B = sqrt_times2_fast(a0 * b0);
     const double iA1 = rcp_fast(A);
-    double wsum = 0.0, kscale = 6.283185307179586476925286766559;   // 2 Kt = kscale / A_final
-#pragma unroll
-    for (int k = 1; k <= AGM_MAX_STEPS; ++k) {
+    // Rolled loop, state in fixed registers.  V_P = 2 V_{P-1} + C_{P+1}^2, so after P passes
+    // sum_{k>=2} C_k^2/2^k = V / 2^{P+1}, and 2 K/sqrt(s) = 2 pi 2^P / A_{P+1}.
+    // The exit is decided ONE PASS AHEAD so that the branch never waits on fresh data:
+    // c_{k+2} = c_{k+1}^2/(4 a_{k+2}) exactly, hence C_{k+1} <= 2^-12 A_k in every lane guarantees
+    // c_{k+2} < 2^-27 a after the next pass, which is then the last (its C only feeds V).
+    double V = 0.0;
+    int P = 0;
+    bool last = false;
+#pragma unroll 1
+    for (;;) {
         const double C = A - B;
-        const double An = A + B;
-        wsum = fma(C * (1.0 / double(1 << (k + 1))), C, wsum);
-        kscale = 6.283185307179586476925286766559 * double(1 << k);
-        const bool conv = __double2hiint(C) + (27 << 20) <= __double2hiint(A);
-        if (k == AGM_MAX_STEPS || __all_sync(0xffffffffu, conv)) { A = An; break; }
-        B = sqrt_times2_fast(A * B);
-        A = An;
+        V = fma(V, 2.0, C * C);
+        ++P;
+        if (last || P == AGM_MAX_STEPS) break;
+        last = __all_sync(0xffffffffu, __double2hiint(C) + (13 << 20) <= __double2hiint(A));
+        const double X = A * B;
+        A = A + B;
+        B = sqrt_times2_fast(X);
     }
-    const double KP2 = kscale * rcp_fast(A);          // 2 K/sqrt(s)
+    A = A + B;
+    const double KP2 = scale_pow2(6.283185307179586476925286766559 * rcp_fast(A), P);   // 2 K/sqrt(s)
     const double q = ri4 * rj;
     pp.rho = ri * rj;
     const double invq = inv4ri * pj.invr;
-    const double W = fma(0.5 * iA1, iA1, wsum * (invq * invq));
+    // 1/q^2 is a normal number far from the exponent limits (V may be 0 for far pairs: scale 1/q^2, not the product)
+    const double W = fma(0.5 * iA1, iA1, V * scale_pow2(invq * invq, -(P + 1)));
     const double Ks = KP2 * (ys * ys);
     const double x = q * W;
     pp.Pc = Ks * fma(2.0, x, 2.0);
@@ -142,12 +156,15 @@ __device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4
 // block, and k_element / k_sum_partials add the slabs in tile order.  TS depends on N only, so a
 // batched build is bitwise equal to single builds.
 // ------------------------------------------------------------------------------------------------
+#ifndef PAIR_MIN_BLOCKS
+#define PAIR_MIN_BLOCKS 5   // resident blocks per SM the register budget is capped for (sweep 4/5/6: 239/247/246 GPair/s)
+#endif
 template <int TS>
-__global__ void __launch_bounds__(TS)
+__global__ void __launch_bounds__(TS, PAIR_MIN_BLOCKS)
 k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
            const double *__restrict__ T, double *__restrict__ Gpart) {
     constexpr int NW = TS / 32;
-    __shared__ JPoint sj[TS];
+    __shared__ JPoint sj[2 * TS];        // every 32-point sub-tile is stored twice in a row: rotated walks need no wrap
     __shared__ double sacc[NW][5][TS];
     const int b = blockIdx.y;
     // linear tile-pair index p = J (J+1)/2 + I, I <= J
@@ -166,23 +183,24 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
     const double tDi = valid ? Tb[ic] : 0.0, tKri = valid ? Tb[N + ic] : 0.0, tKzi = valid ? Tb[2 * N + ic] : 0.0;
     const int jbase = J * TS;
     const int cnt = min(TS, N - jbase);
-    if (tid < cnt) {
+    {
         JPoint pj;
-        const int j = jbase + tid;
-        pj.r = r[j]; pj.z = z[j]; pj.invr = invr[j];
-        pj.tD = Tb[j]; pj.tKr = Tb[N + j]; pj.tKz = Tb[2 * N + j];
-        sj[tid] = pj;
-    } else {
-        // padding of a ragged tile: a far-away point with zero weight (finite tensor, no effect)
-        JPoint pj;
-        pj.r = 1.0; pj.z = 1.0e6; pj.invr = 1.0; pj.tD = 0.0; pj.tKr = 0.0; pj.tKz = 0.0;
-        sj[tid] = pj;
+        if (tid < cnt) {
+            const int j = jbase + tid;
+            pj.r = r[j]; pj.z = z[j]; pj.invr = invr[j];
+            pj.tD = Tb[j]; pj.tKr = Tb[N + j]; pj.tKz = Tb[2 * N + j];
+        } else {
+            // padding of a ragged tile: a far-away point with zero weight (finite tensor, no effect)
+            pj.r = 1.0; pj.z = 1.0e6; pj.invr = 1.0; pj.tD = 0.0; pj.tKr = 0.0; pj.tKz = 0.0;
+        }
+        sj[warp * 64 + lane] = pj;
+        sj[warp * 64 + 32 + lane] = pj;
     }
     __syncthreads();
     PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (I == J) {
         for (int t = 0; t < cnt; ++t) {
-            const JPoint pj = sj[t];
+            const JPoint pj = sj[(t >> 5) * 64 + (t & 31)];
             const PairParts pp = pair_parts<true>(ri, zi, ri4, inv4ri, pj);
             const double UDrr = fma(pj.r * pj.r, pp.Pss, pp.dz2 * pp.P0);
             const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
@@ -200,11 +218,13 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
         // touches 32 different j per step; the j-side sums travel around the lanes with their j
         // (one shuffle per value per step) and need no cross-lane reduction.
         const int nsub = (cnt + 31) >> 5;
+        const int src = (lane + 1) & 31;
         for (int sub = 0; sub < nsub; ++sub) {
             double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
+            const JPoint *pjp = sj + sub * 64 + lane;
 #pragma unroll 1
             for (int k = 0; k < 32; ++k) {
-                const JPoint pj = sj[sub * 32 + ((lane + k) & 31)];
+                const JPoint pj = pjp[k];
                 const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
                 const double dzP0 = pp.dz2 * pp.P0;
                 const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
@@ -224,7 +244,6 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
                 v2 = fma(tDi, UDzz, v2);
                 v3 = fma(UKrr, tKri, fma(UKzr, tKzi, v3));
                 v4 = fma(-nUDrz, tKri, fma(UDzz, tKzi, v4));
-                const int src = (lane + 1) & 31;
                 v0 = __shfl_sync(0xffffffffu, v0, src);
                 v1 = __shfl_sync(0xffffffffu, v1, src);
                 v2 = __shfl_sync(0xffffffffu, v2, src);
