@@ -156,6 +156,10 @@ __device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4
 // block, and k_element / k_sum_partials add the slabs in tile order.  TS depends on N only, so a
 // batched build is bitwise equal to single builds.
 // ------------------------------------------------------------------------------------------------
+#ifndef PAIR_K_UNROLL
+#define PAIR_K_UNROLL 2   // j steps per loop trip (sweep 1/2: 247/253 GPair/s)
+#endif
+constexpr int kPairUnroll = PAIR_K_UNROLL;
 #ifndef PAIR_MIN_BLOCKS
 #define PAIR_MIN_BLOCKS 5   // resident blocks per SM the register budget is capped for (sweep 4/5/6: 239/247/246 GPair/s)
 #endif
@@ -221,10 +225,14 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
         const int src = (lane + 1) & 31;
         for (int sub = 0; sub < nsub; ++sub) {
             double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
-            const JPoint *pjp = sj + sub * 64 + lane;
-#pragma unroll 1
-            for (int k = 0; k < 32; ++k) {
-                const JPoint pj = pjp[k];
+            // explicit 32-bit shared address, advanced by one JPoint per step (three 16-byte loads)
+            unsigned sa = (unsigned)__cvta_generic_to_shared(sj + sub * 64 + lane);
+#pragma unroll kPairUnroll
+            for (int k = 0; k < 32; ++k, sa += (unsigned)sizeof(JPoint)) {
+                JPoint pj;
+                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(pj.r), "=d"(pj.z) : "r"(sa));
+                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+16];" : "=d"(pj.invr), "=d"(pj.tD) : "r"(sa));
+                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+32];" : "=d"(pj.tKr), "=d"(pj.tKz) : "r"(sa));
                 const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
                 const double dzP0 = pp.dz2 * pp.P0;
                 const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
