@@ -333,15 +333,19 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
 }
 
 // ------------------------------------------------------------------------------------------------
-// a4 + a5 (+ element part of a7): Alg. 1 lines 13-23 (L122-131).  grid = (Ne, S, nb),
-// block = Nb*Nb threads, thread (a,b) owns C_e[a][b].  Partial G over the j splits are summed
-// here in fixed order.  Also writes ce = C_e u (u = P_e f_alpha), the element vector of C(f).
+// a4 + a5 (+ element part of a7): Alg. 1 lines 13-23 (L122-131).  grid = (Ne, nb), block = Nb*Nb
+// threads; the block loops over the species (tabulations and G are loaded once per cell).
+// Two phases per species, both thread-per-entry on Nq x Nb = Nb x Nb arrays:
+//   X[q][b] = DDrr_q E0_qb + DDrz_q E1_qb + KKr_q B_qb,   Y[q][b] = DDrz_q E0_qb + DDzz_q E1_qb + KKz_q B_qb
+//   C_e[a][b] = sum_q ( E0_qa X_qb + E1_qa Y_qb )
+// (the same sum as line 23, factored so that the q loop is two FMAs).  Also writes ce = C_e u
+// (u = P_e f_alpha), the element vector of C(f).  G is the tile-order sum of the pair kernel's slabs.
 // ------------------------------------------------------------------------------------------------
 __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gpart,
                           double *__restrict__ Ce, double *__restrict__ ce) {
-    __shared__ double s_c[16][5];
-    __shared__ double s_B[256], s_E0[256], s_E1[256], s_Ce[256], s_u[16];
-    const int e = blockIdx.x, sp = blockIdx.y, b = blockIdx.z;
+    __shared__ double s_g[16][5];      // w_out * (invJ-transformed G_D rr, rz, zz, G_K r, z), species-independent
+    __shared__ double s_B[256], s_E0[256], s_E1[256], s_X[256], s_Y[256], s_Ce[256], s_u[16];
+    const int e = blockIdx.x, b = blockIdx.y;
     const int Nb = ds.Nb, Nq = ds.Nq, N = ds.N;
     const int tid = threadIdx.x;
     s_B[tid] = ds.B[tid]; s_E0[tid] = ds.E0[tid]; s_E1[tid] = ds.E1[tid];
@@ -354,38 +358,42 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
             for (int c = 0; c < 5; ++c) g[c] += G[c * N + gi];
         }
         const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1], w = ds.w_out[gi];
-        const double kf = ds.kfac[sp] * w, df = ds.dfac[sp] * w;
-        s_c[tid][0] = ir * ir * df * g[0];
-        s_c[tid][1] = ir * iz * df * g[1];
-        s_c[tid][2] = iz * iz * df * g[2];
-        s_c[tid][3] = ir * kf * g[3];
-        s_c[tid][4] = iz * kf * g[4];
-    } else if (tid < Nq + Nb) {
-        const int a = tid - Nq;
-        const double *fa = f + ((size_t)b * ds.S + sp) * ds.n;
-        double u = 0.0;
-        for (int t = ds.lptr[e * Nb + a]; t < ds.lptr[e * Nb + a + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
-        s_u[a] = u;
+        s_g[tid][0] = ir * ir * w * g[0];
+        s_g[tid][1] = ir * iz * w * g[1];
+        s_g[tid][2] = iz * iz * w * g[2];
+        s_g[tid][3] = ir * w * g[3];
+        s_g[tid][4] = iz * w * g[4];
     }
-    __syncthreads();
-    const int a = tid / Nb, bb = tid % Nb;
-    double acc = 0.0;
-    for (int q = 0; q < Nq; ++q) {
-        const double e0a = s_E0[q * Nb + a], e1a = s_E1[q * Nb + a];
-        const double e0b = s_E0[q * Nb + bb], e1b = s_E1[q * Nb + bb], bq = s_B[q * Nb + bb];
-        const double t0 = fma(s_c[q][0], e0b, s_c[q][1] * e1b);
-        const double t1 = fma(s_c[q][1], e0b, s_c[q][2] * e1b);
-        const double tk = fma(e0a, s_c[q][3], e1a * s_c[q][4]);
-        acc += fma(e0a, t0, fma(e1a, t1, tk * bq));
-    }
-    const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
-    Ce[mat * Nb * Nb + tid] = acc;
-    s_Ce[tid] = acc;
-    __syncthreads();
-    if (tid < Nb) {
-        double v = 0.0;
-        for (int c = 0; c < Nb; ++c) v = fma(s_Ce[tid * Nb + c], s_u[c], v);
-        ce[mat * Nb + tid] = v;
+    const int a = tid / Nb, bb = tid % Nb;   // phase 1: (q, b) = (a, bb); phase 2: (a, b) = (a, bb)
+    for (int sp = 0; sp < ds.S; ++sp) {
+        __syncthreads();                      // s_g / tabulations ready; previous species done with s_X, s_Y, s_Ce, s_u
+        if (tid < Nb) {
+            const double *fa = f + ((size_t)b * ds.S + sp) * ds.n;
+            double u = 0.0;
+            for (int t = ds.lptr[e * Nb + tid]; t < ds.lptr[e * Nb + tid + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
+            s_u[tid] = u;
+        }
+        {
+            const double kf = ds.kfac[sp], df = ds.dfac[sp];
+            const int q = a;
+            const double e0 = s_E0[q * Nb + bb], e1 = s_E1[q * Nb + bb], bq = s_B[q * Nb + bb];
+            const double drr = df * s_g[q][0], drz = df * s_g[q][1], dzz = df * s_g[q][2];
+            s_X[tid] = fma(drr, e0, fma(drz, e1, kf * s_g[q][3] * bq));
+            s_Y[tid] = fma(drz, e0, fma(dzz, e1, kf * s_g[q][4] * bq));
+        }
+        __syncthreads();
+        double acc = 0.0;
+        for (int q = 0; q < Nq; ++q)
+            acc = fma(s_E0[q * Nb + a], s_X[q * Nb + bb], fma(s_E1[q * Nb + a], s_Y[q * Nb + bb], acc));
+        const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
+        Ce[mat * Nb * Nb + tid] = acc;
+        s_Ce[tid] = acc;
+        __syncthreads();
+        if (tid < Nb) {
+            double v = 0.0;
+            for (int c = 0; c < Nb; ++c) v = fma(s_Ce[tid * Nb + c], s_u[c], v);
+            ce[mat * Nb + tid] = v;
+        }
     }
 }
 
@@ -456,7 +464,7 @@ int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, c
 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    cudaStream_t st) {
-    dim3 grid(ds.Ne, ds.S, nb);
+    dim3 grid(ds.Ne, nb);
     k_element<<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce);
     return 1;
 }
