@@ -72,70 +72,133 @@ __device__ __forceinline__ double scale_pow2(double x, int e) {
 //     W = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(2 A_1^2) + (sum_{k>=2} C_k^2 / 2^k)/q^2   (c_1 = q/(4 a_1))
 //     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2),  Kt = K/sqrt(s)
 // every sum has positive terms except the bracket of P0 (= 2 s E/K: bounded cancellation ~ K/E).
-// The iteration stops for the whole warp once every lane's next c would be < 2^-27 a (the then
-// neglected term is < 6e-17 a).  The test compares exponents with integer ops, one pass ahead.
+// Evaluated with rho2 = 2 r rb = q/2, 2W and 4Kt so that no multiplication by a power of two remains:
+//     g = 1 + q W = 1 + rho2 (2W),  Pss/2 = (4Kt)(2W),  Pc = (4Kt/s) g,  P0 = (4Kt/s)(s - rho2 g)/d2
+//     (s - rho2 g = (s + d2 - q^2 W)/2 because s - d2 = q).
+// The iteration stops for the whole warp once every lane's next c would be <= 2^-26 a (the a used
+// for K is then within 2^-54 a of the limit).  The test compares exponents with integer ops, one
+// pass ahead.
+//
+// FP64 issue cost on sm_100a (measured): 2 cycles per warp instruction and SM
+// sub-partition, 3 cycles for a DFMA with three distinct register operands; 9 cycles dependent
+// latency.  Hence the lock-step evaluation of several pairs per thread and the care for operand count.
 // ------------------------------------------------------------------------------------------------
 struct PairAcc { double drr, drz, dzz, kr, kz; };
-struct __align__(16) JPoint { double r, z, invr, tD, tKr, tKz; };
 
 constexpr int AGM_MAX_STEPS = 8;
+constexpr int AGM_EXIT_SHIFT = 11;   // exit vote: C_{k+1} <= 2^-11 A_k (see pair_parts)
 
-// P0, Pc, Pss of one pair (header above) plus the geometry the tensor entries need.
-struct PairParts { double P0, Pc, Pss, dz, dr, dz2, dr2, rho; };
+// What a thread keeps of one of its i points.
+struct IPoint {
+    double r, z;
+    double r2x;     // 2 r
+    double rr2;     // 2 r^2
+    double c;       // 1/(16 r^2): 1/q^2 = c_i / r_j^2
+    double tD, tKr, tKz;
+};
+// One j point, read from shared memory (SoA there, see k_pair_sym).
+struct JPoint { double r, z, invr2, rr2, tD, tKr, tKz; };
 
-template <bool CHECK_SELF>
-__device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4, double inv4ri, const JPoint &pj) {
-    PairParts pp;
-    const double rj = pj.r;
-    const double sr = ri + rj;
-    pp.dz = zi - pj.z; pp.dr = ri - rj;
-    pp.dz2 = pp.dz * pp.dz; pp.dr2 = pp.dr * pp.dr;
-    double d2 = pp.dr2 + pp.dz2;
-    const double s = fma(sr, sr, pp.dz2);
-    bool self = false;
-    if (CHECK_SELF) {                 // coincident pair (j == i): contributes nothing (reading Q3)
-        self = !(d2 > 0.0);
-        if (self) d2 = 1.0;
+// P0, Pc and Pss/2 of a pair plus the geometry the tensor entries need (rho2 = 2 r_i r_j).
+struct PairParts { double P0, Pc, Pssh, dz, dr, dr2, rho2; };
+
+// NP pairs (i_u, j), u < NP, evaluated in lock-step: NP independent dependency chains per thread
+// through the AGM, one exit vote for all of them.
+template <int NP, bool CHECK_SELF>
+__device__ __forceinline__ void pair_parts(const IPoint (&pi)[NP], const JPoint &pj, PairParts (&pp)[NP]) {
+    double s[NP], ys[NP], yd[NP], iA1[NP], A[NP], B[NP], V[NP];
+    bool self[NP];
+#pragma unroll
+    for (int u = 0; u < NP; ++u) {
+        pp[u].dz = pi[u].z - pj.z; pp[u].dr = pi[u].r - pj.r;
+        const double dz2 = pp[u].dz * pp[u].dz;
+        pp[u].dr2 = pp[u].dr * pp[u].dr;
+        double d2 = pp[u].dr2 + dz2;
+        pp[u].rho2 = pi[u].r2x * pj.r;
+        self[u] = false;
+        if (CHECK_SELF) {             // coincident pair (j == i): contributes nothing (reading Q3)
+            self[u] = !(d2 > 0.0);
+            if (self[u]) d2 = 1.0;
+        }
+        s[u] = fma(2.0, pp[u].rho2, d2);                 // (r_i + r_j)^2 + dz^2 = d2 + 4 r_i r_j
+        double a0, b0;
+        sqrt_rsqrt_fast(s[u], a0, ys[u]);
+        sqrt_rsqrt_fast(d2, b0, yd[u]);
+        A[u] = a0 + b0;                                  // A_1 = 2 a_1
+        B[u] = sqrt_times2_fast(a0 * b0);
+        iA1[u] = rcp_fast(A[u]);
+        V[u] = 0.0;
     }
-    double a0, b0, ys, yd;
-    sqrt_rsqrt_fast(s, a0, ys);
-    sqrt_rsqrt_fast(d2, b0, yd);
-    double A = a0 + b0;               // A_1 = 2 a_1
-    double B = sqrt_times2_fast(a0 * b0);
-    const double iA1 = rcp_fast(A);
     // Rolled loop, state in fixed registers.  V_P = 2 V_{P-1} + C_{P+1}^2, so after P passes
-    // sum_{k>=2} C_k^2/2^k = V / 2^{P+1}, and 2 K/sqrt(s) = 2 pi 2^P / A_{P+1}.
+    // sum_{k>=2} C_k^2/2^k = V / 2^{P+1}, and 4 K/sqrt(s) = 4 pi 2^P / A_{P+1}.
     // The exit is decided ONE PASS AHEAD so that the branch never waits on fresh data:
-    // c_{k+2} = c_{k+1}^2/(4 a_{k+2}) exactly, hence C_{k+1} <= 2^-12 A_k in every lane guarantees
-    // c_{k+2} < 2^-27 a after the next pass, which is then the last (its C only feeds V).
-    double V = 0.0;
+    // c_{k+2} = c_{k+1}^2/(4 a_{k+2}) exactly, hence C_{k+1} <= 2^-11 A_k (c_{k+1} <= 2^-12 a) in every
+    // lane guarantees c_{k+2} <= 2^-26 a after the next pass, which is then the last (its C only feeds
+    // V); the a_{k+2} used for K is then within c_{k+3} <= 2^-54 a of the AGM limit.
     int P = 0;
     bool last = false;
 #pragma unroll 1
     for (;;) {
-        const double C = A - B;
-        V = fma(V, 2.0, C * C);
+        bool conv = true;
+#pragma unroll
+        for (int u = 0; u < NP; ++u) {
+            const double C = A[u] - B[u];
+            V[u] = fma(V[u], 2.0, C * C);
+            conv = conv && (__double2hiint(C) + (AGM_EXIT_SHIFT << 20) <= __double2hiint(A[u]));
+        }
         ++P;
         if (last || P == AGM_MAX_STEPS) break;
-        last = __all_sync(0xffffffffu, __double2hiint(C) + (13 << 20) <= __double2hiint(A));
-        const double X = A * B;
-        A = A + B;
-        B = sqrt_times2_fast(X);
+        last = __all_sync(0xffffffffu, conv);
+#pragma unroll
+        for (int u = 0; u < NP; ++u) {
+            const double X = A[u] * B[u];
+            A[u] = A[u] + B[u];
+            B[u] = sqrt_times2_fast(X);
+        }
     }
-    A = A + B;
-    const double KP2 = scale_pow2(6.283185307179586476925286766559 * rcp_fast(A), P);   // 2 K/sqrt(s)
-    const double q = ri4 * rj;
-    pp.rho = ri * rj;
-    const double invq = inv4ri * pj.invr;
-    // 1/q^2 is a normal number far from the exponent limits (V may be 0 for far pairs: scale 1/q^2, not the product)
-    const double W = fma(0.5 * iA1, iA1, V * scale_pow2(invq * invq, -(P + 1)));
-    const double Ks = KP2 * (ys * ys);
-    const double x = q * W;
-    pp.Pc = Ks * fma(2.0, x, 2.0);
-    pp.P0 = Ks * (yd * yd) * fma(-q, x, s + d2);
-    pp.Pss = 8.0 * (KP2 * W);
-    if (CHECK_SELF && self) { pp.Pss = 0.0; pp.Pc = 0.0; pp.P0 = 0.0; }
-    return pp;
+#pragma unroll
+    for (int u = 0; u < NP; ++u) {
+        const double Af = A[u] + B[u];
+        const double K4 = scale_pow2(12.566370614359172953850573533118 * rcp_fast(Af), P);   // 4 K/sqrt(s)
+        // 2 W = 1/A_1^2 + V 2^-P / q^2.  1/q^2 is a normal number far from the exponent limits (V may be
+        // 0 for far pairs: scale 1/q^2, not the product).
+        const double invq2 = pi[u].c * pj.invr2;
+        const double W2 = fma(iA1[u], iA1[u], V[u] * scale_pow2(invq2, -P));
+        const double g = fma(pp[u].rho2, W2, 1.0);       // 1 + q W
+        const double Kh = K4 * (ys[u] * ys[u]);          // 4 K / s^(3/2)
+        pp[u].Pssh = K4 * W2;
+        pp[u].Pc = Kh * g;
+        pp[u].P0 = (Kh * (yd[u] * yd[u])) * fma(-pp[u].rho2, g, s[u]);   // (s + d2 - q^2 W)/2 = s - rho2 (1 + q W)
+        if (CHECK_SELF && self[u]) { pp[u].Pssh = 0.0; pp[u].Pc = 0.0; pp[u].P0 = 0.0; }
+    }
+}
+
+// The five distinct tensor entries of a pair (Q1) from its parts:
+//   UDrr = U^D_rr(i,j), UDrrT = U^D_rr(j,i), A2 = -U^D_rz(i,j) = -U^K_zr(j,i), A3 = U^D_zz = U^K_zz (both ways),
+//   A4 = U^K_rr (both ways), A5 = U^K_zr(i,j) = U^D_rz(j,i)
+struct PairTensor { double UDrr, UDrrT, A2, A3, A4, A5; };
+
+__device__ __forceinline__ PairTensor pair_tensor(const IPoint &pi, const JPoint &pj, const PairParts &pp) {
+    PairTensor t;
+    const double dzP0 = pp.dz * pp.P0;
+    const double A1 = pp.dz * dzP0;                      // dz^2 P0
+    const double b = pp.dr * dzP0;                       // dz dr P0
+    const double e = pp.dz * pp.Pc;
+    t.A2 = fma(pj.r, e, b);                              // dz (dr P0 + r_j Pc)
+    t.A5 = fma(pi.r, e, -b);                             // dz (-dr P0 + r_i Pc)
+    t.A3 = fma(pp.dr2, pp.P0, pp.rho2 * pp.Pc);          // dr^2 P0 + 2 r_i r_j Pc
+    t.A4 = fma(pp.rho2, pp.Pssh, fma(-pp.dz, e, A1));    // dz^2 (P0 - Pc) + r_i r_j Pss
+    t.UDrr = fma(pj.rr2, pp.Pssh, A1);                   // r_j^2 Pss + dz^2 P0
+    t.UDrrT = fma(pi.rr2, pp.Pssh, A1);
+    return t;
+}
+
+__device__ __forceinline__ void accumulate_i(PairAcc &acc, const JPoint &pj, const PairTensor &t) {
+    acc.drr = fma(pj.tD, t.UDrr, acc.drr);
+    acc.drz = fma(-pj.tD, t.A2, acc.drz);
+    acc.dzz = fma(pj.tD, t.A3, acc.dzz);
+    acc.kr = fma(t.A4, pj.tKr, fma(-t.A2, pj.tKz, acc.kr));
+    acc.kz = fma(t.A5, pj.tKr, fma(t.A3, pj.tKz, acc.kz));
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -145,30 +208,29 @@ __device__ __forceinline__ PairParts pair_parts(double ri, double zi, double ri4
 // so one elliptic evaluation serves the ordered pairs (i,j) and (j,i) (the paper notes the
 // symmetry, L193, and does not exploit it).
 //
-// Points are cut into tiles of TS; block (I <= J, problem b), TS threads, thread t owns
-// i = I*TS + t and walks the j of tile J held in shared memory.  It keeps the i-side sums in
-// registers; the j-side sums rotate around the warp's lanes together with their j (see below) and
-// are parked in shared memory per warp, then added over the warps in warp order.  Diagonal blocks (I == J) do
-// all ordered pairs of the tile with the coincident-pair test.
+// Points are cut into tiles of TS; block (I <= J, problem b), TS/IPT threads, thread t owns the IPT
+// points i_u = I*TS + u*TS/IPT + t and walks the j of tile J held in shared memory, evaluating its
+// IPT pairs (i_u, j) in lock-step.  It keeps the i-side sums in registers; the j-side sums rotate
+// around the warp's lanes together with their j (see below) and are parked in shared memory per
+// warp, then added over the warps in warp order.  Diagonal blocks (I == J) do all ordered pairs of
+// the tile with the coincident-pair test.
 //
 // Deterministic order: Gpart[b][src tile][5][N] holds, for every target
 // point, the partial sum over the points of one source tile; each slot is written by exactly one
-// block, and k_element / k_sum_partials add the slabs in tile order.  TS depends on N only, so a
+// block, and k_sum_partials adds the slabs in tile order.  TS and IPT depend on N only, so a
 // batched build is bitwise equal to single builds.
 // ------------------------------------------------------------------------------------------------
-#ifndef PAIR_K_UNROLL
-#define PAIR_K_UNROLL 2   // j steps per loop trip (sweep 1/2: 247/253 GPair/s)
-#endif
-constexpr int kPairUnroll = PAIR_K_UNROLL;
 #ifndef PAIR_MIN_BLOCKS
-#define PAIR_MIN_BLOCKS 5   // resident blocks per SM the register budget is capped for (sweep 4/5/6: 239/247/246 GPair/s)
+#define PAIR_MIN_BLOCKS 1
 #endif
-template <int TS>
-__global__ void __launch_bounds__(TS, PAIR_MIN_BLOCKS)
+template <int TS, int IPT>
+__global__ void __launch_bounds__(TS / IPT, PAIR_MIN_BLOCKS)
 k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
            const double *__restrict__ T, double *__restrict__ Gpart) {
-    constexpr int NW = TS / 32;
-    __shared__ JPoint sj[2 * TS];        // every 32-point sub-tile is stored twice in a row: rotated walks need no wrap
+    constexpr int NT = TS / IPT;         // threads
+    constexpr int NW = NT / 32;          // warps
+    static_assert(NT % 32 == 0 && NW >= 1, "whole warps");
+    __shared__ double sj[7][TS];         // r, z, 1/r^2, 2 r^2, tD, tKr, tKz of the j tile (SoA: conflict-free LDS.64)
     __shared__ double sacc[NW][5][TS];
     const int b = blockIdx.y;
     // linear tile-pair index p = J (J+1)/2 + I, I <= J
@@ -179,43 +241,42 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
     const int I = p - J * (J + 1) / 2;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const double *Tb = T + (size_t)b * 3 * N;
-    const int i = I * TS + tid;
-    const bool valid = i < N;
-    const int ic = valid ? i : N - 1;
-    const double ri = r[ic], zi = z[ic];
-    const double ri4 = 4.0 * ri, inv4ri = 0.25 * invr[ic], ri2 = ri * ri;
-    const double tDi = valid ? Tb[ic] : 0.0, tKri = valid ? Tb[N + ic] : 0.0, tKzi = valid ? Tb[2 * N + ic] : 0.0;
+    IPoint pi[IPT];
+    bool valid[IPT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        const int i = I * TS + u * NT + tid;
+        valid[u] = i < N;
+        const int ic = valid[u] ? i : N - 1;
+        const double ri = r[ic], iri = invr[ic];
+        pi[u].r = ri; pi[u].z = z[ic]; pi[u].r2x = 2.0 * ri; pi[u].rr2 = 2.0 * ri * ri; pi[u].c = 0.0625 * iri * iri;
+        pi[u].tD = valid[u] ? Tb[ic] : 0.0; pi[u].tKr = valid[u] ? Tb[N + ic] : 0.0; pi[u].tKz = valid[u] ? Tb[2 * N + ic] : 0.0;
+    }
     const int jbase = J * TS;
     const int cnt = min(TS, N - jbase);
-    {
-        JPoint pj;
-        if (tid < cnt) {
-            const int j = jbase + tid;
-            pj.r = r[j]; pj.z = z[j]; pj.invr = invr[j];
-            pj.tD = Tb[j]; pj.tKr = Tb[N + j]; pj.tKz = Tb[2 * N + j];
+    for (int t = tid; t < TS; t += NT) {
+        if (t < cnt) {
+            const int j = jbase + t;
+            const double rj = r[j], irj = invr[j];
+            sj[0][t] = rj; sj[1][t] = z[j]; sj[2][t] = irj * irj; sj[3][t] = 2.0 * rj * rj;
+            sj[4][t] = Tb[j]; sj[5][t] = Tb[N + j]; sj[6][t] = Tb[2 * N + j];
         } else {
             // padding of a ragged tile: a far-away point with zero weight (finite tensor, no effect)
-            pj.r = 1.0; pj.z = 1.0e6; pj.invr = 1.0; pj.tD = 0.0; pj.tKr = 0.0; pj.tKz = 0.0;
+            sj[0][t] = 1.0; sj[1][t] = 1.0e6; sj[2][t] = 1.0; sj[3][t] = 2.0;
+            sj[4][t] = 0.0; sj[5][t] = 0.0; sj[6][t] = 0.0;
         }
-        sj[warp * 64 + lane] = pj;
-        sj[warp * 64 + 32 + lane] = pj;
     }
     __syncthreads();
-    PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
+    PairAcc acc[IPT];
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) acc[u] = {0.0, 0.0, 0.0, 0.0, 0.0};
     if (I == J) {
         for (int t = 0; t < cnt; ++t) {
-            const JPoint pj = sj[(t >> 5) * 64 + (t & 31)];
-            const PairParts pp = pair_parts<true>(ri, zi, ri4, inv4ri, pj);
-            const double UDrr = fma(pj.r * pj.r, pp.Pss, pp.dz2 * pp.P0);
-            const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
-            const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
-            const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
-            const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);
-            acc.drr = fma(pj.tD, UDrr, acc.drr);
-            acc.drz = fma(-pj.tD, nUDrz, acc.drz);
-            acc.dzz = fma(pj.tD, UDzz, acc.dzz);
-            acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
-            acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
+            const JPoint pj = {sj[0][t], sj[1][t], sj[2][t], sj[3][t], sj[4][t], sj[5][t], sj[6][t]};
+            PairParts pp[IPT];
+            pair_parts<IPT, true>(pi, pj, pp);
+#pragma unroll
+            for (int u = 0; u < IPT; ++u) accumulate_i(acc[u], pj, pair_tensor(pi[u], pj, pp[u]));
         }
     } else {
         // Lane t walks the 32 j of a sub-tile in rotated order, j = (t + k) mod 32, so that the warp
@@ -225,33 +286,24 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
         const int src = (lane + 1) & 31;
         for (int sub = 0; sub < nsub; ++sub) {
             double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
-            // explicit 32-bit shared address, advanced by one JPoint per step (three 16-byte loads)
-            unsigned sa = (unsigned)__cvta_generic_to_shared(sj + sub * 64 + lane);
-#pragma unroll kPairUnroll
-            for (int k = 0; k < 32; ++k, sa += (unsigned)sizeof(JPoint)) {
-                JPoint pj;
-                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2];" : "=d"(pj.r), "=d"(pj.z) : "r"(sa));
-                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+16];" : "=d"(pj.invr), "=d"(pj.tD) : "r"(sa));
-                asm volatile("ld.shared.v2.f64 {%0, %1}, [%2+32];" : "=d"(pj.tKr), "=d"(pj.tKz) : "r"(sa));
-                const PairParts pp = pair_parts<false>(ri, zi, ri4, inv4ri, pj);
-                const double dzP0 = pp.dz2 * pp.P0;
-                const double UDrr = fma(pj.r * pj.r, pp.Pss, dzP0);
-                const double UDrrT = fma(ri2, pp.Pss, dzP0);                          // U^D_rr(j,i)
-                const double nUDrz = pp.dz * fma(pp.dr, pp.P0, pj.r * pp.Pc);         // -U^D_rz(i,j)
-                const double UDzz = fma(2.0, pp.rho * pp.Pc, pp.dr2 * pp.P0);
-                const double UKrr = fma(pp.dz2, pp.P0 - pp.Pc, pp.rho * pp.Pss);
-                const double UKzr = pp.dz * fma(-pp.dr, pp.P0, ri * pp.Pc);           // = U^D_rz(j,i)
-                acc.drr = fma(pj.tD, UDrr, acc.drr);
-                acc.drz = fma(-pj.tD, nUDrz, acc.drz);
-                acc.dzz = fma(pj.tD, UDzz, acc.dzz);
-                acc.kr = fma(UKrr, pj.tKr, fma(-nUDrz, pj.tKz, acc.kr));
-                acc.kz = fma(UKzr, pj.tKr, fma(UDzz, pj.tKz, acc.kz));
-                // terms of target j from source i, then pass the sums on with their j
-                v0 = fma(tDi, UDrrT, v0);
-                v1 = fma(tDi, UKzr, v1);
-                v2 = fma(tDi, UDzz, v2);
-                v3 = fma(UKrr, tKri, fma(UKzr, tKzi, v3));
-                v4 = fma(-nUDrz, tKri, fma(UDzz, tKzi, v4));
+#pragma unroll 1
+            for (int k = 0; k < 32; ++k) {
+                const int t = sub * 32 + ((lane + k) & 31);
+                const JPoint pj = {sj[0][t], sj[1][t], sj[2][t], sj[3][t], sj[4][t], sj[5][t], sj[6][t]};
+                PairParts pp[IPT];
+                pair_parts<IPT, false>(pi, pj, pp);
+#pragma unroll
+                for (int u = 0; u < IPT; ++u) {
+                    const PairTensor tt = pair_tensor(pi[u], pj, pp[u]);
+                    accumulate_i(acc[u], pj, tt);
+                    // terms of target j from source i_u
+                    v0 = fma(pi[u].tD, tt.UDrrT, v0);
+                    v1 = fma(pi[u].tD, tt.A5, v1);
+                    v2 = fma(pi[u].tD, tt.A3, v2);
+                    v3 = fma(tt.A4, pi[u].tKr, fma(tt.A5, pi[u].tKz, v3));
+                    v4 = fma(-tt.A2, pi[u].tKr, fma(tt.A3, pi[u].tKz, v4));
+                }
+                // pass the sums on with their j
                 v0 = __shfl_sync(0xffffffffu, v0, src);
                 v1 = __shfl_sync(0xffffffffu, v1, src);
                 v2 = __shfl_sync(0xffffffffu, v2, src);
@@ -263,19 +315,23 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
             sacc[warp][3][jl] = v3; sacc[warp][4][jl] = v4;
         }
     }
-    if (valid) {
-        double *G = Gpart + ((size_t)b * ntiles + J) * 5 * N;
-        G[i] = acc.drr; G[N + i] = acc.drz; G[2 * N + i] = acc.dzz; G[3 * N + i] = acc.kr; G[4 * N + i] = acc.kz;
+#pragma unroll
+    for (int u = 0; u < IPT; ++u) {
+        if (valid[u]) {
+            const int i = I * TS + u * NT + tid;
+            double *G = Gpart + ((size_t)b * ntiles + J) * 5 * N;
+            G[i] = acc[u].drr; G[N + i] = acc[u].drz; G[2 * N + i] = acc[u].dzz; G[3 * N + i] = acc[u].kr; G[4 * N + i] = acc[u].kz;
+        }
     }
     if (I != J) {
         __syncthreads();
-        if (tid < cnt) {
-            double *G = Gpart + ((size_t)b * ntiles + I) * 5 * N + jbase + tid;
+        for (int t = tid; t < cnt; t += NT) {
+            double *G = Gpart + ((size_t)b * ntiles + I) * 5 * N + jbase + t;
 #pragma unroll
             for (int c = 0; c < 5; ++c) {
-                double sum = sacc[0][c][tid];
+                double sum = sacc[0][c][t];
 #pragma unroll
-                for (int w = 1; w < NW; ++w) sum += sacc[w][c][tid];
+                for (int w = 1; w < NW; ++w) sum += sacc[w][c][t];
                 G[(size_t)c * N] = sum;
             }
         }
@@ -456,9 +512,9 @@ int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T
 int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st) {
     const int ts = pair_tile_size(ds.N), nt = pair_tiles(ds.N);
     dim3 grid(nt * (nt + 1) / 2, nb);
-    if (ts == 128) k_pair_sym<128><<<grid, 128, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
-    else if (ts == 64) k_pair_sym<64><<<grid, 64, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
-    else k_pair_sym<32><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    if (ts == 128) k_pair_sym<128, 2><<<grid, 64, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    else if (ts == 64) k_pair_sym<64, 2><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    else k_pair_sym<32, 1><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
     return 1;
 }
 
