@@ -33,10 +33,17 @@ METRIC = "landau_jacobian_gpair_evals_per_s"
 UNIT = "GPair/s"
 WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
 # FP64 flop (2 DFMA + DMUL + DADD) and FP64-pipe instructions the pair kernel executes per ORDERED
-# pair on this workload, ncu-counted (profiles/r01_pair_kernel.md).
-FLOP_PER_PAIR = 82.8
-FP64_INST_PER_PAIR = 56.65
+# pair on this workload, ncu-counted (profiles/r01c_pair_kernel.md).
+FLOP_PER_PAIR = 77.33
+FP64_INST_PER_PAIR = 50.05
+# of which DFMAs with three distinct register operands: they issue in 3 cycles instead of 2
+# (measured), so the issue-cycle cost per ordered pair is 2 x 50.05 + 11.08 SMSP-cycles x 32 lanes.
+FP64_3OP_INST_PER_PAIR = 11.08
 FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
+# dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_sym launch on this workload, from the
+# ncu --set full capture summarised in profiles/r01c_pair_kernel.md (73.9 MB read + 3.880 GB written:
+# the per-source-tile partial slabs; the algorithmic minimum is 24 B/point in + 40 B/point out = 0.16 GB).
+PAIR_KERNEL_DRAM_BYTES = 73.9e6 + 3.8797e9
 
 
 class ClockSampler(threading.Thread):
@@ -82,16 +89,20 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(pw) if pw else None, "reasons": reasons, "samples": len(rows)}
 
 
+CPU_SAMPLE_PROBLEMS = 8      # of the 512: ~0.5 s each on 16 cores, i.e. tens of core-seconds in total
+
+
 def cpu_baseline_sample(wl, inputs):
-    """The oracle as it stands (double instantiation), one problem of the workload."""
+    """The oracle as it stands (double instantiation) on a bounded sample of the workload."""
     from oracle import landau_oracle as oracle
     oracle.build()
     sp = oracle.build_space(wl.mesh, wl.order)
-    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z, 0)
+    fs = [inputs.nodal_f(wl, sp.dof_r, sp.dof_z, b) for b in range(CPU_SAMPLE_PROBLEMS)]
     t0 = time.perf_counter()
-    oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
+    for f in fs:
+        oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
     dt = time.perf_counter() - t0
-    pairs = sp.N * (sp.N - 1)
+    pairs = CPU_SAMPLE_PROBLEMS * sp.N * (sp.N - 1)
     return pairs / dt * 1e-9, dt, os.cpu_count()
 
 
@@ -245,12 +256,14 @@ def run_ours(args):
         nominal_peak = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
         pair_launch_ms = pair_ms / max(pair_cnt, 1)
         achieved = FLOP_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) * 1e-12
-        roof = {"bound": "alu", "kernel": "k_pair_sym<128>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
-                "frac": achieved / nominal_peak, "traffic": None,
+        roof = {"bound": "alu", "kernel": "k_pair_sym<128,2>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
+                "frac": achieved / nominal_peak, "traffic": PAIR_KERNEL_DRAM_BYTES,
                 "peak_source": "derived: SMs x 64 DFMA lanes x 2 x clocks.max.sm (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
                 "peak_probe_measured": peak_flops * 1e-12, "frac_of_probe": achieved / (peak_flops * 1e-12),
                 "flop_per_pair": FLOP_PER_PAIR,
                 "fp64_pipe_frac": FP64_INST_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) / (nominal_peak * 0.5e12),
+                "fp64_issue_bound_frac": (FP64_INST_PER_PAIR + 0.5 * FP64_3OP_INST_PER_PAIR) * pairs_per_step
+                / (pair_launch_ms * 1e-3) / (nominal_peak * 0.5e12),
                 "kernel_ms_per_launch": pair_launch_ms,
                 "kernel_share_of_step": pair_ms / total_ms if world == 1 else None,
                 "kernel_gpair_per_s": pairs_per_step / (pair_launch_ms * 1e-3) * 1e-9}
@@ -272,7 +285,7 @@ def run_ours(args):
                     "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps, "api": "landau_jacobian_host (pinned host buffers)"},
             "roofline": roof,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"1 of the 512 problems (N=4928, a1-a8), double-precision oracle, {cpu_dt:.2f} s"},
+                             "sample": f"{CPU_SAMPLE_PROBLEMS} of the 512 problems (N=4928, a1-a8), double-precision oracle, OpenMP over i, {cpu_dt:.2f} s wall"},
             "per_config": detail,
         }))
     ctx.destroy()
