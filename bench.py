@@ -270,6 +270,7 @@ def run_ours(args):
         cpu_val, cpu_dt, cores = cpu_baseline_sample(wl, inputs)
         detail = [time_single_config(binding, inputs, torch, k) for k in (1, 2, 3, 4)]
         detail.append(time_single_config(binding, inputs, torch, 3, variant="A"))
+        detail += [time_single_config(binding, inputs, torch, k) for k in (6, 7)]   # paper-shaped S = 10 context runs
         h2d = nb * ctx.S * ctx.n * 8
         d2h = nb * ctx.S * (ctx.nnz + ctx.n) * 8
         print(json.dumps({

@@ -149,6 +149,17 @@ def mesh_quadtree(rmin, rmax, zmin, zmax, nbr, nbz, R_in, L_in, R_out, L_out) ->
     return Mesh(rmin, rmax, zmin, zmax, nbr, nbz, lev, ir, iz)
 
 
+def mesh_refine_uniform(m: Mesh) -> Mesh:
+    """Every leaf split into its four children (children in (iz,ir) order, parents in place)."""
+    lev, ir, iz = [], [], []
+    for l, i, j in zip(m.level, m.ir, m.iz):
+        for cj in (0, 1):
+            for ci in (0, 1):
+                lev.append(l + 1); ir.append(2 * i + ci); iz.append(2 * j + cj)
+    return Mesh(m.rmin, m.rmax, m.zmin, m.zmax, m.nbr, m.nbz, np.array(lev, np.int32), np.array(ir, np.int32),
+                np.array(iz, np.int32))
+
+
 @dataclass
 class Species:
     """The ``landau_species`` struct: masses in m_e, charges in e, nu = 1, m0 = m_e (Appendix A)."""
@@ -226,7 +237,8 @@ def mesh_config3(variant: str = "B") -> Mesh:
 
 
 def config(k: int, nbatch: int | None = None, variant: str = "B") -> Workload:
-    """The five BASELINE.json configs (k = 1..5) plus k = 0, a tiny refined Q2 case for tests."""
+    """The five BASELINE.json configs (k = 1..5), k = 0, a tiny refined Q2 case for tests, and
+    k = 6, 7, the paper-shaped ten-species context runs."""
     seed = SEED0 + 1000 * k
     if k == 0:
         mesh = mesh_quadtree(0.0, 4.0, -4.0, 4.0, 2, 4, 1.0, 2, 2.0, 1)
@@ -272,4 +284,17 @@ def config(k: int, nbatch: int | None = None, variant: str = "B") -> Workload:
             zs = rng.uniform(0.0, 1.0)
             comps.append([Component(0, 1.0 - tail, Tb), Component(0, tail, 1.0, zs), Component(1, 1.0, Tb)])
         return Workload(f"cfg5{variant}-batch{nb}-eD-q3-quench", 3, mesh, sp, comps, 0.0, seed)
+    if k in (6, 7):
+        # Paper-shaped context runs: ten species -- e, D+ and
+        # eight effective ionisation states of a heavy ion (m = 184 x 1836), all at the same temperature --
+        # on an 80-cell Q3 mesh (k = 6) and its uniform refinement to 320 cells (k = 7).
+        mesh = mesh_quadtree(0.0, 5.0, -5.0, 5.0, 4, 8, 1.0, 2, 2.5, 1)
+        if k == 7:
+            mesh = mesh_refine_uniform(mesh)
+        mw = 184.0 * 1836.0
+        rows = [(1.0, -1.0, 1.0, 1.0), (3670.0, 1.0, 0.64, 1.0)] + [(mw, float(q), 0.01, 1.0) for q in range(1, 9)]
+        sp = _sp(rows)   # sum q n over ions = 0.64 + 0.01 * 36 = 1 = n_e
+        nb = 1 if nbatch is None else nbatch
+        comps = [[Component(s, rows[s][2], 1.0) for s in range(10)] for _ in range(nb)]
+        return Workload(f"ctx{mesh.ncells}-10sp-q3", 3, mesh, sp, comps, 1e-3, seed)
     raise ValueError(f"unknown config {k}")

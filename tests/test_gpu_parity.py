@@ -94,6 +94,15 @@ def test_refined_configs_full_parity(gpu, oracle, cfg, variant):
     print(f"{wl.name}: worst block error {worst:.2e}")
 
 
+@pytest.mark.parametrize("cfg", [6, 7])
+def test_paper_shaped_ten_species_context_parity(gpu, oracle, cfg):
+    """e + D + 8 heavy-ion charge states on the 80- and 320-cell Q3 meshes."""
+    wl = inputs.config(cfg)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    print(f"{wl.name}: worst block error {worst:.2e}")
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch

@@ -29,7 +29,7 @@ def test_exports_every_declared_symbol(binding):
         assert hasattr(L, name)
 
 
-@pytest.mark.parametrize("cfg", [0, 1, 2, 3, "3A"])
+@pytest.mark.parametrize("cfg", [0, 1, 2, 3, "3A", 6, 7])
 def test_setup_matches_oracle_numbering_and_pattern(binding, oracle, cfg):
     if cfg == "3A":
         wl = inputs.config(3, variant="A")
