@@ -13,7 +13,9 @@ What it computes (PAPER.md = /root/reference/PAPER.md, arxiv 2104.10000):
   (Transform&Assemble, line 23), assembly with hanging-node interpolation (L101, L297);
 * C(f), the weak-form residual (right-hand side of Eq. 4 without E-field and source),
   evaluated DIRECTLY from Eqs. 5-6 at f -- not as J f, so that J f = C(f) is a test;
-* the scaled mass matrix (L280).
+* the scaled mass matrix (L280);
+* the E-field advection term on the left of Eq. 4 (L52) and the operator of a fully implicit step,
+  shift M + A_a - J_a with its residual A_a f_a - C_a(f).
 
 Everything outside the O(N^2) pair loop is plain numpy in fp64 with dense matrices (no
 blocking, no gather lists).  The pair loop is plain C in long double (``_ld``) for parity and
@@ -26,7 +28,8 @@ statement, not code): cell/point/DOF/CSR orderings described in ``Space``.
 Parity pins: tests/test_oracle_pins.py (elliptic closed forms, Legendre relation, brute-force
 azimuthal quadrature of Eq. 3, Rosenbluth potentials of a Maxwellian, exact discrete
 conservation, column sums, J f = C(f), mass integrals, constraint polynomial reproduction,
-Table I counting).  Numerical values of individual Jacobian entries are "parity unpinned" by
+Table I counting; for the advection term: zero row sums, exact integral of d(z)/dz, integration by
+parts against z for a distribution that vanishes on the boundary, vals f = shift M f + F).  Numerical values of individual Jacobian entries are "parity unpinned" by
 the paper (it prints none); they are pinned only through those invariants.
 """
 from __future__ import annotations
@@ -426,6 +429,46 @@ def mass(sp: Space, shift: float) -> np.ndarray:
         P = sp.cell_P[e]
         M[np.ix_(sp.cell_dofs[e], sp.cell_dofs[e])] += P.T @ Me @ P
     return csr_values(sp, M)
+
+
+def advection(sp: Space, species, Ez: float):
+    """E-field term on the left of Eq. 4 (L52): 2 pi int r psi (0, (e_a/m_a) E_z) . grad f, i.e.
+    A_a[i][j] = (e_a m0/m_a) E_z sum_q w_out psi_i d(psi_j)/dz  (charges in e, masses in m0, E in the
+    units of Appendix A: DESIGN.md reading Q14).  Dense blocks [S][n][n]."""
+    S = len(species.mass)
+    A1 = np.zeros((sp.n, sp.n))
+    for e in range(sp.Ne):
+        Ae = np.zeros((sp.Nb, sp.Nb))
+        for q in range(sp.Nq):
+            dpsi_dz = sp.invJ[e, 1] * sp.E[q, :, 1]
+            Ae += sp.w_out[e * sp.Nq + q] * np.outer(sp.B[q], dpsi_dz)
+        P = sp.cell_P[e]
+        A1[np.ix_(sp.cell_dofs[e], sp.cell_dofs[e])] += P.T @ Ae @ P
+    return [float(species.charge[a]) * species.m0 / float(species.mass[a]) * Ez * A1 for a in range(S)]
+
+
+def implicit_operator(sp: Space, species, f: np.ndarray, Ez: float, shift: float, precision: str = "ld"):
+    """What a fully implicit step of Eq. 4 needs about the state f (L75, L280; no source term):
+        vals_a = shift M + A_a - J_a(f)        on the pattern A1, [S][nnz]
+        F_a    = A_a f_a - C_a(f)              [S][n]  (the residual without the d/dt term)
+    F is evaluated from the weak form with physical gradients at the integration points (not as a
+    matrix-vector product), so vals f = shift M f + F is a test of both."""
+    S = f.shape[0]
+    K, D, _ = coefficients(sp, species, f, None, precision)
+    Ce = element_matrices(sp, K, D)
+    A = advection(sp, species, Ez)
+    M1 = mass(sp, shift)
+    vals = np.stack([M1 + csr_values(sp, A[a]) - csr_values(sp, assemble_dense(sp, Ce[a])) for a in range(S)])
+    Cf = collision(sp, species, f, precision, (K, D))
+    _, _, dfz = fields_at_points(sp, f)
+    F = np.zeros((S, sp.n))
+    for a in range(S):
+        fac = float(species.charge[a]) * species.m0 / float(species.mass[a]) * Ez
+        for e in range(sp.Ne):
+            sl = slice(e * sp.Nq, (e + 1) * sp.Nq)
+            fe = sp.B.T @ (sp.w_out[sl] * fac * dfz[a, sl])          # sum_q w psi_i (e/m) E_z df/dz
+            F[a, sp.cell_dofs[e]] += sp.cell_P[e].T @ fe
+    return vals, F - Cf
 
 
 def build_all(mesh, order: int, species, f: np.ndarray, shift: float = 1.0, precision: str = "ld"):

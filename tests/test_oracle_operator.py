@@ -153,3 +153,43 @@ def test_double_and_long_double_instantiations_agree(oracle):
     a = oracle.jacobian(sp, wl.species, f, "ld")
     b = oracle.jacobian(sp, wl.species, f, "d")
     assert np.abs(a - b).max() <= 1e-12 * np.abs(a).max()
+
+
+def test_advection_term_and_implicit_operator_pins(built, oracle):
+    """E-field term of Eq. 4 (L52) and the implicit-step operator shift M + A - J.
+    Pins: d(const)/dz = 0 (row sums); psi = 1 against f = z gives the exact integral
+    (e/m) E_z 2 pi int r dr dz; integration by parts against z for a distribution that vanishes on
+    the z boundaries gives minus the density moment (the force on the species); the residual from
+    the weak form equals the matrix applied to f; the operator is affine in shift and E_z."""
+    wl, sp, f, vals, Cf, mv = built["q3"]
+    spc = wl.species
+    Ez, shift = 0.37, 2.5
+    A = oracle.advection(sp, spc, Ez)
+    S = spc.S
+    R, L = wl.mesh.rmax, wl.mesh.zmax - wl.mesh.zmin
+    M1 = oracle.mass(sp, 1.0)
+    rows = np.repeat(np.arange(sp.n), np.diff(sp.rowptr))
+    Md = np.zeros((sp.n, sp.n)); Md[rows, sp.colidx] = M1
+    for a in range(S):
+        fac = spc.charge[a] * spc.m0 / spc.mass[a] * Ez
+        assert np.abs(A[a].sum(axis=1)).max() <= 1e-12 * np.abs(A[a]).max()            # A 1 = 0
+        assert abs(np.ones(sp.n) @ A[a] @ sp.dof_z - fac * math.pi * R * R * L) <= 1e-11 * abs(fac) * math.pi * R * R * L
+        # z in the FE space: A z = fac * M 1 exactly
+        assert np.abs(A[a] @ sp.dof_z - fac * (Md @ np.ones(sp.n))).max() <= 1e-11 * abs(fac) * np.abs(Md).max() * 10
+    # integration by parts with the electron distribution (e^{-16} at the z boundary, 4 thermal speeds)
+    fe = inputs.maxwellian(1.0, 1.0, 1.0, 0.0, sp.dof_r, sp.dof_z)
+    dens = np.ones(sp.n) @ Md @ fe
+    assert abs(dens - 1.0) < 1e-2                      # int f d^3v = n (coarse Q3 interpolant, cut at 4 v_th)
+    force = sp.dof_z @ A[0] @ fe
+    assert abs(force + spc.charge[0] * Ez * dens) < 1e-5 * abs(Ez)    # exact for f_h up to the boundary term
+    assert abs(np.ones(sp.n) @ A[0] @ fe) < 1e-5 * abs(Ez)                            # no density change
+    # the operator: residual from the weak form == matrix applied to f; affine in (shift, Ez)
+    ov, F = oracle.implicit_operator(sp, spc, f, Ez, shift)
+    for a in range(S):
+        V = np.zeros((sp.n, sp.n)); V[rows, sp.colidx] = ov[a]
+        lhs = V @ f[a]
+        rhs = shift * (Md @ f[a]) + F[a]
+        assert np.abs(lhs - rhs).max() <= 1e-11 * np.abs(lhs).max()
+        assert np.abs(ov[a] - (shift * M1 + A[a][rows, sp.colidx] - vals[a])).max() <= 1e-13 * np.abs(ov[a]).max()
+    ov0, F0 = oracle.implicit_operator(sp, spc, f, 0.0, 0.0)
+    assert np.abs(ov0 + vals).max() <= 1e-13 * np.abs(vals).max() and np.abs(F0 + Cf).max() <= 1e-13 * np.abs(Cf).max()
