@@ -117,6 +117,17 @@ int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double
 /* Step a8: mvals_dev [nnz] = shift * mass matrix on the pattern A1 (same for every species). */
 int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream);
 
+/* Everything a fully implicit step of Eq. 4 ("the mass matrix ... is added to the Jacobian
+ * in all time integrators", L280) needs about the states f, in ONE pass (no source term):
+ *   vals_dev [nb][S][nnz]:  shift * M + A_a(E_z[b]) - J_a(f_b)   on the pattern A1
+ *   F_dev    [nb][S][n]  :  A_a(E_z[b]) f_a - C_a(f_b)           (the residual without the d/dt term)
+ * A_a[i][j] = (e_a m0/m_a) E_z sum_q w psi_i d(psi_j)/dz is the E-field advection term on the left of
+ * Eq. 4 (charges in e, masses in m0, E_z in the units of Appendix A).  Ez_dev: [nb] device
+ * doubles, one field per problem.  vals_dev or F_dev may be NULL.  Same set-up, pair kernel, ordering
+ * and determinism as landau_jacobian_batched. */
+int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez_dev,
+                                     double shift, double *vals_dev, double *F_dev, void *stream);
+
 /* End-to-end variant with HOST buffers (pageable or pinned): copies f to the device, runs
  * landau_jacobian_batched on the ctx's own stream in sub-batches whose device-to-host copies overlap
  * the next sub-batch's build, and synchronises.  Values are bitwise those of the device entry point. */

@@ -47,6 +47,7 @@ SIGNATURES = {
     "landau_jacobian": (c_int, [c_void_p, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_jacobian_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
+    "landau_implicit_operator_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "landau_profile_enable": (c_int, [c_void_p, c_int]),
@@ -205,6 +206,13 @@ class LandauContext:
 
     def mass(self, shift, mvals, stream=None):
         _check(lib().landau_mass(self._h, float(shift), self._ptr(mvals, (self.nnz,)), _stream_ptr(stream)))
+
+    def implicit_operator_batched(self, f, Ez, shift, vals=None, F=None, stream=None):
+        nb = f.shape[0]
+        pv = self._ptr(vals, (nb, self.S, self.nnz)) if vals is not None else None
+        pf = self._ptr(F, (nb, self.S, self.n)) if F is not None else None
+        _check(lib().landau_implicit_operator_batched(self._h, nb, self._ptr(f, (nb, self.S, self.n)), self._ptr(Ez, (nb,)),
+                                                      float(shift), pv, pf, _stream_ptr(stream)))
 
     def jacobian_host(self, f_host, vals_host=None, Cf_host=None):
         """Host buffers: numpy arrays or pinned CPU torch tensors (float64, contiguous)."""

@@ -137,6 +137,7 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
         ds.e2[s] = e2; ds.m0m[s] = mm;
         ds.kfac[s] = species->nu * e2 * mm;
         ds.dfac[s] = -species->nu * e2 * mm * mm;
+        ds.qm[s] = species->charge[s] * mm;
     }
     std::vector<double> invr(hs.N);
     for (int64_t i = 0; i < hs.N; ++i) invr[i] = 1.0 / hs.r[i];
@@ -257,9 +258,24 @@ int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double
     ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
     ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
     ctx->launches += launch_sum_partials(ds, nb, pair_tiles(ds.N), ctx->sc.G, ctx->sc.Gsum, st);
-    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, st);
+    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, nullptr, 0.0, st);
     if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
     if (Cf_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, Cf_dev, st);
+    CK(cudaGetLastError());
+    return LANDAU_OK;
+}
+
+int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez_dev, double shift,
+                                     double *vals_dev, double *F_dev, void *stream) {
+    if (!ctx || !f_dev || !Ez_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    const DeviceSpace &ds = ctx->ds;
+    ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
+    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
+    ctx->launches += launch_sum_partials(ds, nb, pair_tiles(ds.N), ctx->sc.G, ctx->sc.Gsum, st);
+    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, Ez_dev, shift, st);
+    if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
+    if (F_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, F_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }

@@ -396,11 +396,18 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
 //   C_e[a][b] = sum_q ( E0_qa X_qb + E1_qa Y_qb )
 // (the same sum as line 23, factored so that the q loop is two FMAs).  Also writes ce = C_e u
 // (u = P_e f_alpha), the element vector of C(f).  G is the tile-order sum of the pair kernel's slabs.
+// FULL = true builds the operator of a fully implicit step of Eq. 4 (L52, L75, L280) in the same pass:
+//   C_e[a][b] = sum_q w_q [ shift B_qa B_qb + (e_s m0/m_s) E_z B_qa (J^-1 E1)_qb ] - (collision part),
+//   ce = (advection - collision part) u     (the shift term is left to the integrator's residual)
+// through a third factor Z[q][b] (and ZM for the mass part), Ez[b] read per problem.
 // ------------------------------------------------------------------------------------------------
+template <bool FULL>
 __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gpart,
-                          double *__restrict__ Ce, double *__restrict__ ce) {
+                          double *__restrict__ Ce, double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
     __shared__ double s_g[16][5];      // w_out * (invJ-transformed G_D rr, rz, zz, G_K r, z), species-independent
+    __shared__ double s_w[16];         // w_out (FULL only)
     __shared__ double s_B[256], s_E0[256], s_E1[256], s_X[256], s_Y[256], s_Ce[256], s_u[16];
+    __shared__ double s_Z[FULL ? 256 : 1], s_ZM[FULL ? 256 : 1];
     const int e = blockIdx.x, b = blockIdx.y;
     const int Nb = ds.Nb, Nq = ds.Nq, N = ds.N;
     const int tid = threadIdx.x;
@@ -419,7 +426,10 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
         s_g[tid][2] = iz * iz * w * g[2];
         s_g[tid][3] = ir * w * g[3];
         s_g[tid][4] = iz * w * g[4];
+        if (FULL) s_w[tid] = w;
     }
+    const double sgn = FULL ? -1.0 : 1.0;
+    const double ezb = FULL ? Ez[b] : 0.0, izc = ds.invJ[2 * e + 1];
     const int a = tid / Nb, bb = tid % Nb;   // phase 1: (q, b) = (a, bb); phase 2: (a, b) = (a, bb)
     for (int sp = 0; sp < ds.S; ++sp) {
         __syncthreads();                      // s_g / tabulations ready; previous species done with s_X, s_Y, s_Ce, s_u
@@ -430,19 +440,28 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
             s_u[tid] = u;
         }
         {
-            const double kf = ds.kfac[sp], df = ds.dfac[sp];
+            const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
             const int q = a;
             const double e0 = s_E0[q * Nb + bb], e1 = s_E1[q * Nb + bb], bq = s_B[q * Nb + bb];
             const double drr = df * s_g[q][0], drz = df * s_g[q][1], dzz = df * s_g[q][2];
             s_X[tid] = fma(drr, e0, fma(drz, e1, kf * s_g[q][3] * bq));
             s_Y[tid] = fma(drz, e0, fma(dzz, e1, kf * s_g[q][4] * bq));
+            if (FULL) {
+                s_Z[tid] = s_w[q] * (ds.qm[sp] * ezb) * (izc * e1);
+                s_ZM[tid] = s_w[q] * shift * bq;
+            }
         }
         __syncthreads();
-        double acc = 0.0;
-        for (int q = 0; q < Nq; ++q)
+        double acc = 0.0, accM = 0.0;
+        for (int q = 0; q < Nq; ++q) {
             acc = fma(s_E0[q * Nb + a], s_X[q * Nb + bb], fma(s_E1[q * Nb + a], s_Y[q * Nb + bb], acc));
+            if (FULL) {
+                acc = fma(s_B[q * Nb + a], s_Z[q * Nb + bb], acc);
+                accM = fma(s_B[q * Nb + a], s_ZM[q * Nb + bb], accM);
+            }
+        }
         const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
-        Ce[mat * Nb * Nb + tid] = acc;
+        Ce[mat * Nb * Nb + tid] = acc + accM;
         s_Ce[tid] = acc;
         __syncthreads();
         if (tid < Nb) {
@@ -519,9 +538,10 @@ int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, c
 }
 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
-                   cudaStream_t st) {
+                   const double *Ez, double shift, cudaStream_t st) {
     dim3 grid(ds.Ne, nb);
-    k_element<<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce);
+    if (Ez) k_element<true><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
+    else k_element<false><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
     return 1;
 }
 

@@ -24,6 +24,7 @@ struct DeviceSpace {
     double m0m[MAX_SPECIES];   // m0/m_b
     double kfac[MAX_SPECIES];  // nu e_a^2 (m0/m_a)
     double dfac[MAX_SPECIES];  // -nu e_a^2 (m0/m_a)^2
+    double qm[MAX_SPECIES];    // e_a m0/m_a (E-field advection, Eq. 4)
 };
 
 // Scratch for up to max_batch problems.
@@ -38,8 +39,9 @@ struct Scratch {
 // each returns the number of kernels launched
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
 int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st);
+// Ez == nullptr: collision Jacobian C_e; else the implicit-step operator shift M + A_E - J (Ez[nb] device)
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce,
-                   double *ce, cudaStream_t st);
+                   double *ce, const double *Ez, double shift, cudaStream_t st);
 int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st);
 int launch_gather_cf(const DeviceSpace &ds, int nvec, const double *ce, double *Cf, cudaStream_t st);
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);

@@ -103,6 +103,35 @@ def test_paper_shaped_ten_species_context_parity(gpu, oracle, cfg):
     print(f"{wl.name}: worst block error {worst:.2e}")
 
 
+@pytest.mark.parametrize("cfg,variant", [(0, "B"), (3, "A"), (4, "B")])
+def test_implicit_operator_parity(gpu, oracle, cfg, variant):
+    """shift M + A(E_z) - J and A f - C(f) in one pass, against the oracle; two problems
+    with different fields in one batched call; E_z = 0, shift = 0 reproduces -J and -C(f) bitwise."""
+    import torch
+    wl = inputs.config(cfg, variant=variant)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 2)
+    r, z = ctx.dof_coords()
+    f1 = inputs.nodal_f(wl, r, z)
+    f = np.stack([f1, 1.25 * f1])
+    Ez = np.array([0.37, -2.0])
+    shift = 2.5
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.full((2, ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+    F = torch.full((2, ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.from_numpy(Ez).cuda(), shift, vals, F)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    for k in range(2):
+        ov, oF = oracle.implicit_operator(sp, wl.species, f[k], float(Ez[k]), shift)
+        for a in range(ctx.S):
+            assert block_err(vals[k, a].cpu().numpy(), ov[a]) <= TOL, (k, a)
+            assert block_err(F[k, a].cpu().numpy(), oF[a]) <= TOL, (k, a)
+    v0 = torch.zeros_like(vals); F0 = torch.zeros_like(F)
+    ctx.implicit_operator_batched(fd, torch.zeros(2, dtype=torch.float64, device="cuda"), 0.0, v0, F0)
+    vj = torch.zeros_like(vals); cj = torch.zeros_like(F)
+    ctx.jacobian_batched(fd, vj, cj)
+    assert torch.equal(v0, -vj) and torch.equal(F0, -cj)
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch
