@@ -15,7 +15,8 @@ What it computes (PAPER.md = /root/reference/PAPER.md, arxiv 2104.10000):
   evaluated DIRECTLY from Eqs. 5-6 at f -- not as J f, so that J f = C(f) is a test;
 * the scaled mass matrix (L280);
 * the E-field advection term on the left of Eq. 4 (L52) and the operator of a fully implicit step,
-  shift M + A_a - J_a with its residual A_a f_a - C_a(f).
+  shift M + A_a - J_a with its residual A_a f_a - C_a(f) (SURVEY 8(f) NEXT-3);
+* the same operator with species clustered on several grids (section III-C, Table I; NEXT-2).
 
 Everything outside the O(N^2) pair loop is plain numpy in fp64 with dense matrices (no
 blocking, no gather lists).  The pair loop is plain C in long double (``_ld``) for parity and
@@ -479,3 +480,53 @@ def build_all(mesh, order: int, species, f: np.ndarray, shift: float = 1.0, prec
     vals = np.stack([csr_values(sp, assemble_dense(sp, Ce[a])) for a in range(f.shape[0])])
     Cf = collision(sp, species, f, precision, (K, D))
     return sp, vals, Cf, mass(sp, shift)
+
+
+# --------------------------------------------------------------------------------------------
+# Multiple grids (section III-C, Table I): species clustered by thermal speed
+# live on separate meshes; the inner integral of Eqs. 7-8 runs over the UNION of all grids'
+# integration points ("overbar terms are evaluated on the grid for the domain of species beta",
+# L42), each species contributing only at the points of its own grid.
+# --------------------------------------------------------------------------------------------
+
+def build_all_multigrid(meshes, order: int, species, species_grid, f_list, shift: float = 1.0, precision: str = "ld"):
+    """species_grid[a] = grid of species a; f_list[a] = nodal values of species a on ITS grid.
+    Returns (spaces, vals_list, Cf_list, mass_list): per species CSR values / C(f) on its grid's
+    pattern, per grid the scaled mass matrix.  A coincident pair (same location, also when the
+    two points belong to different grids) contributes nothing (reading Q3)."""
+    spaces = [build_space(m, order) for m in meshes]
+    S = len(f_list)
+    off = np.concatenate([[0], np.cumsum([sp.N for sp in spaces])])
+    Ntot = int(off[-1])
+    r = np.concatenate([sp.r for sp in spaces]); z = np.concatenate([sp.z for sp in spaces])
+    w = np.concatenate([sp.w_in for sp in spaces])
+    fq = np.zeros((S, Ntot)); dfr = np.zeros((S, Ntot)); dfz = np.zeros((S, Ntot))
+    for a in range(S):
+        g = int(species_grid[a]); sp = spaces[g]
+        q, dr_, dz_ = fields_at_points(sp, np.asarray(f_list[a])[None, :])
+        sl = slice(off[g], off[g + 1])
+        fq[a, sl], dfr[a, sl], dfz[a, sl] = q[0], dr_[0], dz_[0]
+    e2 = np.asarray(species.charge, dtype=np.float64) ** 2
+    m0m = species.m0 / np.asarray(species.mass, dtype=np.float64)
+    GD, GK = inner_integral(r, z, w, fq, dfr, dfz, e2, m0m, None, precision)
+    vals_list, Cf_list = [], []
+    for a in range(S):
+        g = int(species_grid[a]); sp = spaces[g]
+        sl = slice(off[g], off[g + 1])
+        K = (species.nu * e2[a] * m0m[a] * GK[sl])[None]
+        D = np.zeros((1, sp.N, 2, 2))
+        c = -species.nu * e2[a] * m0m[a] ** 2
+        D[0, :, 0, 0] = c * GD[sl, 0]; D[0, :, 0, 1] = c * GD[sl, 1]; D[0, :, 1, 0] = c * GD[sl, 1]; D[0, :, 1, 1] = c * GD[sl, 2]
+        Ce = element_matrices(sp, K, D)
+        vals_list.append(csr_values(sp, assemble_dense(sp, Ce[0])))
+        # C(f) from the weak form with physical gradients, as in collision()
+        Cf = np.zeros(sp.n)
+        for e in range(sp.Ne):
+            ce = np.zeros(sp.Nb)
+            for q in range(sp.Nq):
+                gi = e * sp.Nq + q
+                flux = K[0, gi] * fq[a, off[g] + gi] + D[0, gi] @ np.array([dfr[a, off[g] + gi], dfz[a, off[g] + gi]])
+                ce += sp.w_out[gi] * ((sp.E[q] * sp.invJ[e][None, :]) @ flux)
+            Cf[sp.cell_dofs[e]] += sp.cell_P[e].T @ ce
+        Cf_list.append(Cf)
+    return spaces, vals_list, Cf_list, [mass(sp, shift) for sp in spaces]

@@ -175,7 +175,9 @@ void SUFFIX(oracle_inner_integral)(int N, int S, const double *r, const double *
     for (int i = i_begin; i < i_end; ++i) {
         real gd[3] = {0, 0, 0}, gk[2] = {0, 0};
         for (int j = 0; j < N; ++j) {
-            if (j == i) continue; /* coincident pair: zero contribution (Q3) */
+            /* coincident pair (d2 = 0): zero contribution (Q3).  On one mesh only j == i
+             * coincides; with several grids (section III-C) points of different grids may too. */
+            if (j == i || (r[j] == r[i] && z[j] == z[i])) continue;
             real UD[3], UK[4];
             tensor2d(r[i], z[i], r[j], z[j], UD, UK);
             real TD = 0, TKr = 0, TKz = 0; /* reset per j (Q4) */

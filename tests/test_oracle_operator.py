@@ -193,3 +193,55 @@ def test_advection_term_and_implicit_operator_pins(built, oracle):
         assert np.abs(ov[a] - (shift * M1 + A[a][rows, sp.colidx] - vals[a])).max() <= 1e-13 * np.abs(ov[a]).max()
     ov0, F0 = oracle.implicit_operator(sp, spc, f, 0.0, 0.0)
     assert np.abs(ov0 + vals).max() <= 1e-13 * np.abs(vals).max() and np.abs(F0 + Cf).max() <= 1e-13 * np.abs(Cf).max()
+
+
+def _grid20():
+    return inputs.mesh_quadtree(0.0, 5.0, -5.0, 5.0, 2, 4, 1.0, 2, 2.5, 1)
+
+
+def test_paper_vertex_count_of_the_20_cell_grid(oracle):
+    """the 20-cell Q3 grid of Fig. 3 has 193 unconstrained vertices (pins the hanging-node
+    constraint counting); Table I: three such grids give N = 960 points and 10 x 193 = 1,930 equations."""
+    (cells, order, n), = _rows("vertex_counts.txt")
+    sp = oracle.build_space(_grid20(), int(order))
+    assert (sp.Ne, sp.n) == (int(cells), int(n))
+    assert 3 * sp.N == 960 and 10 * sp.n == 1930
+
+
+def _scaled(mesh, k):
+    return inputs.Mesh(mesh.rmin * k, mesh.rmax * k, mesh.zmin * k, mesh.zmax * k, mesh.nbr, mesh.nbz, mesh.level, mesh.ir, mesh.iz)
+
+
+def test_multigrid_equals_single_grid_on_identical_meshes_and_conserves(oracle):
+    """Section III-C (L179-206).  (1) Two species on two IDENTICAL grids give the single-grid result (every
+    cross-grid coincident pair is skipped exactly like j = i).  (2) Species on grids of different extent:
+    density per species, total z-momentum and total energy are conserved exactly (z and r^2+z^2 lie in
+    every grid's space)."""
+    wl = inputs.config(0)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z)
+    _, vals, Cf, mv = oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.3)
+    _, mvals, mCf, mm = oracle.build_all_multigrid([wl.mesh, wl.mesh], wl.order, wl.species, [0, 1], [f[0], f[1]], 1.3)
+    for a in range(2):
+        assert np.abs(mvals[a] - vals[a]).max() <= 1e-13 * np.abs(vals[a]).max()
+        assert np.abs(mCf[a] - Cf[a]).max() <= 1e-13 * np.abs(Cf[a]).max()
+        assert np.array_equal(mm[a], mv)
+    # three species, two grids of different extent (electron grid, ion grid 8x smaller: v_th ratio)
+    spc = inputs._sp([(1, -1, 1, 1), (64, 1, 0.6, 1), (128, 2, 0.2, 1)])
+    g0 = inputs.mesh_quadtree(0.0, 4.0, -4.0, 4.0, 2, 4, 1.0, 2, 2.0, 1)
+    g1 = _scaled(g0, 0.125)
+    grids = [0, 1, 1]
+    spaces = [oracle.build_space(g, 2) for g in (g0, g1)]
+    fl = []
+    for a in range(3):
+        s_ = spaces[grids[a]]
+        fa = inputs.maxwellian(spc.mass[a], spc.density[a], 1.0, 0.02 * a, s_.dof_r, s_.dof_z)
+        fl.append(fa * (1.0 + 1e-3 * np.cos(7.0 * np.arange(s_.n))))
+    _, v, C, _ = oracle.build_all_multigrid([g0, g1], 2, spc, grids, fl, 1.0)
+    for a in range(3):
+        assert abs(C[a].sum()) <= 1e-13 * np.abs(C[a]).sum()
+    for psi in (lambda s_: s_.dof_z, lambda s_: 0.5 * (s_.dof_r ** 2 + s_.dof_z ** 2)):
+        num = abs(sum(spc.mass[a] * (psi(spaces[grids[a]]) @ C[a]) for a in range(3)))
+        den = sum(spc.mass[a] * np.abs(psi(spaces[grids[a]]) * C[a]).sum() for a in range(3))
+        assert num <= 1e-12 * den
+    assert abs(spaces[0].dof_z @ C[0]) > 1e-6 * np.abs(spaces[0].dof_z * C[0]).sum()   # the pin bites
