@@ -85,6 +85,27 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
                   landau_ctx **out);
 int landau_destroy(landau_ctx *ctx);
 
+/* Several grids (section III-C, Table I): species clustered by thermal speed live on
+ * separate meshes of one order; the inner integral of Eqs. 7-8 runs over the UNION of all grids'
+ * integration points, each species contributing at the points of its own grid, and the Jacobian
+ * block of a species has its grid's pattern.  meshes: [ngrids] host; species_grid: [S] host,
+ * non-decreasing, every grid used (species are grouped by grid).  Per-problem layouts become
+ *   f, Cf, F: [species][n of its grid]   vals: [species][nnz of its grid]   mvals: [grid][nnz of the grid]
+ * with the sizes from landau_strides / landau_grid_sizes.  Points of different grids that coincide
+ * exactly are treated like j = i (no contribution).  landau_create is the ngrids = 1 case. */
+int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t *species_grid, int order,
+                            const landau_species *species, int max_batch, landau_ctx **out);
+int landau_grid_count(const landau_ctx *ctx, int32_t *ngrids);
+/* Per grid: its species count and first species, n, nnz, integration points, cells (any may be NULL). */
+int landau_grid_sizes(const landau_ctx *ctx, int grid, int32_t *S_g, int32_t *first_species, int64_t *n,
+                      int64_t *nnz, int64_t *N, int64_t *Ne);
+/* Doubles per problem in f / Cf (f_stride) and vals (vals_stride), length of mvals, points of all grids. */
+int landau_strides(const landau_ctx *ctx, int32_t *S, int64_t *f_stride, int64_t *vals_stride,
+                   int64_t *mvals_size, int64_t *N_total);
+int landau_grid_csr_pattern(const landau_ctx *ctx, int grid, const int32_t **rowptr_dev, const int32_t **colidx_dev);
+int landau_grid_csr_pattern_host(const landau_ctx *ctx, int grid, int32_t *rowptr_host, int32_t *colidx_host);
+int landau_grid_dof_coords(const landau_ctx *ctx, int grid, double *r_host, double *z_host);
+
 /* Host-only part of landau_create (no CUDA device needed): runs the same set-up and returns the
  * sizes and, where the pointer is not NULL, the CSR pattern of A1 (rowptr[n+1], colidx[nnz]) and
  * the unknowns' node coordinates ([n] each).  Call once with NULL arrays to get the sizes. */

@@ -36,6 +36,15 @@ _lib = None
 SIGNATURES = {
     "landau_create": (c_int, [POINTER(landau_mesh), c_int, POINTER(landau_species), c_int, POINTER(c_void_p)]),
     "landau_destroy": (c_int, [c_void_p]),
+    "landau_create_multigrid": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), c_int, POINTER(landau_species), c_int,
+                                        POINTER(c_void_p)]),
+    "landau_grid_count": (c_int, [c_void_p, POINTER(c_int32)]),
+    "landau_grid_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_int64), POINTER(c_int64),
+                                  POINTER(c_int64), POINTER(c_int64)]),
+    "landau_strides": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]),
+    "landau_grid_csr_pattern": (c_int, [c_void_p, c_int, POINTER(c_void_p), POINTER(c_void_p)]),
+    "landau_grid_csr_pattern_host": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32)]),
+    "landau_grid_dof_coords": (c_int, [c_void_p, c_int, POINTER(c_double), POINTER(c_double)]),
     "landau_setup_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int64), POINTER(c_int64), POINTER(c_int64),
                                   POINTER(c_int32), POINTER(c_int32), POINTER(c_double), POINTER(c_double)]),
     "landau_sizes": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64), POINTER(c_int64)]),
@@ -236,3 +245,83 @@ class LandauContext:
         c = c_int64()
         _check(lib().landau_launch_count(self._h, ctypes.byref(c)))
         return c.value
+
+
+class LandauMultigridContext:
+    """landau_create_multigrid: species clustered on several grids.  Per-problem layouts are flat:
+    f, Cf, F: [nb][f_stride] (species after species, each with the n of its grid), vals: [nb][vals_stride],
+    mvals: [mvals_size]; `species_slices()` / `vals_slices()` give each species' range."""
+
+    def __init__(self, meshes, species_grid, order: int, species, max_batch: int = 1):
+        L = lib()
+        structs, keep = [], []
+        for m in meshes:
+            st, k = _mesh_struct(m)
+            structs.append(st); keep.append(k)
+        arr = (landau_mesh * len(meshes))(*structs)
+        sg = _i32(species_grid)
+        mass, charge = _f64(species.mass), _f64(species.charge)
+        dens, temp = _f64(species.density), _f64(species.temperature)
+        sp = landau_species(int(mass.shape[0]), _dp(mass), _dp(charge), _dp(dens), _dp(temp), float(species.m0), float(species.nu))
+        h = c_void_p()
+        _check(L.landau_create_multigrid(arr, len(meshes), sg.ctypes.data_as(POINTER(c_int32)), order, ctypes.byref(sp),
+                                         int(max_batch), ctypes.byref(h)))
+        self._h = h
+        S, fs, vs, ms, Nt = c_int32(), c_int64(), c_int64(), c_int64(), c_int64()
+        _check(L.landau_strides(h, ctypes.byref(S), ctypes.byref(fs), ctypes.byref(vs), ctypes.byref(ms), ctypes.byref(Nt)))
+        self.S, self.f_stride, self.vals_stride, self.mvals_size, self.N = S.value, fs.value, vs.value, ms.value, Nt.value
+        ng = c_int32()
+        _check(L.landau_grid_count(h, ctypes.byref(ng)))
+        self.grids = []
+        for g in range(ng.value):
+            Sg, s0, n, nnz, N, Ne = c_int32(), c_int32(), c_int64(), c_int64(), c_int64(), c_int64()
+            _check(L.landau_grid_sizes(h, g, ctypes.byref(Sg), ctypes.byref(s0), ctypes.byref(n), ctypes.byref(nnz), ctypes.byref(N), ctypes.byref(Ne)))
+            self.grids.append(dict(S=Sg.value, first_species=s0.value, n=n.value, nnz=nnz.value, N=N.value, Ne=Ne.value))
+        self.species_grid = [int(g) for g in sg]
+        self.max_batch = int(max_batch)
+
+    destroy = LandauContext.destroy
+    __del__ = LandauContext.__del__
+    _ptr = staticmethod(LandauContext._ptr)
+    launch_count = LandauContext.launch_count
+
+    def species_slices(self):
+        out, o = [], 0
+        for a in range(self.S):
+            n = self.grids[self.species_grid[a]]["n"]
+            out.append(slice(o, o + n)); o += n
+        return out
+
+    def vals_slices(self):
+        out, o = [], 0
+        for a in range(self.S):
+            n = self.grids[self.species_grid[a]]["nnz"]
+            out.append(slice(o, o + n)); o += n
+        return out
+
+    def grid_dof_coords(self, g):
+        n = self.grids[g]["n"]
+        r, z = np.zeros(n), np.zeros(n)
+        _check(lib().landau_grid_dof_coords(self._h, g, _dp(r), _dp(z)))
+        return r, z
+
+    def grid_csr_pattern_host(self, g):
+        rowptr, colidx = np.zeros(self.grids[g]["n"] + 1, np.int32), np.zeros(self.grids[g]["nnz"], np.int32)
+        _check(lib().landau_grid_csr_pattern_host(self._h, g, rowptr.ctypes.data_as(POINTER(c_int32)), colidx.ctypes.data_as(POINTER(c_int32))))
+        return rowptr, colidx
+
+    def jacobian_batched(self, f, vals=None, Cf=None, stream=None):
+        nb = f.shape[0]
+        pv = self._ptr(vals, (nb, self.vals_stride)) if vals is not None else None
+        pc = self._ptr(Cf, (nb, self.f_stride)) if Cf is not None else None
+        _check(lib().landau_jacobian_batched(self._h, nb, self._ptr(f, (nb, self.f_stride)), pv, pc, _stream_ptr(stream)))
+
+    def implicit_operator_batched(self, f, Ez, shift, vals=None, F=None, stream=None):
+        nb = f.shape[0]
+        pv = self._ptr(vals, (nb, self.vals_stride)) if vals is not None else None
+        pf = self._ptr(F, (nb, self.f_stride)) if F is not None else None
+        _check(lib().landau_implicit_operator_batched(self._h, nb, self._ptr(f, (nb, self.f_stride)), self._ptr(Ez, (nb,)),
+                                                      float(shift), pv, pf, _stream_ptr(stream)))
+
+    def mass(self, shift, mvals, stream=None):
+        _check(lib().landau_mass(self._h, float(shift), self._ptr(mvals, (self.mvals_size,)), _stream_ptr(stream)))

@@ -1,11 +1,17 @@
 // C-ABI layer (include/landau.h): context management, argument checking, kernel sequencing.
 // Every step of the path runs in landau_kernels.cu; there is no CPU fallback.
+//
+// A context holds one or several grids (section III-C: species clustered by thermal speed on
+// separate meshes).  Species are grouped by grid in ascending order, so the per-problem layouts are
+//   f, Cf:  [species][n of its grid]      vals: [species][nnz of its grid]
+// i.e. grid-major blocks [S_g][n_g]; with one grid these are the plain [S][n] / [S][nnz].
 #include <cuda_runtime.h>
 
-#include <cstdio>
 #include <algorithm>
+#include <cstdio>
 #include <cstring>
 #include <new>
+#include <numeric>
 #include <string>
 #include <vector>
 
@@ -39,11 +45,26 @@ int upload(const std::vector<T> &v, const T **out, std::vector<void *> &owned) {
     *out = static_cast<const T *>(d);
     return LANDAU_OK;
 }
+
+struct GridState {
+    HostSpace hs;
+    DeviceSpace ds;
+    int s0 = 0;              // first species of this grid
+    size_t foff = 0;         // offset (doubles) of this grid's block inside one problem's f / Cf
+    size_t voff = 0;         // ... inside one problem's vals
+    size_t moff = 0;         // ... inside mvals
+    double *Ce = nullptr;    // [nb][S_g][Ne][Nb*Nb]
+    double *ce = nullptr;    // [nb][S_g][Ne][Nb]
+};
 }  // namespace
 
 struct landau_ctx {
-    HostSpace hs;
-    DeviceSpace ds;
+    std::vector<GridState> grids;
+    int S = 0;                       // all species
+    int64_t Ntot = 0;                // integration points of all grids
+    size_t fstride = 0, vstride = 0, mstride = 0;   // doubles per problem in f / vals; in mvals
+    const double *r = nullptr, *z = nullptr, *invr = nullptr;   // [Ntot] union of the grids' points
+    bool check_all = false;          // points of different grids coincide somewhere
     Scratch sc;
     std::vector<void *> owned;   // device allocations
     int max_batch = 1;
@@ -51,7 +72,7 @@ struct landau_ctx {
     int64_t launches = 0;
     cudaStream_t own_stream = nullptr, copy_stream = nullptr;
     cudaEvent_t chunk_done = nullptr;
-    double *h2d_f = nullptr, *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
+    double *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
     int host_nb = 0;
     bool profiling = false;
     std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;  // recorded, not yet read
@@ -61,15 +82,45 @@ struct landau_ctx {
 namespace {
 // launch_pair bracketed by events when profiling is on
 int timed_pair(landau_ctx *ctx, int nb, double *G, cudaStream_t st) {
-    if (!ctx->profiling) return launch_pair(ctx->ds, nb, ctx->sc.T, G, st);
+    auto go = [&]() { return launch_pair(int(ctx->Ntot), ctx->r, ctx->z, ctx->invr, ctx->check_all, nb, ctx->sc.T, G, st); };
+    if (!ctx->profiling) return go();
     std::pair<cudaEvent_t, cudaEvent_t> ev;
     if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
     else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
     cudaEventRecord(ev.first, st);
-    int k = launch_pair(ctx->ds, nb, ctx->sc.T, G, st);
+    int k = go();
     cudaEventRecord(ev.second, st);
     ctx->prof_events.push_back(ev);
     return k;
+}
+
+// a1-a3 for nb problems: fields + beta sums per grid, pair kernel over the union, tile-order sum
+void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, cudaStream_t st) {
+    for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nb, f_dev + g.foff, ctx->sc.T, st);
+    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
+    ctx->launches += launch_sum_partials(int(ctx->Ntot), nb, pair_tiles(int(ctx->Ntot)), ctx->sc.G, Gsum, st);
+}
+
+// a4-a7 for nb problems; Ez == nullptr: collision Jacobian and C(f), else the implicit-step operator
+void assemble(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez, double shift, double *vals_dev, double *Cf_dev,
+              cudaStream_t st) {
+    for (auto &g : ctx->grids) {
+        ctx->launches += launch_element(g.ds, nb, 1, f_dev + g.foff, ctx->sc.Gsum, g.Ce, g.ce, Ez, shift, st);
+        if (vals_dev) ctx->launches += launch_gather_vals(g.ds, nb, g.ds.S, ctx->vstride, g.Ce, vals_dev + g.voff, st);
+        if (Cf_dev) ctx->launches += launch_gather_cf(g.ds, nb, ctx->fstride, g.ce, Cf_dev + g.foff, st);
+    }
+}
+
+// Do two points of DIFFERENT grids coincide exactly?  (Then every pair must be tested, reading Q3.)
+bool cross_grid_coincidence(const std::vector<GridState> &grids) {
+    struct P { double r, z; int g; };
+    std::vector<P> pts;
+    for (size_t g = 0; g < grids.size(); ++g)
+        for (int64_t i = 0; i < grids[g].hs.N; ++i) pts.push_back({grids[g].hs.r[i], grids[g].hs.z[i], int(g)});
+    std::sort(pts.begin(), pts.end(), [](const P &a, const P &b) { return a.r != b.r ? a.r < b.r : (a.z != b.z ? a.z < b.z : a.g < b.g); });
+    for (size_t i = 1; i < pts.size(); ++i)
+        if (pts[i].r == pts[i - 1].r && pts[i].z == pts[i - 1].z) return true;   // within one grid points never coincide
+    return false;
 }
 }  // namespace
 
@@ -102,14 +153,27 @@ int landau_destroy(landau_ctx *ctx) {
     return LANDAU_OK;
 }
 
-int landau_create(const landau_mesh *mesh, int order, const landau_species *species, int max_batch, landau_ctx **out) {
+int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t *species_grid, int order,
+                            const landau_species *species, int max_batch, landau_ctx **out) {
     if (!out) return LANDAU_EINVAL;
     *out = nullptr;
-    if (!mesh || !species || max_batch < 1) return LANDAU_EINVAL;
+    if (!meshes || !species || ngrids < 1 || max_batch < 1 || max_batch > 65535) return LANDAU_EINVAL;
     if (species->S < 1 || species->S > MAX_SPECIES || !species->mass || !species->charge) return LANDAU_EINVAL;
     if (!(species->m0 > 0.0)) return LANDAU_EINVAL;
-    for (int s = 0; s < species->S; ++s)
+    const int S = species->S;
+    for (int s = 0; s < S; ++s)
         if (!(species->mass[s] > 0.0)) return LANDAU_EINVAL;
+    // species grouped by grid: the map must be non-decreasing and use every grid
+    std::vector<int> sgrid(S, 0);
+    if (ngrids > 1) {
+        if (!species_grid) return LANDAU_EINVAL;
+        for (int s = 0; s < S; ++s) {
+            sgrid[s] = species_grid[s];
+            if (sgrid[s] < 0 || sgrid[s] >= ngrids || (s && sgrid[s] < sgrid[s - 1])) return LANDAU_EINVAL;
+        }
+        for (int g = 0; g < ngrids; ++g)
+            if (std::find(sgrid.begin(), sgrid.end(), g) == sgrid.end()) return LANDAU_EINVAL;
+    }
     int ndev = 0;
     if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1) {
         g_cuda_err = "no CUDA device (this library has no CPU fallback)";
@@ -117,54 +181,83 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
     }
     landau_ctx *ctx = new (std::nothrow) landau_ctx();
     if (!ctx) return LANDAU_ENOMEM;
-    std::string err;
-    int rc;
-    try {
-        rc = build_host_space(*mesh, order, ctx->hs, err);
-    } catch (const std::bad_alloc &) {
-        delete ctx;
-        return LANDAU_ENOMEM;
+    ctx->grids.resize(ngrids);
+    ctx->S = S;
+    ctx->max_batch = max_batch;
+    int rc = LANDAU_OK;
+    for (int g = 0; g < ngrids; ++g) {
+        std::string err;
+        try {
+            rc = build_host_space(meshes[g], order, ctx->grids[g].hs, err);
+        } catch (const std::bad_alloc &) {
+            delete ctx;
+            return LANDAU_ENOMEM;
+        }
+        if (rc != LANDAU_OK) { g_cuda_err = err; delete ctx; return rc; }
     }
-    if (rc != LANDAU_OK) { g_cuda_err = err; delete ctx; return rc; }
-    HostSpace &hs = ctx->hs;
-    if (hs.N > (int64_t(1) << 30) || hs.nnz > (int64_t(1) << 30)) { delete ctx; return LANDAU_EINVAL; }
-    DeviceSpace &ds = ctx->ds;
-    std::memset(&ds, 0, sizeof(ds));
-    ds.p = hs.p; ds.Nq = hs.Nq; ds.Nb = hs.Nb; ds.S = species->S;
-    ds.N = int(hs.N); ds.Ne = int(hs.Ne); ds.n = int(hs.n); ds.nnz = int(hs.nnz);
-    for (int s = 0; s < ds.S; ++s) {
-        const double e2 = species->charge[s] * species->charge[s], mm = species->m0 / species->mass[s];
-        ds.e2[s] = e2; ds.m0m[s] = mm;
-        ds.kfac[s] = species->nu * e2 * mm;
-        ds.dfac[s] = -species->nu * e2 * mm * mm;
-        ds.qm[s] = species->charge[s] * mm;
+    // offsets and sizes
+    std::vector<double> r, z, invr;
+    for (int g = 0; g < ngrids; ++g) {
+        GridState &G = ctx->grids[g];
+        const HostSpace &hs = G.hs;
+        G.s0 = int(std::find(sgrid.begin(), sgrid.end(), g) - sgrid.begin());
+        const int Sg = int(std::count(sgrid.begin(), sgrid.end(), g));
+        G.foff = ctx->fstride; G.voff = ctx->vstride; G.moff = ctx->mstride;
+        ctx->fstride += size_t(Sg) * hs.n; ctx->vstride += size_t(Sg) * hs.nnz; ctx->mstride += size_t(hs.nnz);
+        DeviceSpace &ds = G.ds;
+        std::memset(&ds, 0, sizeof(ds));
+        ds.p = hs.p; ds.Nq = hs.Nq; ds.Nb = hs.Nb; ds.S = Sg;
+        ds.N = int(hs.N); ds.Ne = int(hs.Ne); ds.n = int(hs.n); ds.nnz = int(hs.nnz);
+        ds.poff = int(ctx->Ntot);
+        ctx->Ntot += hs.N;
+        for (int t = 0; t < Sg; ++t) {
+            const int s = G.s0 + t;
+            const double e2 = species->charge[s] * species->charge[s], mm = species->m0 / species->mass[s];
+            ds.e2[t] = e2; ds.m0m[t] = mm;
+            ds.kfac[t] = species->nu * e2 * mm;
+            ds.dfac[t] = -species->nu * e2 * mm * mm;
+            ds.qm[t] = species->charge[s] * mm;
+        }
+        r.insert(r.end(), hs.r.begin(), hs.r.end());
+        z.insert(z.end(), hs.z.begin(), hs.z.end());
+        for (int64_t i = 0; i < hs.N; ++i) invr.push_back(1.0 / hs.r[i]);
     }
-    std::vector<double> invr(hs.N);
-    for (int64_t i = 0; i < hs.N; ++i) invr[i] = 1.0 / hs.r[i];
+    if (ctx->Ntot > (int64_t(1) << 30) || ctx->vstride > (size_t(1) << 32)) { delete ctx; return LANDAU_EINVAL; }
+    ctx->check_all = ngrids > 1 && cross_grid_coincidence(ctx->grids);
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev);
-    ctx->max_batch = max_batch;
 
-#define UP(field, vec)                                                   \
-    if ((rc = upload(vec, &ds.field, ctx->owned)) != LANDAU_OK) { landau_destroy(ctx); return rc; }
-    UP(r, hs.r) UP(z, hs.z) UP(invr, invr) UP(w_in, hs.w_in) UP(w_out, hs.w_out) UP(invJ, hs.invJ)
-    UP(B, hs.B) UP(E0, hs.E0) UP(E1, hs.E1)
-    UP(lptr, hs.lptr) UP(ldof, hs.ldof) UP(lw, hs.lw)
-    UP(rowptr, hs.rowptr) UP(colidx, hs.colidx)
-    UP(gptr, hs.gptr) UP(gidx, hs.gidx) UP(gw, hs.gw)
-    UP(cptr, hs.cptr) UP(cidx, hs.cidx) UP(cw, hs.cw)
-#undef UP
-    // scratch arena
+#define UPC(ptr, vec) \
+    if ((rc = upload(vec, &(ptr), ctx->owned)) != LANDAU_OK) { landau_destroy(ctx); return rc; }
+    UPC(ctx->r, r) UPC(ctx->z, z) UPC(ctx->invr, invr)
     const size_t nbm = size_t(max_batch);
-    const size_t gsz = nbm * pair_tiles(ds.N) * 5 * hs.N;
-    struct { double **p; size_t n; } allocs[] = {
-        {&ctx->sc.T, nbm * 3 * hs.N},
-        {&ctx->sc.G, gsz},
-        {&ctx->sc.Gsum, nbm * 5 * hs.N},
-        {&ctx->sc.Ce, nbm * ds.S * hs.Ne * hs.Nb * hs.Nb},
-        {&ctx->sc.ce, nbm * ds.S * hs.Ne * hs.Nb},
+    for (int g = 0; g < ngrids; ++g) {
+        GridState &G = ctx->grids[g];
+        HostSpace &hs = G.hs;
+        DeviceSpace &ds = G.ds;
+        ds.Ntot = int(ctx->Ntot);
+        ds.fstride = (long long)ctx->fstride;
+        ds.r = ctx->r + ds.poff; ds.z = ctx->z + ds.poff; ds.invr = ctx->invr + ds.poff;
+        UPC(ds.w_in, hs.w_in) UPC(ds.w_out, hs.w_out) UPC(ds.invJ, hs.invJ)
+        UPC(ds.B, hs.B) UPC(ds.E0, hs.E0) UPC(ds.E1, hs.E1)
+        UPC(ds.lptr, hs.lptr) UPC(ds.ldof, hs.ldof) UPC(ds.lw, hs.lw)
+        UPC(ds.rowptr, hs.rowptr) UPC(ds.colidx, hs.colidx)
+        UPC(ds.gptr, hs.gptr) UPC(ds.gidx, hs.gidx) UPC(ds.gw, hs.gw)
+        UPC(ds.cptr, hs.cptr) UPC(ds.cidx, hs.cidx) UPC(ds.cw, hs.cw)
+    }
+#undef UPC
+    // scratch arena
+    struct Alloc { double **p; size_t n; };
+    std::vector<Alloc> allocs = {
+        {&ctx->sc.T, nbm * 3 * ctx->Ntot},
+        {&ctx->sc.G, nbm * pair_tiles(int(ctx->Ntot)) * 5 * ctx->Ntot},
+        {&ctx->sc.Gsum, nbm * 5 * ctx->Ntot},
     };
+    for (auto &G : ctx->grids) {
+        allocs.push_back({&G.Ce, nbm * G.ds.S * G.hs.Ne * G.hs.Nb * G.hs.Nb});
+        allocs.push_back({&G.ce, nbm * G.ds.S * G.hs.Ne * G.hs.Nb});
+    }
     for (auto &a : allocs) {
         void *d = nullptr;
         cudaError_t e = cudaMalloc(&d, a.n * sizeof(double));
@@ -178,6 +271,10 @@ int landau_create(const landau_mesh *mesh, int order, const landau_species *spec
     }
     *out = ctx;
     return LANDAU_OK;
+}
+
+int landau_create(const landau_mesh *mesh, int order, const landau_species *species, int max_batch, landau_ctx **out) {
+    return landau_create_multigrid(mesh, 1, nullptr, order, species, max_batch, out);
 }
 
 int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *nnz, int64_t *N, int32_t *rowptr_host,
@@ -202,51 +299,100 @@ int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *n
     return LANDAU_OK;
 }
 
-int landau_sizes(const landau_ctx *ctx, int32_t *S, int64_t *n, int64_t *nnz, int64_t *N, int64_t *Ne) {
+int landau_grid_count(const landau_ctx *ctx, int32_t *ngrids) {
+    if (!ctx || !ngrids) return LANDAU_EINVAL;
+    *ngrids = int32_t(ctx->grids.size());
+    return LANDAU_OK;
+}
+
+int landau_grid_sizes(const landau_ctx *ctx, int grid, int32_t *S_g, int32_t *first_species, int64_t *n, int64_t *nnz,
+                      int64_t *N, int64_t *Ne) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    const GridState &G = ctx->grids[grid];
+    if (S_g) *S_g = G.ds.S;
+    if (first_species) *first_species = G.s0;
+    if (n) *n = G.hs.n;
+    if (nnz) *nnz = G.hs.nnz;
+    if (N) *N = G.hs.N;
+    if (Ne) *Ne = G.hs.Ne;
+    return LANDAU_OK;
+}
+
+int landau_strides(const landau_ctx *ctx, int32_t *S, int64_t *f_stride, int64_t *vals_stride, int64_t *mvals_size, int64_t *N_total) {
     if (!ctx) return LANDAU_EINVAL;
-    if (S) *S = ctx->ds.S;
-    if (n) *n = ctx->hs.n;
-    if (nnz) *nnz = ctx->hs.nnz;
-    if (N) *N = ctx->hs.N;
-    if (Ne) *Ne = ctx->hs.Ne;
+    if (S) *S = ctx->S;
+    if (f_stride) *f_stride = int64_t(ctx->fstride);
+    if (vals_stride) *vals_stride = int64_t(ctx->vstride);
+    if (mvals_size) *mvals_size = int64_t(ctx->mstride);
+    if (N_total) *N_total = ctx->Ntot;
+    return LANDAU_OK;
+}
+
+int landau_sizes(const landau_ctx *ctx, int32_t *S, int64_t *n, int64_t *nnz, int64_t *N, int64_t *Ne) {
+    if (!ctx || ctx->grids.size() != 1) return LANDAU_EINVAL;
+    const HostSpace &hs = ctx->grids[0].hs;
+    if (S) *S = ctx->S;
+    if (n) *n = hs.n;
+    if (nnz) *nnz = hs.nnz;
+    if (N) *N = hs.N;
+    if (Ne) *Ne = hs.Ne;
+    return LANDAU_OK;
+}
+
+int landau_grid_csr_pattern(const landau_ctx *ctx, int grid, const int32_t **rowptr_dev, const int32_t **colidx_dev) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    if (rowptr_dev) *rowptr_dev = ctx->grids[grid].ds.rowptr;
+    if (colidx_dev) *colidx_dev = ctx->grids[grid].ds.colidx;
+    return LANDAU_OK;
+}
+
+int landau_grid_csr_pattern_host(const landau_ctx *ctx, int grid, int32_t *rowptr_host, int32_t *colidx_host) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    const HostSpace &hs = ctx->grids[grid].hs;
+    if (rowptr_host) std::memcpy(rowptr_host, hs.rowptr.data(), hs.rowptr.size() * sizeof(int32_t));
+    if (colidx_host) std::memcpy(colidx_host, hs.colidx.data(), hs.colidx.size() * sizeof(int32_t));
+    return LANDAU_OK;
+}
+
+int landau_grid_dof_coords(const landau_ctx *ctx, int grid, double *r_host, double *z_host) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    const HostSpace &hs = ctx->grids[grid].hs;
+    if (r_host) std::memcpy(r_host, hs.dof_r.data(), hs.n * sizeof(double));
+    if (z_host) std::memcpy(z_host, hs.dof_z.data(), hs.n * sizeof(double));
     return LANDAU_OK;
 }
 
 int landau_csr_pattern(const landau_ctx *ctx, const int32_t **rowptr_dev, const int32_t **colidx_dev) {
-    if (!ctx) return LANDAU_EINVAL;
-    if (rowptr_dev) *rowptr_dev = ctx->ds.rowptr;
-    if (colidx_dev) *colidx_dev = ctx->ds.colidx;
-    return LANDAU_OK;
+    if (!ctx || ctx->grids.size() != 1) return LANDAU_EINVAL;
+    return landau_grid_csr_pattern(ctx, 0, rowptr_dev, colidx_dev);
 }
 
 int landau_csr_pattern_host(const landau_ctx *ctx, int32_t *rowptr_host, int32_t *colidx_host) {
-    if (!ctx) return LANDAU_EINVAL;
-    if (rowptr_host) std::memcpy(rowptr_host, ctx->hs.rowptr.data(), ctx->hs.rowptr.size() * sizeof(int32_t));
-    if (colidx_host) std::memcpy(colidx_host, ctx->hs.colidx.data(), ctx->hs.colidx.size() * sizeof(int32_t));
-    return LANDAU_OK;
+    if (!ctx || ctx->grids.size() != 1) return LANDAU_EINVAL;
+    return landau_grid_csr_pattern_host(ctx, 0, rowptr_host, colidx_host);
 }
 
 int landau_dof_coords(const landau_ctx *ctx, double *r_host, double *z_host) {
-    if (!ctx) return LANDAU_EINVAL;
-    if (r_host) std::memcpy(r_host, ctx->hs.dof_r.data(), ctx->hs.n * sizeof(double));
-    if (z_host) std::memcpy(z_host, ctx->hs.dof_z.data(), ctx->hs.n * sizeof(double));
-    return LANDAU_OK;
+    if (!ctx || ctx->grids.size() != 1) return LANDAU_EINVAL;
+    return landau_grid_dof_coords(ctx, 0, r_host, z_host);
 }
 
 int landau_points(const landau_ctx *ctx, double *r_host, double *z_host, double *w_host) {
     if (!ctx) return LANDAU_EINVAL;
-    if (r_host) std::memcpy(r_host, ctx->hs.r.data(), ctx->hs.N * sizeof(double));
-    if (z_host) std::memcpy(z_host, ctx->hs.z.data(), ctx->hs.N * sizeof(double));
-    if (w_host) std::memcpy(w_host, ctx->hs.w_in.data(), ctx->hs.N * sizeof(double));
+    size_t off = 0;
+    for (const auto &G : ctx->grids) {   // union of the grids' points, grid by grid
+        const HostSpace &hs = G.hs;
+        if (r_host) std::memcpy(r_host + off, hs.r.data(), hs.N * sizeof(double));
+        if (z_host) std::memcpy(z_host + off, hs.z.data(), hs.N * sizeof(double));
+        if (w_host) std::memcpy(w_host + off, hs.w_in.data(), hs.N * sizeof(double));
+        off += size_t(hs.N);
+    }
     return LANDAU_OK;
 }
 
 int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *G_dev, void *stream) {
     if (!ctx || !f_dev || !G_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
-    cudaStream_t st = static_cast<cudaStream_t>(stream);
-    ctx->launches += launch_fields_beta(ctx->ds, nb, f_dev, ctx->sc.T, st);
-    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
-    ctx->launches += launch_sum_partials(ctx->ds, nb, pair_tiles(ctx->ds.N), ctx->sc.G, G_dev, st);
+    inner_integral(ctx, nb, f_dev, G_dev, static_cast<cudaStream_t>(stream));
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
@@ -254,13 +400,8 @@ int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *
 int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double *vals_dev, double *Cf_dev, void *stream) {
     if (!ctx || !f_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const DeviceSpace &ds = ctx->ds;
-    ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
-    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
-    ctx->launches += launch_sum_partials(ds, nb, pair_tiles(ds.N), ctx->sc.G, ctx->sc.Gsum, st);
-    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, nullptr, 0.0, st);
-    if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
-    if (Cf_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, Cf_dev, st);
+    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+    assemble(ctx, nb, f_dev, nullptr, 0.0, vals_dev, Cf_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
@@ -269,13 +410,8 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
                                      double *vals_dev, double *F_dev, void *stream) {
     if (!ctx || !f_dev || !Ez_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const DeviceSpace &ds = ctx->ds;
-    ctx->launches += launch_fields_beta(ds, nb, f_dev, ctx->sc.T, st);
-    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
-    ctx->launches += launch_sum_partials(ds, nb, pair_tiles(ds.N), ctx->sc.G, ctx->sc.Gsum, st);
-    ctx->launches += launch_element(ds, nb, 1, f_dev, ctx->sc.Gsum, ctx->sc.Ce, ctx->sc.ce, Ez_dev, shift, st);
-    if (vals_dev) ctx->launches += launch_gather_vals(ds, nb * ds.S, ctx->sc.Ce, vals_dev, st);
-    if (F_dev) ctx->launches += launch_gather_cf(ds, nb * ds.S, ctx->sc.ce, F_dev, st);
+    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+    assemble(ctx, nb, f_dev, Ez_dev, shift, vals_dev, F_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
@@ -287,25 +423,27 @@ int landau_jacobian(landau_ctx *ctx, const double *f_dev, double *vals_dev, doub
 int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream) {
     if (!ctx || !mvals_dev) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    ctx->launches += launch_mass_element(ctx->ds, shift, ctx->sc.Ce, st);
-    ctx->launches += launch_gather_vals(ctx->ds, 1, ctx->sc.Ce, mvals_dev, st);
+    for (auto &g : ctx->grids) {
+        ctx->launches += launch_mass_element(g.ds, shift, g.Ce, st);
+        ctx->launches += launch_gather_vals(g.ds, 1, 1, 0, g.Ce, mvals_dev + g.moff, st);
+    }
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
 
 int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *vals_host, double *Cf_host) {
     if (!ctx || !f_host || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
-    const DeviceSpace &ds = ctx->ds;
     if (!ctx->own_stream) {
         CK(cudaStreamCreateWithFlags(&ctx->own_stream, cudaStreamNonBlocking));
         CK(cudaStreamCreateWithFlags(&ctx->copy_stream, cudaStreamNonBlocking));
         CK(cudaEventCreateWithFlags(&ctx->chunk_done, cudaEventDisableTiming));
     }
+    const size_t fsz = ctx->fstride, vsz = ctx->vstride;
     if (ctx->host_nb < nb) {
         if (ctx->d_f) { cudaFree(ctx->d_f); cudaFree(ctx->d_vals); cudaFree(ctx->d_Cf); ctx->d_f = ctx->d_vals = ctx->d_Cf = nullptr; }
-        cudaError_t e = cudaMalloc((void **)&ctx->d_f, size_t(nb) * ds.S * ds.n * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_vals, size_t(nb) * ds.S * ds.nnz * sizeof(double));
-        if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_Cf, size_t(nb) * ds.S * ds.n * sizeof(double));
+        cudaError_t e = cudaMalloc((void **)&ctx->d_f, size_t(nb) * fsz * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_vals, size_t(nb) * vsz * sizeof(double));
+        if (e == cudaSuccess) e = cudaMalloc((void **)&ctx->d_Cf, size_t(nb) * fsz * sizeof(double));
         if (e != cudaSuccess) { ctx->host_nb = 0; return cuda_fail(e, "cudaMalloc(host staging)"); }
         ctx->host_nb = nb;
     }
@@ -313,9 +451,8 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
     // c+1 (the scratch arena is reused in stream order; problems are independent, so the values
     // are bitwise those of one batched call).
     cudaStream_t st = ctx->own_stream, cp = ctx->copy_stream;
-    const size_t fsz = size_t(ds.S) * ds.n, vsz = size_t(ds.S) * ds.nnz;
     CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
-    const int nchunks = nb >= 8 ? 4 : 1;
+    const int nchunks = nb >= 64 ? 8 : (nb >= 8 ? 4 : 1);
     const int cb = (nb + nchunks - 1) / nchunks;
     for (int b0 = 0; b0 < nb; b0 += cb) {
         const int nbc = std::min(cb, nb - b0);

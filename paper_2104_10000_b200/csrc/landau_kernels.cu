@@ -223,7 +223,7 @@ __device__ __forceinline__ void accumulate_i(PairAcc &acc, const JPoint &pj, con
 #ifndef PAIR_MIN_BLOCKS
 #define PAIR_MIN_BLOCKS 1
 #endif
-template <int TS, int IPT>
+template <int TS, int IPT, bool CHECK_ALL>
 __global__ void __launch_bounds__(TS / IPT, PAIR_MIN_BLOCKS)
 k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
            const double *__restrict__ T, double *__restrict__ Gpart) {
@@ -291,7 +291,7 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
                 const int t = sub * 32 + ((lane + k) & 31);
                 const JPoint pj = {sj[0][t], sj[1][t], sj[2][t], sj[3][t], sj[4][t], sj[5][t], sj[6][t]};
                 PairParts pp[IPT];
-                pair_parts<IPT, false>(pi, pj, pp);
+                pair_parts<IPT, CHECK_ALL>(pi, pj, pp);
 #pragma unroll
                 for (int u = 0; u < IPT; ++u) {
                     const PairTensor tt = pair_tensor(pi[u], pj, pp[u]);
@@ -353,7 +353,7 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
     const int q = threadIdx.x;
     const bool valid = e < ds.Ne;
     const int Nb = ds.Nb;
-    const double *fb = f + (size_t)b * ds.S * ds.n;
+    const double *fb = f + (size_t)b * ds.fstride;
     double tD = 0.0, tKr = 0.0, tKz = 0.0;
     double ijr = 0.0, ijz = 0.0;
     if (valid) { ijr = ds.invJ[2 * e]; ijz = ds.invJ[2 * e + 1]; }
@@ -383,8 +383,8 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
     if (valid) {
         const int gi = e * ds.Nq + q;
         const double w = ds.w_in[gi];
-        double *Tb = T + (size_t)b * 3 * ds.N;
-        Tb[gi] = w * tD; Tb[ds.N + gi] = w * tKr; Tb[2 * ds.N + gi] = w * tKz;
+        double *Tb = T + (size_t)b * 3 * ds.Ntot + ds.poff;
+        Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
     }
 }
 
@@ -409,14 +409,14 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
     __shared__ double s_B[256], s_E0[256], s_E1[256], s_X[256], s_Y[256], s_Ce[256], s_u[16];
     __shared__ double s_Z[FULL ? 256 : 1], s_ZM[FULL ? 256 : 1];
     const int e = blockIdx.x, b = blockIdx.y;
-    const int Nb = ds.Nb, Nq = ds.Nq, N = ds.N;
+    const int Nb = ds.Nb, Nq = ds.Nq, N = ds.Ntot;
     const int tid = threadIdx.x;
     s_B[tid] = ds.B[tid]; s_E0[tid] = ds.E0[tid]; s_E1[tid] = ds.E1[tid];
     if (tid < Nq) {
         const int gi = e * Nq + tid;
         double g[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
         for (int js = 0; js < jsplit; ++js) {
-            const double *G = Gpart + ((size_t)b * jsplit + js) * 5 * N;
+            const double *G = Gpart + ((size_t)b * jsplit + js) * 5 * N + ds.poff;
 #pragma unroll
             for (int c = 0; c < 5; ++c) g[c] += G[c * N + gi];
         }
@@ -434,7 +434,7 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
     for (int sp = 0; sp < ds.S; ++sp) {
         __syncthreads();                      // s_g / tabulations ready; previous species done with s_X, s_Y, s_Ce, s_u
         if (tid < Nb) {
-            const double *fa = f + ((size_t)b * ds.S + sp) * ds.n;
+            const double *fa = f + (size_t)b * ds.fstride + (size_t)sp * ds.n;
             double u = 0.0;
             for (int t = ds.lptr[e * Nb + tid]; t < ds.lptr[e * Nb + tid + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
             s_u[tid] = u;
@@ -481,16 +481,17 @@ __global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict_
     Ce[(size_t)e * Nb * Nb + tid] = shift * acc;
 }
 
-// a6 / a7: out[m][k] = sum_{t in [ptr[k], ptr[k+1])} w[t] * src[m*stride + idx[t]], fixed order
-// (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), nmat).
-__global__ void k_gather(int K, size_t stride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+// a6 / a7: out[b][sp][k] = sum_{t in [ptr[k], ptr[k+1])} w[t] * src[(b*S+sp)*stride + idx[t]], fixed order
+// (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), S, nb);
+// problem b's outputs start at out + b*ostride.
+__global__ void k_gather(int K, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
                          const double *__restrict__ w, const double *__restrict__ src, double *__restrict__ out) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= K) return;
-    const double *s = src + (size_t)blockIdx.y * stride;
+    const double *s = src + ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * stride;
     double acc = 0.0;
     for (int t = ptr[k]; t < ptr[k + 1]; ++t) acc = fma(w[t], s[idx[t]], acc);
-    out[(size_t)blockIdx.y * K + k] = acc;
+    out[(size_t)blockIdx.z * ostride + (size_t)blockIdx.y * K + k] = acc;
 }
 
 // Sums the j-split partials (used by landau_inner_integral when jsplit > 1).  grid over 5N x nb.
@@ -528,12 +529,20 @@ int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T
     return 1;
 }
 
-int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st) {
-    const int ts = pair_tile_size(ds.N), nt = pair_tiles(ds.N);
+template <bool CHECK_ALL>
+static void launch_pair_t(int N, const double *r, const double *z, const double *invr, int nb, const double *T, double *Gpart,
+                          cudaStream_t st) {
+    const int ts = pair_tile_size(N), nt = pair_tiles(N);
     dim3 grid(nt * (nt + 1) / 2, nb);
-    if (ts == 128) k_pair_sym<128, 2><<<grid, 64, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
-    else if (ts == 64) k_pair_sym<64, 2><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
-    else k_pair_sym<32, 1><<<grid, 32, 0, st>>>(ds.N, nt, ds.r, ds.z, ds.invr, T, Gpart);
+    if (ts == 128) k_pair_sym<128, 2, CHECK_ALL><<<grid, 64, 0, st>>>(N, nt, r, z, invr, T, Gpart);
+    else if (ts == 64) k_pair_sym<64, 2, CHECK_ALL><<<grid, 32, 0, st>>>(N, nt, r, z, invr, T, Gpart);
+    else k_pair_sym<32, 1, CHECK_ALL><<<grid, 32, 0, st>>>(N, nt, r, z, invr, T, Gpart);
+}
+
+int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
+                double *Gpart, cudaStream_t st) {
+    if (check_all) launch_pair_t<true>(Ntot, r, z, invr, nb, T, Gpart, st);
+    else launch_pair_t<false>(Ntot, r, z, invr, nb, T, Gpart, st);
     return 1;
 }
 
@@ -545,15 +554,15 @@ int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, c
     return 1;
 }
 
-int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st) {
-    dim3 grid((ds.nnz + 255) / 256, nmat);
-    k_gather<<<grid, 256, 0, st>>>(ds.nnz, (size_t)ds.Ne * ds.Nb * ds.Nb, ds.gptr, ds.gidx, ds.gw, Ce, vals);
+int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st) {
+    dim3 grid((ds.nnz + 255) / 256, nspecies, nb);
+    k_gather<<<grid, 256, 0, st>>>(ds.nnz, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
     return 1;
 }
 
-int launch_gather_cf(const DeviceSpace &ds, int nvec, const double *ce, double *Cf, cudaStream_t st) {
-    dim3 grid((ds.n + 255) / 256, nvec);
-    k_gather<<<grid, 256, 0, st>>>(ds.n, (size_t)ds.Ne * ds.Nb, ds.cptr, ds.cidx, ds.cw, ce, Cf);
+int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st) {
+    dim3 grid((ds.n + 255) / 256, ds.S, nb);
+    k_gather<<<grid, 256, 0, st>>>(ds.n, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
     return 1;
 }
 
@@ -562,8 +571,8 @@ int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStr
     return 1;
 }
 
-int launch_sum_partials(const DeviceSpace &ds, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
-    const int n5 = 5 * ds.N;
+int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
+    const int n5 = 5 * Ntot;
     dim3 grid((n5 + 255) / 256, nb);
     k_sum_partials<<<grid, 256, 0, st>>>(n5, jsplit, Gpart, G);
     return 1;

@@ -11,8 +11,13 @@ constexpr int MAX_SPECIES = 16;
 // Device-resident description of one mesh/order/species set (all pointers device memory,
 // shared by every problem of a batch).
 struct DeviceSpace {
-    int p, Nq, Nb, S;
+    int p, Nq, Nb, S;                            // S = species living on this grid
     int N, Ne, n, nnz;
+    // several grids (section III-C): the point-indexed scratch arrays T, G cover the union of
+    // all grids' points (Ntot), this grid's points start at poff; f of problem b starts at f + b*fstride
+    // (f already offset to this grid's first species)
+    int Ntot, poff;
+    long long fstride;
     const double *r, *z, *invr, *w_in, *w_out;  // [N]
     const double *invJ;                          // [Ne][2]
     const double *B, *E0, *E1;                   // [Nq][Nb]
@@ -27,25 +32,28 @@ struct DeviceSpace {
     double qm[MAX_SPECIES];    // e_a m0/m_a (E-field advection, Eq. 4)
 };
 
-// Scratch for up to max_batch problems.
+// Scratch for up to max_batch problems (N = points of all grids together).
 struct Scratch {
     double *T;      // [nb][3][N]
     double *G;      // [nb][ntiles][5][N]: per source tile partial sums of G_D, G_K
     double *Gsum;   // [nb][5][N]: G_D (rr,rz,zz), G_K (r,z) after the tile-order sum
-    double *Ce;     // [nb][S][Ne][Nb*Nb]
-    double *ce;     // [nb][S][Ne][Nb]
 };
 
 // each returns the number of kernels launched
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
-int launch_pair(const DeviceSpace &ds, int nb, const double *T, double *Gpart, cudaStream_t st);
+// pair kernel over the union of points (r, z, invr: [Ntot]); check_all: test every pair for coincidence
+// (needed only when points of different grids coincide), else only the diagonal tiles
+int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
+                double *Gpart, cudaStream_t st);
 // Ez == nullptr: collision Jacobian C_e; else the implicit-step operator shift M + A_E - J (Ez[nb] device)
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce,
                    double *ce, const double *Ez, double shift, cudaStream_t st);
-int launch_gather_vals(const DeviceSpace &ds, int nmat, const double *Ce, double *vals, cudaStream_t st);
-int launch_gather_cf(const DeviceSpace &ds, int nvec, const double *ce, double *Cf, cudaStream_t st);
+// vals / Cf already offset to this grid's first species; ostride = doubles per problem in the output;
+// nspecies = 1 with ostride 0 gathers a single matrix (mass)
+int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st);
+int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st);
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
-int launch_sum_partials(const DeviceSpace &ds, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
+int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
 
 int pair_tile_size(int N);

@@ -160,6 +160,36 @@ def mesh_refine_uniform(m: Mesh) -> Mesh:
                 np.array(iz, np.int32))
 
 
+def mesh_scaled(m: Mesh, k: float) -> Mesh:
+    """The same leaves on a domain scaled by k (a grid for a species cluster with thermal speed k)."""
+    return Mesh(m.rmin * k, m.rmax * k, m.zmin * k, m.zmax * k, m.nbr, m.nbz, m.level, m.ir, m.iz)
+
+
+def multigrid_case(which: str = "paper3"):
+    """Multiple-grid workloads (section III-C, Table I).  Returns
+    (name, order, meshes, species, species_grid, components) with one Component per species.
+      'paper3': ten species on three 20-cell Q3 grids (the 20-cell / 193-vertex grid of Fig. 3, domain
+                5 v_th of its cluster): e | D+ | eight heavy-ion charge states -- 960 points, 1,930 equations;
+      'same2' : two species on two IDENTICAL refined Q2 grids (every point coincides with one of the other grid);
+      'scaled': three species on two refined Q2 grids of different extent."""
+    g20 = mesh_quadtree(0.0, 5.0, -5.0, 5.0, 2, 4, 1.0, 2, 2.5, 1)
+    if which == "paper3":
+        mw = 184.0 * 1836.0
+        rows = [(1.0, -1.0, 1.0, 1.0), (3670.0, 1.0, 0.64, 1.0)] + [(mw, float(q), 0.01, 1.0) for q in range(1, 9)]
+        sp = _sp(rows)
+        meshes = [g20, mesh_scaled(g20, 1.0 / math.sqrt(3670.0)), mesh_scaled(g20, 1.0 / math.sqrt(mw))]
+        grid = [0, 1] + [2] * 8
+        return "mg-paper3-10sp-q3", 3, meshes, sp, grid, [Component(s, rows[s][2], 1.0) for s in range(10)]
+    g = mesh_quadtree(0.0, 4.0, -4.0, 4.0, 2, 4, 1.0, 2, 2.0, 1)
+    if which == "same2":
+        sp = _sp([(1, -1, 1, 1), (4, 1, 1, 1)])
+        return "mg-same2-q2", 2, [g, g], sp, [0, 1], [Component(0, 1, 1), Component(1, 1, 1)]
+    if which == "scaled":
+        sp = _sp([(1, -1, 1, 1), (64, 1, 0.6, 1), (128, 2, 0.2, 1)])
+        return "mg-scaled-q2", 2, [g, mesh_scaled(g, 0.125)], sp, [0, 1, 1], [Component(0, 1, 1), Component(1, 0.6, 1, 0.02), Component(2, 0.2, 1, 0.04)]
+    raise ValueError(which)
+
+
 @dataclass
 class Species:
     """The ``landau_species`` struct: masses in m_e, charges in e, nu = 1, m0 = m_e (Appendix A)."""

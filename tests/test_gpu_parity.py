@@ -132,6 +132,51 @@ def test_implicit_operator_parity(gpu, oracle, cfg, variant):
     assert torch.equal(v0, -vj) and torch.equal(F0, -cj)
 
 
+@pytest.mark.parametrize("which", ["same2", "scaled", "paper3"])
+def test_multigrid_parity(gpu, oracle, which):
+    """SURVEY 8(f) NEXT-2 (section III-C): species on several grids, pair loop over the union of
+    points.  'same2' has every point of grid 1 on top of one of grid 0 (coincident pairs skipped across
+    grids); 'paper3' is Table I's three 20-cell grids with ten species (960 points, 1,930 equations)."""
+    import torch
+    name, order, meshes, spc, sgrid, comps = inputs.multigrid_case(which)
+    ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, 2)
+    if which == "paper3":
+        assert ctx.N == 960 and ctx.f_stride == 1930
+    fl = []
+    for a, c in enumerate(comps):
+        r, z = ctx.grid_dof_coords(sgrid[a])
+        fa = inputs.maxwellian(float(spc.mass[a]), c.n, c.T, c.zs, r, z)
+        fl.append(fa * (1.0 + 1e-3 * np.cos(7.0 * np.arange(r.shape[0]) + a)))
+    f = np.concatenate(fl)
+    fb = np.stack([f, 0.5 * f])
+    vals = torch.full((2, ctx.vals_stride), float("nan"), dtype=torch.float64, device="cuda")
+    Cf = torch.full((2, ctx.f_stride), float("nan"), dtype=torch.float64, device="cuda")
+    mv = torch.full((ctx.mvals_size,), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.jacobian_batched(torch.from_numpy(fb).cuda(), vals, Cf)
+    ctx.mass(1.7, mv)
+    vals, Cf, mv = vals.cpu().numpy(), Cf.cpu().numpy(), mv.cpu().numpy()
+    spaces, ov, oC, om = oracle.build_all_multigrid(meshes, order, spc, sgrid, fl, 1.7)
+    for g, sp_ in enumerate(spaces):
+        rowptr, colidx = ctx.grid_csr_pattern_host(g)
+        assert np.array_equal(rowptr, sp_.rowptr) and np.array_equal(colidx, sp_.colidx)
+    assert block_err(mv, np.concatenate(om)) <= 1e-13
+    fs, vs = ctx.species_slices(), ctx.vals_slices()
+    for a in range(ctx.S):
+        assert block_err(vals[0, vs[a]], ov[a]) <= TOL, (which, a)
+        assert block_err(Cf[0, fs[a]], oC[a]) <= TOL, (which, a)
+        # the operator is quadratic in f: problem 1 (f/2) is a quarter of problem 0 (exact in binary)
+        assert np.array_equal(Cf[1, fs[a]], 0.25 * Cf[0, fs[a]]) and np.array_equal(vals[1, vs[a]], 0.5 * vals[0, vs[a]])
+    # conservation across grids: density per species, total z-momentum and energy
+    psi_z = [spaces[sgrid[a]].dof_z for a in range(ctx.S)]
+    psi_e = [0.5 * (spaces[sgrid[a]].dof_r ** 2 + spaces[sgrid[a]].dof_z ** 2) for a in range(ctx.S)]
+    for a in range(ctx.S):
+        assert abs(Cf[0, fs[a]].sum()) <= 1e-12 * np.abs(Cf[0, fs[a]]).sum()
+    for psi in (psi_z, psi_e):
+        num = abs(sum(spc.mass[a] * (psi[a] @ Cf[0, fs[a]]) for a in range(ctx.S)))
+        den = sum(spc.mass[a] * np.abs(psi[a] * Cf[0, fs[a]]).sum() for a in range(ctx.S))
+        assert num <= 1e-12 * den
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch
