@@ -345,46 +345,58 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
 // Output T[b][3][N] = w_in * (T_D, T_Kr, T_Kz): the weight of the inner sum is folded in here.
 // ------------------------------------------------------------------------------------------------
 constexpr int FIELD_EPB = 8;
+constexpr int FIELD_ROUNDS = 4;   // cells per thread: the tabulation rows stay in registers across them
 
 __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, double *__restrict__ T) {
     __shared__ double s_u[FIELD_EPB][16];
     const int b = blockIdx.y;
-    const int e = blockIdx.x * FIELD_EPB + threadIdx.y;
     const int q = threadIdx.x;
-    const bool valid = e < ds.Ne;
     const int Nb = ds.Nb;
     const double *fb = f + (size_t)b * ds.fstride;
-    double tD = 0.0, tKr = 0.0, tKz = 0.0;
-    double ijr = 0.0, ijz = 0.0;
-    if (valid) { ijr = ds.invJ[2 * e]; ijz = ds.invJ[2 * e + 1]; }
-    for (int sp = 0; sp < ds.S; ++sp) {
-        if (valid) {
-            double u = 0.0;
-            const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
-            for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
-            s_u[threadIdx.y][q] = u;
-        }
-        __syncthreads();
-        if (valid) {
-            double fq = 0.0, g0 = 0.0, g1 = 0.0;
-            for (int a = 0; a < Nb; ++a) {
-                const double u = s_u[threadIdx.y][a];
-                fq = fma(ds.B[q * Nb + a], u, fq);
-                g0 = fma(ds.E0[q * Nb + a], u, g0);
-                g1 = fma(ds.E1[q * Nb + a], u, g1);
-            }
-            const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
-            tD = fma(e2, fq, tD);
-            tKr = fma(em, ijr * g0, tKr);
-            tKz = fma(em, ijz * g1, tKz);
-        }
-        __syncthreads();
+    double *Tb = T + (size_t)b * 3 * ds.Ntot + ds.poff;
+    double tB[16], tE0[16], tE1[16];      // row q of the tabulations
+#pragma unroll
+    for (int a = 0; a < 16; ++a) {
+        const bool in = a < Nb;
+        tB[a] = in ? ds.B[q * Nb + a] : 0.0; tE0[a] = in ? ds.E0[q * Nb + a] : 0.0; tE1[a] = in ? ds.E1[q * Nb + a] : 0.0;
     }
-    if (valid) {
-        const int gi = e * ds.Nq + q;
-        const double w = ds.w_in[gi];
-        double *Tb = T + (size_t)b * 3 * ds.Ntot + ds.poff;
-        Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
+    for (int round = 0; round < FIELD_ROUNDS; ++round) {
+        const int e = (blockIdx.x * FIELD_ROUNDS + round) * FIELD_EPB + threadIdx.y;
+        const bool valid = e < ds.Ne;
+        double tD = 0.0, tKr = 0.0, tKz = 0.0;
+        double ijr = 0.0, ijz = 0.0;
+        if (valid) { ijr = ds.invJ[2 * e]; ijz = ds.invJ[2 * e + 1]; }
+        for (int sp = 0; sp < ds.S; ++sp) {
+            if (valid) {
+                double u = 0.0;
+                const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
+                for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
+                s_u[threadIdx.y][q] = u;
+            }
+            __syncthreads();
+            if (valid) {
+                double fq = 0.0, g0 = 0.0, g1 = 0.0;
+#pragma unroll
+                for (int a = 0; a < 16; ++a) {
+                    if (a < Nb) {
+                        const double u = s_u[threadIdx.y][a];
+                        fq = fma(tB[a], u, fq);
+                        g0 = fma(tE0[a], u, g0);
+                        g1 = fma(tE1[a], u, g1);
+                    }
+                }
+                const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
+                tD = fma(e2, fq, tD);
+                tKr = fma(em, ijr * g0, tKr);
+                tKz = fma(em, ijz * g1, tKz);
+            }
+            __syncthreads();
+        }
+        if (valid) {
+            const int gi = e * ds.Nq + q;
+            const double w = ds.w_in[gi];
+            Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
+        }
     }
 }
 
@@ -472,6 +484,120 @@ __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// a4 + a5 for Q3 (Nb = Nq = 16) on the FP64 tensor cores.  Line 23's contraction
+//   C_e[a][b] = sum_q ( E0_qa X_qb + E1_qa Y_qb [+ B_qa Z_qb] )
+// is a 16 x 16 x 32 (48, 64 with FULL) matrix product per (cell, species):
+// mma.sync.m8n8k4.f64, A = tabulations (row-major, a x q), B = X / Y / Z (col-major, q x b).
+// One WARP per (cell, problem), looping over the species.  In the m8n8k4 layouts lane (g = lane/4,
+// k = lane%4) holds A[g][k] and B[k][g]: with q = 4 ks + k both are the tabulation entry
+// (q, 8 t + g), t = 0, 1 -- so each lane keeps 8 entries of B, E0, E1 in registers for the whole
+// kernel, builds its X, Y entries there and nothing but G, f and the outputs touches memory.
+// Replaces the shared-memory version (k_element) for Q3: 1.49 -> see DESIGN.md 6.2.
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+constexpr int ELQ3_WARPS = 4;   // cells per block
+
+template <bool FULL>
+__global__ void __launch_bounds__(ELQ3_WARPS * 32)
+k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
+             double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
+    const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+    const int e = blockIdx.x * ELQ3_WARPS + warp, b = blockIdx.y;
+    if (e >= ds.Ne) return;
+    const int k = lane & 3, g = lane >> 2;
+    // tabulation entries (q = 4 ks + k, col = 8 t + g)
+    double tB[4][2], tE0[4][2], tE1[4][2];
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks)
+#pragma unroll
+        for (int t = 0; t < 2; ++t) {
+            const int o = (4 * ks + k) * 16 + 8 * t + g;
+            tB[ks][t] = ds.B[o]; tE0[ks][t] = ds.E0[o]; tE1[ks][t] = ds.E1[o];
+        }
+    // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
+    const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1];
+    const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
+    double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
+#pragma unroll
+    for (int ks = 0; ks < 4; ++ks) {
+        const int q = 4 * ks + k;
+        const double w = ds.w_out[e * 16 + q];
+        wq[ks] = w;
+        g0[ks] = ir * ir * w * G[q];
+        g1[ks] = ir * iz * w * G[ds.Ntot + q];
+        g2[ks] = iz * iz * w * G[2 * ds.Ntot + q];
+        g3[ks] = ir * w * G[3 * ds.Ntot + q];
+        g4[ks] = iz * w * G[4 * ds.Ntot + q];
+    }
+    const double sgn = FULL ? -1.0 : 1.0;
+    const double ezb = FULL ? Ez[b] : 0.0;
+    for (int sp = 0; sp < ds.S; ++sp) {
+        // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in)
+        double u = 0.0;
+        if (lane < 16) {
+            const double *fa = f + (size_t)b * ds.fstride + (size_t)sp * ds.n;
+            for (int t = ds.lptr[e * 16 + lane]; t < ds.lptr[e * 16 + lane + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
+        }
+        const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
+        double acc[2][2][2] = {};       // [mt][nt][2]
+        double accM[2][2][2] = {};      // mass part (FULL), kept apart: the element vector excludes it
+#pragma unroll
+        for (int ks = 0; ks < 4; ++ks) {
+            const double drr = df * g0[ks], drz = df * g1[ks], dzz = df * g2[ks], kr = kf * g3[ks], kz = kf * g4[ks];
+            double X[2], Y[2];
+#pragma unroll
+            for (int t = 0; t < 2; ++t) {
+                X[t] = fma(drr, tE0[ks][t], fma(drz, tE1[ks][t], kr * tB[ks][t]));
+                Y[t] = fma(drz, tE0[ks][t], fma(dzz, tE1[ks][t], kz * tB[ks][t]));
+            }
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) {
+                    dmma884(acc[mt][nt], tE0[ks][mt], X[nt]);
+                    dmma884(acc[mt][nt], tE1[ks][mt], Y[nt]);
+                }
+            if (FULL) {
+                const double ca = wq[ks] * (ds.qm[sp] * ezb) * iz, cm = wq[ks] * shift;
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                    for (int nt = 0; nt < 2; ++nt) {
+                        dmma884(acc[mt][nt], tB[ks][mt], ca * tE1[ks][nt]);
+                        dmma884(accM[mt][nt], tB[ks][mt], cm * tB[ks][nt]);
+                    }
+            }
+        }
+        // C fragment: lane holds rows a = 8 mt + g, columns b = 8 nt + 2 k + {0, 1}
+        const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
+        double *C = Ce + mat * 256;
+        double part[2] = {0.0, 0.0};
+#pragma unroll
+        for (int nt = 0; nt < 2; ++nt) {
+            const double u0 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k), u1 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k + 1);
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt) {
+                part[mt] = fma(acc[mt][nt][0], u0, fma(acc[mt][nt][1], u1, part[mt]));
+                double2 v;
+                v.x = FULL ? acc[mt][nt][0] + accM[mt][nt][0] : acc[mt][nt][0];
+                v.y = FULL ? acc[mt][nt][1] + accM[mt][nt][1] : acc[mt][nt][1];
+                *reinterpret_cast<double2 *>(C + (8 * mt + g) * 16 + 8 * nt + 2 * k) = v;
+            }
+        }
+#pragma unroll
+        for (int mt = 0; mt < 2; ++mt) {
+            part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 1);
+            part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 2);
+            if (k == 0) ce[mat * 16 + 8 * mt + g] = part[mt];
+        }
+    }
+}
+
 // a8: element mass matrices, M_e[a][b] = shift sum_q w_out B_qa B_qb (L280).  grid = Ne.
 __global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict__ Ce) {
     const int e = blockIdx.x, Nb = ds.Nb, tid = threadIdx.x;
@@ -524,7 +650,8 @@ int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 1024 ? 64 : 32); }
 int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / ts; }
 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
-    dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
+    constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
+    dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
     k_fields_beta<<<grid, block, 0, st>>>(ds, f, T);
     return 1;
 }
@@ -548,6 +675,12 @@ int launch_pair(int Ntot, const double *r, const double *z, const double *invr, 
 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    const double *Ez, double shift, cudaStream_t st) {
+    if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
+        dim3 grid((ds.Ne + ELQ3_WARPS - 1) / ELQ3_WARPS, nb);
+        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, Ez, shift);
+        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, nullptr, 0.0);
+        return 1;
+    }
     dim3 grid(ds.Ne, nb);
     if (Ez) k_element<true><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
     else k_element<false><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
