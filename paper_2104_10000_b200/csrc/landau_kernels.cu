@@ -646,7 +646,9 @@ __global__ void k_dfma_probe(int iters, double *out) {
 // launchers
 // ------------------------------------------------------------------------------------------------
 // Tile size of the pair kernel: a function of N ONLY (it fixes the summation order).
-int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 1024 ? 64 : 32); }
+// Small N is latency-bound (one warp walks its j tile step by step, ~700 cycles per step): short tiles give
+// more warps and fewer steps (N = 2048: 39 -> 31 us); large N is throughput-bound: two i per thread.
+int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 2560 ? 64 : 32); }
 int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / ts; }
 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
