@@ -44,6 +44,8 @@ FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 
 # ncu --set full capture summarised in profiles/r01c_pair_kernel.md (73.9 MB read + 3.880 GB written:
 # the per-source-tile partial slabs; the algorithmic minimum is 24 B/point in + 40 B/point out = 0.16 GB).
 PAIR_KERNEL_DRAM_BYTES = 73.9e6 + 3.8797e9
+# the same for the rest of the step (fields, slab sum, element matrices, two gathers), profiles/r01d_step_kernels.md (ncu --set full, dram read + write)
+REST_DRAM_BYTES = 6.03e9   # 4.04 GB of it is k_sum_partials reading the slabs
 
 
 class ClockSampler(threading.Thread):
@@ -165,6 +167,44 @@ def time_single_config(binding, inputs, torch, k, variant="B", reps=20):
     return out
 
 
+def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
+    """SURVEY 8(f) rows at the same measurement bar: NEXT-3 (implicit-step operator, config 5) and NEXT-2
+    (the paper's three 20-cell grids with ten species, Table I, 512 problems batched)."""
+    out = {}
+    Ez = torch.full((nb,), 0.3, dtype=torch.float64, device="cuda")
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    ctx5.implicit_operator_batched(f5, Ez, 2.0, vals5, Cf5)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(3):
+        ctx5.implicit_operator_batched(f5, Ez, 2.0, vals5, Cf5)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 3
+    out["implicit_operator_config5"] = {"ms_per_step": ms, "gpair_per_s": nb * ctx5.N * (ctx5.N - 1) / (ms * 1e-3) * 1e-9,
+                                        "what": "shift M + A(E_z) - J and A f - C(f) in one pass (landau_implicit_operator_batched)"}
+    name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("paper3")
+    mg = binding.LandauMultigridContext(meshes, sgrid, order, spc, nb)
+    fl = []
+    for a, c in enumerate(comps):
+        r, z = mg.grid_dof_coords(sgrid[a])
+        fl.append(inputs.maxwellian(float(spc.mass[a]), c.n, c.T, c.zs, r, z))
+    f = torch.from_numpy(np.tile(np.concatenate(fl), (nb, 1))).cuda()
+    v = torch.zeros((nb, mg.vals_stride), dtype=torch.float64, device="cuda")
+    c_ = torch.zeros((nb, mg.f_stride), dtype=torch.float64, device="cuda")
+    mg.jacobian_batched(f, v, c_)
+    torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        mg.jacobian_batched(f, v, c_)
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 5
+    out["multigrid_paper3"] = {"workload": f"{nb} problems x (10 species on 3 grids of 20 Q3 cells: N = {mg.N}, n = {mg.f_stride})",
+                               "ms_per_step": ms, "builds_per_s": nb / (ms * 1e-3),
+                               "gpair_per_s": nb * mg.N * (mg.N - 1) / (ms * 1e-3) * 1e-9}
+    mg.destroy()
+    return out
+
+
 def run_ours(args):
     import torch
     from paper_2104_10000_b200 import binding, inputs
@@ -271,6 +311,23 @@ def run_ours(args):
         detail = [time_single_config(binding, inputs, torch, k) for k in (1, 2, 3, 4)]
         detail.append(time_single_config(binding, inputs, torch, 3, variant="A"))
         detail += [time_single_config(binding, inputs, torch, k) for k in (6, 7)]   # paper-shaped S = 10 context runs
+        next_rows = time_next_rows(binding, inputs, torch, ctx, f, vals, Cf, nb)
+        # everything but the pair kernel (a1, a2, a4-a7): HBM-bound; algorithmic bytes = f in, vals and C(f) out,
+        # G_D/G_K (5 doubles per point) between the two halves of the path
+        rest_ms = (total_ms - pair_ms) / args.steps if world == 1 else None
+        rest_bytes = nb * (ctx.S * 8 * (2 * ctx.n + ctx.nnz) + 40 * ctx.N)
+        hbm_peak = None
+        try:
+            hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
+            hbm_src = "MEASURED_PEAKS.json hbm_gbs"
+        except Exception:
+            hbm_peak, hbm_src = 6460.0, "fallback (B200_PROFILING.md measured copy bandwidth)"
+        roof_rest = None
+        if rest_ms:
+            ach = rest_bytes / (rest_ms * 1e-3) * 1e-9
+            roof_rest = {"bound": "hbm", "kernels": "k_fields_beta + k_sum_partials + k_element_q3 + k_gather x2", "achieved": ach,
+                         "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": hbm_src,
+                         "ms_per_step": rest_ms, "algorithmic_bytes_per_step": rest_bytes, "traffic": REST_DRAM_BYTES}
         h2d = nb * ctx.S * ctx.n * 8
         d2h = nb * ctx.S * (ctx.nnz + ctx.n) * 8
         print(json.dumps({
@@ -287,7 +344,9 @@ def run_ours(args):
             "roofline": roof,
             "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
                              "sample": f"{CPU_SAMPLE_PROBLEMS} of the 512 problems (N=4928, a1-a8), double-precision oracle, OpenMP over i, {cpu_dt:.2f} s wall"},
+            "roofline_rest": roof_rest,
             "per_config": detail,
+            "next_rows": next_rows,
         }))
     ctx.destroy()
     if dist is not None:

@@ -500,15 +500,17 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
-constexpr int ELQ3_WARPS = 4;   // cells per block
+constexpr int ELQ3_WARPS = 4;    // cells per block and round
+#ifndef ELQ3_ROUNDS
+#define ELQ3_ROUNDS 1              // cells per warp (1, 4, 8 measured alike: 0.41-0.42 ms)
+#endif
 
 template <bool FULL>
 __global__ void __launch_bounds__(ELQ3_WARPS * 32)
 k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
              double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
-    const int e = blockIdx.x * ELQ3_WARPS + warp, b = blockIdx.y;
-    if (e >= ds.Ne) return;
+    const int b = blockIdx.y;
     const int k = lane & 3, g = lane >> 2;
     // tabulation entries (q = 4 ks + k, col = 8 t + g)
     double tB[4][2], tE0[4][2], tE1[4][2];
@@ -519,6 +521,11 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
             const int o = (4 * ks + k) * 16 + 8 * t + g;
             tB[ks][t] = ds.B[o]; tE0[ks][t] = ds.E0[o]; tE1[ks][t] = ds.E1[o];
         }
+    const double sgn = FULL ? -1.0 : 1.0;
+    const double ezb = FULL ? Ez[b] : 0.0;
+    for (int round = 0; round < ELQ3_ROUNDS; ++round) {
+    const int e = (blockIdx.x * ELQ3_ROUNDS + round) * ELQ3_WARPS + warp;
+    if (e >= ds.Ne) return;
     // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
     const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1];
     const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
@@ -534,8 +541,6 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
         g3[ks] = ir * w * G[3 * ds.Ntot + q];
         g4[ks] = iz * w * G[4 * ds.Ntot + q];
     }
-    const double sgn = FULL ? -1.0 : 1.0;
-    const double ezb = FULL ? Ez[b] : 0.0;
     for (int sp = 0; sp < ds.S; ++sp) {
         // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in)
         double u = 0.0;
@@ -596,6 +601,7 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
             if (k == 0) ce[mat * 16 + 8 * mt + g] = part[mt];
         }
     }
+    }   // round
 }
 
 // a8: element mass matrices, M_e[a][b] = shift sum_q w_out B_qa B_qb (L280).  grid = Ne.
@@ -678,7 +684,7 @@ int launch_pair(int Ntot, const double *r, const double *z, const double *invr, 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    const double *Ez, double shift, cudaStream_t st) {
     if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
-        dim3 grid((ds.Ne + ELQ3_WARPS - 1) / ELQ3_WARPS, nb);
+        dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
         if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, Ez, shift);
         else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, nullptr, 0.0);
         return 1;
