@@ -16,7 +16,8 @@ What it computes (PAPER.md = /root/reference/PAPER.md, arxiv 2104.10000):
 * the scaled mass matrix (L280);
 * the E-field advection term on the left of Eq. 4 (L52) and the operator of a fully implicit step,
   shift M + A_a - J_a with its residual A_a f_a - C_a(f) (SURVEY 8(f) NEXT-3);
-* the same operator with species clustered on several grids (section III-C, Table I; NEXT-2).
+* the same operator with species clustered on several grids (section III-C, Table I; NEXT-2);
+* the per-species linear solve of the implicit step (section III-G; NEXT-4).
 
 Everything outside the O(N^2) pair loop is plain numpy in fp64 with dense matrices (no
 blocking, no gather lists).  The pair loop is plain C in long double (``_ld``) for parity and
@@ -530,3 +531,39 @@ def build_all_multigrid(meshes, order: int, species, species_grid, f_list, shift
             Cf[sp.cell_dofs[e]] += sp.cell_P[e].T @ ce
         Cf_list.append(Cf)
     return spaces, vals_list, Cf_list, [mass(sp, shift) for sp in spaces]
+
+
+# --------------------------------------------------------------------------------------------
+# Linear solve of the implicit step (section III-G).
+# The paper's band solver is Gaussian elimination WITHOUT pivoting in outer-product form
+# (Golub & Van Loan Alg. 4.3.1) on the RCM-ordered matrix, one independent solve per species.
+# The result it reaches has a plain definition -- x with A x = b -- so the oracle is that
+# definition through a library routine (LAPACK, partial pivoting); the ordering is internal to
+# the device path and does not appear here.  band_lu_outer_product() restates Alg. 4.3.1 itself
+# on a dense array for the pins (L U = A, no fill outside the band).
+# --------------------------------------------------------------------------------------------
+
+def dense_from_csr(sp: Space, vals_one: np.ndarray) -> np.ndarray:
+    rows = np.repeat(np.arange(sp.n), np.diff(sp.rowptr))
+    A = np.zeros((sp.n, sp.n))
+    A[rows, sp.colidx] = vals_one
+    return A
+
+
+def solve_species(sp: Space, vals_one: np.ndarray, rhs_one: np.ndarray) -> np.ndarray:
+    """x = A^-1 b for one species block given its CSR values on the pattern A1."""
+    return np.linalg.solve(dense_from_csr(sp, vals_one), rhs_one)
+
+
+def band_lu_outer_product(A: np.ndarray, p: int, q: int) -> np.ndarray:
+    """Golub & Van Loan Alg. 4.3.1 (L173): for k = 1..n-1: A(k+1:k+p, k) /= A(k,k);
+    A(k+1:k+p, k+1:k+q) -= A(k+1:k+p, k) A(k, k+1:k+q).  Lower bandwidth p, upper q, no pivoting.
+    Returns the factors in one array (unit lower L below the diagonal, U on and above)."""
+    A = np.array(A, dtype=np.float64)
+    n = A.shape[0]
+    for k in range(n - 1):
+        i1 = min(k + p, n - 1)
+        j1 = min(k + q, n - 1)
+        A[k + 1:i1 + 1, k] /= A[k, k]
+        A[k + 1:i1 + 1, k + 1:j1 + 1] -= np.outer(A[k + 1:i1 + 1, k], A[k, k + 1:j1 + 1])
+    return A

@@ -245,3 +245,36 @@ def test_multigrid_equals_single_grid_on_identical_meshes_and_conserves(oracle):
         den = sum(spc.mass[a] * np.abs(psi(spaces[grids[a]]) * C[a]).sum() for a in range(3))
         assert num <= 1e-12 * den
     assert abs(spaces[0].dof_z @ C[0]) > 1e-6 * np.abs(spaces[0].dof_z * C[0]).sum()   # the pin bites
+
+
+def test_linear_solve_pins(built, oracle):
+    """Section III-G (L169-175): per-species solve of the implicit step.  Pins: M x = M 1 gives x = 1;
+    the outer-product band LU (Alg. 4.3.1) reproduces A = L U with no fill outside the band and its
+    triangular solves agree with the library solve and with scipy's banded solver; a manufactured solution."""
+    import scipy.linalg
+    wl, sp, f, vals, Cf, mv = built["q2"]
+    ov, F = oracle.implicit_operator(sp, wl.species, f, 0.2, 3.0)
+    M = oracle.dense_from_csr(sp, oracle.mass(sp, 1.0))
+    assert np.abs(oracle.solve_species(sp, oracle.mass(sp, 1.0), M @ np.ones(sp.n)) - 1.0).max() < 1e-12
+    for a in range(wl.species.S):
+        A = oracle.dense_from_csr(sp, ov[a])
+        rows, cols = np.nonzero(A)
+        p = int((rows - cols).max()); q = int((cols - rows).max())
+        LU = oracle.band_lu_outer_product(A, p, q)
+        L = np.tril(LU, -1) + np.eye(sp.n); U = np.triu(LU)
+        assert np.abs(L @ U - A).max() <= 1e-13 * np.abs(A).max()
+        ii, jj = np.nonzero(LU)
+        assert (ii - jj).max() <= p and (jj - ii).max() <= q                # no fill outside the band
+        xs = np.cos(np.arange(sp.n) * 0.37) + 2.0                            # manufactured solution
+        b = A @ xs
+        x = oracle.solve_species(sp, ov[a], b)
+        cond = np.linalg.cond(A)
+        assert np.abs(x - xs).max() <= 50 * cond * 2.2e-16 * np.abs(xs).max()
+        y = scipy.linalg.solve_triangular(L, b, lower=True, unit_diagonal=True)
+        x2 = scipy.linalg.solve_triangular(U, y)
+        assert np.abs(x2 - x).max() <= 50 * cond * 2.2e-16 * np.abs(x).max()
+        ab = np.zeros((p + q + 1, sp.n))
+        for i, j in zip(rows, cols):
+            ab[q + i - j, j] = A[i, j]
+        x3 = scipy.linalg.solve_banded((p, q), ab, b)
+        assert np.abs(x3 - x).max() <= 50 * cond * 2.2e-16 * np.abs(x).max()
