@@ -57,6 +57,9 @@ SIGNATURES = {
     "landau_jacobian_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
     "landau_implicit_operator_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
+    "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64)]),
+    "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
+    "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "landau_profile_enable": (c_int, [c_void_p, c_int]),
@@ -223,6 +226,22 @@ class LandauContext:
         _check(lib().landau_implicit_operator_batched(self._h, nb, self._ptr(f, (nb, self.S, self.n)), self._ptr(Ez, (nb,)),
                                                       float(shift), pv, pf, _stream_ptr(stream)))
 
+    def band_sizes(self, grid=0):
+        """(half-bandwidth after RCM, doubles per matrix, workspace doubles per problem)."""
+        bw, md, ws = c_int32(), c_int64(), c_int64()
+        _check(lib().landau_band_sizes(self._h, grid, ctypes.byref(bw), ctypes.byref(md), ctypes.byref(ws)))
+        return bw.value, md.value, ws.value
+
+    def band_factor_batched(self, vals, band, stream=None):
+        nb = vals.shape[0]
+        assert band.is_cuda and band.is_contiguous() and band.numel() >= nb * self.band_sizes()[2]
+        _check(lib().landau_band_factor_batched(self._h, nb, c_void_p(vals.data_ptr()), c_void_p(band.data_ptr()), _stream_ptr(stream)))
+
+    def band_solve_batched(self, band, rhs, x, stream=None):
+        nb = rhs.shape[0]
+        _check(lib().landau_band_solve_batched(self._h, nb, c_void_p(band.data_ptr()), c_void_p(rhs.data_ptr()),
+                                               c_void_p(x.data_ptr()), _stream_ptr(stream)))
+
     def jacobian_host(self, f_host, vals_host=None, Cf_host=None):
         """Host buffers: numpy arrays or pinned CPU torch tensors (float64, contiguous)."""
         def hp(a):
@@ -284,6 +303,9 @@ class LandauMultigridContext:
     __del__ = LandauContext.__del__
     _ptr = staticmethod(LandauContext._ptr)
     launch_count = LandauContext.launch_count
+    band_sizes = LandauContext.band_sizes
+    band_factor_batched = LandauContext.band_factor_batched
+    band_solve_batched = LandauContext.band_solve_batched
 
     def species_slices(self):
         out, o = [], 0

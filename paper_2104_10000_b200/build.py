@@ -7,7 +7,7 @@ import subprocess
 HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 LIB = os.path.join(HERE, "liblandau_b200.so")
-SOURCES = ["landau_setup.cpp", "landau_kernels.cu", "landau_api.cu"]
+SOURCES = ["landau_setup.cpp", "landau_kernels.cu", "landau_band.cu", "landau_api.cu"]
 HEADERS = ["landau_internal.h", "landau_kernels.h", os.path.join(ROOT, "include", "landau.h")]
 
 

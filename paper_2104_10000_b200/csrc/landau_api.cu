@@ -53,6 +53,8 @@ struct GridState {
     size_t foff = 0;         // offset (doubles) of this grid's block inside one problem's f / Cf
     size_t voff = 0;         // ... inside one problem's vals
     size_t moff = 0;         // ... inside mvals
+    BandSpace bs;            // band LU of this grid's pattern (RCM order)
+    size_t boff = 0;         // offset (doubles) of this grid's matrices inside one problem's band workspace
     double *Ce = nullptr;    // [nb][S_g][Ne][Nb*Nb]
     double *ce = nullptr;    // [nb][S_g][Ne][Nb]
 };
@@ -63,6 +65,7 @@ struct landau_ctx {
     int S = 0;                       // all species
     int64_t Ntot = 0;                // integration points of all grids
     size_t fstride = 0, vstride = 0, mstride = 0;   // doubles per problem in f / vals; in mvals
+    size_t bstride = 0;                              // doubles per problem in the band-LU workspace
     const double *r = nullptr, *z = nullptr, *invr = nullptr;   // [Ntot] union of the grids' points
     bool check_all = false;          // points of different grids coincide somewhere
     Scratch sc;
@@ -245,6 +248,23 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         UPC(ds.rowptr, hs.rowptr) UPC(ds.colidx, hs.colidx)
         UPC(ds.gptr, hs.gptr) UPC(ds.gidx, hs.gidx) UPC(ds.gw, hs.gw)
         UPC(ds.cptr, hs.cptr) UPC(ds.cidx, hs.cidx) UPC(ds.cw, hs.cw)
+        // band LU: RCM order, half-bandwidth, CSR entry -> band offset
+        std::vector<int32_t> perm, bidx(hs.nnz);
+        int bw = 0;
+        rcm_order(int(hs.n), hs.rowptr, hs.colidx, perm, bw);
+        std::vector<int32_t> pos(hs.n);
+        for (int64_t i = 0; i < hs.n; ++i) pos[perm[i]] = int32_t(i);
+        const int64_t Wb = bw + band_block(bw), LD = 2 * Wb + 1;
+        if (LD * hs.n > (int64_t(1) << 31) - 1) { landau_destroy(ctx); return LANDAU_EINVAL; }
+        for (int64_t i = 0; i < hs.n; ++i)
+            for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) {
+                const int64_t ni = pos[i], nj = pos[hs.colidx[t]];
+                bidx[t] = int32_t((Wb + ni - nj) + nj * LD);
+            }
+        G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = size_t(LD) * hs.n;
+        UPC(G.bs.bidx, bidx) UPC(G.bs.perm, perm)
+        G.boff = ctx->bstride;
+        ctx->bstride += size_t(ds.S) * G.bs.mat_doubles;
     }
 #undef UPC
     // scratch arena
@@ -466,6 +486,44 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
     }
     CK(cudaStreamSynchronize(st));
     CK(cudaStreamSynchronize(cp));
+    return LANDAU_OK;
+}
+
+int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
+                      int64_t *workspace_doubles_per_problem) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    if (half_bandwidth) *half_bandwidth = ctx->grids[grid].bs.bw;
+    if (doubles_per_matrix) *doubles_per_matrix = int64_t(ctx->grids[grid].bs.mat_doubles);
+    if (workspace_doubles_per_problem) *workspace_doubles_per_problem = int64_t(ctx->bstride);
+    return LANDAU_OK;
+}
+
+// band workspace layout: [grid][problem][species of the grid][matrix] -- grid-major so that one launch
+// per grid sees its matrices contiguously
+int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, void *stream) {
+    if (!ctx || !vals_dev || !band_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (auto &g : ctx->grids) {
+        if (band_factor_smem(g.bs.bw) > 227 * 1024) return LANDAU_EINVAL;
+        double *band = band_dev + size_t(nb) * g.boff;
+        ctx->launches += launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, vals_dev + g.voff, band, st);
+        CK(launch_band_factor(g.bs, nb * g.ds.S, band, st));
+        ctx->launches += 1;
+    }
+    CK(cudaGetLastError());
+    return LANDAU_OK;
+}
+
+int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev, void *stream) {
+    if (!ctx || !band_dev || !rhs_dev || !x_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    for (auto &g : ctx->grids) {
+        if ((size_t(g.bs.n) + 33 * 32) * sizeof(double) > 227 * 1024) return LANDAU_EINVAL;
+        const double *band = band_dev + size_t(nb) * g.boff;
+        CK(launch_band_solve(g.bs, nb, g.ds.S, ctx->fstride, band, rhs_dev + g.foff, x_dev + g.foff, st));
+        ctx->launches += 1;
+    }
+    CK(cudaGetLastError());
     return LANDAU_OK;
 }
 

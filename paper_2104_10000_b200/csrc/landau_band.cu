@@ -1,0 +1,370 @@
+// Per-species batched band LU (section III-G): reverse
+// Cuthill-McKee ordering on the host (once per mesh), then on the device, per (problem, species)
+// matrix: scatter of the CSR values into band storage, Gaussian elimination WITHOUT pivoting in
+// outer-product form (Golub & Van Loan Alg. 4.3.1, the paper's choice) -- blocked: KB columns at a
+// time, the B x B outer-product update becomes a rank-KB update of the trailing window from
+// shared-memory panels -- and the two banded triangular solves.  One thread block per matrix
+// (the matrices of a batch are independent: L171, L244).
+//
+// Band storage of one matrix (order n, half-bandwidth bw after RCM, W = bw + KB so that the
+// rectangular panels of a block step stay inside the stored band): LAPACK's layout, element (i,j) at
+// band[(W + i - j) + j*LD], LD = 2W + 1, which is the ordinary column-major matrix
+// A(i,j) = band[W + i + j*(LD-1)] with leading dimension LD-1.  Entries outside the true band are
+// zero and stay zero (no pivoting => no fill outside the band).
+#include <cuda_runtime.h>
+
+#include <algorithm>
+#include <cstdint>
+#include <queue>
+#include <vector>
+
+#include "landau_kernels.h"
+
+namespace landau {
+
+// ------------------------------------------------------------------------------------------------
+// host: reverse Cuthill-McKee on the (structurally symmetric) pattern A1
+// ------------------------------------------------------------------------------------------------
+namespace {
+// BFS level structure from root inside the component; returns the eccentricity, fills order (BFS order)
+int bfs_levels(int root, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int> &level,
+               std::vector<int> &order) {
+    order.clear();
+    order.push_back(root);
+    level[root] = 0;
+    int ecc = 0;
+    for (size_t h = 0; h < order.size(); ++h) {
+        const int v = order[h];
+        for (int t = rowptr[v]; t < rowptr[v + 1]; ++t) {
+            const int u = colidx[t];
+            if (level[u] < 0) { level[u] = level[v] + 1; ecc = std::max(ecc, level[u]); order.push_back(u); }
+        }
+    }
+    return ecc;
+}
+}  // namespace
+
+// perm[new] = old, bw = max |new(i) - new(j)| over the pattern's entries
+void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw) {
+    std::vector<int> deg(n), level(n, -1), order, visited(n, 0);
+    for (int i = 0; i < n; ++i) deg[i] = rowptr[i + 1] - rowptr[i];
+    perm.clear();
+    std::vector<int> cm;
+    for (int seed = 0; seed < n; ++seed) {
+        if (visited[seed]) continue;
+        // pseudo-peripheral node of this component (George & Liu): repeat BFS from a minimum-degree node of the last level
+        int root = seed;
+        std::fill(level.begin(), level.end(), -1);
+        int ecc = bfs_levels(root, rowptr, colidx, level, order);
+        for (int it = 0; it < 8; ++it) {
+            int cand = -1;
+            for (int v : order)
+                if (level[v] == ecc && (cand < 0 || deg[v] < deg[cand])) cand = v;
+            for (int v : order) level[v] = -1;
+            std::vector<int> order2;
+            const int ecc2 = bfs_levels(cand, rowptr, colidx, level, order2);
+            if (ecc2 > ecc) { root = cand; ecc = ecc2; order.swap(order2); }
+            else { for (int v : order2) level[v] = -1; bfs_levels(root, rowptr, colidx, level, order); break; }
+        }
+        // Cuthill-McKee: BFS from root, neighbours in order of increasing degree
+        std::vector<int> q;
+        q.push_back(root);
+        visited[root] = 1;
+        for (size_t h = 0; h < q.size(); ++h) {
+            const int v = q[h];
+            std::vector<int> nb;
+            for (int t = rowptr[v]; t < rowptr[v + 1]; ++t)
+                if (!visited[colidx[t]]) { visited[colidx[t]] = 1; nb.push_back(colidx[t]); }
+            std::sort(nb.begin(), nb.end(), [&](int a, int b) { return deg[a] != deg[b] ? deg[a] < deg[b] : a < b; });
+            q.insert(q.end(), nb.begin(), nb.end());
+        }
+        cm.insert(cm.end(), q.begin(), q.end());
+    }
+    perm.assign(cm.rbegin(), cm.rend());   // reverse
+    std::vector<int> pos(n);
+    for (int i = 0; i < n; ++i) pos[perm[i]] = i;
+    bw = 0;
+    for (int i = 0; i < n; ++i)
+        for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) bw = std::max(bw, std::abs(pos[i] - pos[colidx[t]]));
+}
+
+int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }
+
+// ------------------------------------------------------------------------------------------------
+// device
+// ------------------------------------------------------------------------------------------------
+// scatter the CSR values into the (zeroed) band: band[m][bidx[k]] = vals[...][k]
+// grid = (ceil(nnz/256), S_g, nb)
+__global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, const int32_t *__restrict__ bidx,
+                               const double *__restrict__ vals, double *__restrict__ band) {
+    const int k = blockIdx.x * blockDim.x + threadIdx.x;
+    if (k >= nnz) return;
+    const double v = vals[(size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz + k];
+    band[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * mat_doubles + bidx[k]] = v;
+}
+
+constexpr int BAND_THREADS = 256;
+constexpr int WT_ROWS = 128, WT_COLS = 16;   // warp tile of the window update: 4 rows x 16 columns per lane
+
+// Blocked outer-product band LU, one block per matrix.  Dynamic shared memory:
+// sD[KB][KB+1], sL[KB][MW], sU[KB][MW] with MW = bw rounded up to WT_ROWS (zero padded).
+template <int KB>
+__global__ void __launch_bounds__(BAND_THREADS)
+k_band_factor(int n, int bw, int MW, size_t mat_doubles, double *__restrict__ band_all) {
+    extern __shared__ double smem[];
+    double *sD = smem;                       // [KB][KB+1]
+    double *sL = sD + KB * (KB + 1);         // [KB][MW]: sL[c][i] = L(k0+kb+i, k0+c)
+    double *sU = sL + (size_t)KB * MW;       // [KB][MW]: sU[c][j] = U(k0+c, k0+kb+j)
+    const int W = bw + KB;
+    const size_t lda = 2 * (size_t)W;        // LD - 1
+    double *A = band_all + (size_t)blockIdx.x * mat_doubles + W;   // A(i,j) = A[i + j*lda]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int k0 = 0; k0 < n; k0 += KB) {
+        const int kb = min(KB, n - k0);
+        const int m = min(bw, n - k0 - kb);
+        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+            const int r = t % kb, c = t / kb;
+            sD[r * (KB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
+        }
+        __syncthreads();
+        // diagonal block: unblocked elimination by warp 0, lane = row
+        if (warp == 0) {
+            for (int c = 0; c < kb - 1; ++c) {
+                const double piv = sD[c * (KB + 1) + c];
+                if (lane > c && lane < kb) {
+                    const double l = sD[lane * (KB + 1) + c] / piv;
+                    sD[lane * (KB + 1) + c] = l;
+                    for (int cc = c + 1; cc < kb; ++cc) sD[lane * (KB + 1) + cc] = fma(-l, sD[c * (KB + 1) + cc], sD[lane * (KB + 1) + cc]);
+                }
+                __syncwarp();
+            }
+        }
+        __syncthreads();
+        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+            const int r = t % kb, c = t / kb;
+            A[(k0 + r) + (size_t)(k0 + c) * lda] = sD[r * (KB + 1) + c];
+        }
+        // L panel: row i of A21 times U11^-1 (thread per row); zero padding up to MW
+        for (int i = tid; i < MW; i += BAND_THREADS) {
+            if (i < m) {
+                double x[KB];
+                double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) x[c] = c < kb ? row[(size_t)c * lda] : 0.0;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    if (c < kb) {
+                        double v = x[c];
+#pragma unroll
+                        for (int cc = 0; cc < c; ++cc) v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
+                        v = v / sD[c * (KB + 1) + c];
+                        x[c] = v;
+                        row[(size_t)c * lda] = v;
+                    }
+                    sL[(size_t)c * MW + i] = x[c];
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < KB; ++c) sL[(size_t)c * MW + i] = 0.0;
+            }
+        }
+        // U panel: L11^-1 times column j of A12 (thread per column)
+        for (int j = tid; j < MW; j += BAND_THREADS) {
+            if (j < m) {
+                double y[KB];
+                double *col = A + k0 + (size_t)(k0 + kb + j) * lda;
+#pragma unroll
+                for (int r = 0; r < KB; ++r) y[r] = r < kb ? col[r] : 0.0;
+#pragma unroll
+                for (int r = 0; r < KB; ++r) {
+                    if (r < kb) {
+                        double v = y[r];
+#pragma unroll
+                        for (int rr = 0; rr < r; ++rr) v = fma(-sD[r * (KB + 1) + rr], y[rr], v);
+                        y[r] = v;
+                        col[r] = v;
+                    }
+                    sU[(size_t)r * MW + j] = y[r];
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < KB; ++r) sU[(size_t)r * MW + j] = 0.0;
+            }
+        }
+        __syncthreads();
+        // trailing window A22 (m x m) -= L panel * U panel: warp tiles of WT_ROWS x WT_COLS
+        if (m > 0) {
+            const int trows = (m + WT_ROWS - 1) / WT_ROWS, tcols = (m + WT_COLS - 1) / WT_COLS;
+            double *C0 = A + (k0 + kb) + (size_t)(k0 + kb) * lda;
+            for (int wt = warp; wt < trows * tcols; wt += BAND_THREADS / 32) {
+                const int i0 = (wt % trows) * WT_ROWS + lane, j0 = (wt / trows) * WT_COLS;
+                double acc[4][WT_COLS];
+#pragma unroll
+                for (int ii = 0; ii < 4; ++ii)
+#pragma unroll
+                    for (int jj = 0; jj < WT_COLS; ++jj) acc[ii][jj] = 0.0;
+#pragma unroll 2
+                for (int c = 0; c < KB; ++c) {
+                    double l[4];
+#pragma unroll
+                    for (int ii = 0; ii < 4; ++ii) l[ii] = sL[(size_t)c * MW + i0 + 32 * ii];
+                    const double2 *up = reinterpret_cast<const double2 *>(sU + (size_t)c * MW + j0);
+#pragma unroll
+                    for (int j2 = 0; j2 < WT_COLS / 2; ++j2) {
+                        const double2 u = up[j2];
+#pragma unroll
+                        for (int ii = 0; ii < 4; ++ii) {
+                            acc[ii][2 * j2] = fma(l[ii], u.x, acc[ii][2 * j2]);
+                            acc[ii][2 * j2 + 1] = fma(l[ii], u.y, acc[ii][2 * j2 + 1]);
+                        }
+                    }
+                }
+#pragma unroll
+                for (int jj = 0; jj < WT_COLS; ++jj) {
+                    if (j0 + jj < m) {
+                        double *colp = C0 + (size_t)(j0 + jj) * lda;
+#pragma unroll
+                        for (int ii = 0; ii < 4; ++ii) {
+                            const int i = i0 + 32 * ii;
+                            if (i < m) colp[i] -= acc[ii][jj];
+                        }
+                    }
+                }
+            }
+        }
+        __syncthreads();
+    }
+}
+
+// Banded triangular solves, one block per matrix: x = P^T U^-1 L^-1 P b with the RCM permutation.
+// Blocks of SB columns: the diagonal block by warp 0 (lane = row), the panel below / above by one
+// thread per row with SB independent loads.
+constexpr int SB = 32;
+
+template <int KB>
+__global__ void __launch_bounds__(BAND_THREADS)
+k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
+             const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
+    extern __shared__ double smem[];
+    double *x = smem;                 // [n]
+    double *sD = x + n;               // [SB][SB+1]
+    const int W = bw + KB;
+    const size_t lda = 2 * (size_t)W;
+    const int mat = blockIdx.x;       // = b * S + sp
+    const double *A = band_all + (size_t)mat * mat_doubles + W;
+    const size_t voff = (size_t)(mat / S) * xstride + (size_t)(mat % S) * n;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    for (int i = tid; i < n; i += BAND_THREADS) x[i] = rhs[voff + perm[i]];
+    __syncthreads();
+    // forward: L y = b (unit lower)
+    for (int k0 = 0; k0 < n; k0 += SB) {
+        const int kb = min(SB, n - k0), m = min(bw, n - k0 - kb);
+        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+            const int r = t % kb, c = t / kb;
+            sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double v = lane < kb ? x[k0 + lane] : 0.0;
+            for (int c = 0; c < kb - 1; ++c) {
+                const double xc = __shfl_sync(0xffffffffu, v, c);
+                if (lane > c && lane < kb) v = fma(-sD[lane * (SB + 1) + c], xc, v);
+            }
+            if (lane < kb) x[k0 + lane] = v;
+        }
+        __syncthreads();
+        for (int i = tid; i < m; i += BAND_THREADS) {
+            const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+            double v = x[k0 + kb + i];
+#pragma unroll 8
+            for (int c = 0; c < kb; ++c) v = fma(-row[(size_t)c * lda], x[k0 + c], v);
+            x[k0 + kb + i] = v;
+        }
+        __syncthreads();
+    }
+    // backward: U x = y
+    const int nblk = (n + SB - 1) / SB;
+    for (int blk = nblk - 1; blk >= 0; --blk) {
+        const int k0 = blk * SB, kb = min(SB, n - k0), m = min(bw, k0);
+        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+            const int r = t % kb, c = t / kb;
+            sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
+        }
+        __syncthreads();
+        if (warp == 0) {
+            double v = lane < kb ? x[k0 + lane] : 0.0;
+            for (int c = kb - 1; c >= 0; --c) {
+                if (lane == c) v = v / sD[c * (SB + 1) + c];
+                const double xc = __shfl_sync(0xffffffffu, v, c);
+                if (lane < c) v = fma(-sD[lane * (SB + 1) + c], xc, v);
+            }
+            if (lane < kb) x[k0 + lane] = v;
+        }
+        __syncthreads();
+        for (int i = tid; i < m; i += BAND_THREADS) {
+            const int r = k0 - m + i;
+            const double *row = A + r + (size_t)k0 * lda;
+            double v = x[r];
+#pragma unroll 8
+            for (int c = 0; c < kb; ++c) v = fma(-row[(size_t)c * lda], x[k0 + c], v);
+            x[r] = v;
+        }
+        __syncthreads();
+    }
+    for (int i = tid; i < n; i += BAND_THREADS) xout[voff + perm[i]] = x[i];
+}
+
+// ------------------------------------------------------------------------------------------------
+// launchers
+// ------------------------------------------------------------------------------------------------
+static int band_mw(int bw) { return ((std::max(bw, 1) + WT_ROWS - 1) / WT_ROWS) * WT_ROWS; }
+
+size_t band_factor_smem(int bw) {
+    const int KB = band_block(bw);
+    return sizeof(double) * ((size_t)KB * (KB + 1) + 2 * (size_t)KB * band_mw(bw));
+}
+
+int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st) {
+    cudaMemsetAsync(band, 0, sizeof(double) * (size_t)nb * S * bs.mat_doubles, st);
+    dim3 grid((bs.nnz + 255) / 256, S, nb);
+    k_band_scatter<<<grid, 256, 0, st>>>(bs.nnz, vstride, bs.mat_doubles, bs.bidx, vals, band);
+    return 1;
+}
+
+template <int KB>
+static cudaError_t factor_t(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
+    const size_t smem = band_factor_smem(bs.bw);
+    cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_band_factor<KB><<<nmat, BAND_THREADS, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, band);
+    return cudaSuccess;
+}
+
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
+    switch (band_block(bs.bw)) {
+        case 32: return factor_t<32>(bs, nmat, band, st);
+        case 16: return factor_t<16>(bs, nmat, band, st);
+        default: return factor_t<8>(bs, nmat, band, st);
+    }
+}
+
+template <int KB>
+static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
+                           cudaStream_t st) {
+    const size_t smem = sizeof(double) * ((size_t)bs.n + SB * (SB + 1));
+    cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_band_solve<KB><<<nb * S, BAND_THREADS, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, band, rhs, x);
+    return cudaSuccess;
+}
+
+cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
+                              cudaStream_t st) {
+    switch (band_block(bs.bw)) {
+        case 32: return solve_t<32>(bs, nb, S, xstride, band, rhs, x, st);
+        case 16: return solve_t<16>(bs, nb, S, xstride, band, rhs, x, st);
+        default: return solve_t<8>(bs, nb, S, xstride, band, rhs, x, st);
+    }
+}
+
+}  // namespace landau

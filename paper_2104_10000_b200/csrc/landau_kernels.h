@@ -3,6 +3,7 @@
 #include <cuda_runtime.h>
 
 #include <cstdint>
+#include <vector>
 
 namespace landau {
 
@@ -55,6 +56,21 @@ int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
 int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
+
+// Band LU (landau_band.cu; section III-G)
+struct BandSpace {
+    int n, nnz, bw;            // order, CSR entries, half-bandwidth after RCM
+    size_t mat_doubles;        // (2 (bw + KB) + 1) * n doubles per matrix
+    const int32_t *bidx;       // [nnz] device: CSR entry -> offset in the matrix's band
+    const int32_t *perm;       // [n] device: new -> old
+};
+void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw);
+int band_block(int bw);        // KB, a function of bw only
+size_t band_factor_smem(int bw);
+int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st);
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cudaStream_t st);
+cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
+                              cudaStream_t st);
 
 int pair_tile_size(int N);
 int pair_tiles(int N);

@@ -177,6 +177,44 @@ def test_multigrid_parity(gpu, oracle, which):
         assert num <= 1e-12 * den
 
 
+@pytest.mark.parametrize("cfg,variant", [(0, "B"), (1, "B"), (3, "A"), (3, "B")])
+def test_band_lu_solve_parity(gpu, oracle, cfg, variant):
+    """SURVEY 8(f) NEXT-4 (section III-G): the matrices shift M + A - J of two problems factored and
+    solved on the device (RCM order, no pivoting) against the library solve of the oracle's dense blocks.
+    Tolerance: 50 cond(A) eps on max|x| (forward error of a backward-stable solve), and the residual."""
+    import torch
+    wl = inputs.config(cfg, variant=variant)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 2)
+    r, z = ctx.dof_coords()
+    f1 = inputs.nodal_f(wl, r, z)
+    f = np.stack([f1, 0.8 * f1])
+    Ez = np.array([0.1, -0.3]); shift = 4.0
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.zeros((2, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    F = torch.zeros((2, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.from_numpy(Ez).cuda(), shift, vals, F)
+    bw, md, ws = ctx.band_sizes()
+    band = torch.empty(2 * ws, dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band)
+    rhs = torch.from_numpy(np.cos(0.37 * np.arange(2 * ctx.S * ctx.n)).reshape(2, ctx.S, ctx.n) + 2.0).cuda()
+    x = torch.zeros_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    x2 = rhs.clone()
+    ctx.band_solve_batched(band, x2, x2)                       # in place
+    assert torch.equal(x, x2)
+    sp = oracle.build_space(wl.mesh, wl.order)
+    vals_h, x_h, rhs_h = vals.cpu().numpy(), x.cpu().numpy(), rhs.cpu().numpy()
+    for k in range(2):
+        for a in range(ctx.S):
+            A = oracle.dense_from_csr(sp, vals_h[k, a])
+            xo = oracle.solve_species(sp, vals_h[k, a], rhs_h[k, a])
+            cond = np.linalg.cond(A)
+            assert np.abs(x_h[k, a] - xo).max() <= 50 * cond * 2.2e-16 * np.abs(xo).max(), (k, a, cond)
+            res = np.abs(A @ x_h[k, a] - rhs_h[k, a]).max() / (np.abs(A).sum(axis=1).max() * np.abs(x_h[k, a]).max())
+            assert res <= 1e-13, (k, a, res)
+    print(f"{wl.name}: n = {ctx.n}, half-bandwidth after RCM {bw}")
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch
