@@ -182,6 +182,24 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
     ms = e0.elapsed_time(e1) / 3
     out["implicit_operator_config5"] = {"ms_per_step": ms, "gpair_per_s": nb * ctx5.N * (ctx5.N - 1) / (ms * 1e-3) * 1e-9,
                                         "what": "shift M + A(E_z) - J and A f - C(f) in one pass (landau_implicit_operator_batched)"}
+    # NEXT-4: band LU of the nb * S matrices of the implicit step (vals5 holds them now), then one solve
+    bw, md, ws = ctx5.band_sizes()
+    band = torch.empty(nb * ws, dtype=torch.float64, device="cuda")
+    rhs = torch.ones((nb, ctx5.S, ctx5.n), dtype=torch.float64, device="cuda")
+    x = torch.empty_like(rhs)
+    ctx5.band_factor_batched(vals5, band); ctx5.band_solve_batched(band, rhs, x)
+    torch.cuda.synchronize()
+    e2 = torch.cuda.Event(enable_timing=True)
+    e0.record(); ctx5.band_factor_batched(vals5, band); e1.record(); ctx5.band_solve_batched(band, rhs, x); e2.record()
+    torch.cuda.synchronize()
+    fms, sms_ = e0.elapsed_time(e1), e1.elapsed_time(e2)
+    nmat = nb * ctx5.S
+    flop = 2.0 * ctx5.n * bw * bw * nmat          # Alg. 4.3.1: n outer products of bw x bw, 2 flop each
+    out["band_lu_config5"] = {"matrices": nmat, "n": ctx5.n, "half_bandwidth_rcm": bw, "workspace_gb": nb * ws * 8e-9,
+                              "factor_ms": fms, "solve_ms": sms_, "factor_tflops": flop / (fms * 1e-3) * 1e-12,
+                              "factorizations_per_s": nmat / (fms * 1e-3),
+                              "what": "scatter + blocked outer-product band LU without pivoting, then L/U solves (one rhs)"}
+    del band, rhs, x
     name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("paper3")
     mg = binding.LandauMultigridContext(meshes, sgrid, order, spc, nb)
     fl = []

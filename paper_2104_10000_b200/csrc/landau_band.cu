@@ -88,7 +88,7 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
         for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) bw = std::max(bw, std::abs(pos[i] - pos[colidx[t]]));
 }
 
-int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }
+int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }   // panels must fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
 // device
@@ -103,38 +103,54 @@ __global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, cons
     band[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * mat_doubles + bidx[k]] = v;
 }
 
-constexpr int BAND_THREADS = 256;
-constexpr int WT_ROWS = 128, WT_COLS = 16;   // warp tile of the window update: 4 rows x 16 columns per lane
+constexpr int BAND_THREADS = 512;
+constexpr int WT = 32;   // warp tile of the window update: 32 x 32 = 4 x 4 mma tiles of 8 x 8
 
-// Blocked outer-product band LU, one block per matrix.  Dynamic shared memory:
-// sD[KB][KB+1], sL[KB][MW], sU[KB][MW] with MW = bw rounded up to WT_ROWS (zero padded).
+__device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
+    asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                 : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
+}
+
+// Blocked outer-product band LU, one block per matrix.  Per block step of KB columns:
+//   (1) the KB x KB diagonal block is eliminated by warp 0 in shared memory (lane = row);
+//   (2) one thread per row / column forms the L panel A21 U11^-1 and the U panel L11^-1 A12 (both in the
+//       same pass: two independent substitution chains per thread) and leaves -L and U in shared memory;
+//   (3) the trailing window A22 (bw x bw) += (-L)(U) is a rank-KB update on the FP64 tensor cores
+//       (mma.sync.m8n8k4, 32 x 32 warp tiles, fragments straight from the shared-memory panels).
+// Computed transposed (C^T = U^T (-L)^T) so that a lane's two accumulator entries are two consecutive
+// rows of one column of the column-major window.
+// Dynamic shared memory: sD[KB][KB+1], sDi[KB] (1/pivots), sL[KB][MWP], sU[KB][MWP]; MWP = bw rounded up to
+// WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB>
 __global__ void __launch_bounds__(BAND_THREADS)
-k_band_factor(int n, int bw, int MW, size_t mat_doubles, double *__restrict__ band_all) {
+k_band_factor(int n, int bw, int MWP, size_t mat_doubles, double *__restrict__ band_all) {
     extern __shared__ double smem[];
     double *sD = smem;                       // [KB][KB+1]
-    double *sL = sD + KB * (KB + 1);         // [KB][MW]: sL[c][i] = L(k0+kb+i, k0+c)
-    double *sU = sL + (size_t)KB * MW;       // [KB][MW]: sU[c][j] = U(k0+c, k0+kb+j)
+    double *sDi = sD + KB * (KB + 1);        // [KB]
+    double *sL = sDi + KB;                   // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
+    double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
     const int W = bw + KB;
     const size_t lda = 2 * (size_t)W;        // LD - 1
     double *A = band_all + (size_t)blockIdx.x * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, k = lane & 3;
     for (int k0 = 0; k0 < n; k0 += KB) {
         const int kb = min(KB, n - k0);
         const int m = min(bw, n - k0 - kb);
-        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
-            const int r = t % kb, c = t / kb;
-            sD[r * (KB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
+        for (int t = tid; t < KB * KB; t += BAND_THREADS) {
+            const int r = t % KB, c = t / KB;
+            // a short last block is completed by the identity, so that the panel code needs no kb guards
+            sD[r * (KB + 1) + c] = (r < kb && c < kb) ? A[(k0 + r) + (size_t)(k0 + c) * lda] : (r == c ? 1.0 : 0.0);
         }
         __syncthreads();
-        // diagonal block: unblocked elimination by warp 0, lane = row
         if (warp == 0) {
-            for (int c = 0; c < kb - 1; ++c) {
-                const double piv = sD[c * (KB + 1) + c];
-                if (lane > c && lane < kb) {
-                    const double l = sD[lane * (KB + 1) + c] / piv;
+            for (int c = 0; c < KB; ++c) {
+                const double pinv = 1.0 / sD[c * (KB + 1) + c];
+                if (lane == c) sDi[c] = pinv;
+                if (lane > c && lane < KB) {
+                    const double l = sD[lane * (KB + 1) + c] * pinv;
                     sD[lane * (KB + 1) + c] = l;
-                    for (int cc = c + 1; cc < kb; ++cc) sD[lane * (KB + 1) + cc] = fma(-l, sD[c * (KB + 1) + cc], sD[lane * (KB + 1) + cc]);
+                    for (int cc = c + 1; cc < KB; ++cc) sD[lane * (KB + 1) + cc] = fma(-l, sD[c * (KB + 1) + cc], sD[lane * (KB + 1) + cc]);
                 }
                 __syncwarp();
             }
@@ -144,90 +160,74 @@ k_band_factor(int n, int bw, int MW, size_t mat_doubles, double *__restrict__ ba
             const int r = t % kb, c = t / kb;
             A[(k0 + r) + (size_t)(k0 + c) * lda] = sD[r * (KB + 1) + c];
         }
-        // L panel: row i of A21 times U11^-1 (thread per row); zero padding up to MW
-        for (int i = tid; i < MW; i += BAND_THREADS) {
+        // panels: thread i does row i of the L panel and column i of the U panel
+        for (int i = tid; i < MWP; i += BAND_THREADS) {
             if (i < m) {
-                double x[KB];
+                // the thread's own panel entries live in shared memory (-x in sL, y in sU), not in registers
                 double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
-#pragma unroll
-                for (int c = 0; c < KB; ++c) x[c] = c < kb ? row[(size_t)c * lda] : 0.0;
-#pragma unroll
+                double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
+#pragma unroll 8
                 for (int c = 0; c < KB; ++c) {
-                    if (c < kb) {
-                        double v = x[c];
-#pragma unroll
-                        for (int cc = 0; cc < c; ++cc) v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
-                        v = v / sD[c * (KB + 1) + c];
-                        x[c] = v;
-                        row[(size_t)c * lda] = v;
+                    sL[(size_t)c * MWP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
+                    sU[(size_t)c * MWP + i] = c < kb ? col[c] : 0.0;
+                }
+                for (int c = 0; c < KB; ++c) {
+                    double v = sL[(size_t)c * MWP + i], w = sU[(size_t)c * MWP + i];
+#pragma unroll 4
+                    for (int cc = 0; cc < c; ++cc) {
+                        v = fma(sL[(size_t)cc * MWP + i], sD[cc * (KB + 1) + c], v);      // x U11 = a  (sL holds -x)
+                        w = fma(-sD[c * (KB + 1) + cc], sU[(size_t)cc * MWP + i], w);     // L11 y = a
                     }
-                    sL[(size_t)c * MW + i] = x[c];
+                    v *= sDi[c];
+                    if (c < kb) { row[(size_t)c * lda] = v; col[c] = w; }
+                    sL[(size_t)c * MWP + i] = -v;
+                    sU[(size_t)c * MWP + i] = w;
                 }
             } else {
 #pragma unroll
-                for (int c = 0; c < KB; ++c) sL[(size_t)c * MW + i] = 0.0;
-            }
-        }
-        // U panel: L11^-1 times column j of A12 (thread per column)
-        for (int j = tid; j < MW; j += BAND_THREADS) {
-            if (j < m) {
-                double y[KB];
-                double *col = A + k0 + (size_t)(k0 + kb + j) * lda;
-#pragma unroll
-                for (int r = 0; r < KB; ++r) y[r] = r < kb ? col[r] : 0.0;
-#pragma unroll
-                for (int r = 0; r < KB; ++r) {
-                    if (r < kb) {
-                        double v = y[r];
-#pragma unroll
-                        for (int rr = 0; rr < r; ++rr) v = fma(-sD[r * (KB + 1) + rr], y[rr], v);
-                        y[r] = v;
-                        col[r] = v;
-                    }
-                    sU[(size_t)r * MW + j] = y[r];
-                }
-            } else {
-#pragma unroll
-                for (int r = 0; r < KB; ++r) sU[(size_t)r * MW + j] = 0.0;
+                for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
             }
         }
         __syncthreads();
-        // trailing window A22 (m x m) -= L panel * U panel: warp tiles of WT_ROWS x WT_COLS
         if (m > 0) {
-            const int trows = (m + WT_ROWS - 1) / WT_ROWS, tcols = (m + WT_COLS - 1) / WT_COLS;
+            const int nt = (m + WT - 1) / WT;
             double *C0 = A + (k0 + kb) + (size_t)(k0 + kb) * lda;
-            for (int wt = warp; wt < trows * tcols; wt += BAND_THREADS / 32) {
-                const int i0 = (wt % trows) * WT_ROWS + lane, j0 = (wt / trows) * WT_COLS;
-                double acc[4][WT_COLS];
+            for (int wt = warp; wt < nt * nt; wt += BAND_THREADS / 32) {
+                const int i0 = (wt % nt) * WT, j0 = (wt / nt) * WT;
+                // acc[jb][ib] = C(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g)
+                double acc[4][4][2];
 #pragma unroll
-                for (int ii = 0; ii < 4; ++ii)
+                for (int jb = 0; jb < 4; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    const double *colp = C0 + (size_t)j * lda;
 #pragma unroll
-                    for (int jj = 0; jj < WT_COLS; ++jj) acc[ii][jj] = 0.0;
-#pragma unroll 2
-                for (int c = 0; c < KB; ++c) {
-                    double l[4];
-#pragma unroll
-                    for (int ii = 0; ii < 4; ++ii) l[ii] = sL[(size_t)c * MW + i0 + 32 * ii];
-                    const double2 *up = reinterpret_cast<const double2 *>(sU + (size_t)c * MW + j0);
-#pragma unroll
-                    for (int j2 = 0; j2 < WT_COLS / 2; ++j2) {
-                        const double2 u = up[j2];
-#pragma unroll
-                        for (int ii = 0; ii < 4; ++ii) {
-                            acc[ii][2 * j2] = fma(l[ii], u.x, acc[ii][2 * j2]);
-                            acc[ii][2 * j2 + 1] = fma(l[ii], u.y, acc[ii][2 * j2 + 1]);
-                        }
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        acc[jb][ib][0] = (j < m && i < m) ? colp[i] : 0.0;
+                        acc[jb][ib][1] = (j < m && i + 1 < m) ? colp[i + 1] : 0.0;
                     }
                 }
+#pragma unroll 2
+                for (int c0 = 0; c0 < KB; c0 += 4) {
+                    const double *pu = sU + (size_t)(c0 + k) * MWP + j0 + g;
+                    const double *pl = sL + (size_t)(c0 + k) * MWP + i0 + g;
+                    double fa[4], fb[4];
 #pragma unroll
-                for (int jj = 0; jj < WT_COLS; ++jj) {
-                    if (j0 + jj < m) {
-                        double *colp = C0 + (size_t)(j0 + jj) * lda;
+                    for (int t = 0; t < 4; ++t) { fa[t] = pu[8 * t]; fb[t] = pl[8 * t]; }
 #pragma unroll
-                        for (int ii = 0; ii < 4; ++ii) {
-                            const int i = i0 + 32 * ii;
-                            if (i < m) colp[i] -= acc[ii][jj];
-                        }
+                    for (int jb = 0; jb < 4; ++jb)
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) dmma884(acc[jb][ib], fa[jb], fb[ib]);
+                }
+#pragma unroll
+                for (int jb = 0; jb < 4; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    double *colp = C0 + (size_t)j * lda;
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < m && i < m) colp[i] = acc[jb][ib][0];
+                        if (j < m && i + 1 < m) colp[i + 1] = acc[jb][ib][1];
                     }
                 }
             }
@@ -317,11 +317,11 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-static int band_mw(int bw) { return ((std::max(bw, 1) + WT_ROWS - 1) / WT_ROWS) * WT_ROWS; }
+static int band_mw(int bw) { return ((std::max(bw, 1) + WT - 1) / WT) * WT + 4; }
 
 size_t band_factor_smem(int bw) {
     const int KB = band_block(bw);
-    return sizeof(double) * ((size_t)KB * (KB + 1) + 2 * (size_t)KB * band_mw(bw));
+    return sizeof(double) * ((size_t)KB * (KB + 1) + KB + 2 * (size_t)KB * band_mw(bw));
 }
 
 int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st) {
