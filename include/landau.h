@@ -154,15 +154,17 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
  * form (Golub & Van Loan Alg. 4.3.1, the paper's algorithm; blocked), one independent matrix per (problem,
  * species).  Meant for the matrices of landau_implicit_operator_batched (shift M + A - J); like the paper's
  * solver it does not pivot, so a zero or tiny pivot is not detected.
- * landau_band_sizes: per grid the half-bandwidth after RCM and the doubles one matrix occupies; and the
- * doubles of workspace per problem (all species of all grids).  band_dev: caller-owned workspace of
+ * landau_band_sizes: per grid the half-bandwidth after RCM and the doubles one matrix occupies; the
+ * doubles of workspace per problem (all species of all grids); and the flop of the outer-product updates of
+ * one factorisation (they are confined to the envelope of the ordered pattern, which elimination without
+ * pivoting does not leave: about half of 2 n bw^2 on the refined meshes).  band_dev: caller-owned workspace of
  * nb * workspace_doubles_per_problem doubles; its internal layout belongs to the library.
  * landau_band_factor_batched: vals_dev [nb][vals_stride] (CSR values, layout of landau_jacobian_batched)
  *   -> factors in band_dev.
  * landau_band_solve_batched: rhs_dev, x_dev [nb][f_stride] (layout of f); x = A^-1 rhs per species block;
  *   x_dev may equal rhs_dev.  Both are asynchronous on `stream` and deterministic. */
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
-                      int64_t *workspace_doubles_per_problem);
+                      int64_t *workspace_doubles_per_problem, double *flop_per_factorization);
 int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, void *stream);
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,
                               void *stream);

@@ -57,7 +57,7 @@ SIGNATURES = {
     "landau_jacobian_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
     "landau_implicit_operator_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
-    "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64)]),
+    "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
     "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
@@ -228,8 +228,9 @@ class LandauContext:
 
     def band_sizes(self, grid=0):
         """(half-bandwidth after RCM, doubles per matrix, workspace doubles per problem)."""
-        bw, md, ws = c_int32(), c_int64(), c_int64()
-        _check(lib().landau_band_sizes(self._h, grid, ctypes.byref(bw), ctypes.byref(md), ctypes.byref(ws)))
+        bw, md, ws, fl = c_int32(), c_int64(), c_int64(), c_double()
+        _check(lib().landau_band_sizes(self._h, grid, ctypes.byref(bw), ctypes.byref(md), ctypes.byref(ws), ctypes.byref(fl)))
+        self.band_flop_per_factorization = fl.value
         return bw.value, md.value, ws.value
 
     def band_factor_batched(self, vals, band, stream=None):

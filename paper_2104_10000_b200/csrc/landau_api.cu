@@ -262,6 +262,30 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
                 bidx[t] = int32_t((Wb + ni - nj) + nj * LD);
             }
         G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = size_t(LD) * hs.n;
+        // envelope of the permuted pattern: elimination without pivoting creates no fill left of a row's first
+        // entry / above a column's first entry, so block step s only reaches mlow[s] rows below and mup[s] rows
+        // above its block (<= bw; about half the uniform-band work on the refined meshes)
+        {
+            const int KBs = band_block(bw), nsteps = (int(hs.n) + KBs - 1) / KBs;
+            std::vector<int32_t> first(hs.n), last_with_first(hs.n + 1, 0), mlow(nsteps), mup(nsteps);
+            for (int64_t i = 0; i < hs.n; ++i) first[i] = int32_t(i);
+            for (int64_t i = 0; i < hs.n; ++i)
+                for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t)
+                    first[pos[i]] = std::min(first[pos[i]], pos[hs.colidx[t]]);      // structurally symmetric: rows = columns
+            for (int64_t i = 0; i < hs.n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], int32_t(i));
+            for (int64_t j = 1; j < hs.n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
+            double work = 0.0;
+            for (int st = 0; st < nsteps; ++st) {
+                const int k0 = st * KBs, ke = std::min<int>(k0 + KBs, int(hs.n)) - 1;
+                mlow[st] = std::max(0, last_with_first[ke] - ke);
+                int fmin = k0;
+                for (int j = k0; j <= ke; ++j) fmin = std::min(fmin, int(first[j]));
+                mup[st] = k0 - fmin;
+                work += 2.0 * (ke - k0 + 1) * double(mlow[st]) * double(mlow[st]);
+            }
+            G.bs.flop_per_matrix = work;
+            UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
+        }
         UPC(G.bs.bidx, bidx) UPC(G.bs.perm, perm)
         G.boff = ctx->bstride;
         ctx->bstride += size_t(ds.S) * G.bs.mat_doubles;
@@ -490,8 +514,9 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
 }
 
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
-                      int64_t *workspace_doubles_per_problem) {
+                      int64_t *workspace_doubles_per_problem, double *flop_per_factorization) {
     if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    if (flop_per_factorization) *flop_per_factorization = ctx->grids[grid].bs.flop_per_matrix;
     if (half_bandwidth) *half_bandwidth = ctx->grids[grid].bs.bw;
     if (doubles_per_matrix) *doubles_per_matrix = int64_t(ctx->grids[grid].bs.mat_doubles);
     if (workspace_doubles_per_problem) *workspace_doubles_per_problem = int64_t(ctx->bstride);

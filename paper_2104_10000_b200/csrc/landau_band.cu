@@ -106,6 +106,16 @@ __global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, cons
 constexpr int BAND_THREADS = 512;
 constexpr int WT = 32;   // warp tile of the window update: 32 x 32 = 4 x 4 mma tiles of 8 x 8
 
+// 1/x: MUFU seed and two Newton steps (full double precision up to rounding of the last step)
+__device__ __forceinline__ double rcp_newton(double x) {
+    double y;
+    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
+    double e = fma(-x, y, 1.0);
+    y = fma(y, fma(e, e, e), y);
+    e = fma(-x, y, 1.0);
+    return fma(y, e, y);
+}
+
 __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
     asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
@@ -123,7 +133,7 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB>
 __global__ void __launch_bounds__(BAND_THREADS)
-k_band_factor(int n, int bw, int MWP, size_t mat_doubles, double *__restrict__ band_all) {
+k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restrict__ mlow, double *__restrict__ band_all) {
     extern __shared__ double smem[];
     double *sD = smem;                       // [KB][KB+1]
     double *sDi = sD + KB * (KB + 1);        // [KB]
@@ -136,56 +146,85 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, double *__restrict__ b
     const int g = lane >> 2, k = lane & 3;
     for (int k0 = 0; k0 < n; k0 += KB) {
         const int kb = min(KB, n - k0);
-        const int m = min(bw, n - k0 - kb);
-        for (int t = tid; t < KB * KB; t += BAND_THREADS) {
-            const int r = t % KB, c = t / KB;
-            // a short last block is completed by the identity, so that the panel code needs no kb guards
-            sD[r * (KB + 1) + c] = (r < kb && c < kb) ? A[(k0 + r) + (size_t)(k0 + c) * lda] : (r == c ? 1.0 : 0.0);
-        }
-        __syncthreads();
+        const int m = mlow[k0 / KB];         // rows below / columns right of the block inside the envelope (<= bw)
+        // (1) warp 0: diagonal block, lane = row, the row in registers, pivot rows by shuffle (a short last
+        //     block is completed by the identity, so that no kb guards are needed);
+        //     meanwhile the other warps fetch the raw panel entries into shared memory
         if (warp == 0) {
+            // rows in shared memory, one lane per row; every offset below is a compile-time constant, so the
+            // loads of a column step are issued together
+            double *myrow = sD + lane * (KB + 1);
+#pragma unroll
+            for (int c = 0; c < KB; ++c)
+                myrow[c] = (lane < kb && c < kb) ? A[(k0 + lane) + (size_t)(k0 + c) * lda] : (lane == c ? 1.0 : 0.0);
+            __syncwarp();
+#pragma unroll
             for (int c = 0; c < KB; ++c) {
-                const double pinv = 1.0 / sD[c * (KB + 1) + c];
+                const double *prow = sD + c * (KB + 1);
+                const double pinv = rcp_newton(prow[c]);
                 if (lane == c) sDi[c] = pinv;
-                if (lane > c && lane < KB) {
-                    const double l = sD[lane * (KB + 1) + c] * pinv;
-                    sD[lane * (KB + 1) + c] = l;
-                    for (int cc = c + 1; cc < KB; ++cc) sD[lane * (KB + 1) + cc] = fma(-l, sD[c * (KB + 1) + cc], sD[lane * (KB + 1) + cc]);
+                if (lane > c) {
+                    const double l = myrow[c] * pinv;
+                    myrow[c] = l;
+#pragma unroll
+                    for (int cc = c + 1; cc < KB; ++cc) myrow[cc] = fma(-l, prow[cc], myrow[cc]);
                 }
                 __syncwarp();
             }
+            if (lane < kb) {
+#pragma unroll
+                for (int c = 0; c < KB; ++c)
+                    if (c < kb) A[(k0 + lane) + (size_t)(k0 + c) * lda] = myrow[c];
+            }
+        } else {
+            for (int i = tid - 32; i < MWP; i += BAND_THREADS - 32) {
+                if (i < m) {
+                    const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+                    const double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
+#pragma unroll 16
+                    for (int c = 0; c < KB; ++c) {
+                        sL[(size_t)c * MWP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
+                        sU[(size_t)c * MWP + i] = c < kb ? col[c] : 0.0;
+                    }
+                } else {
+#pragma unroll
+                    for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
+                }
+            }
         }
         __syncthreads();
-        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
-            const int r = t % kb, c = t / kb;
-            A[(k0 + r) + (size_t)(k0 + c) * lda] = sD[r * (KB + 1) + c];
-        }
-        // panels: thread i does row i of the L panel and column i of the U panel
-        for (int i = tid; i < MWP; i += BAND_THREADS) {
-            if (i < m) {
-                // the thread's own panel entries live in shared memory (-x in sL, y in sU), not in registers
+        // (2) panels: thread i does row i of the L panel (x U11 = a) and column i of the U panel (L11 y = a);
+        //     its entries live in shared memory (-x in sL, y in sU), not in registers
+        for (int i = tid; i < m; i += BAND_THREADS) {
+            double x[KB];
+            {   // L panel row: x U11 = a
                 double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
-                double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
-#pragma unroll 8
+#pragma unroll
+                for (int c = 0; c < KB; ++c) x[c] = sL[(size_t)c * MWP + i];
+#pragma unroll
                 for (int c = 0; c < KB; ++c) {
-                    sL[(size_t)c * MWP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
-                    sU[(size_t)c * MWP + i] = c < kb ? col[c] : 0.0;
-                }
-                for (int c = 0; c < KB; ++c) {
-                    double v = sL[(size_t)c * MWP + i], w = sU[(size_t)c * MWP + i];
-#pragma unroll 4
-                    for (int cc = 0; cc < c; ++cc) {
-                        v = fma(sL[(size_t)cc * MWP + i], sD[cc * (KB + 1) + c], v);      // x U11 = a  (sL holds -x)
-                        w = fma(-sD[c * (KB + 1) + cc], sU[(size_t)cc * MWP + i], w);     // L11 y = a
-                    }
+                    double v = x[c];
+#pragma unroll
+                    for (int cc = 0; cc < c; ++cc) v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
                     v *= sDi[c];
-                    if (c < kb) { row[(size_t)c * lda] = v; col[c] = w; }
+                    x[c] = v;
+                    if (c < kb) row[(size_t)c * lda] = v;
                     sL[(size_t)c * MWP + i] = -v;
+                }
+            }
+            {   // U panel column: L11 y = a
+                double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) x[c] = sU[(size_t)c * MWP + i];
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    double w = x[c];
+#pragma unroll
+                    for (int cc = 0; cc < c; ++cc) w = fma(-sD[c * (KB + 1) + cc], x[cc], w);
+                    x[c] = w;
+                    if (c < kb) col[c] = w;
                     sU[(size_t)c * MWP + i] = w;
                 }
-            } else {
-#pragma unroll
-                for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
             }
         }
         __syncthreads();
@@ -194,18 +233,21 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, double *__restrict__ b
             double *C0 = A + (k0 + kb) + (size_t)(k0 + kb) * lda;
             for (int wt = warp; wt < nt * nt; wt += BAND_THREADS / 32) {
                 const int i0 = (wt % nt) * WT, j0 = (wt / nt) * WT;
-                // acc[jb][ib] = C(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g)
+                // acc[jb][ib] = -(L U)(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g).  The C tile is pulled into L2 now and
+                // added at the end, two column blocks at a time (registers: no room for a second 32 x 32 tile;
+                // measured: 256 or 384 threads with the tile prefetched into registers are slower)
                 double acc[4][4][2];
 #pragma unroll
                 for (int jb = 0; jb < 4; ++jb) {
                     const int j = j0 + 8 * jb + g;
-                    const double *colp = C0 + (size_t)j * lda;
-#pragma unroll
-                    for (int ib = 0; ib < 4; ++ib) {
-                        const int i = i0 + 8 * ib + 2 * k;
-                        acc[jb][ib][0] = (j < m && i < m) ? colp[i] : 0.0;
-                        acc[jb][ib][1] = (j < m && i + 1 < m) ? colp[i + 1] : 0.0;
+                    if (j < m && k == 0) {
+                        const double *colp = C0 + (size_t)j * lda + i0;
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp + 16));
+                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp + 31));
                     }
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) { acc[jb][ib][0] = 0.0; acc[jb][ib][1] = 0.0; }
                 }
 #pragma unroll 2
                 for (int c0 = 0; c0 < KB; c0 += 4) {
@@ -220,14 +262,29 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, double *__restrict__ b
                         for (int ib = 0; ib < 4; ++ib) dmma884(acc[jb][ib], fa[jb], fb[ib]);
                 }
 #pragma unroll
-                for (int jb = 0; jb < 4; ++jb) {
-                    const int j = j0 + 8 * jb + g;
-                    double *colp = C0 + (size_t)j * lda;
+                for (int jh = 0; jh < 4; jh += 2) {
+                    double cb[2][4][2];
 #pragma unroll
-                    for (int ib = 0; ib < 4; ++ib) {
-                        const int i = i0 + 8 * ib + 2 * k;
-                        if (j < m && i < m) colp[i] = acc[jb][ib][0];
-                        if (j < m && i + 1 < m) colp[i + 1] = acc[jb][ib][1];
+                    for (int jb = 0; jb < 2; ++jb) {
+                        const int j = j0 + 8 * (jh + jb) + g;
+                        const double *colp = C0 + (size_t)j * lda;
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) {
+                            const int i = i0 + 8 * ib + 2 * k;
+                            cb[jb][ib][0] = (j < m && i < m) ? colp[i] : 0.0;
+                            cb[jb][ib][1] = (j < m && i + 1 < m) ? colp[i + 1] : 0.0;
+                        }
+                    }
+#pragma unroll
+                    for (int jb = 0; jb < 2; ++jb) {
+                        const int j = j0 + 8 * (jh + jb) + g;
+                        double *colp = C0 + (size_t)j * lda;
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) {
+                            const int i = i0 + 8 * ib + 2 * k;
+                            if (j < m && i < m) colp[i] = cb[jb][ib][0] + acc[jh + jb][ib][0];
+                            if (j < m && i + 1 < m) colp[i + 1] = cb[jb][ib][1] + acc[jh + jb][ib][1];
+                        }
                     }
                 }
             }
@@ -244,7 +301,7 @@ constexpr int SB = 32;
 template <int KB>
 __global__ void __launch_bounds__(BAND_THREADS)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
-             const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
+             const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
     extern __shared__ double smem[];
     double *x = smem;                 // [n]
     double *sD = x + n;               // [SB][SB+1]
@@ -258,7 +315,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     __syncthreads();
     // forward: L y = b (unit lower)
     for (int k0 = 0; k0 < n; k0 += SB) {
-        const int kb = min(SB, n - k0), m = min(bw, n - k0 - kb);
+        const int kb = min(SB, n - k0), m = KB == SB ? mlow[k0 / SB] : min(bw, n - k0 - kb);
         for (int t = tid; t < kb * kb; t += BAND_THREADS) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
@@ -285,7 +342,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     // backward: U x = y
     const int nblk = (n + SB - 1) / SB;
     for (int blk = nblk - 1; blk >= 0; --blk) {
-        const int k0 = blk * SB, kb = min(SB, n - k0), m = min(bw, k0);
+        const int k0 = blk * SB, kb = min(SB, n - k0), m = KB == SB ? mup[blk] : min(bw, k0);
         for (int t = tid; t < kb * kb; t += BAND_THREADS) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
@@ -336,7 +393,7 @@ static cudaError_t factor_t(const BandSpace &bs, int nmat, double *band, cudaStr
     const size_t smem = band_factor_smem(bs.bw);
     cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_factor<KB><<<nmat, BAND_THREADS, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, band);
+    k_band_factor<KB><<<nmat, BAND_THREADS, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, bs.mlow, band);
     return cudaSuccess;
 }
 
@@ -354,7 +411,7 @@ static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, c
     const size_t smem = sizeof(double) * ((size_t)bs.n + SB * (SB + 1));
     cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB><<<nb * S, BAND_THREADS, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, band, rhs, x);
+    k_band_solve<KB><<<nb * S, BAND_THREADS, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, band, rhs, x);
     return cudaSuccess;
 }
 

@@ -63,6 +63,8 @@ struct BandSpace {
     size_t mat_doubles;        // (2 (bw + KB) + 1) * n doubles per matrix
     const int32_t *bidx;       // [nnz] device: CSR entry -> offset in the matrix's band
     const int32_t *perm;       // [n] device: new -> old
+    const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
+    double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
 void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw);
 int band_block(int bw);        // KB, a function of bw only
