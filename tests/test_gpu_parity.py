@@ -215,6 +215,39 @@ def test_band_lu_solve_parity(gpu, oracle, cfg, variant):
     print(f"{wl.name}: n = {ctx.n}, half-bandwidth after RCM {bw}")
 
 
+def test_one_implicit_step_through_the_whole_path_conserves(gpu):
+    """Operator -> band LU -> solve chained on the device: one quasi-Newton iteration of backward Euler for
+    Eq. 4 (E_z = 0), (M/dt - J(f0)) delta = C(f0), f1 = f0 + delta.  Because 1^T J_a = 0 and
+    1^T C_a = 0 hold discretely, the step conserves every species' density to the accuracy of the linear
+    solve (residual ~ eps |A| |delta|) -- the density part of the paper's conservation claim (L17) carried
+    through the solver.  (Momentum and energy are conserved by C(f), i.e. at convergence of the iteration,
+    not by one frozen-coefficient step.)"""
+    import torch
+    wl = inputs.config(3, variant="A")
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 1)
+    r, z = ctx.dof_coords()
+    f0 = inputs.nodal_f(wl, r, z)[None]
+    dt = 0.5
+    fd = torch.from_numpy(f0).cuda()
+    vals = torch.zeros((1, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    F = torch.zeros((1, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.zeros(1, dtype=torch.float64, device="cuda"), 1.0 / dt, vals, F)
+    band = torch.empty(ctx.band_sizes()[2], dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band)
+    delta = torch.empty_like(F)
+    ctx.band_solve_batched(band, -F, delta)           # F = -C(f0) here
+    mv = torch.zeros(ctx.nnz, dtype=torch.float64, device="cuda")
+    ctx.mass(1.0, mv)
+    rowptr, colidx = ctx.csr_pattern_host()
+    import scipy.sparse as sps
+    M = sps.csr_matrix((mv.cpu().numpy(), colidx, rowptr), shape=(ctx.n, ctx.n))
+    d = delta.cpu().numpy()[0]
+    assert np.abs(d).max() > 1e-6 * np.abs(f0).max()                      # the step does something
+    for a in range(ctx.S):
+        Md = M @ d[a]
+        assert abs(Md.sum()) <= 1e-9 * np.abs(Md).sum()                   # density of every species (solver accuracy)
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch
