@@ -44,7 +44,7 @@ FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 
 # ncu --set full capture summarised in profiles/r01c_pair_kernel.md (73.9 MB read + 3.880 GB written:
 # the per-source-tile partial slabs; the algorithmic minimum is 24 B/point in + 40 B/point out = 0.16 GB).
 PAIR_KERNEL_DRAM_BYTES = 73.9e6 + 3.8797e9
-# the same for the rest of the step (fields, slab sum, element matrices, two gathers), profiles/r01d_step_kernels.md (ncu --set full, dram read + write)
+# the same for the rest of the step (fields, slab sum, element matrices, two gathers), profiles/r01e_step_kernels.md (ncu --set full, dram read + write)
 REST_DRAM_BYTES = 6.03e9   # 4.04 GB of it is k_sum_partials reading the slabs
 
 
