@@ -248,6 +248,45 @@ def test_one_implicit_step_through_the_whole_path_conserves(gpu):
         assert abs(Md.sum()) <= 1e-9 * np.abs(Md).sum()                   # density of every species (solver accuracy)
 
 
+def test_edge_cases_of_the_next_rows(gpu, oracle):
+    """One-cell mesh through the implicit operator and the band LU (n = 9 < one elimination block); NULL outputs;
+    argument errors of the multigrid constructor."""
+    import torch
+    mesh = inputs.mesh_uniform(0.0, 2.0, -1.0, 1.0, 1, 1)
+    spc = inputs._sp([(1, -1, 1, 1), (2, 1, 1, 1)])
+    wl = inputs.Workload("one-cell-2sp", 2, mesh, spc, [[inputs.Component(0, 1, 1), inputs.Component(1, 1, 1)]], 1e-3, 7)
+    ctx = gpu.LandauContext(mesh, 2, spc, 1)
+    r, z = ctx.dof_coords()
+    f = inputs.nodal_f(wl, r, z)[None]
+    fd = torch.from_numpy(f).cuda()
+    Ez = torch.tensor([0.5], dtype=torch.float64, device="cuda")
+    vals = torch.zeros((1, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, Ez, 3.0, vals, None)          # F skipped
+    ctx.implicit_operator_batched(fd, Ez, 3.0, None, None)          # both skipped
+    sp = oracle.build_space(mesh, 2)
+    ov, _ = oracle.implicit_operator(sp, spc, f[0], 0.5, 3.0)
+    bw, md, ws = ctx.band_sizes()
+    assert ctx.n == 9 and bw == 8
+    band = torch.empty(ws, dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band)
+    rhs = torch.arange(1.0, 1.0 + ctx.S * ctx.n, dtype=torch.float64, device="cuda").reshape(1, ctx.S, ctx.n)
+    x = torch.empty_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    for a in range(ctx.S):
+        assert block_err(vals[0, a].cpu().numpy(), ov[a]) <= TOL
+        xo = oracle.solve_species(sp, ov[a], rhs[0, a].cpu().numpy())
+        assert np.abs(x[0, a].cpu().numpy() - xo).max() <= 1e-10 * np.abs(xo).max()
+    with pytest.raises(gpu.LandauError):
+        ctx.band_solve_batched(band, torch.zeros((2, ctx.S, ctx.n), dtype=torch.float64, device="cuda"),
+                               torch.zeros((2, ctx.S, ctx.n), dtype=torch.float64, device="cuda"))       # nb > max_batch
+    g = inputs.config(0).mesh
+    sp3 = inputs._sp([(1, -1, 1, 1), (4, 1, 1, 1), (8, 1, 1, 1)])
+    for bad in ([1, 0, 1], [0, 0, 0], [0, 2, 2], [0, 1, 5]):         # not grouped / grid unused / out of range
+        with pytest.raises(gpu.LandauError) as ei:
+            gpu.LandauMultigridContext([g, inputs.mesh_scaled(g, 0.5)], bad, 2, sp3, 1)
+        assert ei.value.code == gpu.LANDAU_EINVAL
+
+
 def test_inner_integral_parity(gpu, oracle):
     """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
     import torch
