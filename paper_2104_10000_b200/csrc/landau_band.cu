@@ -88,6 +88,7 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
         for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) bw = std::max(bw, std::abs(pos[i] - pos[colidx[t]]));
 }
 
+// (16-column blocks with two blocks of 256 threads per SM were measured slower at bw = 339: 52 vs 41 ms)
 int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }   // panels must fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
@@ -153,17 +154,20 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
         if (warp == 0) {
             // rows in shared memory, one lane per row; every offset below is a compile-time constant, so the
             // loads of a column step are issued together
-            double *myrow = sD + lane * (KB + 1);
+            double *myrow = sD + min(lane, KB - 1) * (KB + 1);
+            const bool rowlane = lane < KB;        // KB < 32: the upper lanes only follow the warp barriers
+            if (rowlane) {
 #pragma unroll
-            for (int c = 0; c < KB; ++c)
-                myrow[c] = (lane < kb && c < kb) ? A[(k0 + lane) + (size_t)(k0 + c) * lda] : (lane == c ? 1.0 : 0.0);
+                for (int c = 0; c < KB; ++c)
+                    myrow[c] = (lane < kb && c < kb) ? A[(k0 + lane) + (size_t)(k0 + c) * lda] : (lane == c ? 1.0 : 0.0);
+            }
             __syncwarp();
 #pragma unroll
             for (int c = 0; c < KB; ++c) {
                 const double *prow = sD + c * (KB + 1);
                 const double pinv = rcp_newton(prow[c]);
                 if (lane == c) sDi[c] = pinv;
-                if (lane > c) {
+                if (lane > c && rowlane) {
                     const double l = myrow[c] * pinv;
                     myrow[c] = l;
 #pragma unroll
@@ -294,14 +298,14 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
 }
 
 // Banded triangular solves, one block per matrix: x = P^T U^-1 L^-1 P b with the RCM permutation.
-// Blocks of SB columns: the diagonal block by warp 0 (lane = row), the panel below / above by one
-// thread per row with SB independent loads.
-constexpr int SB = 32;
+// Blocks of KB columns (those of the factorisation): the diagonal block by warp 0 (lane = row), the panel
+// below / above, confined to the envelope, by one thread per row with KB independent loads.
 
 template <int KB>
 __global__ void __launch_bounds__(BAND_THREADS)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
              const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
+    constexpr int SB = KB;            // same blocks as the factorisation: panels stay inside the stored band
     extern __shared__ double smem[];
     double *x = smem;                 // [n]
     double *sD = x + n;               // [SB][SB+1]
@@ -315,7 +319,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     __syncthreads();
     // forward: L y = b (unit lower)
     for (int k0 = 0; k0 < n; k0 += SB) {
-        const int kb = min(SB, n - k0), m = KB == SB ? mlow[k0 / SB] : min(bw, n - k0 - kb);
+        const int kb = min(SB, n - k0), m = mlow[k0 / SB];
         for (int t = tid; t < kb * kb; t += BAND_THREADS) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
@@ -342,7 +346,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     // backward: U x = y
     const int nblk = (n + SB - 1) / SB;
     for (int blk = nblk - 1; blk >= 0; --blk) {
-        const int k0 = blk * SB, kb = min(SB, n - k0), m = KB == SB ? mup[blk] : min(bw, k0);
+        const int k0 = blk * SB, kb = min(SB, n - k0), m = mup[blk];
         for (int t = tid; t < kb * kb; t += BAND_THREADS) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
@@ -408,7 +412,7 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cuda
 template <int KB>
 static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
                            cudaStream_t st) {
-    const size_t smem = sizeof(double) * ((size_t)bs.n + SB * (SB + 1));
+    const size_t smem = sizeof(double) * ((size_t)bs.n + KB * (KB + 1));
     cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_band_solve<KB><<<nb * S, BAND_THREADS, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, band, rhs, x);

@@ -248,6 +248,37 @@ def test_one_implicit_step_through_the_whole_path_conserves(gpu):
         assert abs(Md.sum()) <= 1e-9 * np.abs(Md).sum()                   # density of every species (solver accuracy)
 
 
+def test_band_lu_wide_band_uses_the_16_column_blocks(gpu):
+    """A 32 x 32 Q3 mesh (n = 9,409, half-bandwidth > 416): the panels no longer fit shared memory with 32-column
+    blocks, so the 16-column instantiation runs.  Reference: scipy's sparse direct solve of the same CSR matrix
+    (too large for the oracle's dense solve); tolerance through the residual."""
+    import torch
+    import scipy.sparse as sps
+    import scipy.sparse.linalg as spla
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 32, 32)
+    spc = inputs._sp([(1, -1, 1, 1)])
+    wl = inputs.Workload("q3-32x32", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 11)
+    ctx = gpu.LandauContext(mesh, 3, spc, 1)
+    bw, md, ws = ctx.band_sizes()
+    assert 416 < bw <= 850 and ctx.n == 97 * 97, bw
+    r, z = ctx.dof_coords()
+    fd = torch.from_numpy(inputs.nodal_f(wl, r, z)[None]).cuda()
+    vals = torch.zeros((1, 1, ctx.nnz), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.zeros(1, dtype=torch.float64, device="cuda"), 2.0, vals, None)
+    band = torch.empty(ws, dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band)
+    rhs = torch.from_numpy(np.cos(0.01 * np.arange(ctx.n))[None, None] + 2.0).cuda()
+    x = torch.empty_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    rowptr, colidx = ctx.csr_pattern_host()
+    A = sps.csr_matrix((vals.cpu().numpy()[0, 0], colidx, rowptr), shape=(ctx.n, ctx.n))
+    xg, b = x.cpu().numpy()[0, 0], rhs.cpu().numpy()[0, 0]
+    res = np.abs(A @ xg - b).max() / (abs(A).sum(axis=1).max() * np.abs(xg).max())
+    assert res <= 1e-13, res
+    xs = spla.spsolve(A.tocsc(), b)
+    assert np.abs(xg - xs).max() <= 1e-8 * np.abs(xs).max()
+
+
 def test_edge_cases_of_the_next_rows(gpu, oracle):
     """One-cell mesh through the implicit operator and the band LU (n = 9 < one elimination block); NULL outputs;
     argument errors of the multigrid constructor."""
