@@ -254,14 +254,14 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         rcm_order(int(hs.n), hs.rowptr, hs.colidx, perm, bw);
         std::vector<int32_t> pos(hs.n);
         for (int64_t i = 0; i < hs.n; ++i) pos[perm[i]] = int32_t(i);
-        const int64_t Wb = bw + band_block(bw), LD = 2 * Wb + 1;
+        const int64_t Wb = (bw + band_block(bw) + 1) & ~1, LD = 2 * Wb + 1;   // even half-width (band_halfwidth in landau_band.cu)
         if (LD * hs.n > (int64_t(1) << 31) - 1) { landau_destroy(ctx); return LANDAU_EINVAL; }
         for (int64_t i = 0; i < hs.n; ++i)
             for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) {
                 const int64_t ni = pos[i], nj = pos[hs.colidx[t]];
                 bidx[t] = int32_t((Wb + ni - nj) + nj * LD);
             }
-        G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = size_t(LD) * hs.n;
+        G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = (size_t(LD) * hs.n + 1) & ~size_t(1);   // even: every matrix starts 16-byte aligned
         // envelope of the permuted pattern: elimination without pivoting creates no fill left of a row's first
         // entry / above a column's first entry, so block step s only reaches mlow[s] rows below and mup[s] rows
         // above its block (<= bw; about half the uniform-band work on the refined meshes)

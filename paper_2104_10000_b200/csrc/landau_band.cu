@@ -89,6 +89,9 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
 }
 
 // (16-column blocks with two blocks of 256 threads per SM were measured slower at bw = 339: 52 vs 41 ms)
+// stored half-width: bw + KB rounded up to even (16-byte aligned column pairs in the window update)
+__host__ __device__ inline int band_halfwidth(int bw, int KB) { return (bw + KB + 1) & ~1; }
+
 int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }   // panels must fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
@@ -105,7 +108,7 @@ __global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, cons
 }
 
 constexpr int BAND_THREADS = 512;
-constexpr int WT = 32;   // warp tile of the window update: 32 x 32 = 4 x 4 mma tiles of 8 x 8
+constexpr int WT = 32, WTJ = 16;   // warp tile of the window update: 32 rows x 16 columns = 4 x 2 mma tiles of 8 x 8
 
 // 1/x: MUFU seed and two Newton steps (full double precision up to rounding of the last step)
 __device__ __forceinline__ double rcp_newton(double x) {
@@ -140,7 +143,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
     double *sDi = sD + KB * (KB + 1);        // [KB]
     double *sL = sDi + KB;                   // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
     double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
-    const int W = bw + KB;
+    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;        // LD - 1
     double *A = band_all + (size_t)blockIdx.x * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -233,62 +236,55 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
         }
         __syncthreads();
         if (m > 0) {
-            const int nt = (m + WT - 1) / WT;
+            // warp tiles of 32 rows x 16 columns: the accumulators (32 doubles) leave room for the C tile itself
+            // (32 doubles), which is fetched into registers BEFORE the mma loop and so costs no wait afterwards
+            const int nti = (m + WT - 1) / WT, ntj = (m + WTJ - 1) / WTJ;
             double *C0 = A + (k0 + kb) + (size_t)(k0 + kb) * lda;
-            for (int wt = warp; wt < nt * nt; wt += BAND_THREADS / 32) {
-                const int i0 = (wt % nt) * WT, j0 = (wt / nt) * WT;
-                // acc[jb][ib] = -(L U)(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g).  The C tile is pulled into L2 now and
-                // added at the end, two column blocks at a time (registers: no room for a second 32 x 32 tile;
-                // measured: 256 or 384 threads with the tile prefetched into registers are slower)
-                double acc[4][4][2];
+            for (int wt = warp; wt < nti * ntj; wt += BAND_THREADS / 32) {
+                const int i0 = (wt % nti) * WT, j0 = (wt / nti) * WTJ;
+                // acc[jb][ib] = -(L U)(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g)
+                double acc[2][4][2], cb[2][4][2];
 #pragma unroll
-                for (int jb = 0; jb < 4; ++jb) {
+                for (int jb = 0; jb < 2; ++jb) {
                     const int j = j0 + 8 * jb + g;
-                    if (j < m && k == 0) {
-                        const double *colp = C0 + (size_t)j * lda + i0;
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp));
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp + 16));
-                        asm volatile("prefetch.global.L2 [%0];" ::"l"(colp + 31));
-                    }
+                    const double *colp = C0 + (size_t)j * lda;
 #pragma unroll
-                    for (int ib = 0; ib < 4; ++ib) { acc[jb][ib][0] = 0.0; acc[jb][ib][1] = 0.0; }
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < m && i + 1 < m) {      // 16-byte aligned: W, lda and the matrix stride are even, i is even
+                            const double2 v = *reinterpret_cast<const double2 *>(colp + i);
+                            cb[jb][ib][0] = v.x; cb[jb][ib][1] = v.y;
+                        } else {
+                            cb[jb][ib][0] = (j < m && i < m) ? colp[i] : 0.0;
+                            cb[jb][ib][1] = 0.0;
+                        }
+                        acc[jb][ib][0] = 0.0; acc[jb][ib][1] = 0.0;
+                    }
                 }
-#pragma unroll 2
+#pragma unroll 4
                 for (int c0 = 0; c0 < KB; c0 += 4) {
                     const double *pu = sU + (size_t)(c0 + k) * MWP + j0 + g;
                     const double *pl = sL + (size_t)(c0 + k) * MWP + i0 + g;
-                    double fa[4], fb[4];
+                    double fa[2], fb[4];
 #pragma unroll
-                    for (int t = 0; t < 4; ++t) { fa[t] = pu[8 * t]; fb[t] = pl[8 * t]; }
+                    for (int t = 0; t < 2; ++t) fa[t] = pu[8 * t];
 #pragma unroll
-                    for (int jb = 0; jb < 4; ++jb)
+                    for (int t = 0; t < 4; ++t) fb[t] = pl[8 * t];
+#pragma unroll
+                    for (int jb = 0; jb < 2; ++jb)
 #pragma unroll
                         for (int ib = 0; ib < 4; ++ib) dmma884(acc[jb][ib], fa[jb], fb[ib]);
                 }
 #pragma unroll
-                for (int jh = 0; jh < 4; jh += 2) {
-                    double cb[2][4][2];
+                for (int jb = 0; jb < 2; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    double *colp = C0 + (size_t)j * lda;
 #pragma unroll
-                    for (int jb = 0; jb < 2; ++jb) {
-                        const int j = j0 + 8 * (jh + jb) + g;
-                        const double *colp = C0 + (size_t)j * lda;
-#pragma unroll
-                        for (int ib = 0; ib < 4; ++ib) {
-                            const int i = i0 + 8 * ib + 2 * k;
-                            cb[jb][ib][0] = (j < m && i < m) ? colp[i] : 0.0;
-                            cb[jb][ib][1] = (j < m && i + 1 < m) ? colp[i + 1] : 0.0;
-                        }
-                    }
-#pragma unroll
-                    for (int jb = 0; jb < 2; ++jb) {
-                        const int j = j0 + 8 * (jh + jb) + g;
-                        double *colp = C0 + (size_t)j * lda;
-#pragma unroll
-                        for (int ib = 0; ib < 4; ++ib) {
-                            const int i = i0 + 8 * ib + 2 * k;
-                            if (j < m && i < m) colp[i] = cb[jb][ib][0] + acc[jh + jb][ib][0];
-                            if (j < m && i + 1 < m) colp[i + 1] = cb[jb][ib][1] + acc[jh + jb][ib][1];
-                        }
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < m && i + 1 < m)
+                            *reinterpret_cast<double2 *>(colp + i) = make_double2(cb[jb][ib][0] + acc[jb][ib][0], cb[jb][ib][1] + acc[jb][ib][1]);
+                        else if (j < m && i < m) colp[i] = cb[jb][ib][0] + acc[jb][ib][0];
                     }
                 }
             }
@@ -309,7 +305,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     extern __shared__ double smem[];
     double *x = smem;                 // [n]
     double *sD = x + n;               // [SB][SB+1]
-    const int W = bw + KB;
+    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     const int mat = blockIdx.x;       // = b * S + sp
     const double *A = band_all + (size_t)mat * mat_doubles + W;
