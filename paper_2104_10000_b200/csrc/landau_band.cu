@@ -92,7 +92,7 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
 // stored half-width: bw + KB rounded up to even (16-byte aligned column pairs in the window update)
 __host__ __device__ inline int band_halfwidth(int bw, int KB) { return (bw + KB + 1) & ~1; }
 
-int band_block(int bw) { return bw <= 416 ? 32 : (bw <= 850 ? 16 : 8); }   // panels must fit 227 KB of shared memory
+int band_block(int bw) { return bw <= 384 ? 32 : (bw <= 832 ? 16 : 8); }   // panels must fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
 // device
@@ -125,6 +125,39 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
                  : "+d"(c[0]), "+d"(c[1]) : "d"(a), "d"(b));
 }
 
+// KB x KB diagonal block at k0: loaded into shared memory, eliminated without pivoting by ONE warp (lane = row;
+// every offset is a compile-time constant, so the loads of a column step are issued together), L\U written
+// back, 1/pivots left in sDi.  A short last block is completed by the identity (no kb guards later).
+template <int KB>
+__device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0, int kb, double *sD, double *sDi, int lane) {
+    double *myrow = sD + min(lane, KB - 1) * (KB + 1);
+    const bool rowlane = lane < KB;        // KB < 32: the upper lanes only follow the warp barriers
+    if (rowlane) {
+#pragma unroll
+        for (int c = 0; c < KB; ++c)
+            myrow[c] = (lane < kb && c < kb) ? __ldcg(A + (k0 + lane) + (size_t)(k0 + c) * lda) : (lane == c ? 1.0 : 0.0);
+    }
+    __syncwarp();
+#pragma unroll
+    for (int c = 0; c < KB; ++c) {
+        const double *prow = sD + c * (KB + 1);
+        const double pinv = rcp_newton(prow[c]);
+        if (lane == c) sDi[c] = pinv;
+        if (lane > c && rowlane) {
+            const double l = myrow[c] * pinv;
+            myrow[c] = l;
+#pragma unroll
+            for (int cc = c + 1; cc < KB; ++cc) myrow[cc] = fma(-l, prow[cc], myrow[cc]);
+        }
+        __syncwarp();
+    }
+    if (lane < kb) {
+#pragma unroll
+        for (int c = 0; c < KB; ++c)
+            if (c < kb) A[(k0 + lane) + (size_t)(k0 + c) * lda] = myrow[c];
+    }
+}
+
 // Blocked outer-product band LU, one block per matrix.  Per block step of KB columns:
 //   (1) the KB x KB diagonal block is eliminated by warp 0 in shared memory (lane = row);
 //   (2) one thread per row / column forms the L panel A21 U11^-1 and the U panel L11^-1 A12 (both in the
@@ -139,64 +172,36 @@ template <int KB>
 __global__ void __launch_bounds__(BAND_THREADS)
 k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restrict__ mlow, double *__restrict__ band_all) {
     extern __shared__ double smem[];
-    double *sD = smem;                       // [KB][KB+1]
-    double *sDi = sD + KB * (KB + 1);        // [KB]
-    double *sL = sDi + KB;                   // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
+    constexpr int DSZ = KB * (KB + 1) + KB;  // one diagonal-block buffer: sD[KB][KB+1], sDi[KB]
+    double *sL = smem + 2 * DSZ;             // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
     double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;        // LD - 1
     double *A = band_all + (size_t)blockIdx.x * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, k = lane & 3;
+    // Look-ahead: the diagonal block of step s+1 lies in the first 32 x 32 entries of step s's window.  Warp 0
+    // updates those tiles first and then eliminates the next diagonal block while the other warps update the
+    // rest of the window, so the serial elimination is off the critical path (two buffers, swapped per step).
+    int cur = 0;
+    if (warp == 0) factor_diag_block<KB>(A, lda, 0, min(KB, n), smem, smem + KB * (KB + 1), lane);
     for (int k0 = 0; k0 < n; k0 += KB) {
         const int kb = min(KB, n - k0);
         const int m = mlow[k0 / KB];         // rows below / columns right of the block inside the envelope (<= bw)
-        // (1) warp 0: diagonal block, lane = row, the row in registers, pivot rows by shuffle (a short last
-        //     block is completed by the identity, so that no kb guards are needed);
-        //     meanwhile the other warps fetch the raw panel entries into shared memory
-        if (warp == 0) {
-            // rows in shared memory, one lane per row; every offset below is a compile-time constant, so the
-            // loads of a column step are issued together
-            double *myrow = sD + min(lane, KB - 1) * (KB + 1);
-            const bool rowlane = lane < KB;        // KB < 32: the upper lanes only follow the warp barriers
-            if (rowlane) {
-#pragma unroll
-                for (int c = 0; c < KB; ++c)
-                    myrow[c] = (lane < kb && c < kb) ? A[(k0 + lane) + (size_t)(k0 + c) * lda] : (lane == c ? 1.0 : 0.0);
-            }
-            __syncwarp();
-#pragma unroll
-            for (int c = 0; c < KB; ++c) {
-                const double *prow = sD + c * (KB + 1);
-                const double pinv = rcp_newton(prow[c]);
-                if (lane == c) sDi[c] = pinv;
-                if (lane > c && rowlane) {
-                    const double l = myrow[c] * pinv;
-                    myrow[c] = l;
-#pragma unroll
-                    for (int cc = c + 1; cc < KB; ++cc) myrow[cc] = fma(-l, prow[cc], myrow[cc]);
-                }
-                __syncwarp();
-            }
-            if (lane < kb) {
-#pragma unroll
-                for (int c = 0; c < KB; ++c)
-                    if (c < kb) A[(k0 + lane) + (size_t)(k0 + c) * lda] = myrow[c];
-            }
-        } else {
-            for (int i = tid - 32; i < MWP; i += BAND_THREADS - 32) {
-                if (i < m) {
-                    const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
-                    const double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
+        double *sD = smem + cur * DSZ, *sDi = sD + KB * (KB + 1);
+        // (1) raw panel entries into shared memory
+        for (int i = tid; i < MWP; i += BAND_THREADS) {
+            if (i < m) {
+                const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+                const double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
 #pragma unroll 16
-                    for (int c = 0; c < KB; ++c) {
-                        sL[(size_t)c * MWP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
-                        sU[(size_t)c * MWP + i] = c < kb ? col[c] : 0.0;
-                    }
-                } else {
-#pragma unroll
-                    for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
+                for (int c = 0; c < KB; ++c) {
+                    sL[(size_t)c * MWP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
+                    sU[(size_t)c * MWP + i] = c < kb ? col[c] : 0.0;
                 }
+            } else {
+#pragma unroll
+                for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
             }
         }
         __syncthreads();
@@ -240,7 +245,14 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
             // (32 doubles), which is fetched into registers BEFORE the mma loop and so costs no wait afterwards
             const int nti = (m + WT - 1) / WT, ntj = (m + WTJ - 1) / WTJ;
             double *C0 = A + (k0 + kb) + (size_t)(k0 + kb) * lda;
-            for (int wt = warp; wt < nti * ntj; wt += BAND_THREADS / 32) {
+            // warp 0: only the tiles that hold the next diagonal block (row tile 0, column tiles 0 and 1); the
+            // other warps share the rest
+            const int ntiles = nti * ntj, nlook = min(ntj, (KB + WTJ - 1) / WTJ);
+            constexpr int NWRK = BAND_THREADS / 32 - 1;
+            for (int u = (warp == 0 ? 0 : warp - 1); u < (warp == 0 ? nlook : ntiles - nlook); u += (warp == 0 ? 1 : NWRK)) {
+                int wt;
+                if (warp == 0) wt = u * nti;                                   // (ti = 0, tj = u)
+                else { wt = u + 1; if (nlook > 1 && wt >= nti) wt += 1; }      // skip tiles (0,0) and (0,1)
                 const int i0 = (wt % nti) * WT, j0 = (wt / nti) * WTJ;
                 // acc[jb][ib] = -(L U)(i0 + 8 ib + 2k + {0,1}, j0 + 8 jb + g)
                 double acc[2][4][2], cb[2][4][2];
@@ -289,7 +301,14 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
                 }
             }
         }
+        if (warp == 0 && k0 + kb < n) {
+            __threadfence_block();
+            __syncwarp();
+            double *sDn = smem + (cur ^ 1) * DSZ;
+            factor_diag_block<KB>(A, lda, k0 + kb, min(KB, n - k0 - kb), sDn, sDn + KB * (KB + 1), lane);
+        }
         __syncthreads();
+        cur ^= 1;
     }
 }
 
@@ -378,7 +397,7 @@ static int band_mw(int bw) { return ((std::max(bw, 1) + WT - 1) / WT) * WT + 4; 
 
 size_t band_factor_smem(int bw) {
     const int KB = band_block(bw);
-    return sizeof(double) * ((size_t)KB * (KB + 1) + KB + 2 * (size_t)KB * band_mw(bw));
+    return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + 2 * (size_t)KB * band_mw(bw));
 }
 
 int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st) {
