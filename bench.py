@@ -237,8 +237,9 @@ def run_ours(args):
     binding.lib()
     torch.cuda.set_device(local_rank)
     dist = None
-    if world > 1:
+    if world > 1 or "TORCHELASTIC_RUN_ID" in os.environ:      # launched by torchrun: same code path for every N
         import torch.distributed as dist
+        os.environ.setdefault("NCCL_DEBUG", "WARN")           # keep stdout to the one JSON line
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     wl = inputs.config(5)
