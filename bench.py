@@ -222,6 +222,34 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
                                "ms_per_step": ms, "builds_per_s": nb / (ms * 1e-3),
                                "gpair_per_s": nb * mg.N * (mg.N - 1) / (ms * 1e-3) * 1e-9}
     mg.destroy()
+    # The paper's throughput metric (Tables II/III, L246-270): Newton iterations per second on the e + D + 8 heavy
+    # ion species, 80-cell Q3 problem -- here one iteration = implicit-step operator + band LU + solve, all on the
+    # device, nb problems batched (context beside the paper's 7,005 it/s on 6 V100 + 42 P9 cores with a CPU LU).
+    wl = inputs.config(6)
+    c80 = binding.LandauContext(wl.mesh, wl.order, wl.species, nb)
+    r, z = c80.dof_coords()
+    f80 = torch.from_numpy(np.tile(inputs.nodal_f(wl, r, z), (nb, 1, 1))).cuda()
+    v80 = torch.zeros((nb, c80.S, c80.nnz), dtype=torch.float64, device="cuda")
+    F80 = torch.zeros((nb, c80.S, c80.n), dtype=torch.float64, device="cuda")
+    d80 = torch.zeros_like(F80)
+    Ez80 = torch.zeros(nb, dtype=torch.float64, device="cuda")
+    bw80, _, ws80 = c80.band_sizes()
+    band80 = torch.empty(nb * ws80, dtype=torch.float64, device="cuda")
+
+    def newton():
+        c80.implicit_operator_batched(f80, Ez80, 2.0, v80, F80)
+        c80.band_factor_batched(v80, band80)
+        c80.band_solve_batched(band80, F80, d80)
+    newton(); torch.cuda.synchronize()
+    e0.record()
+    for _ in range(5):
+        newton()
+    e1.record(); torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1) / 5
+    out["newton_iteration_ctx80"] = {"workload": f"{nb} problems x (10 species, 80 Q3 cells: N = {c80.N}, n = {c80.n}, RCM half-bandwidth {bw80})",
+                                     "ms_per_batched_iteration": ms, "newton_iterations_per_s": nb / (ms * 1e-3),
+                                     "what": "operator (shift M + A - J, A f - C(f)) + band LU of 10 species blocks + solve, per problem"}
+    c80.destroy()
     return out
 
 

@@ -88,11 +88,14 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
         for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) bw = std::max(bw, std::abs(pos[i] - pos[colidx[t]]));
 }
 
-// (16-column blocks with two blocks of 256 threads per SM were measured slower at bw = 339: 52 vs 41 ms)
 // stored half-width: bw + KB rounded up to even (16-byte aligned column pairs in the window update)
 __host__ __device__ inline int band_halfwidth(int bw, int KB) { return (bw + KB + 1) & ~1; }
 
-int band_block(int bw) { return bw <= 384 ? 32 : (bw <= 832 ? 16 : 8); }   // panels must fit 227 KB of shared memory
+// Block width and threads per matrix, by half-bandwidth (measured, 512 problems):
+//   bw = 178 (n = 745, 5,120 matrices):  KB 16 x 128 threads 17.5 ms | 16 x 256: 23.2 | 32 x 256: 29.4 | 32 x 512: 34.0
+//   bw = 339 (n = 2,767, 1,024 matrices): KB 32 x 256 threads 35.5 ms | 32 x 512: 36.5 | 32 x 128: 51.7 | 16 x 128: 56.1
+// small matrices want several blocks per SM (their steps are dominated by latencies), wide ones the longer panels.
+int band_block(int bw) { return bw <= 256 ? 16 : (bw <= 384 ? 32 : (bw <= 832 ? 16 : 8)); }   // panels must fit 227 KB of shared memory
 
 // ------------------------------------------------------------------------------------------------
 // device
@@ -108,6 +111,9 @@ __global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, cons
 }
 
 constexpr int BAND_THREADS = 512;
+// threads per matrix in the solves (measured: bw = 339: 384 threads 4.2 ms, 256: 4.8, 512: 5.8; bw = 178: 64 threads 2.5 ms,
+// 256: 3.9, 512: 7.6 -- the solves are latency-bound, small blocks leave room for more matrices per SM)
+constexpr int SOLVE_NT32 = 384, SOLVE_NT16 = 64;
 constexpr int WT = 32, WTJ = 16;   // warp tile of the window update: 32 rows x 16 columns = 4 x 2 mma tiles of 8 x 8
 
 // 1/x: MUFU seed and two Newton steps (full double precision up to rounding of the last step)
@@ -168,8 +174,8 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 // rows of one column of the column-major window.
 // Dynamic shared memory: sD[KB][KB+1], sDi[KB] (1/pivots), sL[KB][MWP], sU[KB][MWP]; MWP = bw rounded up to
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
-template <int KB>
-__global__ void __launch_bounds__(BAND_THREADS)
+template <int KB, int NT>
+__global__ void __launch_bounds__(NT)
 k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restrict__ mlow, double *__restrict__ band_all) {
     extern __shared__ double smem[];
     constexpr int DSZ = KB * (KB + 1) + KB;  // one diagonal-block buffer: sD[KB][KB+1], sDi[KB]
@@ -190,7 +196,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
         const int m = mlow[k0 / KB];         // rows below / columns right of the block inside the envelope (<= bw)
         double *sD = smem + cur * DSZ, *sDi = sD + KB * (KB + 1);
         // (1) raw panel entries into shared memory
-        for (int i = tid; i < MWP; i += BAND_THREADS) {
+        for (int i = tid; i < MWP; i += NT) {
             if (i < m) {
                 const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
                 const double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
@@ -207,7 +213,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
         __syncthreads();
         // (2) panels: thread i does row i of the L panel (x U11 = a) and column i of the U panel (L11 y = a);
         //     its entries live in shared memory (-x in sL, y in sU), not in registers
-        for (int i = tid; i < m; i += BAND_THREADS) {
+        for (int i = tid; i < m; i += NT) {
             double x[KB];
             {   // L panel row: x U11 = a
                 double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
@@ -248,7 +254,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
             // warp 0: only the tiles that hold the next diagonal block (row tile 0, column tiles 0 and 1); the
             // other warps share the rest
             const int ntiles = nti * ntj, nlook = min(ntj, (KB + WTJ - 1) / WTJ);
-            constexpr int NWRK = BAND_THREADS / 32 - 1;
+            constexpr int NWRK = NT / 32 - 1;
             for (int u = (warp == 0 ? 0 : warp - 1); u < (warp == 0 ? nlook : ntiles - nlook); u += (warp == 0 ? 1 : NWRK)) {
                 int wt;
                 if (warp == 0) wt = u * nti;                                   // (ti = 0, tj = u)
@@ -316,8 +322,8 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
 // Blocks of KB columns (those of the factorisation): the diagonal block by warp 0 (lane = row), the panel
 // below / above, confined to the envelope, by one thread per row with KB independent loads.
 
-template <int KB>
-__global__ void __launch_bounds__(BAND_THREADS)
+template <int KB, int NT>
+__global__ void __launch_bounds__(NT)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
              const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
     constexpr int SB = KB;            // same blocks as the factorisation: panels stay inside the stored band
@@ -330,12 +336,12 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     const double *A = band_all + (size_t)mat * mat_doubles + W;
     const size_t voff = (size_t)(mat / S) * xstride + (size_t)(mat % S) * n;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-    for (int i = tid; i < n; i += BAND_THREADS) x[i] = rhs[voff + perm[i]];
+    for (int i = tid; i < n; i += NT) x[i] = rhs[voff + perm[i]];
     __syncthreads();
     // forward: L y = b (unit lower)
     for (int k0 = 0; k0 < n; k0 += SB) {
         const int kb = min(SB, n - k0), m = mlow[k0 / SB];
-        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+        for (int t = tid; t < kb * kb; t += NT) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
         }
@@ -349,7 +355,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
             if (lane < kb) x[k0 + lane] = v;
         }
         __syncthreads();
-        for (int i = tid; i < m; i += BAND_THREADS) {
+        for (int i = tid; i < m; i += NT) {
             const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
             double v = x[k0 + kb + i];
 #pragma unroll 8
@@ -362,7 +368,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     const int nblk = (n + SB - 1) / SB;
     for (int blk = nblk - 1; blk >= 0; --blk) {
         const int k0 = blk * SB, kb = min(SB, n - k0), m = mup[blk];
-        for (int t = tid; t < kb * kb; t += BAND_THREADS) {
+        for (int t = tid; t < kb * kb; t += NT) {
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
         }
@@ -377,7 +383,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
             if (lane < kb) x[k0 + lane] = v;
         }
         __syncthreads();
-        for (int i = tid; i < m; i += BAND_THREADS) {
+        for (int i = tid; i < m; i += NT) {
             const int r = k0 - m + i;
             const double *row = A + r + (size_t)k0 * lda;
             double v = x[r];
@@ -387,7 +393,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
         }
         __syncthreads();
     }
-    for (int i = tid; i < n; i += BAND_THREADS) xout[voff + perm[i]] = x[i];
+    for (int i = tid; i < n; i += NT) xout[voff + perm[i]] = x[i];
 }
 
 // ------------------------------------------------------------------------------------------------
@@ -407,39 +413,39 @@ int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const d
     return 1;
 }
 
-template <int KB>
+template <int KB, int NT>
 static cudaError_t factor_t(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
     const size_t smem = band_factor_smem(bs.bw);
-    cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_factor<KB><<<nmat, BAND_THREADS, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, bs.mlow, band);
+    k_band_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, bs.mlow, band);
     return cudaSuccess;
 }
 
 cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
     switch (band_block(bs.bw)) {
-        case 32: return factor_t<32>(bs, nmat, band, st);
-        case 16: return factor_t<16>(bs, nmat, band, st);
-        default: return factor_t<8>(bs, nmat, band, st);
+        case 32: return factor_t<32, 256>(bs, nmat, band, st);
+        case 16: return bs.bw <= 256 ? factor_t<16, 128>(bs, nmat, band, st) : factor_t<16, BAND_THREADS>(bs, nmat, band, st);
+        default: return factor_t<8, BAND_THREADS>(bs, nmat, band, st);
     }
 }
 
-template <int KB>
+template <int KB, int NT>
 static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
                            cudaStream_t st) {
     const size_t smem = sizeof(double) * ((size_t)bs.n + KB * (KB + 1));
-    cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB><<<nb * S, BAND_THREADS, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, band, rhs, x);
+    k_band_solve<KB, NT><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, band, rhs, x);
     return cudaSuccess;
 }
 
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
                               cudaStream_t st) {
     switch (band_block(bs.bw)) {
-        case 32: return solve_t<32>(bs, nb, S, xstride, band, rhs, x, st);
-        case 16: return solve_t<16>(bs, nb, S, xstride, band, rhs, x, st);
-        default: return solve_t<8>(bs, nb, S, xstride, band, rhs, x, st);
+        case 32: return solve_t<32, SOLVE_NT32>(bs, nb, S, xstride, band, rhs, x, st);
+        case 16: return bs.bw <= 256 ? solve_t<16, SOLVE_NT16>(bs, nb, S, xstride, band, rhs, x, st) : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, band, rhs, x, st);
+        default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, band, rhs, x, st);
     }
 }
 
