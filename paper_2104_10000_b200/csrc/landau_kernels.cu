@@ -507,7 +507,7 @@ constexpr int ELQ3_WARPS = 4;    // cells per block and round
 
 template <bool FULL>
 __global__ void __launch_bounds__(ELQ3_WARPS * 32)
-k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
+k_element_q3(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
              double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y;
@@ -528,18 +528,25 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
     if (e >= ds.Ne) return;
     // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
     const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1];
-    const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
+    // jsplit == 1: Gsum holds the tile-order sum; jsplit > 1: the pair kernel's slabs are summed here, in the
+    // same order and with the same additions as k_sum_partials (small batches: one launch less)
     double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
         const int q = 4 * ks + k;
+        double gs[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
+        for (int js = 0; js < jsplit; ++js) {
+            const double *G = Gsum + ((size_t)b * jsplit + js) * 5 * ds.Ntot + ds.poff + e * 16;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) gs[c] += G[(size_t)c * ds.Ntot + q];
+        }
         const double w = ds.w_out[e * 16 + q];
         wq[ks] = w;
-        g0[ks] = ir * ir * w * G[q];
-        g1[ks] = ir * iz * w * G[ds.Ntot + q];
-        g2[ks] = iz * iz * w * G[2 * ds.Ntot + q];
-        g3[ks] = ir * w * G[3 * ds.Ntot + q];
-        g4[ks] = iz * w * G[4 * ds.Ntot + q];
+        g0[ks] = ir * ir * w * gs[0];
+        g1[ks] = ir * iz * w * gs[1];
+        g2[ks] = iz * iz * w * gs[2];
+        g3[ks] = ir * w * gs[3];
+        g4[ks] = iz * w * gs[4];
     }
     for (int sp = 0; sp < ds.S; ++sp) {
         // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in)
@@ -683,15 +690,39 @@ int launch_pair(int Ntot, const double *r, const double *z, const double *invr, 
 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    const double *Ez, double shift, cudaStream_t st) {
-    if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
+    if (ds.Nb == 16) {   // Q3: FP64 tensor cores, warp per cell
         dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
-        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, Ez, shift);
-        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, nullptr, 0.0);
+        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
+        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
         return 1;
     }
     dim3 grid(ds.Ne, nb);
     if (Ez) k_element<true><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
     else k_element<false><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
+    return 1;
+}
+
+// both gathers of a build in one launch: blocks [0, bv) of grid.x do the CSR values, the rest C(f)
+__global__ void k_gather2(DeviceSpace ds, int bv, size_t vstride, size_t fstride, const double *__restrict__ Ce,
+                          const double *__restrict__ ce, double *__restrict__ vals, double *__restrict__ Cf) {
+    const bool isv = (int)blockIdx.x < bv;
+    const int K = isv ? ds.nnz : ds.n;
+    const int kk = (isv ? blockIdx.x : blockIdx.x - bv) * blockDim.x + threadIdx.x;
+    if (kk >= K) return;
+    const int32_t *ptr = isv ? ds.gptr : ds.cptr, *idx = isv ? ds.gidx : ds.cidx;
+    const double *w = isv ? ds.gw : ds.cw;
+    const size_t stride = isv ? (size_t)ds.Ne * ds.Nb * ds.Nb : (size_t)ds.Ne * ds.Nb;
+    const double *s = (isv ? Ce : ce) + ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * stride;
+    double acc = 0.0;
+    for (int t = ptr[kk]; t < ptr[kk + 1]; ++t) acc = fma(w[t], s[idx[t]], acc);
+    (isv ? vals : Cf)[(size_t)blockIdx.z * (isv ? vstride : fstride) + (size_t)blockIdx.y * K + kk] = acc;
+}
+
+int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fstride, const double *Ce, const double *ce,
+                       double *vals, double *Cf, cudaStream_t st) {
+    const int bv = (ds.nnz + 255) / 256, bc = (ds.n + 255) / 256;
+    dim3 grid(bv + bc, ds.S, nb);
+    k_gather2<<<grid, 256, 0, st>>>(ds, bv, vstride, fstride, Ce, ce, vals, Cf);
     return 1;
 }
 

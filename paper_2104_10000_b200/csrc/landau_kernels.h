@@ -53,6 +53,8 @@ int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, c
 // nspecies = 1 with ostride 0 gathers a single matrix (mass)
 int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st);
 int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st);
+int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fstride, const double *Ce, const double *ce,
+                       double *vals, double *Cf, cudaStream_t st);
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
 int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
