@@ -159,8 +159,28 @@ def time_single_config(binding, inputs, torch, k, variant="B", reps=20):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1) / reps
     pair_ms, cnt = ctx.profile_read()
+    ctx.profile_enable(False)
+    # the same build captured once in a CUDA graph and replayed (the library makes no synchronising call)
+    graph_ms = None
+    try:
+        side = torch.cuda.Stream()
+        with torch.cuda.stream(side):
+            ctx.jacobian(f, vals, Cf)
+            torch.cuda.synchronize()
+            g = torch.cuda.CUDAGraph()
+            with torch.cuda.graph(g, stream=side):
+                ctx.jacobian(f, vals, Cf)
+            g.replay()
+            e0.record()
+            for _ in range(reps):
+                g.replay()
+            e1.record()
+            torch.cuda.synchronize()
+            graph_ms = e0.elapsed_time(e1) / reps
+    except Exception as exc:   # reported, not fatal
+        graph_ms = f"unavailable: {exc}"
     pairs = ctx.N * (ctx.N - 1)
-    out = {"config": wl.name, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz, "ms_per_build": ms,
+    out = {"config": wl.name, "graph_replay_ms_per_build": graph_ms, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz, "ms_per_build": ms,
            "builds_per_s": 1e3 / ms, "gpair_per_s": pairs / (ms * 1e-3) * 1e-9,
            "pair_kernel_ms": pair_ms / max(cnt, 1), "pair_kernel_gpair_per_s": pairs / (pair_ms / max(cnt, 1) * 1e-3) * 1e-9}
     ctx.destroy()
