@@ -214,35 +214,25 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
         // (2) panels: thread i does row i of the L panel (x U11 = a) and column i of the U panel (L11 y = a);
         //     its entries live in shared memory (-x in sL, y in sU), not in registers
         for (int i = tid; i < m; i += NT) {
-            double x[KB];
-            {   // L panel row: x U11 = a
-                double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+            // two independent substitution chains per thread, interleaved: x U11 = a (L row), L11 y = a (U column)
+            double x[KB], y[KB];
+            double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
+            double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
 #pragma unroll
-                for (int c = 0; c < KB; ++c) x[c] = sL[(size_t)c * MWP + i];
+            for (int c = 0; c < KB; ++c) { x[c] = sL[(size_t)c * MWP + i]; y[c] = sU[(size_t)c * MWP + i]; }
 #pragma unroll
-                for (int c = 0; c < KB; ++c) {
-                    double v = x[c];
+            for (int c = 0; c < KB; ++c) {
+                double v = x[c], w = y[c];
 #pragma unroll
-                    for (int cc = 0; cc < c; ++cc) v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
-                    v *= sDi[c];
-                    x[c] = v;
-                    if (c < kb) row[(size_t)c * lda] = v;
-                    sL[(size_t)c * MWP + i] = -v;
+                for (int cc = 0; cc < c; ++cc) {
+                    v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
+                    w = fma(-sD[c * (KB + 1) + cc], y[cc], w);
                 }
-            }
-            {   // U panel column: L11 y = a
-                double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
-#pragma unroll
-                for (int c = 0; c < KB; ++c) x[c] = sU[(size_t)c * MWP + i];
-#pragma unroll
-                for (int c = 0; c < KB; ++c) {
-                    double w = x[c];
-#pragma unroll
-                    for (int cc = 0; cc < c; ++cc) w = fma(-sD[c * (KB + 1) + cc], x[cc], w);
-                    x[c] = w;
-                    if (c < kb) col[c] = w;
-                    sU[(size_t)c * MWP + i] = w;
-                }
+                v *= sDi[c];
+                x[c] = v; y[c] = w;
+                if (c < kb) { row[(size_t)c * lda] = v; col[c] = w; }
+                sL[(size_t)c * MWP + i] = -v;
+                sU[(size_t)c * MWP + i] = w;
             }
         }
         __syncthreads();
