@@ -97,28 +97,28 @@ int timed_pair(landau_ctx *ctx, int nb, double *G, cudaStream_t st) {
     return k;
 }
 
-// (Summing the pair kernel's slabs inside the element kernel for small batches, to save a launch, was measured
-// slower: N = 2048 single build 68 -> 88 us; the separate, fully parallel k_sum_partials stays.)
-constexpr int FUSE_SLAB_SUM_MAX_NB = 0;
-
-// a1-a3 for nb problems: fields + beta sums per grid, pair kernel over the union, tile-order sum (Gsum != null)
+// a1-a3 for nb problems: fields + beta sums per grid, pair kernel over the union, tile-order sum
 void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, cudaStream_t st) {
     for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nb, f_dev + g.foff, ctx->sc.T, st);
     ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
-    if (Gsum) ctx->launches += launch_sum_partials(int(ctx->Ntot), nb, pair_tiles(int(ctx->Ntot)), ctx->sc.G, Gsum, st);
+    ctx->launches += launch_sum_partials(int(ctx->Ntot), nb, pair_tiles(int(ctx->Ntot)), ctx->sc.G, Gsum, st);
 }
 
+// Small batches are launch-latency bound: both gathers then go in one launch (3-7 us per single build); large
+// batches keep the two launches (the merged kernel is 10 % slower there).
+constexpr int MERGED_GATHER_MAX_NB = 8;
+
 // a4-a7 for nb problems; Ez == nullptr: collision Jacobian and C(f), else the implicit-step operator
-void assemble(landau_ctx *ctx, int nb, bool slabs, const double *f_dev, const double *Ez, double shift, double *vals_dev,
-              double *Cf_dev, cudaStream_t st) {
-    const int jsplit = slabs ? pair_tiles(int(ctx->Ntot)) : 1;
-    const double *G = slabs ? ctx->sc.G : ctx->sc.Gsum;
+void assemble(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez, double shift, double *vals_dev, double *Cf_dev,
+              cudaStream_t st) {
     for (auto &g : ctx->grids) {
-        ctx->launches += launch_element(g.ds, nb, jsplit, f_dev + g.foff, G, g.Ce, g.ce, Ez, shift, st);
-        if (vals_dev && Cf_dev)
+        ctx->launches += launch_element(g.ds, nb, 1, f_dev + g.foff, ctx->sc.Gsum, g.Ce, g.ce, Ez, shift, st);
+        if (vals_dev && Cf_dev && nb <= MERGED_GATHER_MAX_NB) {
             ctx->launches += launch_gather_both(g.ds, nb, ctx->vstride, ctx->fstride, g.Ce, g.ce, vals_dev + g.voff, Cf_dev + g.foff, st);
-        else if (vals_dev) ctx->launches += launch_gather_vals(g.ds, nb, g.ds.S, ctx->vstride, g.Ce, vals_dev + g.voff, st);
-        else if (Cf_dev) ctx->launches += launch_gather_cf(g.ds, nb, ctx->fstride, g.ce, Cf_dev + g.foff, st);
+            continue;
+        }
+        if (vals_dev) ctx->launches += launch_gather_vals(g.ds, nb, g.ds.S, ctx->vstride, g.Ce, vals_dev + g.voff, st);
+        if (Cf_dev) ctx->launches += launch_gather_cf(g.ds, nb, ctx->fstride, g.ce, Cf_dev + g.foff, st);
     }
 }
 
@@ -452,9 +452,8 @@ int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *
 int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double *vals_dev, double *Cf_dev, void *stream) {
     if (!ctx || !f_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool slabs = nb <= FUSE_SLAB_SUM_MAX_NB;
-    inner_integral(ctx, nb, f_dev, slabs ? nullptr : ctx->sc.Gsum, st);
-    assemble(ctx, nb, slabs, f_dev, nullptr, 0.0, vals_dev, Cf_dev, st);
+    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+    assemble(ctx, nb, f_dev, nullptr, 0.0, vals_dev, Cf_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }
@@ -463,9 +462,8 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
                                      double *vals_dev, double *F_dev, void *stream) {
     if (!ctx || !f_dev || !Ez_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    const bool slabs = nb <= FUSE_SLAB_SUM_MAX_NB;
-    inner_integral(ctx, nb, f_dev, slabs ? nullptr : ctx->sc.Gsum, st);
-    assemble(ctx, nb, slabs, f_dev, Ez_dev, shift, vals_dev, F_dev, st);
+    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+    assemble(ctx, nb, f_dev, Ez_dev, shift, vals_dev, F_dev, st);
     CK(cudaGetLastError());
     return LANDAU_OK;
 }

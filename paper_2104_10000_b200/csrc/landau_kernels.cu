@@ -507,7 +507,7 @@ constexpr int ELQ3_WARPS = 4;    // cells per block and round
 
 template <bool FULL>
 __global__ void __launch_bounds__(ELQ3_WARPS * 32)
-k_element_q3(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
+k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
              double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y;
@@ -528,25 +528,19 @@ k_element_q3(DeviceSpace ds, int jsplit, const double *__restrict__ f, const dou
     if (e >= ds.Ne) return;
     // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
     const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1];
-    // jsplit == 1: Gsum holds the tile-order sum; jsplit > 1: the pair kernel's slabs are summed here, in the
-    // same order and with the same additions as k_sum_partials (small batches: one launch less)
+    // (summing the pair kernel's slabs here instead of in k_sum_partials was measured slower for every batch size)
+    const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
     double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
 #pragma unroll
     for (int ks = 0; ks < 4; ++ks) {
         const int q = 4 * ks + k;
-        double gs[5] = {0.0, 0.0, 0.0, 0.0, 0.0};
-        for (int js = 0; js < jsplit; ++js) {
-            const double *G = Gsum + ((size_t)b * jsplit + js) * 5 * ds.Ntot + ds.poff + e * 16;
-#pragma unroll
-            for (int c = 0; c < 5; ++c) gs[c] += G[(size_t)c * ds.Ntot + q];
-        }
         const double w = ds.w_out[e * 16 + q];
         wq[ks] = w;
-        g0[ks] = ir * ir * w * gs[0];
-        g1[ks] = ir * iz * w * gs[1];
-        g2[ks] = iz * iz * w * gs[2];
-        g3[ks] = ir * w * gs[3];
-        g4[ks] = iz * w * gs[4];
+        g0[ks] = ir * ir * w * G[q];
+        g1[ks] = ir * iz * w * G[ds.Ntot + q];
+        g2[ks] = iz * iz * w * G[2 * ds.Ntot + q];
+        g3[ks] = ir * w * G[3 * ds.Ntot + q];
+        g4[ks] = iz * w * G[4 * ds.Ntot + q];
     }
     for (int sp = 0; sp < ds.S; ++sp) {
         // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in)
@@ -690,10 +684,10 @@ int launch_pair(int Ntot, const double *r, const double *z, const double *invr, 
 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    const double *Ez, double shift, cudaStream_t st) {
-    if (ds.Nb == 16) {   // Q3: FP64 tensor cores, warp per cell
+    if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
         dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
-        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
-        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
+        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, Ez, shift);
+        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, nullptr, 0.0);
         return 1;
     }
     dim3 grid(ds.Ne, nb);
