@@ -279,6 +279,20 @@ def test_band_lu_wide_band_uses_the_16_column_blocks(gpu):
     assert np.abs(xg - xs).max() <= 1e-8 * np.abs(xs).max()
 
 
+def test_deeply_refined_mesh_parity(gpu, oracle):
+    """Six refinement levels toward the origin (cells from 2 down to 0.03, Gauss points 2e-3 from the axis, cell size
+    ratios 64:1 across hanging-node chains): near pairs with k' = d/sqrt(s) ~ 1e-3 need the most AGM passes, far /
+    near-axis pairs the small-m accuracy.  Cold electrons + ions resolved only by the finest cells."""
+    mesh = inputs.mesh_quadtree(0.0, 8.0, -8.0, 8.0, 4, 8, 0.3, 6, 1.5, 3)
+    spc = inputs._sp([(1, -1, 1, 0.01), (3670, 1, 1, 0.01)])
+    comps = [[inputs.Component(0, 0.98, 0.01), inputs.Component(0, 0.02, 1.0, 0.5), inputs.Component(1, 1.0, 20.0)]]
+    wl = inputs.Workload("deep-refined-q3", 3, mesh, spc, comps, 1e-3, 13)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    assert ctx.Ne == 332
+    worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    print(f"{wl.name}: worst block error {worst:.2e}")
+
+
 def test_edge_cases_of_the_next_rows(gpu, oracle):
     """One-cell mesh through the implicit operator and the band LU (n = 9 < one elimination block); NULL outputs;
     argument errors of the multigrid constructor."""
