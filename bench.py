@@ -33,17 +33,17 @@ METRIC = "landau_jacobian_gpair_evals_per_s"
 UNIT = "GPair/s"
 WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
 # FP64 flop (2 DFMA + DMUL + DADD) and FP64-pipe instructions the pair kernel executes per ORDERED
-# pair on this workload, ncu-counted (profiles/r01c_pair_kernel.md).
-FLOP_PER_PAIR = 77.33
-FP64_INST_PER_PAIR = 50.05
+# pair on this workload, ncu-counted (profiles/r01e_pair_kernel.md).
+FLOP_PER_PAIR = 75.27
+FP64_INST_PER_PAIR = 48.51
 # of which DFMAs with three distinct register operands: they issue in 3 cycles instead of 2
-# (measured), so the issue-cycle cost per ordered pair is 2 x 50.05 + 11.08 SMSP-cycles x 32 lanes.
-FP64_3OP_INST_PER_PAIR = 11.08
+# (measured), so the issue-cycle cost per ordered pair is 2 x 48.51 + 11.09 SMSP-cycles x 32 lanes.
+FP64_3OP_INST_PER_PAIR = 11.09
 FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
 # dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_sym launch on this workload, from the
-# ncu --set full capture summarised in profiles/r01c_pair_kernel.md (73.9 MB read + 3.880 GB written:
+# ncu --set full capture summarised in profiles/r01e_pair_kernel.md (68.7 MB read + 3.879 GB written:
 # the per-source-tile partial slabs; the algorithmic minimum is 24 B/point in + 40 B/point out = 0.16 GB).
-PAIR_KERNEL_DRAM_BYTES = 73.9e6 + 3.8797e9
+PAIR_KERNEL_DRAM_BYTES = 68.7e6 + 3.8789e9
 # the same for the rest of the step (fields, slab sum, element matrices, two gathers), profiles/r01e_step_kernels.md (ncu --set full, dram read + write)
 REST_DRAM_BYTES = 6.03e9   # 4.04 GB of it is k_sum_partials reading the slabs
 
