@@ -18,6 +18,26 @@
 
 namespace landau {
 
+// Programmatic dependent launch (small batches only, see launch_k): lets the next kernel of the chain be
+// scheduled while this one runs; every kernel waits here for its predecessor's results before touching memory.
+// Both instructions do nothing in a launch without the attribute.
+__device__ __forceinline__ void pdl_prologue() {
+    asm volatile("griddepcontrol.launch_dependents;");
+    asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
+template <class... KArgs, class... Args>
+static void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool pdl, Args... args) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = st;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+    attr[0].val.programmaticStreamSerializationAllowed = 1;
+    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
+    cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
+}
+constexpr int PDL_MAX_NB = 8;   // launch-latency bound batches
+
 // ------------------------------------------------------------------------------------------------
 // fast fp64 reciprocal / square roots: MUFU seed (relative error < 2^-19 including the truncation
 // of the operand to its high word) + ONE cubic correction on the DFMA pipe (error ~ seed^3 < 1e-17).
@@ -246,6 +266,7 @@ template <int TS, int IPT, bool CHECK_ALL>
 __global__ void __launch_bounds__(TS / IPT, PAIR_MIN_BLOCKS)
 k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
            const double *__restrict__ T, double *__restrict__ Gpart) {
+    pdl_prologue();
     constexpr int NT = TS / IPT;         // threads
     constexpr int NW = NT / 32;          // warps
     static_assert(NT % 32 == 0 && NW >= 1, "whole warps");
@@ -367,6 +388,7 @@ constexpr int FIELD_EPB = 8;
 constexpr int FIELD_ROUNDS = 4;   // cells per thread: the tabulation rows stay in registers across them
 
 __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, double *__restrict__ T) {
+    pdl_prologue();
     __shared__ double s_u[FIELD_EPB][16];
     const int b = blockIdx.y;
     const int q = threadIdx.x;
@@ -435,6 +457,7 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
 template <bool FULL>
 __global__ void k_element(DeviceSpace ds, int jsplit, const double *__restrict__ f, const double *__restrict__ Gpart,
                           double *__restrict__ Ce, double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
+    pdl_prologue();
     __shared__ double s_g[16][5];      // w_out * (invJ-transformed G_D rr, rz, zz, G_K r, z), species-independent
     __shared__ double s_w[16];         // w_out (FULL only)
     __shared__ double s_B[256], s_E0[256], s_E1[256], s_X[256], s_Y[256], s_Ce[256], s_u[16];
@@ -528,6 +551,7 @@ template <bool FULL>
 __global__ void __launch_bounds__(ELQ3_WARPS * 32)
 k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
              double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
+    pdl_prologue();
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y;
     const int k = lane & 3, g = lane >> 2;
@@ -638,6 +662,7 @@ __global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict_
 // problem b's outputs start at out + b*ostride.
 __global__ void k_gather(int K, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
                          const double *__restrict__ w, const double *__restrict__ src, double *__restrict__ out) {
+    pdl_prologue();
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= K) return;
     const double *s = src + ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * stride;
@@ -648,6 +673,7 @@ __global__ void k_gather(int K, size_t stride, size_t ostride, const int32_t *__
 
 // Sums the j-split partials (used by landau_inner_integral when jsplit > 1).  grid over 5N x nb.
 __global__ void k_sum_partials(int n5, int jsplit, const double *__restrict__ Gpart, double *__restrict__ G) {
+    pdl_prologue();
     const int t = blockIdx.x * blockDim.x + threadIdx.x;
     if (t >= n5) return;
     const size_t b = blockIdx.y;
@@ -680,7 +706,7 @@ int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
     constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
     dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
-    k_fields_beta<<<grid, block, 0, st>>>(ds, f, T);
+    launch_k(k_fields_beta, grid, block, st, nb <= PDL_MAX_NB, ds, f, T);
     return 1;
 }
 
@@ -689,9 +715,10 @@ static void launch_pair_t(int N, const double *r, const double *z, const double 
                           cudaStream_t st) {
     const int ts = pair_tile_size(N), nt = pair_tiles(N);
     dim3 grid(nt * (nt + 1) / 2, nb);
-    if (ts == 128) k_pair_sym<128, 2, CHECK_ALL><<<grid, 64, 0, st>>>(N, nt, r, z, invr, T, Gpart);
-    else if (ts == 64) k_pair_sym<64, 2, CHECK_ALL><<<grid, 32, 0, st>>>(N, nt, r, z, invr, T, Gpart);
-    else k_pair_sym<32, 1, CHECK_ALL><<<grid, 32, 0, st>>>(N, nt, r, z, invr, T, Gpart);
+    const bool pdl = nb <= PDL_MAX_NB;
+    if (ts == 128) launch_k(k_pair_sym<128, 2, CHECK_ALL>, grid, dim3(64), st, pdl, N, nt, r, z, invr, T, Gpart);
+    else if (ts == 64) launch_k(k_pair_sym<64, 2, CHECK_ALL>, grid, dim3(32), st, pdl, N, nt, r, z, invr, T, Gpart);
+    else launch_k(k_pair_sym<32, 1, CHECK_ALL>, grid, dim3(32), st, pdl, N, nt, r, z, invr, T, Gpart);
 }
 
 int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
@@ -705,19 +732,20 @@ int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, c
                    const double *Ez, double shift, cudaStream_t st) {
     if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
         dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
-        if (Ez) k_element_q3<true><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, Ez, shift);
-        else k_element_q3<false><<<grid, ELQ3_WARPS * 32, 0, st>>>(ds, f, G, Ce, ce, nullptr, 0.0);
+        if (Ez) launch_k(k_element_q3<true>, grid, dim3(ELQ3_WARPS * 32), st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, Ez, shift);
+        else launch_k(k_element_q3<false>, grid, dim3(ELQ3_WARPS * 32), st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, (const double *)nullptr, 0.0);
         return 1;
     }
     dim3 grid(ds.Ne, nb);
-    if (Ez) k_element<true><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, Ez, shift);
-    else k_element<false><<<grid, ds.Nb * ds.Nb, 0, st>>>(ds, jsplit, f, G, Ce, ce, nullptr, 0.0);
+    if (Ez) launch_k(k_element<true>, grid, dim3(ds.Nb * ds.Nb), st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, Ez, shift);
+    else launch_k(k_element<false>, grid, dim3(ds.Nb * ds.Nb), st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, (const double *)nullptr, 0.0);
     return 1;
 }
 
 // both gathers of a build in one launch: blocks [0, bv) of grid.x do the CSR values, the rest C(f)
 __global__ void k_gather2(DeviceSpace ds, int bv, size_t vstride, size_t fstride, const double *__restrict__ Ce,
                           const double *__restrict__ ce, double *__restrict__ vals, double *__restrict__ Cf) {
+    pdl_prologue();
     const bool isv = (int)blockIdx.x < bv;
     const int K = isv ? ds.nnz : ds.n;
     const int kk = (isv ? blockIdx.x : blockIdx.x - bv) * blockDim.x + threadIdx.x;
@@ -735,7 +763,7 @@ int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fst
                        double *vals, double *Cf, cudaStream_t st) {
     const int bv = (ds.nnz + 255) / 256, bc = (ds.n + 255) / 256;
     dim3 grid(bv + bc, ds.S, nb);
-    k_gather2<<<grid, 256, 0, st>>>(ds, bv, vstride, fstride, Ce, ce, vals, Cf);
+    launch_k(k_gather2, grid, dim3(256), st, nb <= PDL_MAX_NB, ds, bv, vstride, fstride, Ce, ce, vals, Cf);
     return 1;
 }
 
@@ -759,7 +787,7 @@ int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStr
 int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
     const int n5 = 5 * Ntot;
     dim3 grid((n5 + 255) / 256, nb);
-    k_sum_partials<<<grid, 256, 0, st>>>(n5, jsplit, Gpart, G);
+    launch_k(k_sum_partials, grid, dim3(256), st, nb <= PDL_MAX_NB, n5, jsplit, Gpart, G);
     return 1;
 }
 
