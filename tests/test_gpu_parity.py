@@ -381,6 +381,33 @@ def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu):
     assert np.array_equal(v1, v3) and np.array_equal(c1, c3)      # batch shape == split shape, bitwise
 
 
+def test_no_state_carried_between_calls(gpu):
+    """A, then a different problem and a different batch size, then A again in the same context: bitwise the
+    same A (nothing is read from scratch that the call itself did not write); also through the implicit
+    operator and the band LU, whose workspace is poisoned with NaN in between."""
+    import torch
+    wl = inputs.config(5, nbatch=6, variant="A")
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 6)
+    r, z = ctx.dof_coords()
+    f = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in range(6)])).cuda()
+
+    def build(fb):
+        nb = fb.shape[0]
+        v = torch.full((nb, ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+        c = torch.full((nb, ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+        ctx.implicit_operator_batched(fb, torch.full((nb,), 0.2, dtype=torch.float64, device="cuda"), 3.0, v, c)
+        band = torch.full((nb * ctx.band_sizes()[2],), float("nan"), dtype=torch.float64, device="cuda")
+        ctx.band_factor_batched(v, band)
+        x = torch.full_like(c, float("nan"))
+        ctx.band_solve_batched(band, c, x)
+        return v, c, x
+    a1 = build(f[:2])
+    build(7.0 * f[1:6])
+    a2 = build(f[:2])
+    for p, q in zip(a1, a2):
+        assert torch.isfinite(p).all() and torch.equal(p, q)
+
+
 def test_host_entry_point_equals_device_entry_point(gpu):
     import torch
     wl = inputs.config(5, nbatch=3, variant="A")
