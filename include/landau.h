@@ -42,7 +42,14 @@
  * stream) and do NOT synchronise; inputs are never modified; the CALLER owns f/vals/Cf/mvals,
  * the ctx owns pattern, gather lists, point arrays and scratch.  A ctx must not be used from two
  * streams at once (it owns one scratch arena).  There is no CPU fallback: without a CUDA device
- * landau_create fails with LANDAU_ECUDA.
+ * landau_create fails with LANDAU_ECUDA.  The device entry points make no synchronising call and allocate
+ * nothing, so a build can be captured in a CUDA graph; results are bitwise reproducible and a batched call
+ * equals the same problems built one by one.
+ *
+ * Beyond a1-a8: the operator of a fully implicit step in one pass (landau_implicit_operator_batched:
+ * E-field advection of Eq. 4 and the shifted mass matrix added), several grids for species clustered by
+ * thermal speed (landau_create_multigrid, section III-C), and the per-species batched band LU of section
+ * III-G (landau_band_*), so that a Newton iteration can stay on the device.
  */
 #ifndef LANDAU_H
 #define LANDAU_H
