@@ -658,17 +658,28 @@ __global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict_
 }
 
 // a6 / a7: out[b][sp][k] = sum_{t in [ptr[k], ptr[k+1])} w[t] * src[(b*S+sp)*stride + idx[t]], fixed order
-// (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), S, nb);
+// (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), ceil(S/2), nb);
 // problem b's outputs start at out + b*ostride.
-__global__ void k_gather(int K, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+__global__ void k_gather(int K, int S, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
                          const double *__restrict__ w, const double *__restrict__ src, double *__restrict__ out) {
     pdl_prologue();
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= K) return;
-    const double *s = src + ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * stride;
-    double acc = 0.0;
-    for (int t = ptr[k]; t < ptr[k + 1]; ++t) acc = fma(w[t], s[idx[t]], acc);
-    out[(size_t)blockIdx.z * ostride + (size_t)blockIdx.y * K + k] = acc;
+    // the lists are the same for every species: one walk serves two species blocks (blockIdx.y = species pair)
+    const int sp0 = 2 * blockIdx.y;
+    const bool two = sp0 + 1 < S;
+    const double *s0 = src + ((size_t)blockIdx.z * S + sp0) * stride;
+    const double *s1 = s0 + (two ? stride : 0);
+    double acc0 = 0.0, acc1 = 0.0;
+    for (int t = ptr[k]; t < ptr[k + 1]; ++t) {
+        const double wt = w[t];
+        const int it = idx[t];
+        acc0 = fma(wt, s0[it], acc0);
+        acc1 = fma(wt, s1[it], acc1);
+    }
+    double *o = out + (size_t)blockIdx.z * ostride + (size_t)sp0 * K + k;
+    o[0] = acc0;
+    if (two) o[K] = acc1;
 }
 
 // Sums the j-split partials (used by landau_inner_integral when jsplit > 1).  grid over 5N x nb.
@@ -768,14 +779,14 @@ int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fst
 }
 
 int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st) {
-    dim3 grid((ds.nnz + 255) / 256, nspecies, nb);
-    k_gather<<<grid, 256, 0, st>>>(ds.nnz, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
+    dim3 grid((ds.nnz + 255) / 256, (nspecies + 1) / 2, nb);
+    k_gather<<<grid, 256, 0, st>>>(ds.nnz, nspecies, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
     return 1;
 }
 
 int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st) {
-    dim3 grid((ds.n + 255) / 256, ds.S, nb);
-    k_gather<<<grid, 256, 0, st>>>(ds.n, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
+    dim3 grid((ds.n + 255) / 256, (ds.S + 1) / 2, nb);
+    k_gather<<<grid, 256, 0, st>>>(ds.n, ds.S, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
     return 1;
 }
 
