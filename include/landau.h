@@ -170,6 +170,11 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
  *   -> factors in band_dev.
  * landau_band_solve_batched: rhs_dev, x_dev [nb][f_stride] (layout of f); x = A^-1 rhs per species block;
  *   x_dev may equal rhs_dev.  Both are asynchronous on `stream` and deterministic. */
+/* Host-only (no CUDA device needed): the RCM order landau_create computes for this mesh and order --
+ * perm_host[n] (new index -> unknown), the half-bandwidth it gives, the block width the factorisation will
+ * use and the flop of its outer-product updates inside the envelope.  Any output may be NULL. */
+int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_host, int32_t *half_bandwidth,
+                           int32_t *block_columns, double *flop_per_factorization);
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
                       int64_t *workspace_doubles_per_problem, double *flop_per_factorization);
 int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, void *stream);

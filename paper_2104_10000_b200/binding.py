@@ -57,6 +57,7 @@ SIGNATURES = {
     "landau_jacobian_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_mass": (c_int, [c_void_p, c_double, c_void_p, c_void_p]),
     "landau_implicit_operator_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
+    "landau_band_order_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32), POINTER(c_double)]),
     "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
     "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
@@ -130,6 +131,18 @@ def landau_setup_host(mesh, order: int):
     _check(L.landau_setup_host(ctypes.byref(m), order, None, None, None, rowptr.ctypes.data_as(POINTER(c_int32)),
                                colidx.ctypes.data_as(POINTER(c_int32)), _dp(dr), _dp(dz)))
     return dict(n=n.value, nnz=nnz.value, N=N.value, rowptr=rowptr, colidx=colidx, dof_r=dr, dof_z=dz)
+
+
+def landau_band_order_host(mesh, order: int):
+    """Host-only: dict(perm, bw, block_columns, flop) of the band LU's RCM order for this mesh."""
+    L = lib()
+    m, keep = _mesh_struct(mesh)
+    n = landau_setup_host(mesh, order)["n"]
+    perm = np.zeros(n, np.int32)
+    bw, kb, fl = c_int32(), c_int32(), c_double()
+    _check(L.landau_band_order_host(ctypes.byref(m), order, perm.ctypes.data_as(POINTER(c_int32)), ctypes.byref(bw), ctypes.byref(kb),
+                                    ctypes.byref(fl)))
+    return dict(perm=perm, bw=bw.value, block_columns=kb.value, flop=fl.value)
 
 
 def landau_fp64_peak_probe(iters: int = 1 << 16):

@@ -351,6 +351,43 @@ int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *n
     return LANDAU_OK;
 }
 
+int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_host, int32_t *half_bandwidth,
+                           int32_t *block_columns, double *flop_per_factorization) {
+    if (!mesh) return LANDAU_EINVAL;
+    HostSpace hs;
+    std::string err;
+    int rc;
+    try {
+        rc = build_host_space(*mesh, order, hs, err);
+    } catch (const std::bad_alloc &) {
+        return LANDAU_ENOMEM;
+    }
+    if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
+    std::vector<int32_t> perm;
+    int bw = 0;
+    rcm_order(int(hs.n), hs.rowptr, hs.colidx, perm, bw);
+    if (perm_host) std::memcpy(perm_host, perm.data(), perm.size() * sizeof(int32_t));
+    if (half_bandwidth) *half_bandwidth = bw;
+    const int KBs = band_block(bw);
+    if (block_columns) *block_columns = KBs;
+    if (flop_per_factorization) {      // the envelope work of landau_create, recomputed from the order
+        std::vector<int32_t> pos(hs.n), first(hs.n), last_with_first(hs.n + 1, 0);
+        for (int64_t i = 0; i < hs.n; ++i) { pos[perm[i]] = int32_t(i); first[i] = int32_t(i); }
+        for (int64_t i = 0; i < hs.n; ++i)
+            for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) first[pos[i]] = std::min(first[pos[i]], pos[hs.colidx[t]]);
+        for (int64_t i = 0; i < hs.n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], int32_t(i));
+        for (int64_t j = 1; j < hs.n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
+        double work = 0.0;
+        for (int k0 = 0; k0 < int(hs.n); k0 += KBs) {
+            const int ke = std::min<int>(k0 + KBs, int(hs.n)) - 1;
+            const double m = std::max(0, last_with_first[ke] - ke);
+            work += 2.0 * (ke - k0 + 1) * m * m;
+        }
+        *flop_per_factorization = work;
+    }
+    return LANDAU_OK;
+}
+
 int landau_grid_count(const landau_ctx *ctx, int32_t *ngrids) {
     if (!ctx || !ngrids) return LANDAU_EINVAL;
     *ngrids = int32_t(ctx->grids.size());
