@@ -111,3 +111,22 @@ def test_band_order_is_a_valid_bandwidth_reducing_permutation(binding, cfg):
         assert bo["bw"] < 0.5 * bw_natural
     assert bo["block_columns"] in (8, 16, 32)
     assert 0 < bo["flop"] <= 2.0 * n * bo["bw"] ** 2
+
+
+def test_multigrid_argument_checks_need_no_gpu(binding):
+    """landau_create_multigrid validates its species -> grid map before it looks for a device: bad maps give
+    LANDAU_EINVAL everywhere; a good one gives LANDAU_ECUDA on a machine without a GPU."""
+    import torch
+    g = inputs.config(0).mesh
+    sp3 = inputs._sp([(1, -1, 1, 1), (4, 1, 1, 1), (8, 1, 1, 1)])
+    for bad in ([1, 0, 1], [0, 0, 0], [0, 2, 2], [0, 1, 5], [-1, 0, 1]):
+        with pytest.raises(binding.LandauError) as ei:
+            binding.LandauMultigridContext([g, inputs.mesh_scaled(g, 0.5)], bad, 2, sp3, 1)
+        assert ei.value.code == binding.LANDAU_EINVAL, bad
+    with pytest.raises(binding.LandauError) as ei:
+        binding.LandauMultigridContext([g, inputs.mesh_scaled(g, 0.5)], [0, 1, 1], 2, sp3, 0)      # max_batch < 1
+    assert ei.value.code == binding.LANDAU_EINVAL
+    if not torch.cuda.is_available():
+        with pytest.raises(binding.LandauError) as ei:
+            binding.LandauMultigridContext([g, inputs.mesh_scaled(g, 0.5)], [0, 1, 1], 2, sp3, 1)
+        assert ei.value.code == binding.LANDAU_ECUDA
