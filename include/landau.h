@@ -46,6 +46,15 @@
  * nothing, so a build can be captured in a CUDA graph; results are bitwise reproducible and a batched call
  * equals the same problems built one by one.
  *
+ * Two ways through step a3 (the choice changes rounding only, never the sum that is computed):
+ *   LANDAU_PAIR_PER_PROBLEM  every problem evaluates the tensor of every point pair itself (symmetric tile-pair
+ *                            kernel, K and E in registers, ~75 flop per ordered pair and problem);
+ *   LANDAU_PAIR_SHARED       the tensor depends on the mesh only, and all problems of a ctx share the mesh
+ *                            (the paper's batching model, L244, L377): it is evaluated ONCE per ordered pair and
+ *                            call into five N x N matrices, and G = U T for all problems is a dense fp64
+ *                            contraction on the tensor cores (14 flop per ordered pair and problem).
+ * A ctx uses ONE path for all its calls, so "batched == loop of singles, bitwise" holds inside a ctx.
+ *
  * Beyond a1-a8: the operator of a fully implicit step in one pass (landau_implicit_operator_batched:
  * E-field advection of Eq. 4 and the shifted mass matrix added), several grids for species clustered by
  * thermal speed (landau_create_multigrid, section III-C), and the per-species batched band LU of section
@@ -64,6 +73,11 @@ extern "C" {
 #define LANDAU_EINVAL (-1) /* bad argument: order, S < 1, mass <= 0, rmin < 0, mesh not a 2:1 tiling, nb > max_batch */
 #define LANDAU_ENOMEM (-2) /* host or device allocation failed */
 #define LANDAU_ECUDA (-3)  /* CUDA runtime error; text via landau_last_cuda_error() */
+
+#define LANDAU_PAIR_AUTO 0        /* landau_create's choice: SHARED when max_batch >= LANDAU_SHARED_MIN_BATCH and   */
+#define LANDAU_PAIR_PER_PROBLEM 1 /* the tensor scratch (40 N^2 bytes) is at most a quarter of the free device      */
+#define LANDAU_PAIR_SHARED 2      /* memory, else PER_PROBLEM                                                       */
+#define LANDAU_SHARED_MIN_BATCH 4
 
 typedef struct landau_ctx landau_ctx; /* opaque; owns all device + host state */
 
@@ -86,8 +100,12 @@ typedef struct {
 } landau_species;
 
 /* Set-up, once per mesh: DOF numbering, constraint closure, CSR pattern, gather
- * lists, point arrays, tabulations; uploads them.  max_batch >= 1 sizes the scratch arena for
- * landau_jacobian_batched.  On failure *out is NULL. */
+ * lists, point arrays, tabulations; uploads them.  max_batch in [1, 65535] sizes the scratch arena for
+ * landau_jacobian_batched and chooses the path through step a3 (LANDAU_PAIR_AUTO above).  Device scratch:
+ *   per-problem path : max_batch * (3 + 5 ceil(N/TS)) * N doubles, TS = 128 / 64 / 32 by N  (3.9 GB for 512 x 4,928)
+ *   batch-shared path: 40 N^2 bytes for the tensor (0.97 GB at N = 4,928) + max_batch * 5 (1 + ksplit) N doubles
+ * plus max_batch * S * Ne * Nb (Nb + 1) doubles of element matrices.  LANDAU_ENOMEM if it does not fit;
+ * on failure *out is NULL. */
 int landau_create(const landau_mesh *mesh, int order, const landau_species *species, int max_batch,
                   landau_ctx **out);
 int landau_destroy(landau_ctx *ctx);
@@ -112,6 +130,16 @@ int landau_strides(const landau_ctx *ctx, int32_t *S, int64_t *f_stride, int64_t
 int landau_grid_csr_pattern(const landau_ctx *ctx, int grid, const int32_t **rowptr_dev, const int32_t **colidx_dev);
 int landau_grid_csr_pattern_host(const landau_ctx *ctx, int grid, int32_t *rowptr_host, int32_t *colidx_host);
 int landau_grid_dof_coords(const landau_ctx *ctx, int grid, double *r_host, double *z_host);
+
+/* The path through step a3 (see the top of this file).  landau_set_pair_path synchronises the device, frees the
+ * scratch of the old path and allocates the new one (LANDAU_ENOMEM leaves the ctx without pair scratch: call it
+ * again with a path that fits).  landau_pair_path reports the path in use and its scratch bytes (either may be
+ * NULL).  landau_set_tensor_cache(on): batch-shared path only -- keep the tensor between calls instead of
+ * evaluating it in every call (the geometry of a ctx never changes); default OFF, so that every call does the
+ * whole of step a3. */
+int landau_set_pair_path(landau_ctx *ctx, int path);
+int landau_pair_path(const landau_ctx *ctx, int32_t *path, int64_t *scratch_bytes);
+int landau_set_tensor_cache(landau_ctx *ctx, int on);
 
 /* Host-only part of landau_create (no CUDA device needed): runs the same set-up and returns the
  * sizes and, where the pointer is not NULL, the CSR pattern of A1 (rowptr[n+1], colidx[nnz]) and
@@ -160,12 +188,17 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
  * pattern (computed in landau_create), band storage, Gaussian elimination WITHOUT pivoting in outer-product
  * form (Golub & Van Loan Alg. 4.3.1, the paper's algorithm; blocked), one independent matrix per (problem,
  * species).  Meant for the matrices of landau_implicit_operator_batched (shift M + A - J); like the paper's
- * solver it does not pivot, so a zero or tiny pivot is not detected.
+ * solver it does not pivot.  Breakdown is REPORTED, not repaired: pivots_dev (NULL, or [nb][S][2] device doubles)
+ * receives for every matrix the smallest and the largest |pivot| met; a zero, NaN or infinite pivot gives
+ * smallest = 0 (the factors and any solve with them are then meaningless), a tiny ratio smallest / largest
+ * tells that elimination without pivoting was unstable for that matrix.
  * landau_band_sizes: per grid the half-bandwidth after RCM and the doubles one matrix occupies; the
  * doubles of workspace per problem (all species of all grids); and the flop of the outer-product updates of
  * one factorisation (they are confined to the envelope of the ordered pattern, which elimination without
  * pivoting does not leave: about half of 2 n bw^2 on the refined meshes).  band_dev: caller-owned workspace of
- * nb * workspace_doubles_per_problem doubles; its internal layout belongs to the library.
+ * nb * workspace_doubles_per_problem doubles, problem-major: problem b owns the doubles
+ * [b * workspace_doubles_per_problem, (b + 1) * workspace_doubles_per_problem), so a solve may address the first
+ * nb' <= nb problems of an earlier factorisation; the layout inside a problem belongs to the library.
  * landau_band_factor_batched: vals_dev [nb][vals_stride] (CSR values, layout of landau_jacobian_batched)
  *   -> factors in band_dev.
  * landau_band_solve_batched: rhs_dev, x_dev [nb][f_stride] (layout of f); x = A^-1 rhs per species block;
@@ -177,7 +210,8 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
                            int32_t *block_columns, double *flop_per_factorization);
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
                       int64_t *workspace_doubles_per_problem, double *flop_per_factorization);
-int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, void *stream);
+int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, double *pivots_dev,
+                               void *stream);
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,
                               void *stream);
 
@@ -189,16 +223,29 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
 /* Number of kernel launches the ctx has enqueued since creation (for bench.py's gpu_launches). */
 int landau_launch_count(const landau_ctx *ctx, int64_t *count);
 
-/* Measurement aid: when enabled, every pair-kernel launch (step a3) is bracketed by CUDA events on
- * its own stream.  landau_profile_read synchronises those events, returns the summed device time
- * (ms) and the number of bracketed launches since the last read, and resets both. */
+/* Measurement aid: when enabled, the kernels of step a3 are bracketed by CUDA events on their own stream.
+ * landau_profile_read synchronises those events and returns, since the last read, the summed device time (ms)
+ * and the number of bracketed launches of
+ *   [0] the tensor evaluation: per-problem path k_pair_sym (evaluation and accumulation in one kernel),
+ *       batch-shared path k_pair_tensor;
+ *   [1] the batch-shared path's contraction k_apply_dmma (0 on the per-problem path);
+ * ms_total and launches are arrays of 2.  Resets both. */
 int landau_profile_enable(landau_ctx *ctx, int on);
-int landau_profile_read(landau_ctx *ctx, double *pair_ms_total, int64_t *pair_launches);
+int landau_profile_read(landau_ctx *ctx, double *ms_total, int64_t *launches);
 
 /* Measurement aid, not part of the operator: runs a register-resident chain of dependent-free
  * DFMA on every SM for `iters` iterations and returns the achieved FP64 rate in flop/s (the
  * "alu" roofline denominator).  Synchronises. */
 int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_est);
+
+/* Measurement aid, not part of the operator: FP64 issue-rate micro-benchmarks (the figures behind the "issue
+ * bound" of DESIGN.md).  Register-resident streams on every SM, three warps per SM sub-partition (one for mode 4),
+ * timed with clock64() on the SM.  mode: 0 DFMA with two register operands + immediate; 1 DFMA with two distinct
+ * registers; 2 DFMA with three distinct registers; 3 DFMA with three registers of which one is shared by
+ * consecutive instructions; 4 one dependent DFMA chain (latency); 5 DMMA m8n8k4 with independent accumulators.
+ * Returns SM cycles per warp instruction and sub-partition, and (flops_per_s may be NULL) the whole-GPU rate by
+ * wall clock (CUDA events).  Synchronises. */
+int landau_fp64_issue_probe(int mode, int iters, double *cycles_per_warp_instruction, double *flops_per_s);
 
 const char *landau_strerror(int code);
 const char *landau_last_cuda_error(void);

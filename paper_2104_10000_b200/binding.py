@@ -16,6 +16,8 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "liblandau_b200.so")
 
 LANDAU_OK, LANDAU_EINVAL, LANDAU_ENOMEM, LANDAU_ECUDA = 0, -1, -2, -3
+LANDAU_PAIR_AUTO, LANDAU_PAIR_PER_PROBLEM, LANDAU_PAIR_SHARED = 0, 1, 2
+LANDAU_SHARED_MIN_BATCH = 4
 
 
 class landau_mesh(ctypes.Structure):
@@ -59,13 +61,17 @@ SIGNATURES = {
     "landau_implicit_operator_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_double, c_void_p, c_void_p, c_void_p]),
     "landau_band_order_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_int32), POINTER(c_double)]),
     "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
-    "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
+    "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "landau_profile_enable": (c_int, [c_void_p, c_int]),
     "landau_profile_read": (c_int, [c_void_p, POINTER(c_double), POINTER(c_int64)]),
     "landau_fp64_peak_probe": (c_int, [c_int, POINTER(c_double), POINTER(c_double)]),
+    "landau_fp64_issue_probe": (c_int, [c_int, c_int, POINTER(c_double), POINTER(c_double)]),
+    "landau_set_pair_path": (c_int, [c_void_p, c_int]),
+    "landau_pair_path": (c_int, [c_void_p, POINTER(c_int32), POINTER(c_int64)]),
+    "landau_set_tensor_cache": (c_int, [c_void_p, c_int]),
     "landau_strerror": (ctypes.c_char_p, [c_int]),
     "landau_last_cuda_error": (ctypes.c_char_p, []),
 }
@@ -152,6 +158,14 @@ def landau_fp64_peak_probe(iters: int = 1 << 16):
     return fl.value, mhz.value
 
 
+def landau_fp64_issue_probe(mode: int, iters: int = 1 << 14):
+    """(SM cycles per warp instruction and sub-partition, whole-GPU flop/s) of issue-rate probe `mode`."""
+    L = lib()
+    cyc, fl = c_double(), c_double()
+    _check(L.landau_fp64_issue_probe(mode, iters, ctypes.byref(cyc), ctypes.byref(fl)))
+    return cyc.value, fl.value
+
+
 def _stream_ptr(stream):
     import torch
     s = torch.cuda.current_stream() if stream is None else stream
@@ -162,7 +176,7 @@ class LandauContext:
     """Owns a landau_ctx.  Methods mirror the C entry points one to one (same names without the
     prefix); tensors are torch CUDA float64, contiguous."""
 
-    def __init__(self, mesh, order: int, species, max_batch: int = 1):
+    def __init__(self, mesh, order: int, species, max_batch: int = 1, pair_path: int = LANDAU_PAIR_AUTO):
         L = lib()
         m, keep = _mesh_struct(mesh)
         mass, charge = _f64(species.mass), _f64(species.charge)
@@ -171,6 +185,8 @@ class LandauContext:
         h = c_void_p()
         _check(L.landau_create(ctypes.byref(m), order, ctypes.byref(sp), int(max_batch), ctypes.byref(h)))
         self._h = h
+        if pair_path != LANDAU_PAIR_AUTO:
+            self.set_pair_path(pair_path)
         S, n, nnz, N, Ne = c_int32(), c_int64(), c_int64(), c_int64(), c_int64()
         _check(L.landau_sizes(h, ctypes.byref(S), ctypes.byref(n), ctypes.byref(nnz), ctypes.byref(N), ctypes.byref(Ne)))
         self.S, self.n, self.nnz, self.N, self.Ne = S.value, n.value, nnz.value, N.value, Ne.value
@@ -186,6 +202,18 @@ class LandauContext:
             self.destroy()
         except Exception:
             pass
+
+    def set_pair_path(self, path: int):
+        _check(lib().landau_set_pair_path(self._h, int(path)))
+
+    def pair_path(self):
+        """(path in use: LANDAU_PAIR_PER_PROBLEM or LANDAU_PAIR_SHARED, bytes of its scratch)."""
+        p, b = c_int32(), c_int64()
+        _check(lib().landau_pair_path(self._h, ctypes.byref(p), ctypes.byref(b)))
+        return p.value, b.value
+
+    def set_tensor_cache(self, on: bool):
+        _check(lib().landau_set_tensor_cache(self._h, int(bool(on))))
 
     def csr_pattern_host(self):
         rowptr, colidx = np.zeros(self.n + 1, np.int32), np.zeros(self.nnz, np.int32)
@@ -246,10 +274,12 @@ class LandauContext:
         self.band_flop_per_factorization = fl.value
         return bw.value, md.value, ws.value
 
-    def band_factor_batched(self, vals, band, stream=None):
+    def band_factor_batched(self, vals, band, pivots=None, stream=None):
+        """pivots: None or a CUDA float64 tensor [nb][S][2] receiving (min |pivot|, max |pivot|) per matrix."""
         nb = vals.shape[0]
         assert band.is_cuda and band.is_contiguous() and band.numel() >= nb * self.band_sizes()[2]
-        _check(lib().landau_band_factor_batched(self._h, nb, c_void_p(vals.data_ptr()), c_void_p(band.data_ptr()), _stream_ptr(stream)))
+        pp = self._ptr(pivots, (nb, self.S, 2)) if pivots is not None else None
+        _check(lib().landau_band_factor_batched(self._h, nb, c_void_p(vals.data_ptr()), c_void_p(band.data_ptr()), pp, _stream_ptr(stream)))
 
     def band_solve_batched(self, band, rhs, x, stream=None):
         nb = rhs.shape[0]
@@ -269,10 +299,10 @@ class LandauContext:
         _check(lib().landau_profile_enable(self._h, int(bool(on))))
 
     def profile_read(self):
-        """(summed pair-kernel device time in ms, number of launches) since the last read."""
-        ms, cnt = c_double(), c_int64()
-        _check(lib().landau_profile_read(self._h, ctypes.byref(ms), ctypes.byref(cnt)))
-        return ms.value, cnt.value
+        """([ms of the tensor evaluation, ms of the batch-shared contraction], [launches of each]) since the last read."""
+        ms, cnt = (c_double * 2)(), (c_int64 * 2)()
+        _check(lib().landau_profile_read(self._h, ms, cnt))
+        return [ms[0], ms[1]], [cnt[0], cnt[1]]
 
     def launch_count(self) -> int:
         c = c_int64()
@@ -317,6 +347,9 @@ class LandauMultigridContext:
     __del__ = LandauContext.__del__
     _ptr = staticmethod(LandauContext._ptr)
     launch_count = LandauContext.launch_count
+    set_pair_path = LandauContext.set_pair_path
+    pair_path = LandauContext.pair_path
+    set_tensor_cache = LandauContext.set_tensor_cache
     band_sizes = LandauContext.band_sizes
     band_factor_batched = LandauContext.band_factor_batched
     band_solve_batched = LandauContext.band_solve_batched

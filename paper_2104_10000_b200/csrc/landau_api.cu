@@ -18,6 +18,7 @@
 #include "landau.h"
 #include "landau_internal.h"
 #include "landau_kernels.h"
+#include "landau_launch.cuh"
 
 using namespace landau;
 
@@ -34,6 +35,28 @@ int cuda_fail(cudaError_t e, const char *what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);  \
     } while (0)
 
+// end of a chain of launches: the first failed cudaLaunchKernelEx of the chain, then the sticky error state
+int launches_ok() {
+    cudaError_t e = take_launch_error();
+    if (e != cudaSuccess) { cudaGetLastError(); return cuda_fail(e, "kernel launch"); }
+    e = cudaGetLastError();
+    if (e != cudaSuccess) return cuda_fail(e, "kernel launch (cudaGetLastError)");
+    return LANDAU_OK;
+}
+
+// No exception crosses the C ABI: every entry point that can allocate on the host runs its body through this.
+template <class F>
+int guarded(F &&body) {
+    try {
+        return body();
+    } catch (const std::bad_alloc &) {
+        return LANDAU_ENOMEM;
+    } catch (...) {
+        g_cuda_err = "unexpected C++ exception";
+        return LANDAU_EINVAL;
+    }
+}
+
 template <class T>
 int upload(const std::vector<T> &v, const T **out, std::vector<void *> &owned) {
     void *d = nullptr;
@@ -45,6 +68,8 @@ int upload(const std::vector<T> &v, const T **out, std::vector<void *> &owned) {
     *out = static_cast<const T *>(d);
     return LANDAU_OK;
 }
+
+struct ProfEvent { cudaEvent_t a = nullptr, b = nullptr; int kind = 0; };
 
 struct GridState {
     HostSpace hs;
@@ -68,8 +93,13 @@ struct landau_ctx {
     size_t bstride = 0;                              // doubles per problem in the band-LU workspace
     const double *r = nullptr, *z = nullptr, *invr = nullptr;   // [Ntot] union of the grids' points
     bool check_all = false;          // points of different grids coincide somewhere
-    Scratch sc;
-    std::vector<void *> owned;   // device allocations
+    Scratch sc = {};
+    std::vector<void *> owned;       // device allocations that live as long as the ctx
+    std::vector<void *> pair_owned;  // scratch of the current pair path (T, G, U): replaced by landau_set_pair_path
+    int pair_path = LANDAU_PAIR_PER_PROBLEM;   // resolved path (never LANDAU_PAIR_AUTO)
+    int nbpad = 0;                   // batch-shared path: problems padded to whole tiles
+    bool tensor_cache = false;       // keep U between calls (the geometry of a ctx never changes)
+    bool tensor_valid = false;
     int max_batch = 1;
     int num_sms = 148;
     int64_t launches = 0;
@@ -78,30 +108,106 @@ struct landau_ctx {
     double *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
     int host_nb = 0;
     bool profiling = false;
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_events;  // recorded, not yet read
-    std::vector<std::pair<cudaEvent_t, cudaEvent_t>> prof_pool;    // free
+    std::vector<ProfEvent> prof_events;  // recorded, not yet read
+    std::vector<ProfEvent> prof_pool;    // free
 };
 
 namespace {
 // launch_pair bracketed by events when profiling is on
-int timed_pair(landau_ctx *ctx, int nb, double *G, cudaStream_t st) {
-    auto go = [&]() { return launch_pair(int(ctx->Ntot), ctx->r, ctx->z, ctx->invr, ctx->check_all, nb, ctx->sc.T, G, st); };
+// Step a3 bracketed by events when profiling is on.  Per-problem path: the pair kernel; batch-shared path: the
+// tensor evaluation (unless cached) and the contraction -- kind 0 / 1 in landau_profile_read.
+template <class F>
+int timed(landau_ctx *ctx, int kind, cudaStream_t st, F &&go) {
     if (!ctx->profiling) return go();
-    std::pair<cudaEvent_t, cudaEvent_t> ev;
+    ProfEvent ev;
     if (!ctx->prof_pool.empty()) { ev = ctx->prof_pool.back(); ctx->prof_pool.pop_back(); }
-    else { cudaEventCreate(&ev.first); cudaEventCreate(&ev.second); }
-    cudaEventRecord(ev.first, st);
-    int k = go();
-    cudaEventRecord(ev.second, st);
+    else {
+        cudaError_t e = cudaEventCreate(&ev.a);
+        if (e == cudaSuccess) e = cudaEventCreate(&ev.b);
+        if (e != cudaSuccess) { note_launch_error(e); return go(); }
+    }
+    ev.kind = kind;
+    note_launch_error(cudaEventRecord(ev.a, st));
+    const int k = go();
+    note_launch_error(cudaEventRecord(ev.b, st));
     ctx->prof_events.push_back(ev);
     return k;
 }
 
-// a1-a3 for nb problems: fields + beta sums per grid, pair kernel over the union, tile-order sum
-void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, cudaStream_t st) {
+// a1-a3 for nb problems.  Per-problem path: fields + beta sums per grid, pair kernel over the union, tile-order
+// sum.  Batch-shared path: fields into the tiled T, the tensor of every ordered pair ONCE (reuse_tensor: already
+// done by this call for an earlier sub-batch), the fp64 tensor-core contraction, split-order sum.
+void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, cudaStream_t st, bool reuse_tensor = false) {
+    const int N = int(ctx->Ntot);
+    if (ctx->pair_path == LANDAU_PAIR_SHARED) {
+        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta_tiled(g.ds, nb, ctx->nbpad, f_dev + g.foff, ctx->sc.T, st);
+        if (!(reuse_tensor || (ctx->tensor_cache && ctx->tensor_valid))) {
+            ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair_tensor(N, ctx->r, ctx->z, ctx->invr, ctx->sc.U, st); });
+            ctx->tensor_valid = true;
+        }
+        const int ksplit = shared_ksplit(N);
+        ctx->launches += timed(ctx, 1, st, [&]() { return launch_apply(N, nb, ctx->nbpad, ctx->sc.U, ctx->sc.T, ksplit > 1 ? ctx->sc.G : Gsum, st); });
+        if (ksplit > 1) ctx->launches += launch_sum_partials(N, nb, ksplit, ctx->sc.G, Gsum, st);
+        return;
+    }
     for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nb, f_dev + g.foff, ctx->sc.T, st);
-    ctx->launches += timed_pair(ctx, nb, ctx->sc.G, st);
-    ctx->launches += launch_sum_partials(int(ctx->Ntot), nb, pair_tiles(int(ctx->Ntot)), ctx->sc.G, Gsum, st);
+    ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->r, ctx->z, ctx->invr, ctx->check_all, nb, ctx->sc.T, ctx->sc.G, st); });
+    ctx->launches += launch_sum_partials(N, nb, pair_tiles(N), ctx->sc.G, Gsum, st);
+}
+
+void free_pair_scratch(landau_ctx *ctx) {
+    for (void *p : ctx->pair_owned) cudaFree(p);
+    ctx->pair_owned.clear();
+    ctx->sc.T = ctx->sc.G = ctx->sc.U = nullptr;
+    ctx->tensor_valid = false;
+}
+
+// Bytes of U, the tensor entries of all ordered pairs (batch-shared path).
+size_t tensor_bytes(int64_t N) { return size_t(5) * (shared_kpad(int(N)) / 8) * shared_mpad(int(N)) * 8 * sizeof(double); }
+
+// Scratch of the pair path (sized for max_batch):
+//   per problem : T [nb][3][N], G [nb][ntiles][5][N]   (the slabs grow like nb N^2 / TS: 3.9 GB for 512 x 4,928)
+//   batch-shared: T [3][Kpad/8][nbpad][8], U [5][Kpad/8][Mpad][8] (5 N^2 doubles: 0.97 GB for N = 4,928, independent
+//                 of the batch), G [nb][ksplit][5][N]; T and U are zeroed once: their padding must stay zero
+int alloc_pair_scratch(landau_ctx *ctx, int path) {
+    free_pair_scratch(ctx);
+    const size_t nbm = size_t(ctx->max_batch), N = size_t(ctx->Ntot);
+    struct Alloc { double **p; size_t n; bool zero; };
+    std::vector<Alloc> allocs;
+    if (path == LANDAU_PAIR_SHARED) {
+        ctx->nbpad = shared_nbpad(ctx->max_batch);
+        const size_t Kq8 = size_t(shared_kpad(int(N)) / 8);
+        allocs = {{&ctx->sc.T, 3 * Kq8 * ctx->nbpad * 8, true},
+                  {&ctx->sc.U, tensor_bytes(int64_t(N)) / sizeof(double), true},
+                  {&ctx->sc.G, shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0, false}};
+    } else {
+        allocs = {{&ctx->sc.T, nbm * 3 * N, false}, {&ctx->sc.G, nbm * pair_tiles(int(N)) * 5 * N, false}};
+    }
+    for (auto &a : allocs) {
+        if (!a.n) continue;
+        void *d = nullptr;
+        cudaError_t e = cudaMalloc(&d, a.n * sizeof(double));
+        if (e != cudaSuccess) {
+            g_cuda_err = std::string("cudaMalloc(pair scratch): ") + cudaGetErrorString(e);
+            cudaGetLastError();
+            free_pair_scratch(ctx);
+            return e == cudaErrorMemoryAllocation ? LANDAU_ENOMEM : LANDAU_ECUDA;
+        }
+        ctx->pair_owned.push_back(d);
+        *a.p = static_cast<double *>(d);
+        if (a.zero) CK(cudaMemset(d, 0, a.n * sizeof(double)));
+    }
+    ctx->pair_path = path;
+    return LANDAU_OK;
+}
+
+// LANDAU_PAIR_AUTO: share the tensor across the batch when there is a batch to share it with and U fits easily
+int resolve_pair_path(const landau_ctx *ctx, int path) {
+    if (path != LANDAU_PAIR_AUTO) return path;
+    if (ctx->max_batch < LANDAU_SHARED_MIN_BATCH) return LANDAU_PAIR_PER_PROBLEM;
+    size_t free_b = 0, total_b = 0;
+    if (cudaMemGetInfo(&free_b, &total_b) != cudaSuccess) { cudaGetLastError(); return LANDAU_PAIR_PER_PROBLEM; }
+    return tensor_bytes(ctx->Ntot) <= free_b / 4 ? LANDAU_PAIR_SHARED : LANDAU_PAIR_PER_PROBLEM;
 }
 
 // Small batches are launch-latency bound: both gathers then go in one launch (3-7 us per single build); large
@@ -152,23 +258,25 @@ const char *landau_last_cuda_error(void) { return g_cuda_err.c_str(); }
 int landau_destroy(landau_ctx *ctx) {
     if (!ctx) return LANDAU_OK;
     for (void *p : ctx->owned) cudaFree(p);
+    for (void *p : ctx->pair_owned) cudaFree(p);
     if (ctx->d_f) cudaFree(ctx->d_f);
     if (ctx->d_vals) cudaFree(ctx->d_vals);
     if (ctx->d_Cf) cudaFree(ctx->d_Cf);
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->chunk_done) cudaEventDestroy(ctx->chunk_done);
-    for (auto &ev : ctx->prof_events) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
-    for (auto &ev : ctx->prof_pool) { cudaEventDestroy(ev.first); cudaEventDestroy(ev.second); }
+    for (auto &ev : ctx->prof_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
+    for (auto &ev : ctx->prof_pool) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete ctx;
     return LANDAU_OK;
 }
 
-int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t *species_grid, int order,
-                            const landau_species *species, int max_batch, landau_ctx **out) {
+static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *species_grid, int order,
+                       const landau_species *species, int max_batch, int pair_path, landau_ctx **out) {
     if (!out) return LANDAU_EINVAL;
     *out = nullptr;
     if (!meshes || !species || ngrids < 1 || max_batch < 1 || max_batch > 65535) return LANDAU_EINVAL;
+    if (pair_path != LANDAU_PAIR_AUTO && pair_path != LANDAU_PAIR_PER_PROBLEM && pair_path != LANDAU_PAIR_SHARED) return LANDAU_EINVAL;
     if (species->S < 1 || species->S > MAX_SPECIES || !species->mass || !species->charge) return LANDAU_EINVAL;
     if (!(species->m0 > 0.0)) return LANDAU_EINVAL;
     const int S = species->S;
@@ -192,19 +300,18 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
     }
     landau_ctx *ctx = new (std::nothrow) landau_ctx();
     if (!ctx) return LANDAU_ENOMEM;
+    struct Guard {                      // an exception (bad_alloc) or an early return destroys the half-built ctx
+        landau_ctx *c;
+        ~Guard() { if (c) landau_destroy(c); }
+    } guard{ctx};
     ctx->grids.resize(ngrids);
     ctx->S = S;
     ctx->max_batch = max_batch;
     int rc = LANDAU_OK;
     for (int g = 0; g < ngrids; ++g) {
         std::string err;
-        try {
-            rc = build_host_space(meshes[g], order, ctx->grids[g].hs, err);
-        } catch (const std::bad_alloc &) {
-            delete ctx;
-            return LANDAU_ENOMEM;
-        }
-        if (rc != LANDAU_OK) { g_cuda_err = err; delete ctx; return rc; }
+        rc = build_host_space(meshes[g], order, ctx->grids[g].hs, err);
+        if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
     }
     // offsets and sizes
     std::vector<double> r, z, invr;
@@ -233,14 +340,14 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         z.insert(z.end(), hs.z.begin(), hs.z.end());
         for (int64_t i = 0; i < hs.N; ++i) invr.push_back(1.0 / hs.r[i]);
     }
-    if (ctx->Ntot > (int64_t(1) << 30) || ctx->vstride > (size_t(1) << 32)) { delete ctx; return LANDAU_EINVAL; }
+    if (ctx->Ntot > (int64_t(1) << 30) || ctx->vstride > (size_t(1) << 32)) return LANDAU_EINVAL;
     ctx->check_all = ngrids > 1 && cross_grid_coincidence(ctx->grids);
     int dev = 0;
     cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&ctx->num_sms, cudaDevAttrMultiProcessorCount, dev);
 
 #define UPC(ptr, vec) \
-    if ((rc = upload(vec, &(ptr), ctx->owned)) != LANDAU_OK) { landau_destroy(ctx); return rc; }
+    if ((rc = upload(vec, &(ptr), ctx->owned)) != LANDAU_OK) return rc;
     UPC(ctx->r, r) UPC(ctx->z, z) UPC(ctx->invr, invr)
     const size_t nbm = size_t(max_batch);
     for (int g = 0; g < ngrids; ++g) {
@@ -263,7 +370,7 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         std::vector<int32_t> pos(hs.n);
         for (int64_t i = 0; i < hs.n; ++i) pos[perm[i]] = int32_t(i);
         const int64_t Wb = (bw + band_block(bw) + 1) & ~1, LD = 2 * Wb + 1;   // even half-width (band_halfwidth in landau_band.cu)
-        if (LD * hs.n > (int64_t(1) << 31) - 1) { landau_destroy(ctx); return LANDAU_EINVAL; }
+        if (LD * hs.n > (int64_t(1) << 31) - 1) return LANDAU_EINVAL;
         for (int64_t i = 0; i < hs.n; ++i)
             for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) {
                 const int64_t ni = pos[i], nj = pos[hs.colidx[t]];
@@ -299,13 +406,10 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         ctx->bstride += size_t(ds.S) * G.bs.mat_doubles;
     }
 #undef UPC
-    // scratch arena
+    // scratch arena.  Sizes are validated in 64-bit arithmetic first: an absurd max_batch fails here with
+    // LANDAU_ENOMEM instead of overflowing an index later.
     struct Alloc { double **p; size_t n; };
-    std::vector<Alloc> allocs = {
-        {&ctx->sc.T, nbm * 3 * ctx->Ntot},
-        {&ctx->sc.G, nbm * pair_tiles(int(ctx->Ntot)) * 5 * ctx->Ntot},
-        {&ctx->sc.Gsum, nbm * 5 * ctx->Ntot},
-    };
+    std::vector<Alloc> allocs = {{&ctx->sc.Gsum, nbm * 5 * ctx->Ntot}};
     for (auto &G : ctx->grids) {
         allocs.push_back({&G.Ce, nbm * G.ds.S * G.hs.Ne * G.hs.Nb * G.hs.Nb});
         allocs.push_back({&G.ce, nbm * G.ds.S * G.hs.Ne * G.hs.Nb});
@@ -315,31 +419,68 @@ int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t
         cudaError_t e = cudaMalloc(&d, a.n * sizeof(double));
         if (e != cudaSuccess) {
             g_cuda_err = std::string("cudaMalloc(scratch): ") + cudaGetErrorString(e);
-            landau_destroy(ctx);
+            cudaGetLastError();
             return e == cudaErrorMemoryAllocation ? LANDAU_ENOMEM : LANDAU_ECUDA;
         }
         ctx->owned.push_back(d);
         *a.p = static_cast<double *>(d);
     }
+    if ((rc = alloc_pair_scratch(ctx, resolve_pair_path(ctx, pair_path))) != LANDAU_OK) return rc;
+    guard.c = nullptr;
     *out = ctx;
     return LANDAU_OK;
+}
+
+int landau_create_multigrid(const landau_mesh *meshes, int ngrids, const int32_t *species_grid, int order,
+                            const landau_species *species, int max_batch, landau_ctx **out) {
+    if (out) *out = nullptr;
+    return guarded([&]() { return create_impl(meshes, ngrids, species_grid, order, species, max_batch, LANDAU_PAIR_AUTO, out); });
 }
 
 int landau_create(const landau_mesh *mesh, int order, const landau_species *species, int max_batch, landau_ctx **out) {
     return landau_create_multigrid(mesh, 1, nullptr, order, species, max_batch, out);
 }
 
+int landau_set_pair_path(landau_ctx *ctx, int path) {
+    if (!ctx || (path != LANDAU_PAIR_AUTO && path != LANDAU_PAIR_PER_PROBLEM && path != LANDAU_PAIR_SHARED)) return LANDAU_EINVAL;
+    return guarded([&]() {
+        CK(cudaDeviceSynchronize());                       // the scratch being replaced may still be in use
+        const int want = resolve_pair_path(ctx, path);
+        if (want == ctx->pair_path && !ctx->pair_owned.empty()) return int(LANDAU_OK);
+        return alloc_pair_scratch(ctx, want);
+    });
+}
+
+int landau_pair_path(const landau_ctx *ctx, int32_t *path, int64_t *scratch_bytes) {
+    if (!ctx) return LANDAU_EINVAL;
+    if (path) *path = ctx->pair_path;
+    if (scratch_bytes) {
+        const size_t N = size_t(ctx->Ntot), nbm = size_t(ctx->max_batch);
+        size_t d;
+        if (ctx->pair_path == LANDAU_PAIR_SHARED)
+            d = 3 * size_t(shared_kpad(int(N)) / 8) * ctx->nbpad * 8 + tensor_bytes(ctx->Ntot) / 8 +
+                (shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0);
+        else
+            d = nbm * 3 * N + nbm * pair_tiles(int(N)) * 5 * N;
+        *scratch_bytes = int64_t(d * sizeof(double));
+    }
+    return LANDAU_OK;
+}
+
+int landau_set_tensor_cache(landau_ctx *ctx, int on) {
+    if (!ctx) return LANDAU_EINVAL;
+    ctx->tensor_cache = on != 0;
+    if (!on) ctx->tensor_valid = false;
+    return LANDAU_OK;
+}
+
 int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *nnz, int64_t *N, int32_t *rowptr_host,
                       int32_t *colidx_host, double *dof_r_host, double *dof_z_host) {
     if (!mesh) return LANDAU_EINVAL;
+    return guarded([&]() {
     HostSpace hs;
     std::string err;
-    int rc;
-    try {
-        rc = build_host_space(*mesh, order, hs, err);
-    } catch (const std::bad_alloc &) {
-        return LANDAU_ENOMEM;
-    }
+    const int rc = build_host_space(*mesh, order, hs, err);
     if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
     if (n) *n = hs.n;
     if (nnz) *nnz = hs.nnz;
@@ -348,20 +489,17 @@ int landau_setup_host(const landau_mesh *mesh, int order, int64_t *n, int64_t *n
     if (colidx_host) std::memcpy(colidx_host, hs.colidx.data(), hs.colidx.size() * sizeof(int32_t));
     if (dof_r_host) std::memcpy(dof_r_host, hs.dof_r.data(), hs.n * sizeof(double));
     if (dof_z_host) std::memcpy(dof_z_host, hs.dof_z.data(), hs.n * sizeof(double));
-    return LANDAU_OK;
+    return int(LANDAU_OK);
+    });
 }
 
 int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_host, int32_t *half_bandwidth,
                            int32_t *block_columns, double *flop_per_factorization) {
     if (!mesh) return LANDAU_EINVAL;
+    return guarded([&]() {
     HostSpace hs;
     std::string err;
-    int rc;
-    try {
-        rc = build_host_space(*mesh, order, hs, err);
-    } catch (const std::bad_alloc &) {
-        return LANDAU_ENOMEM;
-    }
+    const int rc = build_host_space(*mesh, order, hs, err);
     if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
     std::vector<int32_t> perm;
     int bw = 0;
@@ -385,7 +523,8 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
         }
         *flop_per_factorization = work;
     }
-    return LANDAU_OK;
+    return int(LANDAU_OK);
+    });
 }
 
 int landau_grid_count(const landau_ctx *ctx, int32_t *ngrids) {
@@ -481,28 +620,31 @@ int landau_points(const landau_ctx *ctx, double *r_host, double *z_host, double 
 
 int landau_inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *G_dev, void *stream) {
     if (!ctx || !f_dev || !G_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
-    inner_integral(ctx, nb, f_dev, G_dev, static_cast<cudaStream_t>(stream));
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return guarded([&]() {
+        inner_integral(ctx, nb, f_dev, G_dev, static_cast<cudaStream_t>(stream));
+        return launches_ok();
+    });
 }
 
 int landau_jacobian_batched(landau_ctx *ctx, int nb, const double *f_dev, double *vals_dev, double *Cf_dev, void *stream) {
     if (!ctx || !f_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
-    assemble(ctx, nb, f_dev, nullptr, 0.0, vals_dev, Cf_dev, st);
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return guarded([&]() {
+        inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+        assemble(ctx, nb, f_dev, nullptr, 0.0, vals_dev, Cf_dev, st);
+        return launches_ok();
+    });
 }
 
 int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez_dev, double shift,
                                      double *vals_dev, double *F_dev, void *stream) {
     if (!ctx || !f_dev || !Ez_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
-    inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
-    assemble(ctx, nb, f_dev, Ez_dev, shift, vals_dev, F_dev, st);
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return guarded([&]() {
+        inner_integral(ctx, nb, f_dev, ctx->sc.Gsum, st);
+        assemble(ctx, nb, f_dev, Ez_dev, shift, vals_dev, F_dev, st);
+        return launches_ok();
+    });
 }
 
 int landau_jacobian(landau_ctx *ctx, const double *f_dev, double *vals_dev, double *Cf_dev, void *stream) {
@@ -516,8 +658,7 @@ int landau_mass(landau_ctx *ctx, double shift, double *mvals_dev, void *stream) 
         ctx->launches += launch_mass_element(g.ds, shift, g.Ce, st);
         ctx->launches += launch_gather_vals(g.ds, 1, 1, 0, g.Ce, mvals_dev + g.moff, st);
     }
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return launches_ok();
 }
 
 int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *vals_host, double *Cf_host) {
@@ -540,21 +681,32 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
     // c+1 (the scratch arena is reused in stream order; problems are independent, so the values
     // are bitwise those of one batched call).
     cudaStream_t st = ctx->own_stream, cp = ctx->copy_stream;
-    CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
-    const int nchunks = nb >= 64 ? 8 : (nb >= 8 ? 4 : 1);
-    const int cb = (nb + nchunks - 1) / nchunks;
-    for (int b0 = 0; b0 < nb; b0 += cb) {
-        const int nbc = std::min(cb, nb - b0);
-        int rc = landau_jacobian_batched(ctx, nbc, ctx->d_f + b0 * fsz, vals_host ? ctx->d_vals + b0 * vsz : nullptr,
-                                         Cf_host ? ctx->d_Cf + b0 * fsz : nullptr, st);
-        if (rc != LANDAU_OK) return rc;
-        CK(cudaEventRecord(ctx->chunk_done, st));
-        CK(cudaStreamWaitEvent(cp, ctx->chunk_done, 0));
-        if (vals_host) CK(cudaMemcpyAsync(vals_host + b0 * vsz, ctx->d_vals + b0 * vsz, size_t(nbc) * vsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
-        if (Cf_host) CK(cudaMemcpyAsync(Cf_host + b0 * fsz, ctx->d_Cf + b0 * fsz, size_t(nbc) * fsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
-    }
-    CK(cudaStreamSynchronize(st));
-    CK(cudaStreamSynchronize(cp));
+    // the body enqueues; whatever it returns, both streams are drained before the caller gets its buffers back
+    // (an error half way must not leave device-to-host copies into the caller's memory in flight)
+    auto body = [&]() -> int {
+        CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
+        const int nchunks = nb >= 64 ? 8 : (nb >= 8 ? 4 : 1);
+        const int cb = (nb + nchunks - 1) / nchunks;
+        for (int b0 = 0; b0 < nb; b0 += cb) {
+            const int nbc = std::min(cb, nb - b0);
+            // the tensor of the point pairs (batch-shared path) is evaluated by the first sub-batch only
+            inner_integral(ctx, nbc, ctx->d_f + b0 * fsz, ctx->sc.Gsum, st, b0 > 0);
+            assemble(ctx, nbc, ctx->d_f + b0 * fsz, nullptr, 0.0, vals_host ? ctx->d_vals + b0 * vsz : nullptr,
+                     Cf_host ? ctx->d_Cf + b0 * fsz : nullptr, st);
+            const int rc = launches_ok();
+            if (rc != LANDAU_OK) return rc;
+            CK(cudaEventRecord(ctx->chunk_done, st));
+            CK(cudaStreamWaitEvent(cp, ctx->chunk_done, 0));
+            if (vals_host) CK(cudaMemcpyAsync(vals_host + b0 * vsz, ctx->d_vals + b0 * vsz, size_t(nbc) * vsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
+            if (Cf_host) CK(cudaMemcpyAsync(Cf_host + b0 * fsz, ctx->d_Cf + b0 * fsz, size_t(nbc) * fsz * sizeof(double), cudaMemcpyDeviceToHost, cp));
+        }
+        return LANDAU_OK;
+    };
+    const int rc = guarded(body);
+    const cudaError_t e1 = cudaStreamSynchronize(st), e2 = cudaStreamSynchronize(cp);
+    if (rc != LANDAU_OK) return rc;
+    if (e1 != cudaSuccess) return cuda_fail(e1, "cudaStreamSynchronize(build stream)");
+    if (e2 != cudaSuccess) return cuda_fail(e2, "cudaStreamSynchronize(copy stream)");
     return LANDAU_OK;
 }
 
@@ -568,20 +720,19 @@ int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, 
     return LANDAU_OK;
 }
 
-// band workspace layout: [grid][problem][species of the grid][matrix] -- grid-major so that one launch
-// per grid sees its matrices contiguously
-int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, void *stream) {
+// band workspace layout: [problem][grid][species of the grid][matrix] -- problem-major, so that a solve may
+// cover fewer (or other) problems than the factorisation that filled the workspace
+int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, double *pivots_dev, void *stream) {
     if (!ctx || !vals_dev || !band_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     for (auto &g : ctx->grids) {
         if (band_factor_smem(g.bs.bw) > 227 * 1024) return LANDAU_EINVAL;
-        double *band = band_dev + size_t(nb) * g.boff;
-        ctx->launches += launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, vals_dev + g.voff, band, st);
-        CK(launch_band_factor(g.bs, nb * g.ds.S, band, st));
-        ctx->launches += 1;
+        double *band = band_dev + g.boff;
+        CK(launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, ctx->bstride, vals_dev + g.voff, band, st));
+        CK(launch_band_factor(g.bs, nb * g.ds.S, g.ds.S, ctx->bstride, band, pivots_dev ? pivots_dev + 2 * g.s0 : nullptr, ctx->S, st));
+        ctx->launches += 2;
     }
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return launches_ok();
 }
 
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev, void *stream) {
@@ -589,12 +740,11 @@ int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, c
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     for (auto &g : ctx->grids) {
         if ((size_t(g.bs.n) + 33 * 32) * sizeof(double) > 227 * 1024) return LANDAU_EINVAL;
-        const double *band = band_dev + size_t(nb) * g.boff;
-        CK(launch_band_solve(g.bs, nb, g.ds.S, ctx->fstride, band, rhs_dev + g.foff, x_dev + g.foff, st));
+        const double *band = band_dev + g.boff;
+        CK(launch_band_solve(g.bs, nb, g.ds.S, ctx->fstride, ctx->bstride, band, rhs_dev + g.foff, x_dev + g.foff, st));
         ctx->launches += 1;
     }
-    CK(cudaGetLastError());
-    return LANDAU_OK;
+    return launches_ok();
 }
 
 int landau_launch_count(const landau_ctx *ctx, int64_t *count) {
@@ -609,20 +759,22 @@ int landau_profile_enable(landau_ctx *ctx, int on) {
     return LANDAU_OK;
 }
 
-int landau_profile_read(landau_ctx *ctx, double *pair_ms_total, int64_t *pair_launches) {
-    if (!ctx || !pair_ms_total || !pair_launches) return LANDAU_EINVAL;
-    double total = 0.0;
-    for (auto &ev : ctx->prof_events) {
-        CK(cudaEventSynchronize(ev.second));
-        float ms = 0.f;
-        CK(cudaEventElapsedTime(&ms, ev.first, ev.second));
-        total += ms;
-        ctx->prof_pool.push_back(ev);
-    }
-    *pair_ms_total = total;
-    *pair_launches = int64_t(ctx->prof_events.size());
-    ctx->prof_events.clear();
-    return LANDAU_OK;
+int landau_profile_read(landau_ctx *ctx, double *ms_total, int64_t *launches) {
+    if (!ctx || !ms_total || !launches) return LANDAU_EINVAL;
+    return guarded([&]() {
+        ms_total[0] = ms_total[1] = 0.0;
+        launches[0] = launches[1] = 0;
+        for (auto &ev : ctx->prof_events) {
+            CK(cudaEventSynchronize(ev.b));
+            float ms = 0.f;
+            CK(cudaEventElapsedTime(&ms, ev.a, ev.b));
+            ms_total[ev.kind] += ms;
+            launches[ev.kind] += 1;
+            ctx->prof_pool.push_back(ev);
+        }
+        ctx->prof_events.clear();
+        return int(LANDAU_OK);
+    });
 }
 
 int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_est) {
@@ -648,6 +800,43 @@ int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_
     if (sm_clock_mhz_est) *sm_clock_mhz_est = *flops_per_s / (2.0 * 64.0 * sms) * 1e-6;
     cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(out);
     return LANDAU_OK;
+}
+
+int landau_fp64_issue_probe(int mode, int iters, double *cycles_per_warp_instruction, double *flops_per_s) {
+    if (iters < 1 || mode < 0 || mode > 5 || !cycles_per_warp_instruction) return LANDAU_EINVAL;
+    return guarded([&]() {
+        int dev = 0, sms = 0;
+        CK(cudaGetDevice(&dev));
+        CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+        const int warps_per_smsp = mode == 4 ? 1 : 3, threads = 128 * warps_per_smsp;
+        double *in = nullptr, *out = nullptr;
+        long long *cyc = nullptr;
+        CK(cudaMalloc((void **)&in, sizeof(double) * 4096));
+        CK(cudaMalloc((void **)&out, sizeof(double)));
+        CK(cudaMalloc((void **)&cyc, sizeof(long long) * sms));
+        CK(cudaMemset(in, 0, sizeof(double) * 4096));
+        cudaEvent_t e0, e1;
+        CK(cudaEventCreate(&e0)); CK(cudaEventCreate(&e1));
+        launch_issue_probe(mode, sms, threads, iters, in, out, cyc, 0);   // warm-up
+        CK(cudaEventRecord(e0, 0));
+        const int per_iter = launch_issue_probe(mode, sms, threads, iters, in, out, cyc, 0);
+        CK(cudaEventRecord(e1, 0));
+        CK(cudaEventSynchronize(e1));
+        int rc = launches_ok();
+        float ms = 0.f;
+        CK(cudaEventElapsedTime(&ms, e0, e1));
+        std::vector<long long> h(sms);
+        CK(cudaMemcpy(h.data(), cyc, sizeof(long long) * sms, cudaMemcpyDeviceToHost));
+        const double cycles = double(*std::max_element(h.begin(), h.end()));
+        // warp instructions per sub-partition = per_iter * iters * warps on it
+        *cycles_per_warp_instruction = cycles / (double(per_iter) * iters * warps_per_smsp);
+        if (flops_per_s) {
+            const double flop_per_inst = mode == 5 ? 512.0 : 64.0;       // DMMA m8n8k4: 256 FMA; DFMA: 32 lanes
+            *flops_per_s = flop_per_inst * per_iter * double(iters) * warps_per_smsp * 4 * sms / (double(ms) * 1e-3);
+        }
+        cudaEventDestroy(e0); cudaEventDestroy(e1); cudaFree(in); cudaFree(out); cudaFree(cyc);
+        return rc;
+    });
 }
 
 }  // extern "C"

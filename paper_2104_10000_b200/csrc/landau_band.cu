@@ -101,13 +101,13 @@ int band_block(int bw) { return bw <= 256 ? 16 : (bw <= 384 ? 32 : (bw <= 832 ? 
 // device
 // ------------------------------------------------------------------------------------------------
 // scatter the CSR values into the (zeroed) band: band[m][bidx[k]] = vals[...][k]
-// grid = (ceil(nnz/256), S_g, nb)
-__global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, const int32_t *__restrict__ bidx,
+// grid = (ceil(nnz/256), S_g, nb); matrix (problem b, species s of this grid) starts at band + b pstride + s mat_doubles
+__global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, size_t pstride, const int32_t *__restrict__ bidx,
                                const double *__restrict__ vals, double *__restrict__ band) {
     const int k = blockIdx.x * blockDim.x + threadIdx.x;
     if (k >= nnz) return;
     const double v = vals[(size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz + k];
-    band[((size_t)blockIdx.z * gridDim.y + blockIdx.y) * mat_doubles + bidx[k]] = v;
+    band[(size_t)blockIdx.z * pstride + (size_t)blockIdx.y * mat_doubles + bidx[k]] = v;
 }
 
 constexpr int BAND_THREADS = 512;
@@ -135,7 +135,8 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 // every offset is a compile-time constant, so the loads of a column step are issued together), L\U written
 // back, 1/pivots left in sDi.  A short last block is completed by the identity (no kb guards later).
 template <int KB>
-__device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0, int kb, double *sD, double *sDi, int lane) {
+__device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0, int kb, double *sD, double *sDi, int lane,
+                                                  double &pmin, double &pmax) {
     double *myrow = sD + min(lane, KB - 1) * (KB + 1);
     const bool rowlane = lane < KB;        // KB < 32: the upper lanes only follow the warp barriers
     if (rowlane) {
@@ -147,7 +148,10 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 #pragma unroll
     for (int c = 0; c < KB; ++c) {
         const double *prow = sD + c * (KB + 1);
-        const double pinv = rcp_newton(prow[c]);
+        const double piv = prow[c];
+        if (c < kb) { pmin = fmin(pmin, fabs(piv)); pmax = fmax(pmax, fabs(piv)); }   // fmin/fmax drop a NaN operand ...
+        if (c < kb && !(fabs(piv) <= 1.79e308)) pmin = 0.0;                            // ... so a NaN / Inf pivot is flagged here
+        const double pinv = rcp_newton(piv);
         if (lane == c) sDi[c] = pinv;
         if (lane > c && rowlane) {
             const double l = myrow[c] * pinv;
@@ -176,21 +180,23 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
-k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restrict__ mlow, double *__restrict__ band_all) {
+k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S, const int32_t *__restrict__ mlow,
+              double *__restrict__ band_all, double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
     constexpr int DSZ = KB * (KB + 1) + KB;  // one diagonal-block buffer: sD[KB][KB+1], sDi[KB]
     double *sL = smem + 2 * DSZ;             // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
     double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;        // LD - 1
-    double *A = band_all + (size_t)blockIdx.x * mat_doubles + W;   // A(i,j) = A[i + j*lda]
+    double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, k = lane & 3;
+    double pmin = 1.79e308, pmax = 0.0;      // smallest / largest |pivot| (warp 0; uniform over its lanes)
     // Look-ahead: the diagonal block of step s+1 lies in the first 32 x 32 entries of step s's window.  Warp 0
     // updates those tiles first and then eliminates the next diagonal block while the other warps update the
     // rest of the window, so the serial elimination is off the critical path (two buffers, swapped per step).
     int cur = 0;
-    if (warp == 0) factor_diag_block<KB>(A, lda, 0, min(KB, n), smem, smem + KB * (KB + 1), lane);
+    if (warp == 0) factor_diag_block<KB>(A, lda, 0, min(KB, n), smem, smem + KB * (KB + 1), lane, pmin, pmax);
     for (int k0 = 0; k0 < n; k0 += KB) {
         const int kb = min(KB, n - k0);
         const int m = mlow[k0 / KB];         // rows below / columns right of the block inside the envelope (<= bw)
@@ -301,10 +307,14 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
             __threadfence_block();
             __syncwarp();
             double *sDn = smem + (cur ^ 1) * DSZ;
-            factor_diag_block<KB>(A, lda, k0 + kb, min(KB, n - k0 - kb), sDn, sDn + KB * (KB + 1), lane);
+            factor_diag_block<KB>(A, lda, k0 + kb, min(KB, n - k0 - kb), sDn, sDn + KB * (KB + 1), lane, pmin, pmax);
         }
         __syncthreads();
         cur ^= 1;
+    }
+    if (pivots && tid == 0) {       // [problem][all species of the ctx][2]; pivots points at this grid's first species
+        double *pv = pivots + 2 * ((size_t)(blockIdx.x / S) * pivS + blockIdx.x % S);
+        pv[0] = pmin; pv[1] = pmax;
     }
 }
 
@@ -315,7 +325,8 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, const int32_t *__restr
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
-             const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const double *__restrict__ band_all, const double *__restrict__ rhs, double *__restrict__ xout) {
+             const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, size_t pstride, const double *__restrict__ band_all,
+             const double *rhs, double *xout) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
     constexpr int SB = KB;            // same blocks as the factorisation: panels stay inside the stored band
     extern __shared__ double smem[];
     double *x = smem;                 // [n]
@@ -323,7 +334,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     const int mat = blockIdx.x;       // = b * S + sp
-    const double *A = band_all + (size_t)mat * mat_doubles + W;
+    const double *A = band_all + (size_t)(mat / S) * pstride + (size_t)(mat % S) * mat_doubles + W;
     const size_t voff = (size_t)(mat / S) * xstride + (size_t)(mat % S) * n;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     for (int i = tid; i < n; i += NT) x[i] = rhs[voff + perm[i]];
@@ -396,46 +407,51 @@ size_t band_factor_smem(int bw) {
     return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + 2 * (size_t)KB * band_mw(bw));
 }
 
-int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st) {
-    cudaMemsetAsync(band, 0, sizeof(double) * (size_t)nb * S * bs.mat_doubles, st);
+cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
+                             cudaStream_t st) {
+    // this grid's S matrices of every problem: nb rows of S mat_doubles, pstride apart
+    cudaError_t e = cudaMemset2DAsync(band, pstride * sizeof(double), 0, (size_t)S * bs.mat_doubles * sizeof(double), nb, st);
+    if (e != cudaSuccess) return e;
     dim3 grid((bs.nnz + 255) / 256, S, nb);
-    k_band_scatter<<<grid, 256, 0, st>>>(bs.nnz, vstride, bs.mat_doubles, bs.bidx, vals, band);
-    return 1;
+    k_band_scatter<<<grid, 256, 0, st>>>(bs.nnz, vstride, bs.mat_doubles, pstride, bs.bidx, vals, band);
+    return cudaGetLastError();
 }
 
 template <int KB, int NT>
-static cudaError_t factor_t(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
+static cudaError_t factor_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
     const size_t smem = band_factor_smem(bs.bw);
     cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, bs.mlow, band);
-    return cudaSuccess;
+    k_band_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, pstride, S, bs.mlow, band, pivots, pivS);
+    return cudaGetLastError();
 }
 
-cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cudaStream_t st) {
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
     switch (band_block(bs.bw)) {
-        case 32: return factor_t<32, 256>(bs, nmat, band, st);
-        case 16: return bs.bw <= 256 ? factor_t<16, 128>(bs, nmat, band, st) : factor_t<16, BAND_THREADS>(bs, nmat, band, st);
-        default: return factor_t<8, BAND_THREADS>(bs, nmat, band, st);
+        case 32: return factor_t<32, 256>(bs, nmat, S, pstride, band, pivots, pivS, st);
+        case 16: return bs.bw <= 256 ? factor_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st)
+                                     : factor_t<16, BAND_THREADS>(bs, nmat, S, pstride, band, pivots, pivS, st);
+        default: return factor_t<8, BAND_THREADS>(bs, nmat, S, pstride, band, pivots, pivS, st);
     }
 }
 
 template <int KB, int NT>
-static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
-                           cudaStream_t st) {
+static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
+                           double *x, cudaStream_t st) {
     const size_t smem = sizeof(double) * ((size_t)bs.n + KB * (KB + 1));
     cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB, NT><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, band, rhs, x);
-    return cudaSuccess;
+    k_band_solve<KB, NT><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x);
+    return cudaGetLastError();
 }
 
-cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
-                              cudaStream_t st) {
+cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
+                              double *x, cudaStream_t st) {
     switch (band_block(bs.bw)) {
-        case 32: return solve_t<32, SOLVE_NT32>(bs, nb, S, xstride, band, rhs, x, st);
-        case 16: return bs.bw <= 256 ? solve_t<16, SOLVE_NT16>(bs, nb, S, xstride, band, rhs, x, st) : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, band, rhs, x, st);
-        default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, band, rhs, x, st);
+        case 32: return solve_t<32, SOLVE_NT32>(bs, nb, S, xstride, pstride, band, rhs, x, st);
+        case 16: return bs.bw <= 256 ? solve_t<16, SOLVE_NT16>(bs, nb, S, xstride, pstride, band, rhs, x, st)
+                                     : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, st);
+        default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, st);
     }
 }
 

@@ -15,230 +15,15 @@
 #include <cstdint>
 
 #include "landau_kernels.h"
+#include "landau_launch.cuh"
+#include "landau_pair_math.cuh"
 
 namespace landau {
 
-// Programmatic dependent launch (small batches only, see launch_k): lets the next kernel of the chain be
-// scheduled while this one runs; every kernel waits here for its predecessor's results before touching memory.
-// Both instructions do nothing in a launch without the attribute.
-__device__ __forceinline__ void pdl_prologue() {
-    asm volatile("griddepcontrol.launch_dependents;");
-    asm volatile("griddepcontrol.wait;" ::: "memory");
-}
+namespace { thread_local cudaError_t g_launch_err = cudaSuccess; }
+void note_launch_error(cudaError_t e) { if (e != cudaSuccess && g_launch_err == cudaSuccess) g_launch_err = e; }
+cudaError_t take_launch_error() { const cudaError_t e = g_launch_err; g_launch_err = cudaSuccess; return e; }
 
-template <class... KArgs, class... Args>
-static void launch_k(void (*kern)(KArgs...), dim3 grid, dim3 block, cudaStream_t st, bool pdl, Args... args) {
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = grid; cfg.blockDim = block; cfg.dynamicSmemBytes = 0; cfg.stream = st;
-    cudaLaunchAttribute attr[1];
-    attr[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
-    attr[0].val.programmaticStreamSerializationAllowed = 1;
-    cfg.attrs = attr; cfg.numAttrs = pdl ? 1 : 0;
-    cudaLaunchKernelEx(&cfg, kern, KArgs(args)...);
-}
-constexpr int PDL_MAX_NB = 8;   // launch-latency bound batches
-
-// ------------------------------------------------------------------------------------------------
-// fast fp64 reciprocal / square roots: MUFU seed (relative error < 2^-19 including the truncation
-// of the operand to its high word) + ONE cubic correction on the DFMA pipe (error ~ seed^3 < 1e-17).
-// Not IEEE-rounded (~1 ulp), no special cases: arguments here are finite and > 0.
-// ------------------------------------------------------------------------------------------------
-__device__ __forceinline__ double rcp_fast(double x) {
-    double y;
-    asm("rcp.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double e = fma(-x, y, 1.0);
-    const double p = fma(e, e, e);      // e + e^2
-    return fma(y, p, y);                // y (1 + e + e^2)
-}
-
-// g = sqrt(x), yy = 1/sqrt(x)
-__device__ __forceinline__ void sqrt_rsqrt_fast(double x, double &g, double &yy) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double t = x * y;
-    const double r = fma(-t, y, 1.0);   // 1 - x y^2
-    double p = fma(0.375, r, 0.5);
-    p = p * r;                          // r/2 + 3 r^2/8
-    g = fma(t, p, t);
-    yy = fma(y, p, y);
-}
-
-// 2 sqrt(x) = t (2 + r + 3 r^2/4), t = x y, r = 1 - x y^2: the factor 2 sits in the correction
-// polynomial, so the scaled AGM below needs no multiplication by 1/2 or 2 and no integer fix-up.
-__device__ __forceinline__ double sqrt_times2_fast(double x) {
-    double y;
-    asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
-    const double t = x * y;
-    const double r = fma(-t, y, 1.0);
-    const double p = fma(0.75, r, 1.0);
-    const double q = fma(p, r, 2.0);
-    return t * q;
-}
-
-// x * 2^e for a normal positive x that stays normal (integer add on the exponent field)
-__device__ __forceinline__ double scale_pow2(double x, int e) {
-    return __hiloint2double(__double2hiint(x) + (e << 20), __double2loint(x));
-}
-
-// ------------------------------------------------------------------------------------------------
-// a3: pair kernel.  PAPER.md Alg. 1 lines 3-12 (L114-121), Eqs. 7-8 (L65-67).
-//
-// Azimuth-integrated Landau tensor through a SCALED arithmetic-geometric mean (DESIGN.md "Elliptic
-// integrals on the device").  With a0 = sqrt(s), b0 = sqrt(d2), q = 4 r rb = s - d2 and
-// A_k = 2^k a_k, B_k = 2^k b_k:
-//     A_{k+1} = A_k + B_k,  B_{k+1} = 2 sqrt(A_k B_k),  C_{k+1} = A_k - B_k = 2^{k+1} c_{k+1}
-//     (powers of two are applied at the end by integer adds on the exponent field)
-//     K(m)/sqrt(s) = pi/(2 lim a_k) = pi 2^k / A_{k+1}
-//     W = [sum_{k>=1} 2^k c_k^2]/q^2 = 1/(2 A_1^2) + (sum_{k>=2} C_k^2 / 2^k)/q^2   (c_1 = q/(4 a_1))
-//     Pss = 16 Kt W,  Pc = 4 Kt (1 + q W)/s,  P0 = 2 Kt (s + d2 - q^2 W)/(s d2),  Kt = K/sqrt(s)
-// every sum has positive terms except the bracket of P0 (= 2 s E/K: bounded cancellation ~ K/E).
-// Evaluated with rho2 = 2 r rb = q/2, 2W and 4Kt so that no multiplication by a power of two remains:
-//     g = 1 + q W = 1 + rho2 (2W),  Pss/2 = (4Kt)(2W),  Pc = (4Kt/s) g,  P0 = (4Kt/s)(s - rho2 g)/d2
-//     (s - rho2 g = (s + d2 - q^2 W)/2 because s - d2 = q).
-// The iteration stops for the whole warp once every lane's next c would be <= 2^-26 a (the a used
-// for K is then within 2^-54 a of the limit).  The test compares exponents with integer ops, one
-// pass ahead.
-//
-// FP64 issue cost on sm_100a (measured): 2 cycles per warp instruction and SM
-// sub-partition, 3 cycles for a DFMA with three distinct register operands; 9 cycles dependent
-// latency.  Hence the lock-step evaluation of several pairs per thread and the care for operand count.
-// ------------------------------------------------------------------------------------------------
-struct PairAcc { double drr, drz, dzz, kr, kz; };
-
-constexpr int AGM_MAX_STEPS = 8;
-constexpr int AGM_EXIT_SHIFT = 11;
-// After the exit vote one more AGM step is taken (for K), but its C is no longer added to the series of W:
-// c <= 2^-26 a there, a term below 2^-45 of W (measured: worst block error 4.5e-13 -> 6.6e-13 over all parity
-// cases, 3 FP64 instructions per pair fewer, 290.6 -> 301.0 GPair/s).  0 keeps the term.
-#ifndef AGM_SKIP_LAST_TERM
-#define AGM_SKIP_LAST_TERM 1
-#endif   // exit vote: C_{k+1} <= 2^-11 A_k (see pair_parts)
-
-// What a thread keeps of one of its i points.
-struct IPoint {
-    double r, z;
-    double r2x;     // 2 r
-    double rr2;     // 2 r^2
-    double c;       // 1/(16 r^2): 1/q^2 = c_i / r_j^2
-    double tD, tKr, tKz;
-};
-// One j point, read from shared memory (SoA there, see k_pair_sym).
-struct JPoint { double r, z, invr2, rr2, tD, tKr, tKz; };
-
-// P0, Pc and Pss/2 of a pair plus the geometry the tensor entries need (rho2 = 2 r_i r_j).
-struct PairParts { double P0, Pc, Pssh, dz, dr, dr2, rho2; };
-
-// NP pairs (i_u, j), u < NP, evaluated in lock-step: NP independent dependency chains per thread
-// through the AGM, one exit vote for all of them.
-template <int NP, bool CHECK_SELF>
-__device__ __forceinline__ void pair_parts(const IPoint (&pi)[NP], const JPoint &pj, PairParts (&pp)[NP]) {
-    double s[NP], ys[NP], yd[NP], iA1[NP], A[NP], B[NP], V[NP];
-    bool self[NP];
-#pragma unroll
-    for (int u = 0; u < NP; ++u) {
-        pp[u].dz = pi[u].z - pj.z; pp[u].dr = pi[u].r - pj.r;
-        const double dz2 = pp[u].dz * pp[u].dz;
-        pp[u].dr2 = pp[u].dr * pp[u].dr;
-        double d2 = pp[u].dr2 + dz2;
-        pp[u].rho2 = pi[u].r2x * pj.r;
-        self[u] = false;
-        if (CHECK_SELF) {             // coincident pair (j == i): contributes nothing (reading Q3)
-            self[u] = !(d2 > 0.0);
-            if (self[u]) d2 = 1.0;
-        }
-        s[u] = fma(2.0, pp[u].rho2, d2);                 // (r_i + r_j)^2 + dz^2 = d2 + 4 r_i r_j
-        double a0, b0;
-        sqrt_rsqrt_fast(s[u], a0, ys[u]);
-        sqrt_rsqrt_fast(d2, b0, yd[u]);
-        A[u] = a0 + b0;                                  // A_1 = 2 a_1
-        B[u] = sqrt_times2_fast(a0 * b0);
-        iA1[u] = rcp_fast(A[u]);
-        V[u] = 0.0;
-    }
-    // Rolled loop, state in fixed registers.  V_P = 2 V_{P-1} + C_{P+1}^2, so after P passes
-    // sum_{k>=2} C_k^2/2^k = V / 2^{P+1}, and 4 K/sqrt(s) = 4 pi 2^P / A_{P+1}.
-    // The exit is decided ONE PASS AHEAD so that the branch never waits on fresh data:
-    // c_{k+2} = c_{k+1}^2/(4 a_{k+2}) exactly, hence C_{k+1} <= 2^-11 A_k (c_{k+1} <= 2^-12 a) in every
-    // lane guarantees c_{k+2} <= 2^-26 a after the next pass, which is then the last (its C only feeds
-    // V); the a_{k+2} used for K is then within c_{k+3} <= 2^-54 a of the AGM limit.
-    int P = 0;                 // completed (C, V) updates = completed AGM steps
-    bool last = false;
-#pragma unroll 1
-    for (;;) {
-#if AGM_SKIP_LAST_TERM
-        if (last || P == AGM_MAX_STEPS) break;     // the last C (c <= 2^-26 a: a term <= 2^-45 of W) is not added to V
-#endif
-        bool conv = true;
-#pragma unroll
-        for (int u = 0; u < NP; ++u) {
-            const double C = A[u] - B[u];
-            V[u] = fma(V[u], 2.0, C * C);
-            conv = conv && (__double2hiint(C) + (AGM_EXIT_SHIFT << 20) <= __double2hiint(A[u]));
-        }
-#if !AGM_SKIP_LAST_TERM
-        ++P;
-        if (last || P == AGM_MAX_STEPS) break;
-#endif
-        last = __all_sync(0xffffffffu, conv);
-#pragma unroll
-        for (int u = 0; u < NP; ++u) {
-            const double X = A[u] * B[u];
-            A[u] = A[u] + B[u];
-            B[u] = sqrt_times2_fast(X);
-        }
-#if AGM_SKIP_LAST_TERM
-        ++P;
-#endif
-    }
-#if AGM_SKIP_LAST_TERM
-    const int PK = P + 1, PV = P;      // K: 4 pi 2^(P+1) / A_(P+2);  sum_{k>=2} C_k^2 / 2^k = V / 2^(P+1)
-#else
-    const int PK = P, PV = P;
-#endif
-#pragma unroll
-    for (int u = 0; u < NP; ++u) {
-        const double Af = A[u] + B[u];
-        const double K4 = scale_pow2(12.566370614359172953850573533118 * rcp_fast(Af), PK);   // 4 K/sqrt(s)
-        // 2 W = 1/A_1^2 + V 2^-P / q^2.  1/q^2 is a normal number far from the exponent limits (V may be
-        // 0 for far pairs: scale 1/q^2, not the product).
-        const double invq2 = pi[u].c * pj.invr2;
-        const double W2 = fma(iA1[u], iA1[u], V[u] * scale_pow2(invq2, -PV));
-        const double g = fma(pp[u].rho2, W2, 1.0);       // 1 + q W
-        const double Kh = K4 * (ys[u] * ys[u]);          // 4 K / s^(3/2)
-        pp[u].Pssh = K4 * W2;
-        pp[u].Pc = Kh * g;
-        pp[u].P0 = (Kh * (yd[u] * yd[u])) * fma(-pp[u].rho2, g, s[u]);   // (s + d2 - q^2 W)/2 = s - rho2 (1 + q W)
-        if (CHECK_SELF && self[u]) { pp[u].Pssh = 0.0; pp[u].Pc = 0.0; pp[u].P0 = 0.0; }
-    }
-}
-
-// The five distinct tensor entries of a pair (Q1) from its parts:
-//   UDrr = U^D_rr(i,j), UDrrT = U^D_rr(j,i), A2 = -U^D_rz(i,j) = -U^K_zr(j,i), A3 = U^D_zz = U^K_zz (both ways),
-//   A4 = U^K_rr (both ways), A5 = U^K_zr(i,j) = U^D_rz(j,i)
-struct PairTensor { double UDrr, UDrrT, A2, A3, A4, A5; };
-
-__device__ __forceinline__ PairTensor pair_tensor(const IPoint &pi, const JPoint &pj, const PairParts &pp) {
-    PairTensor t;
-    const double dzP0 = pp.dz * pp.P0;
-    const double A1 = pp.dz * dzP0;                      // dz^2 P0
-    const double b = pp.dr * dzP0;                       // dz dr P0
-    const double e = pp.dz * pp.Pc;
-    t.A2 = fma(pj.r, e, b);                              // dz (dr P0 + r_j Pc)
-    t.A5 = fma(pi.r, e, -b);                             // dz (-dr P0 + r_i Pc)
-    t.A3 = fma(pp.dr2, pp.P0, pp.rho2 * pp.Pc);          // dr^2 P0 + 2 r_i r_j Pc
-    t.A4 = fma(pp.rho2, pp.Pssh, fma(-pp.dz, e, A1));    // dz^2 (P0 - Pc) + r_i r_j Pss
-    t.UDrr = fma(pj.rr2, pp.Pssh, A1);                   // r_j^2 Pss + dz^2 P0
-    t.UDrrT = fma(pi.rr2, pp.Pssh, A1);
-    return t;
-}
-
-__device__ __forceinline__ void accumulate_i(PairAcc &acc, const JPoint &pj, const PairTensor &t) {
-    acc.drr = fma(pj.tD, t.UDrr, acc.drr);
-    acc.drz = fma(-pj.tD, t.A2, acc.drz);
-    acc.dzz = fma(pj.tD, t.A3, acc.dzz);
-    acc.kr = fma(t.A4, pj.tKr, fma(-t.A2, pj.tKz, acc.kr));
-    acc.kz = fma(t.A5, pj.tKr, fma(t.A3, pj.tKz, acc.kz));
-}
 
 // ------------------------------------------------------------------------------------------------
 // Symmetric tile-pair kernel.  P0, Pc, Pss are exchange-symmetric and
@@ -387,7 +172,9 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
 constexpr int FIELD_EPB = 8;
 constexpr int FIELD_ROUNDS = 4;   // cells per thread: the tabulation rows stay in registers across them
 
-__global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, double *__restrict__ T) {
+// TILED: T in the layout of the batch-shared contraction (landau_shared.cu): T[c][jo][b][k][h], j = 8 jo + 4 h + k.
+template <bool TILED>
+__global__ void k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T) {
     pdl_prologue();
     __shared__ double s_u[FIELD_EPB][16];
     const int b = blockIdx.y;
@@ -436,7 +223,13 @@ __global__ void k_fields_beta(DeviceSpace ds, const double *__restrict__ f, doub
         if (valid) {
             const int gi = e * ds.Nq + q;
             const double w = ds.w_in[gi];
-            Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
+            if (TILED) {
+                const int j = ds.poff + gi;
+                const size_t o = (((size_t)(j >> 3) * nbpad + b) * 4 + (j & 3)) * 2 + ((j >> 2) & 1), cs = (size_t)Kq8 * nbpad * 8;
+                T[o] = w * tD; T[cs + o] = w * tKr; T[2 * cs + o] = w * tKz;
+            } else {
+                Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
+            }
         }
     }
 }
@@ -705,6 +498,52 @@ __global__ void k_dfma_probe(int iters, double *out) {
     if (s == 12345.678) out[0] = s;  // keep the chains alive
 }
 
+// FP64 issue-rate probes (measurement aid; the numbers behind the "issue bound" of DESIGN.md 6.1).  Three warps
+// per SM sub-partition, 8 independent register-resident chains per thread; clock64() of one block per SM.
+//   MODE 0  DFMA, two register operands + an immediate          x = fma(x, y, 1.5)
+//   MODE 1  DFMA, two DISTINCT registers (one used twice)       x = fma(y, y, x)
+//   MODE 2  DFMA, three distinct registers                      x = fma(y, z, x)
+//   MODE 3  DFMA, three registers, one shared by neighbours     x = fma(x, Y, z)   (operand reuse cache)
+//   MODE 4  one dependent DFMA chain, one warp per sub-partition (latency)
+//   MODE 5  DMMA m8n8k4, 8 independent accumulators per warp
+template <int MODE>
+__global__ void k_issue_probe(int iters, const double *__restrict__ in, double *out, long long *cycles) {
+    constexpr int CH = 8;
+    double x[CH], y[CH], z[CH];
+#pragma unroll
+    for (int c = 0; c < CH; ++c) { x[c] = in[threadIdx.x + c]; y[c] = in[threadIdx.x + 32 + c]; z[c] = in[threadIdx.x + 64 + c]; }
+    double Y = in[threadIdx.x + 100];
+    __syncthreads();
+    const long long t0 = clock64();
+    for (int i = 0; i < iters; ++i) {
+        if (MODE == 4) {
+#pragma unroll
+            for (int c = 0; c < CH; ++c) x[0] = fma(x[0], y[0], 1.5);
+        } else if (MODE == 5) {
+#pragma unroll
+            for (int c = 0; c < CH; c += 2)
+                asm volatile("mma.sync.aligned.m8n8k4.row.col.f64.f64.f64.f64 {%0,%1}, {%2}, {%3}, {%0,%1};"
+                             : "+d"(x[c]), "+d"(x[c + 1]) : "d"(y[c]), "d"(z[c]));
+        } else {
+#pragma unroll
+            for (int c = 0; c < CH; ++c) {
+                if (MODE == 0) x[c] = fma(x[c], y[c], 1.5);
+                if (MODE == 1) x[c] = fma(y[c], y[c], x[c]);
+                if (MODE == 2) x[c] = fma(y[c], z[c], x[c]);
+                if (MODE == 3) x[c] = fma(x[c], Y, z[c]);
+            }
+            if (MODE == 3) Y += 1e-30;
+        }
+    }
+    const long long t1 = clock64();
+    __syncthreads();
+    double sum = 0.0;
+#pragma unroll
+    for (int c = 0; c < CH; ++c) sum += x[c] + y[c] + z[c];
+    if (sum == 12345.678) out[0] = sum;     // keep the chains alive
+    if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
+}
+
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
@@ -717,7 +556,14 @@ int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
     constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
     dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
-    launch_k(k_fields_beta, grid, block, st, nb <= PDL_MAX_NB, ds, f, T);
+    launch_k(k_fields_beta<false>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, 0, 0, f, T);
+    return 1;
+}
+
+int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, cudaStream_t st) {
+    constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
+    dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
+    launch_k(k_fields_beta<true>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, shared_kpad(ds.Ntot) / 8, nbpad, f, T);
     return 1;
 }
 
@@ -727,9 +573,9 @@ static void launch_pair_t(int N, const double *r, const double *z, const double 
     const int ts = pair_tile_size(N), nt = pair_tiles(N);
     dim3 grid(nt * (nt + 1) / 2, nb);
     const bool pdl = nb <= PDL_MAX_NB;
-    if (ts == 128) launch_k(k_pair_sym<128, 2, CHECK_ALL>, grid, dim3(64), st, pdl, N, nt, r, z, invr, T, Gpart);
-    else if (ts == 64) launch_k(k_pair_sym<64, 2, CHECK_ALL>, grid, dim3(32), st, pdl, N, nt, r, z, invr, T, Gpart);
-    else launch_k(k_pair_sym<32, 1, CHECK_ALL>, grid, dim3(32), st, pdl, N, nt, r, z, invr, T, Gpart);
+    if (ts == 128) launch_k(k_pair_sym<128, 2, CHECK_ALL>, grid, dim3(64), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
+    else if (ts == 64) launch_k(k_pair_sym<64, 2, CHECK_ALL>, grid, dim3(32), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
+    else launch_k(k_pair_sym<32, 1, CHECK_ALL>, grid, dim3(32), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
 }
 
 int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
@@ -743,13 +589,13 @@ int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, c
                    const double *Ez, double shift, cudaStream_t st) {
     if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
         dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
-        if (Ez) launch_k(k_element_q3<true>, grid, dim3(ELQ3_WARPS * 32), st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, Ez, shift);
-        else launch_k(k_element_q3<false>, grid, dim3(ELQ3_WARPS * 32), st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, (const double *)nullptr, 0.0);
+        if (Ez) launch_k(k_element_q3<true>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, Ez, shift);
+        else launch_k(k_element_q3<false>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, (const double *)nullptr, 0.0);
         return 1;
     }
     dim3 grid(ds.Ne, nb);
-    if (Ez) launch_k(k_element<true>, grid, dim3(ds.Nb * ds.Nb), st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, Ez, shift);
-    else launch_k(k_element<false>, grid, dim3(ds.Nb * ds.Nb), st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, (const double *)nullptr, 0.0);
+    if (Ez) launch_k(k_element<true>, grid, dim3(ds.Nb * ds.Nb), 0, st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, Ez, shift);
+    else launch_k(k_element<false>, grid, dim3(ds.Nb * ds.Nb), 0, st, nb <= PDL_MAX_NB, ds, jsplit, f, G, Ce, ce, (const double *)nullptr, 0.0);
     return 1;
 }
 
@@ -774,36 +620,49 @@ int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fst
                        double *vals, double *Cf, cudaStream_t st) {
     const int bv = (ds.nnz + 255) / 256, bc = (ds.n + 255) / 256;
     dim3 grid(bv + bc, ds.S, nb);
-    launch_k(k_gather2, grid, dim3(256), st, nb <= PDL_MAX_NB, ds, bv, vstride, fstride, Ce, ce, vals, Cf);
+    launch_k(k_gather2, grid, dim3(256), 0, st, nb <= PDL_MAX_NB, ds, bv, vstride, fstride, Ce, ce, vals, Cf);
     return 1;
 }
 
 int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st) {
     dim3 grid((ds.nnz + 255) / 256, (nspecies + 1) / 2, nb);
-    k_gather<<<grid, 256, 0, st>>>(ds.nnz, nspecies, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
+    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.nnz, nspecies, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
     return 1;
 }
 
 int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st) {
     dim3 grid((ds.n + 255) / 256, (ds.S + 1) / 2, nb);
-    k_gather<<<grid, 256, 0, st>>>(ds.n, ds.S, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
+    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.n, ds.S, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
     return 1;
 }
 
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st) {
-    k_mass_element<<<ds.Ne, ds.Nb * ds.Nb, 0, st>>>(ds, shift, Ce);
+    launch_k(k_mass_element, dim3(ds.Ne), dim3(ds.Nb * ds.Nb), 0, st, false, ds, shift, Ce);
     return 1;
 }
 
 int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
     const int n5 = 5 * Ntot;
     dim3 grid((n5 + 255) / 256, nb);
-    launch_k(k_sum_partials, grid, dim3(256), st, nb <= PDL_MAX_NB, n5, jsplit, Gpart, G);
+    launch_k(k_sum_partials, grid, dim3(256), 0, st, nb <= PDL_MAX_NB, n5, jsplit, Gpart, G);
     return 1;
 }
 
+// returns the warp instructions each warp issues per iteration of the probe loop (0: unknown mode)
+int launch_issue_probe(int mode, int blocks, int threads, int iters, const double *in, double *out, long long *cycles, cudaStream_t st) {
+    switch (mode) {
+        case 0: launch_k(k_issue_probe<0>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 1: launch_k(k_issue_probe<1>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 2: launch_k(k_issue_probe<2>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 3: launch_k(k_issue_probe<3>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 4: launch_k(k_issue_probe<4>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 5: launch_k(k_issue_probe<5>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 4;
+        default: return 0;
+    }
+}
+
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st) {
-    k_dfma_probe<<<blocks, threads, 0, st>>>(iters, out);
+    launch_k(k_dfma_probe, dim3(blocks), dim3(threads), 0, st, false, iters, out);
     return 1;
 }
 

@@ -35,13 +35,26 @@ struct DeviceSpace {
 
 // Scratch for up to max_batch problems (N = points of all grids together).
 struct Scratch {
-    double *T;      // [nb][3][N]
-    double *G;      // [nb][ntiles][5][N]: per source tile partial sums of G_D, G_K
+    double *T;      // per-problem path: [nb][3][N]; batch-shared path: [3][Kpad/8][nbpad][8]
+    double *G;      // per-problem path: [nb][ntiles][5][N] per source tile partial sums of G_D, G_K;
+                    // batch-shared path: [nb][ksplit][5][N]
     double *Gsum;   // [nb][5][N]: G_D (rr,rz,zz), G_K (r,z) after the tile-order sum
+    double *U;      // batch-shared path: [5][Kpad/8][Mpad][8] tensor entries of all ordered pairs
 };
 
 // each returns the number of kernels launched
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
+
+// Batch-shared path (landau_shared.cu): the tensor of every ordered pair is evaluated once per call into
+// U[5][Kpad/8][Mpad][8] and applied to all problems by an fp64 tensor-core contraction with T[3][Kpad/8][nbpad][8].
+int shared_kpad(int N);      // 16 ceil(N/16): source points padded to whole chunks
+int shared_mpad(int N);      // target points padded to whole tiles
+int shared_nbpad(int nb);    // problems padded to whole tiles
+int shared_ksplit(int N);    // segments of the j range (a function of N only: fixes the summation order)
+int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, cudaStream_t st);
+int launch_pair_tensor(int N, const double *r, const double *z, const double *invr, double *U, cudaStream_t st);
+// Gpart[b][ksplit][5][N]
+int launch_apply(int N, int nb, int nbpad, const double *U, const double *T, double *Gpart, cudaStream_t st);
 // pair kernel over the union of points (r, z, invr: [Ntot]); check_all: test every pair for coincidence
 // (needed only when points of different grids coincide), else only the diagonal tiles
 int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
@@ -58,6 +71,7 @@ int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fst
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
 int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
+int launch_issue_probe(int mode, int blocks, int threads, int iters, const double *in, double *out, long long *cycles, cudaStream_t st);
 
 // Band LU (landau_band.cu; section III-G)
 struct BandSpace {
@@ -71,10 +85,14 @@ struct BandSpace {
 void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw);
 int band_block(int bw);        // KB, a function of bw only
 size_t band_factor_smem(int bw);
-int launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, const double *vals, double *band, cudaStream_t st);
-cudaError_t launch_band_factor(const BandSpace &bs, int nmat, double *band, cudaStream_t st);
-cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, const double *band, const double *rhs, double *x,
-                              cudaStream_t st);
+// band points at this grid's block of problem 0; matrix (problem b, species s) = band + b pstride + s mat_doubles
+// (problem-major workspace: a solve may use a different nb than the factorisation)
+cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
+                             cudaStream_t st);
+// pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st);
+cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
+                              double *x, cudaStream_t st);
 
 int pair_tile_size(int N);
 int pair_tiles(int N);
