@@ -7,15 +7,25 @@ problems on the refined Q3 mesh "3B" (308 cells, 4,928 points, 2 species), one
 landau_jacobian_batched call.  value = ordered point pairs N(N-1) x problems / time, whole job.
 
   python bench.py [--gpus N] [--steps K] [--warmup W] [--impl ours|reference]
+  python bench.py --kernel-run single|batched|main     # launches only (for ncu), prints the launch plan
+  python bench.py --summarise-ncu RAW.csv [...]        # ncu --page raw --csv export(s) -> roofline-input CSV on stdout
 
 N > 1: launched by torchrun, one rank per GPU; the problems are independent (weak scaling: every
 rank builds its own 512 problems, no data-path collective).
 --impl reference: times the CPU oracle (double instantiation) on the host cores on a bounded
 sample of the same workload.
+
+The step goes through the library's default path for a batch (LANDAU_PAIR_SHARED, include/landau.h): the tensor
+of every ordered point pair is evaluated once per call (k_pair_tensor) and applied to all problems by an fp64
+tensor-core contraction (k_apply_dmma); `value` still counts N(N-1) pair interactions per problem, `builds_per_s`
+is the unambiguous figure.  The per-problem path (k_pair_sym: every problem evaluates every pair itself) is timed
+on the same workload and reported under `per_problem_path`.
 """
 from __future__ import annotations
 
 import argparse
+import csv
+import hashlib
 import json
 import os
 import subprocess
@@ -32,24 +42,43 @@ import numpy as np
 METRIC = "landau_jacobian_gpair_evals_per_s"
 UNIT = "GPair/s"
 WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cells, 4928 points)"
-# FP64 flop (2 DFMA + DMUL + DADD) and FP64-pipe instructions the pair kernel executes per ORDERED
-# pair on this workload, ncu-counted (profiles/r01e_pair_kernel.md).
-FLOP_PER_PAIR = 75.27
-FP64_INST_PER_PAIR = 48.51
-# of which DFMAs with three distinct register operands: they issue in 3 cycles instead of 2
-# (measured), so the issue-cycle cost per ordered pair is 2 x 48.51 + 11.09 SMSP-cycles x 32 lanes.
-FP64_3OP_INST_PER_PAIR = 11.09
-FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock (B200: 148 x 64 x 2 x 1.965 GHz = 37.2 TF)
-# dram__bytes_read.sum + dram__bytes_write.sum of one k_pair_sym launch on this workload, from the
-# ncu --set full capture summarised in profiles/r01e_pair_kernel.md (68.7 MB read + 3.879 GB written:
-# the per-source-tile partial slabs; the algorithmic minimum is 24 B/point in + 40 B/point out = 0.16 GB).
-PAIR_KERNEL_DRAM_BYTES = 68.7e6 + 3.8789e9
-# the same for the rest of the step (fields, slab sum, element matrices, two gathers), profiles/r01e_step_kernels.md (ncu --set full, dram read + write)
-REST_DRAM_BYTES = 6.03e9   # 4.04 GB of it is k_sum_partials reading the slabs
+FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock = 4 sub-partitions x one DMMA.8x8x4 (256 FMA) per 16 clocks
+APPLY_FLOP_PER_PAIR = 14.0  # k_apply_dmma: seven products per ordered pair and problem (landau_shared.cu)
+CSRC = os.path.join(ROOT, "paper_2104_10000_b200", "csrc")
+KERNEL_SOURCES = ["landau_kernels.cu", "landau_shared.cu", "landau_pair_math.cuh", "landau_launch.cuh", "landau_kernels.h"]
+ROOFLINE_INPUTS = os.path.join(ROOT, "profiles", "r02_roofline_inputs.csv")
+
+# (key, inputs.config number, variant, problems of the batched run: >= 10 ms of pair work on the per-problem path)
+CONFIGS = [("cfg1", 1, "B", 8192), ("cfg2", 2, "B", 512), ("cfg3A", 3, "A", 1024), ("cfg3B", 3, "B", 256),
+           ("cfg4B", 4, "B", 256), ("ctx80", 6, "B", 1024), ("ctx320", 7, "B", 128)]
+
+
+def kernel_source_sha() -> str:
+    h = hashlib.sha256()
+    for name in KERNEL_SOURCES:
+        h.update(open(os.path.join(CSRC, name), "rb").read())
+    return h.hexdigest()[:16]
+
+
+def load_roofline_inputs():
+    """profiles/r02_roofline_inputs.csv (written by `bench.py --summarise-ncu`): ncu-counted FP64 instructions and
+    DRAM bytes per launch, keyed by (kernel, workload).  Rows whose source hash differs from the kernel sources in
+    the tree are ignored (the numbers then print as null)."""
+    out = {}
+    try:
+        sha = kernel_source_sha()
+        with open(ROOFLINE_INPUTS) as fh:
+            for row in csv.DictReader(l for l in fh if not l.startswith("#")):
+                if row["source_sha"] == sha:
+                    out[(row["kernel"], row["workload"])] = {k: (float(v) if v not in ("", None) else None)
+                                                             for k, v in row.items() if k not in ("kernel", "workload", "source_sha")}
+    except Exception:
+        pass
+    return out
 
 
 class ClockSampler(threading.Thread):
-    """One `nvidia-smi -lms 50` process sampling clocks / throttle reasons DURING the timed region
+    """One `nvidia-smi -lms 20` process sampling clocks / throttle reasons DURING the timed region
     (B200_PROFILING.md recipe); its lines are read by this thread."""
 
     QUERY = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
@@ -60,7 +89,7 @@ class ClockSampler(threading.Thread):
         self.rows, self.proc = [], None
         try:
             self.proc = subprocess.Popen(["nvidia-smi", f"--query-gpu={self.QUERY}", "--format=csv,noheader,nounits",
-                                          "-lms", "50", "-i", str(index)], stdout=subprocess.PIPE, text=True)
+                                          "-lms", "20", "-i", str(index)], stdout=subprocess.PIPE, text=True)
         except Exception:
             self.proc = None
 
@@ -91,25 +120,50 @@ class ClockSampler(threading.Thread):
                 "power_w_max": max(pw) if pw else None, "reasons": reasons, "samples": len(rows)}
 
 
-CPU_SAMPLE_PROBLEMS = 8      # of the 512: ~0.5 s each on 16 cores, i.e. tens of core-seconds in total
-
-
-def cpu_baseline_sample(wl, inputs):
-    """The oracle as it stands (double instantiation) on a bounded sample of the workload."""
-    from oracle import landau_oracle as oracle
-    oracle.build()
-    sp = oracle.build_space(wl.mesh, wl.order)
-    fs = [inputs.nodal_f(wl, sp.dof_r, sp.dof_z, b) for b in range(CPU_SAMPLE_PROBLEMS)]
+# ------------------------------------------------------------------------------------------------------------------
+# CPU baseline: the oracle as it stands (double instantiation of the pair loop, OpenMP over i; numpy for the rest)
+# ------------------------------------------------------------------------------------------------------------------
+def oracle_step(oracle, sp, species, f):
+    """Steps a1-a7 of one problem on an already built Space (the GPU side's ctx is created outside its timed region
+    as well): pair loop + scaling, element matrices, dense assembly -> CSR values, C(f).  Returns
+    (seconds of the whole step, seconds of the pair loop alone)."""
     t0 = time.perf_counter()
-    for f in fs:
-        oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
-    dt = time.perf_counter() - t0
-    pairs = CPU_SAMPLE_PROBLEMS * sp.N * (sp.N - 1)
-    return pairs / dt * 1e-9, dt, os.cpu_count()
+    fq, dfr, dfz = oracle.fields_at_points(sp, f)
+    e2 = np.asarray(species.charge, dtype=np.float64) ** 2
+    m0m = species.m0 / np.asarray(species.mass, dtype=np.float64)
+    t1 = time.perf_counter()
+    oracle.inner_integral(sp.r, sp.z, sp.w_in, fq, dfr, dfz, e2, m0m, None, "d")
+    t_pair = time.perf_counter() - t1
+    K, D, _ = oracle.coefficients(sp, species, f, None, "d")          # (runs the pair loop again: subtracted below)
+    Ce = oracle.element_matrices(sp, K, D)
+    for a in range(f.shape[0]):
+        oracle.csr_values(sp, oracle.assemble_dense(sp, Ce[a]))
+    oracle.collision(sp, species, f, "d", (K, D))
+    t_all = time.perf_counter() - t0
+    return t_all - t_pair, t_pair      # the pair loop ran twice: count it once
+
+
+def cpu_baseline(oracle, inputs, wl, problems, reps=1):
+    """Median over `reps` of the oracle's time for the listed problems of a workload."""
+    sp = oracle.build_space(wl.mesh, wl.order)
+    fs = [inputs.nodal_f(wl, sp.dof_r, sp.dof_z, b) for b in problems]
+    tot, pair = [], []
+    for _ in range(reps):
+        ta = tp = 0.0
+        for f in fs:
+            a, p = oracle_step(oracle, sp, wl.species, f)
+            ta += a; tp += p
+        tot.append(ta); pair.append(tp)
+    pairs = len(problems) * sp.N * (sp.N - 1)
+    t, tpair = float(np.median(tot)), float(np.median(pair))
+    return {"value": pairs / t * 1e-9, "unit": UNIT, "cores": os.cpu_count(), "kind": "oracle",
+            "builds_per_s": len(problems) / t, "seconds": t, "pair_loop_only_gpair_per_s": pairs / tpair * 1e-9,
+            "pair_loop_share": tpair / t, "reps": reps}
 
 
 def run_reference(args):
-    """--impl reference: the CPU oracle on the host cores, each step one problem of config 5."""
+    """--impl reference: the CPU oracle on the host cores, each step one problem of config 5 (a1-a7 on a Space
+    built once, as the GPU arm's ctx is)."""
     rank = int(os.environ.get("RANK", "0"))
     if rank != 0:
         return
@@ -122,13 +176,13 @@ def run_reference(args):
     times = []
     for k in range(args.warmup + args.steps):
         f = inputs.nodal_f(wl, sp.dof_r, sp.dof_z, k)
-        t0 = time.perf_counter()
-        oracle.build_all(wl.mesh, wl.order, wl.species, f, 1.0, precision="d")
+        t, _ = oracle_step(oracle, sp, wl.species, f)
         if k >= args.warmup:
-            times.append(time.perf_counter() - t0)
-    ms = 1e3 * float(np.mean(times))
+            times.append(t)
+    ms = 1e3 * float(np.median(times))
     val = pairs / (ms * 1e-3) * 1e-9
-    sample = "1 of the 512 problems per step (full N=4928 mesh, a1-a8), double-precision oracle, OpenMP over i"
+    sample = ("1 of the 512 problems per step (full N=4928 mesh, a1-a7 on a Space built once), double-precision oracle, "
+              "OpenMP over i in the pair loop, numpy elsewhere; median step")
     print(json.dumps({
         "impl": "reference", "metric": METRIC, "value": val, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
         "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -139,51 +193,130 @@ def run_reference(args):
     }))
 
 
-def time_single_config(binding, inputs, torch, k, variant="B", reps=20):
-    """Single-problem build (split launch shape) of configs 1-4: device time per build."""
-    wl = inputs.config(k, variant=variant)
-    ctx = binding.LandauContext(wl.mesh, wl.order, wl.species, 1)
+# ------------------------------------------------------------------------------------------------------------------
+# GPU timing helpers
+# ------------------------------------------------------------------------------------------------------------------
+def make_problem(binding, inputs, torch, wl, nb, path=0):
+    ctx = binding.LandauContext(wl.mesh, wl.order, wl.species, nb, pair_path=path)
     r, z = ctx.dof_coords()
-    f = torch.from_numpy(inputs.nodal_f(wl, r, z)).cuda()
-    vals = torch.zeros((ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
-    Cf = torch.zeros((ctx.S, ctx.n), dtype=torch.float64, device="cuda")
-    for _ in range(3):
-        ctx.jacobian(f, vals, Cf)
+    nprob = len(wl.components)
+    f1 = [inputs.nodal_f(wl, r, z, b) for b in range(min(nb, nprob))]
+    f = np.stack([f1[b % len(f1)] for b in range(nb)])
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.zeros((nb, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    Cf = torch.zeros((nb, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    return ctx, fd, vals, Cf
+
+
+def timed_steps(torch, fn, steps, flush=None, warmup=3):
+    for _ in range(warmup):
+        fn()
     torch.cuda.synchronize()
-    ctx.profile_enable(True)
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    e0.record()
+    evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
+    for a, b in evs:
+        if flush is not None:
+            flush.add_(1.0)                  # L2 flush between timed iterations (outside the events)
+        a.record(); fn(); b.record()
+    torch.cuda.synchronize()
+    return [a.elapsed_time(b) for a, b in evs]
+
+
+def a3_profile(ctx, torch, fn, reps):
+    """Device time per launch of the step-a3 kernels: (tensor evaluation ms, contraction ms) via landau_profile_*."""
+    ctx.profile_enable(True); ctx.profile_read()
     for _ in range(reps):
-        ctx.jacobian(f, vals, Cf)
-    e1.record()
+        fn()
     torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / reps
-    pair_ms, cnt = ctx.profile_read()
+    ms, cnt = ctx.profile_read()
     ctx.profile_enable(False)
-    # the same build captured once in a CUDA graph and replayed (the library makes no synchronising call)
+    return [m / c if c else None for m, c in zip(ms, cnt)]
+
+
+def fp64_roof(kind, kernel, flop_per_pair, pairs, ms, peak, probe, extra=None):
+    ach = flop_per_pair * pairs / (ms * 1e-3) * 1e-12 if (flop_per_pair and ms) else None
+    d = {"bound": kind, "kernel": kernel, "achieved": ach, "peak": peak, "unit": "TFLOP/s", "frac": ach / peak if ach else None,
+         "frac_of_probe": ach / probe if (ach and probe) else None, "flop_per_pair": flop_per_pair,
+         "kernel_ms_per_launch": ms, "kernel_gpair_per_s": pairs / (ms * 1e-3) * 1e-9 if ms else None}
+    if extra:
+        d.update(extra)
+    return d
+
+
+def pair_sym_roof(rin, key, kname, pairs, ms, peak, probe, issue):
+    """Roofline entry of the per-problem pair kernel from the ncu-counted instruction mix of workload `key`."""
+    c = rin.get((kname, key)) or rin.get(("k_pair_sym", key))
+    if not c or not ms:
+        return fp64_roof("alu", kname, None, pairs, ms, peak, probe, {"note": "no ncu counters for this source revision"})
+    upl = c["units_per_launch"]
+    dfma, dmul, dadd = c["dfma"] / upl, c["dmul"] / upl, c["dadd"] / upl     # thread instructions per ordered pair
+    flop = 2 * dfma + dmul + dadd
+    inst = dfma + dmul + dadd
+    extra = {"fp64_inst_per_pair": inst, "dfma_share_of_fp64_inst": dfma / inst,
+             "fp64_pipe_frac": inst * pairs / (ms * 1e-3) / (peak * 0.5e12),
+             "traffic": (c.get("dram_read") or 0) + (c.get("dram_write") or 0) if c.get("dram_read") is not None else None,
+             "ncu_fp64_pipe_pct": c.get("fp64_pipe_pct"), "ncu_issue_active_pct": c.get("issue_active_pct")}
+    if c.get("dfma_3reg") is not None and issue:
+        # issue cycles per pair on the FP64 port: measured cycles per instruction class (landau_fp64_issue_probe)
+        three = c["dfma_3reg"] / upl
+        cyc = (inst - three) * issue["two_operand"] + three * issue["three_operand_reuse_mix"]
+        extra["fp64_issue_bound_frac"] = cyc * pairs / 32.0 / (ms * 1e-3) / (issue["smsp"] * issue["clock_hz"])
+    return fp64_roof("alu", kname, flop, pairs, ms, peak, probe, extra)
+
+
+def pair_kernel_name(N):
+    return "k_pair_sym<128,2>" if N >= 4096 else ("k_pair_sym<64,2>" if N >= 2560 else "k_pair_sym<32,1>")
+
+
+def time_config(binding, inputs, torch, oracle, key, k, variant, nb_batched, rin, peaks, flush, with_cpu=True):
+    """One BASELINE config (or context run): single build (per-problem path, as landau_create chooses for
+    max_batch = 1), a batch through both paths, the CPU oracle."""
+    wl = inputs.config(k, variant=variant)
+    out = {"config": wl.name}
+    # --- single build -------------------------------------------------------------------------------------------
+    ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, 1)
+    N, pairs = ctx.N, ctx.N * (ctx.N - 1)
+    out.update({"N": N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz})
+    ms = float(np.median(timed_steps(torch, lambda: ctx.jacobian(fd[0], vals[0], Cf[0]), 20)))
+    pk = a3_profile(ctx, torch, lambda: ctx.jacobian(fd[0], vals[0], Cf[0]), 10)[0]
     graph_ms = None
-    try:
+    try:        # the same build captured once in a CUDA graph and replayed (the library makes no synchronising call)
         side = torch.cuda.Stream()
         with torch.cuda.stream(side):
-            ctx.jacobian(f, vals, Cf)
+            ctx.jacobian(fd[0], vals[0], Cf[0])
             torch.cuda.synchronize()
             g = torch.cuda.CUDAGraph()
             with torch.cuda.graph(g, stream=side):
-                ctx.jacobian(f, vals, Cf)
+                ctx.jacobian(fd[0], vals[0], Cf[0])
             g.replay()
-            e0.record()
-            for _ in range(reps):
-                g.replay()
-            e1.record()
-            torch.cuda.synchronize()
-            graph_ms = e0.elapsed_time(e1) / reps
+            graph_ms = float(np.median(timed_steps(torch, g.replay, 20)))
     except Exception as exc:   # reported, not fatal
         graph_ms = f"unavailable: {exc}"
-    pairs = ctx.N * (ctx.N - 1)
-    out = {"config": wl.name, "graph_replay_ms_per_build": graph_ms, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz, "ms_per_build": ms,
-           "builds_per_s": 1e3 / ms, "gpair_per_s": pairs / (ms * 1e-3) * 1e-9,
-           "pair_kernel_ms": pair_ms / max(cnt, 1), "pair_kernel_gpair_per_s": pairs / (pair_ms / max(cnt, 1) * 1e-3) * 1e-9}
+    kname = pair_kernel_name(N)
+    out["single"] = {"path": "per-problem", "ms_per_build": ms, "graph_replay_ms_per_build": graph_ms, "builds_per_s": 1e3 / ms,
+                     "gpair_per_s": pairs / (ms * 1e-3) * 1e-9,
+                     "roofline": pair_sym_roof(rin, key + ":single", kname, pairs, pk, peaks["fp64"], peaks["probe"], peaks["issue"])}
     ctx.destroy()
+    # --- batch, both paths --------------------------------------------------------------------------------------
+    nb = nb_batched
+    out["batched"] = {"problems": nb}
+    for path, pname in ((binding.LANDAU_PAIR_SHARED, "shared"), (binding.LANDAU_PAIR_PER_PROBLEM, "per_problem")):
+        ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, nb, path)
+        fn = lambda: ctx.jacobian_batched(fd, vals, Cf)
+        ms = float(np.median(timed_steps(torch, fn, 5, flush)))
+        pk = a3_profile(ctx, torch, fn, 3)
+        e = {"ms_per_step": ms, "builds_per_s": nb / (ms * 1e-3), "gpair_per_s": nb * pairs / (ms * 1e-3) * 1e-9}
+        if path == binding.LANDAU_PAIR_SHARED:
+            e["tensor_eval_ms"] = pk[0]
+            e["roofline"] = fp64_roof("tensor", "k_apply_dmma", APPLY_FLOP_PER_PAIR, nb * pairs, pk[1], peaks["fp64"], peaks["dmma_probe"])
+        else:
+            e["roofline"] = pair_sym_roof(rin, key + ":batched", kname, nb * pairs, pk[0], peaks["fp64"], peaks["probe"], peaks["issue"])
+        out["batched"][pname] = e
+        ctx.destroy()
+        del fd, vals, Cf
+    # --- CPU oracle ---------------------------------------------------------------------------------------------
+    if with_cpu:
+        out["cpu_baseline"] = cpu_baseline(oracle, inputs, wl, [0], reps=3)
+        out["cpu_baseline"]["sample"] = "one build (a1-a7 on a Space built once), median of 3"
     return out
 
 
@@ -192,25 +325,19 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
     (the paper's three 20-cell grids with ten species, Table I, 512 problems batched)."""
     out = {}
     Ez = torch.full((nb,), 0.3, dtype=torch.float64, device="cuda")
-    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    ctx5.implicit_operator_batched(f5, Ez, 2.0, vals5, Cf5)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(3):
-        ctx5.implicit_operator_batched(f5, Ez, 2.0, vals5, Cf5)
-    e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 3
+    ms = float(np.median(timed_steps(torch, lambda: ctx5.implicit_operator_batched(f5, Ez, 2.0, vals5, Cf5), 3, warmup=1)))
     out["implicit_operator_config5"] = {"ms_per_step": ms, "gpair_per_s": nb * ctx5.N * (ctx5.N - 1) / (ms * 1e-3) * 1e-9,
                                         "what": "shift M + A(E_z) - J and A f - C(f) in one pass (landau_implicit_operator_batched)"}
     # NEXT-4: band LU of the nb * S matrices of the implicit step (vals5 holds them now), then one solve
     bw, md, ws = ctx5.band_sizes()
     band = torch.empty(nb * ws, dtype=torch.float64, device="cuda")
     rhs = torch.ones((nb, ctx5.S, ctx5.n), dtype=torch.float64, device="cuda")
+    piv = torch.zeros((nb, ctx5.S, 2), dtype=torch.float64, device="cuda")
     x = torch.empty_like(rhs)
-    ctx5.band_factor_batched(vals5, band); ctx5.band_solve_batched(band, rhs, x)
+    ctx5.band_factor_batched(vals5, band, piv); ctx5.band_solve_batched(band, rhs, x)
     torch.cuda.synchronize()
-    e2 = torch.cuda.Event(enable_timing=True)
-    e0.record(); ctx5.band_factor_batched(vals5, band); e1.record(); ctx5.band_solve_batched(band, rhs, x); e2.record()
+    e0, e1, e2 = (torch.cuda.Event(enable_timing=True) for _ in range(3))
+    e0.record(); ctx5.band_factor_batched(vals5, band, piv); e1.record(); ctx5.band_solve_batched(band, rhs, x); e2.record()
     torch.cuda.synchronize()
     fms, sms_ = e0.elapsed_time(e1), e1.elapsed_time(e2)
     nmat = nb * ctx5.S
@@ -220,7 +347,8 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
                               "factor_ms": fms, "solve_ms": sms_, "factor_tflops": flop / (fms * 1e-3) * 1e-12,
                               "factor_tflops_uniform_band_equiv": flop_band / (fms * 1e-3) * 1e-12,
                               "factorizations_per_s": nmat / (fms * 1e-3),
-                              "what": "scatter + blocked outer-product band LU without pivoting, then L/U solves (one rhs)"}
+                              "min_pivot_ratio": float((piv[:, :, 0] / piv[:, :, 1]).min()),
+                              "what": "scatter + blocked outer-product band LU without pivoting (pivot report on), then L/U solves (one rhs)"}
     del band, rhs, x
     name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("paper3")
     mg = binding.LandauMultigridContext(meshes, sgrid, order, spc, nb)
@@ -231,13 +359,7 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
     f = torch.from_numpy(np.tile(np.concatenate(fl), (nb, 1))).cuda()
     v = torch.zeros((nb, mg.vals_stride), dtype=torch.float64, device="cuda")
     c_ = torch.zeros((nb, mg.f_stride), dtype=torch.float64, device="cuda")
-    mg.jacobian_batched(f, v, c_)
-    torch.cuda.synchronize()
-    e0.record()
-    for _ in range(5):
-        mg.jacobian_batched(f, v, c_)
-    e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 5
+    ms = float(np.median(timed_steps(torch, lambda: mg.jacobian_batched(f, v, c_), 5, warmup=1)))
     out["multigrid_paper3"] = {"workload": f"{nb} problems x (10 species on 3 grids of 20 Q3 cells: N = {mg.N}, n = {mg.f_stride})",
                                "ms_per_step": ms, "builds_per_s": nb / (ms * 1e-3),
                                "gpair_per_s": nb * mg.N * (mg.N - 1) / (ms * 1e-3) * 1e-9}
@@ -260,17 +382,28 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
         c80.implicit_operator_batched(f80, Ez80, 2.0, v80, F80)
         c80.band_factor_batched(v80, band80)
         c80.band_solve_batched(band80, F80, d80)
-    newton(); torch.cuda.synchronize()
-    e0.record()
-    for _ in range(5):
-        newton()
-    e1.record(); torch.cuda.synchronize()
-    ms = e0.elapsed_time(e1) / 5
+    ms = float(np.median(timed_steps(torch, newton, 5, warmup=1)))
     out["newton_iteration_ctx80"] = {"workload": f"{nb} problems x (10 species, 80 Q3 cells: N = {c80.N}, n = {c80.n}, RCM half-bandwidth {bw80})",
                                      "ms_per_batched_iteration": ms, "newton_iterations_per_s": nb / (ms * 1e-3),
                                      "what": "operator (shift M + A - J, A f - C(f)) + band LU of 10 species blocks + solve, per problem"}
     c80.destroy()
     return out
+
+
+def measure_peaks(binding, sms, sm_max_mhz):
+    """FP64 denominators: derived (SMs x 64 lanes x 2 x max clock; the same for DFMA and DMMA.8x8x4, one per 16 clocks
+    and sub-partition) and measured on this GPU by the in-library probes."""
+    nominal = sms * FP64_LANES_PER_SM * 2 * sm_max_mhz * 1e6 * 1e-12
+    probe, _ = binding.landau_fp64_peak_probe(1 << 16)
+    cyc = {m: binding.landau_fp64_issue_probe(m)[0] for m in range(5)}
+    dmma_cyc, dmma_flops = binding.landau_fp64_issue_probe(5)
+    issue = {"two_operand": cyc[1], "immediate_operand": cyc[0], "three_operand": cyc[2], "three_operand_shared": cyc[3],
+             "three_operand_reuse_mix": 0.5 * (cyc[2] + cyc[3]), "dependent_latency": cyc[4], "dmma_8x8x4": dmma_cyc,
+             "smsp": sms * 4, "clock_hz": sm_max_mhz * 1e6,
+             "what": "SM cycles per FP64 warp instruction and sub-partition, landau_fp64_issue_probe modes 0-5"}
+    return {"fp64": nominal, "probe": probe * 1e-12, "dmma_probe": dmma_flops * 1e-12, "issue": issue,
+            "source": "derived: SMs x 64 FP64 lanes x 2 x clocks.max.sm (DESIGN.md 8); MEASURED_PEAKS.json has no fp64 entry; "
+                      "probe = landau_fp64_peak_probe (DFMA), dmma_probe = landau_fp64_issue_probe(5), both measured in this run"}
 
 
 def run_ours(args):
@@ -293,6 +426,7 @@ def run_ours(args):
     wl = inputs.config(5)
     nb = wl.nbatch
     ctx = binding.LandauContext(wl.mesh, wl.order, wl.species, nb)
+    path, scratch_bytes = ctx.pair_path()
     r, z = ctx.dof_coords()
     # every rank builds its own 512 problems (weak scaling); problem seeds are offset by rank
     f_host = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in range(nb)])).pin_memory()
@@ -322,18 +456,16 @@ def run_ours(args):
     evs = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     barrier()
     t_begin = time.perf_counter()
-    t_wall = t_begin
     for k in range(args.steps):
         flush.add_(1.0)                      # L2 flush between timed iterations (outside the events)
         evs[k][0].record()
         ctx.jacobian_batched(f, vals, Cf)
         evs[k][1].record()
     barrier()
-    t_wall = time.perf_counter() - t_wall
+    t_wall = time.perf_counter() - t_begin
     launches = ctx.launch_count() - l0
     step_ms = [a.elapsed_time(b) for a, b in evs]
-    total_ms = float(sum(step_ms))
-    pair_ms, pair_cnt = ctx.profile_read()
+    a3_ms, a3_cnt = ctx.profile_read()
     ctx.profile_enable(False)
     clocks = sampler.stop(t_begin, t_begin + t_wall)
 
@@ -343,77 +475,110 @@ def run_ours(args):
     ctx.jacobian_host(f_host, vals_host, Cf_host)        # warm-up (allocates staging)
     barrier()
     e2e_steps = max(1, min(args.steps, 5))
-    t0 = time.perf_counter()
+    e2e_times = []
     for _ in range(e2e_steps):
+        t0 = time.perf_counter()
         ctx.jacobian_host(f_host, vals_host, Cf_host)    # synchronises
+        e2e_times.append((time.perf_counter() - t0) * 1e3)
     barrier()
-    e2e_ms = (time.perf_counter() - t0) * 1e3
     assert torch.equal(vals_host[-1], vals[-1].cpu())
 
-    t = torch.tensor([total_ms, e2e_ms], dtype=torch.float64, device="cuda")
+    t = torch.tensor([float(np.median(step_ms)), float(np.mean(step_ms)), float(np.median(e2e_times))], dtype=torch.float64, device="cuda")
     if dist is not None:
         dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    total_ms, e2e_ms = float(t[0]), float(t[1])
-    ms_per_step = total_ms / args.steps
+    ms_per_step, ms_mean, e2e_ms = float(t[0]), float(t[1]), float(t[2])
     value = world * pairs_per_step / (ms_per_step * 1e-3) * 1e-9
-    e2e_value = world * pairs_per_step / (e2e_ms / e2e_steps * 1e-3) * 1e-9
+    e2e_value = world * pairs_per_step / (e2e_ms * 1e-3) * 1e-9
 
     if rank == 0:
-        peak_flops, _ = binding.landau_fp64_peak_probe(1 << 16)
+        from oracle import landau_oracle as oracle
+        oracle.build()
+        rin = load_roofline_inputs()
         sm_max = clocks["sm_max_mhz"] or 1965.0
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
-        nominal_peak = sms * FP64_LANES_PER_SM * 2 * sm_max * 1e6 * 1e-12
-        pair_launch_ms = pair_ms / max(pair_cnt, 1)
-        achieved = FLOP_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) * 1e-12
-        roof = {"bound": "alu", "kernel": "k_pair_sym<128,2>", "achieved": achieved, "peak": nominal_peak, "unit": "TFLOP/s",
-                "frac": achieved / nominal_peak, "traffic": PAIR_KERNEL_DRAM_BYTES,
-                "peak_source": "derived: SMs x 64 DFMA lanes x 2 x clocks.max.sm (DESIGN.md); MEASURED_PEAKS.json has no fp64 entry",
-                "peak_probe_measured": peak_flops * 1e-12, "frac_of_probe": achieved / (peak_flops * 1e-12),
-                "flop_per_pair": FLOP_PER_PAIR,
-                "fp64_pipe_frac": FP64_INST_PER_PAIR * pairs_per_step / (pair_launch_ms * 1e-3) / (nominal_peak * 0.5e12),
-                "fp64_issue_bound_frac": (FP64_INST_PER_PAIR + 0.5 * FP64_3OP_INST_PER_PAIR) * pairs_per_step
-                / (pair_launch_ms * 1e-3) / (nominal_peak * 0.5e12),
-                "kernel_ms_per_launch": pair_launch_ms,
-                "kernel_share_of_step": pair_ms / total_ms if world == 1 else None,
-                "kernel_gpair_per_s": pairs_per_step / (pair_launch_ms * 1e-3) * 1e-9}
-        cpu_val, cpu_dt, cores = cpu_baseline_sample(wl, inputs)
-        detail = [time_single_config(binding, inputs, torch, k) for k in (1, 2, 3, 4)]
-        detail.append(time_single_config(binding, inputs, torch, 3, variant="A"))
-        detail += [time_single_config(binding, inputs, torch, k) for k in (6, 7)]   # paper-shaped S = 10 context runs
+        peaks = measure_peaks(binding, sms, sm_max)
+        tensor_ms = a3_ms[0] / a3_cnt[0] if a3_cnt[0] else None
+        apply_ms = a3_ms[1] / a3_cnt[1] if a3_cnt[1] else None
+        shared = path == binding.LANDAU_PAIR_SHARED
+        if shared:
+            c = rin.get(("k_apply_dmma", "cfg5:main")) or {}
+            roof = fp64_roof("tensor", "k_apply_dmma<4,2>", APPLY_FLOP_PER_PAIR, pairs_per_step, apply_ms, peaks["fp64"], peaks["dmma_probe"], {
+                "traffic": (c.get("dram_read", 0) + c.get("dram_write", 0)) if c else None,
+                "ncu_fp64_pipe_pct": c.get("fp64_pipe_pct") if c else None,
+                "peak_source": peaks["source"], "peak_probe_measured": peaks["dmma_probe"],
+                "kernel_share_of_step": apply_ms / ms_per_step if world == 1 else None,
+                "what": "fp64 mma.sync.m8n8k4 (DMMA.8x8x4) contraction G = U T: 7 products = 14 flop per ordered pair and problem"})
+            c = rin.get(("k_pair_tensor", "cfg5:main"))
+            tens = None
+            if c and tensor_ms:
+                upl = c["units_per_launch"]
+                fl = (2 * c["dfma"] + c["dmul"] + c["dadd"]) / upl
+                tens = fp64_roof("alu", "k_pair_tensor", fl, ctx.N * (ctx.N - 1), tensor_ms, peaks["fp64"], peaks["probe"],
+                                 {"traffic": c["dram_read"] + c["dram_write"], "what": "one tensor evaluation per ORDERED pair and call (K, E by the scaled AGM), all problems share it"})
+        else:
+            roof = pair_sym_roof(rin, "cfg5:main", "k_pair_sym<128,2>", pairs_per_step, tensor_ms, peaks["fp64"], peaks["probe"], peaks["issue"])
+            tens = None
+        # the per-problem path on the same workload (round 1's headline kernel), and the tensor cache
+        ctx.set_pair_path(binding.LANDAU_PAIR_PER_PROBLEM)
+        pp_ms = float(np.median(timed_steps(torch, lambda: ctx.jacobian_batched(f, vals, Cf), 5, flush)))
+        pp_k = a3_profile(ctx, torch, lambda: ctx.jacobian_batched(f, vals, Cf), 3)[0]
+        per_problem = {"ms_per_step": pp_ms, "gpair_per_s": pairs_per_step / (pp_ms * 1e-3) * 1e-9, "builds_per_s": nb / (pp_ms * 1e-3),
+                       "roofline": pair_sym_roof(rin, "cfg5:per_problem", "k_pair_sym<128,2>", pairs_per_step, pp_k, peaks["fp64"], peaks["probe"], peaks["issue"]),
+                       "what": "LANDAU_PAIR_PER_PROBLEM: every problem evaluates every pair's tensor itself (symmetric tile pairs)"}
+        ctx.set_pair_path(binding.LANDAU_PAIR_AUTO)
+        ctx.set_tensor_cache(True)
+        tc_ms = float(np.median(timed_steps(torch, lambda: ctx.jacobian_batched(f, vals, Cf), 5, flush)))
+        ctx.set_tensor_cache(False)
+        cached = {"ms_per_step": tc_ms, "gpair_per_s": pairs_per_step / (tc_ms * 1e-3) * 1e-9, "builds_per_s": nb / (tc_ms * 1e-3),
+                  "what": "landau_set_tensor_cache(1): the pair tensor kept between calls (off by default and in `value`)"}
+        # CPU baseline on a bounded sample of the headline workload
+        cpu = cpu_baseline(oracle, inputs, wl, list(range(CPU_SAMPLE_PROBLEMS)))
+        cpu["sample"] = (f"{CPU_SAMPLE_PROBLEMS} of the 512 problems (N=4928, a1-a7 on a Space built once), double-precision oracle, "
+                         f"OpenMP over i in the pair loop, {cpu['seconds']:.2f} s wall")
+        detail = [time_config(binding, inputs, torch, oracle, key, k, var, nbb, rin, peaks, flush) for key, k, var, nbb in CONFIGS]
         next_rows = time_next_rows(binding, inputs, torch, ctx, f, vals, Cf, nb)
-        # everything but the pair kernel (a1, a2, a4-a7): HBM-bound; algorithmic bytes = f in, vals and C(f) out,
+        # everything but step a3's kernels (a1, a2, a4-a7): HBM-bound; algorithmic bytes = f in, vals and C(f) out,
         # G_D/G_K (5 doubles per point) between the two halves of the path
-        rest_ms = (total_ms - pair_ms) / args.steps if world == 1 else None
+        a3_total = (tensor_ms or 0.0) + (apply_ms or 0.0)
+        rest_ms = ms_per_step - a3_total if world == 1 else None
         rest_bytes = nb * (ctx.S * 8 * (2 * ctx.n + ctx.nnz) + 40 * ctx.N)
-        hbm_peak = None
         try:
             hbm_peak = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))["hbm_gbs"]
             hbm_src = "MEASURED_PEAKS.json hbm_gbs"
         except Exception:
-            hbm_peak, hbm_src = 6460.0, "fallback (B200_PROFILING.md measured copy bandwidth)"
+            hbm_peak, hbm_src = 6650.0, "fallback (B200_PROFILING.md)"
         roof_rest = None
         if rest_ms:
             ach = rest_bytes / (rest_ms * 1e-3) * 1e-9
+            c = rin.get(("rest", "cfg5:main")) or {}
             roof_rest = {"bound": "hbm", "kernels": "k_fields_beta + k_sum_partials + k_element_q3 + k_gather x2", "achieved": ach,
                          "peak": hbm_peak, "unit": "GB/s", "frac": ach / hbm_peak, "peak_source": hbm_src,
-                         "ms_per_step": rest_ms, "algorithmic_bytes_per_step": rest_bytes, "traffic": REST_DRAM_BYTES}
+                         "ms_per_step": rest_ms, "algorithmic_bytes_per_step": rest_bytes,
+                         "traffic": (c.get("dram_read", 0) + c.get("dram_write", 0)) if c else None}
         h2d = nb * ctx.S * ctx.n * 8
         d2h = nb * ctx.S * (ctx.nnz + ctx.n) * 8
         print(json.dumps({
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-            "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic",
+            "ms_per_step": ms_per_step, "ms_per_step_mean": ms_mean, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic",
             "config": {"workload": WORKLOAD, "problems_per_gpu": nb, "N": ctx.N, "S": ctx.S, "n": ctx.n, "nnz": ctx.nnz,
-                       "pairs_per_step_per_gpu": pairs_per_step, "l2": "256 MiB flush write between timed steps; outputs 0.7 GB > L2"},
+                       "pairs_per_step_per_gpu": pairs_per_step, "l2": "256 MiB flush write between timed steps; outputs 0.7 GB > L2",
+                       "pair_path": "LANDAU_PAIR_SHARED" if shared else "LANDAU_PAIR_PER_PROBLEM", "pair_scratch_bytes": scratch_bytes,
+                       "value_counts": "N(N-1) ordered pair interactions per problem; on the shared path the tensor of a pair is "
+                                       "evaluated once per call (inside the timed step) and applied to all 512 problems"},
             "builds_per_s": world * nb / (ms_per_step * 1e-3),
             "wall_ms_per_step_incl_flush": t_wall * 1e3 / args.steps,
             "clocks": clocks, "gpu_launches": launches,
             "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "ms_per_step": e2e_ms / e2e_steps, "steps": e2e_steps, "api": "landau_jacobian_host (pinned host buffers)"},
+                    "ms_per_step": e2e_ms, "steps": e2e_steps, "api": "landau_jacobian_host (pinned host buffers), median"},
             "roofline": roof,
-            "cpu_baseline": {"value": cpu_val, "unit": UNIT, "cores": cores, "kind": "oracle",
-                             "sample": f"{CPU_SAMPLE_PROBLEMS} of the 512 problems (N=4928, a1-a8), double-precision oracle, OpenMP over i, {cpu_dt:.2f} s wall"},
+            "roofline_tensor_eval": tens,
+            "cpu_baseline": cpu,
             "roofline_rest": roof_rest,
+            "fp64_peaks": {k: v for k, v in peaks.items() if k != "source"},
+            "per_problem_path": per_problem,
+            "tensor_cache_on": cached,
+            "roofline_inputs": {"file": os.path.relpath(ROOFLINE_INPUTS, ROOT), "source_sha": kernel_source_sha(), "rows_matching": len(rin)},
             "per_config": detail,
             "next_rows": next_rows,
         }))
@@ -422,14 +587,111 @@ def run_ours(args):
         dist.destroy_process_group()
 
 
+CPU_SAMPLE_PROBLEMS = 8      # of the 512: ~0.5 s each on 16 cores, i.e. tens of core-seconds in total
+
+
+# ------------------------------------------------------------------------------------------------------------------
+# ncu support: launch plans and the summariser of raw exports
+# ------------------------------------------------------------------------------------------------------------------
+def kernel_run(which):
+    """Launches for an ncu pass, nothing timed.  Prints one line per launch group: workload key, kernel regex,
+    units (ordered pairs) per launch -- the summariser needs them to turn counters into per-pair figures.
+      single : one single build (per-problem path) of every per_config entry, in CONFIGS order
+      batched: the batched run of every per_config entry through the per-problem path, then the shared path
+      main   : config 5, shared path (one step), then per-problem path (one step)"""
+    import torch
+    from paper_2104_10000_b200 import binding, inputs
+    binding.lib()
+    plan = []
+    if which == "main":
+        wl = inputs.config(5)
+        for path, tag in ((binding.LANDAU_PAIR_SHARED, "cfg5:main"), (binding.LANDAU_PAIR_PER_PROBLEM, "cfg5:per_problem")):
+            ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, wl.nbatch, path)
+            ctx.jacobian_batched(fd, vals, Cf)
+            torch.cuda.synchronize()
+            plan.append({"workload": tag, "N": ctx.N, "problems": wl.nbatch, "pairs_per_launch": wl.nbatch * ctx.N * (ctx.N - 1),
+                         "tensor_pairs_per_launch": ctx.N * (ctx.N - 1)})
+            ctx.destroy()
+            del fd, vals, Cf
+    else:
+        for key, k, var, nbb in CONFIGS:
+            wl = inputs.config(k, variant=var)
+            nb = 1 if which == "single" else nbb
+            paths = [binding.LANDAU_PAIR_PER_PROBLEM] + ([binding.LANDAU_PAIR_SHARED] if which == "batched" else [])
+            for path in paths:
+                ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, nb, path)
+                ctx.jacobian_batched(fd, vals, Cf)
+                torch.cuda.synchronize()
+                plan.append({"workload": f"{key}:{which}" + (":shared" if path == binding.LANDAU_PAIR_SHARED else ""), "N": ctx.N,
+                             "problems": nb, "pairs_per_launch": nb * ctx.N * (ctx.N - 1), "tensor_pairs_per_launch": ctx.N * (ctx.N - 1)})
+                ctx.destroy()
+                del fd, vals, Cf
+    print(json.dumps({"kernel_run": which, "source_sha": kernel_source_sha(), "plan": plan}))
+
+
+NCU_COLS = {
+    "dfma": "smsp__sass_thread_inst_executed_op_dfma_pred_on.sum", "dmul": "smsp__sass_thread_inst_executed_op_dmul_pred_on.sum",
+    "dadd": "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum", "dram_read": "dram__bytes_read.sum", "dram_write": "dram__bytes_write.sum",
+    "time_ns": "gpu__time_duration.sum", "fp64_pipe_pct": "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active",
+    "issue_active_pct": "smsp__issue_active.avg.pct_of_peak_sustained_active", "inst_executed": "smsp__inst_executed.sum",
+}
+
+
+def summarise_ncu(paths, plan_file):
+    """ncu `--page raw --csv` exports + the JSON line `--kernel-run` printed for the same command -> CSV rows
+    (kernel, workload, source_sha, units_per_launch, counters per launch).  The n-th launch of a pair kernel
+    (k_pair_sym / k_pair_tensor / k_apply_dmma) in the export belongs to the n-th entry of the plan that runs it."""
+    plan = json.loads(open(plan_file).read().strip().splitlines()[-1])
+    sha = plan["source_sha"]
+    w = csv.writer(sys.stdout)
+    cols = list(NCU_COLS)
+    w.writerow(["kernel", "workload", "source_sha", "units_per_launch"] + cols)
+    for p in paths:
+        rows = list(csv.DictReader(l for l in open(p) if l.startswith('"')))
+        rows = [r for r in rows if r.get("ID", "").strip().isdigit()]          # drop the units row
+        def val(r, col):
+            v = r.get(col, "")
+            try:
+                return float(v.replace(",", ""))
+            except Exception:
+                return None
+        seq = {"k_pair_sym": [], "k_pair_tensor": [], "k_apply_dmma": []}
+        rest = {}
+        for r in rows:
+            name = r["Kernel Name"]
+            hit = next((k for k in seq if k in name), None)
+            if hit:
+                seq[hit].append(r)
+            elif "landau::" in name or name.startswith("k_"):
+                rest.setdefault("rest", []).append(r)
+        for kern, lst in seq.items():
+            entries = [e for e in plan["plan"] if (kern == "k_pair_sym") == (not e["workload"].endswith(":shared") and e["workload"] != "cfg5:main")]
+            for r, e in zip(lst, entries):
+                units = e["tensor_pairs_per_launch"] if kern == "k_pair_tensor" else e["pairs_per_launch"]
+                short = r["Kernel Name"].split("(")[0].replace("landau::", "").replace("void ", "")
+                w.writerow([short if kern == "k_pair_sym" else kern, e["workload"], sha, units] + [val(r, NCU_COLS[c]) for c in cols])
+        if rest.get("rest") and plan["kernel_run"] == "main":
+            # the other kernels of the FIRST step (shared path): summed
+            n_first = len(rest["rest"]) // 2
+            tot = {c: sum((val(r, NCU_COLS[c]) or 0.0) for r in rest["rest"][:n_first]) for c in cols}
+            w.writerow(["rest", "cfg5:main", sha, plan["plan"][0]["pairs_per_launch"]] + [tot[c] for c in cols])
+
+
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--kernel-run", default=None, choices=["single", "batched", "main"])
+    ap.add_argument("--summarise-ncu", nargs="+", default=None, metavar="RAW.csv")
+    ap.add_argument("--plan", default=None, help="file holding the JSON line --kernel-run printed (for --summarise-ncu)")
     args = ap.parse_args()
-    if args.impl == "reference":
+    if args.summarise_ncu:
+        summarise_ncu(args.summarise_ncu, args.plan)
+    elif args.kernel_run:
+        kernel_run(args.kernel_run)
+    elif args.impl == "reference":
         run_reference(args)
     else:
         args.warmup = max(args.warmup, 3)

@@ -1,7 +1,13 @@
 """GPU parity: the CUDA path (through the C ABI) against the CPU oracle, element by element, on
 the same seeded inputs.  Tolerance (BASELINE.json north_star; reading R): per species
 block max|x_gpu - x_ref| / max|x_ref| <= 1e-10 for Jacobian values and C(f); conservation
-residuals of the GPU's C(f) < 1e-12 relative; integer work (pattern) bit-exact."""
+residuals of the GPU's C(f) < 1e-12 relative; integer work (pattern) bit-exact.
+
+Step a3 has two paths (include/landau.h): PER (every problem evaluates the pair tensor itself, k_pair_sym) and
+SHARED (tensor once per call, fp64 tensor-core contraction, k_pair_tensor + k_apply_dmma).  The parity cases run
+on both; the sizes are chosen so that every instantiation the launchers can select is compared with the oracle:
+k_pair_sym<32,1>, <64,2>, <128,2>, each with and without the all-pairs coincidence test, k_apply_dmma<1,2>,
+<2,2>, <4,2>, k_band_factor / k_band_solve with 8-, 16- and 32-column blocks."""
 import numpy as np
 import pytest
 
@@ -9,6 +15,8 @@ from paper_2104_10000_b200 import inputs
 
 pytestmark = pytest.mark.gpu
 TOL = 1e-10
+PER, SHARED = 1, 2          # LANDAU_PAIR_PER_PROBLEM, LANDAU_PAIR_SHARED
+PATHS = [pytest.param(PER, id="per-problem"), pytest.param(SHARED, id="shared")]
 
 
 @pytest.fixture(scope="module")
@@ -40,9 +48,11 @@ def conservation_residuals(dof_r, dof_z, mass, Cf):
     return max(out)
 
 
-def run_gpu(gpu, wl, problems, max_batch=None, batched=True):
+def run_gpu(gpu, wl, problems, max_batch=None, batched=True, path=0):
     import torch
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, max_batch or len(problems))
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, max_batch or len(problems), pair_path=path)
+    if path:
+        assert ctx.pair_path()[0] == path
     r, z = ctx.dof_coords()
     f = np.stack([inputs.nodal_f(wl, r, z, b) for b in problems])
     fd = torch.from_numpy(f).cuda()
@@ -78,27 +88,44 @@ def check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, problems):
     return worst
 
 
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("cfg", [0, 1, 2])
-def test_small_configs_full_parity(gpu, oracle, cfg):
+def test_small_configs_full_parity(gpu, oracle, cfg, path):
     wl = inputs.config(cfg)
-    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0], path=path)
     worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
     print(f"{wl.name}: worst block error {worst:.2e}")
 
 
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("cfg,variant", [(3, "A"), (3, "B"), (4, "B")])
-def test_refined_configs_full_parity(gpu, oracle, cfg, variant):
+def test_refined_configs_full_parity(gpu, oracle, cfg, variant, path):
     wl = inputs.config(cfg, variant=variant)
-    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0], path=path)
     worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
     print(f"{wl.name}: worst block error {worst:.2e}")
 
 
+@pytest.mark.parametrize("path", PATHS)
+def test_table1_single_grid_mesh_parity_uses_the_64_point_tiles(gpu, oracle, path):
+    """A uniform 10 x 20 Q3 mesh -- the single-grid case of the paper's Table I (3,200 integration points, L195-199;
+    tests/golden/table1_counts.txt) -- has 2,560 <= N < 4,096, the range in which the per-problem pair kernel runs
+    as k_pair_sym<64,2>: the whole path against the oracle, element by element."""
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 10, 20)
+    spc = inputs._sp([(1, -1, 1, 1), (3670, 1, 1, 1)])
+    wl = inputs.Workload("table1-10x20-q3", 3, mesh, spc, [[inputs.Component(0, 1, 1), inputs.Component(1, 1, 1)]], 1e-3, 21)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0], path=path)
+    assert ctx.N == 3200
+    worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
+    print(f"{wl.name}: worst block error {worst:.2e}")
+
+
+@pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("cfg", [6, 7])
-def test_paper_shaped_ten_species_context_parity(gpu, oracle, cfg):
+def test_paper_shaped_ten_species_context_parity(gpu, oracle, cfg, path):
     """e + D + 8 heavy-ion charge states on the 80- and 320-cell Q3 meshes."""
     wl = inputs.config(cfg)
-    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0], path=path)
     worst = check_against_oracle(oracle, wl, ctx, f, vals, Cf, mv, [0])
     print(f"{wl.name}: worst block error {worst:.2e}")
 
@@ -132,14 +159,32 @@ def test_implicit_operator_parity(gpu, oracle, cfg, variant):
     assert torch.equal(v0, -vj) and torch.equal(F0, -cj)
 
 
-@pytest.mark.parametrize("which", ["same2", "scaled", "paper3"])
-def test_multigrid_parity(gpu, oracle, which):
+def _multigrid_case(which):
+    """inputs.multigrid_case, plus two cases with IDENTICAL Q3 grids (every point coincides with one of the other
+    grid, so every pair is tested for coincidence) whose point totals select the 64- and 128-point tiles of the
+    per-problem pair kernel: 'same2-q3-80' = 2 x 1,280 = 2,560 points, 'same2-q3-128' = 2 x 2,048 = 4,096 points."""
+    if which in ("same2-q3-80", "same2-q3-128"):
+        m = inputs.config(6).mesh if which == "same2-q3-80" else inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 8, 16)
+        spc = inputs._sp([(1, -1, 1, 1), (4, 1, 1, 1)])
+        return which, 3, [m, m], spc, [0, 1], [inputs.Component(0, 1, 1), inputs.Component(1, 1, 1)]
+    return inputs.multigrid_case(which)
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("which", ["same2", "scaled", "paper3", "same2-q3-80", "same2-q3-128"])
+def test_multigrid_parity(gpu, oracle, which, path):
     """SURVEY 8(f) NEXT-2 (section III-C): species on several grids, pair loop over the union of
-    points.  'same2' has every point of grid 1 on top of one of grid 0 (coincident pairs skipped across
+    points.  'same2*' have every point of grid 1 on top of one of grid 0 (coincident pairs skipped across
     grids); 'paper3' is Table I's three 20-cell grids with ten species (960 points, 1,930 equations)."""
     import torch
-    name, order, meshes, spc, sgrid, comps = inputs.multigrid_case(which)
+    name, order, meshes, spc, sgrid, comps = _multigrid_case(which)
     ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, 2)
+    ctx.set_pair_path(path)
+    assert ctx.pair_path()[0] == path
+    if which == "same2-q3-80":
+        assert ctx.N == 2560
+    if which == "same2-q3-128":
+        assert ctx.N == 4096
     if which == "paper3":
         assert ctx.N == 960 and ctx.f_stride == 1930
     fl = []
@@ -332,11 +377,27 @@ def test_edge_cases_of_the_next_rows(gpu, oracle):
         assert ei.value.code == gpu.LANDAU_EINVAL
 
 
-def test_inner_integral_parity(gpu, oracle):
-    """Steps a1-a3 alone: G_D, G_K at every integration point (several tiles + ragged tail)."""
+def _inner_case(which):
+    if which == "q2-180":         # 5 tiles of 32 + a tail of 20
+        return inputs.config(0)
+    if which == "q3-2048":        # 64 whole tiles of 32
+        return inputs.config(2)
+    if which == "q3-2992":        # 46 tiles of 64 + a tail of 48
+        mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 11, 17)
+        spc = inputs._sp([(1, -1, 1, 1), (25, 1, 1, 1)])
+        return inputs.Workload("q3-11x17", 3, mesh, spc, [[inputs.Component(0, 1, 1), inputs.Component(1, 1, 1, 0.2)]], 1e-3, 31)
+    return inputs.config(3)       # 'q3-4928': 38 tiles of 128 + a tail of 64
+
+
+@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("which", ["q2-180", "q3-2048", "q3-2992", "q3-4928"])
+def test_inner_integral_parity(gpu, oracle, which, path):
+    """Steps a1-a3 alone: G_D, G_K at every integration point, one case per tile size of the per-problem pair
+    kernel (32 / 64 / 128 points), each with a ragged last tile, and the same cases through the shared path
+    (ragged last chunk of 16 source points, ragged target tile, 1 / 2 / 4 splits of the source range)."""
     import torch
-    wl = inputs.config(2)
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 1)
+    wl = _inner_case(which)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 1, pair_path=path)
     r, z = ctx.dof_coords()
     f = inputs.nodal_f(wl, r, z)
     G = torch.zeros((1, 5, ctx.N), dtype=torch.float64, device="cuda")
@@ -344,26 +405,33 @@ def test_inner_integral_parity(gpu, oracle):
     G = G.cpu().numpy()[0]
     sp = oracle.build_space(wl.mesh, wl.order)
     pr, pz, pw = ctx.points()
-    assert np.abs(pr - sp.r).max() < 1e-14 and np.abs(pz - sp.z).max() < 1e-14 and np.abs(pw - sp.w_in).max() < 1e-15
+    assert np.abs(pr - sp.r).max() < 1e-14 and np.abs(pz - sp.z).max() < 1e-14 and np.abs(pw - sp.w_in).max() <= 1e-15 * sp.w_in.max()
     _, _, (GD, GK) = oracle.coefficients(sp, wl.species, f)
     ref = np.concatenate([GD.T, GK.T])
     for c in range(5):
         assert block_err(G[c], ref[c]) <= 1e-12, c
 
 
-def test_config5_batched_full_size(gpu, oracle):
+@pytest.mark.parametrize("path", PATHS)
+def test_config5_batched_full_size(gpu, oracle, path):
     """BASELINE config 5 at full size (512 problems, the launch shape bench.py times): sampled
     problems against the oracle one by one; conservation (holds at any size) on all 512."""
     wl = inputs.config(5)
     problems = list(range(wl.nbatch))
-    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, problems)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, problems, path=path)
     assert np.isfinite(vals).all() and np.isfinite(Cf).all()
     sp = oracle.build_space(wl.mesh, wl.order)
     for k in problems:
         assert conservation_residuals(sp.dof_r, sp.dof_z, wl.species.mass, Cf[k]) < 1e-12, k
-    # extremes of bulk temperature + first/last
+    # first, last, and the extremes of bulk temperature, tail fraction and z-shift (SURVEY 8(d)), filled up to 8
     Tb = [wl.components[b][0].T for b in problems]
-    sample = sorted({0, wl.nbatch - 1, int(np.argmin(Tb)), int(np.argmax(Tb))})
+    tail = [wl.components[b][1].n for b in problems]
+    zs = [wl.components[b][1].zs for b in problems]
+    sample = {0, wl.nbatch - 1}
+    for q in (Tb, tail, zs):
+        sample |= {int(np.argmin(q)), int(np.argmax(q))}
+    sample = sorted(sample | set(range(101, 101 + 8 - len(sample))))
+    assert len(sample) >= 8
     for k in sample:
         _, ovals, oCf, _ = oracle.build_all(wl.mesh, wl.order, wl.species, f[k], 1.0)
         for a in range(2):
@@ -371,14 +439,26 @@ def test_config5_batched_full_size(gpu, oracle):
             assert block_err(Cf[k, a], oCf[a]) <= TOL, (k, a)
 
 
-def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu):
+@pytest.mark.parametrize("path", PATHS)
+def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu, path):
+    """Inside one path a problem's result does not depend on the batch it is built in: 24 problems in one call,
+    again, one by one, and (other tile shapes of the shared path's contraction) in calls of 17 + 7."""
+    import torch
     wl = inputs.config(5, nbatch=24, variant="A")
     problems = list(range(24))
-    _, _, v1, c1, _ = run_gpu(gpu, wl, problems, batched=True)
-    _, _, v2, c2, _ = run_gpu(gpu, wl, problems, batched=True)
-    _, _, v3, c3, _ = run_gpu(gpu, wl, problems, batched=False)
+    _, _, v1, c1, _ = run_gpu(gpu, wl, problems, batched=True, path=path)
+    _, _, v2, c2, _ = run_gpu(gpu, wl, problems, batched=True, path=path)
+    _, _, v3, c3, _ = run_gpu(gpu, wl, problems, batched=False, path=path)
     assert np.array_equal(v1, v2) and np.array_equal(c1, c2)      # run-to-run determinism
     assert np.array_equal(v1, v3) and np.array_equal(c1, c3)      # batch shape == split shape, bitwise
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 24, pair_path=path)
+    r, z = ctx.dof_coords()
+    fd = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in problems])).cuda()
+    v4 = torch.zeros((24, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    c4 = torch.zeros((24, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    ctx.jacobian_batched(fd[:17], v4[:17], c4[:17])
+    ctx.jacobian_batched(fd[17:], v4[17:], c4[17:])
+    assert np.array_equal(v4.cpu().numpy(), v1) and np.array_equal(c4.cpu().numpy(), c1)
 
 
 def test_no_state_carried_between_calls(gpu):
@@ -450,3 +530,181 @@ def test_edge_cases(gpu, oracle):
     check_against_oracle(oracle, wl16, ctx, f, vals, Cf, mv, [0])
     with pytest.raises(gpu.LandauError):
         gpu.LandauContext(m16, 2, inputs._sp(rows + [(2.0, 1, 1, 1)]))   # S = 17 > 16
+
+
+def test_band_lu_widest_band_uses_the_8_column_blocks(gpu):
+    """A 47 x 47 Q3 mesh (n = 20,164, RCM half-bandwidth 843 > 832): the panels only fit shared memory with
+    8-column blocks, so k_band_factor<8,512> / k_band_solve<8,512> run.  Reference: scipy's sparse direct solve of
+    the same CSR matrix; the pivot report must show a healthy elimination."""
+    import torch
+    import scipy.sparse as sps
+    import scipy.sparse.linalg as spla
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 47, 47)
+    spc = inputs._sp([(1, -1, 1, 1)])
+    wl = inputs.Workload("q3-47x47", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 12)
+    ctx = gpu.LandauContext(mesh, 3, spc, 1)
+    bw, md, ws = ctx.band_sizes()
+    assert bw > 832 and ctx.n == 142 * 142, bw
+    assert gpu.landau_band_order_host(mesh, 3)["block_columns"] == 8
+    r, z = ctx.dof_coords()
+    fd = torch.from_numpy(inputs.nodal_f(wl, r, z)[None]).cuda()
+    vals = torch.zeros((1, 1, ctx.nnz), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.zeros(1, dtype=torch.float64, device="cuda"), 2.0, vals, None)
+    band = torch.empty(ws, dtype=torch.float64, device="cuda")
+    piv = torch.full((1, 1, 2), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band, piv)
+    rhs = torch.from_numpy(np.cos(0.01 * np.arange(ctx.n))[None, None] + 2.0).cuda()
+    x = torch.empty_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    pmin, pmax = piv.cpu().numpy()[0, 0]
+    assert 0.0 < pmin <= pmax and pmin > 1e-8 * pmax
+    rowptr, colidx = ctx.csr_pattern_host()
+    A = sps.csr_matrix((vals.cpu().numpy()[0, 0], colidx, rowptr), shape=(ctx.n, ctx.n))
+    xg, b = x.cpu().numpy()[0, 0], rhs.cpu().numpy()[0, 0]
+    res = np.abs(A @ xg - b).max() / (abs(A).sum(axis=1).max() * np.abs(xg).max())
+    assert res <= 1e-13, res
+    xs = spla.spsolve(A.tocsc(), b)
+    assert np.abs(xg - xs).max() <= 1e-8 * np.abs(xs).max()
+
+
+def test_band_lu_reports_breakdown_instead_of_returning_nan_silently(gpu, oracle):
+    """landau_band_factor_batched's pivot report: for sound matrices the smallest and largest |pivot| equal those of
+    Alg. 4.3.1 (Golub & Van Loan) run by the oracle on the RCM-ordered dense block; a matrix with
+    a zero pivot is flagged by smallest = 0 while its neighbours in the batch are untouched."""
+    import torch
+    wl = inputs.config(0)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 3)
+    r, z = ctx.dof_coords()
+    f = np.stack([inputs.nodal_f(wl, r, z)] * 3)
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.zeros((3, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fd, torch.zeros(3, dtype=torch.float64, device="cuda"), 3.0, vals, None)
+    vals[1, 0].zero_()                                   # problem 1, species 0: the zero matrix
+    bw, md, ws = ctx.band_sizes()
+    band = torch.empty(3 * ws, dtype=torch.float64, device="cuda")
+    piv = torch.full((3, ctx.S, 2), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band, piv)
+    piv = piv.cpu().numpy()
+    assert piv[1, 0, 0] == 0.0                           # breakdown reported
+    sp = oracle.build_space(wl.mesh, wl.order)
+    perm = gpu.landau_band_order_host(wl.mesh, wl.order)["perm"]
+    for (k, a) in [(0, 0), (0, 1), (1, 1), (2, 0), (2, 1)]:
+        A = oracle.dense_from_csr(sp, vals[k, a].cpu().numpy())[np.ix_(perm, perm)]
+        LU = oracle.band_lu_outer_product(A, bw, bw)
+        d = np.abs(np.diag(LU))
+        assert abs(piv[k, a, 0] - d.min()) <= 1e-10 * d.min() and abs(piv[k, a, 1] - d.max()) <= 1e-10 * d.max(), (k, a)
+    rhs = torch.ones((3, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
+    x = torch.empty_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    assert torch.isfinite(x[0]).all() and torch.isfinite(x[2]).all() and torch.isfinite(x[1, 1]).all()
+    assert torch.equal(x[0], x[2])
+
+
+def test_multigrid_implicit_operator_band_lu_and_partial_solve(gpu, oracle):
+    """Several grids through NEXT-3 and NEXT-4 together: the implicit-step operator of the 'scaled' two-grid case
+    (blocks = each grid's mass + advection - its Jacobian block), band LU of every species block, solves; then a
+    solve of the FIRST problem only against the workspace factored for two (problem-major workspace)."""
+    import torch
+    name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("scaled")
+    ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, 2)
+    fl = []
+    for a, c in enumerate(comps):
+        r, z = ctx.grid_dof_coords(sgrid[a])
+        fl.append(inputs.maxwellian(float(spc.mass[a]), c.n, c.T, c.zs, r, z))
+    f = np.concatenate(fl)
+    fb = torch.from_numpy(np.stack([f, 0.7 * f])).cuda()
+    Ez, shift = np.array([0.2, -0.1]), 5.0
+    vals = torch.full((2, ctx.vals_stride), float("nan"), dtype=torch.float64, device="cuda")
+    F = torch.full((2, ctx.f_stride), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.implicit_operator_batched(fb, torch.from_numpy(Ez).cuda(), shift, vals, F)
+    vj = torch.zeros_like(vals); cj = torch.zeros_like(F); mv = torch.zeros(ctx.mvals_size, dtype=torch.float64, device="cuda")
+    ctx.jacobian_batched(fb, vj, cj)
+    ctx.mass(shift, mv)
+    spaces = [oracle.build_space(m, order) for m in meshes]
+    fs, vs = ctx.species_slices(), ctx.vals_slices()
+    moff = np.concatenate([[0], np.cumsum([g["nnz"] for g in ctx.grids])])
+    vals_h, F_h, vj_h, cj_h, mv_h = (t.cpu().numpy() for t in (vals, F, vj, cj, mv))
+    one = inputs._sp([(1, 1, 1, 1)])
+    for k in range(2):
+        for a in range(ctx.S):
+            g = sgrid[a]
+            qm = float(spc.charge[a] * spc.m0 / spc.mass[a])
+            Aadv = qm * oracle.csr_values(spaces[g], oracle.advection(spaces[g], one, float(Ez[k]))[0])   # unit species, scaled
+            ref = mv_h[moff[g]:moff[g + 1]] + Aadv - vj_h[k, vs[a]]
+            assert block_err(vals_h[k, vs[a]], ref) <= 1e-12, (k, a)
+    bw, md, ws = ctx.band_sizes()
+    band = torch.empty(2 * ws, dtype=torch.float64, device="cuda")
+    piv = torch.zeros((2, ctx.S, 2), dtype=torch.float64, device="cuda")
+    ctx.band_factor_batched(vals, band, piv)
+    assert (piv[:, :, 0] > 0).all()
+    rhs = torch.from_numpy(np.cos(0.3 * np.arange(2 * ctx.f_stride)).reshape(2, ctx.f_stride) + 2.0).cuda()
+    x = torch.empty_like(rhs)
+    ctx.band_solve_batched(band, rhs, x)
+    x_h, rhs_h = x.cpu().numpy(), rhs.cpu().numpy()
+    for k in range(2):
+        for a in range(ctx.S):
+            A = oracle.dense_from_csr(spaces[sgrid[a]], vals_h[k, vs[a]])
+            xo = np.linalg.solve(A, rhs_h[k, fs[a]])
+            assert np.abs(x_h[k, fs[a]] - xo).max() <= 50 * np.linalg.cond(A) * 2.2e-16 * np.abs(xo).max(), (k, a)
+    x1 = torch.empty((1, ctx.f_stride), dtype=torch.float64, device="cuda")
+    ctx.band_solve_batched(band, rhs[:1].contiguous(), x1)       # nb = 1 against the workspace factored with nb = 2
+    assert torch.equal(x1[0], x[0])
+
+
+def test_pair_paths_can_be_switched_and_the_tensor_cache_changes_nothing(gpu):
+    """landau_set_pair_path replaces the scratch of step a3 inside a live ctx; both paths give the same sums up to
+    rounding; with the tensor cache on, calls skip k_pair_tensor (one launch fewer) and are bitwise equal to a
+    call that evaluates it again."""
+    import torch
+    wl = inputs.config(5, nbatch=5, variant="A")
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 5)
+    assert ctx.pair_path()[0] == gpu.LANDAU_PAIR_SHARED           # max_batch >= LANDAU_SHARED_MIN_BATCH
+    assert gpu.LandauContext(wl.mesh, wl.order, wl.species, 3).pair_path()[0] == gpu.LANDAU_PAIR_PER_PROBLEM
+    r, z = ctx.dof_coords()
+    fd = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in range(5)])).cuda()
+
+    def build():
+        v = torch.full((5, ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+        c = torch.full((5, ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+        l0 = ctx.launch_count()
+        ctx.jacobian_batched(fd, v, c)
+        torch.cuda.synchronize()
+        return v, c, ctx.launch_count() - l0
+    vs, cs, ls = build()
+    ctx.set_tensor_cache(True)
+    v1, c1, l1 = build()
+    v2, c2, l2 = build()
+    assert l1 == ls - 1 and l2 == ls - 1        # the tensor of the call before the switch is still valid
+    assert torch.equal(v1, vs) and torch.equal(v2, vs) and torch.equal(c2, cs)
+    ctx.set_tensor_cache(False)
+    assert build()[2] == ls
+    ctx.set_pair_path(gpu.LANDAU_PAIR_PER_PROBLEM)
+    path, nbytes = ctx.pair_path()
+    assert path == gpu.LANDAU_PAIR_PER_PROBLEM and nbytes > 0
+    vp, cp, _ = build()
+    for a in range(ctx.S):
+        assert block_err(vp[:, a].cpu().numpy(), vs[:, a].cpu().numpy()) <= 1e-12
+        assert block_err(cp[:, a].cpu().numpy(), cs[:, a].cpu().numpy()) <= 1e-12
+    ctx.set_pair_path(gpu.LANDAU_PAIR_AUTO)
+    assert ctx.pair_path()[0] == gpu.LANDAU_PAIR_SHARED
+    v3, c3, _ = build()
+    assert torch.equal(v3, vs) and torch.equal(c3, cs)
+
+
+def test_a_batch_that_cannot_fit_fails_cleanly_with_enomem(gpu):
+    """max_batch = 65,535 with 16 species on mesh 3B asks for 660 GB of element matrices: landau_create returns
+    LANDAU_ENOMEM (nothing is left allocated: a normal ctx can be created and used right after)."""
+    import torch
+    mesh = inputs.mesh_config3("B")
+    rows = [(1.0 + 3.0 * s, (-1) ** s * (1 + s % 3), 1.0, 1.0) for s in range(16)]
+    free0 = torch.cuda.mem_get_info()[0]
+    with pytest.raises(gpu.LandauError) as ei:
+        gpu.LandauContext(mesh, 3, inputs._sp(rows), 65535)
+    assert ei.value.code == gpu.LANDAU_ENOMEM
+    with pytest.raises(gpu.LandauError) as ei:
+        gpu.LandauContext(mesh, 3, inputs._sp(rows), 65536)        # beyond the documented range of max_batch
+    assert ei.value.code == gpu.LANDAU_EINVAL
+    assert abs(torch.cuda.mem_get_info()[0] - free0) < (64 << 20)
+    wl = inputs.config(0)
+    ctx, f, vals, Cf, mv = run_gpu(gpu, wl, [0])
+    assert np.isfinite(vals).all()

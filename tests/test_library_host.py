@@ -130,3 +130,27 @@ def test_multigrid_argument_checks_need_no_gpu(binding):
         with pytest.raises(binding.LandauError) as ei:
             binding.LandauMultigridContext([g, inputs.mesh_scaled(g, 0.5)], [0, 1, 1], 2, sp3, 1)
         assert ei.value.code == binding.LANDAU_ECUDA
+
+
+def test_new_entry_points_check_their_arguments_without_a_gpu(binding):
+    """Path selection, tensor cache, issue probe and the max_batch range: bad arguments give LANDAU_EINVAL before any
+    device is looked for."""
+    import ctypes
+    L = binding.lib()
+    assert L.landau_set_pair_path(None, binding.LANDAU_PAIR_SHARED) == binding.LANDAU_EINVAL
+    assert L.landau_pair_path(None, None, None) == binding.LANDAU_EINVAL
+    assert L.landau_set_tensor_cache(None, 1) == binding.LANDAU_EINVAL
+    cyc = ctypes.c_double()
+    assert L.landau_fp64_issue_probe(6, 16, ctypes.byref(cyc), None) == binding.LANDAU_EINVAL       # unknown mode
+    assert L.landau_fp64_issue_probe(0, 0, ctypes.byref(cyc), None) == binding.LANDAU_EINVAL        # iters < 1
+    assert L.landau_fp64_issue_probe(0, 16, None, None) == binding.LANDAU_EINVAL
+    wl = inputs.config(1)
+    for bad_batch in (0, 65536):
+        with pytest.raises(binding.LandauError) as ei:
+            binding.LandauContext(wl.mesh, wl.order, wl.species, bad_batch)
+        assert ei.value.code == binding.LANDAU_EINVAL
+    assert (binding.LANDAU_PAIR_AUTO, binding.LANDAU_PAIR_PER_PROBLEM, binding.LANDAU_PAIR_SHARED) == (0, 1, 2)
+    hdr = open(os.path.join(os.path.dirname(__file__), "..", "include", "landau.h")).read()
+    for name, val in (("LANDAU_PAIR_AUTO", 0), ("LANDAU_PAIR_PER_PROBLEM", 1), ("LANDAU_PAIR_SHARED", 2),
+                      ("LANDAU_SHARED_MIN_BATCH", binding.LANDAU_SHARED_MIN_BATCH)):
+        assert re.search(rf"#define {name} {val}\b", hdr), name
