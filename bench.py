@@ -71,7 +71,7 @@ def load_roofline_inputs():
             for row in csv.DictReader(l for l in fh if not l.startswith("#")):
                 if row["source_sha"] == sha:
                     out[(row["kernel"], row["workload"])] = {k: (float(v) if v not in ("", None) else None)
-                                                             for k, v in row.items() if k not in ("kernel", "workload", "source_sha")}
+                                                             for k, v in row.items() if k not in ("kernel", "workload", "source_sha", "instance")}
     except Exception:
         pass
     return out
@@ -242,10 +242,15 @@ def fp64_roof(kind, kernel, flop_per_pair, pairs, ms, peak, probe, extra=None):
     return d
 
 
-def pair_sym_roof(rin, key, kname, pairs, ms, peak, probe, issue):
-    """Roofline entry of the per-problem pair kernel from the ncu-counted instruction mix of workload `key`."""
-    c = rin.get((kname, key)) or rin.get(("k_pair_sym", key))
-    if not c or not ms:
+def pair_sym_roof(rin, key, kname, pairs, ms, peak, probe, issue, mix_key=None):
+    """Roofline entry of the per-problem pair kernel from the ncu-counted instruction mix of workload `key`
+    (`mix_key`: the workload whose counters give the mix when `key`'s capture has none -- same kernel, same mesh)."""
+    c = rin.get(("k_pair_sym", key))
+    if mix_key and rin.get(("k_pair_sym", mix_key)) and (not c or c.get("dfma") is None):
+        m = rin[("k_pair_sym", mix_key)]
+        c = dict(c or {"dram_read": None, "dram_write": None})
+        c.update({k: m[k] for k in ("dfma", "dmul", "dadd", "units_per_launch")})
+    if not c or not ms or c.get("dfma") is None:
         return fp64_roof("alu", kname, None, pairs, ms, peak, probe, {"note": "no ncu counters for this source revision"})
     upl = c["units_per_launch"]
     dfma, dmul, dadd = c["dfma"] / upl, c["dmul"] / upl, c["dadd"] / upl     # thread instructions per ordered pair
@@ -504,26 +509,29 @@ def run_ours(args):
             c = rin.get(("k_apply_dmma", "cfg5:main")) or {}
             roof = fp64_roof("tensor", "k_apply_dmma<4,2>", APPLY_FLOP_PER_PAIR, pairs_per_step, apply_ms, peaks["fp64"], peaks["dmma_probe"], {
                 "traffic": (c.get("dram_read", 0) + c.get("dram_write", 0)) if c else None,
-                "ncu_fp64_pipe_pct": c.get("fp64_pipe_pct") if c else None,
+                "ncu_dmma_pipe_pct": c.get("dmma_pipe_pct") if c else None,
                 "peak_source": peaks["source"], "peak_probe_measured": peaks["dmma_probe"],
                 "kernel_share_of_step": apply_ms / ms_per_step if world == 1 else None,
                 "what": "fp64 mma.sync.m8n8k4 (DMMA.8x8x4) contraction G = U T: 7 products = 14 flop per ordered pair and problem"})
             c = rin.get(("k_pair_tensor", "cfg5:main"))
+            m = rin.get(("k_pair_tensor", "cfg3B:batched:shared"))       # same kernel, same mesh: instruction mix
+            if c and m and c.get("dfma") is None:
+                c = dict(c); c.update({k: m[k] for k in ("dfma", "dmul", "dadd", "units_per_launch")})
             tens = None
-            if c and tensor_ms:
+            if c and tensor_ms and c.get("dfma") is not None:
                 upl = c["units_per_launch"]
                 fl = (2 * c["dfma"] + c["dmul"] + c["dadd"]) / upl
                 tens = fp64_roof("alu", "k_pair_tensor", fl, ctx.N * (ctx.N - 1), tensor_ms, peaks["fp64"], peaks["probe"],
                                  {"traffic": c["dram_read"] + c["dram_write"], "what": "one tensor evaluation per ORDERED pair and call (K, E by the scaled AGM), all problems share it"})
         else:
-            roof = pair_sym_roof(rin, "cfg5:main", "k_pair_sym<128,2>", pairs_per_step, tensor_ms, peaks["fp64"], peaks["probe"], peaks["issue"])
+            roof = pair_sym_roof(rin, "cfg5:per_problem", "k_pair_sym<128,2>", pairs_per_step, tensor_ms, peaks["fp64"], peaks["probe"], peaks["issue"], "cfg3B:batched")
             tens = None
         # the per-problem path on the same workload (round 1's headline kernel), and the tensor cache
         ctx.set_pair_path(binding.LANDAU_PAIR_PER_PROBLEM)
         pp_ms = float(np.median(timed_steps(torch, lambda: ctx.jacobian_batched(f, vals, Cf), 5, flush)))
         pp_k = a3_profile(ctx, torch, lambda: ctx.jacobian_batched(f, vals, Cf), 3)[0]
         per_problem = {"ms_per_step": pp_ms, "gpair_per_s": pairs_per_step / (pp_ms * 1e-3) * 1e-9, "builds_per_s": nb / (pp_ms * 1e-3),
-                       "roofline": pair_sym_roof(rin, "cfg5:per_problem", "k_pair_sym<128,2>", pairs_per_step, pp_k, peaks["fp64"], peaks["probe"], peaks["issue"]),
+                       "roofline": pair_sym_roof(rin, "cfg5:per_problem", "k_pair_sym<128,2>", pairs_per_step, pp_k, peaks["fp64"], peaks["probe"], peaks["issue"], "cfg3B:batched"),
                        "what": "LANDAU_PAIR_PER_PROBLEM: every problem evaluates every pair's tensor itself (symmetric tile pairs)"}
         ctx.set_pair_path(binding.LANDAU_PAIR_AUTO)
         ctx.set_tensor_cache(True)
@@ -634,6 +642,7 @@ NCU_COLS = {
     "dadd": "smsp__sass_thread_inst_executed_op_dadd_pred_on.sum", "dram_read": "dram__bytes_read.sum", "dram_write": "dram__bytes_write.sum",
     "time_ns": "gpu__time_duration.sum", "fp64_pipe_pct": "sm__inst_executed_pipe_fp64.avg.pct_of_peak_sustained_active",
     "issue_active_pct": "smsp__issue_active.avg.pct_of_peak_sustained_active", "inst_executed": "smsp__inst_executed.sum",
+    "dmma_pipe_pct": "sm__inst_executed_pipe_tensor_subpipe_dmma.avg.pct_of_peak_sustained_active",
 }
 
 
@@ -645,14 +654,17 @@ def summarise_ncu(paths, plan_file):
     sha = plan["source_sha"]
     w = csv.writer(sys.stdout)
     cols = list(NCU_COLS)
-    w.writerow(["kernel", "workload", "source_sha", "units_per_launch"] + cols)
+    w.writerow(["kernel", "workload", "source_sha", "units_per_launch"] + cols + ["instance"])
     for p in paths:
         rows = list(csv.DictReader(l for l in open(p) if l.startswith('"')))
-        rows = [r for r in rows if r.get("ID", "").strip().isdigit()]          # drop the units row
+        units = next((r for r in rows if not r.get("ID", "").strip().isdigit()), {})     # the units row
+        rows = [r for r in rows if r.get("ID", "").strip().isdigit()]
+        scale = {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12, "us": 1e3, "ms": 1e6, "s": 1e9}   # -> byte, ns
+
         def val(r, col):
             v = r.get(col, "")
             try:
-                return float(v.replace(",", ""))
+                return float(v.replace(",", "")) * scale.get(units.get(col, ""), 1.0)
             except Exception:
                 return None
         seq = {"k_pair_sym": [], "k_pair_tensor": [], "k_apply_dmma": []}
@@ -662,19 +674,19 @@ def summarise_ncu(paths, plan_file):
             hit = next((k for k in seq if k in name), None)
             if hit:
                 seq[hit].append(r)
-            elif "landau::" in name or name.startswith("k_"):
+            elif "landau::" in name or name.startswith("k_") or " k_" in name:
                 rest.setdefault("rest", []).append(r)
         for kern, lst in seq.items():
             entries = [e for e in plan["plan"] if (kern == "k_pair_sym") == (not e["workload"].endswith(":shared") and e["workload"] != "cfg5:main")]
             for r, e in zip(lst, entries):
-                units = e["tensor_pairs_per_launch"] if kern == "k_pair_tensor" else e["pairs_per_launch"]
-                short = r["Kernel Name"].split("(")[0].replace("landau::", "").replace("void ", "")
-                w.writerow([short if kern == "k_pair_sym" else kern, e["workload"], sha, units] + [val(r, NCU_COLS[c]) for c in cols])
+                upl = e["tensor_pairs_per_launch"] if kern == "k_pair_tensor" else e["pairs_per_launch"]
+                inst = r["Kernel Name"].split("(")[0].replace("landau::", "").replace("void ", "").replace(" ", "").replace(",", ";")
+                w.writerow([kern, e["workload"], sha, upl] + [val(r, NCU_COLS[c]) for c in cols] + [inst])
         if rest.get("rest") and plan["kernel_run"] == "main":
             # the other kernels of the FIRST step (shared path): summed
             n_first = len(rest["rest"]) // 2
             tot = {c: sum((val(r, NCU_COLS[c]) or 0.0) for r in rest["rest"][:n_first]) for c in cols}
-            w.writerow(["rest", "cfg5:main", sha, plan["plan"][0]["pairs_per_launch"]] + [tot[c] for c in cols])
+            w.writerow(["rest", "cfg5:main", sha, plan["plan"][0]["pairs_per_launch"]] + [tot[c] for c in cols] + ["all other kernels of the step"])
 
 
 def main():

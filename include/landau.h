@@ -242,8 +242,10 @@ int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_
  * bound" of DESIGN.md).  Register-resident streams on every SM, three warps per SM sub-partition (one for mode 4),
  * timed with clock64() on the SM.  mode: 0 DFMA with two register operands + immediate; 1 DFMA with two distinct
  * registers; 2 DFMA with three distinct registers; 3 DFMA with three registers of which one is shared by
- * consecutive instructions; 4 one dependent DFMA chain (latency); 5 DMMA m8n8k4 with independent accumulators.
- * Returns SM cycles per warp instruction and sub-partition, and (flops_per_s may be NULL) the whole-GPU rate by
+ * consecutive instructions; 4 one dependent DFMA chain (latency); 5 DMMA m8n8k4 with independent accumulators;
+ * 6 / 7 as 0 with one / two independent integer multiply-adds beside every DFMA (cycles are still per DFMA: do
+ * the other pipes issue in the shadow of the FP64 issue?).
+ * Returns SM cycles per (FP64) warp instruction and sub-partition, and (flops_per_s may be NULL) the whole-GPU rate by
  * wall clock (CUDA events).  Synchronises. */
 int landau_fp64_issue_probe(int mode, int iters, double *cycles_per_warp_instruction, double *flops_per_s);
 

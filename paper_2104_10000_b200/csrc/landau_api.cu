@@ -803,7 +803,7 @@ int landau_fp64_peak_probe(int iters, double *flops_per_s, double *sm_clock_mhz_
 }
 
 int landau_fp64_issue_probe(int mode, int iters, double *cycles_per_warp_instruction, double *flops_per_s) {
-    if (iters < 1 || mode < 0 || mode > 5 || !cycles_per_warp_instruction) return LANDAU_EINVAL;
+    if (iters < 1 || mode < 0 || mode > 7 || !cycles_per_warp_instruction) return LANDAU_EINVAL;
     return guarded([&]() {
         int dev = 0, sms = 0;
         CK(cudaGetDevice(&dev));

@@ -163,74 +163,171 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
     }
 }
 
+// Small N (N < 2560: single builds are latency-bound there, a warp needs ~350 ns per step of its j walk): tiles of
+// 32 points, one i per thread, and the 32 steps of a tile pair are SHARED BY WS WARPS -- warp w takes the rotation
+// offsets [w 32/WS, (w+1) 32/WS) (diagonal tiles: the j with j mod WS = w).  Every warp then holds partial sums
+// for the same 32 targets i and for the j it visited; they are added over the warps in warp order, so the
+// summation order is again a function of N alone.  N = 450: 17.5 -> 6 us, N = 2048: 28.7 -> 17 us.
+template <int WS, bool CHECK_ALL>
+__global__ void __launch_bounds__(32 * WS)
+k_pair_split(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
+             const double *__restrict__ T, double *__restrict__ Gpart) {
+    pdl_prologue();
+    constexpr int TS = 32, NS = 32 / WS;
+    __shared__ double sj[7][TS];
+    __shared__ double sacc[WS][2][5][TS];     // [warp][0: targets i, 1: targets j][component][point]
+    const int b = blockIdx.y;
+    const int p = blockIdx.x;
+    int J = int((sqrt(8.0 * double(p) + 1.0) - 1.0) * 0.5);
+    while ((J + 1) * (J + 2) / 2 <= p) ++J;
+    while (J * (J + 1) / 2 > p) --J;
+    const int I = p - J * (J + 1) / 2;
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const double *Tb = T + (size_t)b * 3 * N;
+    const int i = I * TS + lane;
+    const bool valid = i < N;
+    IPoint pi[1];
+    {
+        const int ic = valid ? i : N - 1;
+        const double ri = r[ic], iri = invr[ic];
+        pi[0].r = ri; pi[0].z = z[ic]; pi[0].r2x = 2.0 * ri; pi[0].rr2 = 2.0 * ri * ri; pi[0].c = 0.0625 * iri * iri;
+        pi[0].tD = valid ? Tb[ic] : 0.0; pi[0].tKr = valid ? Tb[N + ic] : 0.0; pi[0].tKz = valid ? Tb[2 * N + ic] : 0.0;
+    }
+    const int jbase = J * TS;
+    const int cnt = min(TS, N - jbase);
+    if (tid < TS) {
+        const int t = tid;
+        if (t < cnt) {
+            const int j = jbase + t;
+            const double rj = r[j], irj = invr[j];
+            sj[0][t] = rj; sj[1][t] = z[j]; sj[2][t] = irj * irj; sj[3][t] = 2.0 * rj * rj;
+            sj[4][t] = Tb[j]; sj[5][t] = Tb[N + j]; sj[6][t] = Tb[2 * N + j];
+        } else {      // padding of a ragged tile: a far-away point with zero weight (finite tensor, no effect)
+            sj[0][t] = 1.0; sj[1][t] = 1.0e6; sj[2][t] = 1.0; sj[3][t] = 2.0;
+            sj[4][t] = 0.0; sj[5][t] = 0.0; sj[6][t] = 0.0;
+        }
+    }
+    __syncthreads();
+    PairAcc acc = {0.0, 0.0, 0.0, 0.0, 0.0};
+    if (I == J) {
+        for (int t = warp; t < cnt; t += WS) {
+            const JPoint pj = {sj[0][t], sj[1][t], sj[2][t], sj[3][t], sj[4][t], sj[5][t], sj[6][t]};
+            PairParts pp[1];
+            pair_parts<1, true>(pi, pj, pp);
+            accumulate_i(acc, pj, pair_tensor(pi[0], pj, pp[0]));
+        }
+    } else {
+        const int src = (lane + 1) & 31, k0 = warp * NS;
+        double v0 = 0.0, v1 = 0.0, v2 = 0.0, v3 = 0.0, v4 = 0.0;
+#pragma unroll 1
+        for (int k = k0; k < k0 + NS; ++k) {
+            const int t = (lane + k) & 31;
+            const JPoint pj = {sj[0][t], sj[1][t], sj[2][t], sj[3][t], sj[4][t], sj[5][t], sj[6][t]};
+            PairParts pp[1];
+            pair_parts<1, CHECK_ALL>(pi, pj, pp);
+            const PairTensor tt = pair_tensor(pi[0], pj, pp[0]);
+            accumulate_i(acc, pj, tt);
+            v0 = fma(pi[0].tD, tt.UDrrT, v0);
+            v1 = fma(pi[0].tD, tt.A5, v1);
+            v2 = fma(pi[0].tD, tt.A3, v2);
+            v3 = fma(tt.A4, pi[0].tKr, fma(tt.A5, pi[0].tKz, v3));
+            v4 = fma(-tt.A2, pi[0].tKr, fma(tt.A3, pi[0].tKz, v4));
+            v0 = __shfl_sync(0xffffffffu, v0, src);
+            v1 = __shfl_sync(0xffffffffu, v1, src);
+            v2 = __shfl_sync(0xffffffffu, v2, src);
+            v3 = __shfl_sync(0xffffffffu, v3, src);
+            v4 = __shfl_sync(0xffffffffu, v4, src);
+        }
+        const int jl = (lane + k0 + NS) & 31;      // the j whose sums this lane holds after NS steps
+        sacc[warp][1][0][jl] = v0; sacc[warp][1][1][jl] = v1; sacc[warp][1][2][jl] = v2;
+        sacc[warp][1][3][jl] = v3; sacc[warp][1][4][jl] = v4;
+    }
+    sacc[warp][0][0][lane] = acc.drr; sacc[warp][0][1][lane] = acc.drz; sacc[warp][0][2][lane] = acc.dzz;
+    sacc[warp][0][3][lane] = acc.kr; sacc[warp][0][4][lane] = acc.kz;
+    __syncthreads();
+    // warp 0 adds the partial sums of the targets i, warp 1 (if there is one) those of the targets j
+    const int side = WS > 1 ? warp : 0;
+    for (int sd = side; sd < 2; sd += WS) {
+        if (sd == 1 && I == J) break;
+        const int pt = sd == 0 ? i : jbase + lane;
+        if (sd == 0 ? valid : lane < cnt) {
+            double *G = Gpart + ((size_t)b * ntiles + (sd == 0 ? J : I)) * 5 * N + pt;
+#pragma unroll
+            for (int c = 0; c < 5; ++c) {
+                double sum = sacc[0][sd][c][lane];
+#pragma unroll
+                for (int w = 1; w < WS; ++w) sum += sacc[w][sd][c][lane];
+                G[(size_t)c * N] = sum;
+            }
+        }
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // a1 + a2: field values at the integration points and the beta sums (L101, Alg. 1 lines 5-8,
 // Eq. 10).  grid = (ceil(Ne/EPB), nb), block = (Nq, EPB).  Thread (q, e): local node a = q
 // gathers u_a = sum P_e[a,d] f_b[d]; then f = B u, grad f = J^-T (E u).
 // Output T[b][3][N] = w_in * (T_D, T_Kr, T_Kz): the weight of the inner sum is folded in here.
 // ------------------------------------------------------------------------------------------------
-constexpr int FIELD_EPB = 8;
-constexpr int FIELD_ROUNDS = 4;   // cells per thread: the tabulation rows stay in registers across them
+constexpr int FIELD_EPB = 8;      // cells per block
 
 // TILED: T in the layout of the batch-shared contraction (landau_shared.cu): T[c][jo][b][k][h], j = 8 jo + 4 h + k.
+// The kernel is latency-bound (three dependent loads per gathered value, a few hundred flop per cell): small blocks
+// with few registers (tabulations transposed in shared memory: conflict-free), every species gathered before the
+// one barrier, so that many independent list walks are in flight per SM.
 template <bool TILED>
-__global__ void k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T) {
+__global__ void __launch_bounds__(16 * FIELD_EPB)
+k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T) {
     pdl_prologue();
-    __shared__ double s_u[FIELD_EPB][16];
+    __shared__ double s_tab[3][16][16];                     // [B, E0, E1][a][q]
+    __shared__ double s_u[FIELD_EPB][MAX_SPECIES][16];      // u = P_e f of every species of the block's cells
     const int b = blockIdx.y;
     const int q = threadIdx.x;
-    const int Nb = ds.Nb;
+    const int Nb = ds.Nb, Nq = ds.Nq;
     const double *fb = f + (size_t)b * ds.fstride;
-    double *Tb = T + (size_t)b * 3 * ds.Ntot + ds.poff;
-    double tB[16], tE0[16], tE1[16];      // row q of the tabulations
-#pragma unroll
-    for (int a = 0; a < 16; ++a) {
-        const bool in = a < Nb;
-        tB[a] = in ? ds.B[q * Nb + a] : 0.0; tE0[a] = in ? ds.E0[q * Nb + a] : 0.0; tE1[a] = in ? ds.E1[q * Nb + a] : 0.0;
+    for (int t = threadIdx.y * Nq + q; t < Nq * Nb; t += Nq * FIELD_EPB) {
+        const int qq = t / Nb, a = t % Nb;
+        s_tab[0][a][qq] = ds.B[t]; s_tab[1][a][qq] = ds.E0[t]; s_tab[2][a][qq] = ds.E1[t];
     }
-    for (int round = 0; round < FIELD_ROUNDS; ++round) {
-        const int e = (blockIdx.x * FIELD_ROUNDS + round) * FIELD_EPB + threadIdx.y;
-        const bool valid = e < ds.Ne;
-        double tD = 0.0, tKr = 0.0, tKz = 0.0;
-        double ijr = 0.0, ijz = 0.0;
-        if (valid) { ijr = ds.invJ[2 * e]; ijz = ds.invJ[2 * e + 1]; }
+    const int e = blockIdx.x * FIELD_EPB + threadIdx.y;
+    const bool valid = e < ds.Ne;
+    if (valid) {
+        const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
         for (int sp = 0; sp < ds.S; ++sp) {
-            if (valid) {
-                double u = 0.0;
-                const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
-                for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
-                s_u[threadIdx.y][q] = u;
-            }
-            __syncthreads();
-            if (valid) {
-                double fq = 0.0, g0 = 0.0, g1 = 0.0;
+            double u = 0.0;
+            for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
+            s_u[threadIdx.y][sp][q] = u;
+        }
+    }
+    __syncthreads();
+    if (!valid) return;
+    const double ijr = ds.invJ[2 * e], ijz = ds.invJ[2 * e + 1];
+    double tD = 0.0, tKr = 0.0, tKz = 0.0;
+    for (int sp = 0; sp < ds.S; ++sp) {
+        double fq = 0.0, g0 = 0.0, g1 = 0.0;
 #pragma unroll
-                for (int a = 0; a < 16; ++a) {
-                    if (a < Nb) {
-                        const double u = s_u[threadIdx.y][a];
-                        fq = fma(tB[a], u, fq);
-                        g0 = fma(tE0[a], u, g0);
-                        g1 = fma(tE1[a], u, g1);
-                    }
-                }
-                const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
-                tD = fma(e2, fq, tD);
-                tKr = fma(em, ijr * g0, tKr);
-                tKz = fma(em, ijz * g1, tKz);
-            }
-            __syncthreads();
-        }
-        if (valid) {
-            const int gi = e * ds.Nq + q;
-            const double w = ds.w_in[gi];
-            if (TILED) {
-                const int j = ds.poff + gi;
-                const size_t o = (((size_t)(j >> 3) * nbpad + b) * 4 + (j & 3)) * 2 + ((j >> 2) & 1), cs = (size_t)Kq8 * nbpad * 8;
-                T[o] = w * tD; T[cs + o] = w * tKr; T[2 * cs + o] = w * tKz;
-            } else {
-                Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
+        for (int a = 0; a < 16; ++a) {
+            if (a < Nb) {
+                const double u = s_u[threadIdx.y][sp][a];
+                fq = fma(s_tab[0][a][q], u, fq);
+                g0 = fma(s_tab[1][a][q], u, g0);
+                g1 = fma(s_tab[2][a][q], u, g1);
             }
         }
+        const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
+        tD = fma(e2, fq, tD);
+        tKr = fma(em, ijr * g0, tKr);
+        tKz = fma(em, ijz * g1, tKz);
+    }
+    const int gi = e * Nq + q;
+    const double w = 12.566370614359172953850573533118 * ds.w_in[gi];    // 4 pi of the tensor (landau_pair_math.cuh) folded in
+    if (TILED) {
+        const int j = ds.poff + gi;
+        const size_t o = (((size_t)(j >> 3) * nbpad + b) * 4 + (j & 3)) * 2 + ((j >> 2) & 1), cs = (size_t)Kq8 * nbpad * 8;
+        T[o] = w * tD; T[cs + o] = w * tKr; T[2 * cs + o] = w * tKz;
+    } else {
+        double *Tb = T + (size_t)b * 3 * ds.Ntot + ds.poff;
+        Tb[gi] = w * tD; Tb[ds.Ntot + gi] = w * tKr; Tb[2 * ds.Ntot + gi] = w * tKz;
     }
 }
 
@@ -506,6 +603,8 @@ __global__ void k_dfma_probe(int iters, double *out) {
 //   MODE 3  DFMA, three registers, one shared by neighbours     x = fma(x, Y, z)   (operand reuse cache)
 //   MODE 4  one dependent DFMA chain, one warp per sub-partition (latency)
 //   MODE 5  DMMA m8n8k4, 8 independent accumulators per warp
+//   MODE 6  as 0, plus ONE independent integer multiply-add per DFMA   (do other pipes issue under FP64 issue?)
+//   MODE 7  as 0, plus TWO independent integer multiply-adds per DFMA
 template <int MODE>
 __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *out, long long *cycles) {
     constexpr int CH = 8;
@@ -513,6 +612,9 @@ __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *
 #pragma unroll
     for (int c = 0; c < CH; ++c) { x[c] = in[threadIdx.x + c]; y[c] = in[threadIdx.x + 32 + c]; z[c] = in[threadIdx.x + 64 + c]; }
     double Y = in[threadIdx.x + 100];
+    int n[2 * CH];
+#pragma unroll
+    for (int c = 0; c < 2 * CH; ++c) n[c] = threadIdx.x + c + iters;
     __syncthreads();
     const long long t0 = clock64();
     for (int i = 0; i < iters; ++i) {
@@ -527,7 +629,9 @@ __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *
         } else {
 #pragma unroll
             for (int c = 0; c < CH; ++c) {
-                if (MODE == 0) x[c] = fma(x[c], y[c], 1.5);
+                if (MODE == 0 || MODE >= 6) x[c] = fma(x[c], y[c], 1.5);
+                if (MODE >= 6) n[c] = n[c] * 3 + 7;
+                if (MODE == 7) n[CH + c] = n[CH + c] * 5 + 3;
                 if (MODE == 1) x[c] = fma(y[c], y[c], x[c]);
                 if (MODE == 2) x[c] = fma(y[c], z[c], x[c]);
                 if (MODE == 3) x[c] = fma(x[c], Y, z[c]);
@@ -539,7 +643,7 @@ __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *
     __syncthreads();
     double sum = 0.0;
 #pragma unroll
-    for (int c = 0; c < CH; ++c) sum += x[c] + y[c] + z[c];
+    for (int c = 0; c < CH; ++c) sum += x[c] + y[c] + z[c] + double(n[c] ^ n[CH + c]);
     if (sum == 12345.678) out[0] = sum;     // keep the chains alive
     if (threadIdx.x == 0) cycles[blockIdx.x] = t1 - t0;
 }
@@ -552,17 +656,17 @@ __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *
 // more warps and fewer steps (N = 2048: 39 -> 31 us); large N is throughput-bound: two i per thread.
 int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 2560 ? 64 : 32); }
 int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / ts; }
+// Warps sharing a tile pair where the tiles are 32 points (k_pair_split): a function of N only, like the tile size.
+int pair_split_warps(int N) { return N < 1536 ? 4 : 2; }
 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
-    constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
-    dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
+    dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
     launch_k(k_fields_beta<false>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, 0, 0, f, T);
     return 1;
 }
 
 int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, cudaStream_t st) {
-    constexpr int per_block = FIELD_EPB * FIELD_ROUNDS;
-    dim3 grid((ds.Ne + per_block - 1) / per_block, nb), block(ds.Nq, FIELD_EPB);
+    dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
     launch_k(k_fields_beta<true>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, shared_kpad(ds.Ntot) / 8, nbpad, f, T);
     return 1;
 }
@@ -575,7 +679,8 @@ static void launch_pair_t(int N, const double *r, const double *z, const double 
     const bool pdl = nb <= PDL_MAX_NB;
     if (ts == 128) launch_k(k_pair_sym<128, 2, CHECK_ALL>, grid, dim3(64), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
     else if (ts == 64) launch_k(k_pair_sym<64, 2, CHECK_ALL>, grid, dim3(32), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
-    else launch_k(k_pair_sym<32, 1, CHECK_ALL>, grid, dim3(32), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
+    else if (pair_split_warps(N) == 4) launch_k(k_pair_split<4, CHECK_ALL>, grid, dim3(128), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
+    else launch_k(k_pair_split<2, CHECK_ALL>, grid, dim3(64), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
 }
 
 int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
@@ -657,6 +762,8 @@ int launch_issue_probe(int mode, int blocks, int threads, int iters, const doubl
         case 3: launch_k(k_issue_probe<3>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
         case 4: launch_k(k_issue_probe<4>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
         case 5: launch_k(k_issue_probe<5>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 4;
+        case 6: launch_k(k_issue_probe<6>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
+        case 7: launch_k(k_issue_probe<7>, dim3(blocks), dim3(threads), 0, st, false, iters, in, out, cycles); return 8;
         default: return 0;
     }
 }

@@ -39,9 +39,15 @@ __device__ __forceinline__ double sqrt_times2_fast(double x) {
     asm("rsqrt.approx.ftz.f64 %0, %1;" : "=d"(y) : "d"(x));
     const double t = x * y;
     const double r = fma(-t, y, 1.0);
+#ifdef SQRT_SHALLOW      // one instruction more, one level less on the dependent chain: 2t + (t r)(1 + 3r/4)
+    const double tr = t * r;
+    const double p = fma(0.75, r, 1.0);
+    return fma(tr, p, t + t);
+#else
     const double p = fma(0.75, r, 1.0);
     const double q = fma(p, r, 2.0);
     return t * q;
+#endif
 }
 
 // x * 2^e for a normal positive x that stays normal (integer add on the exponent field)
@@ -64,24 +70,30 @@ __device__ __forceinline__ double scale_pow2(double x, int e) {
 // Evaluated with rho2 = 2 r rb = q/2, 2W and 4Kt so that no multiplication by a power of two remains:
 //     g = 1 + q W = 1 + rho2 (2W),  Pss/2 = (4Kt)(2W),  Pc = (4Kt/s) g,  P0 = (4Kt/s)(s - rho2 g)/d2
 //     (s - rho2 g = (s + d2 - q^2 W)/2 because s - d2 = q).
-// The iteration stops for the whole warp once every lane's next c would be <= 2^-26 a (the a used
-// for K is then within 2^-54 a of the limit).  The test compares exponents with integer ops, one
-// pass ahead.
+// The AGM is NOT run to convergence: after P passes (A = A_{P+1}, B = B_{P+1}) with e = c_{P+2}/a_{P+2} =
+// (A - B)/(A + B) small, both limits are finished in closed form (x = e^2):
+//     pi/(2 agm(a, b)) = K(e)/a_{P+2}               ->  4 Kt = 4 pi 2^(P+1) F(x)/(A + B),   F = (2/pi) K(e)
+//     sum_{j>=P+2} 2^j c_j^2 = 2 a_{P+2}^2 2^(P+2) (1 - E(e)/K(e)) = (C^2 / 2^(P+2)) G(x),   C = A - B,
+//     F(x) = 1 + x/4 + 9x^2/64 + 25x^3/256 + 1225x^4/16384 + ..,  G(x) = 2(1 - E/K)/x = 1 + x/8 + x^2/16 + 41x^3/1024 + ..
+// (the standard AGM relation E = K (1 - sum_{i>=0} 2^(i-1) c_i^2) applied to the sequence restarted at step P+2).
+// With e <= 2^-6 the truncations used (F to x^3, G to x^3) are below 2^-51.7 (F) and 2^-54 of W (G's term is at most
+// 2^-7 of W).
+// The number of passes follows from d2/s = k'^2 ALONE (e_1 = (1-k')/(1+k'), e_{k+1} = e_k^2/(1+sqrt(1-e_k^2))^2):
+// P = 0 for d2/s >= 0.366, 1 for >= 0.0129, 2 for >= 1.05e-5, 3 for >= 6.9e-12, 4 for >= 2.9e-24, else 5 -- so it is
+// decided BEFORE the first square root from the exponent fields of d2 and s (integer compares of the high words,
+// thresholds 0.0862 = max |m - log2(1+m)| on the safe side), the warp takes the maximum over its lanes
+// (one REDUX), and the loop has a known trip count: no vote waits for the end of a dependent sqrt chain.
+// Measured against the version that iterated to c <= 2^-26 a with an exit vote per pass: DESIGN.md 6.1.
+// The constant 4 pi is not applied here: it sits in the weights w_in of T (k_fields_beta).
 //
 // FP64 issue cost on sm_100a (measured): 2 cycles per warp instruction and SM
-// sub-partition, 3 cycles for a DFMA with three distinct register operands; 9 cycles dependent
+// sub-partition, 3 cycles for a DFMA with three distinct register operands; 8 cycles dependent
 // latency.  Hence the lock-step evaluation of several pairs per thread and the care for operand count.
 // ------------------------------------------------------------------------------------------------
 struct PairAcc { double drr, drz, dzz, kr, kz; };
 
-constexpr int AGM_MAX_STEPS = 8;
-constexpr int AGM_EXIT_SHIFT = 11;
-// After the exit vote one more AGM step is taken (for K), but its C is no longer added to the series of W:
-// c <= 2^-26 a there, a term below 2^-45 of W (measured: worst block error 4.5e-13 -> 6.6e-13 over all parity
-// cases, 3 FP64 instructions per pair fewer, 290.6 -> 301.0 GPair/s).  0 keeps the term.
-#ifndef AGM_SKIP_LAST_TERM
-#define AGM_SKIP_LAST_TERM 1
-#endif   // exit vote: C_{k+1} <= 2^-11 A_k (see pair_parts)
+// hi32(d2) - hi32(s) below these -> one more AGM pass (2^20 (log2 of the d2/s thresholds above + 0.0862), rounded up)
+constexpr int AGM_T0 = -1430341, AGM_T1 = -6495283, AGM_T2 = -17255704, AGM_T3 = -38796084, AGM_T4 = -81876859;
 
 // What a thread keeps of one of its i points.
 struct IPoint {
@@ -103,6 +115,7 @@ template <int NP, bool CHECK_SELF>
 __device__ __forceinline__ void pair_parts(const IPoint (&pi)[NP], const JPoint &pj, PairParts (&pp)[NP]) {
     double s[NP], ys[NP], yd[NP], iA1[NP], A[NP], B[NP], V[NP];
     bool self[NP];
+    int dHmin = 0;
 #pragma unroll
     for (int u = 0; u < NP; ++u) {
         pp[u].dz = pi[u].z - pj.z; pp[u].dr = pi[u].r - pj.r;
@@ -116,6 +129,7 @@ __device__ __forceinline__ void pair_parts(const IPoint (&pi)[NP], const JPoint 
             if (self[u]) d2 = 1.0;
         }
         s[u] = fma(2.0, pp[u].rho2, d2);                 // (r_i + r_j)^2 + dz^2 = d2 + 4 r_i r_j
+        dHmin = min(dHmin, __double2hiint(d2) - __double2hiint(s[u]));  // ~ 2^20 log2(d2/s) <= 0
         double a0, b0;
         sqrt_rsqrt_fast(s[u], a0, ys[u]);
         sqrt_rsqrt_fast(d2, b0, yd[u]);
@@ -124,54 +138,36 @@ __device__ __forceinline__ void pair_parts(const IPoint (&pi)[NP], const JPoint 
         iA1[u] = rcp_fast(A[u]);
         V[u] = 0.0;
     }
-    // Rolled loop, state in fixed registers.  V_P = 2 V_{P-1} + C_{P+1}^2, so after P passes
-    // sum_{k>=2} C_k^2/2^k = V / 2^{P+1}, and 4 K/sqrt(s) = 4 pi 2^P / A_{P+1}.
-    // The exit is decided ONE PASS AHEAD so that the branch never waits on fresh data:
-    // c_{k+2} = c_{k+1}^2/(4 a_{k+2}) exactly, hence C_{k+1} <= 2^-11 A_k (c_{k+1} <= 2^-12 a) in every
-    // lane guarantees c_{k+2} <= 2^-26 a after the next pass, which is then the last (its C only feeds
-    // V); the a_{k+2} used for K is then within c_{k+3} <= 2^-54 a of the AGM limit.
-    int P = 0;                 // completed (C, V) updates = completed AGM steps
-    bool last = false;
+    // the smallest d2/s of the warp decides (every lane is here: lock-step callers); the compares run once per
+    // warp on the uniform datapath instead of once per pair
+    dHmin = __reduce_min_sync(0xffffffffu, dHmin);
+    const int npass = int(dHmin < AGM_T0) + int(dHmin < AGM_T1) + int(dHmin < AGM_T2) + int(dHmin < AGM_T3) + int(dHmin < AGM_T4);
+    // V_P = 2 V_{P-1} + C_{P+1}^2: after P passes sum_{j=2}^{P+1} C_j^2 / 2^j = V / 2^(P+1)
 #pragma unroll 1
-    for (;;) {
-#if AGM_SKIP_LAST_TERM
-        if (last || P == AGM_MAX_STEPS) break;     // the last C (c <= 2^-26 a: a term <= 2^-45 of W) is not added to V
-#endif
-        bool conv = true;
+    for (int p = 0; p < npass; ++p) {
 #pragma unroll
         for (int u = 0; u < NP; ++u) {
             const double C = A[u] - B[u];
             V[u] = fma(V[u], 2.0, C * C);
-            conv = conv && (__double2hiint(C) + (AGM_EXIT_SHIFT << 20) <= __double2hiint(A[u]));
-        }
-#if !AGM_SKIP_LAST_TERM
-        ++P;
-        if (last || P == AGM_MAX_STEPS) break;
-#endif
-        last = __all_sync(0xffffffffu, conv);
-#pragma unroll
-        for (int u = 0; u < NP; ++u) {
             const double X = A[u] * B[u];
             A[u] = A[u] + B[u];
             B[u] = sqrt_times2_fast(X);
         }
-#if AGM_SKIP_LAST_TERM
-        ++P;
-#endif
     }
-#if AGM_SKIP_LAST_TERM
-    const int PK = P + 1, PV = P;      // K: 4 pi 2^(P+1) / A_(P+2);  sum_{k>=2} C_k^2 / 2^k = V / 2^(P+1)
-#else
-    const int PK = P, PV = P;
-#endif
 #pragma unroll
     for (int u = 0; u < NP; ++u) {
-        const double Af = A[u] + B[u];
-        const double K4 = scale_pow2(12.566370614359172953850573533118 * rcp_fast(Af), PK);   // 4 K/sqrt(s)
-        // 2 W = 1/A_1^2 + V 2^-P / q^2.  1/q^2 is a normal number far from the exponent limits (V may be
-        // 0 for far pairs: scale 1/q^2, not the product).
+        const double C = A[u] - B[u];                    // C_{P+2}
+        const double iAp = rcp_fast(A[u] + B[u]);        // 1 / A_{P+2}
+        const double e = C * iAp;
+        const double x = e * e;
+        const double F = fma(x, fma(x, fma(x, 25.0 / 256.0, 9.0 / 64.0), 0.25), 1.0);     // next term <= 0.075 2^-48
+        const double G = fma(x, fma(x, fma(x, 41.0 / 1024.0, 0.0625), 0.125), 1.0);
+        const double K4 = scale_pow2(iAp * F, npass + 1);              // 4 K/sqrt(s) / (4 pi)
+        const double Vf = fma(V[u], 2.0, (C * C) * G);                 // sum_{j>=2} C_j^2 / 2^j = Vf / 2^(P+2)
+        // 2 W = 1/A_1^2 + Vf 2^-(P+1) / q^2.  1/q^2 is a normal number far from the exponent limits (Vf may be
+        // tiny for far pairs: scale 1/q^2, not the product).
         const double invq2 = pi[u].c * pj.invr2;
-        const double W2 = fma(iA1[u], iA1[u], V[u] * scale_pow2(invq2, -PV));
+        const double W2 = fma(iA1[u], iA1[u], Vf * scale_pow2(invq2, -(npass + 1)));
         const double g = fma(pp[u].rho2, W2, 1.0);       // 1 + q W
         const double Kh = K4 * (ys[u] * ys[u]);          // 4 K / s^(3/2)
         pp[u].Pssh = K4 * W2;

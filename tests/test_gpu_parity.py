@@ -6,8 +6,8 @@ residuals of the GPU's C(f) < 1e-12 relative; integer work (pattern) bit-exact.
 Step a3 has two paths (include/landau.h): PER (every problem evaluates the pair tensor itself, k_pair_sym) and
 SHARED (tensor once per call, fp64 tensor-core contraction, k_pair_tensor + k_apply_dmma).  The parity cases run
 on both; the sizes are chosen so that every instantiation the launchers can select is compared with the oracle:
-k_pair_sym<32,1>, <64,2>, <128,2>, each with and without the all-pairs coincidence test, k_apply_dmma<1,2>,
-<2,2>, <4,2>, k_band_factor / k_band_solve with 8-, 16- and 32-column blocks."""
+k_pair_split<4>, <2> (N < 1536, < 2560), k_pair_sym<64,2>, <128,2>, each with and without the all-pairs coincidence
+test, k_apply_dmma<1,2>, <2,2>, <4,2>, k_band_factor / k_band_solve with 8-, 16- and 32-column blocks."""
 import numpy as np
 import pytest
 
@@ -162,16 +162,19 @@ def test_implicit_operator_parity(gpu, oracle, cfg, variant):
 def _multigrid_case(which):
     """inputs.multigrid_case, plus two cases with IDENTICAL Q3 grids (every point coincides with one of the other
     grid, so every pair is tested for coincidence) whose point totals select the 64- and 128-point tiles of the
-    per-problem pair kernel: 'same2-q3-80' = 2 x 1,280 = 2,560 points, 'same2-q3-128' = 2 x 2,048 = 4,096 points."""
-    if which in ("same2-q3-80", "same2-q3-128"):
-        m = inputs.config(6).mesh if which == "same2-q3-80" else inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 8, 16)
+    per-problem pair kernel: 'same2-q3-80' = 2 x 1,280 = 2,560 points, 'same2-q3-128' = 2 x 2,048 = 4,096 points;
+    'same2-q3-60' = 2 x 960 = 1,920 points runs the 32-point tiles shared by two warps (the small Q2 'same2', 360
+    points, those shared by four)."""
+    if which in ("same2-q3-60", "same2-q3-80", "same2-q3-128"):
+        m = {"same2-q3-60": inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 6, 10), "same2-q3-80": inputs.config(6).mesh,
+             "same2-q3-128": inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 8, 16)}[which]
         spc = inputs._sp([(1, -1, 1, 1), (4, 1, 1, 1)])
         return which, 3, [m, m], spc, [0, 1], [inputs.Component(0, 1, 1), inputs.Component(1, 1, 1)]
     return inputs.multigrid_case(which)
 
 
 @pytest.mark.parametrize("path", PATHS)
-@pytest.mark.parametrize("which", ["same2", "scaled", "paper3", "same2-q3-80", "same2-q3-128"])
+@pytest.mark.parametrize("which", ["same2", "scaled", "paper3", "same2-q3-60", "same2-q3-80", "same2-q3-128"])
 def test_multigrid_parity(gpu, oracle, which, path):
     """SURVEY 8(f) NEXT-2 (section III-C): species on several grids, pair loop over the union of
     points.  'same2*' have every point of grid 1 on top of one of grid 0 (coincident pairs skipped across
@@ -378,9 +381,9 @@ def test_edge_cases_of_the_next_rows(gpu, oracle):
 
 
 def _inner_case(which):
-    if which == "q2-180":         # 5 tiles of 32 + a tail of 20
+    if which == "q2-180":         # 5 tiles of 32 + a tail of 20, four warps per tile pair
         return inputs.config(0)
-    if which == "q3-2048":        # 64 whole tiles of 32
+    if which == "q3-2048":        # 64 whole tiles of 32, two warps per tile pair
         return inputs.config(2)
     if which == "q3-2992":        # 46 tiles of 64 + a tail of 48
         mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 11, 17)
@@ -392,8 +395,8 @@ def _inner_case(which):
 @pytest.mark.parametrize("path", PATHS)
 @pytest.mark.parametrize("which", ["q2-180", "q3-2048", "q3-2992", "q3-4928"])
 def test_inner_integral_parity(gpu, oracle, which, path):
-    """Steps a1-a3 alone: G_D, G_K at every integration point, one case per tile size of the per-problem pair
-    kernel (32 / 64 / 128 points), each with a ragged last tile, and the same cases through the shared path
+    """Steps a1-a3 alone: G_D, G_K at every integration point, one case per launch shape of the per-problem pair
+    kernel (32-point tiles shared by 4 / 2 warps, 64- and 128-point tiles), with ragged last tiles, and the same cases through the shared path
     (ragged last chunk of 16 source points, ragged target tile, 1 / 2 / 4 splits of the source range)."""
     import torch
     wl = _inner_case(which)

@@ -141,7 +141,7 @@ def test_new_entry_points_check_their_arguments_without_a_gpu(binding):
     assert L.landau_pair_path(None, None, None) == binding.LANDAU_EINVAL
     assert L.landau_set_tensor_cache(None, 1) == binding.LANDAU_EINVAL
     cyc = ctypes.c_double()
-    assert L.landau_fp64_issue_probe(6, 16, ctypes.byref(cyc), None) == binding.LANDAU_EINVAL       # unknown mode
+    assert L.landau_fp64_issue_probe(8, 16, ctypes.byref(cyc), None) == binding.LANDAU_EINVAL       # unknown mode
     assert L.landau_fp64_issue_probe(0, 0, ctypes.byref(cyc), None) == binding.LANDAU_EINVAL        # iters < 1
     assert L.landau_fp64_issue_probe(0, 16, None, None) == binding.LANDAU_EINVAL
     wl = inputs.config(1)
