@@ -45,7 +45,7 @@ WORKLOAD = "config5: 512 problems x (2 species e+D, Q3 quadtree mesh 3B: 308 cel
 FP64_LANES_PER_SM = 64      # DFMA lanes per SM per clock = 4 sub-partitions x one DMMA.8x8x4 (256 FMA) per 16 clocks
 APPLY_FLOP_PER_PAIR = 14.0  # k_apply_dmma: seven products per ordered pair and problem (landau_shared.cu)
 CSRC = os.path.join(ROOT, "paper_2104_10000_b200", "csrc")
-KERNEL_SOURCES = ["landau_kernels.cu", "landau_shared.cu", "landau_pair_math.cuh", "landau_launch.cuh", "landau_kernels.h"]
+KERNEL_SOURCES = ["landau_kernels.cu", "landau_shared.cu", "landau_pair_math.cuh", "landau_launch.cuh"]
 ROOFLINE_INPUTS = os.path.join(ROOT, "profiles", "r02_roofline_inputs.csv")
 
 # (key, inputs.config number, variant, problems of the batched run: >= 10 ms of pair work on the per-problem path)
@@ -69,9 +69,13 @@ def load_roofline_inputs():
         sha = kernel_source_sha()
         with open(ROOFLINE_INPUTS) as fh:
             for row in csv.DictReader(l for l in fh if not l.startswith("#")):
-                if row["source_sha"] == sha:
-                    out[(row["kernel"], row["workload"])] = {k: (float(v) if v not in ("", None) else None)
-                                                             for k, v in row.items() if k not in ("kernel", "workload", "source_sha", "instance")}
+                if row["source_sha"] == sha:      # several captures of one launch (counter pass, full set) are merged
+                    d = out.setdefault((row["kernel"], row["workload"]), {})
+                    for k, v in row.items():
+                        if k not in ("kernel", "workload", "source_sha", "instance") and v not in ("", None):
+                            d[k] = float(v)
+                        elif k not in ("kernel", "workload", "source_sha", "instance"):
+                            d.setdefault(k, None)
     except Exception:
         pass
     return out
@@ -269,7 +273,7 @@ def pair_sym_roof(rin, key, kname, pairs, ms, peak, probe, issue, mix_key=None):
 
 
 def pair_kernel_name(N):
-    return "k_pair_sym<128,2>" if N >= 4096 else ("k_pair_sym<64,2>" if N >= 2560 else "k_pair_sym<32,1>")
+    return "k_pair_sym<128,2>" if N >= 4096 else ("k_pair_sym<64,2>" if N >= 2560 else ("k_pair_split<2>" if N >= 1536 else "k_pair_split<4>"))
 
 
 def time_config(binding, inputs, torch, oracle, key, k, variant, nb_batched, rin, peaks, flush, with_cpu=True):
@@ -667,11 +671,11 @@ def summarise_ncu(paths, plan_file):
                 return float(v.replace(",", "")) * scale.get(units.get(col, ""), 1.0)
             except Exception:
                 return None
-        seq = {"k_pair_sym": [], "k_pair_tensor": [], "k_apply_dmma": []}
+        seq = {"k_pair_sym": [], "k_pair_tensor": [], "k_apply_dmma": []}      # k_pair_sym: also its small-N form k_pair_split
         rest = {}
         for r in rows:
             name = r["Kernel Name"]
-            hit = next((k for k in seq if k in name), None)
+            hit = next((k for k in seq if k in name), "k_pair_sym" if "k_pair_split" in name else None)
             if hit:
                 seq[hit].append(r)
             elif "landau::" in name or name.startswith("k_") or " k_" in name:
