@@ -475,13 +475,30 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
         g3[ks] = ir * w * G[3 * ds.Ntot + q];
         g4[ks] = iz * w * G[4 * ds.Ntot + q];
     }
-    for (int sp = 0; sp < ds.S; ++sp) {
-        // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in)
+    // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in).  The list of the node is
+    // the same for every species: its first four items are read once per cell, and the u of species sp + 1 is
+    // gathered while species sp is multiplied (the kernel is bound by the latency of these dependent loads).
+    int lt0 = 0, lt1 = 0, ld[4] = {0, 0, 0, 0};
+    double lwv[4] = {0.0, 0.0, 0.0, 0.0};
+    if (lane < 16) {
+        lt0 = ds.lptr[e * 16 + lane]; lt1 = ds.lptr[e * 16 + lane + 1];
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (lt0 + q < lt1) { ld[q] = ds.ldof[lt0 + q]; lwv[q] = ds.lw[lt0 + q]; }
+    }
+    auto gather_u = [&](int sp) {
         double u = 0.0;
-        if (lane < 16) {
-            const double *fa = f + (size_t)b * ds.fstride + (size_t)sp * ds.n;
-            for (int t = ds.lptr[e * 16 + lane]; t < ds.lptr[e * 16 + lane + 1]; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
-        }
+        const double *fa = f + (size_t)b * ds.fstride + (size_t)sp * ds.n;
+#pragma unroll
+        for (int q = 0; q < 4; ++q)
+            if (lt0 + q < lt1) u = fma(lwv[q], fa[ld[q]], u);
+        for (int t = lt0 + 4; t < lt1; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
+        return u;
+    };
+    double u_next = gather_u(0);
+    for (int sp = 0; sp < ds.S; ++sp) {
+        const double u = u_next;
+        if (sp + 1 < ds.S) u_next = gather_u(sp + 1);
         const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
         double acc[2][2][2] = {};       // [mt][nt][2]
         double accM[2][2][2] = {};      // mass part (FULL), kept apart: the element vector excludes it
