@@ -105,6 +105,8 @@ struct landau_ctx {
     int64_t launches = 0;
     cudaStream_t own_stream = nullptr, copy_stream = nullptr;
     cudaEvent_t chunk_done = nullptr;
+    cudaStream_t side_stream = nullptr;              // batch-shared path: the tensor evaluation runs beside a1 + a2
+    cudaEvent_t side_fork = nullptr, side_join = nullptr;
     double *d_f = nullptr, *d_vals = nullptr, *d_Cf = nullptr;  // landau_jacobian_host staging
     int host_nb = 0;
     bool profiling = false;
@@ -140,8 +142,29 @@ int timed(landau_ctx *ctx, int kind, cudaStream_t st, F &&go) {
 void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, cudaStream_t st, bool reuse_tensor = false) {
     const int N = int(ctx->Ntot);
     if (ctx->pair_path == LANDAU_PAIR_SHARED) {
+        const bool eval_tensor = !(reuse_tensor || (ctx->tensor_cache && ctx->tensor_valid));
+        // The tensor depends on the geometry only and a1 + a2 on f only: for a large batch the two run side by side
+        // (fork / join through events, legal under stream capture too); k_fields_beta is latency-bound and leaves
+        // the FP64 pipes and the memory system to k_pair_tensor.
+        bool forked = false;
+        if (eval_tensor && nb > PDL_MAX_NB) {
+            if (!ctx->side_stream) {
+                cudaError_t e = cudaStreamCreateWithFlags(&ctx->side_stream, cudaStreamNonBlocking);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->side_fork, cudaEventDisableTiming);
+                if (e == cudaSuccess) e = cudaEventCreateWithFlags(&ctx->side_join, cudaEventDisableTiming);
+                if (e != cudaSuccess) { note_launch_error(e); return; }
+            }
+            note_launch_error(cudaEventRecord(ctx->side_fork, st));          // after every earlier user of U on st
+            note_launch_error(cudaStreamWaitEvent(ctx->side_stream, ctx->side_fork, 0));
+            cudaStream_t ss = ctx->side_stream;
+            ctx->launches += timed(ctx, 0, ss, [&]() { return launch_pair_tensor(N, ctx->r, ctx->z, ctx->invr, ctx->sc.U, ss); });
+            note_launch_error(cudaEventRecord(ctx->side_join, ss));
+            ctx->tensor_valid = true;
+            forked = true;
+        }
         for (auto &g : ctx->grids) ctx->launches += launch_fields_beta_tiled(g.ds, nb, ctx->nbpad, f_dev + g.foff, ctx->sc.T, st);
-        if (!(reuse_tensor || (ctx->tensor_cache && ctx->tensor_valid))) {
+        if (forked) note_launch_error(cudaStreamWaitEvent(st, ctx->side_join, 0));
+        else if (eval_tensor) {
             ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair_tensor(N, ctx->r, ctx->z, ctx->invr, ctx->sc.U, st); });
             ctx->tensor_valid = true;
         }
@@ -265,6 +288,9 @@ int landau_destroy(landau_ctx *ctx) {
     if (ctx->own_stream) cudaStreamDestroy(ctx->own_stream);
     if (ctx->copy_stream) cudaStreamDestroy(ctx->copy_stream);
     if (ctx->chunk_done) cudaEventDestroy(ctx->chunk_done);
+    if (ctx->side_stream) cudaStreamDestroy(ctx->side_stream);
+    if (ctx->side_fork) cudaEventDestroy(ctx->side_fork);
+    if (ctx->side_join) cudaEventDestroy(ctx->side_join);
     for (auto &ev : ctx->prof_events) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     for (auto &ev : ctx->prof_pool) { cudaEventDestroy(ev.a); cudaEventDestroy(ev.b); }
     delete ctx;
