@@ -185,14 +185,17 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
                                      double shift, double *vals_dev, double *F_dev, void *stream);
 
 /* Per-species batched band LU (section III-G): reverse Cuthill-McKee ordering of the
- * pattern (computed in landau_create), band storage, Gaussian elimination WITHOUT pivoting in outer-product
+ * pattern (computed in landau_create; RCM's result depends on its starting node, so it is run from a
+ * pseudo-peripheral node, from the unknowns at the corners of the domain and from the one nearest the origin,
+ * the plain (z, r) sweep is a candidate too, and among the orders within 10 % of the narrowest band the one with
+ * the least envelope work is kept), band storage, Gaussian elimination WITHOUT pivoting in outer-product
  * form (Golub & Van Loan Alg. 4.3.1, the paper's algorithm; blocked), one independent matrix per (problem,
  * species).  Meant for the matrices of landau_implicit_operator_batched (shift M + A - J); like the paper's
  * solver it does not pivot.  Breakdown is REPORTED, not repaired: pivots_dev (NULL, or [nb][S][2] device doubles)
  * receives for every matrix the smallest and the largest |pivot| met; a zero, NaN or infinite pivot gives
  * smallest = 0 (the factors and any solve with them are then meaningless), a tiny ratio smallest / largest
  * tells that elimination without pivoting was unstable for that matrix.
- * landau_band_sizes: per grid the half-bandwidth after RCM and the doubles one matrix occupies; the
+ * landau_band_sizes: per grid the half-bandwidth of the chosen order and the doubles one matrix occupies; the
  * doubles of workspace per problem (all species of all grids); and the flop of the outer-product updates of
  * one factorisation (they are confined to the envelope of the ordered pattern, which elimination without
  * pivoting does not leave: about half of 2 n bw^2 on the refined meshes).  band_dev: caller-owned workspace of
@@ -202,8 +205,10 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
  * landau_band_factor_batched: vals_dev [nb][vals_stride] (CSR values, layout of landau_jacobian_batched)
  *   -> factors in band_dev.
  * landau_band_solve_batched: rhs_dev, x_dev [nb][f_stride] (layout of f); x = A^-1 rhs per species block;
- *   x_dev may equal rhs_dev.  Both are asynchronous on `stream` and deterministic. */
-/* Host-only (no CUDA device needed): the RCM order landau_create computes for this mesh and order --
+ *   x_dev may equal rhs_dev.  Both are asynchronous on `stream` and deterministic.  The solve keeps the vector of a
+ *   matrix in shared memory up to n ~ 28,000 unknowns; beyond that it works in a ctx-owned device scratch of
+ *   max_batch * S * n doubles, allocated (synchronously) by the first such call. */
+/* Host-only (no CUDA device needed): the band order landau_create chooses for this mesh and order --
  * perm_host[n] (new index -> unknown), the half-bandwidth it gives, the block width the factorisation will
  * use and the flop of its outer-product updates inside the envelope.  Any output may be NULL. */
 int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_host, int32_t *half_bandwidth,

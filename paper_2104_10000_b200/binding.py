@@ -140,7 +140,7 @@ def landau_setup_host(mesh, order: int):
 
 
 def landau_band_order_host(mesh, order: int):
-    """Host-only: dict(perm, bw, block_columns, flop) of the band LU's RCM order for this mesh."""
+    """Host-only: dict(perm, bw, block_columns, flop) of the band LU's order (best RCM start or sweep) for this mesh."""
     L = lib()
     m, keep = _mesh_struct(mesh)
     n = landau_setup_host(mesh, order)["n"]
@@ -268,7 +268,7 @@ class LandauContext:
                                                       float(shift), pv, pf, _stream_ptr(stream)))
 
     def band_sizes(self, grid=0):
-        """(half-bandwidth after RCM, doubles per matrix, workspace doubles per problem)."""
+        """(half-bandwidth of the band order, doubles per matrix, workspace doubles per problem)."""
         bw, md, ws, fl = c_int32(), c_int64(), c_int64(), c_double()
         _check(lib().landau_band_sizes(self._h, grid, ctypes.byref(bw), ctypes.byref(md), ctypes.byref(ws), ctypes.byref(fl)))
         self.band_flop_per_factorization = fl.value

@@ -82,6 +82,7 @@ struct GridState {
     size_t boff = 0;         // offset (doubles) of this grid's matrices inside one problem's band workspace
     double *Ce = nullptr;    // [nb][S_g][Ne][Nb*Nb]
     double *ce = nullptr;    // [nb][S_g][Ne][Nb]
+    double *solve_x = nullptr;   // band solve: permuted vectors of orders too large for shared memory (lazy)
 };
 }  // namespace
 
@@ -392,7 +393,7 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         // band LU: RCM order, half-bandwidth, CSR entry -> band offset
         std::vector<int32_t> perm, bidx(hs.nnz);
         int bw = 0;
-        rcm_order(int(hs.n), hs.rowptr, hs.colidx, perm, bw);
+        rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
         std::vector<int32_t> pos(hs.n);
         for (int64_t i = 0; i < hs.n; ++i) pos[perm[i]] = int32_t(i);
         const int64_t Wb = (bw + band_block(bw) + 1) & ~1, LD = 2 * Wb + 1;   // even half-width (band_halfwidth in landau_band.cu)
@@ -403,28 +404,12 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
                 bidx[t] = int32_t((Wb + ni - nj) + nj * LD);
             }
         G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = (size_t(LD) * hs.n + 1) & ~size_t(1);   // even: every matrix starts 16-byte aligned
-        // envelope of the permuted pattern: elimination without pivoting creates no fill left of a row's first
-        // entry / above a column's first entry, so block step s only reaches mlow[s] rows below and mup[s] rows
-        // above its block (<= bw; about half the uniform-band work on the refined meshes)
+        // envelope of the permuted pattern: block step s only reaches mlow[s] rows below and mup[s] rows above its
+        // block (<= bw; about half the uniform-band work on the refined meshes)
         {
-            const int KBs = band_block(bw), nsteps = (int(hs.n) + KBs - 1) / KBs;
-            std::vector<int32_t> first(hs.n), last_with_first(hs.n + 1, 0), mlow(nsteps), mup(nsteps);
-            for (int64_t i = 0; i < hs.n; ++i) first[i] = int32_t(i);
-            for (int64_t i = 0; i < hs.n; ++i)
-                for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t)
-                    first[pos[i]] = std::min(first[pos[i]], pos[hs.colidx[t]]);      // structurally symmetric: rows = columns
-            for (int64_t i = 0; i < hs.n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], int32_t(i));
-            for (int64_t j = 1; j < hs.n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
-            double work = 0.0;
-            for (int st = 0; st < nsteps; ++st) {
-                const int k0 = st * KBs, ke = std::min<int>(k0 + KBs, int(hs.n)) - 1;
-                mlow[st] = std::max(0, last_with_first[ke] - ke);
-                int fmin = k0;
-                for (int j = k0; j <= ke; ++j) fmin = std::min(fmin, int(first[j]));
-                mup[st] = k0 - fmin;
-                work += 2.0 * (ke - k0 + 1) * double(mlow[st]) * double(mlow[st]);
-            }
-            G.bs.flop_per_matrix = work;
+            std::vector<int32_t> mlow, mup;
+            int bw2 = 0;
+            G.bs.flop_per_matrix = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow, &mup);
             UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
         }
         UPC(G.bs.bidx, bidx) UPC(G.bs.perm, perm)
@@ -529,25 +514,13 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
     if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
     std::vector<int32_t> perm;
     int bw = 0;
-    rcm_order(int(hs.n), hs.rowptr, hs.colidx, perm, bw);
+    rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
     if (perm_host) std::memcpy(perm_host, perm.data(), perm.size() * sizeof(int32_t));
     if (half_bandwidth) *half_bandwidth = bw;
-    const int KBs = band_block(bw);
-    if (block_columns) *block_columns = KBs;
+    if (block_columns) *block_columns = band_block(bw);
     if (flop_per_factorization) {      // the envelope work of landau_create, recomputed from the order
-        std::vector<int32_t> pos(hs.n), first(hs.n), last_with_first(hs.n + 1, 0);
-        for (int64_t i = 0; i < hs.n; ++i) { pos[perm[i]] = int32_t(i); first[i] = int32_t(i); }
-        for (int64_t i = 0; i < hs.n; ++i)
-            for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) first[pos[i]] = std::min(first[pos[i]], pos[hs.colidx[t]]);
-        for (int64_t i = 0; i < hs.n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], int32_t(i));
-        for (int64_t j = 1; j < hs.n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
-        double work = 0.0;
-        for (int k0 = 0; k0 < int(hs.n); k0 += KBs) {
-            const int ke = std::min<int>(k0 + KBs, int(hs.n)) - 1;
-            const double m = std::max(0, last_with_first[ke] - ke);
-            work += 2.0 * (ke - k0 + 1) * m * m;
-        }
-        *flop_per_factorization = work;
+        int bw2 = 0;
+        *flop_per_factorization = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr);
     }
     return int(LANDAU_OK);
     });
@@ -764,13 +737,27 @@ int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, 
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev, void *stream) {
     if (!ctx || !band_dev || !rhs_dev || !x_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
+    return guarded([&]() {
     for (auto &g : ctx->grids) {
-        if ((size_t(g.bs.n) + 33 * 32) * sizeof(double) > 227 * 1024) return LANDAU_EINVAL;
+        // the permuted vector of a matrix is kept in shared memory when it fits (n up to ~28,000), else in a
+        // ctx-owned global scratch allocated at the first such call (max_batch * S_g * n doubles)
+        double *xg = nullptr;
+        if (band_solve_smem(g.bs.n, g.bs.bw) > 227 * 1024) {
+            if (!g.solve_x) {
+                void *d = nullptr;
+                cudaError_t e = cudaMalloc(&d, size_t(ctx->max_batch) * g.ds.S * g.bs.n * sizeof(double));
+                if (e != cudaSuccess) { cudaGetLastError(); g_cuda_err = std::string("cudaMalloc(band solve scratch): ") + cudaGetErrorString(e); return int(e == cudaErrorMemoryAllocation ? LANDAU_ENOMEM : LANDAU_ECUDA); }
+                ctx->owned.push_back(d);
+                g.solve_x = static_cast<double *>(d);
+            }
+            xg = g.solve_x;
+        }
         const double *band = band_dev + g.boff;
-        CK(launch_band_solve(g.bs, nb, g.ds.S, ctx->fstride, ctx->bstride, band, rhs_dev + g.foff, x_dev + g.foff, st));
+        CK(launch_band_solve(g.bs, nb, g.ds.S, ctx->fstride, ctx->bstride, band, rhs_dev + g.foff, x_dev + g.foff, xg, st));
         ctx->launches += 1;
     }
     return launches_ok();
+    });
 }
 
 int landau_launch_count(const landau_ctx *ctx, int64_t *count) {

@@ -44,27 +44,32 @@ int bfs_levels(int root, const std::vector<int32_t> &rowptr, const std::vector<i
 }
 }  // namespace
 
-// perm[new] = old, bw = max |new(i) - new(j)| over the pattern's entries
-void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw) {
+namespace {
+// Reverse Cuthill-McKee.  forced_root >= 0: its component is numbered first, starting there; every other component
+// starts at a pseudo-peripheral node (George & Liu).  perm[new] = old.
+void rcm_from(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, int forced_root, std::vector<int32_t> &perm) {
     std::vector<int> deg(n), level(n, -1), order, visited(n, 0);
     for (int i = 0; i < n; ++i) deg[i] = rowptr[i + 1] - rowptr[i];
     perm.clear();
     std::vector<int> cm;
-    for (int seed = 0; seed < n; ++seed) {
+    for (int pass = forced_root >= 0 ? -1 : 0; pass < n; ++pass) {
+        const int seed = pass < 0 ? forced_root : pass;
         if (visited[seed]) continue;
-        // pseudo-peripheral node of this component (George & Liu): repeat BFS from a minimum-degree node of the last level
         int root = seed;
-        std::fill(level.begin(), level.end(), -1);
-        int ecc = bfs_levels(root, rowptr, colidx, level, order);
-        for (int it = 0; it < 8; ++it) {
-            int cand = -1;
-            for (int v : order)
-                if (level[v] == ecc && (cand < 0 || deg[v] < deg[cand])) cand = v;
-            for (int v : order) level[v] = -1;
-            std::vector<int> order2;
-            const int ecc2 = bfs_levels(cand, rowptr, colidx, level, order2);
-            if (ecc2 > ecc) { root = cand; ecc = ecc2; order.swap(order2); }
-            else { for (int v : order2) level[v] = -1; bfs_levels(root, rowptr, colidx, level, order); break; }
+        if (pass >= 0) {
+            // pseudo-peripheral node of this component: repeat BFS from a minimum-degree node of the last level
+            std::fill(level.begin(), level.end(), -1);
+            int ecc = bfs_levels(root, rowptr, colidx, level, order);
+            for (int it = 0; it < 8; ++it) {
+                int cand = -1;
+                for (int v : order)
+                    if (level[v] == ecc && (cand < 0 || deg[v] < deg[cand])) cand = v;
+                for (int v : order) level[v] = -1;
+                std::vector<int> order2;
+                const int ecc2 = bfs_levels(cand, rowptr, colidx, level, order2);
+                if (ecc2 > ecc) { root = cand; ecc = ecc2; order.swap(order2); }
+                else { for (int v : order2) level[v] = -1; bfs_levels(root, rowptr, colidx, level, order); break; }
+            }
         }
         // Cuthill-McKee: BFS from root, neighbours in order of increasing degree
         std::vector<int> q;
@@ -81,11 +86,94 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
         cm.insert(cm.end(), q.begin(), q.end());
     }
     perm.assign(cm.rbegin(), cm.rend());   // reverse
-    std::vector<int> pos(n);
-    for (int i = 0; i < n; ++i) pos[perm[i]] = i;
+}
+}  // namespace
+
+// Half-bandwidth of an order and, per block step of KB = band_block(bw) columns, the rows below / columns right of the
+// block that elimination without pivoting can reach (mlow) and the rows above it (mup): no fill is created left of
+// a row's first entry / above a column's first entry, so the reach is the monotone hull of the envelope.
+// Returns the window-update work of one factorisation, 2 KB sum mlow^2 flop.
+double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int &bw, std::vector<int32_t> *mlow_out, std::vector<int32_t> *mup_out) {
+    std::vector<int32_t> pos(n), first(n), last_with_first(n + 1, 0);
+    for (int i = 0; i < n; ++i) { pos[perm[i]] = i; first[i] = i; }
     bw = 0;
     for (int i = 0; i < n; ++i)
-        for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) bw = std::max(bw, std::abs(pos[i] - pos[colidx[t]]));
+        for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) {
+            const int pi = pos[i], pj = pos[colidx[t]];
+            bw = std::max(bw, std::abs(pi - pj));
+            first[pi] = std::min<int32_t>(first[pi], pj);              // structurally symmetric: rows = columns
+        }
+    for (int i = 0; i < n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], i);
+    for (int j = 1; j < n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
+    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB;
+    if (mlow_out) mlow_out->assign(nsteps, 0);
+    if (mup_out) mup_out->assign(nsteps, 0);
+    double work = 0.0;
+    for (int st = 0; st < nsteps; ++st) {
+        const int k0 = st * KB, ke = std::min(k0 + KB, n) - 1;
+        const int m = std::max(0, last_with_first[ke] - ke);
+        int fmin = k0;
+        for (int j = k0; j <= ke; ++j) fmin = std::min(fmin, int(first[j]));
+        if (mlow_out) (*mlow_out)[st] = m;
+        if (mup_out) (*mup_out)[st] = k0 - fmin;
+        work += 2.0 * (ke - k0 + 1) * double(m) * double(m);
+    }
+    return work;
+}
+
+// The order of the band LU (section III-G: reverse Cuthill-McKee).  RCM's result depends on its starting
+// node, and on the high-order elements of this discretisation (every cell a clique of 16 or 9 unknowns) a
+// pseudo-peripheral start is often not the best one; the cost of the factorisation is the envelope work above, which
+// is cheap to evaluate.  So several candidates are tried (selection rule at the end of the function):
+//   RCM from a pseudo-peripheral node, from the unknowns at the four corners of the domain and from the one nearest
+//   the origin (where the refinement sits), and the plain sweep (z, then r) -- the optimum on uniform meshes, where
+//   the BFS levels of RCM are L-shaped rings of cells and twice as long as a row of the mesh.
+// dof_r / dof_z may be null (only the pseudo-peripheral RCM is then tried).  perm[new] = old.
+void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const double *dof_r, const double *dof_z,
+               std::vector<int32_t> &perm, int &bw) {
+    std::vector<int> roots = {-1};
+    std::vector<int32_t> sweep;
+    if (dof_r && dof_z && n > 0) {
+        double rmin = dof_r[0], rmax = dof_r[0], zmin = dof_z[0], zmax = dof_z[0];
+        for (int i = 1; i < n; ++i) {
+            rmin = std::min(rmin, dof_r[i]); rmax = std::max(rmax, dof_r[i]);
+            zmin = std::min(zmin, dof_z[i]); zmax = std::max(zmax, dof_z[i]);
+        }
+        const double tr[5] = {rmin, rmax, rmin, rmax, 0.0}, tz[5] = {zmin, zmin, zmax, zmax, 0.0};
+        for (int c = 0; c < 5; ++c) {
+            int best = 0;
+            double bd = 1e300;
+            for (int i = 0; i < n; ++i) {
+                const double d = (dof_r[i] - tr[c]) * (dof_r[i] - tr[c]) + (dof_z[i] - tz[c]) * (dof_z[i] - tz[c]);
+                if (d < bd) { bd = d; best = i; }
+            }
+            if (std::find(roots.begin(), roots.end(), best) == roots.end()) roots.push_back(best);
+        }
+        sweep.resize(n);
+        for (int i = 0; i < n; ++i) sweep[i] = i;
+        std::stable_sort(sweep.begin(), sweep.end(), [&](int a, int b) { return dof_z[a] != dof_z[b] ? dof_z[a] < dof_z[b] : dof_r[a] < dof_r[b]; });
+    }
+    // The half-bandwidth fixes the storage, the shared-memory panels (blocks per SM) and the kernel configuration;
+    // the envelope work is what the window updates cost.  So: among the candidates within 10 % of the narrowest
+    // band, the one with the least work (measured on B200: always the fastest of the set).
+    struct Cand { std::vector<int32_t> perm; int bw; double work; };
+    std::vector<Cand> cands;
+    for (size_t c = 0; c < roots.size() + (sweep.empty() ? 0 : 1); ++c) {
+        Cand k;
+        if (c < roots.size()) rcm_from(n, rowptr, colidx, roots[c], k.perm);
+        else k.perm = sweep;
+        k.work = band_envelope(n, rowptr, colidx, k.perm, k.bw, nullptr, nullptr);
+        cands.push_back(std::move(k));
+    }
+    int bw_min = cands[0].bw;
+    for (const Cand &k : cands) bw_min = std::min(bw_min, k.bw);
+    const int bw_ok = bw_min + std::max(8, bw_min / 10);
+    const Cand *best = nullptr;
+    for (const Cand &k : cands)
+        if (k.bw <= bw_ok && (!best || k.work < best->work || (k.work == best->work && k.bw < best->bw))) best = &k;
+    perm = best->perm;
+    bw = best->bw;
 }
 
 // stored half-width: bw + KB rounded up to even (16-byte aligned column pairs in the window update)
@@ -322,15 +410,17 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
 // Blocks of KB columns (those of the factorisation): the diagonal block by warp 0 (lane = row), the panel
 // below / above, confined to the envelope, by one thread per row with KB independent loads.
 
-template <int KB, int NT>
+// XG: the permuted vector of a matrix lives in global memory (xg + matrix * n) instead of shared memory -- for
+// orders n beyond the 227 KB of an SM (n > ~28,000); the block barriers order those accesses just the same.
+template <int KB, int NT, bool XG>
 __global__ void __launch_bounds__(NT)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
              const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, size_t pstride, const double *__restrict__ band_all,
-             const double *rhs, double *xout) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
+             const double *rhs, double *xout, double *xg) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
     constexpr int SB = KB;            // same blocks as the factorisation: panels stay inside the stored band
     extern __shared__ double smem[];
-    double *x = smem;                 // [n]
-    double *sD = x + n;               // [SB][SB+1]
+    double *x = XG ? xg + (size_t)blockIdx.x * n : smem;    // [n]
+    double *sD = XG ? smem : smem + n;                      // [SB][SB+1]
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     const int mat = blockIdx.x;       // = b * S + sp
@@ -435,23 +525,35 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstr
     }
 }
 
+// bytes of shared memory the solve needs with the vector on chip
+size_t band_solve_smem(int n, int bw) {
+    const int KB = band_block(bw);
+    return sizeof(double) * ((size_t)n + (size_t)KB * (KB + 1));
+}
+
 template <int KB, int NT>
 static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
-                           double *x, cudaStream_t st) {
-    const size_t smem = sizeof(double) * ((size_t)bs.n + KB * (KB + 1));
-    cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+                           double *x, double *xg, cudaStream_t st) {
+    if (xg) {        // vector in global memory: only the diagonal block in shared memory
+        const size_t smem = sizeof(double) * KB * (KB + 1);
+        k_band_solve<KB, NT, true><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x, xg);
+        return cudaGetLastError();
+    }
+    const size_t smem = band_solve_smem(bs.n, bs.bw);
+    cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB, NT><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x);
+    k_band_solve<KB, NT, false><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x, nullptr);
     return cudaGetLastError();
 }
 
+// xg: nullptr (the vector of a matrix fits shared memory) or scratch of nb * S * n doubles
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
-                              double *x, cudaStream_t st) {
+                              double *x, double *xg, cudaStream_t st) {
     switch (band_block(bs.bw)) {
-        case 32: return solve_t<32, SOLVE_NT32>(bs, nb, S, xstride, pstride, band, rhs, x, st);
-        case 16: return bs.bw <= 256 ? solve_t<16, SOLVE_NT16>(bs, nb, S, xstride, pstride, band, rhs, x, st)
-                                     : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, st);
-        default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, st);
+        case 32: return solve_t<32, SOLVE_NT32>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st);
+        case 16: return bs.bw <= 256 ? solve_t<16, SOLVE_NT16>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st)
+                                     : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st);
+        default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st);
     }
 }
 

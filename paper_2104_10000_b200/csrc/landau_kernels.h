@@ -82,7 +82,12 @@ struct BandSpace {
     const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
-void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, std::vector<int32_t> &perm, int &bw);
+// order of the band LU: the cheapest (envelope work) of RCM from several starting nodes and the (z, r) sweep
+void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const double *dof_r, const double *dof_z,
+               std::vector<int32_t> &perm, int &bw);
+// half-bandwidth, per-block-step reach inside the envelope (mlow, mup; may be null) and window-update flop of an order
+double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int &bw, std::vector<int32_t> *mlow, std::vector<int32_t> *mup);
 int band_block(int bw);        // KB, a function of bw only
 size_t band_factor_smem(int bw);
 // band points at this grid's block of problem 0; matrix (problem b, species s) = band + b pstride + s mat_doubles
@@ -91,8 +96,10 @@ cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride,
                              cudaStream_t st);
 // pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
 cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st);
+// xg: nullptr, or scratch of nb * S * n doubles for the permuted vectors when band_solve_smem(n, bw) exceeds an SM
+size_t band_solve_smem(int n, int bw);
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
-                              double *x, cudaStream_t st);
+                              double *x, double *xg, cudaStream_t st);
 
 int pair_tile_size(int N);
 int pair_tiles(int N);

@@ -297,18 +297,20 @@ def test_one_implicit_step_through_the_whole_path_conserves(gpu):
 
 
 def test_band_lu_wide_band_uses_the_16_column_blocks(gpu):
-    """A 32 x 32 Q3 mesh (n = 9,409, half-bandwidth > 416): the panels no longer fit shared memory with 32-column
-    blocks, so the 16-column instantiation runs.  Reference: scipy's sparse direct solve of the same CSR matrix
-    (too large for the oracle's dense solve); tolerance through the residual."""
+    """A 46 x 46 Q3 mesh (n = 19,321; the best order is the row sweep, half-bandwidth 3 x 139 + 3 = 420 > 416): the
+    panels no longer fit shared memory with 32-column blocks, so the 16-column, 512-thread instantiation runs.
+    Reference: scipy's sparse direct solve of the same CSR matrix (too large for the oracle's dense solve);
+    tolerance through the residual."""
     import torch
     import scipy.sparse as sps
     import scipy.sparse.linalg as spla
-    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 32, 32)
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 46, 46)
     spc = inputs._sp([(1, -1, 1, 1)])
-    wl = inputs.Workload("q3-32x32", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 11)
+    wl = inputs.Workload("q3-46x46", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 11)
     ctx = gpu.LandauContext(mesh, 3, spc, 1)
     bw, md, ws = ctx.band_sizes()
-    assert 416 < bw <= 850 and ctx.n == 97 * 97, bw
+    assert 416 < bw <= 832 and ctx.n == 139 * 139, bw
+    assert gpu.landau_band_order_host(mesh, 3)["block_columns"] == 16
     r, z = ctx.dof_coords()
     fd = torch.from_numpy(inputs.nodal_f(wl, r, z)[None]).cuda()
     vals = torch.zeros((1, 1, ctx.nnz), dtype=torch.float64, device="cuda")
@@ -536,18 +538,18 @@ def test_edge_cases(gpu, oracle):
 
 
 def test_band_lu_widest_band_uses_the_8_column_blocks(gpu):
-    """A 47 x 47 Q3 mesh (n = 20,164, RCM half-bandwidth 843 > 832): the panels only fit shared memory with
-    8-column blocks, so k_band_factor<8,512> / k_band_solve<8,512> run.  Reference: scipy's sparse direct solve of
-    the same CSR matrix; the pivot report must show a healthy elimination."""
+    """A 92 x 92 Q3 mesh (n = 76,729, N = 135,424 points; half-bandwidth of the row sweep 3 x 277 + 3 = 834 > 832):
+    the panels only fit shared memory with 8-column blocks, so k_band_factor<8,512> / k_band_solve<8,512> run.
+    Reference: scipy's sparse direct solve of the same CSR matrix; the pivot report must show a healthy elimination."""
     import torch
     import scipy.sparse as sps
     import scipy.sparse.linalg as spla
-    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 47, 47)
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 92, 92)
     spc = inputs._sp([(1, -1, 1, 1)])
-    wl = inputs.Workload("q3-47x47", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 12)
+    wl = inputs.Workload("q3-92x92", 3, mesh, spc, [[inputs.Component(0, 1, 1)]], 1e-3, 12)
     ctx = gpu.LandauContext(mesh, 3, spc, 1)
     bw, md, ws = ctx.band_sizes()
-    assert bw > 832 and ctx.n == 142 * 142, bw
+    assert bw > 832 and ctx.n == 277 * 277, bw
     assert gpu.landau_band_order_host(mesh, 3)["block_columns"] == 8
     r, z = ctx.dof_coords()
     fd = torch.from_numpy(inputs.nodal_f(wl, r, z)[None]).cuda()
