@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <cmath>
 #include <cstdint>
 #include <queue>
 #include <vector>
@@ -126,9 +127,10 @@ double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vecto
 // node, and on the high-order elements of this discretisation (every cell a clique of 16 or 9 unknowns) a
 // pseudo-peripheral start is often not the best one; the cost of the factorisation is the envelope work above, which
 // is cheap to evaluate.  So several candidates are tried (selection rule at the end of the function):
-//   RCM from a pseudo-peripheral node, from the unknowns at the four corners of the domain and from the one nearest
-//   the origin (where the refinement sits), and the plain sweep (z, then r) -- the optimum on uniform meshes, where
-//   the BFS levels of RCM are L-shaped rings of cells and twice as long as a row of the mesh.
+//   RCM from a pseudo-peripheral node, from the unknowns at the four corners of the domain, from the one nearest the
+//   origin (where the refinement sits) and from up to ~100 unknowns spread along the boundary, and the plain sweep
+//   (z, then r) -- the optimum on uniform meshes, where the BFS levels of RCM are L-shaped rings of cells and twice
+//   as long as a row of the mesh.
 // dof_r / dof_z may be null (only the pseudo-peripheral RCM is then tried).  perm[new] = old.
 void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const double *dof_r, const double *dof_z,
                std::vector<int32_t> &perm, int &bw) {
@@ -149,6 +151,23 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
                 if (d < bd) { bd = d; best = i; }
             }
             if (std::find(roots.begin(), roots.end(), best) == roots.end()) roots.push_back(best);
+        }
+        // ... and from unknowns spread evenly along the boundary of the domain (on the refined meshes the best start is
+        // often an axis node near the refined region), as many as a budget of ~3e5 node visits allows
+        {
+            const double tol = 1e-12 * std::max(rmax - rmin, zmax - zmin), rc = 0.5 * (rmin + rmax), zc = 0.5 * (zmin + zmax);
+            std::vector<int> bnd;
+            for (int i = 0; i < n; ++i)
+                if (dof_r[i] - rmin <= tol || rmax - dof_r[i] <= tol || dof_z[i] - zmin <= tol || zmax - dof_z[i] <= tol) bnd.push_back(i);
+            std::sort(bnd.begin(), bnd.end(), [&](int a, int b) {
+                const double ta = std::atan2(dof_z[a] - zc, dof_r[a] - rc), tb = std::atan2(dof_z[b] - zc, dof_r[b] - rc);
+                return ta != tb ? ta < tb : a < b;
+            });
+            const int want = std::min<int>(int(bnd.size()), std::max(0, 300000 / n - int(roots.size())));
+            for (int c = 0; c < want; ++c) {
+                const int v = bnd[size_t(c) * bnd.size() / want];
+                if (std::find(roots.begin(), roots.end(), v) == roots.end()) roots.push_back(v);
+            }
         }
         sweep.resize(n);
         for (int i = 0; i < n; ++i) sweep[i] = i;
