@@ -226,14 +226,16 @@ def timed_steps(torch, fn, steps, flush=None, warmup=3):
 
 
 def a3_profile(ctx, torch, fn, reps):
-    """Device time per launch of the step-a3 kernels: (tensor evaluation ms, contraction ms) via landau_profile_*."""
+    """Device time per CALL of the step-a3 kernels: (tensor evaluation or per-problem pair kernel ms, contraction ms)
+    via landau_profile_* (a call of the per-problem path launches its pair kernel once per group of problems: the
+    launches of a call are added up)."""
     ctx.profile_enable(True); ctx.profile_read()
     for _ in range(reps):
         fn()
     torch.cuda.synchronize()
     ms, cnt = ctx.profile_read()
     ctx.profile_enable(False)
-    return [m / c if c else None for m, c in zip(ms, cnt)]
+    return [m / reps if c else None for m, c in zip(ms, cnt)]
 
 
 def fp64_roof(kind, kernel, flop_per_pair, pairs, ms, peak, probe, extra=None):
@@ -506,8 +508,8 @@ def run_ours(args):
         sm_max = clocks["sm_max_mhz"] or 1965.0
         sms = torch.cuda.get_device_properties(local_rank).multi_processor_count
         peaks = measure_peaks(binding, sms, sm_max)
-        tensor_ms = a3_ms[0] / a3_cnt[0] if a3_cnt[0] else None
-        apply_ms = a3_ms[1] / a3_cnt[1] if a3_cnt[1] else None
+        tensor_ms = a3_ms[0] / len(step_ms) if a3_cnt[0] else None      # per step (the per-problem path launches its
+        apply_ms = a3_ms[1] / len(step_ms) if a3_cnt[1] else None       # pair kernel once per group of problems)
         shared = path == binding.LANDAU_PAIR_SHARED
         if shared:
             c = rin.get(("k_apply_dmma", "cfg5:main")) or {}

@@ -102,7 +102,9 @@ typedef struct {
 /* Set-up, once per mesh: DOF numbering, constraint closure, CSR pattern, gather
  * lists, point arrays, tabulations; uploads them.  max_batch in [1, 65535] sizes the scratch arena for
  * landau_jacobian_batched and chooses the path through step a3 (LANDAU_PAIR_AUTO above).  Device scratch:
- *   per-problem path : max_batch * (3 + 5 ceil(N/TS)) * N doubles, TS = 128 / 64 / 32 by N  (3.9 GB for 512 x 4,928)
+ *   per-problem path : chunk * (3 + 5 ceil(N/TS)) * N doubles, TS = 128 / 64 / 32 by N; a batch is processed in groups
+ *                      of chunk = min(max_batch, 1 GB / (40 ceil(N/TS) N bytes)) >= 1 problems: at most ~1 GB whatever
+ *                      the batch (139 problems per group at N = 4,928)
  *   batch-shared path: 40 N^2 bytes for the tensor (0.97 GB at N = 4,928) + max_batch * 5 (1 + ksplit) N doubles
  * plus max_batch * S * Ne * Nb (Nb + 1) doubles of element matrices.  LANDAU_ENOMEM if it does not fit;
  * on failure *out is NULL. */

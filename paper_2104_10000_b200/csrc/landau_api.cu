@@ -99,6 +99,7 @@ struct landau_ctx {
     std::vector<void *> pair_owned;  // scratch of the current pair path (T, G, U): replaced by landau_set_pair_path
     int pair_path = LANDAU_PAIR_PER_PROBLEM;   // resolved path (never LANDAU_PAIR_AUTO)
     int nbpad = 0;                   // batch-shared path: problems padded to whole tiles
+    int pp_chunk = 1;                // per-problem path: problems per group (their slabs stay in L2)
     bool tensor_cache = false;       // keep U between calls (the geometry of a ctx never changes)
     bool tensor_valid = false;
     int max_batch = 1;
@@ -174,9 +175,16 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
         if (ksplit > 1) ctx->launches += launch_sum_partials(N, nb, ksplit, ctx->sc.G, Gsum, st);
         return;
     }
-    for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nb, f_dev + g.foff, ctx->sc.T, st);
-    ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->r, ctx->z, ctx->invr, ctx->check_all, nb, ctx->sc.T, ctx->sc.G, st); });
-    ctx->launches += launch_sum_partials(N, nb, pair_tiles(N), ctx->sc.G, Gsum, st);
+    // Per-problem path: a group of pp_chunk problems at a time, so that the per-source-tile slabs (ntiles * 5 N doubles
+    // per problem) do not grow with the batch (at most PP_SLAB_BYTES of scratch; groups are large enough that the
+    // last wave of a launch costs < 1 %).  Problems are independent: the grouping changes no value.
+    for (int b0 = 0; b0 < nb; b0 += ctx->pp_chunk) {
+        const int nbc = std::min(ctx->pp_chunk, nb - b0);
+        const double *fc = f_dev + size_t(b0) * ctx->fstride;
+        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nbc, fc + g.foff, ctx->sc.T, st);
+        ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->r, ctx->z, ctx->invr, ctx->check_all, nbc, ctx->sc.T, ctx->sc.G, st); });
+        ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N), ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
+    }
 }
 
 void free_pair_scratch(landau_ctx *ctx) {
@@ -186,11 +194,20 @@ void free_pair_scratch(landau_ctx *ctx) {
     ctx->tensor_valid = false;
 }
 
+// Problems per group on the per-problem path: as many as keep the group's slabs within PP_SLAB_BYTES, at least one.
+// (Groups small enough for the slabs to stay in L2, 32 MB, were measured: the partial last wave of every pair-kernel
+// launch then costs more than the DRAM round trip of the slabs saves.)
+constexpr size_t PP_SLAB_BYTES = size_t(1) << 30;
+int pp_chunk_size(int max_batch, int64_t N) {
+    const size_t per_problem = size_t(pair_tiles(int(N))) * 5 * size_t(N) * sizeof(double);
+    return int(std::max<size_t>(1, std::min<size_t>(size_t(max_batch), PP_SLAB_BYTES / std::max<size_t>(per_problem, 1))));
+}
+
 // Bytes of U, the tensor entries of all ordered pairs (batch-shared path).
 size_t tensor_bytes(int64_t N) { return size_t(5) * (shared_kpad(int(N)) / 8) * shared_mpad(int(N)) * 8 * sizeof(double); }
 
 // Scratch of the pair path (sized for max_batch):
-//   per problem : T [nb][3][N], G [nb][ntiles][5][N]   (the slabs grow like nb N^2 / TS: 3.9 GB for 512 x 4,928)
+//   per problem : T [chunk][3][N], G [chunk][ntiles][5][N] for a group of `chunk` problems (slabs of a group <= 1 GB)
 //   batch-shared: T [3][Kpad/8][nbpad][8], U [5][Kpad/8][Mpad][8] (5 N^2 doubles: 0.97 GB for N = 4,928, independent
 //                 of the batch), G [nb][ksplit][5][N]; T and U are zeroed once: their padding must stay zero
 int alloc_pair_scratch(landau_ctx *ctx, int path) {
@@ -205,7 +222,9 @@ int alloc_pair_scratch(landau_ctx *ctx, int path) {
                   {&ctx->sc.U, tensor_bytes(int64_t(N)) / sizeof(double), true},
                   {&ctx->sc.G, shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0, false}};
     } else {
-        allocs = {{&ctx->sc.T, nbm * 3 * N, false}, {&ctx->sc.G, nbm * pair_tiles(int(N)) * 5 * N, false}};
+        ctx->pp_chunk = pp_chunk_size(ctx->max_batch, int64_t(N));
+        const size_t nbc = size_t(ctx->pp_chunk);
+        allocs = {{&ctx->sc.T, nbc * 3 * N, false}, {&ctx->sc.G, nbc * pair_tiles(int(N)) * 5 * N, false}};
     }
     for (auto &a : allocs) {
         if (!a.n) continue;
@@ -472,7 +491,7 @@ int landau_pair_path(const landau_ctx *ctx, int32_t *path, int64_t *scratch_byte
             d = 3 * size_t(shared_kpad(int(N)) / 8) * ctx->nbpad * 8 + tensor_bytes(ctx->Ntot) / 8 +
                 (shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0);
         else
-            d = nbm * 3 * N + nbm * pair_tiles(int(N)) * 5 * N;
+            d = size_t(ctx->pp_chunk) * (3 * N + pair_tiles(int(N)) * 5 * N);
         *scratch_bytes = int64_t(d * sizeof(double));
     }
     return LANDAU_OK;
@@ -683,11 +702,12 @@ int landau_jacobian_host(landau_ctx *ctx, int nb, const double *f_host, double *
     // the body enqueues; whatever it returns, both streams are drained before the caller gets its buffers back
     // (an error half way must not leave device-to-host copies into the caller's memory in flight)
     auto body = [&]() -> int {
-        CK(cudaMemcpyAsync(ctx->d_f, f_host, size_t(nb) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
         const int nchunks = nb >= 64 ? 8 : (nb >= 8 ? 4 : 1);
         const int cb = (nb + nchunks - 1) / nchunks;
         for (int b0 = 0; b0 < nb; b0 += cb) {
             const int nbc = std::min(cb, nb - b0);
+            // inputs chunk by chunk as well: the first results leave for the host after 1/nchunks of the upload
+            CK(cudaMemcpyAsync(ctx->d_f + b0 * fsz, f_host + b0 * fsz, size_t(nbc) * fsz * sizeof(double), cudaMemcpyHostToDevice, st));
             // the tensor of the point pairs (batch-shared path) is evaluated by the first sub-batch only
             inner_integral(ctx, nbc, ctx->d_f + b0 * fsz, ctx->sc.Gsum, st, b0 > 0);
             assemble(ctx, nbc, ctx->d_f + b0 * fsz, nullptr, 0.0, vals_host ? ctx->d_vals + b0 * vsz : nullptr,

@@ -425,6 +425,9 @@ def test_config5_batched_full_size(gpu, oracle, path):
     problems = list(range(wl.nbatch))
     ctx, f, vals, Cf, mv = run_gpu(gpu, wl, problems, path=path)
     assert np.isfinite(vals).all() and np.isfinite(Cf).all()
+    # scratch of step a3 does not grow with the batch beyond ~1 GB on either path (per-problem: the batch goes
+    # through the pair kernel in groups of 139 problems, so this call is 139 + 139 + 139 + 95)
+    assert ctx.pair_path()[1] <= 1.6e9
     sp = oracle.build_space(wl.mesh, wl.order)
     for k in problems:
         assert conservation_residuals(sp.dof_r, sp.dof_z, wl.species.mass, Cf[k]) < 1e-12, k
