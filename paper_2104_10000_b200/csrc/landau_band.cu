@@ -283,7 +283,7 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 //       (mma.sync.m8n8k4, 32 x 32 warp tiles, fragments straight from the shared-memory panels).
 // Computed transposed (C^T = U^T (-L)^T) so that a lane's two accumulator entries are two consecutive
 // rows of one column of the column-major window.
-// Dynamic shared memory: sD[KB][KB+1], sDi[KB] (1/pivots), sL[KB][MWP], sU[KB][MWP]; MWP = bw rounded up to
+// Dynamic shared memory: 2 x (sD[KB][KB+1], sDi[KB] (1/pivots)), sDs[KB][KB], sL[KB][MWP], sU[KB][MWP]; MWP = bw rounded up to
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
@@ -291,7 +291,8 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
               double *__restrict__ band_all, double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
     constexpr int DSZ = KB * (KB + 1) + KB;  // one diagonal-block buffer: sD[KB][KB+1], sDi[KB]
-    double *sL = smem + 2 * DSZ;             // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
+    double *sDs = smem + 2 * DSZ;            // [KB][KB]: the current L11 \ U11 with 16-byte aligned rows (panel substitutions)
+    double *sL = sDs + KB * KB;              // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
     double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;        // LD - 1
@@ -304,6 +305,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
     // rest of the window, so the serial elimination is off the critical path (two buffers, swapped per step).
     int cur = 0;
     if (warp == 0) factor_diag_block<KB>(A, lda, 0, min(KB, n), smem, smem + KB * (KB + 1), lane, pmin, pmax);
+    __syncthreads();                         // phase (1) of the first step already reads the eliminated block
     for (int k0 = 0; k0 < n; k0 += KB) {
         const int kb = min(KB, n - k0);
         const int m = mlow[k0 / KB];         // rows below / columns right of the block inside the envelope (<= bw)
@@ -323,29 +325,46 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
                 for (int c = 0; c < KB; ++c) { sL[(size_t)c * MWP + i] = 0.0; sU[(size_t)c * MWP + i] = 0.0; }
             }
         }
+        for (int t = tid; t < KB * KB; t += NT) sDs[t] = sD[(t / KB) * (KB + 1) + t % KB];
         __syncthreads();
-        // (2) panels: thread i does row i of the L panel (x U11 = a) and column i of the U panel (L11 y = a);
-        //     its entries live in shared memory (-x in sL, y in sU), not in registers
+        // (2) panels: thread i does row i of the L panel (x U11 = a) and column i of the U panel (L11 y = a), two
+        //     independent substitution chains, interleaved.  The phase is bound by the warp-uniform loads of the
+        //     diagonal block, so both chains walk ROWS of it, two entries per 16-byte load: the L row right-looking
+        //     (x_c -= x_t U11[t][c] for c > t as soon as x_t is final), the U column left-looking
+        //     (y_t -= L11[t][cc] y_cc for cc < t).  Every sum runs in ascending index order.
         for (int i = tid; i < m; i += NT) {
-            // two independent substitution chains per thread, interleaved: x U11 = a (L row), L11 y = a (U column)
             double x[KB], y[KB];
             double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
             double *col = A + k0 + (size_t)(k0 + kb + i) * lda;
 #pragma unroll
             for (int c = 0; c < KB; ++c) { x[c] = sL[(size_t)c * MWP + i]; y[c] = sU[(size_t)c * MWP + i]; }
 #pragma unroll
-            for (int c = 0; c < KB; ++c) {
-                double v = x[c], w = y[c];
+            for (int t = 0; t < KB; ++t) {
+                const double *drow = sDs + t * KB;
+                x[t] *= sDi[t];
+                const double xt = -x[t];
+                if ((t + 1) < KB && ((t + 1) & 1)) x[t + 1] = fma(xt, drow[t + 1], x[t + 1]);
 #pragma unroll
-                for (int cc = 0; cc < c; ++cc) {
-                    v = fma(-x[cc], sD[cc * (KB + 1) + c], v);
-                    w = fma(-sD[c * (KB + 1) + cc], y[cc], w);
+                for (int c = (t + 2) & ~1; c < KB; c += 2) {
+                    const double2 u = *reinterpret_cast<const double2 *>(drow + c);
+                    x[c] = fma(xt, u.x, x[c]);
+                    x[c + 1] = fma(xt, u.y, x[c + 1]);
                 }
-                v *= sDi[c];
-                x[c] = v; y[c] = w;
-                if (c < kb) { row[(size_t)c * lda] = v; col[c] = w; }
-                sL[(size_t)c * MWP + i] = -v;
-                sU[(size_t)c * MWP + i] = w;
+                double w = y[t];
+#pragma unroll
+                for (int cc = 0; cc + 1 < t; cc += 2) {
+                    const double2 l = *reinterpret_cast<const double2 *>(drow + cc);
+                    w = fma(-l.x, y[cc], w);
+                    w = fma(-l.y, y[cc + 1], w);
+                }
+                if (t & 1) w = fma(-drow[t - 1], y[t - 1], w);
+                y[t] = w;
+            }
+#pragma unroll
+            for (int c = 0; c < KB; ++c) {
+                if (c < kb) { row[(size_t)c * lda] = x[c]; col[c] = y[c]; }
+                sL[(size_t)c * MWP + i] = -x[c];
+                sU[(size_t)c * MWP + i] = y[c];
             }
         }
         __syncthreads();
@@ -513,7 +532,7 @@ static int band_mw(int bw) { return ((std::max(bw, 1) + WT - 1) / WT) * WT + 4; 
 
 size_t band_factor_smem(int bw) {
     const int KB = band_block(bw);
-    return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + 2 * (size_t)KB * band_mw(bw));
+    return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + (size_t)KB * KB + 2 * (size_t)KB * band_mw(bw));
 }
 
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
