@@ -218,6 +218,10 @@ __global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, size
 }
 
 constexpr int BAND_THREADS = 512;
+#ifndef BAND16_MIN_BLOCKS
+#define BAND16_MIN_BLOCKS 3        // narrow-band instantiation (16 columns x 128 threads): three blocks per SM (168 registers); compiled
+                                   // for four (128 registers) it was measured slower (ten-species 80-cell: 14.5 against 14.3 ms)
+#endif
 // threads per matrix in the solves (measured: bw = 339: 384 threads 4.2 ms, 256: 4.8, 512: 5.8; bw = 178: 64 threads 2.5 ms,
 // 256: 3.9, 512: 7.6 -- the solves are latency-bound, small blocks leave room for more matrices per SM)
 constexpr int SOLVE_NT32 = 384, SOLVE_NT16 = 64;
@@ -286,7 +290,7 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 // Dynamic shared memory: 2 x (sD[KB][KB+1], sDi[KB] (1/pivots)), sDs[KB][KB], sL[KB][MWP], sU[KB][MWP]; MWP = bw rounded up to
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB, int NT>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, (KB == 16 && NT == 128) ? BAND16_MIN_BLOCKS : 1)
 k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S, const int32_t *__restrict__ mlow,
               double *__restrict__ band_all, double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
