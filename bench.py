@@ -612,12 +612,32 @@ def kernel_run(which):
     units (ordered pairs) per launch -- the summariser needs them to turn counters into per-pair figures.
       single : one single build (per-problem path) of every per_config entry, in CONFIGS order
       batched: the batched run of every per_config entry through the per-problem path, then the shared path
-      main   : config 5, shared path (one step), then per-problem path (one step)"""
+      main   : config 5, shared path (one step), then per-problem path (one step)
+      lu     : band LU (fill, factorisation, solve) of config 5's and the ten-species 80-cell problem's matrices"""
     import torch
     from paper_2104_10000_b200 import binding, inputs
     binding.lib()
     plan = []
-    if which == "main":
+    if which == "lu":
+        # SURVEY 8(f) NEXT-4: operator -> band fill -> factorisation -> one solve, for the 1,024 matrices of config 5 and the
+        # 5,120 of the ten-species 80-cell problem (the two workloads of next_rows.band_lu_config5 / newton_iteration_ctx80)
+        for tag, k in (("cfg5:lu", 5), ("ctx80:lu", 6)):
+            wl = inputs.config(k)
+            nb = 512
+            ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, nb)
+            Ez = torch.full((nb,), 0.3, dtype=torch.float64, device="cuda")
+            ctx.implicit_operator_batched(fd, Ez, 2.0, vals, Cf)
+            bw, md, ws = ctx.band_sizes()
+            band = torch.empty(nb * ws, dtype=torch.float64, device="cuda")
+            piv = torch.zeros((nb, ctx.S, 2), dtype=torch.float64, device="cuda")
+            ctx.band_factor_batched(vals, band, piv)
+            ctx.band_solve_batched(band, Cf, Cf)
+            torch.cuda.synchronize()
+            plan.append({"workload": tag, "matrices": nb * ctx.S, "n": ctx.n, "half_bandwidth": bw,
+                         "flop_per_factorization": ctx.band_flop_per_factorization})
+            ctx.destroy()
+            del fd, vals, Cf, band
+    elif which == "main":
         wl = inputs.config(5)
         for path, tag in ((binding.LANDAU_PAIR_SHARED, "cfg5:main"), (binding.LANDAU_PAIR_PER_PROBLEM, "cfg5:per_problem")):
             ctx, fd, vals, Cf = make_problem(binding, inputs, torch, wl, wl.nbatch, path)
@@ -701,7 +721,7 @@ def main():
     ap.add_argument("--steps", type=int, default=20)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
-    ap.add_argument("--kernel-run", default=None, choices=["single", "batched", "main"])
+    ap.add_argument("--kernel-run", default=None, choices=["single", "batched", "main", "lu"])
     ap.add_argument("--summarise-ncu", nargs="+", default=None, metavar="RAW.csv")
     ap.add_argument("--plan", default=None, help="file holding the JSON line --kernel-run printed (for --summarise-ncu)")
     args = ap.parse_args()

@@ -448,6 +448,39 @@ def test_config5_batched_full_size(gpu, oracle, path):
 
 
 @pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("cfg,variant,nb", [(1, "B", 8192), (2, "B", 512), (3, "A", 1024)])
+def test_per_config_batches_of_the_bench_at_full_size(gpu, oracle, cfg, variant, nb, path):
+    """The batched launches bench.py times for configs 1, 2 and 3A (`per_config[*].batched`: 8,192 / 512 / 1,024 problems,
+    both paths through step a3) at full size: every problem gets its own f (the config's f, each species scaled by
+    a problem-dependent factor), all outputs finite, conservation on a spread of problems, and sampled problems
+    against the oracle one by one."""
+    import torch
+    wl = inputs.config(cfg, variant=variant)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, nb, pair_path=path)
+    r, z = ctx.dof_coords()
+    f0 = inputs.nodal_f(wl, r, z)
+    S = wl.species.S
+    scale = 1.0 + 0.3 * np.sin(0.37 * np.arange(nb)[:, None] + 1.3 * np.arange(S)[None, :])       # [nb][S], in [0.7, 1.3]
+    f = f0[None] * scale[:, :, None]
+    fd = torch.from_numpy(f).cuda()
+    vals = torch.full((nb, ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+    Cf = torch.full((nb, ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+    ctx.jacobian_batched(fd, vals, Cf)
+    torch.cuda.synchronize()
+    assert bool(torch.isfinite(vals).all()) and bool(torch.isfinite(Cf).all())
+    sp = oracle.build_space(wl.mesh, wl.order)
+    Cf_h = Cf.cpu().numpy()
+    for k in range(0, nb, max(1, nb // 64)):
+        assert conservation_residuals(sp.dof_r, sp.dof_z, wl.species.mass, Cf_h[k]) < 1e-12, k
+    for k in (0, nb // 2 + 1, nb - 1):
+        _, ovals, oCf, _ = oracle.build_all(wl.mesh, wl.order, wl.species, f[k], 1.0)
+        vk = vals[k].cpu().numpy()
+        for a in range(S):
+            assert block_err(vk[a], ovals[a]) <= TOL, (k, a)
+            assert block_err(Cf_h[k, a], oCf[a]) <= TOL, (k, a)
+
+
+@pytest.mark.parametrize("path", PATHS)
 def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu, path):
     """Inside one path a problem's result does not depend on the batch it is built in: 24 problems in one call,
     again, one by one, and (other tile shapes of the shared path's contraction) in calls of 17 + 7."""
