@@ -366,7 +366,7 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
             }
 #pragma unroll
             for (int c = 0; c < KB; ++c) {
-                if (c < kb) { row[(size_t)c * lda] = x[c]; col[c] = y[c]; }
+                if (c < kb) { __stcs(row + (size_t)c * lda, x[c]); __stcs(col + c, y[c]); }     // final L / U entries: evict first, the L2 is for the windows
                 sL[(size_t)c * MWP + i] = -x[c];
                 sU[(size_t)c * MWP + i] = y[c];
             }
