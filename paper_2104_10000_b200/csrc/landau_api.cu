@@ -409,29 +409,24 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         UPC(ds.rowptr, hs.rowptr) UPC(ds.colidx, hs.colidx)
         UPC(ds.gptr, hs.gptr) UPC(ds.gidx, hs.gidx) UPC(ds.gw, hs.gw)
         UPC(ds.cptr, hs.cptr) UPC(ds.cidx, hs.cidx) UPC(ds.cw, hs.cw)
-        // band LU: RCM order, half-bandwidth, CSR entry -> band offset
-        std::vector<int32_t> perm, bidx(hs.nnz);
+        // band LU: order, half-bandwidth, envelope per block step, fill lists per band column
+        std::vector<int32_t> perm;
         int bw = 0;
         rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
-        std::vector<int32_t> pos(hs.n);
-        for (int64_t i = 0; i < hs.n; ++i) pos[perm[i]] = int32_t(i);
         const int64_t Wb = (bw + band_block(bw) + 1) & ~1, LD = 2 * Wb + 1;   // even half-width (band_halfwidth in landau_band.cu)
         if (LD * hs.n > (int64_t(1) << 31) - 1) return LANDAU_EINVAL;
-        for (int64_t i = 0; i < hs.n; ++i)
-            for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) {
-                const int64_t ni = pos[i], nj = pos[hs.colidx[t]];
-                bidx[t] = int32_t((Wb + ni - nj) + nj * LD);
-            }
         G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = (size_t(LD) * hs.n + 1) & ~size_t(1);   // even: every matrix starts 16-byte aligned
         // envelope of the permuted pattern: block step s only reaches mlow[s] rows below and mup[s] rows above its
         // block (<= bw; about half the uniform-band work on the refined meshes)
         {
-            std::vector<int32_t> mlow, mup;
+            std::vector<int32_t> mlow, mup, zlo, zcnt, fptr, fsrc, foff;
             int bw2 = 0;
             G.bs.flop_per_matrix = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow, &mup);
+            band_fill_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, mlow, mup, zlo, zcnt, fptr, fsrc, foff);
             UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
+            UPC(G.bs.zlo, zlo) UPC(G.bs.zcnt, zcnt) UPC(G.bs.fptr, fptr) UPC(G.bs.fsrc, fsrc) UPC(G.bs.foff, foff)
         }
-        UPC(G.bs.bidx, bidx) UPC(G.bs.perm, perm)
+        UPC(G.bs.perm, perm)
         G.boff = ctx->bstride;
         ctx->bstride += size_t(ds.S) * G.bs.mat_doubles;
     }

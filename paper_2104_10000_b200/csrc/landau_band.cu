@@ -207,14 +207,23 @@ int band_block(int bw) { return bw <= 256 ? 16 : (bw <= 384 ? 32 : (bw <= 832 ? 
 // ------------------------------------------------------------------------------------------------
 // device
 // ------------------------------------------------------------------------------------------------
-// scatter the CSR values into the (zeroed) band: band[m][bidx[k]] = vals[...][k]
-// grid = (ceil(nnz/256), S_g, nb); matrix (problem b, species s of this grid) starts at band + b pstride + s mat_doubles
-__global__ void k_band_scatter(int nnz, size_t vstride, size_t mat_doubles, size_t pstride, const int32_t *__restrict__ bidx,
-                               const double *__restrict__ vals, double *__restrict__ band) {
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= nnz) return;
-    const double v = vals[(size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz + k];
-    band[(size_t)blockIdx.z * pstride + (size_t)blockIdx.y * mat_doubles + bidx[k]] = v;
+// Band fill: zero fill and scatter of the CSR values in one pass, one warp per band column.  Only the rows of a column
+// that the factorisation and the solves can touch are written (the union of the block steps' squares, DESIGN.md 6.4:
+// about three quarters of the stored band); the rest of the workspace is never read and stays as the caller left it.
+// grid = (ceil(n / FILL_WARPS), S_g, nb); matrix (problem b, species s of this grid) starts at band + b pstride + s mat_doubles
+constexpr int FILL_WARPS = 8;
+__global__ void __launch_bounds__(32 * FILL_WARPS)
+k_band_fill(int n, int nnz, size_t LD, size_t vstride, size_t mat_doubles, size_t pstride, const int32_t *__restrict__ zlo,
+            const int32_t *__restrict__ zcnt, const int32_t *__restrict__ fptr, const int32_t *__restrict__ fsrc,
+            const int32_t *__restrict__ foff, const double *__restrict__ vals, double *__restrict__ band) {
+    const int lane = threadIdx.x & 31, pj = blockIdx.x * FILL_WARPS + (threadIdx.x >> 5);
+    if (pj >= n) return;
+    double *col = band + (size_t)blockIdx.z * pstride + (size_t)blockIdx.y * mat_doubles + (size_t)pj * LD;
+    const int z0 = zlo[pj], zc = zcnt[pj];
+    for (int r = lane; r < zc; r += 32) col[z0 + r] = 0.0;
+    __syncwarp();                                  // orders the zeros before the values of this column (same warp)
+    const double *v = vals + (size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz;
+    for (int t = fptr[pj] + lane; t < fptr[pj + 1]; t += 32) col[foff[t]] = v[fsrc[t]];
 }
 
 constexpr int BAND_THREADS = 512;
@@ -541,12 +550,44 @@ size_t band_factor_smem(int bw) {
 
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st) {
-    // this grid's S matrices of every problem: nb rows of S mat_doubles, pstride apart
-    cudaError_t e = cudaMemset2DAsync(band, pstride * sizeof(double), 0, (size_t)S * bs.mat_doubles * sizeof(double), nb, st);
-    if (e != cudaSuccess) return e;
-    dim3 grid((bs.nnz + 255) / 256, S, nb);
-    k_band_scatter<<<grid, 256, 0, st>>>(bs.nnz, vstride, bs.mat_doubles, pstride, bs.bidx, vals, band);
+    const int W = band_halfwidth(bs.bw, band_block(bs.bw));
+    dim3 grid((bs.n + FILL_WARPS - 1) / FILL_WARPS, S, nb);
+    k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
+                                                 bs.fsrc, bs.foff, vals, band);
     return cudaGetLastError();
+}
+
+// Host: the fill lists of BandSpace for an order (perm[new] = old, pos = its inverse) and its envelope (mlow, mup per
+// block step of KB columns).  Column j (new numbering, block step s_j) is touched in the rows of every square
+// [k0(s), E(s)]^2, E(s) = ke(s) + mlow[s], that contains it -- the diagonal block, panels and window of step s -- and
+// by the backward solve up to mup[s_j] rows above its block: rows k0(first s with E(s) >= j) ... E(s_j).
+void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int bw, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, std::vector<int32_t> &zlo,
+                     std::vector<int32_t> &zcnt, std::vector<int32_t> &fptr, std::vector<int32_t> &fsrc, std::vector<int32_t> &foff) {
+    const int KB = band_block(bw), W = band_halfwidth(bw, KB), nsteps = (n + KB - 1) / KB;
+    std::vector<int32_t> pos(n), E(nsteps);
+    for (int i = 0; i < n; ++i) pos[perm[i]] = i;
+    for (int s = 0; s < nsteps; ++s) E[s] = std::min(n - 1, std::min(s * KB + KB, n) - 1 + mlow[s]);
+    zlo.assign(n, 0); zcnt.assign(n, 0); fptr.assign(n + 1, 0);
+    fsrc.clear(); foff.clear();
+    int s0 = 0;
+    for (int j = 0; j < n; ++j) {
+        const int sj = j / KB;
+        while (E[s0] < j) ++s0;                                    // E is non-decreasing and E[sj] >= j
+        const int rs = std::min(s0 * KB, std::max(0, sj * KB - mup[sj])), re = E[sj];
+        zlo[j] = W + rs - j;
+        zcnt[j] = re - rs + 1;
+        const int jo = perm[j];
+        for (int t = rowptr[jo]; t < rowptr[jo + 1]; ++t) {        // structurally symmetric: rows of column jo = columns of row jo
+            const int io = colidx[t];
+            const int32_t *b = colidx.data() + rowptr[io], *e = colidx.data() + rowptr[io + 1];
+            const int32_t *hit = std::lower_bound(b, e, int32_t(jo));
+            if (hit == e || *hit != jo) continue;                  // (not symmetric here: no entry (io, jo))
+            fsrc.push_back(int32_t(hit - colidx.data()));
+            foff.push_back(int32_t(W + pos[io] - j));
+        }
+        fptr[j + 1] = int32_t(fsrc.size());
+    }
 }
 
 template <int KB, int NT>

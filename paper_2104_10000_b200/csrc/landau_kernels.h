@@ -77,8 +77,11 @@ int launch_issue_probe(int mode, int blocks, int threads, int iters, const doubl
 struct BandSpace {
     int n, nnz, bw;            // order, CSR entries, half-bandwidth after RCM
     size_t mat_doubles;        // (2 (bw + KB) + 1) * n doubles per matrix
-    const int32_t *bidx;       // [nnz] device: CSR entry -> offset in the matrix's band
     const int32_t *perm;       // [n] device: new -> old
+    // fill lists per band column (new numbering): the rows of the column inside the region the factorisation and the
+    // solves touch (zeroed: zlo = offset of the first one inside the column, zcnt of them), and the CSR entries of the
+    // column (fsrc = index into the species' CSR values, foff = offset inside the column), fptr[n + 1]
+    const int32_t *zlo, *zcnt, *fptr, *fsrc, *foff;
     const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
@@ -92,6 +95,9 @@ int band_block(int bw);        // KB, a function of bw only
 size_t band_factor_smem(int bw);
 // band points at this grid's block of problem 0; matrix (problem b, species s) = band + b pstride + s mat_doubles
 // (problem-major workspace: a solve may use a different nb than the factorisation)
+void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int bw, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, std::vector<int32_t> &zlo,
+                     std::vector<int32_t> &zcnt, std::vector<int32_t> &fptr, std::vector<int32_t> &fsrc, std::vector<int32_t> &foff);
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st);
 // pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
