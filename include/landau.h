@@ -217,6 +217,19 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
                            int32_t *block_columns, double *flop_per_factorization);
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
                       int64_t *workspace_doubles_per_problem, double *flop_per_factorization);
+/* Two kernels factor the band, with the same storage and the same L, U up to rounding order:
+ *   LANDAU_BAND_FRONT  gathers, per block step, only the rows / columns inside the ENVELOPE of the ordered pattern (LU
+ *                      without pivoting keeps it; on the refined meshes a third of the rows a band step spans) into a
+ *                      dense front in shared memory, eliminates there and scatters back;
+ *   LANDAU_BAND_HULL   updates the whole window of a block step in place (the monotone hull of the envelope).
+ * LANDAU_BAND_AUTO (the default) takes the front kernel whenever the largest front fits the shared memory of an SM.
+ * landau_band_set_method returns LANDAU_EINVAL for LANDAU_BAND_FRONT when it does not fit; landau_band_method reports
+ * the kernel in use for a grid and the longest active list (rows of the largest front beside its block). */
+#define LANDAU_BAND_AUTO 0
+#define LANDAU_BAND_HULL 1
+#define LANDAU_BAND_FRONT 2
+int landau_band_set_method(landau_ctx *ctx, int method);
+int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max);
 int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, double *pivots_dev,
                                void *stream);
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,

@@ -17,6 +17,7 @@ LIB_PATH = os.path.join(_HERE, "liblandau_b200.so")
 
 LANDAU_OK, LANDAU_EINVAL, LANDAU_ENOMEM, LANDAU_ECUDA = 0, -1, -2, -3
 LANDAU_PAIR_AUTO, LANDAU_PAIR_PER_PROBLEM, LANDAU_PAIR_SHARED = 0, 1, 2
+LANDAU_BAND_AUTO, LANDAU_BAND_HULL, LANDAU_BAND_FRONT = 0, 1, 2
 LANDAU_SHARED_MIN_BATCH = 4
 
 
@@ -63,6 +64,8 @@ SIGNATURES = {
     "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
     "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "landau_band_set_method": (c_int, [c_void_p, c_int]),
+    "landau_band_method": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32)]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "landau_profile_enable": (c_int, [c_void_p, c_int]),
@@ -273,6 +276,16 @@ class LandauContext:
         _check(lib().landau_band_sizes(self._h, grid, ctypes.byref(bw), ctypes.byref(md), ctypes.byref(ws), ctypes.byref(fl)))
         self.band_flop_per_factorization = fl.value
         return bw.value, md.value, ws.value
+
+    def band_set_method(self, method):
+        """LANDAU_BAND_AUTO / _HULL / _FRONT: which kernel factors the band (include/landau.h)."""
+        _check(lib().landau_band_set_method(self._h, int(method)))
+
+    def band_method(self, grid=0):
+        """(kernel in use for the grid: LANDAU_BAND_HULL or _FRONT, rows of the largest front beside its block)."""
+        m, r = c_int32(), c_int32()
+        _check(lib().landau_band_method(self._h, grid, ctypes.byref(m), ctypes.byref(r)))
+        return m.value, r.value
 
     def band_factor_batched(self, vals, band, pivots=None, stream=None):
         """pivots: None or a CUDA float64 tensor [nb][S][2] receiving (min |pivot|, max |pivot|) per matrix."""

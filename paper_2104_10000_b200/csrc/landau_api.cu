@@ -83,6 +83,7 @@ struct GridState {
     double *Ce = nullptr;    // [nb][S_g][Ne][Nb*Nb]
     double *ce = nullptr;    // [nb][S_g][Ne][Nb]
     double *solve_x = nullptr;   // band solve: permuted vectors of orders too large for shared memory (lazy)
+    bool front_fits = false;     // the fronts of the envelope factorisation fit shared memory
 };
 }  // namespace
 
@@ -253,6 +254,8 @@ int resolve_pair_path(const landau_ctx *ctx, int path) {
     return tensor_bytes(ctx->Ntot) <= free_b / 4 ? LANDAU_PAIR_SHARED : LANDAU_PAIR_PER_PROBLEM;
 }
 
+constexpr double FRONT_MAX_WORK_RATIO = 0.5;     // LANDAU_BAND_AUTO: front kernel when its flops are at most half the hull's
+
 // Small batches are launch-latency bound: both gathers then go in one launch (3-7 us per single build); large
 // batches keep the two launches (the merged kernel is 10 % slower there).
 constexpr int MERGED_GATHER_MAX_NB = 8;
@@ -413,7 +416,7 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         std::vector<int32_t> perm;
         int bw = 0;
         rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
-        const int64_t Wb = (bw + band_block(bw) + 1) & ~1, LD = 2 * Wb + 1;   // even half-width (band_halfwidth in landau_band.cu)
+        const int64_t Wb = band_stored_halfwidth(bw), LD = 2 * Wb + 1;
         if (LD * hs.n > (int64_t(1) << 31) - 1) return LANDAU_EINVAL;
         G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = (size_t(LD) * hs.n + 1) & ~size_t(1);   // even: every matrix starts 16-byte aligned
         // envelope of the permuted pattern: block step s only reaches mlow[s] rows below and mup[s] rows above its
@@ -425,6 +428,14 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             band_fill_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, mlow, mup, zlo, zcnt, fptr, fsrc, foff);
             UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
             UPC(G.bs.zlo, zlo) UPC(G.bs.zcnt, zcnt) UPC(G.bs.fptr, fptr) UPC(G.bs.fsrc, fsrc) UPC(G.bs.foff, foff)
+            std::vector<int32_t> act_ptr, act_idx;
+            G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &G.bs.front_flop);
+            if (act_idx.empty()) act_idx.push_back(0);
+            UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
+            G.front_fits = band_front_smem(bw, G.bs.na_max) <= size_t(225) * 1024 && G.bs.na_max <= 160;   // + 1 KB the driver reserves per block; FRONT_IR
+            // AUTO: the front kernel pays a gather and a scatter of its window per block step; it wins where the envelope
+            // is jagged (refined meshes: a sixth of the hull's flops), not on uniform meshes (front = hull)
+            G.bs.front = G.front_fits && G.bs.front_flop <= FRONT_MAX_WORK_RATIO * G.bs.flop_per_matrix;
         }
         UPC(G.bs.perm, perm)
         G.boff = ctx->bstride;
@@ -747,6 +758,23 @@ int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, 
         ctx->launches += 2;
     }
     return launches_ok();
+}
+
+int landau_band_set_method(landau_ctx *ctx, int method) {
+    if (!ctx || method < LANDAU_BAND_AUTO || method > LANDAU_BAND_FRONT) return LANDAU_EINVAL;
+    for (auto &g : ctx->grids) {
+        if (method == LANDAU_BAND_FRONT && !g.front_fits) return LANDAU_EINVAL;
+        g.bs.front = method == LANDAU_BAND_HULL ? false
+                     : (method == LANDAU_BAND_FRONT ? true : g.front_fits && g.bs.front_flop <= FRONT_MAX_WORK_RATIO * g.bs.flop_per_matrix);
+    }
+    return LANDAU_OK;
+}
+
+int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max) {
+    if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
+    if (method) *method = ctx->grids[grid].bs.front ? LANDAU_BAND_FRONT : LANDAU_BAND_HULL;
+    if (front_rows_max) *front_rows_max = ctx->grids[grid].bs.na_max;
+    return LANDAU_OK;
 }
 
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev, void *stream) {

@@ -196,7 +196,9 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
 }
 
 // stored half-width: bw + KB rounded up to even (16-byte aligned column pairs in the window update)
-__host__ __device__ inline int band_halfwidth(int bw, int KB) { return (bw + KB + 1) & ~1; }
+// (at least 2 KB - 1: the front kernel always lists the rows of the NEXT block, up to 2 KB - 1 below a block's first column)
+__host__ __device__ inline int band_halfwidth(int bw, int KB) { return ((bw > KB - 1 ? bw : KB - 1) + KB + 1) & ~1; }
+int band_stored_halfwidth(int bw) { return band_halfwidth(bw, band_block(bw)); }
 
 // Block width and threads per matrix, by half-bandwidth (measured, 512 problems):
 //   bw = 178 (n = 745, 5,120 matrices):  KB 16 x 128 threads 17.5 ms | 16 x 256: 23.2 | 32 x 256: 29.4 | 32 x 512: 34.0
@@ -457,6 +459,280 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Front (envelope) factorisation.  The band kernel above updates the whole m x m hull of a block step; but LU without
+// pivoting keeps the ENVELOPE, and in the ordered Landau matrices the envelope is jagged: at config 5 a block step
+// reaches m = 230 rows of which only ~80 have their first entry at or before the block.  This kernel gathers exactly
+// those rows / columns (BandSpace::act_*) into a dense front in shared memory -- raw panels sL / sU and the window
+// sW[na][na] -- runs the same three phases as the band kernel on it (diagonal block by warp 0 with look-ahead, panel
+// substitutions, rank-KB window update on the FP64 tensor cores, now shared memory to shared memory) and scatters the
+// window back: a sixth of the flops and no read-modify-write of the window through L2.  Same storage, same L and U
+// (up to the order of the sums inside a window entry: unchanged, the update of a step is one mma chain either way).
+// ------------------------------------------------------------------------------------------------
+__device__ __forceinline__ void named_bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+__device__ __forceinline__ void named_bar_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
+
+// SIGNAL > 0: the warp arrives at named barrier SIGNAL (of `nthreads` threads) once it has copied the block out of src
+template <int KB, int SIGNAL>
+__device__ __forceinline__ void factor_diag_src(const double *src, size_t lds, double *Aout, size_t lda, int kb, double *sD, double *sDi,
+                                                int lane, double &pmin, double &pmax, int nthreads = 0) {
+    double *myrow = sD + min(lane, KB - 1) * (KB + 1);
+    const bool rowlane = lane < KB;
+    if (rowlane) {
+#pragma unroll
+        for (int c = 0; c < KB; ++c) myrow[c] = (lane < kb && c < kb) ? src[lane + (size_t)c * lds] : (lane == c ? 1.0 : 0.0);
+    }
+    __syncwarp();
+    if (SIGNAL > 0) named_bar_arrive(SIGNAL, nthreads);
+#pragma unroll
+    for (int c = 0; c < KB; ++c) {
+        const double *prow = sD + c * (KB + 1);
+        const double piv = prow[c];
+        if (c < kb) { pmin = fmin(pmin, fabs(piv)); pmax = fmax(pmax, fabs(piv)); }
+        if (c < kb && !(fabs(piv) <= 1.79e308)) pmin = 0.0;
+        const double pinv = rcp_newton(piv);
+        if (lane == c) sDi[c] = pinv;
+        if (lane > c && rowlane) {
+            const double l = myrow[c] * pinv;
+            myrow[c] = l;
+#pragma unroll
+            for (int cc = c + 1; cc < KB; ++cc) myrow[cc] = fma(-l, prow[cc], myrow[cc]);
+        }
+        __syncwarp();
+    }
+    if (lane < kb) {
+#pragma unroll
+        for (int c = 0; c < KB; ++c)
+            if (c < kb) Aout[lane + (size_t)c * lda] = myrow[c];
+    }
+}
+
+// Dynamic shared memory (doubles): 2 x (sD[KB][KB+1], sDi[KB]), sDs[KB][KB], sL[KB][LDP], sU[KB][LDP], sW[na_max][LDW]
+// (column-major window, LDW = 8 mod 16: the 16-byte accesses of a C tile are bank-conflict free), then na_max ints.
+//
+// Schedule of a block step (warp 0 = the "pivot" warp, warps 1 .. NW-1 = workers):
+//   all      copy of the eliminated diagonal block, panel substitutions (one chain per thread)          [block barriers]
+//   warp 0   the window tiles that hold the next diagonal block, then its elimination (the serial part of the method)
+//   workers  the other window tiles | scatter of the window back to the band | next step's list and gather
+// so the elimination of the next diagonal block runs beside the workers' memory phases.  Named barriers: 1 = warp 0's
+// tiles are done (workers wait), 2 = warp 0 has copied the block out of the window (the workers' gather may overwrite it),
+// 3, 4 = among the workers (scatter done / next list loaded).
+constexpr int FRONT_JC = 4, FRONT_IR = 5;      // window gather: columns per warp and pass, rows per lane (fronts of up to 160 rows)
+template <int KB, int NT>
+__global__ void __launch_bounds__(NT)
+k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, size_t pstride, int S,
+               const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, double *__restrict__ band_all,
+               double *__restrict__ pivots, int pivS) {
+    extern __shared__ double smem[];
+    constexpr int DSZ = KB * (KB + 1) + KB;
+    constexpr int NW = NT / 32, NWW = NW - 1, NTW = NT - 32;      // warps, worker warps, worker threads
+    static_assert(NW >= 2, "a pivot warp and at least one worker");
+    double *sDs = smem + 2 * DSZ;
+    double *sL = sDs + KB * KB;                  // sL[c][i] = -L(act[i], k0 + c)
+    double *sU = sL + (size_t)KB * LDP;          // sU[c][j] = U(k0 + c, act[j])
+    double *sW = sU + (size_t)KB * LDP;          // sW[i + j LDW] = A(act[i], act[j])
+    int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * na_max);
+    const int W = band_halfwidth(bw, KB);
+    const size_t lda = 2 * (size_t)W;
+    double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, k = lane & 3;
+    double pmin = 1.79e308, pmax = 0.0;
+
+    // gather of a step's front by the threads [t0, t0 + nt): raw panels (thread = active row / column), window (warp = columns)
+    auto gather = [&](int k0, int kb, int na, int t, int nt) {
+        for (int i = t; i < LDP; i += nt) {
+            if (i < na) {
+                const int gi = sAct[i];
+                const double *row = A + gi + (size_t)k0 * lda;
+                const double *col = A + k0 + (size_t)gi * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    sL[(size_t)c * LDP + i] = c < kb ? row[(size_t)c * lda] : 0.0;
+                    sU[(size_t)c * LDP + i] = c < kb ? col[c] : 0.0;
+                }
+            } else {
+#pragma unroll
+                for (int c = 0; c < KB; ++c) { sL[(size_t)c * LDP + i] = 0.0; sU[(size_t)c * LDP + i] = 0.0; }
+            }
+        }
+        // a warp takes FRONT_JC columns at a time and issues all their loads (FRONT_JC x FRONT_IR per lane) before the
+        // first store: the gather is bound by the latency of these loads, not by their number
+        int gr[FRONT_IR];
+#pragma unroll
+        for (int r = 0; r < FRONT_IR; ++r) gr[r] = lane + 32 * r < na ? sAct[lane + 32 * r] : -1;
+        for (int j0 = (t >> 5) * FRONT_JC; j0 < na; j0 += (nt >> 5) * FRONT_JC) {
+            double v[FRONT_JC][FRONT_IR];
+#pragma unroll
+            for (int q = 0; q < FRONT_JC; ++q) {
+                const double *colp = A + (size_t)sAct[min(j0 + q, na - 1)] * lda;
+#pragma unroll
+                for (int r = 0; r < FRONT_IR; ++r) v[q][r] = gr[r] >= 0 ? colp[gr[r]] : 0.0;
+            }
+#pragma unroll
+            for (int q = 0; q < FRONT_JC; ++q)
+                if (j0 + q < na) {
+#pragma unroll
+                    for (int r = 0; r < FRONT_IR; ++r)
+                        if (gr[r] >= 0) sW[lane + 32 * r + (size_t)(j0 + q) * LDW] = v[q][r];
+                }
+        }
+    };
+
+    // prologue: first diagonal block (warp 0), first list and front (everybody)
+    if (warp == 0) factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * (KB + 1), lane, pmin, pmax);
+    {
+        const int na = act_ptr[1] - act_ptr[0];
+        for (int i = tid; i < na; i += NT) sAct[i] = act_idx[act_ptr[0] + i];
+        __syncthreads();
+        gather(0, min(KB, n), na, tid, NT);
+    }
+    int cur = 0;
+    for (int k0 = 0, step = 0; k0 < n; k0 += KB, ++step) {
+        const int kb = min(KB, n - k0), kbn = min(KB, n - k0 - kb);      // this block, the next one
+        const int na = act_ptr[step + 1] - act_ptr[step];
+        double *sD = smem + cur * DSZ, *sDi = sD + KB * (KB + 1);
+        __syncthreads();                        // this step's front is gathered, its diagonal block eliminated
+        for (int t = tid; t < KB * KB; t += NT) sDs[t] = sD[(t / KB) * (KB + 1) + t % KB];
+        __syncthreads();
+        // panel substitutions, one chain per thread: items [0, na) are rows of the L panel (x U11 = a, right-looking),
+        // items [na, 2 na) columns of the U panel (L11 y = a, left-looking); sums in ascending index order
+        for (int it = tid; it < 2 * na; it += NT) {
+            const bool isL = it < na;
+            const int i = isL ? it : it - na;
+            const int gi = sAct[i];
+            double x[KB];
+            double *pan = isL ? sL : sU;
+#pragma unroll
+            for (int c = 0; c < KB; ++c) x[c] = pan[(size_t)c * LDP + i];
+            if (isL) {
+#pragma unroll
+                for (int t = 0; t < KB; ++t) {
+                    const double *drow = sDs + t * KB;
+                    x[t] *= sDi[t];
+                    const double xt = -x[t];
+                    if ((t + 1) < KB && ((t + 1) & 1)) x[t + 1] = fma(xt, drow[t + 1], x[t + 1]);
+#pragma unroll
+                    for (int c = (t + 2) & ~1; c < KB; c += 2) {
+                        const double2 u = *reinterpret_cast<const double2 *>(drow + c);
+                        x[c] = fma(xt, u.x, x[c]);
+                        x[c + 1] = fma(xt, u.y, x[c + 1]);
+                    }
+                }
+                double *row = A + gi + (size_t)k0 * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    if (c < kb) __stcs(row + (size_t)c * lda, x[c]);
+                    sL[(size_t)c * LDP + i] = -x[c];
+                }
+            } else {
+#pragma unroll
+                for (int t = 0; t < KB; ++t) {
+                    const double *drow = sDs + t * KB;
+                    double w = x[t];
+#pragma unroll
+                    for (int cc = 0; cc + 1 < t; cc += 2) {
+                        const double2 l = *reinterpret_cast<const double2 *>(drow + cc);
+                        w = fma(-l.x, x[cc], w);
+                        w = fma(-l.y, x[cc + 1], w);
+                    }
+                    if (t & 1) w = fma(-drow[t - 1], x[t - 1], w);
+                    x[t] = w;
+                }
+                double *col = A + k0 + (size_t)gi * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    if (c < kb) __stcs(col + c, x[c]);
+                    sU[(size_t)c * LDP + i] = x[c];
+                }
+            }
+        }
+        __syncthreads();
+        // window update in shared memory: sW += (-L)(U), warp tiles of 32 rows x 16 columns as in the band kernel
+        const int nti = (na + WT - 1) / WT, ntj = (na + WTJ - 1) / WTJ;
+        const int ntiles = nti * ntj, nlook = min(ntj, (KB + WTJ - 1) / WTJ);
+        auto do_tile = [&](int wt) {
+                const int i0 = (wt % nti) * WT, j0 = (wt / nti) * WTJ;
+                double acc[2][4][2];
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    const double *colp = sW + (size_t)j * LDW;
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < na && i + 1 < na) {
+                            const double2 v = *reinterpret_cast<const double2 *>(colp + i);
+                            acc[jb][ib][0] = v.x; acc[jb][ib][1] = v.y;
+                        } else {
+                            acc[jb][ib][0] = (j < na && i < na) ? colp[i] : 0.0;
+                            acc[jb][ib][1] = 0.0;
+                        }
+                    }
+                }
+#pragma unroll 4
+                for (int c0 = 0; c0 < KB; c0 += 4) {
+                    const double *pu = sU + (size_t)(c0 + k) * LDP + j0 + g;
+                    const double *pl = sL + (size_t)(c0 + k) * LDP + i0 + g;
+                    double fa[2], fb[4];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) fa[t] = pu[8 * t];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) fb[t] = pl[8 * t];
+#pragma unroll
+                    for (int jb = 0; jb < 2; ++jb)
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) dmma884(acc[jb][ib], fa[jb], fb[ib]);
+                }
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    double *colp = sW + (size_t)j * LDW;
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < na && i + 1 < na) *reinterpret_cast<double2 *>(colp + i) = make_double2(acc[jb][ib][0], acc[jb][ib][1]);
+                        else if (j < na && i < na) colp[i] = acc[jb][ib][0];
+                    }
+                }
+        };
+        if (warp == 0) {
+            for (int u = 0; u < nlook; ++u) do_tile(u * nti);                  // (ti = 0, tj = u): rows / columns of the next block
+            __threadfence_block();
+            __syncwarp();
+            named_bar_arrive(1, NT);
+            if (kbn > 0) {
+                double *sDn = smem + (cur ^ 1) * DSZ;
+                factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * (KB + 1), lane, pmin, pmax, NT);
+            } else named_bar_arrive(2, NT);
+        } else {
+            for (int u = warp - 1; u < ntiles - nlook; u += NWW) {
+                int wt = u + 1;
+                if (nlook > 1 && wt >= nti) wt += 1;                           // skip tiles (0,0) and (0,1)
+                do_tile(wt);
+            }
+            named_bar_sync(1, NT);                                             // every tile of the window is done
+            // the updated window back to the band (the next diagonal block is warp 0's: it writes it eliminated)
+            for (int j = warp - 1; j < na; j += NWW) {
+                double *colp = A + (size_t)sAct[j] * lda;
+                for (int i = lane; i < na; i += 32)
+                    if (i >= kbn || j >= kbn) colp[sAct[i]] = sW[i + (size_t)j * LDW];
+            }
+            named_bar_sync(3, NTW);                                            // the workers have read sAct and written the band
+            const int nan = kbn > 0 ? act_ptr[step + 2] - act_ptr[step + 1] : 0;
+            for (int i = tid - 32; i < nan; i += NTW) sAct[i] = act_idx[act_ptr[step + 1] + i];
+            named_bar_sync(4, NTW);
+            named_bar_sync(2, NT);                                             // warp 0 has its block out of the window
+            if (kbn > 0) gather(k0 + kb, kbn, nan, tid - 32, NTW);
+        }
+        cur ^= 1;
+    }
+    if (pivots && tid == 0) {
+        double *pv = pivots + 2 * ((size_t)(blockIdx.x / S) * pivS + blockIdx.x % S);
+        pv[0] = pmin; pv[1] = pmax;
+    }
+}
+
 // Banded triangular solves, one block per matrix: x = P^T U^-1 L^-1 P b with the RCM permutation.
 // Blocks of KB columns (those of the factorisation): the diagonal block by warp 0 (lane = row), the panel
 // below / above, confined to the envelope, by one thread per row with KB independent loads.
@@ -538,6 +814,34 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     for (int i = tid; i < n; i += NT) xout[voff + perm[i]] = x[i];
 }
 
+// Host: the active list of every block step (BandSpace::act_*).  LU without pivoting keeps the envelope: row i of L
+// starts at first[i] (its first entry in the ordered pattern), column j of U likewise (the pattern is structurally
+// symmetric).  So block step s (columns k0 .. ke) only involves the rows / columns i > ke with first[i] <= ke; the
+// next block's rows are always listed (first, in order) so that its diagonal block is the leading corner of the front.
+int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                      int bw, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop) {
+    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB;
+    std::vector<int32_t> pos(n), first(n);
+    for (int i = 0; i < n; ++i) { pos[perm[i]] = i; first[i] = i; }
+    for (int i = 0; i < n; ++i)
+        for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) first[pos[i]] = std::min<int32_t>(first[pos[i]], pos[colidx[t]]);
+    act_ptr.assign(nsteps + 1, 0);
+    act_idx.clear();
+    int na_max = 0;
+    double work = 0.0;
+    for (int s = 0; s < nsteps; ++s) {
+        const int ke = std::min(s * KB + KB, n) - 1, nxt = std::min(ke + KB, n - 1);
+        for (int i = ke + 1; i < n && i <= std::min(n - 1, ke + bw + KB); ++i)      // first[i] >= i - bw
+            if (i <= nxt || first[i] <= ke) act_idx.push_back(i);
+        act_ptr[s + 1] = int32_t(act_idx.size());
+        const int na = act_ptr[s + 1] - act_ptr[s];
+        na_max = std::max(na_max, na);
+        work += 2.0 * (ke - s * KB + 1) * double(na) * double(na);
+    }
+    if (front_flop) *front_flop = work;
+    return na_max;
+}
+
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
@@ -567,7 +871,8 @@ void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
     const int KB = band_block(bw), W = band_halfwidth(bw, KB), nsteps = (n + KB - 1) / KB;
     std::vector<int32_t> pos(n), E(nsteps);
     for (int i = 0; i < n; ++i) pos[perm[i]] = i;
-    for (int s = 0; s < nsteps; ++s) E[s] = std::min(n - 1, std::min(s * KB + KB, n) - 1 + mlow[s]);
+    // (the front kernel lists the next block's rows whether the envelope reaches them or not: at least KB rows)
+    for (int s = 0; s < nsteps; ++s) E[s] = std::min(n - 1, std::min(s * KB + KB, n) - 1 + std::max(mlow[s], KB));
     zlo.assign(n, 0); zcnt.assign(n, 0); fptr.assign(n + 1, 0);
     fsrc.clear(); foff.clear();
     int s0 = 0;
@@ -599,7 +904,32 @@ static cudaError_t factor_t(const BandSpace &bs, int nmat, int S, size_t pstride
     return cudaGetLastError();
 }
 
+static int front_ldw(int na_max) { return ((std::max(na_max, 1) + 7) / 16) * 16 + 8; }      // >= na_max, = 8 mod 16
+
+size_t band_front_smem(int bw, int na_max) {
+    const int KB = band_block(bw);
+    return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + (size_t)KB * KB + 2 * (size_t)KB * band_mw(na_max) +
+                             (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(na_max + 2) / 2);
+}
+
+template <int KB, int NT>
+static cudaError_t front_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+    const size_t smem = band_front_smem(bs.bw, bs.na_max);
+    cudaError_t e = cudaFuncSetAttribute(k_front_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_front_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
+                                                   pstride, S, bs.act_ptr, bs.act_idx, band, pivots, pivS);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+    if (bs.front) {
+        switch (band_block(bs.bw)) {
+            case 32: return front_t<32, 256>(bs, nmat, S, pstride, band, pivots, pivS, st);
+            case 16: return front_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
+            default: return front_t<8, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
+        }
+    }
     switch (band_block(bs.bw)) {
         case 32: return factor_t<32, 256>(bs, nmat, S, pstride, band, pivots, pivS, st);
         case 16: return bs.bw <= 256 ? factor_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st)

@@ -82,6 +82,13 @@ struct BandSpace {
     // solves touch (zeroed: zlo = offset of the first one inside the column, zcnt of them), and the CSR entries of the
     // column (fsrc = index into the species' CSR values, foff = offset inside the column), fptr[n + 1]
     const int32_t *zlo, *zcnt, *fptr, *fsrc, *foff;
+    // front (envelope) factorisation: per block step the rows / columns that elimination can reach -- the next block's,
+    // then every later row whose envelope starts at or before the block (ascending) -- act_ptr[steps + 1], act_idx;
+    // na_max = the longest list; front = true when the front of every step fits shared memory
+    const int32_t *act_ptr, *act_idx;
+    int na_max;
+    double front_flop;         // window-update flop of one factorisation by the front kernel (2 KB sum na_s^2)
+    bool front;
     const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
@@ -92,12 +99,17 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
 double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
                      int &bw, std::vector<int32_t> *mlow, std::vector<int32_t> *mup);
 int band_block(int bw);        // KB, a function of bw only
+int band_stored_halfwidth(int bw);   // W: the band stores 2 W + 1 diagonals (bw + KB, at least 2 KB - 1, rounded up to even)
 size_t band_factor_smem(int bw);
 // band points at this grid's block of problem 0; matrix (problem b, species s) = band + b pstride + s mat_doubles
 // (problem-major workspace: a solve may use a different nb than the factorisation)
 void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
                      int bw, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, std::vector<int32_t> &zlo,
                      std::vector<int32_t> &zcnt, std::vector<int32_t> &fptr, std::vector<int32_t> &fsrc, std::vector<int32_t> &foff);
+// active lists of the front factorisation (see BandSpace); returns the longest list
+int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                      int bw, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop);
+size_t band_front_smem(int bw, int na_max);     // dynamic shared memory of the front kernel
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st);
 // pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
