@@ -472,39 +472,56 @@ k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S,
 __device__ __forceinline__ void named_bar_sync(int id, int nthreads) { asm volatile("bar.sync %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 __device__ __forceinline__ void named_bar_arrive(int id, int nthreads) { asm volatile("bar.arrive %0, %1;" ::"r"(id), "r"(nthreads) : "memory"); }
 
-// SIGNAL > 0: the warp arrives at named barrier SIGNAL (of `nthreads` threads) once it has copied the block out of src
+// KB x KB block eliminated without pivoting by one warp, lane = row, the row in REGISTERS and the pivot row passed
+// around by shuffles (the shared-memory version of the band kernel spends its time on the round trip of every row
+// through shared memory and a warp barrier per column; here a column costs one reciprocal and 2 (KB - c) shuffles).
+// L\U goes to sD[KB][KB+1], 1/pivots to sDi, and to Aout (global, leading dimension lda); a short block is completed
+// by the identity.  Returns (smallest, largest |pivot|), smallest = 0 for a zero / NaN / infinite pivot.
+// SIGNAL > 0: the warp arrives at named barrier SIGNAL (of `nthreads` threads) once it has the block out of src.
+// Not inlined: compiled on its own the rows stay in registers (inlined into the front kernel they went to the stack).
 template <int KB, int SIGNAL>
-__device__ __forceinline__ void factor_diag_src(const double *src, size_t lds, double *Aout, size_t lda, int kb, double *sD, double *sDi,
-                                                int lane, double &pmin, double &pmax, int nthreads = 0) {
-    double *myrow = sD + min(lane, KB - 1) * (KB + 1);
-    const bool rowlane = lane < KB;
-    if (rowlane) {
+__device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, double *Aout, size_t lda, int kb, double *sD, double *sDi,
+                                                int lane, int nthreads) {
+    double r[KB];
+    double pmin = 1.79e308, pmax = 0.0;
+    const int row = min(lane, KB - 1);
 #pragma unroll
-        for (int c = 0; c < KB; ++c) myrow[c] = (lane < kb && c < kb) ? src[lane + (size_t)c * lds] : (lane == c ? 1.0 : 0.0);
+    for (int c = 0; c < KB; ++c) r[c] = (lane < kb && c < kb) ? src[row + (size_t)c * lds] : (lane == c ? 1.0 : 0.0);
+    if (SIGNAL > 0) {
+        double keep = 0.0;                 // the loads above must have RETURNED before the barrier lets others overwrite src
+#pragma unroll
+        for (int c = 0; c < KB; ++c) keep += r[c];
+        if (keep == 1.2345e300) r[0] = keep;
+        __syncwarp();
+        named_bar_arrive(SIGNAL, nthreads);
     }
-    __syncwarp();
-    if (SIGNAL > 0) named_bar_arrive(SIGNAL, nthreads);
 #pragma unroll
     for (int c = 0; c < KB; ++c) {
-        const double *prow = sD + c * (KB + 1);
-        const double piv = prow[c];
-        if (c < kb) { pmin = fmin(pmin, fabs(piv)); pmax = fmax(pmax, fabs(piv)); }
-        if (c < kb && !(fabs(piv) <= 1.79e308)) pmin = 0.0;
+        const double piv = __shfl_sync(0xffffffffu, r[c], c);
+        if (c < kb) { pmin = fmin(pmin, fabs(piv)); pmax = fmax(pmax, fabs(piv)); }   // fmin/fmax drop a NaN operand ...
+        if (c < kb && !(fabs(piv) <= 1.79e308)) pmin = 0.0;                            // ... so a NaN / Inf pivot is flagged here
         const double pinv = rcp_newton(piv);
         if (lane == c) sDi[c] = pinv;
-        if (lane > c && rowlane) {
-            const double l = myrow[c] * pinv;
-            myrow[c] = l;
+        const bool below = lane > c;
+        const double l = r[c] * pinv;
+        if (below) r[c] = l;
 #pragma unroll
-            for (int cc = c + 1; cc < KB; ++cc) myrow[cc] = fma(-l, prow[cc], myrow[cc]);
+        for (int cc = c + 1; cc < KB; ++cc) {
+            const double pr = __shfl_sync(0xffffffffu, r[cc], c);
+            if (below) r[cc] = fma(-l, pr, r[cc]);
         }
-        __syncwarp();
+    }
+    if (lane < KB) {
+#pragma unroll
+        for (int c = 0; c < KB; ++c) sD[lane * (KB + 1) + c] = r[c];
     }
     if (lane < kb) {
 #pragma unroll
         for (int c = 0; c < KB; ++c)
-            if (c < kb) Aout[lane + (size_t)c * lda] = myrow[c];
+            if (c < kb) Aout[lane + (size_t)c * lda] = r[c];
     }
+    __syncwarp();
+    return make_double2(pmin, pmax);
 }
 
 // Dynamic shared memory (doubles): 2 x (sD[KB][KB+1], sDi[KB]), sDs[KB][KB], sL[KB][LDP], sU[KB][LDP], sW[na_max][LDW]
@@ -580,7 +597,10 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
     };
 
     // prologue: first diagonal block (warp 0), first list and front (everybody)
-    if (warp == 0) factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * (KB + 1), lane, pmin, pmax);
+    if (warp == 0) {
+        const double2 pv = factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * (KB + 1), lane, NT);
+        pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
+    }
     {
         const int na = act_ptr[1] - act_ptr[0];
         for (int i = tid; i < na; i += NT) sAct[i] = act_idx[act_ptr[0] + i];
@@ -703,7 +723,8 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
             named_bar_arrive(1, NT);
             if (kbn > 0) {
                 double *sDn = smem + (cur ^ 1) * DSZ;
-                factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * (KB + 1), lane, pmin, pmax, NT);
+                const double2 pv = factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * (KB + 1), lane, NT);
+                pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
             } else named_bar_arrive(2, NT);
         } else {
             for (int u = warp - 1; u < ntiles - nlook; u += NWW) {
@@ -925,7 +946,7 @@ static cudaError_t front_t(const BandSpace &bs, int nmat, int S, size_t pstride,
 cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
     if (bs.front) {
         switch (band_block(bs.bw)) {
-            case 32: return front_t<32, 256>(bs, nmat, S, pstride, band, pivots, pivS, st);
+            case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);
             case 16: return front_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
             default: return front_t<8, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
         }
