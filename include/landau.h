@@ -228,6 +228,10 @@ int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, 
 #define LANDAU_BAND_AUTO 0
 #define LANDAU_BAND_HULL 1
 #define LANDAU_BAND_FRONT 2
+/* Host-only: for the band order of this mesh, the rows of the largest front beside its block, the flop of the front
+ * kernel's window updates (compare landau_band_order_host's flop: the hull kernel's) and whether the largest front
+ * fits shared memory.  Any output may be NULL. */
+int landau_band_front_host(const landau_mesh *mesh, int order, int32_t *front_rows_max, double *front_flop, int32_t *fits);
 int landau_band_set_method(landau_ctx *ctx, int method);
 int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max);
 int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, double *pivots_dev,

@@ -64,6 +64,7 @@ SIGNATURES = {
     "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
     "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "landau_band_front_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), POINTER(c_double), POINTER(c_int32)]),
     "landau_band_set_method": (c_int, [c_void_p, c_int]),
     "landau_band_method": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32)]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
@@ -152,6 +153,15 @@ def landau_band_order_host(mesh, order: int):
     _check(L.landau_band_order_host(ctypes.byref(m), order, perm.ctypes.data_as(POINTER(c_int32)), ctypes.byref(bw), ctypes.byref(kb),
                                     ctypes.byref(fl)))
     return dict(perm=perm, bw=bw.value, block_columns=kb.value, flop=fl.value)
+
+
+def landau_band_front_host(mesh, order: int):
+    """Host-only: dict(rows_max, flop, fits) of the front (envelope) factorisation for this mesh's band order."""
+    L = lib()
+    m, keep = _mesh_struct(mesh)
+    r, fl, fits = c_int32(), c_double(), c_int32()
+    _check(L.landau_band_front_host(ctypes.byref(m), order, ctypes.byref(r), ctypes.byref(fl), ctypes.byref(fits)))
+    return dict(rows_max=r.value, flop=fl.value, fits=bool(fits.value))
 
 
 def landau_fp64_peak_probe(iters: int = 1 << 16):

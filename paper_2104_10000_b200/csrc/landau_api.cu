@@ -432,7 +432,7 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &G.bs.front_flop);
             if (act_idx.empty()) act_idx.push_back(0);
             UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
-            G.front_fits = band_front_smem(bw, G.bs.na_max) <= size_t(225) * 1024 && G.bs.na_max <= 160;   // + 1 KB the driver reserves per block; FRONT_IR
+            G.front_fits = band_front_smem(bw, G.bs.na_max) <= size_t(225) * 1024 && G.bs.na_max <= 160 && band_block(bw) >= 16;   // + 1 KB the driver reserves per block; FRONT_IR rows per lane
             // AUTO: the front kernel pays a gather and a scatter of its window per block step; it wins where the envelope
             // is jagged (refined meshes: a sixth of the hull's flops), not on uniform meshes (front = hull)
             G.bs.front = G.front_fits && G.bs.front_flop <= FRONT_MAX_WORK_RATIO * G.bs.flop_per_matrix;
@@ -548,6 +548,25 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
         *flop_per_factorization = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr);
     }
     return int(LANDAU_OK);
+    });
+}
+
+int landau_band_front_host(const landau_mesh *mesh, int order, int32_t *front_rows_max, double *front_flop, int32_t *fits) {
+    if (!mesh) return LANDAU_EINVAL;
+    return guarded([&]() {
+        HostSpace hs;
+        std::string err;
+        const int rc = build_host_space(*mesh, order, hs, err);
+        if (rc != LANDAU_OK) { g_cuda_err = err; return rc; }
+        std::vector<int32_t> perm, act_ptr, act_idx;
+        int bw = 0;
+        rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
+        double fl = 0.0;
+        const int na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &fl);
+        if (front_rows_max) *front_rows_max = na_max;
+        if (front_flop) *front_flop = fl;
+        if (fits) *fits = band_front_smem(bw, na_max) <= size_t(225) * 1024 && na_max <= 160 && band_block(bw) >= 16;
+        return int(LANDAU_OK);
     });
 }
 

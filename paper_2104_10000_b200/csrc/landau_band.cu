@@ -948,7 +948,7 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstr
         switch (band_block(bs.bw)) {
             case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);
             case 16: return front_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
-            default: return front_t<8, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
+            default: break;      // 8-column blocks mean bw > 832: no front of that size fits (front is false then)
         }
     }
     switch (band_block(bs.bw)) {

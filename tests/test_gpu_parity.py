@@ -225,14 +225,22 @@ def test_multigrid_parity(gpu, oracle, which, path):
         assert num <= 1e-12 * den
 
 
+HULL, FRONT = 1, 2          # LANDAU_BAND_HULL, LANDAU_BAND_FRONT
+
+
+@pytest.mark.parametrize("method", [pytest.param(HULL, id="hull"), pytest.param(FRONT, id="front")])
 @pytest.mark.parametrize("cfg,variant", [(0, "B"), (1, "B"), (3, "A"), (3, "B")])
-def test_band_lu_solve_parity(gpu, oracle, cfg, variant):
+def test_band_lu_solve_parity(gpu, oracle, cfg, variant, method):
     """SURVEY 8(f) NEXT-4 (section III-G): the matrices shift M + A - J of two problems factored and
-    solved on the device (RCM order, no pivoting) against the library solve of the oracle's dense blocks.
-    Tolerance: 50 cond(A) eps on max|x| (forward error of a backward-stable solve), and the residual."""
+    solved on the device (RCM order, no pivoting) against the library solve of the oracle's dense blocks, with both
+    factorisation kernels: the front (envelope) kernel -- 16-column blocks for configs 0, 1, 3A, 32-column blocks for
+    3B -- and the hull kernel.  The band workspace is NaN-filled first: neither kernel may read what the fill did not
+    write.  Tolerance: 50 cond(A) eps on max|x| (forward error of a backward-stable solve), and the residual."""
     import torch
     wl = inputs.config(cfg, variant=variant)
     ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 2)
+    ctx.band_set_method(method)
+    assert ctx.band_method()[0] == method
     r, z = ctx.dof_coords()
     f1 = inputs.nodal_f(wl, r, z)
     f = np.stack([f1, 0.8 * f1])
@@ -242,7 +250,7 @@ def test_band_lu_solve_parity(gpu, oracle, cfg, variant):
     F = torch.zeros((2, ctx.S, ctx.n), dtype=torch.float64, device="cuda")
     ctx.implicit_operator_batched(fd, torch.from_numpy(Ez).cuda(), shift, vals, F)
     bw, md, ws = ctx.band_sizes()
-    band = torch.empty(2 * ws, dtype=torch.float64, device="cuda")
+    band = torch.full((2 * ws,), float("nan"), dtype=torch.float64, device="cuda")
     ctx.band_factor_batched(vals, band)
     rhs = torch.from_numpy(np.cos(0.37 * np.arange(2 * ctx.S * ctx.n)).reshape(2, ctx.S, ctx.n) + 2.0).cuda()
     x = torch.zeros_like(rhs)
@@ -261,6 +269,48 @@ def test_band_lu_solve_parity(gpu, oracle, cfg, variant):
             res = np.abs(A @ x_h[k, a] - rhs_h[k, a]).max() / (np.abs(A).sum(axis=1).max() * np.abs(x_h[k, a]).max())
             assert res <= 1e-13, (k, a, res)
     print(f"{wl.name}: n = {ctx.n}, half-bandwidth after RCM {bw}")
+
+
+def test_band_lu_front_and_hull_kernels_agree_and_auto_chooses(gpu):
+    """The two factorisation kernels give the same solution up to rounding (they eliminate the same entries; only
+    the order inside a rank-KB update differs); LANDAU_BAND_AUTO takes the front kernel on the refined meshes (its
+    flops are a sixth of the hull's) and the hull kernel on the uniform Q3 mesh (front = hull there); forcing the front
+    kernel where the largest front cannot fit shared memory is refused; both are bitwise reproducible."""
+    import torch
+    for cfg, variant, want in ((3, "B", FRONT), (6, "B", FRONT), (2, "B", HULL)):
+        wl = inputs.config(cfg, variant=variant)
+        ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 2)
+        assert ctx.band_method()[0] == want, (wl.name, ctx.band_method())
+        r, z = ctx.dof_coords()
+        f1 = inputs.nodal_f(wl, r, z)
+        fd = torch.from_numpy(np.stack([f1, 0.9 * f1])).cuda()
+        vals = torch.zeros((2, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
+        ctx.implicit_operator_batched(fd, torch.tensor([0.2, -0.1], dtype=torch.float64, device="cuda"), 3.0, vals, None)
+        bw, md, ws = ctx.band_sizes()
+        rhs = torch.from_numpy(np.sin(0.11 * np.arange(2 * ctx.S * ctx.n)).reshape(2, ctx.S, ctx.n) + 1.5).cuda()
+        sols = {}
+        for method in (HULL, FRONT, FRONT):
+            ctx.band_set_method(method)
+            band = torch.full((2 * ws,), float("nan"), dtype=torch.float64, device="cuda")
+            piv = torch.zeros((2, ctx.S, 2), dtype=torch.float64, device="cuda")
+            x = torch.empty_like(rhs)
+            ctx.band_factor_batched(vals, band, piv)
+            ctx.band_solve_batched(band, rhs, x)
+            sols.setdefault(method, []).append((x.clone(), piv.clone()))
+        (xh, ph), (xf, pf), (xf2, pf2) = sols[HULL][0], sols[FRONT][0], sols[FRONT][1]
+        assert torch.equal(xf, xf2) and torch.equal(pf, pf2)
+        assert bool(torch.isfinite(xf).all())
+        assert float((xf - xh).abs().max() / xh.abs().max()) <= 1e-12
+        assert float(((pf - ph).abs() / ph.abs()).max()) <= 1e-10          # the same pivots
+        ctx.band_set_method(0)
+        assert ctx.band_method()[0] == want
+        ctx.destroy()
+    mesh = inputs.mesh_uniform(0.0, 5.0, -5.0, 5.0, 46, 46)                # fronts of 420 rows: no shared memory for them
+    ctx = gpu.LandauContext(mesh, 3, inputs._sp([(1, -1, 1, 1)]), 1)
+    assert ctx.band_method()[0] == HULL
+    with pytest.raises(gpu.LandauError) as ei:
+        ctx.band_set_method(FRONT)
+    assert ei.value.code == gpu.LANDAU_EINVAL
 
 
 def test_one_implicit_step_through_the_whole_path_conserves(gpu):

@@ -136,6 +136,34 @@ def test_band_order_is_a_valid_bandwidth_reducing_permutation(binding, cfg):
     assert bo["flop"] <= _envelope_work(hs["rowptr"], hs["colidx"], np.asarray(p), bo["block_columns"])
 
 
+@pytest.mark.parametrize("cfg", [0, 2, 3, 6])
+def test_front_lists_of_the_envelope_factorisation(binding, cfg):
+    """Host logic of the front kernel: LU without pivoting keeps the envelope, so block step s involves, beside its
+    own block, the next block's rows and every later row whose first entry lies at or before the block.  Recomputed
+    here from that definition: the longest list and the flop 2 KB sum na_s^2 must match; on the refined meshes the
+    front does a fraction of the hull's flops, on the uniform mesh about the same."""
+    wl = inputs.config(cfg)
+    hs = binding.landau_setup_host(wl.mesh, wl.order)
+    bo = binding.landau_band_order_host(wl.mesh, wl.order)
+    fr = binding.landau_band_front_host(wl.mesh, wl.order)
+    n, KB = hs["n"], bo["block_columns"]
+    pos = np.empty(n, int); pos[bo["perm"]] = np.arange(n)
+    rows = np.repeat(np.arange(n), np.diff(hs["rowptr"]))
+    first = np.arange(n)
+    np.minimum.at(first, pos[rows], pos[hs["colidx"]])
+    rows_max, flop = 0, 0.0
+    for k0 in range(0, n, KB):
+        ke = min(k0 + KB, n) - 1
+        act = {i for i in range(ke + 1, n) if i <= ke + KB or first[i] <= ke}
+        rows_max = max(rows_max, len(act))
+        flop += 2.0 * (ke - k0 + 1) * len(act) ** 2
+    assert fr["rows_max"] == rows_max and fr["flop"] == flop and fr["fits"]
+    if cfg in (3, 6):
+        assert fr["flop"] < 0.3 * bo["flop"]
+    if cfg == 2:
+        assert fr["flop"] > 0.6 * bo["flop"]
+
+
 def test_multigrid_argument_checks_need_no_gpu(binding):
     """landau_create_multigrid validates its species -> grid map before it looks for a device: bad maps give
     LANDAU_EINVAL everywhere; a good one gives LANDAU_ECUDA on a machine without a GPU."""
