@@ -352,14 +352,17 @@ def time_next_rows(binding, inputs, torch, ctx5, f5, vals5, Cf5, nb):
     torch.cuda.synchronize()
     fms, sms_ = e0.elapsed_time(e1), e1.elapsed_time(e2)
     nmat = nb * ctx5.S
-    flop = ctx5.band_flop_per_factorization * nmat     # outer-product updates inside the envelope (executed)
+    method, front_rows = ctx5.band_method()
+    flop = ctx5.band_flop_in_use * nmat                # window updates executed by the kernel in use (front: inside the envelope)
     flop_band = 2.0 * ctx5.n * bw * bw * nmat          # Alg. 4.3.1 on the uniform band: n outer products of bw x bw
     out["band_lu_config5"] = {"matrices": nmat, "n": ctx5.n, "half_bandwidth": bw, "workspace_gb": nb * ws * 8e-9,
+                              "kernel": "front (envelope)" if method == binding.LANDAU_BAND_FRONT else "hull", "front_rows_max": front_rows,
+                              "hull_flop_per_factorization": ctx5.band_flop_per_factorization,
                               "factor_ms": fms, "solve_ms": sms_, "factor_tflops": flop / (fms * 1e-3) * 1e-12,
                               "factor_tflops_uniform_band_equiv": flop_band / (fms * 1e-3) * 1e-12,
                               "factorizations_per_s": nmat / (fms * 1e-3),
                               "min_pivot_ratio": float((piv[:, :, 0] / piv[:, :, 1]).min()),
-                              "what": "scatter + blocked outer-product band LU without pivoting (pivot report on), then L/U solves (one rhs)"}
+                              "what": "fill + blocked outer-product LU without pivoting inside the envelope (pivot report on), then L/U solves (one rhs)"}
     del band, rhs, x
     name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("paper3")
     mg = binding.LandauMultigridContext(meshes, sgrid, order, spc, nb)
@@ -630,11 +633,14 @@ def kernel_run(which):
             bw, md, ws = ctx.band_sizes()
             band = torch.empty(nb * ws, dtype=torch.float64, device="cuda")
             piv = torch.zeros((nb, ctx.S, 2), dtype=torch.float64, device="cuda")
-            ctx.band_factor_batched(vals, band, piv)
+            for method in (binding.LANDAU_BAND_AUTO, binding.LANDAU_BAND_HULL):       # the kernel in use, then the hull kernel
+                ctx.band_set_method(method)
+                ctx.band_factor_batched(vals, band, piv)
+                m, rows = ctx.band_method()
+                plan.append({"workload": tag + (":hull" if m == binding.LANDAU_BAND_HULL else ":front"), "matrices": nb * ctx.S, "n": ctx.n,
+                             "half_bandwidth": bw, "front_rows_max": rows, "flop_per_factorization": ctx.band_flop_in_use})
             ctx.band_solve_batched(band, Cf, Cf)
             torch.cuda.synchronize()
-            plan.append({"workload": tag, "matrices": nb * ctx.S, "n": ctx.n, "half_bandwidth": bw,
-                         "flop_per_factorization": ctx.band_flop_per_factorization})
             ctx.destroy()
             del fd, vals, Cf, band
     elif which == "main":

@@ -224,7 +224,8 @@ int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, 
  *   LANDAU_BAND_HULL   updates the whole window of a block step in place (the monotone hull of the envelope).
  * LANDAU_BAND_AUTO (the default) takes the front kernel whenever the largest front fits the shared memory of an SM.
  * landau_band_set_method returns LANDAU_EINVAL for LANDAU_BAND_FRONT when it does not fit; landau_band_method reports
- * the kernel in use for a grid and the longest active list (rows of the largest front beside its block). */
+ * the kernel in use for a grid, the longest active list (rows of the largest front beside its block) and the flop of
+ * the window updates of one factorisation by that kernel.  Outputs may be NULL. */
 #define LANDAU_BAND_AUTO 0
 #define LANDAU_BAND_HULL 1
 #define LANDAU_BAND_FRONT 2
@@ -233,7 +234,7 @@ int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, 
  * fits shared memory.  Any output may be NULL. */
 int landau_band_front_host(const landau_mesh *mesh, int order, int32_t *front_rows_max, double *front_flop, int32_t *fits);
 int landau_band_set_method(landau_ctx *ctx, int method);
-int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max);
+int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max, double *flop_per_factorization);
 int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, double *band_dev, double *pivots_dev,
                                void *stream);
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,

@@ -66,7 +66,7 @@ SIGNATURES = {
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_front_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), POINTER(c_double), POINTER(c_int32)]),
     "landau_band_set_method": (c_int, [c_void_p, c_int]),
-    "landau_band_method": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32)]),
+    "landau_band_method": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_double)]),
     "landau_jacobian_host": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p]),
     "landau_launch_count": (c_int, [c_void_p, POINTER(c_int64)]),
     "landau_profile_enable": (c_int, [c_void_p, c_int]),
@@ -293,8 +293,9 @@ class LandauContext:
 
     def band_method(self, grid=0):
         """(kernel in use for the grid: LANDAU_BAND_HULL or _FRONT, rows of the largest front beside its block)."""
-        m, r = c_int32(), c_int32()
-        _check(lib().landau_band_method(self._h, grid, ctypes.byref(m), ctypes.byref(r)))
+        m, r, fl = c_int32(), c_int32(), c_double()
+        _check(lib().landau_band_method(self._h, grid, ctypes.byref(m), ctypes.byref(r), ctypes.byref(fl)))
+        self.band_flop_in_use = fl.value
         return m.value, r.value
 
     def band_factor_batched(self, vals, band, pivots=None, stream=None):

@@ -789,10 +789,12 @@ int landau_band_set_method(landau_ctx *ctx, int method) {
     return LANDAU_OK;
 }
 
-int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max) {
+int landau_band_method(const landau_ctx *ctx, int grid, int32_t *method, int32_t *front_rows_max, double *flop_per_factorization) {
     if (!ctx || grid < 0 || grid >= int(ctx->grids.size())) return LANDAU_EINVAL;
-    if (method) *method = ctx->grids[grid].bs.front ? LANDAU_BAND_FRONT : LANDAU_BAND_HULL;
-    if (front_rows_max) *front_rows_max = ctx->grids[grid].bs.na_max;
+    const BandSpace &bs = ctx->grids[grid].bs;
+    if (method) *method = bs.front ? LANDAU_BAND_FRONT : LANDAU_BAND_HULL;
+    if (front_rows_max) *front_rows_max = bs.na_max;
+    if (flop_per_factorization) *flop_per_factorization = bs.front ? bs.front_flop : bs.flop_per_matrix;
     return LANDAU_OK;
 }
 
