@@ -475,7 +475,7 @@ __device__ __forceinline__ void named_bar_arrive(int id, int nthreads) { asm vol
 // KB x KB block eliminated without pivoting by one warp, lane = row, the row in REGISTERS and the pivot row passed
 // around by shuffles (the shared-memory version of the band kernel spends its time on the round trip of every row
 // through shared memory and a warp barrier per column; here a column costs one reciprocal and 2 (KB - c) shuffles).
-// L\U goes to sD[KB][KB+1], 1/pivots to sDi, and to Aout (global, leading dimension lda); a short block is completed
+// L\U goes to sD[KB][KB], 1/pivots to sDi, and to Aout (global, leading dimension lda); a short block is completed
 // by the identity.  Returns (smallest, largest |pivot|), smallest = 0 for a zero / NaN / infinite pivot.
 // SIGNAL > 0: the warp arrives at named barrier SIGNAL (of `nthreads` threads) once it has the block out of src.
 // Not inlined: compiled on its own the rows stay in registers (inlined into the front kernel they went to the stack).
@@ -511,9 +511,9 @@ __device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, d
             if (below) r[cc] = fma(-l, pr, r[cc]);
         }
     }
-    if (lane < KB) {
+    if (lane < KB) {                       // rows 16-byte aligned: the substitutions read them with 16-byte loads
 #pragma unroll
-        for (int c = 0; c < KB; ++c) sD[lane * (KB + 1) + c] = r[c];
+        for (int c = 0; c < KB; ++c) sD[lane * KB + c] = r[c];
     }
     if (lane < kb) {
 #pragma unroll
@@ -524,8 +524,9 @@ __device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, d
     return make_double2(pmin, pmax);
 }
 
-// Dynamic shared memory (doubles): 2 x (sD[KB][KB+1], sDi[KB]), sDs[KB][KB], sL[KB][LDP], sU[KB][LDP], sW[na_max][LDW]
-// (column-major window, LDW = 8 mod 16: the 16-byte accesses of a C tile are bank-conflict free), then na_max ints.
+// Dynamic shared memory (doubles): 2 x (sD[KB][KB], sDi[KB]), sL[KB][LDP], sU[KB][LDP], sW[na_max][LDW]
+// (column-major window, LDW = 8 mod 16: the 16-byte accesses of a C tile are bank-conflict free), then 2 na_max ints
+// (this step's list and the next one's).
 //
 // Schedule of a block step (warp 0 = the "pivot" warp, warps 1 .. NW-1 = workers):
 //   all      copy of the eliminated diagonal block, panel substitutions (one chain per thread)          [block barriers]
@@ -533,7 +534,7 @@ __device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, d
 //   workers  the other window tiles | scatter of the window back to the band | next step's list and gather
 // so the elimination of the next diagonal block runs beside the workers' memory phases.  Named barriers: 1 = warp 0's
 // tiles are done (workers wait), 2 = warp 0 has copied the block out of the window (the workers' gather may overwrite it),
-// 3, 4 = among the workers (scatter done / next list loaded).
+// 3 = among the workers (scatter done).
 constexpr int FRONT_JC = 4, FRONT_IR = 5;      // window gather: columns per warp and pass, rows per lane (fronts of up to 160 rows)
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
@@ -541,14 +542,13 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
                const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, double *__restrict__ band_all,
                double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
-    constexpr int DSZ = KB * (KB + 1) + KB;
+    constexpr int DSZ = KB * KB + KB;
     constexpr int NW = NT / 32, NWW = NW - 1, NTW = NT - 32;      // warps, worker warps, worker threads
     static_assert(NW >= 2, "a pivot warp and at least one worker");
-    double *sDs = smem + 2 * DSZ;
-    double *sL = sDs + KB * KB;                  // sL[c][i] = -L(act[i], k0 + c)
+    double *sL = smem + 2 * DSZ;                 // sL[c][i] = -L(act[i], k0 + c)
     double *sU = sL + (size_t)KB * LDP;          // sU[c][j] = U(k0 + c, act[j])
     double *sW = sU + (size_t)KB * LDP;          // sW[i + j LDW] = A(act[i], act[j])
-    int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * na_max);
+    int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * na_max), *sActN = sAct + na_max;    // this step's list, the next one's
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
@@ -598,7 +598,7 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
 
     // prologue: first diagonal block (warp 0), first list and front (everybody)
     if (warp == 0) {
-        const double2 pv = factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * (KB + 1), lane, NT);
+        const double2 pv = factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * KB, lane, NT);
         pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
     }
     {
@@ -611,10 +611,10 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
     for (int k0 = 0, step = 0; k0 < n; k0 += KB, ++step) {
         const int kb = min(KB, n - k0), kbn = min(KB, n - k0 - kb);      // this block, the next one
         const int na = act_ptr[step + 1] - act_ptr[step];
-        double *sD = smem + cur * DSZ, *sDi = sD + KB * (KB + 1);
+        const double *sDs = smem + cur * DSZ, *sDi = sDs + KB * KB;     // the eliminated diagonal block (rows), 1 / pivots
+        const int nan = kbn > 0 ? act_ptr[step + 2] - act_ptr[step + 1] : 0;
         __syncthreads();                        // this step's front is gathered, its diagonal block eliminated
-        for (int t = tid; t < KB * KB; t += NT) sDs[t] = sD[(t / KB) * (KB + 1) + t % KB];
-        __syncthreads();
+        for (int i = tid; i < nan; i += NT) sActN[i] = act_idx[act_ptr[step + 1] + i];      // the next list, for the workers' gather
         // panel substitutions, one chain per thread: items [0, na) are rows of the L panel (x U11 = a, right-looking),
         // items [na, 2 na) columns of the U panel (L11 y = a, left-looking); sums in ascending index order
         for (int it = tid; it < 2 * na; it += NT) {
@@ -723,7 +723,7 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
             named_bar_arrive(1, NT);
             if (kbn > 0) {
                 double *sDn = smem + (cur ^ 1) * DSZ;
-                const double2 pv = factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * (KB + 1), lane, NT);
+                const double2 pv = factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * KB, lane, NT);
                 pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
             } else named_bar_arrive(2, NT);
         } else {
@@ -739,14 +739,14 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
                 for (int i = lane; i < na; i += 32)
                     if (i >= kbn || j >= kbn) colp[sAct[i]] = sW[i + (size_t)j * LDW];
             }
-            named_bar_sync(3, NTW);                                            // the workers have read sAct and written the band
-            const int nan = kbn > 0 ? act_ptr[step + 2] - act_ptr[step + 1] : 0;
-            for (int i = tid - 32; i < nan; i += NTW) sAct[i] = act_idx[act_ptr[step + 1] + i];
-            named_bar_sync(4, NTW);
+            named_bar_sync(3, NTW);                                            // the workers have written the band
             named_bar_sync(2, NT);                                             // warp 0 has its block out of the window
+            { int *t1 = sAct; sAct = sActN; sActN = t1; }
             if (kbn > 0) gather(k0 + kb, kbn, nan, tid - 32, NTW);
+            { int *t1 = sAct; sAct = sActN; sActN = t1; }
         }
         cur ^= 1;
+        { int *t1 = sAct; sAct = sActN; sActN = t1; }
     }
     if (pivots && tid == 0) {
         double *pv = pivots + 2 * ((size_t)(blockIdx.x / S) * pivS + blockIdx.x % S);
@@ -929,8 +929,8 @@ static int front_ldw(int na_max) { return ((std::max(na_max, 1) + 7) / 16) * 16 
 
 size_t band_front_smem(int bw, int na_max) {
     const int KB = band_block(bw);
-    return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + (size_t)KB * KB + 2 * (size_t)KB * band_mw(na_max) +
-                             (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(na_max + 2) / 2);
+    return sizeof(double) * (2 * ((size_t)KB * KB + KB) + 2 * (size_t)KB * band_mw(na_max) +
+                             (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(2 * na_max + 2) / 2);
 }
 
 template <int KB, int NT>
