@@ -274,7 +274,10 @@ def pair_sym_roof(rin, key, kname, pairs, ms, peak, probe, issue, mix_key=None):
     return fp64_roof("alu", kname, flop, pairs, ms, peak, probe, extra)
 
 
-def pair_kernel_name(N):
+def pair_kernel_name(N, latency=False):
+    """The per-problem pair kernel a context runs: latency tiling (contexts for fewer than 4 problems) or throughput tiling."""
+    if latency:
+        return "k_pair_sym<128,2>" if N >= 16384 else ("k_pair_sym<64,2>" if N >= 8192 else ("k_pair_split<2>" if N >= 2048 else "k_pair_split<4>"))
     return "k_pair_sym<128,2>" if N >= 4096 else ("k_pair_sym<64,2>" if N >= 2560 else ("k_pair_split<2>" if N >= 1536 else "k_pair_split<4>"))
 
 
@@ -303,9 +306,9 @@ def time_config(binding, inputs, torch, oracle, key, k, variant, nb_batched, rin
     except Exception as exc:   # reported, not fatal
         graph_ms = f"unavailable: {exc}"
     kname = pair_kernel_name(N)
-    out["single"] = {"path": "per-problem", "ms_per_build": ms, "graph_replay_ms_per_build": graph_ms, "builds_per_s": 1e3 / ms,
+    out["single"] = {"path": "per-problem (latency tiling)", "ms_per_build": ms, "graph_replay_ms_per_build": graph_ms, "builds_per_s": 1e3 / ms,
                      "gpair_per_s": pairs / (ms * 1e-3) * 1e-9,
-                     "roofline": pair_sym_roof(rin, key + ":single", kname, pairs, pk, peaks["fp64"], peaks["probe"], peaks["issue"])}
+                     "roofline": pair_sym_roof(rin, key + ":single", pair_kernel_name(N, True), pairs, pk, peaks["fp64"], peaks["probe"], peaks["issue"])}
     ctx.destroy()
     # --- batch, both paths --------------------------------------------------------------------------------------
     nb = nb_batched

@@ -102,7 +102,9 @@ typedef struct {
 /* Set-up, once per mesh: DOF numbering, constraint closure, CSR pattern, gather
  * lists, point arrays, tabulations; uploads them.  max_batch in [1, 65535] sizes the scratch arena for
  * landau_jacobian_batched and chooses the path through step a3 (LANDAU_PAIR_AUTO above).  Device scratch:
- *   per-problem path : chunk * (3 + 5 ceil(N/TS)) * N doubles, TS = 128 / 64 / 32 by N; a batch is processed in groups
+ *   per-problem path : chunk * (3 + 5 ceil(N/TS)) * N doubles, TS = 128 / 64 / 32 by N (max_batch < 4, a context for
+ *                      single builds: 32 up to N = 8,192 -- more, shorter blocks balance one build over the SMs -- which
+ *                      is why results of contexts with different max_batch may differ in the last bits); a batch is processed in groups
  *                      of chunk = min(max_batch, 1 GB / (40 ceil(N/TS) N bytes)) >= 1 problems: at most ~1 GB whatever
  *                      the batch (139 problems per group at N = 4,928)
  *   batch-shared path: 40 N^2 bytes for the tensor (0.97 GB at N = 4,928) + max_batch * 5 (1 + ksplit) N doubles

@@ -101,6 +101,7 @@ struct landau_ctx {
     int pair_path = LANDAU_PAIR_PER_PROBLEM;   // resolved path (never LANDAU_PAIR_AUTO)
     int nbpad = 0;                   // batch-shared path: problems padded to whole tiles
     int pp_chunk = 1;                // per-problem path: problems per group (their slabs stay in L2)
+    bool latency_tiles = false;      // per-problem path: short tiles (context made for single builds, max_batch < LANDAU_SHARED_MIN_BATCH)
     bool tensor_cache = false;       // keep U between calls (the geometry of a ctx never changes)
     bool tensor_valid = false;
     int max_batch = 1;
@@ -183,8 +184,8 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
         const int nbc = std::min(ctx->pp_chunk, nb - b0);
         const double *fc = f_dev + size_t(b0) * ctx->fstride;
         for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nbc, fc + g.foff, ctx->sc.T, st);
-        ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->r, ctx->z, ctx->invr, ctx->check_all, nbc, ctx->sc.T, ctx->sc.G, st); });
-        ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N), ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
+        ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->latency_tiles, ctx->r, ctx->z, ctx->invr, ctx->check_all, nbc, ctx->sc.T, ctx->sc.G, st); });
+        ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N, ctx->latency_tiles), ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
     }
 }
 
@@ -199,8 +200,8 @@ void free_pair_scratch(landau_ctx *ctx) {
 // (Groups small enough for the slabs to stay in L2, 32 MB, were measured: the partial last wave of every pair-kernel
 // launch then costs more than the DRAM round trip of the slabs saves.)
 constexpr size_t PP_SLAB_BYTES = size_t(1) << 30;
-int pp_chunk_size(int max_batch, int64_t N) {
-    const size_t per_problem = size_t(pair_tiles(int(N))) * 5 * size_t(N) * sizeof(double);
+int pp_chunk_size(int max_batch, int64_t N, bool latency) {
+    const size_t per_problem = size_t(pair_tiles(int(N), latency)) * 5 * size_t(N) * sizeof(double);
     return int(std::max<size_t>(1, std::min<size_t>(size_t(max_batch), PP_SLAB_BYTES / std::max<size_t>(per_problem, 1))));
 }
 
@@ -223,9 +224,9 @@ int alloc_pair_scratch(landau_ctx *ctx, int path) {
                   {&ctx->sc.U, tensor_bytes(int64_t(N)) / sizeof(double), true},
                   {&ctx->sc.G, shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0, false}};
     } else {
-        ctx->pp_chunk = pp_chunk_size(ctx->max_batch, int64_t(N));
+        ctx->pp_chunk = pp_chunk_size(ctx->max_batch, int64_t(N), ctx->latency_tiles);
         const size_t nbc = size_t(ctx->pp_chunk);
-        allocs = {{&ctx->sc.T, nbc * 3 * N, false}, {&ctx->sc.G, nbc * pair_tiles(int(N)) * 5 * N, false}};
+        allocs = {{&ctx->sc.T, nbc * 3 * N, false}, {&ctx->sc.G, nbc * pair_tiles(int(N), ctx->latency_tiles) * 5 * N, false}};
     }
     for (auto &a : allocs) {
         if (!a.n) continue;
@@ -356,6 +357,7 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
     ctx->grids.resize(ngrids);
     ctx->S = S;
     ctx->max_batch = max_batch;
+    ctx->latency_tiles = max_batch < LANDAU_SHARED_MIN_BATCH;
     int rc = LANDAU_OK;
     for (int g = 0; g < ngrids; ++g) {
         std::string err;
@@ -497,7 +499,7 @@ int landau_pair_path(const landau_ctx *ctx, int32_t *path, int64_t *scratch_byte
             d = 3 * size_t(shared_kpad(int(N)) / 8) * ctx->nbpad * 8 + tensor_bytes(ctx->Ntot) / 8 +
                 (shared_ksplit(int(N)) > 1 ? nbm * shared_ksplit(int(N)) * 5 * N : 0);
         else
-            d = size_t(ctx->pp_chunk) * (3 * N + pair_tiles(int(N)) * 5 * N);
+            d = size_t(ctx->pp_chunk) * (3 * N + pair_tiles(int(N), ctx->latency_tiles) * 5 * N);
         *scratch_bytes = int64_t(d * sizeof(double));
     }
     return LANDAU_OK;

@@ -668,13 +668,20 @@ __global__ void k_issue_probe(int iters, const double *__restrict__ in, double *
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
-// Tile size of the pair kernel: a function of N ONLY (it fixes the summation order).
+// Tile size of the pair kernel: a function of N and of the context's tiling policy ONLY (it fixes the summation
+// order; the policy is fixed at landau_create, so inside a context a batched build equals single builds bitwise).
 // Small N is latency-bound (one warp walks its j tile step by step, ~700 cycles per step): short tiles give
 // more warps and fewer steps (N = 2048: 39 -> 31 us); large N is throughput-bound: two i per thread.
-int pair_tile_size(int N) { return N >= 4096 ? 128 : (N >= 2560 ? 64 : 32); }
-int pair_tiles(int N) { const int ts = pair_tile_size(N); return (N + ts - 1) / ts; }
-// Warps sharing a tile pair where the tiles are 32 points (k_pair_split): a function of N only, like the tile size.
-int pair_split_warps(int N) { return N < 1536 ? 4 : 2; }
+// latency = true (contexts created for fewer than LANDAU_SHARED_MIN_BATCH problems: single builds): 32-point tiles up to
+// N = 8,192 -- a single build of N = 4,928 is 780 blocks of 128-point tile pairs on 888 slots, under one wave with a
+// 5 : 6 imbalance between SMs; 11,935 short blocks balance (pair kernel 115 -> 101 us).
+int pair_tile_size(int N, bool latency) {
+    if (latency) return N >= 16384 ? 128 : (N >= 8192 ? 64 : 32);
+    return N >= 4096 ? 128 : (N >= 2560 ? 64 : 32);
+}
+int pair_tiles(int N, bool latency) { const int ts = pair_tile_size(N, latency); return (N + ts - 1) / ts; }
+// Warps sharing a tile pair where the tiles are 32 points (k_pair_split): a function of N and the policy, like the tile size.
+int pair_split_warps(int N, bool latency) { return N < (latency ? 2048 : 1536) ? 4 : 2; }
 
 int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
     dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
@@ -689,21 +696,21 @@ int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const dou
 }
 
 template <bool CHECK_ALL>
-static void launch_pair_t(int N, const double *r, const double *z, const double *invr, int nb, const double *T, double *Gpart,
+static void launch_pair_t(int N, bool latency, const double *r, const double *z, const double *invr, int nb, const double *T, double *Gpart,
                           cudaStream_t st) {
-    const int ts = pair_tile_size(N), nt = pair_tiles(N);
+    const int ts = pair_tile_size(N, latency), nt = pair_tiles(N, latency);
     dim3 grid(nt * (nt + 1) / 2, nb);
     const bool pdl = nb <= PDL_MAX_NB;
     if (ts == 128) launch_k(k_pair_sym<128, 2, CHECK_ALL>, grid, dim3(64), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
     else if (ts == 64) launch_k(k_pair_sym<64, 2, CHECK_ALL>, grid, dim3(32), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
-    else if (pair_split_warps(N) == 4) launch_k(k_pair_split<4, CHECK_ALL>, grid, dim3(128), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
+    else if (pair_split_warps(N, latency) == 4) launch_k(k_pair_split<4, CHECK_ALL>, grid, dim3(128), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
     else launch_k(k_pair_split<2, CHECK_ALL>, grid, dim3(64), 0, st, pdl, N, nt, r, z, invr, T, Gpart);
 }
 
-int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
+int launch_pair(int Ntot, bool latency, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
                 double *Gpart, cudaStream_t st) {
-    if (check_all) launch_pair_t<true>(Ntot, r, z, invr, nb, T, Gpart, st);
-    else launch_pair_t<false>(Ntot, r, z, invr, nb, T, Gpart, st);
+    if (check_all) launch_pair_t<true>(Ntot, latency, r, z, invr, nb, T, Gpart, st);
+    else launch_pair_t<false>(Ntot, latency, r, z, invr, nb, T, Gpart, st);
     return 1;
 }
 

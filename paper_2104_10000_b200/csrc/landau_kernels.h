@@ -57,7 +57,8 @@ int launch_pair_tensor(int N, const double *r, const double *z, const double *in
 int launch_apply(int N, int nb, int nbpad, const double *U, const double *T, double *Gpart, cudaStream_t st);
 // pair kernel over the union of points (r, z, invr: [Ntot]); check_all: test every pair for coincidence
 // (needed only when points of different grids coincide), else only the diagonal tiles
-int launch_pair(int Ntot, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
+// latency: the tiling policy of the context (pair_tile_size)
+int launch_pair(int Ntot, bool latency, const double *r, const double *z, const double *invr, bool check_all, int nb, const double *T,
                 double *Gpart, cudaStream_t st);
 // Ez == nullptr: collision Jacobian C_e; else the implicit-step operator shift M + A_E - J (Ez[nb] device)
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce,
@@ -119,7 +120,7 @@ size_t band_solve_smem(int n, int bw);
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
                               double *x, double *xg, cudaStream_t st);
 
-int pair_tile_size(int N);
-int pair_tiles(int N);
+int pair_tile_size(int N, bool latency);
+int pair_tiles(int N, bool latency);
 
 }  // namespace landau

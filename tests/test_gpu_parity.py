@@ -16,7 +16,18 @@ from paper_2104_10000_b200 import inputs
 pytestmark = pytest.mark.gpu
 TOL = 1e-10
 PER, SHARED = 1, 2          # LANDAU_PAIR_PER_PROBLEM, LANDAU_PAIR_SHARED
-PATHS = [pytest.param(PER, id="per-problem"), pytest.param(SHARED, id="shared")]
+PER_BATCH = 3               # (tests only) LANDAU_PAIR_PER_PROBLEM in a context made for >= 4 problems: the per-problem pair
+                            # kernel then runs with its throughput tiling (k_pair_sym<64,2> / <128,2> from N = 2,560 / 4,096),
+                            # in a context for fewer with the latency tiling (k_pair_split up to N = 8,192)
+PATHS = [pytest.param(PER, id="per-problem"), pytest.param(PER_BATCH, id="per-problem-batch-tiles"), pytest.param(SHARED, id="shared")]
+
+
+PATHS_BATCH = [pytest.param(PER, id="per-problem"), pytest.param(SHARED, id="shared")]      # contexts for >= 4 problems anyway
+
+
+def ctx_args(path, nb):
+    """(max_batch, pair_path) of a context that builds nb problems on `path`."""
+    return (max(nb, 4), PER) if path == PER_BATCH else (nb, path)
 
 
 @pytest.fixture(scope="module")
@@ -50,7 +61,8 @@ def conservation_residuals(dof_r, dof_z, mass, Cf):
 
 def run_gpu(gpu, wl, problems, max_batch=None, batched=True, path=0):
     import torch
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, max_batch or len(problems), pair_path=path)
+    mb, path = ctx_args(path, max_batch or len(problems))
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, mb, pair_path=path)
     if path:
         assert ctx.pair_path()[0] == path
     r, z = ctx.dof_coords()
@@ -181,7 +193,8 @@ def test_multigrid_parity(gpu, oracle, which, path):
     grids); 'paper3' is Table I's three 20-cell grids with ten species (960 points, 1,930 equations)."""
     import torch
     name, order, meshes, spc, sgrid, comps = _multigrid_case(which)
-    ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, 2)
+    mb, path = ctx_args(path, 2)
+    ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, mb)
     ctx.set_pair_path(path)
     assert ctx.pair_path()[0] == path
     if which == "same2-q3-80":
@@ -452,7 +465,8 @@ def test_inner_integral_parity(gpu, oracle, which, path):
     (ragged last chunk of 16 source points, ragged target tile, 1 / 2 / 4 splits of the source range)."""
     import torch
     wl = _inner_case(which)
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 1, pair_path=path)
+    mb, path = ctx_args(path, 1)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, mb, pair_path=path)
     r, z = ctx.dof_coords()
     f = inputs.nodal_f(wl, r, z)
     G = torch.zeros((1, 5, ctx.N), dtype=torch.float64, device="cuda")
@@ -467,7 +481,7 @@ def test_inner_integral_parity(gpu, oracle, which, path):
         assert block_err(G[c], ref[c]) <= 1e-12, c
 
 
-@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("path", PATHS_BATCH)
 def test_config5_batched_full_size(gpu, oracle, path):
     """BASELINE config 5 at full size (512 problems, the launch shape bench.py times): sampled
     problems against the oracle one by one; conservation (holds at any size) on all 512."""
@@ -497,7 +511,7 @@ def test_config5_batched_full_size(gpu, oracle, path):
             assert block_err(Cf[k, a], oCf[a]) <= TOL, (k, a)
 
 
-@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("path", PATHS_BATCH)
 @pytest.mark.parametrize("cfg,variant,nb", [(1, "B", 8192), (2, "B", 512), (3, "A", 1024)])
 def test_per_config_batches_of_the_bench_at_full_size(gpu, oracle, cfg, variant, nb, path):
     """The batched launches bench.py times for configs 1, 2 and 3A (`per_config[*].batched`: 8,192 / 512 / 1,024 problems,
@@ -506,7 +520,8 @@ def test_per_config_batches_of_the_bench_at_full_size(gpu, oracle, cfg, variant,
     against the oracle one by one."""
     import torch
     wl = inputs.config(cfg, variant=variant)
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, nb, pair_path=path)
+    mb, path = ctx_args(path, nb)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, mb, pair_path=path)
     r, z = ctx.dof_coords()
     f0 = inputs.nodal_f(wl, r, z)
     S = wl.species.S
@@ -530,7 +545,7 @@ def test_per_config_batches_of_the_bench_at_full_size(gpu, oracle, cfg, variant,
             assert block_err(Cf_h[k, a], oCf[a]) <= TOL, (k, a)
 
 
-@pytest.mark.parametrize("path", PATHS)
+@pytest.mark.parametrize("path", PATHS_BATCH)
 def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu, path):
     """Inside one path a problem's result does not depend on the batch it is built in: 24 problems in one call,
     again, one by one, and (other tile shapes of the shared path's contraction) in calls of 17 + 7."""
@@ -542,7 +557,7 @@ def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu, path):
     _, _, v3, c3, _ = run_gpu(gpu, wl, problems, batched=False, path=path)
     assert np.array_equal(v1, v2) and np.array_equal(c1, c2)      # run-to-run determinism
     assert np.array_equal(v1, v3) and np.array_equal(c1, c3)      # batch shape == split shape, bitwise
-    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 24, pair_path=path)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 24, pair_path=ctx_args(path, 24)[1])
     r, z = ctx.dof_coords()
     fd = torch.from_numpy(np.stack([inputs.nodal_f(wl, r, z, b) for b in problems])).cuda()
     v4 = torch.zeros((24, ctx.S, ctx.nnz), dtype=torch.float64, device="cuda")
