@@ -711,15 +711,39 @@ def summarise_ncu(paths, plan_file):
                 seq[hit].append(r)
             elif "landau::" in name or name.startswith("k_") or " k_" in name:
                 rest.setdefault("rest", []).append(r)
+        pct_cols = [c for c in cols if c.endswith("_pct")]
         for kern, lst in seq.items():
             entries = [e for e in plan["plan"] if (kern == "k_pair_sym") == (not e["workload"].endswith(":shared") and e["workload"] != "cfg5:main")]
-            for r, e in zip(lst, entries):
+            pos = 0
+            for e in entries:
+                if pos >= len(lst):
+                    break
+                # the per-problem path sends a batch through its pair kernel in groups of problems (grid.y = problems of the
+                # launch): the launches of one plan entry are added up (counters summed, percentages weighted by time)
+                grp, seen = [], 0
+                while pos < len(lst) and (not grp or (kern == "k_pair_sym" and seen < e["problems"])):
+                    r = lst[pos]; pos += 1
+                    grp.append(r)
+                    try:
+                        seen += int(r["Grid Size"].strip("() ").split(",")[1])
+                    except Exception:
+                        seen = e["problems"]
                 upl = e["tensor_pairs_per_launch"] if kern == "k_pair_tensor" else e["pairs_per_launch"]
-                inst = r["Kernel Name"].split("(")[0].replace("landau::", "").replace("void ", "").replace(" ", "").replace(",", ";")
-                w.writerow([kern, e["workload"], sha, upl] + [val(r, NCU_COLS[c]) for c in cols] + [inst])
+                inst = grp[0]["Kernel Name"].split("(")[0].replace("landau::", "").replace("void ", "").replace(" ", "").replace(",", ";")
+                tsum = sum((val(r, NCU_COLS["time_ns"]) or 0.0) for r in grp) or 1.0
+                out = []
+                for c in cols:
+                    vs = [(val(r, NCU_COLS[c]), val(r, NCU_COLS["time_ns"]) or 0.0) for r in grp]
+                    if any(v is None for v, _ in vs):
+                        out.append(None)
+                    elif c in pct_cols:
+                        out.append(sum(v * t for v, t in vs) / tsum)
+                    else:
+                        out.append(sum(v for v, _ in vs))
+                w.writerow([kern, e["workload"], sha, upl] + out + [inst + (f" x{len(grp)} launches" if len(grp) > 1 else "")])
         if rest.get("rest") and plan["kernel_run"] == "main":
-            # the other kernels of the FIRST step (shared path): summed
-            n_first = len(rest["rest"]) // 2
+            # the other kernels of the FIRST step (shared path: everything before the per-problem step's k_fields_beta<0>): summed
+            n_first = next((i for i, r in enumerate(rest["rest"]) if "k_fields_beta<0>" in r["Kernel Name"].replace("(bool)", "").replace(" ", "")), len(rest["rest"]) // 2)
             tot = {c: sum((val(r, NCU_COLS[c]) or 0.0) for r in rest["rest"][:n_first]) for c in cols}
             w.writerow(["rest", "cfg5:main", sha, plan["plan"][0]["pairs_per_launch"]] + [tot[c] for c in cols] + ["all other kernels of the step"])
 
