@@ -9,6 +9,7 @@
 
 #include <algorithm>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -433,6 +434,19 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             std::vector<int32_t> act_ptr, act_idx;
             G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &G.bs.front_flop);
             if (act_idx.empty()) act_idx.push_back(0);
+            {
+                std::vector<int32_t> act_slot, slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src;
+                band_slot_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, band_front_ldw(G.bs.na_max), act_ptr, act_idx, G.bs.na_max, act_slot,
+                                slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src);
+                if (slot_hi.empty()) slot_hi.push_back(0);
+                UPC(G.bs.slot_hi, slot_hi)
+                if (act_slot.empty()) act_slot.push_back(0);
+                if (new_pos.empty()) new_pos.push_back(0);
+                if (ld_dst.empty()) { ld_dst.push_back(0); ld_src.push_back(0); }
+                UPC(G.bs.act_slot, act_slot) UPC(G.bs.new_ptr, new_ptr) UPC(G.bs.new_pos, new_pos)
+                UPC(G.bs.ld_ptr, ld_ptr) UPC(G.bs.ld_dst, ld_dst) UPC(G.bs.ld_src, ld_src)
+                G.bs.slot = band_block(bw) == 16 && band_slot_smem(bw, G.bs.na_max) <= size_t(225) * 1024;
+            }
             UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
             G.front_fits = band_front_smem(bw, G.bs.na_max) <= size_t(225) * 1024 && G.bs.na_max <= 160 && band_block(bw) >= 16;   // + 1 KB the driver reserves per block; FRONT_IR rows per lane
             // AUTO: the front kernel pays a gather and a scatter of its window per block step; it wins where the envelope

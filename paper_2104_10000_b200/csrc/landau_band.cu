@@ -14,6 +14,7 @@
 #include <cuda_runtime.h>
 
 #include <algorithm>
+#include <functional>
 #include <cmath>
 #include <cstdint>
 #include <queue>
@@ -481,12 +482,15 @@ __device__ __forceinline__ void named_bar_arrive(int id, int nthreads) { asm vol
 // Not inlined: compiled on its own the rows stay in registers (inlined into the front kernel they went to the stack).
 template <int KB, int SIGNAL>
 __device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, double *Aout, size_t lda, int kb, double *sD, double *sDi,
-                                                int lane, int nthreads) {
+                                                int lane, int nthreads, const int *ps = nullptr) {
+    // ps != nullptr: block entry (r, c) is src[ps[r] + ps[c] lds] (rows / columns of the block by their window slots)
     double r[KB];
     double pmin = 1.79e308, pmax = 0.0;
     const int row = min(lane, KB - 1);
+    const int myoff = (ps && lane < kb) ? ps[row] : row;
 #pragma unroll
-    for (int c = 0; c < KB; ++c) r[c] = (lane < kb && c < kb) ? src[row + (size_t)c * lds] : (lane == c ? 1.0 : 0.0);
+    for (int c = 0; c < KB; ++c)
+        r[c] = (lane < kb && c < kb) ? src[myoff + (size_t)((ps && c < kb) ? ps[c] : c) * lds] : (lane == c ? 1.0 : 0.0);
     if (SIGNAL > 0) {
         double keep = 0.0;                 // the loads above must have RETURNED before the barrier lets others overwrite src
 #pragma unroll
@@ -754,6 +758,255 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
     }
 }
 
+// ------------------------------------------------------------------------------------------------
+// Slot kernel: the front kernel with a window that never moves.  Every active row owns a slot (band_slot_lists) -- its
+// row and column of sW, its column of sL / sU -- so per block step
+//   all      panel substitutions over the active rows; rank-KB update of ALL NS x NS slots on the FP64 tensor cores (free
+//            slots hold zero panels: their window entries are garbage nobody reads)
+//   warp 0   takes the next diagonal block out of the window by the slots of the next block's rows and eliminates it
+//   workers  meanwhile: the next step's raw panels ARE the window's columns / rows at those pivot slots (shared memory
+//            to shared memory); the pivot slots are freed; the rows that ENTER are assembled into free slots: slot row and
+//            column zeroed, their original entries read from the band by the step's load list (~50 per row)
+// Window entries leave only as L and U, written to the band by the substitutions: no scatter, no gather of the window.
+// Shared memory (doubles): 2 x (sD[KB][KB], sDi[KB]), sL[KB][LDP], sU[KB][LDP], sW[NS][LDW], then 5 NS ints.
+// Named barriers: 2 = warp 0 has the block out of the window, 3 / 4 / 5 = among the workers.
+// ------------------------------------------------------------------------------------------------
+constexpr int SLOT_LB = 8;                     // band loads a worker thread keeps in flight when it assembles entering rows
+template <int KB, int NT>
+__global__ void __launch_bounds__(NT)
+k_slot_factor(int n, int bw, int LDP, int LDW, int NS, size_t mat_doubles, size_t pstride, int S,
+              const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, const int32_t *__restrict__ act_slot,
+              const int32_t *__restrict__ slot_hi, const int32_t *__restrict__ new_ptr, const int32_t *__restrict__ new_pos, const int32_t *__restrict__ ld_ptr,
+              const int32_t *__restrict__ ld_dst, const int32_t *__restrict__ ld_src, double *__restrict__ band_all,
+              double *__restrict__ pivots, int pivS) {
+    extern __shared__ double smem[];
+    constexpr int DSZ = KB * KB + KB;
+    constexpr int NW = NT / 32, NTW = NT - 32;
+    static_assert(NW >= 2, "a pivot warp and at least one worker");
+    double *sL = smem + 2 * DSZ;                 // sL[c][slot] = -L(row of slot, k0 + c)
+    double *sU = sL + (size_t)KB * LDP;          // sU[c][slot] = U(k0 + c, row of slot)
+    double *sW = sU + (size_t)KB * LDP;          // sW[slot_i + slot_j LDW] = A(row_i, row_j)
+    int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * NS), *sSlot = sAct + NS;      // this step's list: global row, slot
+    int *sActN = sSlot + NS, *sSlotN = sActN + NS, *sNew = sSlotN + NS;                   // the next step's; positions of its entering rows
+    const int W = band_halfwidth(bw, KB);
+    const size_t lda = 2 * (size_t)W;
+    double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
+    const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+    const int g = lane >> 2, k = lane & 3;
+    double pmin = 1.79e308, pmax = 0.0;
+
+    // assembly of the rows entering at `step` by the threads t = 0 .. nt-1 (list and slots of that step in la / ls, the
+    // positions of the entering rows in ln): slot rows / columns zeroed, (after the caller's barrier) original entries loaded
+    auto zero_new = [&](int nnew, const int *ls, const int *ln, int t, int nt) {
+        for (int e = t; e < nnew * NS; e += nt) {
+            const int sn = ls[ln[e / NS]], o = e % NS;
+            sW[sn + (size_t)o * LDW] = 0.0;
+            sW[o + (size_t)sn * LDW] = 0.0;
+        }
+    };
+    auto load_new = [&](int step, int t, int nt) {
+        const int e0 = ld_ptr[step], e1 = ld_ptr[step + 1];
+        for (int e = e0 + t; e < e1; e += SLOT_LB * nt) {
+            double v[SLOT_LB];
+            int d[SLOT_LB];
+#pragma unroll
+            for (int q = 0; q < SLOT_LB; ++q) {
+                const int eq = e + q * nt;
+                d[q] = eq < e1 ? ld_dst[eq] : -1;
+                v[q] = eq < e1 ? A[ld_src[eq]] : 0.0;
+            }
+#pragma unroll
+            for (int q = 0; q < SLOT_LB; ++q)
+                if (d[q] >= 0) sW[d[q]] = v[q];
+        }
+    };
+    // raw panels of the step whose block starts at k0 (kb columns): thread per list position; carried rows from the
+    // window's pivot columns / rows (slots in ps), entering rows from the band; all loads of a row before its stores
+    auto raw_panels = [&](int k0, int kb, int na, const int *la, const int *ls, const int *ps, const int *ln, int nnew, int t, int nt) {
+        for (int i = t; i < na; i += nt) {
+            const int gi = la[i], sl = ls[i];
+            bool isnew = ps == nullptr;
+            for (int q = 0; q < nnew; ++q) isnew |= ln[q] == i;
+#pragma unroll 1
+            for (int side = 0; side < 2; ++side) {          // the L row, then the U column: KB staging registers at a time
+                double pa[KB];
+                if (isnew) {
+                    const double *src = side == 0 ? A + gi + (size_t)k0 * lda : A + k0 + (size_t)gi * lda;
+                    const size_t st = side == 0 ? lda : 1;
+#pragma unroll
+                    for (int c = 0; c < KB; ++c) pa[c] = c < kb ? src[(size_t)c * st] : 0.0;
+                } else {
+#pragma unroll
+                    for (int c = 0; c < KB; ++c) {
+                        const int pc = ps[min(c, kb - 1)];
+                        pa[c] = c < kb ? (side == 0 ? sW[sl + (size_t)pc * LDW] : sW[pc + (size_t)sl * LDW]) : 0.0;
+                    }
+                }
+                double *pan = side == 0 ? sL : sU;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) pan[(size_t)c * LDP + sl] = pa[c];
+            }
+        }
+    };
+
+    // prologue: first diagonal block (warp 0); everything zero, then the first front assembled from the band
+    if (warp == 0) {
+        const double2 pv = factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * KB, lane, NT);
+        pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
+    }
+    {
+        const int na = act_ptr[1] - act_ptr[0], nnew = new_ptr[1] - new_ptr[0];
+        for (int i = tid; i < na; i += NT) { sAct[i] = act_idx[act_ptr[0] + i]; sSlot[i] = act_slot[act_ptr[0] + i]; }
+        for (int i = tid; i < nnew; i += NT) sNew[i] = new_pos[new_ptr[0] + i];
+        for (int i = tid; i < 2 * KB * LDP; i += NT) sL[i] = 0.0;                  // sL and sU are contiguous
+        for (int i = tid; i < LDW * NS; i += NT) sW[i] = 0.0;
+        __syncthreads();
+        raw_panels(0, min(KB, n), na, sAct, sSlot, nullptr, sNew, nnew, tid, NT);
+        load_new(0, tid, NT);
+    }
+    int cur = 0;
+    for (int k0 = 0, step = 0; k0 < n; k0 += KB, ++step) {
+        const int kb = min(KB, n - k0), kbn = min(KB, n - k0 - kb);      // this block, the next one
+        const int na = act_ptr[step + 1] - act_ptr[step];
+        const int hi = slot_hi[step];            // slots in use are below hi (the lowest free slot is taken first: hi ~ na)
+        const int nti = (hi + WT - 1) / WT, ntj = (hi + WTJ - 1) / WTJ, ntiles = nti * ntj;
+        const int a1 = act_ptr[step + 1], nan = kbn > 0 ? act_ptr[step + 2] - a1 : 0;     // the next step's list
+        const int nn0 = kbn > 0 ? new_ptr[step + 1] : 0, nnew = kbn > 0 ? new_ptr[step + 2] - nn0 : 0;
+        const double *sDs = smem + cur * DSZ, *sDi = sDs + KB * KB;     // the eliminated diagonal block (rows), 1 / pivots
+        __syncthreads();                        // this step's front is in place, its diagonal block eliminated
+        for (int i = tid; i < nan; i += NT) { sActN[i] = act_idx[a1 + i]; sSlotN[i] = act_slot[a1 + i]; }
+        for (int i = tid; i < nnew; i += NT) sNew[i] = new_pos[nn0 + i];
+        // panel substitutions, one chain per thread: items [0, na) are rows of the L panel (x U11 = a, right-looking),
+        // items [na, 2 na) columns of the U panel (L11 y = a, left-looking); sums in ascending index order
+        for (int it = tid; it < 2 * na; it += NT) {
+            const bool isL = it < na;
+            const int pos = isL ? it : it - na;
+            const int gi = sAct[pos], i = sSlot[pos];
+            double x[KB];
+            double *pan = isL ? sL : sU;
+#pragma unroll
+            for (int c = 0; c < KB; ++c) x[c] = pan[(size_t)c * LDP + i];
+            if (isL) {
+#pragma unroll
+                for (int t = 0; t < KB; ++t) {
+                    const double *drow = sDs + t * KB;
+                    x[t] *= sDi[t];
+                    const double xt = -x[t];
+                    if ((t + 1) < KB && ((t + 1) & 1)) x[t + 1] = fma(xt, drow[t + 1], x[t + 1]);
+#pragma unroll
+                    for (int c = (t + 2) & ~1; c < KB; c += 2) {
+                        const double2 u = *reinterpret_cast<const double2 *>(drow + c);
+                        x[c] = fma(xt, u.x, x[c]);
+                        x[c + 1] = fma(xt, u.y, x[c + 1]);
+                    }
+                }
+                double *row = A + gi + (size_t)k0 * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    if (c < kb) __stcs(row + (size_t)c * lda, x[c]);
+                    sL[(size_t)c * LDP + i] = -x[c];
+                }
+            } else {
+#pragma unroll
+                for (int t = 0; t < KB; ++t) {
+                    const double *drow = sDs + t * KB;
+                    double w = x[t];
+#pragma unroll
+                    for (int cc = 0; cc + 1 < t; cc += 2) {
+                        const double2 l = *reinterpret_cast<const double2 *>(drow + cc);
+                        w = fma(-l.x, x[cc], w);
+                        w = fma(-l.y, x[cc + 1], w);
+                    }
+                    if (t & 1) w = fma(-drow[t - 1], x[t - 1], w);
+                    x[t] = w;
+                }
+                double *col = A + k0 + (size_t)gi * lda;
+#pragma unroll
+                for (int c = 0; c < KB; ++c) {
+                    if (c < kb) __stcs(col + c, x[c]);
+                    sU[(size_t)c * LDP + i] = x[c];
+                }
+            }
+        }
+        __syncthreads();
+        // window update over all slots: sW += (-L)(U), warp tiles of 32 rows x 16 columns as in the band kernel
+        for (int wt = warp; wt < ntiles; wt += NW) {
+                const int i0 = (wt % nti) * WT, j0 = (wt / nti) * WTJ;
+                double acc[2][4][2];
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    const double *colp = sW + (size_t)j * LDW;
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < NS && i + 1 < NS) {
+                            const double2 v = *reinterpret_cast<const double2 *>(colp + i);
+                            acc[jb][ib][0] = v.x; acc[jb][ib][1] = v.y;
+                        } else {
+                            acc[jb][ib][0] = (j < NS && i < NS) ? colp[i] : 0.0;
+                            acc[jb][ib][1] = 0.0;
+                        }
+                    }
+                }
+#pragma unroll 4
+                for (int c0 = 0; c0 < KB; c0 += 4) {
+                    const double *pu = sU + (size_t)(c0 + k) * LDP + j0 + g;
+                    const double *pl = sL + (size_t)(c0 + k) * LDP + i0 + g;
+                    double fa[2], fb[4];
+#pragma unroll
+                    for (int t = 0; t < 2; ++t) fa[t] = pu[8 * t];
+#pragma unroll
+                    for (int t = 0; t < 4; ++t) fb[t] = pl[8 * t];
+#pragma unroll
+                    for (int jb = 0; jb < 2; ++jb)
+#pragma unroll
+                        for (int ib = 0; ib < 4; ++ib) dmma884(acc[jb][ib], fa[jb], fb[ib]);
+                }
+#pragma unroll
+                for (int jb = 0; jb < 2; ++jb) {
+                    const int j = j0 + 8 * jb + g;
+                    double *colp = sW + (size_t)j * LDW;
+#pragma unroll
+                    for (int ib = 0; ib < 4; ++ib) {
+                        const int i = i0 + 8 * ib + 2 * k;
+                        if (j < NS && i + 1 < NS) *reinterpret_cast<double2 *>(colp + i) = make_double2(acc[jb][ib][0], acc[jb][ib][1]);
+                        else if (j < NS && i < NS) colp[i] = acc[jb][ib][0];
+                    }
+                }
+        }
+        __syncthreads();
+        if (warp == 0) {
+            // the next block's rows are the first kbn of this step's list: its diagonal block by their slots
+            if (kbn > 0) {
+                double *sDn = smem + (cur ^ 1) * DSZ;
+                const double2 pv = factor_diag_src<KB, 2>(sW, LDW, A + (k0 + kb) + (size_t)(k0 + kb) * lda, lda, kbn, sDn, sDn + KB * KB, lane, NT, sSlot);
+                pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
+            } else named_bar_arrive(2, NT);
+        } else {
+            const int t = tid - 32;
+            // the pivot rows leave: their panel entries back to zero (free slots must hold zero panels) ...
+            for (int e = t; e < kbn * KB; e += NTW) {
+                const int sl = sSlot[e / KB], c = e % KB;
+                sL[(size_t)c * LDP + sl] = 0.0; sU[(size_t)c * LDP + sl] = 0.0;
+            }
+            named_bar_sync(4, NTW);             // ... before an entering row that takes such a slot writes its own
+            if (kbn > 0) raw_panels(k0 + kb, kbn, nan, sActN, sSlotN, sSlot, sNew, nnew, t, NTW);
+            named_bar_sync(3, NTW);             // the workers have read the pivot columns / rows of the window
+            named_bar_sync(2, NT);              // warp 0 has its block out of it
+            zero_new(nnew, sSlotN, sNew, t, NTW);
+            named_bar_sync(5, NTW);
+            if (kbn > 0) load_new(step + 1, t, NTW);
+        }
+        cur ^= 1;
+        { int *t1 = sAct; sAct = sActN; sActN = t1; t1 = sSlot; sSlot = sSlotN; sSlotN = t1; }
+    }
+    if (pivots && tid == 0) {
+        double *pv = pivots + 2 * ((size_t)(blockIdx.x / S) * pivS + blockIdx.x % S);
+        pv[0] = pmin; pv[1] = pmax;
+    }
+}
+
 // Banded triangular solves, one block per matrix: x = P^T U^-1 L^-1 P b with the RCM permutation.
 // Blocks of KB columns (those of the factorisation): the diagonal block by warp 0 (lane = row), the panel
 // below / above, confined to the envelope, by one thread per row with KB independent loads.
@@ -863,6 +1116,59 @@ int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vect
     return na_max;
 }
 
+// Host: lists of the slot kernel (k_slot_factor).  A row keeps ONE place (row and column index) in the shared-memory
+// window for as long as it is active -- a row that becomes a pivot row frees its slot, a row that enters takes the lowest
+// free one (na_max slots suffice: the pivot rows of a step have been taken out before that step's new rows arrive) -- so
+// the window is never re-packed and never travels.  Per block step s: act_slot (aligned with act_idx), new_pos (positions
+// in list s of the rows that ENTER at step s) and the load list of step s: the original entries (i, j) of the matrix
+// with i entering and j in list s (or both entering), as (offset in the window, offset in the band) -- the entering rows are
+// assembled sparsely, everything else of their rows / columns is zero.
+void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int bw, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
+                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src) {
+    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB, W = band_halfwidth(bw, KB);
+    const long long lda = 2LL * W;
+    std::vector<int32_t> pos(n);
+    for (int i = 0; i < n; ++i) pos[perm[i]] = i;
+    act_slot.assign(act_idx.size(), 0);
+    new_ptr.assign(nsteps + 1, 0); ld_ptr.assign(nsteps + 1, 0); slot_hi.assign(nsteps, 0);
+    new_pos.clear(); ld_dst.clear(); ld_src.clear();
+    std::vector<int32_t> slot_of(n, -1), entered(n, -1);
+    std::vector<int> free_slots;                          // kept sorted descending: pop_back gives the lowest
+    for (int k = na_max - 1; k >= 0; --k) free_slots.push_back(k);
+    for (int s = 0; s < nsteps; ++s) {
+        if (s > 0) {                                      // the rows of block s (the first entries of list s-1) have left
+            const int k0 = s * KB, ke = std::min(k0 + KB, n) - 1;
+            for (int i = k0; i <= ke; ++i)
+                if (slot_of[i] >= 0) { free_slots.push_back(slot_of[i]); slot_of[i] = -1; }
+            std::sort(free_slots.begin(), free_slots.end(), std::greater<int>());
+        }
+        for (int q = act_ptr[s]; q < act_ptr[s + 1]; ++q) {
+            const int i = act_idx[q];
+            if (slot_of[i] < 0) {
+                slot_of[i] = free_slots.back(); free_slots.pop_back();
+                entered[i] = s;
+                new_pos.push_back(q - act_ptr[s]);
+            }
+            act_slot[q] = slot_of[i];
+            slot_hi[s] = std::max(slot_hi[s], slot_of[i] + 1);
+        }
+        new_ptr[s + 1] = int32_t(new_pos.size());
+        for (int t = new_ptr[s]; t < new_ptr[s + 1]; ++t) {
+            const int i = act_idx[act_ptr[s] + new_pos[t]], io = perm[i], si = slot_of[i];
+            for (int u = rowptr[io]; u < rowptr[io + 1]; ++u) {
+                const int j = pos[colidx[u]];
+                if (slot_of[j] < 0) continue;            // not in this step's list: eliminated, in the block, or not yet active
+                // (i, j) and, unless j enters at this step too (its own pass covers it), (j, i)
+                ld_dst.push_back(int32_t(si + slot_of[j] * ldw)); ld_src.push_back(int32_t(i + j * lda));
+                if (entered[j] != s) { ld_dst.push_back(int32_t(slot_of[j] + si * ldw)); ld_src.push_back(int32_t(j + i * lda)); }
+            }
+        }
+        ld_ptr[s + 1] = int32_t(ld_dst.size());
+    }
+}
+
 // ------------------------------------------------------------------------------------------------
 // launchers
 // ------------------------------------------------------------------------------------------------
@@ -943,7 +1249,30 @@ static cudaError_t front_t(const BandSpace &bs, int nmat, int S, size_t pstride,
     return cudaGetLastError();
 }
 
+int band_front_ldw(int na_max) { return front_ldw(na_max); }
+
+size_t band_slot_smem(int bw, int na_max) {
+    const int KB = band_block(bw);
+    return sizeof(double) * (2 * ((size_t)KB * KB + KB) + 2 * (size_t)KB * band_mw(na_max) +
+                             (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(5 * na_max + 2) / 2);
+}
+
+template <int KB, int NT>
+static cudaError_t slot_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+    const size_t smem = band_slot_smem(bs.bw, bs.na_max);
+    cudaError_t e = cudaFuncSetAttribute(k_slot_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
+    if (e != cudaSuccess) return e;
+    k_slot_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
+                                                  pstride, S, bs.act_ptr, bs.act_idx, bs.act_slot, bs.slot_hi, bs.new_ptr, bs.new_pos, bs.ld_ptr, bs.ld_dst,
+                                                  bs.ld_src, band, pivots, pivS);
+    return cudaGetLastError();
+}
+
 cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+    // the front family: 16-column blocks take the slot kernel (measured: ten-species 80-cell 9.1 -> 7.4 ms, mesh 3A 5.6 -> 4.3),
+    // 32-column blocks the gather / scatter kernel (config 5: 14.2 against 18.7 ms with slots -- its look-ahead of the next
+    // diagonal block and the smaller tile sweep outweigh the round trip of the window there)
+    if (bs.front && bs.slot && band_block(bs.bw) == 16) return slot_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
     if (bs.front) {
         switch (band_block(bs.bw)) {
             case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);

@@ -90,6 +90,9 @@ struct BandSpace {
     int na_max;
     double front_flop;         // window-update flop of one factorisation by the front kernel (2 KB sum na_s^2)
     bool front;
+    // slot kernel (band_slot_lists): slot of every list entry, entering rows per step, load list of the entering rows
+    const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_src;   // slot_hi[s]: slots in use at step s are below it
+    bool slot;
     const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
@@ -110,6 +113,12 @@ void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
 // active lists of the front factorisation (see BandSpace); returns the longest list
 int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
                       int bw, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop);
+void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
+                     int bw, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
+                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src);
+int band_front_ldw(int na_max);
+size_t band_slot_smem(int bw, int na_max);
 size_t band_front_smem(int bw, int na_max);     // dynamic shared memory of the front kernel
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st);
