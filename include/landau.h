@@ -222,7 +222,8 @@ int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, 
 /* Two kernels factor the band, with the same storage and the same L, U up to rounding order:
  *   LANDAU_BAND_FRONT  gathers, per block step, only the rows / columns inside the ENVELOPE of the ordered pattern (LU
  *                      without pivoting keeps it; on the refined meshes a third of the rows a band step spans) into a
- *                      dense front in shared memory, eliminates there and scatters back;
+ *                      dense front in shared memory, eliminates there and scatters back (32-column blocks), or keeps the
+ *                      front in shared memory for its whole life, every active row in a fixed slot (16-column blocks);
  *   LANDAU_BAND_HULL   updates the whole window of a block step in place (the monotone hull of the envelope).
  * LANDAU_BAND_AUTO (the default) takes the front kernel whenever the largest front fits the shared memory of an SM.
  * landau_band_set_method returns LANDAU_EINVAL for LANDAU_BAND_FRONT when it does not fit; landau_band_method reports
