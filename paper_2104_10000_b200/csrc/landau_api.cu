@@ -430,6 +430,13 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             G.bs.flop_per_matrix = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow, &mup);
             band_fill_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, mlow, mup, zlo, zcnt, fptr, fsrc, foff);
             UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
+            {
+                std::vector<int32_t> pos(hs.n), first(hs.n);
+                for (int64_t i = 0; i < hs.n; ++i) { pos[perm[i]] = int32_t(i); first[i] = int32_t(i); }
+                for (int64_t i = 0; i < hs.n; ++i)
+                    for (int t = hs.rowptr[i]; t < hs.rowptr[i + 1]; ++t) first[pos[i]] = std::min(first[pos[i]], pos[hs.colidx[t]]);
+                UPC(G.bs.first, first)
+            }
             UPC(G.bs.zlo, zlo) UPC(G.bs.zcnt, zcnt) UPC(G.bs.fptr, fptr) UPC(G.bs.fsrc, fsrc) UPC(G.bs.foff, foff)
             std::vector<int32_t> act_ptr, act_idx;
             G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &G.bs.front_flop);

@@ -1016,12 +1016,16 @@ k_slot_factor(int n, int bw, int LDP, int LDW, int NS, size_t mat_doubles, size_
 template <int KB, int NT, bool XG>
 __global__ void __launch_bounds__(NT)
 k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
-             const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, size_t pstride, const double *__restrict__ band_all,
-             const double *rhs, double *xout, double *xg) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
+             const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const int32_t *__restrict__ first, size_t pstride,
+             const double *__restrict__ band_all, const double *rhs, double *xout, double *xg) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
+    // first[i]: the column of row i's first entry in the ordered pattern = the row of column i's first entry (the
+    // pattern is structurally symmetric).  L and U vanish outside the envelope -- L(i, j) for j < first[i], U(i, j) for
+    // i < first[j] -- so those entries are not read: on the refined meshes two thirds of what a block step's panels span.
     constexpr int SB = KB;            // same blocks as the factorisation: panels stay inside the stored band
     extern __shared__ double smem[];
     double *x = XG ? xg + (size_t)blockIdx.x * n : smem;    // [n]
     double *sD = XG ? smem : smem + n;                      // [SB][SB+1]
+    int *sF = reinterpret_cast<int *>(sD + SB * (SB + 1));  // [SB] first rows of the current block's columns (backward sweep)
     const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     const int mat = blockIdx.x;       // = b * S + sp
@@ -1048,10 +1052,13 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
         }
         __syncthreads();
         for (int i = tid; i < m; i += NT) {
+            const int c0 = first[k0 + kb + i] - k0;                 // row entries left of this are zero (c0 >= kb: the whole row)
+            if (c0 >= kb) continue;
             const double *row = A + (k0 + kb + i) + (size_t)k0 * lda;
             double v = x[k0 + kb + i];
 #pragma unroll 8
-            for (int c = 0; c < kb; ++c) v = fma(-row[(size_t)c * lda], x[k0 + c], v);
+            for (int c = 0; c < kb; ++c)
+                if (c >= c0) v = fma(-row[(size_t)c * lda], x[k0 + c], v);
             x[k0 + kb + i] = v;
         }
         __syncthreads();
@@ -1064,6 +1071,7 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
             const int r = t % kb, c = t / kb;
             sD[r * (SB + 1) + c] = A[(k0 + r) + (size_t)(k0 + c) * lda];
         }
+        if (tid < SB) sF[tid] = tid < kb ? first[k0 + tid] : n;
         __syncthreads();
         if (warp == 0) {
             double v = lane < kb ? x[k0 + lane] : 0.0;
@@ -1080,7 +1088,8 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
             const double *row = A + r + (size_t)k0 * lda;
             double v = x[r];
 #pragma unroll 8
-            for (int c = 0; c < kb; ++c) v = fma(-row[(size_t)c * lda], x[k0 + c], v);
+            for (int c = 0; c < kb; ++c)
+                if (sF[c] <= r) v = fma(-row[(size_t)c * lda], x[k0 + c], v);     // U(r, k0 + c) is zero above the column's first row
             x[r] = v;
         }
         __syncthreads();
@@ -1291,21 +1300,21 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstr
 // bytes of shared memory the solve needs with the vector on chip
 size_t band_solve_smem(int n, int bw) {
     const int KB = band_block(bw);
-    return sizeof(double) * ((size_t)n + (size_t)KB * (KB + 1));
+    return sizeof(double) * ((size_t)n + (size_t)KB * (KB + 1) + KB / 2);
 }
 
 template <int KB, int NT>
 static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
                            double *x, double *xg, cudaStream_t st) {
     if (xg) {        // vector in global memory: only the diagonal block in shared memory
-        const size_t smem = sizeof(double) * KB * (KB + 1);
-        k_band_solve<KB, NT, true><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x, xg);
+        const size_t smem = sizeof(double) * (KB * (KB + 1) + KB / 2);
+        k_band_solve<KB, NT, true><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, bs.first, pstride, band, rhs, x, xg);
         return cudaGetLastError();
     }
     const size_t smem = band_solve_smem(bs.n, bs.bw);
     cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB, NT, false><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, pstride, band, rhs, x, nullptr);
+    k_band_solve<KB, NT, false><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, bs.first, pstride, band, rhs, x, nullptr);
     return cudaGetLastError();
 }
 

@@ -94,6 +94,7 @@ struct BandSpace {
     const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_src;   // slot_hi[s]: slots in use at step s are below it
     bool slot;
     const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
+    const int32_t *first;      // [n] device: first column of row i = first row of column i in the ordered pattern
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
 // order of the band LU: the cheapest (envelope work) of RCM from several starting nodes and the (z, r) sweep
