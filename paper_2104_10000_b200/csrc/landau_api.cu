@@ -167,7 +167,7 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
             ctx->tensor_valid = true;
             forked = true;
         }
-        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta_tiled(g.ds, nb, ctx->nbpad, f_dev + g.foff, ctx->sc.T, st);
+        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta_tiled(g.ds, nb, ctx->nbpad, f_dev + g.foff, ctx->sc.T, g.ce, st);
         if (forked) note_launch_error(cudaStreamWaitEvent(st, ctx->side_join, 0));
         else if (eval_tensor) {
             ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair_tensor(N, ctx->r, ctx->z, ctx->invr, ctx->sc.U, st); });
@@ -184,7 +184,7 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
     for (int b0 = 0; b0 < nb; b0 += ctx->pp_chunk) {
         const int nbc = std::min(ctx->pp_chunk, nb - b0);
         const double *fc = f_dev + size_t(b0) * ctx->fstride;
-        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nbc, fc + g.foff, ctx->sc.T, st);
+        for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nbc, fc + g.foff, ctx->sc.T, g.ce + size_t(b0) * g.ds.S * g.ds.Ne * g.ds.Nb, st);
         ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->latency_tiles, ctx->r, ctx->z, ctx->invr, ctx->check_all, nbc, ctx->sc.T, ctx->sc.G, st); });
         ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N, ctx->latency_tiles), ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
     }
@@ -415,6 +415,16 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         UPC(ds.rowptr, hs.rowptr) UPC(ds.colidx, hs.colidx)
         UPC(ds.gptr, hs.gptr) UPC(ds.gidx, hs.gidx) UPC(ds.gw, hs.gw)
         UPC(ds.cptr, hs.cptr) UPC(ds.cidx, hs.cidx) UPC(ds.cw, hs.cw)
+        {
+            auto heads = [](const std::vector<int32_t> &ptr, const std::vector<int32_t> &idx, const std::vector<double> &w) {
+                std::vector<GatherHead> h(ptr.size() - 1, GatherHead{0.0, 0, 0});       // an empty list adds 0 * src[0]
+                for (size_t k = 0; k + 1 < ptr.size(); ++k)
+                    if (ptr[k + 1] > ptr[k]) h[k] = GatherHead{w[ptr[k]], idx[ptr[k]], 0};
+                return h;
+            };
+            const std::vector<GatherHead> gh = heads(hs.gptr, hs.gidx, hs.gw), ch = heads(hs.cptr, hs.cidx, hs.cw);
+            UPC(ds.ghead, gh) UPC(ds.chead, ch)
+        }
         // band LU: order, half-bandwidth, envelope per block step, fill lists per band column
         std::vector<int32_t> perm;
         int bw = 0;

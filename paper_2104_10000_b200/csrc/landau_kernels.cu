@@ -277,7 +277,7 @@ constexpr int FIELD_EPB = 8;      // cells per block
 // one barrier, so that many independent list walks are in flight per SM.
 template <bool TILED>
 __global__ void __launch_bounds__(16 * FIELD_EPB)
-k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T) {
+k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T, double *__restrict__ uout) {
     pdl_prologue();
     __shared__ double s_tab[3][16][16];                     // [B, E0, E1][a][q]
     __shared__ double s_u[FIELD_EPB][MAX_SPECIES][16];      // u = P_e f of every species of the block's cells
@@ -297,6 +297,9 @@ k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, 
             double u = 0.0;
             for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
             s_u[threadIdx.y][sp][q] = u;
+            // u = P_e f is needed again by the element kernel (C_e u): kept in the element vector's own slots, which
+            // k_element_q3 reads before it overwrites them -- one coalesced load there instead of a second list walk
+            uout[(((size_t)b * ds.S + sp) * ds.Ne + e) * Nb + q] = u;
         }
     }
     __syncthreads();
@@ -434,17 +437,47 @@ __device__ __forceinline__ void dmma884(double (&c)[2], double a, double b) {
 
 constexpr int ELQ3_WARPS = 4;    // cells per block and round
 #ifndef ELQ3_ROUNDS
-#define ELQ3_ROUNDS 1              // cells per warp (1, 4, 8 measured alike: 0.41-0.42 ms)
+#define ELQ3_ROUNDS 4              // cells per warp in a large batch (the next cell's inputs are fetched while this one is multiplied)
 #endif
+#ifndef ELQ3_MIN_BLOCKS
+#define ELQ3_MIN_BLOCKS 4
+#endif
+// inputs of a cell, staged per warp in shared memory: G (5 x 16), w_out (16), u (S x 16), invJ (2)
+constexpr int ELQ3_ROUNDS_MIN_NB = 64;
+constexpr int ELQ3_IN_W = 80, ELQ3_IN_U = 96, ELQ3_IN_J = 96 + 16 * MAX_SPECIES, ELQ3_IN = ELQ3_IN_J + 2;
 
+__device__ __forceinline__ void cp_async8(double *dst_shared, const double *src) {
+    asm volatile("cp.async.ca.shared.global [%0], [%1], 8;" ::"r"((uint32_t)__cvta_generic_to_shared(dst_shared)), "l"(src) : "memory");
+}
+
+// One warp per cell, `rounds` cells one after the other (cell e_r = (blockIdx.x rounds + r) ELQ3_WARPS + warp).  The
+// kernel is bound by the latency of its loads (a cell is 2 us of them against 0.5 us of tensor work): the inputs of
+// cell r + 1 are copied asynchronously into the warp's second buffer while cell r is multiplied and stored.
 template <bool FULL>
-__global__ void __launch_bounds__(ELQ3_WARPS * 32)
-k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restrict__ Gsum, double *__restrict__ Ce,
-             double *__restrict__ ce, const double *__restrict__ Ez, double shift) {
+__global__ void __launch_bounds__(ELQ3_WARPS * 32, FULL ? 3 : ELQ3_MIN_BLOCKS)
+k_element_q3(DeviceSpace ds, int rounds, const double *__restrict__ Gsum, double *__restrict__ Ce, double *__restrict__ ce,
+             const double *__restrict__ Ez, double shift) {
     pdl_prologue();
+    __shared__ double s_in[ELQ3_WARPS][2][ELQ3_IN];
     const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
     const int b = blockIdx.y;
     const int k = lane & 3, g = lane >> 2;
+    const size_t ustep = (size_t)ds.Ne * 16;
+    // u = P_e f (hanging-node interpolation folded in) was left by k_fields_beta in the cell's element-vector slots; it
+    // is fetched before those slots are overwritten with C_e u below (this warp is the only one that touches them)
+    auto prefetch = [&](int e, int buf) {
+        double *dst = s_in[warp][buf];
+        const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
+        for (int t = lane; t < 80; t += 32) cp_async8(dst + t, G + (size_t)(t >> 4) * ds.Ntot + (t & 15));
+        if (lane < 16) cp_async8(dst + ELQ3_IN_W + lane, ds.w_out + e * 16 + lane);
+        else if (lane < 18) cp_async8(dst + ELQ3_IN_J + lane - 16, ds.invJ + 2 * e + lane - 16);
+        const double *ub = ce + ((size_t)b * ds.S * ds.Ne + e) * 16;
+        for (int t = lane; t < 16 * ds.S; t += 32) cp_async8(dst + ELQ3_IN_U + t, ub + (size_t)(t >> 4) * ustep + (t & 15));
+        asm volatile("cp.async.commit_group;" ::: "memory");
+    };
+    const int e_first = blockIdx.x * rounds * ELQ3_WARPS + warp;
+    if (e_first >= ds.Ne) return;
+    prefetch(e_first, 0);
     // tabulation entries (q = 4 ks + k, col = 8 t + g)
     double tB[4][2], tE0[4][2], tE1[4][2];
 #pragma unroll
@@ -456,103 +489,90 @@ k_element_q3(DeviceSpace ds, const double *__restrict__ f, const double *__restr
         }
     const double sgn = FULL ? -1.0 : 1.0;
     const double ezb = FULL ? Ez[b] : 0.0;
-    for (int round = 0; round < ELQ3_ROUNDS; ++round) {
-    const int e = (blockIdx.x * ELQ3_ROUNDS + round) * ELQ3_WARPS + warp;
-    if (e >= ds.Ne) return;
-    // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
-    const double ir = ds.invJ[2 * e], iz = ds.invJ[2 * e + 1];
-    // (summing the pair kernel's slabs here instead of in k_sum_partials was measured slower for every batch size)
-    const double *G = Gsum + (size_t)b * 5 * ds.Ntot + ds.poff + e * 16;
-    double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
-#pragma unroll
-    for (int ks = 0; ks < 4; ++ks) {
-        const int q = 4 * ks + k;
-        const double w = ds.w_out[e * 16 + q];
-        wq[ks] = w;
-        g0[ks] = ir * ir * w * G[q];
-        g1[ks] = ir * iz * w * G[ds.Ntot + q];
-        g2[ks] = iz * iz * w * G[2 * ds.Ntot + q];
-        g3[ks] = ir * w * G[3 * ds.Ntot + q];
-        g4[ks] = iz * w * G[4 * ds.Ntot + q];
-    }
-    // u = P_e f: lanes 0..15 gather their local node (hanging-node interpolation folded in).  The list of the node is
-    // the same for every species: its first four items are read once per cell, and the u of species sp + 1 is
-    // gathered while species sp is multiplied (the kernel is bound by the latency of these dependent loads).
-    int lt0 = 0, lt1 = 0, ld[4] = {0, 0, 0, 0};
-    double lwv[4] = {0.0, 0.0, 0.0, 0.0};
-    if (lane < 16) {
-        lt0 = ds.lptr[e * 16 + lane]; lt1 = ds.lptr[e * 16 + lane + 1];
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (lt0 + q < lt1) { ld[q] = ds.ldof[lt0 + q]; lwv[q] = ds.lw[lt0 + q]; }
-    }
-    auto gather_u = [&](int sp) {
-        double u = 0.0;
-        const double *fa = f + (size_t)b * ds.fstride + (size_t)sp * ds.n;
-#pragma unroll
-        for (int q = 0; q < 4; ++q)
-            if (lt0 + q < lt1) u = fma(lwv[q], fa[ld[q]], u);
-        for (int t = lt0 + 4; t < lt1; ++t) u = fma(ds.lw[t], fa[ds.ldof[t]], u);
-        return u;
-    };
-    double u_next = gather_u(0);
-    for (int sp = 0; sp < ds.S; ++sp) {
-        const double u = u_next;
-        if (sp + 1 < ds.S) u_next = gather_u(sp + 1);
-        const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
-        double acc[2][2][2] = {};       // [mt][nt][2]
-        double accM[2][2][2] = {};      // mass part (FULL), kept apart: the element vector excludes it
+    for (int round = 0; round < rounds; ++round) {
+        const int e = e_first + round * ELQ3_WARPS;
+        if (e >= ds.Ne) break;
+        const bool more = round + 1 < rounds && e + ELQ3_WARPS < ds.Ne;
+        if (more) {
+            prefetch(e + ELQ3_WARPS, (round + 1) & 1);
+            asm volatile("cp.async.wait_group 1;" ::: "memory");
+        } else {
+            asm volatile("cp.async.wait_group 0;" ::: "memory");
+        }
+        __syncwarp();
+        const double *in = s_in[warp][round & 1];
+        // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
+        // (summing the pair kernel's slabs here instead of in k_sum_partials was measured slower for every batch size)
+        const double ir = in[ELQ3_IN_J], iz = in[ELQ3_IN_J + 1];
+        double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks) {
-            const double drr = df * g0[ks], drz = df * g1[ks], dzz = df * g2[ks], kr = kf * g3[ks], kz = kf * g4[ks];
-            double X[2], Y[2];
+            const int q = 4 * ks + k;
+            const double w = in[ELQ3_IN_W + q];
+            wq[ks] = w;
+            g0[ks] = ir * ir * w * in[q];
+            g1[ks] = ir * iz * w * in[16 + q];
+            g2[ks] = iz * iz * w * in[32 + q];
+            g3[ks] = ir * w * in[48 + q];
+            g4[ks] = iz * w * in[64 + q];
+        }
+        for (int sp = 0; sp < ds.S; ++sp) {
+            const double u = in[ELQ3_IN_U + 16 * sp + (lane & 15)];
+            const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
+            double acc[2][2][2] = {};       // [mt][nt][2]
+            double accM[2][2][2] = {};      // mass part (FULL), kept apart: the element vector excludes it
 #pragma unroll
-            for (int t = 0; t < 2; ++t) {
-                X[t] = fma(drr, tE0[ks][t], fma(drz, tE1[ks][t], kr * tB[ks][t]));
-                Y[t] = fma(drz, tE0[ks][t], fma(dzz, tE1[ks][t], kz * tB[ks][t]));
-            }
+            for (int ks = 0; ks < 4; ++ks) {
+                const double drr = df * g0[ks], drz = df * g1[ks], dzz = df * g2[ks], kr = kf * g3[ks], kz = kf * g4[ks];
+                double X[2], Y[2];
 #pragma unroll
-            for (int mt = 0; mt < 2; ++mt)
-#pragma unroll
-                for (int nt = 0; nt < 2; ++nt) {
-                    dmma884(acc[mt][nt], tE0[ks][mt], X[nt]);
-                    dmma884(acc[mt][nt], tE1[ks][mt], Y[nt]);
+                for (int t = 0; t < 2; ++t) {
+                    X[t] = fma(drr, tE0[ks][t], fma(drz, tE1[ks][t], kr * tB[ks][t]));
+                    Y[t] = fma(drz, tE0[ks][t], fma(dzz, tE1[ks][t], kz * tB[ks][t]));
                 }
-            if (FULL) {
-                const double ca = wq[ks] * (ds.qm[sp] * ezb) * iz, cm = wq[ks] * shift;
 #pragma unroll
                 for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
                     for (int nt = 0; nt < 2; ++nt) {
-                        dmma884(acc[mt][nt], tB[ks][mt], ca * tE1[ks][nt]);
-                        dmma884(accM[mt][nt], tB[ks][mt], cm * tB[ks][nt]);
+                        dmma884(acc[mt][nt], tE0[ks][mt], X[nt]);
+                        dmma884(acc[mt][nt], tE1[ks][mt], Y[nt]);
                     }
-            }
-        }
-        // C fragment: lane holds rows a = 8 mt + g, columns b = 8 nt + 2 k + {0, 1}
-        const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
-        double *C = Ce + mat * 256;
-        double part[2] = {0.0, 0.0};
+                if (FULL) {
+                    const double ca = wq[ks] * (ds.qm[sp] * ezb) * iz, cm = wq[ks] * shift;
 #pragma unroll
-        for (int nt = 0; nt < 2; ++nt) {
-            const double u0 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k), u1 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k + 1);
+                    for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                        for (int nt = 0; nt < 2; ++nt) {
+                            dmma884(acc[mt][nt], tB[ks][mt], ca * tE1[ks][nt]);
+                            dmma884(accM[mt][nt], tB[ks][mt], cm * tB[ks][nt]);
+                        }
+                }
+            }
+            // C fragment: lane holds rows a = 8 mt + g, columns b = 8 nt + 2 k + {0, 1}
+            const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
+            double *C = Ce + mat * 256;
+            double part[2] = {0.0, 0.0};
+#pragma unroll
+            for (int nt = 0; nt < 2; ++nt) {
+                const double u0 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k), u1 = __shfl_sync(0xffffffffu, u, 8 * nt + 2 * k + 1);
+#pragma unroll
+                for (int mt = 0; mt < 2; ++mt) {
+                    part[mt] = fma(acc[mt][nt][0], u0, fma(acc[mt][nt][1], u1, part[mt]));
+                    double2 v;
+                    v.x = FULL ? acc[mt][nt][0] + accM[mt][nt][0] : acc[mt][nt][0];
+                    v.y = FULL ? acc[mt][nt][1] + accM[mt][nt][1] : acc[mt][nt][1];
+                    *reinterpret_cast<double2 *>(C + (8 * mt + g) * 16 + 8 * nt + 2 * k) = v;
+                }
+            }
 #pragma unroll
             for (int mt = 0; mt < 2; ++mt) {
-                part[mt] = fma(acc[mt][nt][0], u0, fma(acc[mt][nt][1], u1, part[mt]));
-                double2 v;
-                v.x = FULL ? acc[mt][nt][0] + accM[mt][nt][0] : acc[mt][nt][0];
-                v.y = FULL ? acc[mt][nt][1] + accM[mt][nt][1] : acc[mt][nt][1];
-                *reinterpret_cast<double2 *>(C + (8 * mt + g) * 16 + 8 * nt + 2 * k) = v;
+                part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 1);
+                part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 2);
+                if (k == 0) ce[mat * 16 + 8 * mt + g] = part[mt];
             }
         }
-#pragma unroll
-        for (int mt = 0; mt < 2; ++mt) {
-            part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 1);
-            part[mt] += __shfl_xor_sync(0xffffffffu, part[mt], 2);
-            if (k == 0) ce[mat * 16 + 8 * mt + g] = part[mt];
-        }
+        __syncwarp();       // the buffer is refilled two rounds on
     }
-    }   // round
 }
 
 // a8: element mass matrices, M_e[a][b] = shift sum_q w_out B_qa B_qb (L280).  grid = Ne.
@@ -567,26 +587,53 @@ __global__ void k_mass_element(DeviceSpace ds, double shift, double *__restrict_
 // a6 / a7: out[b][sp][k] = sum_{t in [ptr[k], ptr[k+1])} w[t] * src[(b*S+sp)*stride + idx[t]], fixed order
 // (owner computes; replaces the paper's atomic MatSetValues, L165-167).  grid = (ceil(K/256), ceil(S/2), nb);
 // problem b's outputs start at out + b*ostride.
-__global__ void k_gather(int K, int S, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
-                         const double *__restrict__ w, const double *__restrict__ src, double *__restrict__ out) {
+#ifndef GATHER_EPT
+#define GATHER_EPT 2               // outputs per thread (independent list walks in flight)
+#endif
+#ifndef GATHER_MIN_BLOCKS
+#define GATHER_MIN_BLOCKS 8
+#endif
+__global__ void __launch_bounds__(256, GATHER_MIN_BLOCKS)
+k_gather(int K, int S, size_t stride, size_t ostride, const int32_t *__restrict__ ptr, const int32_t *__restrict__ idx,
+         const double *__restrict__ w, const GatherHead *__restrict__ head, const double *__restrict__ src, double *__restrict__ out) {
     pdl_prologue();
-    const int k = blockIdx.x * blockDim.x + threadIdx.x;
-    if (k >= K) return;
     // the lists are the same for every species: one walk serves two species blocks (blockIdx.y = species pair)
     const int sp0 = 2 * blockIdx.y;
     const bool two = sp0 + 1 < S;
     const double *s0 = src + ((size_t)blockIdx.z * S + sp0) * stride;
     const double *s1 = s0 + (two ? stride : 0);
-    double acc0 = 0.0, acc1 = 0.0;
-    for (int t = ptr[k]; t < ptr[k + 1]; ++t) {
-        const double wt = w[t];
-        const int it = idx[t];
-        acc0 = fma(wt, s0[it], acc0);
-        acc1 = fma(wt, s1[it], acc1);
+    // the first item comes with the list bounds (GatherHead), the others -- cells sharing the entry, hanging-node
+    // interpolation -- from the list; same items in the same order as one walk of the list
+    int k[GATHER_EPT], t0[GATHER_EPT], t1[GATHER_EPT];
+    double2 hw[GATHER_EPT];
+    double acc0[GATHER_EPT], acc1[GATHER_EPT];
+#pragma unroll
+    for (int u = 0; u < GATHER_EPT; ++u) {
+        k[u] = (blockIdx.x * GATHER_EPT + u) * 256 + threadIdx.x;
+        const int kc = min(k[u], K - 1);
+        t0[u] = ptr[kc]; t1[u] = ptr[kc + 1];
+        hw[u] = *reinterpret_cast<const double2 *>(head + kc);
     }
-    double *o = out + (size_t)blockIdx.z * ostride + (size_t)sp0 * K + k;
-    o[0] = acc0;
-    if (two) o[K] = acc1;
+#pragma unroll
+    for (int u = 0; u < GATHER_EPT; ++u) {
+        const int i0 = __double2loint(hw[u].y);
+        acc0[u] = s0[i0]; acc1[u] = s1[i0];
+    }
+#pragma unroll
+    for (int u = 0; u < GATHER_EPT; ++u) {
+        acc0[u] = fma(hw[u].x, acc0[u], 0.0); acc1[u] = fma(hw[u].x, acc1[u], 0.0);
+        for (int t = t0[u] + 1; t < t1[u]; ++t) {
+            const double wt = w[t];
+            const int it = idx[t];
+            acc0[u] = fma(wt, s0[it], acc0[u]);
+            acc1[u] = fma(wt, s1[it], acc1[u]);
+        }
+        if (k[u] < K) {
+            double *o = out + (size_t)blockIdx.z * ostride + (size_t)sp0 * K + k[u];
+            o[0] = acc0[u];
+            if (two) o[K] = acc1[u];
+        }
+    }
 }
 
 // Sums the j-split partials (used by landau_inner_integral when jsplit > 1).  grid over 5N x nb.
@@ -683,15 +730,15 @@ int pair_tiles(int N, bool latency) { const int ts = pair_tile_size(N, latency);
 // Warps sharing a tile pair where the tiles are 32 points (k_pair_split): a function of N and the policy, like the tile size.
 int pair_split_warps(int N, bool latency) { return N < (latency ? 2048 : 1536) ? 4 : 2; }
 
-int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st) {
+int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, double *u, cudaStream_t st) {
     dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
-    launch_k(k_fields_beta<false>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, 0, 0, f, T);
+    launch_k(k_fields_beta<false>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, 0, 0, f, T, u);
     return 1;
 }
 
-int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, cudaStream_t st) {
+int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, double *u, cudaStream_t st) {
     dim3 grid((ds.Ne + FIELD_EPB - 1) / FIELD_EPB, nb), block(ds.Nq, FIELD_EPB);
-    launch_k(k_fields_beta<true>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, shared_kpad(ds.Ntot) / 8, nbpad, f, T);
+    launch_k(k_fields_beta<true>, grid, block, 0, st, nb <= PDL_MAX_NB, ds, shared_kpad(ds.Ntot) / 8, nbpad, f, T, u);
     return 1;
 }
 
@@ -717,9 +764,11 @@ int launch_pair(int Ntot, bool latency, const double *r, const double *z, const 
 int launch_element(const DeviceSpace &ds, int nb, int jsplit, const double *f, const double *G, double *Ce, double *ce,
                    const double *Ez, double shift, cudaStream_t st) {
     if (ds.Nb == 16 && jsplit == 1) {   // Q3: FP64 tensor cores, warp per cell
-        dim3 grid((ds.Ne + ELQ3_WARPS * ELQ3_ROUNDS - 1) / (ELQ3_WARPS * ELQ3_ROUNDS), nb);
-        if (Ez) launch_k(k_element_q3<true>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, Ez, shift);
-        else launch_k(k_element_q3<false>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, f, G, Ce, ce, (const double *)nullptr, 0.0);
+        // several cells per warp pay in a batch (prefetch); a small batch needs every warp it can get
+        const int rounds = nb >= ELQ3_ROUNDS_MIN_NB ? ELQ3_ROUNDS : 1;
+        dim3 grid((ds.Ne + ELQ3_WARPS * rounds - 1) / (ELQ3_WARPS * rounds), nb);
+        if (Ez) launch_k(k_element_q3<true>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, rounds, G, Ce, ce, Ez, shift);
+        else launch_k(k_element_q3<false>, grid, dim3(ELQ3_WARPS * 32), 0, st, nb <= PDL_MAX_NB, ds, rounds, G, Ce, ce, (const double *)nullptr, 0.0);
         return 1;
     }
     dim3 grid(ds.Ne, nb);
@@ -740,8 +789,11 @@ __global__ void k_gather2(DeviceSpace ds, int bv, size_t vstride, size_t fstride
     const double *w = isv ? ds.gw : ds.cw;
     const size_t stride = isv ? (size_t)ds.Ne * ds.Nb * ds.Nb : (size_t)ds.Ne * ds.Nb;
     const double *s = (isv ? Ce : ce) + ((size_t)blockIdx.z * gridDim.y + blockIdx.y) * stride;
-    double acc = 0.0;
-    for (int t = ptr[kk]; t < ptr[kk + 1]; ++t) acc = fma(w[t], s[idx[t]], acc);
+    const GatherHead *head = isv ? ds.ghead : ds.chead;
+    const int t0 = ptr[kk], t1 = ptr[kk + 1];
+    const double2 hw = *reinterpret_cast<const double2 *>(head + kk);
+    double acc = fma(hw.x, s[__double2loint(hw.y)], 0.0);
+    for (int t = t0 + 1; t < t1; ++t) acc = fma(w[t], s[idx[t]], acc);
     (isv ? vals : Cf)[(size_t)blockIdx.z * (isv ? vstride : fstride) + (size_t)blockIdx.y * K + kk] = acc;
 }
 
@@ -754,14 +806,14 @@ int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fst
 }
 
 int launch_gather_vals(const DeviceSpace &ds, int nb, int nspecies, size_t ostride, const double *Ce, double *vals, cudaStream_t st) {
-    dim3 grid((ds.nnz + 255) / 256, (nspecies + 1) / 2, nb);
-    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.nnz, nspecies, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, Ce, vals);
+    dim3 grid((ds.nnz + 256 * GATHER_EPT - 1) / (256 * GATHER_EPT), (nspecies + 1) / 2, nb);
+    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.nnz, nspecies, (size_t)ds.Ne * ds.Nb * ds.Nb, ostride, ds.gptr, ds.gidx, ds.gw, ds.ghead, Ce, vals);
     return 1;
 }
 
 int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double *ce, double *Cf, cudaStream_t st) {
-    dim3 grid((ds.n + 255) / 256, (ds.S + 1) / 2, nb);
-    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.n, ds.S, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ce, Cf);
+    dim3 grid((ds.n + 256 * GATHER_EPT - 1) / (256 * GATHER_EPT), (ds.S + 1) / 2, nb);
+    launch_k(k_gather, grid, dim3(256), 0, st, false, ds.n, ds.S, (size_t)ds.Ne * ds.Nb, ostride, ds.cptr, ds.cidx, ds.cw, ds.chead, ce, Cf);
     return 1;
 }
 

@@ -11,6 +11,10 @@ constexpr int MAX_SPECIES = 16;
 
 // Device-resident description of one mesh/order/species set (all pointers device memory,
 // shared by every problem of a batch).
+// First item (weight, source index) of a gather list: read with the list bounds, not after them, so that the
+// source value of the (usual) one-item list is two dependent loads away instead of three.
+struct GatherHead { double w; int32_t idx; int32_t pad; };
+
 struct DeviceSpace {
     int p, Nq, Nb, S;                            // S = species living on this grid
     int N, Ne, n, nnz;
@@ -26,6 +30,7 @@ struct DeviceSpace {
     const int32_t *rowptr, *colidx;
     const int32_t *gptr, *gidx; const double *gw;
     const int32_t *cptr, *cidx; const double *cw;
+    const GatherHead *ghead, *chead;         // first item of every list, one 16-byte word per output (k_gather)
     double e2[MAX_SPECIES];    // e_b^2
     double m0m[MAX_SPECIES];   // m0/m_b
     double kfac[MAX_SPECIES];  // nu e_a^2 (m0/m_a)
@@ -43,7 +48,7 @@ struct Scratch {
 };
 
 // each returns the number of kernels launched
-int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, cudaStream_t st);
+int launch_fields_beta(const DeviceSpace &ds, int nb, const double *f, double *T, double *u, cudaStream_t st);
 
 // Batch-shared path (landau_shared.cu): the tensor of every ordered pair is evaluated once per call into
 // U[5][Kpad/8][Mpad][8] and applied to all problems by an fp64 tensor-core contraction with T[3][Kpad/8][nbpad][8].
@@ -51,7 +56,7 @@ int shared_kpad(int N);      // 16 ceil(N/16): source points padded to whole chu
 int shared_mpad(int N);      // target points padded to whole tiles
 int shared_nbpad(int nb);    // problems padded to whole tiles
 int shared_ksplit(int N);    // segments of the j range (a function of N only: fixes the summation order)
-int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, cudaStream_t st);
+int launch_fields_beta_tiled(const DeviceSpace &ds, int nb, int nbpad, const double *f, double *T, double *u, cudaStream_t st);
 int launch_pair_tensor(int N, const double *r, const double *z, const double *invr, double *U, cudaStream_t st);
 // Gpart[b][ksplit][5][N]
 int launch_apply(int N, int nb, int nbpad, const double *U, const double *T, double *Gpart, cudaStream_t st);
