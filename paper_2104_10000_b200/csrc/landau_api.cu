@@ -422,8 +422,9 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
                     if (ptr[k + 1] > ptr[k]) h[k] = GatherHead{w[ptr[k]], idx[ptr[k]], 0};
                 return h;
             };
-            const std::vector<GatherHead> gh = heads(hs.gptr, hs.gidx, hs.gw), ch = heads(hs.cptr, hs.cidx, hs.cw);
-            UPC(ds.ghead, gh) UPC(ds.chead, ch)
+            const std::vector<GatherHead> gh = heads(hs.gptr, hs.gidx, hs.gw), ch = heads(hs.cptr, hs.cidx, hs.cw),
+                                          lh = heads(hs.lptr, hs.ldof, hs.lw);
+            UPC(ds.ghead, gh) UPC(ds.chead, ch) UPC(ds.lhead, lh)
         }
         // band LU: order, half-bandwidth, envelope per block step, fill lists per band column
         std::vector<int32_t> perm;

@@ -270,6 +270,7 @@ k_pair_split(int N, int ntiles, const double *__restrict__ r, const double *__re
 // Output T[b][3][N] = w_in * (T_D, T_Kr, T_Kz): the weight of the inner sum is folded in here.
 // ------------------------------------------------------------------------------------------------
 constexpr int FIELD_EPB = 8;      // cells per block
+constexpr int FIELD_SG = 2;       // species sharing one read of the tabulations
 
 // TILED: T in the layout of the batch-shared contraction (landau_shared.cu): T[c][jo][b][k][h], j = 8 jo + 4 h + k.
 // The kernel is latency-bound (three dependent loads per gathered value, a few hundred flop per cell): small blocks
@@ -292,10 +293,13 @@ k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, 
     const int e = blockIdx.x * FIELD_EPB + threadIdx.y;
     const bool valid = e < ds.Ne;
     if (valid) {
+        // the first item of the node's list (for a node that does not hang: the only one) comes with the bounds
         const int t0 = ds.lptr[e * Nb + q], t1 = ds.lptr[e * Nb + q + 1];
+        const double2 hw = *reinterpret_cast<const double2 *>(ds.lhead + e * Nb + q);
+        const int d0 = __double2loint(hw.y);
         for (int sp = 0; sp < ds.S; ++sp) {
-            double u = 0.0;
-            for (int t = t0; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
+            double u = fma(hw.x, fb[(size_t)sp * ds.n + d0], 0.0);
+            for (int t = t0 + 1; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
             s_u[threadIdx.y][sp][q] = u;
             // u = P_e f is needed again by the element kernel (C_e u): kept in the element vector's own slots, which
             // k_element_q3 reads before it overwrites them -- one coalesced load there instead of a second list walk
@@ -306,21 +310,34 @@ k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, 
     if (!valid) return;
     const double ijr = ds.invJ[2 * e], ijz = ds.invJ[2 * e + 1];
     double tD = 0.0, tKr = 0.0, tKz = 0.0;
-    for (int sp = 0; sp < ds.S; ++sp) {
-        double fq = 0.0, g0 = 0.0, g1 = 0.0;
+    // the kernel's time is shared-memory bandwidth (three tabulation words per node and species): FIELD_SG species share them
+    for (int sp0 = 0; sp0 < ds.S; sp0 += FIELD_SG) {
+        double fq[FIELD_SG], g0[FIELD_SG], g1[FIELD_SG];
+#pragma unroll
+        for (int s = 0; s < FIELD_SG; ++s) { fq[s] = 0.0; g0[s] = 0.0; g1[s] = 0.0; }
 #pragma unroll
         for (int a = 0; a < 16; ++a) {
             if (a < Nb) {
-                const double u = s_u[threadIdx.y][sp][a];
-                fq = fma(s_tab[0][a][q], u, fq);
-                g0 = fma(s_tab[1][a][q], u, g0);
-                g1 = fma(s_tab[2][a][q], u, g1);
+                const double tb = s_tab[0][a][q], t0 = s_tab[1][a][q], t1 = s_tab[2][a][q];
+#pragma unroll
+                for (int s = 0; s < FIELD_SG; ++s) {
+                    const double u = s_u[threadIdx.y][min(sp0 + s, ds.S - 1)][a];
+                    fq[s] = fma(tb, u, fq[s]);
+                    g0[s] = fma(t0, u, g0[s]);
+                    g1[s] = fma(t1, u, g1[s]);
+                }
             }
         }
-        const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
-        tD = fma(e2, fq, tD);
-        tKr = fma(em, ijr * g0, tKr);
-        tKz = fma(em, ijz * g1, tKz);
+#pragma unroll
+        for (int s = 0; s < FIELD_SG; ++s) {
+            if (sp0 + s < ds.S) {
+                const int sp = sp0 + s;
+                const double e2 = ds.e2[sp], em = ds.e2[sp] * ds.m0m[sp];
+                tD = fma(e2, fq[s], tD);
+                tKr = fma(em, ijr * g0[s], tKr);
+                tKz = fma(em, ijz * g1[s], tKz);
+            }
+        }
     }
     const int gi = e * Nq + q;
     const double w = 12.566370614359172953850573533118 * ds.w_in[gi];    // 4 pi of the tensor (landau_pair_math.cuh) folded in

@@ -30,7 +30,7 @@ struct DeviceSpace {
     const int32_t *rowptr, *colidx;
     const int32_t *gptr, *gidx; const double *gw;
     const int32_t *cptr, *cidx; const double *cw;
-    const GatherHead *ghead, *chead;         // first item of every list, one 16-byte word per output (k_gather)
+    const GatherHead *ghead, *chead, *lhead; // first item of every list, one 16-byte word per output (k_gather) / local node (k_fields_beta)
     double e2[MAX_SPECIES];    // e_b^2
     double m0m[MAX_SPECIES];   // m0/m_b
     double kfac[MAX_SPECIES];  // nu e_a^2 (m0/m_a)

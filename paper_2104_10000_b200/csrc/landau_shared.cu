@@ -49,7 +49,9 @@ __global__ void __launch_bounds__(PT_THREADS)
 k_pair_tensor(int N, int Kq8, int Mpad, const double *__restrict__ r, const double *__restrict__ z,
               const double *__restrict__ invr, double *__restrict__ U) {
     __shared__ double sj[5][8 * PT_OCTETS];               // r, z, 2r, 2r^2, 1/(16 r^2) of the source points
-    __shared__ double2 so[5][4][PT_THREADS];              // one octet of results, [c][k][thread] = (h=0, h=1)
+    // one octet of results, [c][k][thread] = (h=0, h=1).  Rows padded by two words: the copy-out reads (k, point) =
+    // (lane % 4, lane / 4), and with rows of 128 x 16 bytes the four k of a point would share a bank (4-way conflict)
+    __shared__ double2 so[5][4][PT_THREADS + 2];
     const int tid = threadIdx.x;
     const int i = blockIdx.x * PT_THREADS + tid;
     const int jbase = blockIdx.y * 8 * PT_OCTETS;
