@@ -281,7 +281,9 @@ __global__ void __launch_bounds__(16 * FIELD_EPB)
 k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, double *__restrict__ T, double *__restrict__ uout) {
     pdl_prologue();
     __shared__ double s_tab[3][16][16];                     // [B, E0, E1][a][q]
-    __shared__ double s_u[FIELD_EPB][MAX_SPECIES][16];      // u = P_e f of every species of the block's cells
+    // u = P_e f of every species of the block's cells; a cell's row padded by two words: the two cells of a warp read
+    // the same (species, node) and would otherwise hit one bank
+    __shared__ double s_u[FIELD_EPB][MAX_SPECIES * 16 + 2];
     const int b = blockIdx.y;
     const int q = threadIdx.x;
     const int Nb = ds.Nb, Nq = ds.Nq;
@@ -300,7 +302,7 @@ k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, 
         for (int sp = 0; sp < ds.S; ++sp) {
             double u = fma(hw.x, fb[(size_t)sp * ds.n + d0], 0.0);
             for (int t = t0 + 1; t < t1; ++t) u = fma(ds.lw[t], fb[(size_t)sp * ds.n + ds.ldof[t]], u);
-            s_u[threadIdx.y][sp][q] = u;
+            s_u[threadIdx.y][sp * 16 + q] = u;
             // u = P_e f is needed again by the element kernel (C_e u): kept in the element vector's own slots, which
             // k_element_q3 reads before it overwrites them -- one coalesced load there instead of a second list walk
             uout[(((size_t)b * ds.S + sp) * ds.Ne + e) * Nb + q] = u;
@@ -321,7 +323,7 @@ k_fields_beta(DeviceSpace ds, int Kq8, int nbpad, const double *__restrict__ f, 
                 const double tb = s_tab[0][a][q], t0 = s_tab[1][a][q], t1 = s_tab[2][a][q];
 #pragma unroll
                 for (int s = 0; s < FIELD_SG; ++s) {
-                    const double u = s_u[threadIdx.y][min(sp0 + s, ds.S - 1)][a];
+                    const double u = s_u[threadIdx.y][min(sp0 + s, ds.S - 1) * 16 + a];
                     fq[s] = fma(tb, u, fq[s]);
                     g0[s] = fma(t0, u, g0[s]);
                     g1[s] = fma(t1, u, g1[s]);
