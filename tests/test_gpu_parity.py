@@ -567,6 +567,61 @@ def test_batched_equals_loop_of_singles_bitwise_and_is_deterministic(gpu, path):
     assert np.array_equal(v4.cpu().numpy(), v1) and np.array_equal(c4.cpu().numpy(), c1)
 
 
+@pytest.mark.parametrize("path", PATHS_BATCH)
+def test_calls_of_64_and_more_problems_equal_smaller_calls_bitwise(gpu, path):
+    """From 64 problems per call on, a warp of `k_element_q3` takes four cells one after the other and prefetches the
+    next cell's inputs (cp.async, two shared-memory buffers); below, one cell per warp.  Same values, bitwise: mesh 3A
+    (98 cells: the last block and the last rounds are ragged), Jacobian and implicit-step operator, 70 problems in one
+    call against 35 + 35; and Table I's three 20-cell grids with ten species, 64 problems against 32 + 32."""
+    import torch
+    wl = inputs.config(3, variant="A")
+    nb = 70
+    mb, pth = ctx_args(path, nb)
+    ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, mb, pair_path=pth)
+    r, z = ctx.dof_coords()
+    f0 = inputs.nodal_f(wl, r, z)
+    scale = 1.0 + 0.3 * np.sin(0.41 * np.arange(nb)[:, None] + 1.1 * np.arange(ctx.S)[None, :])
+    fd = torch.from_numpy(f0[None] * scale[:, :, None]).cuda()
+    Ez = torch.from_numpy(0.1 + 0.01 * np.arange(nb)).cuda()
+    out = []
+    for split in ((nb,), (35, 35)):
+        v = torch.full((nb, ctx.S, ctx.nnz), float("nan"), dtype=torch.float64, device="cuda")
+        c = torch.full((nb, ctx.S, ctx.n), float("nan"), dtype=torch.float64, device="cuda")
+        vi, ci = torch.full_like(v, float("nan")), torch.full_like(c, float("nan"))
+        b0 = 0
+        for m in split:
+            ctx.jacobian_batched(fd[b0:b0 + m], v[b0:b0 + m], c[b0:b0 + m])
+            ctx.implicit_operator_batched(fd[b0:b0 + m], Ez[b0:b0 + m], 2.0, vi[b0:b0 + m], ci[b0:b0 + m])
+            b0 += m
+        out.append([t.cpu().numpy() for t in (v, c, vi, ci)])
+    for a, b in zip(*out):
+        assert np.isfinite(a).all() and np.array_equal(a, b)
+    ctx.destroy()
+    name, order, meshes, spc, sgrid, comps = inputs.multigrid_case("paper3")
+    nb = 64
+    mb, pth = ctx_args(path, nb)
+    ctx = gpu.LandauMultigridContext(meshes, sgrid, order, spc, mb)
+    ctx.set_pair_path(pth)
+    fl = []
+    for a, c in enumerate(comps):
+        r, z = ctx.grid_dof_coords(sgrid[a])
+        fl.append(inputs.maxwellian(float(spc.mass[a]), c.n, c.T, c.zs, r, z))
+    f = np.concatenate(fl)
+    fd = torch.from_numpy(f[None] * (1.0 + 0.2 * np.cos(0.3 * np.arange(nb)))[:, None]).cuda()
+    out = []
+    for split in ((nb,), (32, 32)):
+        v = torch.full((nb, ctx.vals_stride), float("nan"), dtype=torch.float64, device="cuda")
+        c = torch.full((nb, ctx.f_stride), float("nan"), dtype=torch.float64, device="cuda")
+        b0 = 0
+        for m in split:
+            ctx.jacobian_batched(fd[b0:b0 + m], v[b0:b0 + m], c[b0:b0 + m])
+            b0 += m
+        out.append([v.cpu().numpy(), c.cpu().numpy()])
+    for a, b in zip(*out):
+        assert np.isfinite(a).all() and np.array_equal(a, b)
+    ctx.destroy()
+
+
 def test_no_state_carried_between_calls(gpu):
     """A, then a different problem and a different batch size, then A again in the same context: bitwise the
     same A (nothing is read from scratch that the call itself did not write); also through the implicit
