@@ -257,6 +257,24 @@ int resolve_pair_path(const landau_ctx *ctx, int path) {
 }
 
 constexpr double FRONT_MAX_WORK_RATIO = 0.5;     // LANDAU_BAND_AUTO: front kernel when its flops are at most half the hull's
+constexpr size_t FRONT_SMEM_MAX = size_t(225) * 1024;        // + 1 KB the driver reserves per block
+constexpr size_t SLOT_SMEM_TWO_PER_SM = size_t(112) * 1024;  // two blocks of the slot kernel on an SM
+
+// Columns per block step of the FACTORISATION.  band_block(bw) unless that is 32 and the envelope is so jagged that the
+// slot kernel with 16-column blocks keeps two matrices per SM (config 5: fill + factor 14.2 -> 10.8 ms; where its
+// window needs an SM for itself -- the ten-species 320-cell mesh -- 32-column blocks with look-ahead stay ahead).  The
+// solves keep band_block(bw) in either case: L and U do not depend on the blocking, and a 16-column solve of a band
+// that wide takes twice as long (config 5: 5.9 against 3.45 ms).
+int band_factor_block(const HostSpace &hs, const std::vector<int32_t> &perm, int bw) {
+    const int kb = band_block(bw);
+    if (kb != 32) return kb;
+    std::vector<int32_t> ap, ai;
+    double f16 = 0.0;
+    const int na16 = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, 16, ap, ai, &f16);
+    int bw2 = 0;
+    const double hull16 = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr, 16);
+    return band_slot_smem(16, na16) <= SLOT_SMEM_TWO_PER_SM && na16 <= 160 && f16 <= FRONT_MAX_WORK_RATIO * hull16 ? 16 : kb;
+}
 
 // Small batches are launch-latency bound: both gathers then go in one launch (3-7 us per single build); large
 // batches keep the two launches (the merged kernel is 10 % slower there).
@@ -432,15 +450,20 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
         const int64_t Wb = band_stored_halfwidth(bw), LD = 2 * Wb + 1;
         if (LD * hs.n > (int64_t(1) << 31) - 1) return LANDAU_EINVAL;
+        const int kb = band_factor_block(hs, perm, bw), kbs = band_block(bw);        // kb <= kbs: the stored width covers both
+        G.bs.kb = kb; G.bs.W = int(Wb);
         G.bs.n = int(hs.n); G.bs.nnz = int(hs.nnz); G.bs.bw = bw; G.bs.mat_doubles = (size_t(LD) * hs.n + 1) & ~size_t(1);   // even: every matrix starts 16-byte aligned
         // envelope of the permuted pattern: block step s only reaches mlow[s] rows below and mup[s] rows above its
         // block (<= bw; about half the uniform-band work on the refined meshes)
         {
-            std::vector<int32_t> mlow, mup, zlo, zcnt, fptr, fsrc, foff;
+            std::vector<int32_t> mlow, mup, mlow_s, mup_s, zlo, zcnt, fptr, fsrc, foff;
             int bw2 = 0;
-            G.bs.flop_per_matrix = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow, &mup);
-            band_fill_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, mlow, mup, zlo, zcnt, fptr, fsrc, foff);
+            G.bs.flop_per_matrix = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow, &mup, kb);
+            if (kbs != kb) band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, &mlow_s, &mup_s, kbs);
+            band_fill_lists(int(hs.n), hs.rowptr, hs.colidx, perm, int(Wb), kb, mlow, mup, kbs, mlow_s, mup_s, zlo, zcnt, fptr, fsrc, foff);
             UPC(G.bs.mlow, mlow) UPC(G.bs.mup, mup)
+            if (kbs != kb) { UPC(G.bs.mlow_s, mlow_s) UPC(G.bs.mup_s, mup_s) }
+            else { G.bs.mlow_s = G.bs.mlow; G.bs.mup_s = G.bs.mup; }
             {
                 std::vector<int32_t> pos(hs.n), first(hs.n);
                 for (int64_t i = 0; i < hs.n; ++i) { pos[perm[i]] = int32_t(i); first[i] = int32_t(i); }
@@ -450,11 +473,11 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             }
             UPC(G.bs.zlo, zlo) UPC(G.bs.zcnt, zcnt) UPC(G.bs.fptr, fptr) UPC(G.bs.fsrc, fsrc) UPC(G.bs.foff, foff)
             std::vector<int32_t> act_ptr, act_idx;
-            G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &G.bs.front_flop);
+            G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, act_ptr, act_idx, &G.bs.front_flop);
             if (act_idx.empty()) act_idx.push_back(0);
             {
                 std::vector<int32_t> act_slot, slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src;
-                band_slot_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, band_front_ldw(G.bs.na_max), act_ptr, act_idx, G.bs.na_max, act_slot,
+                band_slot_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, int(Wb), band_front_ldw(G.bs.na_max), act_ptr, act_idx, G.bs.na_max, act_slot,
                                 slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src);
                 if (slot_hi.empty()) slot_hi.push_back(0);
                 UPC(G.bs.slot_hi, slot_hi)
@@ -463,10 +486,10 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
                 if (ld_dst.empty()) { ld_dst.push_back(0); ld_src.push_back(0); }
                 UPC(G.bs.act_slot, act_slot) UPC(G.bs.new_ptr, new_ptr) UPC(G.bs.new_pos, new_pos)
                 UPC(G.bs.ld_ptr, ld_ptr) UPC(G.bs.ld_dst, ld_dst) UPC(G.bs.ld_src, ld_src)
-                G.bs.slot = band_block(bw) == 16 && band_slot_smem(bw, G.bs.na_max) <= size_t(225) * 1024;
+                G.bs.slot = kb == 16 && band_slot_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX;
             }
             UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
-            G.front_fits = band_front_smem(bw, G.bs.na_max) <= size_t(225) * 1024 && G.bs.na_max <= 160 && band_block(bw) >= 16;   // + 1 KB the driver reserves per block; FRONT_IR rows per lane
+            G.front_fits = band_front_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX && G.bs.na_max <= 160 && kb >= 16;   // FRONT_IR rows per lane
             // AUTO: the front kernel pays a gather and a scatter of its window per block step; it wins where the envelope
             // is jagged (refined meshes: a sixth of the hull's flops), not on uniform meshes (front = hull)
             G.bs.front = G.front_fits && G.bs.front_flop <= FRONT_MAX_WORK_RATIO * G.bs.flop_per_matrix;
@@ -576,10 +599,11 @@ int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_hos
     rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
     if (perm_host) std::memcpy(perm_host, perm.data(), perm.size() * sizeof(int32_t));
     if (half_bandwidth) *half_bandwidth = bw;
-    if (block_columns) *block_columns = band_block(bw);
+    const int kb = band_factor_block(hs, perm, bw);
+    if (block_columns) *block_columns = kb;
     if (flop_per_factorization) {      // the envelope work of landau_create, recomputed from the order
         int bw2 = 0;
-        *flop_per_factorization = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr);
+        *flop_per_factorization = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr, kb);
     }
     return int(LANDAU_OK);
     });
@@ -596,10 +620,11 @@ int landau_band_front_host(const landau_mesh *mesh, int order, int32_t *front_ro
         int bw = 0;
         rcm_order(int(hs.n), hs.rowptr, hs.colidx, hs.dof_r.data(), hs.dof_z.data(), perm, bw);
         double fl = 0.0;
-        const int na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, bw, act_ptr, act_idx, &fl);
+        const int kb = band_factor_block(hs, perm, bw);
+        const int na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, act_ptr, act_idx, &fl);
         if (front_rows_max) *front_rows_max = na_max;
         if (front_flop) *front_flop = fl;
-        if (fits) *fits = band_front_smem(bw, na_max) <= size_t(225) * 1024 && na_max <= 160 && band_block(bw) >= 16;
+        if (fits) *fits = band_front_smem(kb, na_max) <= FRONT_SMEM_MAX && na_max <= 160 && kb >= 16;
         return int(LANDAU_OK);
     });
 }
@@ -804,7 +829,7 @@ int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, 
     if (!ctx || !vals_dev || !band_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(stream);
     for (auto &g : ctx->grids) {
-        if (band_factor_smem(g.bs.bw) > 227 * 1024) return LANDAU_EINVAL;
+        if (band_factor_smem(g.bs.bw, g.bs.kb) > 227 * 1024) return LANDAU_EINVAL;
         double *band = band_dev + g.boff;
         CK(launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, ctx->bstride, vals_dev + g.voff, band, st));
         CK(launch_band_factor(g.bs, nb * g.ds.S, g.ds.S, ctx->bstride, band, pivots_dev ? pivots_dev + 2 * g.s0 : nullptr, ctx->S, st));

@@ -96,7 +96,7 @@ void rcm_from(int n, const std::vector<int32_t> &rowptr, const std::vector<int32
 // a row's first entry / above a column's first entry, so the reach is the monotone hull of the envelope.
 // Returns the window-update work of one factorisation, 2 KB sum mlow^2 flop.
 double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int &bw, std::vector<int32_t> *mlow_out, std::vector<int32_t> *mup_out) {
+                     int &bw, std::vector<int32_t> *mlow_out, std::vector<int32_t> *mup_out, int KB_in) {
     std::vector<int32_t> pos(n), first(n), last_with_first(n + 1, 0);
     for (int i = 0; i < n; ++i) { pos[perm[i]] = i; first[i] = i; }
     bw = 0;
@@ -108,7 +108,7 @@ double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vecto
         }
     for (int i = 0; i < n; ++i) last_with_first[first[i]] = std::max<int32_t>(last_with_first[first[i]], i);
     for (int j = 1; j < n; ++j) last_with_first[j] = std::max(last_with_first[j], last_with_first[j - 1]);
-    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB;
+    const int KB = KB_in > 0 ? KB_in : band_block(bw), nsteps = (n + KB - 1) / KB;
     if (mlow_out) mlow_out->assign(nsteps, 0);
     if (mup_out) mup_out->assign(nsteps, 0);
     double work = 0.0;
@@ -303,14 +303,13 @@ __device__ __forceinline__ void factor_diag_block(double *A, size_t lda, int k0,
 // WT, plus 4 (row stride = 4 mod 16 doubles: the fragment loads are bank-conflict free), zero padded.
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT, (KB == 16 && NT == 128) ? BAND16_MIN_BLOCKS : 1)
-k_band_factor(int n, int bw, int MWP, size_t mat_doubles, size_t pstride, int S, const int32_t *__restrict__ mlow,
+k_band_factor(int n, int W, int MWP, size_t mat_doubles, size_t pstride, int S, const int32_t *__restrict__ mlow,
               double *__restrict__ band_all, double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
     constexpr int DSZ = KB * (KB + 1) + KB;  // one diagonal-block buffer: sD[KB][KB+1], sDi[KB]
     double *sDs = smem + 2 * DSZ;            // [KB][KB]: the current L11 \ U11 with 16-byte aligned rows (panel substitutions)
     double *sL = sDs + KB * KB;              // [KB][MWP]: sL[c][i] = -L(k0+kb+i, k0+c)
     double *sU = sL + (size_t)KB * MWP;      // [KB][MWP]: sU[c][j] = U(k0+c, k0+kb+j)
-    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;        // LD - 1
     double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -542,7 +541,7 @@ __device__ __noinline__ double2 factor_diag_src(const double *src, size_t lds, d
 constexpr int FRONT_JC = 4, FRONT_IR = 5;      // window gather: columns per warp and pass, rows per lane (fronts of up to 160 rows)
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
-k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, size_t pstride, int S,
+k_front_factor(int n, int W, int LDP, int LDW, int na_max, size_t mat_doubles, size_t pstride, int S,
                const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, double *__restrict__ band_all,
                double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
@@ -553,7 +552,6 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
     double *sU = sL + (size_t)KB * LDP;          // sU[c][j] = U(k0 + c, act[j])
     double *sW = sU + (size_t)KB * LDP;          // sW[i + j LDW] = A(act[i], act[j])
     int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * na_max), *sActN = sAct + na_max;    // this step's list, the next one's
-    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -774,7 +772,7 @@ k_front_factor(int n, int bw, int LDP, int LDW, int na_max, size_t mat_doubles, 
 constexpr int SLOT_LB = 8;                     // band loads a worker thread keeps in flight when it assembles entering rows
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
-k_slot_factor(int n, int bw, int LDP, int LDW, int NS, size_t mat_doubles, size_t pstride, int S,
+k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t pstride, int S,
               const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, const int32_t *__restrict__ act_slot,
               const int32_t *__restrict__ slot_hi, const int32_t *__restrict__ new_ptr, const int32_t *__restrict__ new_pos, const int32_t *__restrict__ ld_ptr,
               const int32_t *__restrict__ ld_dst, const int32_t *__restrict__ ld_src, double *__restrict__ band_all,
@@ -788,7 +786,6 @@ k_slot_factor(int n, int bw, int LDP, int LDW, int NS, size_t mat_doubles, size_
     double *sW = sU + (size_t)KB * LDP;          // sW[slot_i + slot_j LDW] = A(row_i, row_j)
     int *sAct = reinterpret_cast<int *>(sW + (size_t)LDW * NS), *sSlot = sAct + NS;      // this step's list: global row, slot
     int *sActN = sSlot + NS, *sSlotN = sActN + NS, *sNew = sSlotN + NS;                   // the next step's; positions of its entering rows
-    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
@@ -1015,7 +1012,7 @@ k_slot_factor(int n, int bw, int LDP, int LDW, int NS, size_t mat_doubles, size_
 // orders n beyond the 227 KB of an SM (n > ~28,000); the block barriers order those accesses just the same.
 template <int KB, int NT, bool XG>
 __global__ void __launch_bounds__(NT)
-k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
+k_band_solve(int n, int W, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
              const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const int32_t *__restrict__ first, size_t pstride,
              const double *__restrict__ band_all, const double *rhs, double *xout, double *xg) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
     // first[i]: the column of row i's first entry in the ordered pattern = the row of column i's first entry (the
@@ -1026,7 +1023,6 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
     double *x = XG ? xg + (size_t)blockIdx.x * n : smem;    // [n]
     double *sD = XG ? smem : smem + n;                      // [SB][SB+1]
     int *sF = reinterpret_cast<int *>(sD + SB * (SB + 1));  // [SB] first rows of the current block's columns (backward sweep)
-    const int W = band_halfwidth(bw, KB);
     const size_t lda = 2 * (size_t)W;
     const int mat = blockIdx.x;       // = b * S + sp
     const double *A = band_all + (size_t)(mat / S) * pstride + (size_t)(mat % S) * mat_doubles + W;
@@ -1102,12 +1098,14 @@ k_band_solve(int n, int bw, size_t mat_doubles, size_t xstride, int S, const int
 // symmetric).  So block step s (columns k0 .. ke) only involves the rows / columns i > ke with first[i] <= ke; the
 // next block's rows are always listed (first, in order) so that its diagonal block is the leading corner of the front.
 int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                      int bw, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop) {
-    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB;
+                      int KB, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop) {
+    const int nsteps = (n + KB - 1) / KB;
     std::vector<int32_t> pos(n), first(n);
     for (int i = 0; i < n; ++i) { pos[perm[i]] = i; first[i] = i; }
     for (int i = 0; i < n; ++i)
         for (int t = rowptr[i]; t < rowptr[i + 1]; ++t) first[pos[i]] = std::min<int32_t>(first[pos[i]], pos[colidx[t]]);
+    int bw = 0;                            // a row i can only be active at a step with i - first[i] <= bw
+    for (int i = 0; i < n; ++i) bw = std::max(bw, i - int(first[i]));
     act_ptr.assign(nsteps + 1, 0);
     act_idx.clear();
     int na_max = 0;
@@ -1133,10 +1131,10 @@ int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vect
 // with i entering and j in list s (or both entering), as (offset in the window, offset in the band) -- the entering rows are
 // assembled sparsely, everything else of their rows / columns is zero.
 void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int bw, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     int KB, int W, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
                      std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
                      std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src) {
-    const int KB = band_block(bw), nsteps = (n + KB - 1) / KB, W = band_halfwidth(bw, KB);
+    const int nsteps = (n + KB - 1) / KB;
     const long long lda = 2LL * W;
     std::vector<int32_t> pos(n);
     for (int i = 0; i < n; ++i) pos[perm[i]] = i;
@@ -1183,14 +1181,13 @@ void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
 // ------------------------------------------------------------------------------------------------
 static int band_mw(int bw) { return ((std::max(bw, 1) + WT - 1) / WT) * WT + 4; }
 
-size_t band_factor_smem(int bw) {
-    const int KB = band_block(bw);
+size_t band_factor_smem(int bw, int KB) {
     return sizeof(double) * (2 * ((size_t)KB * (KB + 1) + KB) + (size_t)KB * KB + 2 * (size_t)KB * band_mw(bw));
 }
 
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st) {
-    const int W = band_halfwidth(bs.bw, band_block(bs.bw));
+    const int W = bs.W;
     dim3 grid((bs.n + FILL_WARPS - 1) / FILL_WARPS, S, nb);
     k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
                                                  bs.fsrc, bs.foff, vals, band);
@@ -1202,22 +1199,38 @@ cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride,
 // [k0(s), E(s)]^2, E(s) = ke(s) + mlow[s], that contains it -- the diagonal block, panels and window of step s -- and
 // by the backward solve up to mup[s_j] rows above its block: rows k0(first s with E(s) >= j) ... E(s_j).
 void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int bw, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, std::vector<int32_t> &zlo,
+                     int W, int KB, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, int KBs,
+                     const std::vector<int32_t> &mlow_s, const std::vector<int32_t> &mup_s, std::vector<int32_t> &zlo,
                      std::vector<int32_t> &zcnt, std::vector<int32_t> &fptr, std::vector<int32_t> &fsrc, std::vector<int32_t> &foff) {
-    const int KB = band_block(bw), W = band_halfwidth(bw, KB), nsteps = (n + KB - 1) / KB;
-    std::vector<int32_t> pos(n), E(nsteps);
+    std::vector<int32_t> pos(n);
     for (int i = 0; i < n; ++i) pos[perm[i]] = i;
-    // (the front kernel lists the next block's rows whether the envelope reaches them or not: at least KB rows)
-    for (int s = 0; s < nsteps; ++s) E[s] = std::min(n - 1, std::min(s * KB + KB, n) - 1 + std::max(mlow[s], KB));
+    // rows [lo[j], hi[j]] of column j for blocks of kb columns with the envelope (ml, mu)
+    auto ranges = [n](int kb, const std::vector<int32_t> &ml, const std::vector<int32_t> &mu, std::vector<int32_t> &lo, std::vector<int32_t> &hi) {
+        const int nsteps = (n + kb - 1) / kb;
+        std::vector<int32_t> E(nsteps);
+        // (the front kernel lists the next block's rows whether the envelope reaches them or not: at least kb rows)
+        for (int s = 0; s < nsteps; ++s) E[s] = std::min(n - 1, std::min(s * kb + kb, n) - 1 + std::max(int(ml[s]), kb));
+        lo.assign(n, 0); hi.assign(n, 0);
+        int s0 = 0;
+        for (int j = 0; j < n; ++j) {
+            const int sj = j / kb;
+            while (E[s0] < j) ++s0;                                // E is non-decreasing and E[sj] >= j
+            lo[j] = std::min(s0 * kb, std::max(0, sj * kb - int(mu[sj])));
+            hi[j] = E[sj];
+        }
+    };
+    // the factorisation's blocks and, where the solves walk the band in blocks of another width (KBs), theirs as well
+    std::vector<int32_t> lo, hi, lo_s, hi_s;
+    ranges(KB, mlow, mup, lo, hi);
+    if (KBs != KB) {
+        ranges(KBs, mlow_s, mup_s, lo_s, hi_s);
+        for (int j = 0; j < n; ++j) { lo[j] = std::min(lo[j], lo_s[j]); hi[j] = std::max(hi[j], hi_s[j]); }
+    }
     zlo.assign(n, 0); zcnt.assign(n, 0); fptr.assign(n + 1, 0);
     fsrc.clear(); foff.clear();
-    int s0 = 0;
     for (int j = 0; j < n; ++j) {
-        const int sj = j / KB;
-        while (E[s0] < j) ++s0;                                    // E is non-decreasing and E[sj] >= j
-        const int rs = std::min(s0 * KB, std::max(0, sj * KB - mup[sj])), re = E[sj];
-        zlo[j] = W + rs - j;
-        zcnt[j] = re - rs + 1;
+        zlo[j] = W + lo[j] - j;
+        zcnt[j] = hi[j] - lo[j] + 1;
         const int jo = perm[j];
         for (int t = rowptr[jo]; t < rowptr[jo + 1]; ++t) {        // structurally symmetric: rows of column jo = columns of row jo
             const int io = colidx[t];
@@ -1233,45 +1246,43 @@ void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
 
 template <int KB, int NT>
 static cudaError_t factor_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
-    const size_t smem = band_factor_smem(bs.bw);
+    const size_t smem = band_factor_smem(bs.bw, KB);
     cudaError_t e = cudaFuncSetAttribute(k_band_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.bw), bs.mat_doubles, pstride, S, bs.mlow, band, pivots, pivS);
+    k_band_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.W, band_mw(bs.bw), bs.mat_doubles, pstride, S, bs.mlow, band, pivots, pivS);
     return cudaGetLastError();
 }
 
 static int front_ldw(int na_max) { return ((std::max(na_max, 1) + 7) / 16) * 16 + 8; }      // >= na_max, = 8 mod 16
 
-size_t band_front_smem(int bw, int na_max) {
-    const int KB = band_block(bw);
+size_t band_front_smem(int KB, int na_max) {
     return sizeof(double) * (2 * ((size_t)KB * KB + KB) + 2 * (size_t)KB * band_mw(na_max) +
                              (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(2 * na_max + 2) / 2);
 }
 
 template <int KB, int NT>
 static cudaError_t front_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
-    const size_t smem = band_front_smem(bs.bw, bs.na_max);
+    const size_t smem = band_front_smem(bs.kb, bs.na_max);
     cudaError_t e = cudaFuncSetAttribute(k_front_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_front_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
+    k_front_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.W, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
                                                    pstride, S, bs.act_ptr, bs.act_idx, band, pivots, pivS);
     return cudaGetLastError();
 }
 
 int band_front_ldw(int na_max) { return front_ldw(na_max); }
 
-size_t band_slot_smem(int bw, int na_max) {
-    const int KB = band_block(bw);
+size_t band_slot_smem(int KB, int na_max) {
     return sizeof(double) * (2 * ((size_t)KB * KB + KB) + 2 * (size_t)KB * band_mw(na_max) +
                              (size_t)front_ldw(na_max) * std::max(na_max, 1) + (size_t)(5 * na_max + 2) / 2);
 }
 
 template <int KB, int NT>
 static cudaError_t slot_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
-    const size_t smem = band_slot_smem(bs.bw, bs.na_max);
+    const size_t smem = band_slot_smem(bs.kb, bs.na_max);
     cudaError_t e = cudaFuncSetAttribute(k_slot_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_slot_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.bw, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
+    k_slot_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.W, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
                                                   pstride, S, bs.act_ptr, bs.act_idx, bs.act_slot, bs.slot_hi, bs.new_ptr, bs.new_pos, bs.ld_ptr, bs.ld_dst,
                                                   bs.ld_src, band, pivots, pivS);
     return cudaGetLastError();
@@ -1281,15 +1292,15 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstr
     // the front family: 16-column blocks take the slot kernel (measured: ten-species 80-cell 9.1 -> 7.4 ms, mesh 3A 5.6 -> 4.3),
     // 32-column blocks the gather / scatter kernel (config 5: 14.2 against 18.7 ms with slots -- its look-ahead of the next
     // diagonal block and the smaller tile sweep outweigh the round trip of the window there)
-    if (bs.front && bs.slot && band_block(bs.bw) == 16) return slot_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
+    if (bs.front && bs.slot && bs.kb == 16) return slot_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
     if (bs.front) {
-        switch (band_block(bs.bw)) {
+        switch (bs.kb) {
             case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);
             case 16: return front_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
             default: break;      // 8-column blocks mean bw > 832: no front of that size fits (front is false then)
         }
     }
-    switch (band_block(bs.bw)) {
+    switch (bs.kb) {
         case 32: return factor_t<32, 256>(bs, nmat, S, pstride, band, pivots, pivS, st);
         case 16: return bs.bw <= 256 ? factor_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st)
                                      : factor_t<16, BAND_THREADS>(bs, nmat, S, pstride, band, pivots, pivS, st);
@@ -1308,13 +1319,13 @@ static cudaError_t solve_t(const BandSpace &bs, int nb, int S, size_t xstride, s
                            double *x, double *xg, cudaStream_t st) {
     if (xg) {        // vector in global memory: only the diagonal block in shared memory
         const size_t smem = sizeof(double) * (KB * (KB + 1) + KB / 2);
-        k_band_solve<KB, NT, true><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, bs.first, pstride, band, rhs, x, xg);
+        k_band_solve<KB, NT, true><<<nb * S, NT, smem, st>>>(bs.n, bs.W, bs.mat_doubles, xstride, S, bs.perm, bs.mlow_s, bs.mup_s, bs.first, pstride, band, rhs, x, xg);
         return cudaGetLastError();
     }
     const size_t smem = band_solve_smem(bs.n, bs.bw);
     cudaError_t e = cudaFuncSetAttribute(k_band_solve<KB, NT, false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
-    k_band_solve<KB, NT, false><<<nb * S, NT, smem, st>>>(bs.n, bs.bw, bs.mat_doubles, xstride, S, bs.perm, bs.mlow, bs.mup, bs.first, pstride, band, rhs, x, nullptr);
+    k_band_solve<KB, NT, false><<<nb * S, NT, smem, st>>>(bs.n, bs.W, bs.mat_doubles, xstride, S, bs.perm, bs.mlow_s, bs.mup_s, bs.first, pstride, band, rhs, x, nullptr);
     return cudaGetLastError();
 }
 

@@ -82,7 +82,8 @@ int launch_issue_probe(int mode, int blocks, int threads, int iters, const doubl
 // Band LU (landau_band.cu; section III-G)
 struct BandSpace {
     int n, nnz, bw;            // order, CSR entries, half-bandwidth after RCM
-    size_t mat_doubles;        // (2 (bw + KB) + 1) * n doubles per matrix
+    int kb, W;                 // columns per block step of the factorisation (the solves: band_block(bw)); stored half-width
+    size_t mat_doubles;        // (2 W + 1) * n doubles per matrix
     const int32_t *perm;       // [n] device: new -> old
     // fill lists per band column (new numbering): the rows of the column inside the region the factorisation and the
     // solves touch (zeroed: zlo = offset of the first one inside the column, zcnt of them), and the CSR entries of the
@@ -98,7 +99,8 @@ struct BandSpace {
     // slot kernel (band_slot_lists): slot of every list entry, entering rows per step, load list of the entering rows
     const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_src;   // slot_hi[s]: slots in use at step s are below it
     bool slot;
-    const int32_t *mlow, *mup; // [ceil(n/KB)] device: rows below / above block step s inside the envelope
+    const int32_t *mlow, *mup; // [ceil(n/kb)] device: rows below / above block step s inside the envelope
+    const int32_t *mlow_s, *mup_s;   // the same for the solves' block steps of band_block(bw) columns (= mlow, mup when kb is that)
     const int32_t *first;      // [n] device: first column of row i = first row of column i in the ordered pattern
     double flop_per_matrix;    // 2 KB sum mlow^2: window-update flop of one factorisation
 };
@@ -107,25 +109,27 @@ void rcm_order(int n, const std::vector<int32_t> &rowptr, const std::vector<int3
                std::vector<int32_t> &perm, int &bw);
 // half-bandwidth, per-block-step reach inside the envelope (mlow, mup; may be null) and window-update flop of an order
 double band_envelope(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int &bw, std::vector<int32_t> *mlow, std::vector<int32_t> *mup);
-int band_block(int bw);        // KB, a function of bw only
-int band_stored_halfwidth(int bw);   // W: the band stores 2 W + 1 diagonals (bw + KB, at least 2 KB - 1, rounded up to even)
-size_t band_factor_smem(int bw);
+                     int &bw, std::vector<int32_t> *mlow, std::vector<int32_t> *mup, int KB = 0);     // KB = 0: band_block(bw)
+int band_block(int bw);        // columns per block step, a function of bw only: the solves', and the factorisation's unless
+                               // band_factor_block() finds that narrower blocks pay
+int band_stored_halfwidth(int bw);   // W: the band stores 2 W + 1 diagonals (bw + KB, at least 2 KB - 1, rounded up to even; KB = band_block(bw))
+size_t band_factor_smem(int bw, int KB);
 // band points at this grid's block of problem 0; matrix (problem b, species s) = band + b pstride + s mat_doubles
 // (problem-major workspace: a solve may use a different nb than the factorisation)
 void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int bw, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, std::vector<int32_t> &zlo,
+                     int W, int KB, const std::vector<int32_t> &mlow, const std::vector<int32_t> &mup, int KBs,
+                     const std::vector<int32_t> &mlow_s, const std::vector<int32_t> &mup_s, std::vector<int32_t> &zlo,
                      std::vector<int32_t> &zcnt, std::vector<int32_t> &fptr, std::vector<int32_t> &fsrc, std::vector<int32_t> &foff);
 // active lists of the front factorisation (see BandSpace); returns the longest list
 int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                      int bw, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop);
+                      int KB, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop);
 void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int bw, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     int KB, int W, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
                      std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
                      std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src);
 int band_front_ldw(int na_max);
-size_t band_slot_smem(int bw, int na_max);
-size_t band_front_smem(int bw, int na_max);     // dynamic shared memory of the front kernel
+size_t band_slot_smem(int KB, int na_max);
+size_t band_front_smem(int KB, int na_max);     // dynamic shared memory of the front kernel
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st);
 // pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
