@@ -487,6 +487,20 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
                 UPC(G.bs.act_slot, act_slot) UPC(G.bs.new_ptr, new_ptr) UPC(G.bs.new_pos, new_pos)
                 UPC(G.bs.ld_ptr, ld_ptr) UPC(G.bs.ld_dst, ld_dst) UPC(G.bs.ld_src, ld_src)
                 G.bs.slot = kb == 16 && band_slot_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX;
+                {   // the slot kernel's zero lists (BandSpace::zlo_e ...)
+                    const int n = int(hs.n), nsteps = (n + kb - 1) / kb;
+                    std::vector<int32_t> ent_idx, zlo_e(n, 0), zcnt_e(n, 0);
+                    for (int j = 0; j < std::min(kb, n); ++j) { zlo_e[j] = int32_t(Wb) - j; zcnt_e[j] = std::min(kb, n); }    // first diagonal block
+                    for (int st = 0; st < nsteps; ++st)
+                        for (int t = new_ptr[st]; t < new_ptr[st + 1]; ++t) {
+                            const int gi = act_idx[act_ptr[st] + new_pos[t]], k0 = st * kb;
+                            ent_idx.push_back(gi);
+                            zlo_e[gi] = int32_t(Wb) + k0 - gi;          // column gi: the rows of the block it enters beside
+                            zcnt_e[gi] = std::min(k0 + kb, n) - k0;
+                        }
+                    if (ent_idx.empty()) ent_idx.push_back(0);
+                    UPC(G.bs.ent_idx, ent_idx) UPC(G.bs.zlo_e, zlo_e) UPC(G.bs.zcnt_e, zcnt_e)
+                }
             }
             UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
             G.front_fits = band_front_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX && G.bs.na_max <= 160 && kb >= 16;   // FRONT_IR rows per lane

@@ -218,12 +218,17 @@ constexpr int FILL_WARPS = 8;
 __global__ void __launch_bounds__(32 * FILL_WARPS)
 k_band_fill(int n, int nnz, size_t LD, size_t vstride, size_t mat_doubles, size_t pstride, const int32_t *__restrict__ zlo,
             const int32_t *__restrict__ zcnt, const int32_t *__restrict__ fptr, const int32_t *__restrict__ fsrc,
-            const int32_t *__restrict__ foff, const double *__restrict__ vals, double *__restrict__ band) {
+            const int32_t *__restrict__ foff, const int32_t *__restrict__ ent_ptr, const int32_t *__restrict__ ent_idx, int KB, int W,
+            const double *__restrict__ vals, double *__restrict__ band) {
     const int lane = threadIdx.x & 31, pj = blockIdx.x * FILL_WARPS + (threadIdx.x >> 5);
     if (pj >= n) return;
     double *col = band + (size_t)blockIdx.z * pstride + (size_t)blockIdx.y * mat_doubles + (size_t)pj * LD;
     const int z0 = zlo[pj], zc = zcnt[pj];
     for (int r = lane; r < zc; r += 32) col[z0 + r] = 0.0;
+    if (ent_ptr) {          // slot kernel: the rows that enter the front at this column's block step (read as dense panel rows)
+        const int sj = pj / KB;
+        for (int t = ent_ptr[sj] + lane; t < ent_ptr[sj + 1]; t += 32) col[W + ent_idx[t] - pj] = 0.0;
+    }
     __syncwarp();                                  // orders the zeros before the values of this column (same warp)
     const double *v = vals + (size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz;
     for (int t = fptr[pj] + lane; t < fptr[pj + 1]; t += 32) col[foff[t]] = v[fsrc[t]];
@@ -1189,8 +1194,17 @@ cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride,
                              cudaStream_t st) {
     const int W = bs.W;
     dim3 grid((bs.n + FILL_WARPS - 1) / FILL_WARPS, S, nb);
-    k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
-                                                 bs.fsrc, bs.foff, vals, band);
+    // The slot kernel reads nothing of the band but the entries scattered here (its load lists) and writes every entry of
+    // L and U inside the envelope, and the solves read nothing outside the envelope: no zero fill.  The hull kernel and the
+    // gather / scatter front kernel read whole rows of the band: zeros wherever they can look.
+    // In their place (zlo_e, zcnt_e, ent_idx): what that kernel reads as dense panel rows -- the first diagonal block, and
+    // of every row / column the KB entries beside the block at whose step it enters the front.
+    if (bs.front && bs.slot && bs.kb == 16)
+        k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo_e, bs.zcnt_e,
+                                                     bs.fptr, bs.fsrc, bs.foff, bs.new_ptr, bs.ent_idx, bs.kb, W, vals, band);
+    else
+        k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
+                                                     bs.fsrc, bs.foff, nullptr, nullptr, bs.kb, W, vals, band);
     return cudaGetLastError();
 }
 

@@ -99,6 +99,11 @@ struct BandSpace {
     // slot kernel (band_slot_lists): slot of every list entry, entering rows per step, load list of the entering rows
     const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_src;   // slot_hi[s]: slots in use at step s are below it
     bool slot;
+    // what the fill zeroes when the slot kernel factors (it reads the band through its load lists, except the first
+    // diagonal block and the KB entries of an entering row / column beside the block of its entering step): per column
+    // the rows [zlo_e, zlo_e + zcnt_e) (offsets inside the column), and ent_idx[new_ptr[s] .. new_ptr[s + 1]) = the rows
+    // entering at step s, zeroed in the columns of block s
+    const int32_t *zlo_e, *zcnt_e, *ent_idx;
     const int32_t *mlow, *mup; // [ceil(n/kb)] device: rows below / above block step s inside the envelope
     const int32_t *mlow_s, *mup_s;   // the same for the solves' block steps of band_block(bw) columns (= mlow, mup when kb is that)
     const int32_t *first;      // [n] device: first column of row i = first row of column i in the ordered pattern
