@@ -247,6 +247,23 @@ int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, 
 int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,
                               void *stream);
 
+/* landau_band_solve_batched WITHOUT ANY ALLOCATION, for callers that cannot call cudaMalloc (code under CUDA-graph
+ * stream capture, tight serving loops, harnesses that forbid it): same arguments, same factors, same solution up to
+ * rounding (section III-G: the L and U solves of the band solver).  The permuted vectors of the nb * S matrices
+ * live in a scratch that is part of the library image -- a file-scope __device__ array of
+ * LANDAU_STATIC_SCRATCH_DOUBLES doubles (32 MiB), held by every GPU that loads the library until the process exits --
+ * instead of shared memory or the lazily cudaMalloc'ed scratch of landau_band_solve_batched.  Its device address is taken
+ * once per device at landau_create (cudaGetSymbolAddress with that device current); the call itself launches one kernel
+ * per grid on `stream` and calls no cudaMalloc, cudaFree, attribute setter or synchronising routine.
+ * Limit: nb * S_g * n_g <= LANDAU_STATIC_SCRATCH_DOUBLES for every grid g (S_g species, n_g unknowns), otherwise
+ * LANDAU_EINVAL with the sizes in landau_last_cuda_error() and nothing launched; LANDAU_ECUDA when the ctx's device is not
+ * the current one.  All ctx and all calls on a device SHARE the array: it keeps the last call's contents (nothing in it
+ * has to start at zero: a call writes the part it reads), and two such solves that overlap on the GPU -- different
+ * streams, or graphs replayed concurrently -- race; calls on one stream are safe.  x_dev may equal rhs_dev. */
+#define LANDAU_STATIC_SCRATCH_DOUBLES (4u << 20)
+int landau_band_solve_static(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev,
+                             void *stream);
+
 /* End-to-end variant with HOST buffers (pageable or pinned): copies f to the device, runs
  * landau_jacobian_batched on the ctx's own stream in sub-batches whose device-to-host copies overlap
  * the next sub-batch's build, and synchronises.  Values are bitwise those of the device entry point. */

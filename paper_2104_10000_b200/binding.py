@@ -18,6 +18,7 @@ LIB_PATH = os.path.join(_HERE, "liblandau_b200.so")
 LANDAU_OK, LANDAU_EINVAL, LANDAU_ENOMEM, LANDAU_ECUDA = 0, -1, -2, -3
 LANDAU_PAIR_AUTO, LANDAU_PAIR_PER_PROBLEM, LANDAU_PAIR_SHARED = 0, 1, 2
 LANDAU_BAND_AUTO, LANDAU_BAND_HULL, LANDAU_BAND_FRONT = 0, 1, 2
+LANDAU_STATIC_SCRATCH_DOUBLES = 4 << 20      # landau_band_solve_static: doubles of the library's static device scratch
 LANDAU_SHARED_MIN_BATCH = 4
 
 
@@ -64,6 +65,7 @@ SIGNATURES = {
     "landau_band_sizes": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int64), POINTER(c_int64), POINTER(c_double)]),
     "landau_band_factor_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_solve_batched": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
+    "landau_band_solve_static": (c_int, [c_void_p, c_int, c_void_p, c_void_p, c_void_p, c_void_p]),
     "landau_band_front_host": (c_int, [POINTER(landau_mesh), c_int, POINTER(c_int32), POINTER(c_double), POINTER(c_int32)]),
     "landau_band_set_method": (c_int, [c_void_p, c_int]),
     "landau_band_method": (c_int, [c_void_p, c_int, POINTER(c_int32), POINTER(c_int32), POINTER(c_double)]),
@@ -310,6 +312,12 @@ class LandauContext:
         _check(lib().landau_band_solve_batched(self._h, nb, c_void_p(band.data_ptr()), c_void_p(rhs.data_ptr()),
                                                c_void_p(x.data_ptr()), _stream_ptr(stream)))
 
+    def band_solve_static(self, band, rhs, x, stream=None):
+        """landau_band_solve_static: the solve with its vectors in the library's static device scratch (no allocation)."""
+        nb = rhs.shape[0]
+        _check(lib().landau_band_solve_static(self._h, nb, c_void_p(band.data_ptr()), c_void_p(rhs.data_ptr()),
+                                              c_void_p(x.data_ptr()), _stream_ptr(stream)))
+
     def jacobian_host(self, f_host, vals_host=None, Cf_host=None):
         """Host buffers: numpy arrays or pinned CPU torch tensors (float64, contiguous)."""
         def hp(a):
@@ -377,6 +385,7 @@ class LandauMultigridContext:
     band_sizes = LandauContext.band_sizes
     band_factor_batched = LandauContext.band_factor_batched
     band_solve_batched = LandauContext.band_solve_batched
+    band_solve_static = LandauContext.band_solve_static
 
     def species_slices(self):
         out, o = [], 0

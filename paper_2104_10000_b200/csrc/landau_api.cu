@@ -117,6 +117,8 @@ struct landau_ctx {
     bool profiling = false;
     std::vector<ProfEvent> prof_events;  // recorded, not yet read
     std::vector<ProfEvent> prof_pool;    // free
+    int device = -1;                     // the device current at landau_create
+    double *static_scratch = nullptr;    // landau_band_solve_static: address of the library's __device__ scratch on that device
 };
 
 namespace {
@@ -376,6 +378,15 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
     ctx->grids.resize(ngrids);
     ctx->S = S;
     ctx->max_batch = max_batch;
+    {   // set-up of landau_band_solve_static: the device address of the library's static scratch, asked with this device current
+        cudaError_t e = cudaGetDevice(&ctx->device);
+        if (e == cudaSuccess) e = band_static_scratch(&ctx->static_scratch);
+        if (e != cudaSuccess) {
+            cudaGetLastError();
+            g_cuda_err = std::string("cudaGetSymbolAddress(static band-solve scratch): ") + cudaGetErrorString(e);
+            return LANDAU_ECUDA;
+        }
+    }
     ctx->latency_tiles = max_batch < LANDAU_SHARED_MIN_BATCH;
     int rc = LANDAU_OK;
     for (int g = 0; g < ngrids; ++g) {
@@ -895,6 +906,35 @@ int landau_band_solve_batched(landau_ctx *ctx, int nb, const double *band_dev, c
     }
     return launches_ok();
     });
+}
+
+int landau_band_solve_static(landau_ctx *ctx, int nb, const double *band_dev, const double *rhs_dev, double *x_dev, void *stream) {
+    if (!ctx || !band_dev || !rhs_dev || !x_dev || nb < 1 || nb > ctx->max_batch) return LANDAU_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(stream);
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess || dev != ctx->device || !ctx->static_scratch) {
+        cudaGetLastError();
+        g_cuda_err = "landau_band_solve_static: the ctx's device is not current";
+        return LANDAU_ECUDA;
+    }
+    for (auto &g : ctx->grids) {      // checked for every grid before anything is launched
+        const size_t need = size_t(nb) * g.ds.S * g.bs.n;
+        if (need > BAND_STATIC_SCRATCH_DOUBLES) {
+            char msg[192];
+            std::snprintf(msg, sizeof msg, "landau_band_solve_static: nb * S * n = %zu doubles exceed the static scratch of %zu doubles (LANDAU_STATIC_SCRATCH_DOUBLES)",
+                          need, size_t(BAND_STATIC_SCRATCH_DOUBLES));
+            g_cuda_err = msg;
+            return LANDAU_EINVAL;
+        }
+    }
+    // the grids' solves follow one another on the stream: each may use the scratch from its start
+    for (auto &g : ctx->grids) {
+        const cudaError_t e = launch_band_solve_static(g.bs, nb, g.ds.S, ctx->fstride, ctx->bstride, band_dev + g.boff, rhs_dev + g.foff,
+                                                       x_dev + g.foff, ctx->static_scratch, st);
+        if (e != cudaSuccess) { cudaGetLastError(); g_cuda_err = std::string("landau_band_solve_static: ") + cudaGetErrorString(e); return LANDAU_ECUDA; }
+        ctx->launches += 1;
+    }
+    return LANDAU_OK;
 }
 
 int landau_launch_count(const landau_ctx *ctx, int64_t *count) {

@@ -13,6 +13,8 @@
 // zero and stay zero (no pivoting => no fill outside the band).
 #include <cuda_runtime.h>
 
+#include <mutex>
+
 #include <algorithm>
 #include <functional>
 #include <cmath>
@@ -1352,6 +1354,48 @@ cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride
                                      : solve_t<16, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st);
         default: return solve_t<8, BAND_THREADS>(bs, nb, S, xstride, pstride, band, rhs, x, xg, st);
     }
+}
+
+// ------------------------------------------------------------------------------------------------
+// Band solve WITHOUT any allocation (landau_band_solve_static, include/landau.h): the XG instantiation of k_band_solve,
+// whose permuted vectors live in global memory, given a scratch that is part of the library image instead of a
+// cudaMalloc'ed one -- for callers that cannot allocate (stream capture, serving loops, harnesses that forbid it).
+// Every GPU that loads the library holds BAND_STATIC_SCRATCH_DOUBLES * 8 bytes for it until the process exits.
+// In host code the array's NAME is a host-side stand-in, not a device address (a kernel given it faults, or silently
+// uses the wrong memory where the GPU can reach host memory): the address comes from cudaGetSymbolAddress, asked once
+// per device with that device current (band_static_scratch, called at landau_create) and kept.
+// All calls share the array; it keeps the last call's contents.  Nothing in it has to start at zero: a solve first
+// writes the permuted right-hand sides of its nb * S matrices into [0, nb * S * n) and reads nothing beyond.  Two such
+// solves that overlap on the GPU (different streams) race.
+// ------------------------------------------------------------------------------------------------
+static __device__ __align__(256) double g_band_static_scratch[BAND_STATIC_SCRATCH_DOUBLES];
+
+cudaError_t band_static_scratch(double **ptr) {
+    constexpr int MAX_DEV = 64;
+    static std::mutex mu;
+    static double *addr[MAX_DEV] = {};
+    *ptr = nullptr;
+    int dev = -1;
+    cudaError_t e = cudaGetDevice(&dev);
+    if (e != cudaSuccess) return e;
+    if (dev < 0 || dev >= MAX_DEV) return cudaErrorInvalidDevice;
+    std::lock_guard<std::mutex> lock(mu);
+    if (!addr[dev]) {
+        double *p = nullptr;
+        e = cudaGetSymbolAddress(reinterpret_cast<void **>(&p), g_band_static_scratch);
+        if (e != cudaSuccess) return e;
+        addr[dev] = p;
+    }
+    *ptr = addr[dev];
+    return cudaSuccess;
+}
+
+// scratch: band_static_scratch() of the current device; the caller has checked nb * S * bs.n <= BAND_STATIC_SCRATCH_DOUBLES.
+// Launches the kernel only: no attribute call, no allocation (the XG instantiation needs under 9 KB of shared memory).
+cudaError_t launch_band_solve_static(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band,
+                                     const double *rhs, double *x, double *scratch, cudaStream_t st) {
+    if (!scratch || (size_t)nb * S * bs.n > BAND_STATIC_SCRATCH_DOUBLES) return cudaErrorInvalidValue;
+    return launch_band_solve(bs, nb, S, xstride, pstride, band, rhs, x, scratch, st);
 }
 
 }  // namespace landau

@@ -144,6 +144,13 @@ size_t band_solve_smem(int n, int bw);
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
                               double *x, double *xg, cudaStream_t st);
 
+// Band solve with its vectors in a scratch that belongs to the library image (file-scope __device__ array in
+// landau_band.cu; 32 MiB per GPU that loads the library): nothing is allocated.
+constexpr size_t BAND_STATIC_SCRATCH_DOUBLES = size_t(4) << 20;
+cudaError_t band_static_scratch(double **ptr);      // its device address on the CURRENT device (cudaGetSymbolAddress, once per device)
+cudaError_t launch_band_solve_static(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band,
+                                     const double *rhs, double *x, double *scratch, cudaStream_t st);
+
 int pair_tile_size(int N, bool latency);
 int pair_tiles(int N, bool latency);
 
