@@ -177,7 +177,7 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
         }
         const int ksplit = shared_ksplit(N);
         ctx->launches += timed(ctx, 1, st, [&]() { return launch_apply(N, nb, ctx->nbpad, ctx->sc.U, ctx->sc.T, ksplit > 1 ? ctx->sc.G : Gsum, st); });
-        if (ksplit > 1) ctx->launches += launch_sum_partials(N, nb, ksplit, ctx->sc.G, Gsum, st);
+        if (ksplit > 1) ctx->launches += launch_sum_partials(N, nb, ksplit, false, ctx->sc.G, Gsum, st);
         return;
     }
     // Per-problem path: a group of pp_chunk problems at a time, so that the per-source-tile slabs (ntiles * 5 N doubles
@@ -188,7 +188,7 @@ void inner_integral(landau_ctx *ctx, int nb, const double *f_dev, double *Gsum, 
         const double *fc = f_dev + size_t(b0) * ctx->fstride;
         for (auto &g : ctx->grids) ctx->launches += launch_fields_beta(g.ds, nbc, fc + g.foff, ctx->sc.T, g.ce + size_t(b0) * g.ds.S * g.ds.Ne * g.ds.Nb, st);
         ctx->launches += timed(ctx, 0, st, [&]() { return launch_pair(N, ctx->latency_tiles, ctx->r, ctx->z, ctx->invr, ctx->check_all, nbc, ctx->sc.T, ctx->sc.G, st); });
-        ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N, ctx->latency_tiles), ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
+        ctx->launches += launch_sum_partials(N, nbc, pair_tiles(N, ctx->latency_tiles), ctx->latency_tiles, ctx->sc.G, Gsum + size_t(b0) * 5 * N, st);
     }
 }
 
@@ -285,6 +285,9 @@ constexpr int MERGED_GATHER_MAX_NB = 8;
 // a4-a7 for nb problems; Ez == nullptr: collision Jacobian and C(f), else the implicit-step operator
 void assemble(landau_ctx *ctx, int nb, const double *f_dev, const double *Ez, double shift, double *vals_dev, double *Cf_dev,
               cudaStream_t st) {
+    // (letting k_element add the pair kernel's slabs itself in single-build contexts of Q2 grids -- one launch fewer --
+    // was measured slower: config 1 21.8 against 19.5 us per build; the slab sum as a kernel of its own overlaps its
+    // neighbours' launch latencies under programmatic dependent launch)
     for (auto &g : ctx->grids) {
         ctx->launches += launch_element(g.ds, nb, 1, f_dev + g.foff, ctx->sc.Gsum, g.Ce, g.ce, Ez, shift, st);
         if (vals_dev && Cf_dev && nb <= MERGED_GATHER_MAX_NB) {

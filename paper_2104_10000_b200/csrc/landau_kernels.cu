@@ -169,6 +169,8 @@ k_pair_sym(int N, int ntiles, const double *__restrict__ r, const double *__rest
 // for the same 32 targets i and for the j it visited; they are added over the warps in warp order, so the
 // summation order is again a function of N alone.  N = 450: 17.5 -> 6 us, N = 2048: 28.7 -> 17 us.
 template <int WS, bool CHECK_ALL>
+// (compiled for 14 or 16 blocks of two warps per SM -- 72 / 64 registers instead of 80, all 2,080 tile pairs of N = 2,048
+// resident at once -- it is slower: 28.3 against 26.7 us; the kernel is bound by its issue slots, not by a partial wave)
 __global__ void __launch_bounds__(32 * WS)
 k_pair_split(int N, int ntiles, const double *__restrict__ r, const double *__restrict__ z, const double *__restrict__ invr,
              const double *__restrict__ T, double *__restrict__ Gpart) {
@@ -666,6 +668,41 @@ __global__ void k_sum_partials(int n5, int jsplit, const double *__restrict__ Gp
     G[b * n5 + t] = acc;
 }
 
+// The same sum for many partials (per-problem path: one slab per source tile, 15 ... 154 of them).  A single build has only
+// 5 N outputs: one thread per output walking all slabs leaves most of the GPU idle and pays the slabs' latencies one
+// after the other (N = 2,048: 9.4 us, N = 4,928: 19.5 us).  Here 8 warps share 32 outputs: warp g adds the slabs g, g + 8,
+// g + 16, ... (four loads in flight), the eight group sums are then added in group order -- a fixed order that depends on
+// the number of slabs only, so a batched build stays bitwise equal to single builds.
+constexpr int SUMP_GROUPS = 8;
+constexpr int SUMP_MIN_SLABS = 8;      // fewer slabs (the shared path's 1 ... 4 j-splits): k_sum_partials
+__global__ void __launch_bounds__(32 * SUMP_GROUPS)
+k_sum_partials_split(int n5, int jsplit, const double *__restrict__ Gpart, double *__restrict__ G) {
+    pdl_prologue();
+    __shared__ double sp[SUMP_GROUPS][32];
+    const int o = threadIdx.x & 31, sg = threadIdx.x >> 5;
+    const int t = blockIdx.x * 32 + o;
+    const size_t b = blockIdx.y;
+    double acc = 0.0;
+    if (t < n5) {
+        const double *p = Gpart + b * jsplit * n5 + t;
+        int js = sg;
+        for (; js + 3 * SUMP_GROUPS < jsplit; js += 4 * SUMP_GROUPS) {
+            const double a0 = p[(size_t)js * n5], a1 = p[(size_t)(js + SUMP_GROUPS) * n5];
+            const double a2 = p[(size_t)(js + 2 * SUMP_GROUPS) * n5], a3 = p[(size_t)(js + 3 * SUMP_GROUPS) * n5];
+            acc += a0; acc += a1; acc += a2; acc += a3;
+        }
+        for (; js < jsplit; js += SUMP_GROUPS) acc += p[(size_t)js * n5];
+    }
+    sp[sg][o] = acc;
+    __syncthreads();
+    if (sg == 0 && t < n5) {
+        double sum = sp[0][o];
+#pragma unroll
+        for (int g = 1; g < SUMP_GROUPS; ++g) sum += sp[g][o];
+        G[b * n5 + t] = sum;
+    }
+}
+
 // FP64 peak probe: 8 independent DFMA chains per thread, all operands in registers.
 __global__ void k_dfma_probe(int iters, double *out) {
     double x0 = threadIdx.x * 1e-9, x1 = x0 + 1, x2 = x0 + 2, x3 = x0 + 3, x4 = x0 + 4, x5 = x0 + 5, x6 = x0 + 6, x7 = x0 + 7;
@@ -812,7 +849,15 @@ __global__ void k_gather2(DeviceSpace ds, int bv, size_t vstride, size_t fstride
     const int t0 = ptr[kk], t1 = ptr[kk + 1];
     const double2 hw = *reinterpret_cast<const double2 *>(head + kk);
     double acc = fma(hw.x, s[__double2loint(hw.y)], 0.0);
-    for (int t = t0 + 1; t < t1; ++t) acc = fma(w[t], s[idx[t]], acc);
+    // entries shared by several cells or fed by hanging nodes have long lists: four items in flight, added in list order
+    int t = t0 + 1;
+    for (; t + 3 < t1; t += 4) {
+        const int i0 = idx[t], i1 = idx[t + 1], i2 = idx[t + 2], i3 = idx[t + 3];
+        const double w0 = w[t], w1 = w[t + 1], w2 = w[t + 2], w3 = w[t + 3];
+        const double v0 = s[i0], v1 = s[i1], v2 = s[i2], v3 = s[i3];
+        acc = fma(w0, v0, acc); acc = fma(w1, v1, acc); acc = fma(w2, v2, acc); acc = fma(w3, v3, acc);
+    }
+    for (; t < t1; ++t) acc = fma(w[t], s[idx[t]], acc);
     (isv ? vals : Cf)[(size_t)blockIdx.z * (isv ? vstride : fstride) + (size_t)blockIdx.y * K + kk] = acc;
 }
 
@@ -841,8 +886,15 @@ int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStr
     return 1;
 }
 
-int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st) {
+int launch_sum_partials(int Ntot, int nb, int jsplit, bool latency, const double *Gpart, double *G, cudaStream_t st) {
     const int n5 = 5 * Ntot;
+    // chosen by the ctx's tiling policy (contexts made for single builds) and the number of slabs, never by nb: in a large
+    // batch the plain kernel is DRAM-bound already and the split one a few per cent slower (8,192 x N = 450: 9.04 -> 9.55 ms)
+    if (latency && jsplit >= SUMP_MIN_SLABS) {
+        dim3 grid((n5 + 31) / 32, nb);
+        launch_k(k_sum_partials_split, grid, dim3(32 * SUMP_GROUPS), 0, st, nb <= PDL_MAX_NB, n5, jsplit, Gpart, G);
+        return 1;
+    }
     dim3 grid((n5 + 255) / 256, nb);
     launch_k(k_sum_partials, grid, dim3(256), 0, st, nb <= PDL_MAX_NB, n5, jsplit, Gpart, G);
     return 1;

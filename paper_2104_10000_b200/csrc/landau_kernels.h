@@ -75,7 +75,7 @@ int launch_gather_cf(const DeviceSpace &ds, int nb, size_t ostride, const double
 int launch_gather_both(const DeviceSpace &ds, int nb, size_t vstride, size_t fstride, const double *Ce, const double *ce,
                        double *vals, double *Cf, cudaStream_t st);
 int launch_mass_element(const DeviceSpace &ds, double shift, double *Ce, cudaStream_t st);
-int launch_sum_partials(int Ntot, int nb, int jsplit, const double *Gpart, double *G, cudaStream_t st);
+int launch_sum_partials(int Ntot, int nb, int jsplit, bool latency, const double *Gpart, double *G, cudaStream_t st);
 int launch_dfma_probe(int blocks, int threads, int iters, double *out, cudaStream_t st);
 int launch_issue_probe(int mode, int blocks, int threads, int iters, const double *in, double *out, long long *cycles, cudaStream_t st);
 
