@@ -490,31 +490,18 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             G.bs.na_max = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, act_ptr, act_idx, &G.bs.front_flop);
             if (act_idx.empty()) act_idx.push_back(0);
             {
-                std::vector<int32_t> act_slot, slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src;
-                band_slot_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, int(Wb), band_front_ldw(G.bs.na_max), act_ptr, act_idx, G.bs.na_max, act_slot,
-                                slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_src);
+                std::vector<int32_t> act_slot, slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_csr, d0_csr;
+                band_slot_lists(int(hs.n), hs.rowptr, hs.colidx, perm, kb, band_front_ldp(G.bs.na_max), band_front_ldw(G.bs.na_max), act_ptr, act_idx, G.bs.na_max, act_slot,
+                                slot_hi, new_ptr, new_pos, ld_ptr, ld_dst, ld_csr, d0_csr);
                 if (slot_hi.empty()) slot_hi.push_back(0);
                 UPC(G.bs.slot_hi, slot_hi)
                 if (act_slot.empty()) act_slot.push_back(0);
                 if (new_pos.empty()) new_pos.push_back(0);
-                if (ld_dst.empty()) { ld_dst.push_back(0); ld_src.push_back(0); }
+                if (ld_dst.empty()) { ld_dst.push_back(0); ld_csr.push_back(-1); }
                 UPC(G.bs.act_slot, act_slot) UPC(G.bs.new_ptr, new_ptr) UPC(G.bs.new_pos, new_pos)
-                UPC(G.bs.ld_ptr, ld_ptr) UPC(G.bs.ld_dst, ld_dst) UPC(G.bs.ld_src, ld_src)
+                UPC(G.bs.ld_ptr, ld_ptr) UPC(G.bs.ld_dst, ld_dst) UPC(G.bs.ld_csr, ld_csr)
+                UPC(G.bs.d0_csr, d0_csr)
                 G.bs.slot = kb == 16 && band_slot_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX;
-                {   // the slot kernel's zero lists (BandSpace::zlo_e ...)
-                    const int n = int(hs.n), nsteps = (n + kb - 1) / kb;
-                    std::vector<int32_t> ent_idx, zlo_e(n, 0), zcnt_e(n, 0);
-                    for (int j = 0; j < std::min(kb, n); ++j) { zlo_e[j] = int32_t(Wb) - j; zcnt_e[j] = std::min(kb, n); }    // first diagonal block
-                    for (int st = 0; st < nsteps; ++st)
-                        for (int t = new_ptr[st]; t < new_ptr[st + 1]; ++t) {
-                            const int gi = act_idx[act_ptr[st] + new_pos[t]], k0 = st * kb;
-                            ent_idx.push_back(gi);
-                            zlo_e[gi] = int32_t(Wb) + k0 - gi;          // column gi: the rows of the block it enters beside
-                            zcnt_e[gi] = std::min(k0 + kb, n) - k0;
-                        }
-                    if (ent_idx.empty()) ent_idx.push_back(0);
-                    UPC(G.bs.ent_idx, ent_idx) UPC(G.bs.zlo_e, zlo_e) UPC(G.bs.zcnt_e, zcnt_e)
-                }
             }
             UPC(G.bs.act_ptr, act_ptr) UPC(G.bs.act_idx, act_idx)
             G.front_fits = band_front_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX && G.bs.na_max <= 160 && kb >= 16;   // FRONT_IR rows per lane
@@ -859,9 +846,11 @@ int landau_band_factor_batched(landau_ctx *ctx, int nb, const double *vals_dev, 
     for (auto &g : ctx->grids) {
         if (band_factor_smem(g.bs.bw, g.bs.kb) > 227 * 1024) return LANDAU_EINVAL;
         double *band = band_dev + g.boff;
-        CK(launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, ctx->bstride, vals_dev + g.voff, band, st));
-        CK(launch_band_factor(g.bs, nb * g.ds.S, g.ds.S, ctx->bstride, band, pivots_dev ? pivots_dev + 2 * g.s0 : nullptr, ctx->S, st));
-        ctx->launches += 2;
+        const bool fill = band_needs_fill(g.bs);
+        if (fill) CK(launch_band_fill(g.bs, nb, g.ds.S, ctx->vstride, ctx->bstride, vals_dev + g.voff, band, st));
+        CK(launch_band_factor(g.bs, nb * g.ds.S, g.ds.S, ctx->bstride, vals_dev + g.voff, ctx->vstride, band,
+                              pivots_dev ? pivots_dev + 2 * g.s0 : nullptr, ctx->S, st));
+        ctx->launches += fill ? 2 : 1;
     }
     return launches_ok();
 }

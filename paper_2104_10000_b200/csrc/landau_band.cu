@@ -220,17 +220,12 @@ constexpr int FILL_WARPS = 8;
 __global__ void __launch_bounds__(32 * FILL_WARPS)
 k_band_fill(int n, int nnz, size_t LD, size_t vstride, size_t mat_doubles, size_t pstride, const int32_t *__restrict__ zlo,
             const int32_t *__restrict__ zcnt, const int32_t *__restrict__ fptr, const int32_t *__restrict__ fsrc,
-            const int32_t *__restrict__ foff, const int32_t *__restrict__ ent_ptr, const int32_t *__restrict__ ent_idx, int KB, int W,
-            const double *__restrict__ vals, double *__restrict__ band) {
+            const int32_t *__restrict__ foff, const double *__restrict__ vals, double *__restrict__ band) {
     const int lane = threadIdx.x & 31, pj = blockIdx.x * FILL_WARPS + (threadIdx.x >> 5);
     if (pj >= n) return;
     double *col = band + (size_t)blockIdx.z * pstride + (size_t)blockIdx.y * mat_doubles + (size_t)pj * LD;
     const int z0 = zlo[pj], zc = zcnt[pj];
     for (int r = lane; r < zc; r += 32) col[z0 + r] = 0.0;
-    if (ent_ptr) {          // slot kernel: the rows that enter the front at this column's block step (read as dense panel rows)
-        const int sj = pj / KB;
-        for (int t = ent_ptr[sj] + lane; t < ent_ptr[sj + 1]; t += 32) col[W + ent_idx[t] - pj] = 0.0;
-    }
     __syncwarp();                                  // orders the zeros before the values of this column (same warp)
     const double *v = vals + (size_t)blockIdx.z * vstride + (size_t)blockIdx.y * nnz;
     for (int t = fptr[pj] + lane; t < fptr[pj + 1]; t += 32) col[foff[t]] = v[fsrc[t]];
@@ -776,14 +771,15 @@ k_front_factor(int n, int W, int LDP, int LDW, int na_max, size_t mat_doubles, s
 // Shared memory (doubles): 2 x (sD[KB][KB], sDi[KB]), sL[KB][LDP], sU[KB][LDP], sW[NS][LDW], then 5 NS ints.
 // Named barriers: 2 = warp 0 has the block out of the window, 3 / 4 / 5 = among the workers.
 // ------------------------------------------------------------------------------------------------
+constexpr int SLOT_NO_DST = INT32_MIN;
 constexpr int SLOT_LB = 8;                     // band loads a worker thread keeps in flight when it assembles entering rows
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
 k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t pstride, int S,
               const int32_t *__restrict__ act_ptr, const int32_t *__restrict__ act_idx, const int32_t *__restrict__ act_slot,
               const int32_t *__restrict__ slot_hi, const int32_t *__restrict__ new_ptr, const int32_t *__restrict__ new_pos, const int32_t *__restrict__ ld_ptr,
-              const int32_t *__restrict__ ld_dst, const int32_t *__restrict__ ld_src, double *__restrict__ band_all,
-              double *__restrict__ pivots, int pivS) {
+              const int32_t *__restrict__ ld_dst, const int32_t *__restrict__ ld_csr, const int32_t *__restrict__ d0_csr, const double *__restrict__ vals_all, size_t vstride, int nnz,
+              double *__restrict__ band_all, double *__restrict__ pivots, int pivS) {
     extern __shared__ double smem[];
     constexpr int DSZ = KB * KB + KB;
     constexpr int NW = NT / 32, NTW = NT - 32;
@@ -795,6 +791,9 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
     int *sActN = sSlot + NS, *sSlotN = sActN + NS, *sNew = sSlotN + NS;                   // the next step's; positions of its entering rows
     const size_t lda = 2 * (size_t)W;
     double *A = band_all + (size_t)(blockIdx.x / S) * pstride + (size_t)(blockIdx.x % S) * mat_doubles + W;   // A(i,j) = A[i + j*lda]
+    // The matrix itself is read from the CSR values (lists of CSR indices, -1 = no entry): the band workspace needs no
+    // fill for this kernel and only ever holds L and U.
+    const double *V = vals_all + (size_t)(blockIdx.x / S) * vstride + (size_t)(blockIdx.x % S) * nnz;
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, k = lane & 3;
     double pmin = 1.79e308, pmax = 0.0;
@@ -816,29 +815,29 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
 #pragma unroll
             for (int q = 0; q < SLOT_LB; ++q) {
                 const int eq = e + q * nt;
-                d[q] = eq < e1 ? ld_dst[eq] : -1;
-                v[q] = eq < e1 ? A[ld_src[eq]] : 0.0;
+                d[q] = eq < e1 ? ld_dst[eq] : SLOT_NO_DST;
+                const int cs = eq < e1 ? ld_csr[eq] : -1;
+                v[q] = cs >= 0 ? V[cs] : 0.0;
             }
 #pragma unroll
             for (int q = 0; q < SLOT_LB; ++q)
-                if (d[q] >= 0) sW[d[q]] = v[q];
+                if (d[q] != SLOT_NO_DST) sW[d[q]] = v[q];      // (negative offsets: the panels sL, sU in front of the window)
         }
     };
     // raw panels of the step whose block starts at k0 (kb columns): thread per list position; carried rows from the
-    // window's pivot columns / rows (slots in ps), entering rows from the band; all loads of a row before its stores
-    auto raw_panels = [&](int k0, int kb, int na, const int *la, const int *ls, const int *ps, const int *ln, int nnew, int t, int nt) {
+    // window's pivot columns / rows (slots in ps), entering rows zero (their few entries beside the block come with the
+    // step's load list, which reaches into the panels); all loads of a row before its stores
+    auto raw_panels = [&](int kb, int na, const int *ls, const int *ps, const int *ln, int nnew, int t, int nt) {
         for (int i = t; i < na; i += nt) {
-            const int gi = la[i], sl = ls[i];
+            const int sl = ls[i];
             bool isnew = ps == nullptr;
             for (int q = 0; q < nnew; ++q) isnew |= ln[q] == i;
 #pragma unroll 1
             for (int side = 0; side < 2; ++side) {          // the L row, then the U column: KB staging registers at a time
                 double pa[KB];
                 if (isnew) {
-                    const double *src = side == 0 ? A + gi + (size_t)k0 * lda : A + k0 + (size_t)gi * lda;
-                    const size_t st = side == 0 ? lda : 1;
 #pragma unroll
-                    for (int c = 0; c < KB; ++c) pa[c] = c < kb ? src[(size_t)c * st] : 0.0;
+                    for (int c = 0; c < KB; ++c) pa[c] = 0.0;
                 } else {
 #pragma unroll
                     for (int c = 0; c < KB; ++c) {
@@ -853,7 +852,16 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
         }
     };
 
-    // prologue: first diagonal block (warp 0); everything zero, then the first front assembled from the band
+    // prologue: first diagonal block (warp 0; copied from the matrix into its place in the band first); everything zero,
+    // then the first front assembled from the matrix
+    {
+        const int kb0 = min(KB, n);
+        for (int e = tid; e < kb0 * kb0; e += NT) {
+            const int i = e % kb0, j = e / kb0, cs = d0_csr[i + j * KB];
+            A[i + (size_t)j * lda] = cs >= 0 ? V[cs] : 0.0;
+        }
+        __syncthreads();
+    }
     if (warp == 0) {
         const double2 pv = factor_diag_src<KB, 0>(A, lda, A, lda, min(KB, n), smem, smem + KB * KB, lane, NT);
         pmin = fmin(pmin, pv.x); pmax = fmax(pmax, pv.y);
@@ -865,7 +873,8 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
         for (int i = tid; i < 2 * KB * LDP; i += NT) sL[i] = 0.0;                  // sL and sU are contiguous
         for (int i = tid; i < LDW * NS; i += NT) sW[i] = 0.0;
         __syncthreads();
-        raw_panels(0, min(KB, n), na, sAct, sSlot, nullptr, sNew, nnew, tid, NT);
+        raw_panels(min(KB, n), na, sSlot, nullptr, sNew, nnew, tid, NT);
+        __syncthreads();                        // the load list also writes panel entries of these rows
         load_new(0, tid, NT);
     }
     int cur = 0;
@@ -995,7 +1004,7 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
                 sL[(size_t)c * LDP + sl] = 0.0; sU[(size_t)c * LDP + sl] = 0.0;
             }
             named_bar_sync(4, NTW);             // ... before an entering row that takes such a slot writes its own
-            if (kbn > 0) raw_panels(k0 + kb, kbn, nan, sActN, sSlotN, sSlot, sNew, nnew, t, NTW);
+            if (kbn > 0) raw_panels(kbn, nan, sSlotN, sSlot, sNew, nnew, t, NTW);
             named_bar_sync(3, NTW);             // the workers have read the pivot columns / rows of the window
             named_bar_sync(2, NT);              // warp 0 has its block out of it
             zero_new(nnew, sSlotN, sNew, t, NTW);
@@ -1135,19 +1144,31 @@ int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vect
 // free one (na_max slots suffice: the pivot rows of a step have been taken out before that step's new rows arrive) -- so
 // the window is never re-packed and never travels.  Per block step s: act_slot (aligned with act_idx), new_pos (positions
 // in list s of the rows that ENTER at step s) and the load list of step s: the original entries (i, j) of the matrix
-// with i entering and j in list s (or both entering), as (offset in the window, offset in the band) -- the entering rows are
-// assembled sparsely, everything else of their rows / columns is zero.
+// with i entering and j in list s (or both entering), as (offset in the window, index into the CSR values) -- the entering
+// rows are assembled sparsely, everything else of their rows / columns is zero.  The list of step s also carries the
+// entries of the entering rows beside the block of that step, A(i, k0 + c) and A(k0 + c, i): they belong into the raw
+// panels sL[c ldp + slot], sU[c ldp + slot], which lie in front of the window in shared memory (negative offsets).
+// d0_csr[i + j KB]: CSR index of the entry (i, j) of the first diagonal block, -1 where the matrix has none.
 void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int KB, int W, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     int KB, int ldp, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
                      std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
-                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src) {
+                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_csr, std::vector<int32_t> &d0_csr) {
     const int nsteps = (n + KB - 1) / KB;
-    const long long lda = 2LL * W;
     std::vector<int32_t> pos(n);
     for (int i = 0; i < n; ++i) pos[perm[i]] = i;
+    // CSR index of the entry (i, j) (new numbering) or -1
+    auto csr_of = [&](int i, int j) {
+        const int io = perm[i], jo = perm[j];
+        const int32_t *b = colidx.data() + rowptr[io], *e = colidx.data() + rowptr[io + 1];
+        const int32_t *hit = std::lower_bound(b, e, int32_t(jo));
+        return (hit != e && *hit == jo) ? int32_t(hit - colidx.data()) : int32_t(-1);
+    };
+    d0_csr.assign((size_t)KB * KB, -1);
+    for (int j = 0; j < std::min(KB, n); ++j)
+        for (int i = 0; i < std::min(KB, n); ++i) d0_csr[i + (size_t)j * KB] = csr_of(i, j);
     act_slot.assign(act_idx.size(), 0);
     new_ptr.assign(nsteps + 1, 0); ld_ptr.assign(nsteps + 1, 0); slot_hi.assign(nsteps, 0);
-    new_pos.clear(); ld_dst.clear(); ld_src.clear();
+    new_pos.clear(); ld_dst.clear(); ld_csr.clear();
     std::vector<int32_t> slot_of(n, -1), entered(n, -1);
     std::vector<int> free_slots;                          // kept sorted descending: pop_back gives the lowest
     for (int k = na_max - 1; k >= 0; --k) free_slots.push_back(k);
@@ -1175,8 +1196,14 @@ void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
                 const int j = pos[colidx[u]];
                 if (slot_of[j] < 0) continue;            // not in this step's list: eliminated, in the block, or not yet active
                 // (i, j) and, unless j enters at this step too (its own pass covers it), (j, i)
-                ld_dst.push_back(int32_t(si + slot_of[j] * ldw)); ld_src.push_back(int32_t(i + j * lda));
-                if (entered[j] != s) { ld_dst.push_back(int32_t(slot_of[j] + si * ldw)); ld_src.push_back(int32_t(j + i * lda)); }
+                ld_dst.push_back(int32_t(si + slot_of[j] * ldw)); ld_csr.push_back(int32_t(u));
+                if (entered[j] != s) { ld_dst.push_back(int32_t(slot_of[j] + si * ldw)); ld_csr.push_back(csr_of(j, i)); }
+            }
+            const int k0 = s * KB;                        // beside the block: sL at -2 KB ldp, sU at -KB ldp from the window
+            for (int c = 0; c < KB && k0 + c < n; ++c) {
+                const int32_t cl = csr_of(i, k0 + c), cu = csr_of(k0 + c, i);
+                if (cl >= 0) { ld_dst.push_back(int32_t(-2 * KB * ldp + c * ldp + si)); ld_csr.push_back(cl); }
+                if (cu >= 0) { ld_dst.push_back(int32_t(-KB * ldp + c * ldp + si)); ld_csr.push_back(cu); }
             }
         }
         ld_ptr[s + 1] = int32_t(ld_dst.size());
@@ -1196,17 +1223,9 @@ cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride,
                              cudaStream_t st) {
     const int W = bs.W;
     dim3 grid((bs.n + FILL_WARPS - 1) / FILL_WARPS, S, nb);
-    // The slot kernel reads nothing of the band but the entries scattered here (its load lists) and writes every entry of
-    // L and U inside the envelope, and the solves read nothing outside the envelope: no zero fill.  The hull kernel and the
-    // gather / scatter front kernel read whole rows of the band: zeros wherever they can look.
-    // In their place (zlo_e, zcnt_e, ent_idx): what that kernel reads as dense panel rows -- the first diagonal block, and
-    // of every row / column the KB entries beside the block at whose step it enters the front.
-    if (bs.front && bs.slot && bs.kb == 16)
-        k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo_e, bs.zcnt_e,
-                                                     bs.fptr, bs.fsrc, bs.foff, bs.new_ptr, bs.ent_idx, bs.kb, W, vals, band);
-    else
-        k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
-                                                     bs.fsrc, bs.foff, nullptr, nullptr, bs.kb, W, vals, band);
+    // (not launched when the slot kernel factors: band_needs_fill)
+    k_band_fill<<<grid, 32 * FILL_WARPS, 0, st>>>(bs.n, bs.nnz, 2 * (size_t)W + 1, vstride, bs.mat_doubles, pstride, bs.zlo, bs.zcnt, bs.fptr,
+                                                 bs.fsrc, bs.foff, vals, band);
     return cudaGetLastError();
 }
 
@@ -1287,6 +1306,7 @@ static cudaError_t front_t(const BandSpace &bs, int nmat, int S, size_t pstride,
 }
 
 int band_front_ldw(int na_max) { return front_ldw(na_max); }
+int band_front_ldp(int na_max) { return band_mw(na_max); }       // leading dimension of the raw panels
 
 size_t band_slot_smem(int KB, int na_max) {
     return sizeof(double) * (2 * ((size_t)KB * KB + KB) + 2 * (size_t)KB * band_mw(na_max) +
@@ -1294,21 +1314,27 @@ size_t band_slot_smem(int KB, int na_max) {
 }
 
 template <int KB, int NT>
-static cudaError_t slot_t(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+static cudaError_t slot_t(const BandSpace &bs, int nmat, int S, size_t pstride, const double *vals, size_t vstride, double *band, double *pivots,
+                          int pivS, cudaStream_t st) {
     const size_t smem = band_slot_smem(bs.kb, bs.na_max);
     cudaError_t e = cudaFuncSetAttribute(k_slot_factor<KB, NT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem);
     if (e != cudaSuccess) return e;
     k_slot_factor<KB, NT><<<nmat, NT, smem, st>>>(bs.n, bs.W, band_mw(bs.na_max), front_ldw(bs.na_max), std::max(bs.na_max, 1), bs.mat_doubles,
                                                   pstride, S, bs.act_ptr, bs.act_idx, bs.act_slot, bs.slot_hi, bs.new_ptr, bs.new_pos, bs.ld_ptr, bs.ld_dst,
-                                                  bs.ld_src, band, pivots, pivS);
+                                                  bs.ld_csr, bs.d0_csr, vals, vstride, bs.nnz, band, pivots, pivS);
     return cudaGetLastError();
 }
 
-cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st) {
+// true: launch_band_fill first.  The slot kernel reads the matrix from the CSR values itself and writes every entry of
+// L and U inside the envelope (the solves read nothing outside it): no fill, the workspace may hold anything.
+bool band_needs_fill(const BandSpace &bs) { return !(bs.front && bs.slot && bs.kb == 16); }
+
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, const double *vals, size_t vstride, double *band,
+                               double *pivots, int pivS, cudaStream_t st) {
     // the front family: 16-column blocks take the slot kernel (measured: ten-species 80-cell 9.1 -> 7.4 ms, mesh 3A 5.6 -> 4.3),
     // 32-column blocks the gather / scatter kernel (config 5: 14.2 against 18.7 ms with slots -- its look-ahead of the next
     // diagonal block and the smaller tile sweep outweigh the round trip of the window there)
-    if (bs.front && bs.slot && bs.kb == 16) return slot_t<16, 128>(bs, nmat, S, pstride, band, pivots, pivS, st);
+    if (!band_needs_fill(bs)) return slot_t<16, 128>(bs, nmat, S, pstride, vals, vstride, band, pivots, pivS, st);
     if (bs.front) {
         switch (bs.kb) {
             case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);

@@ -97,13 +97,9 @@ struct BandSpace {
     double front_flop;         // window-update flop of one factorisation by the front kernel (2 KB sum na_s^2)
     bool front;
     // slot kernel (band_slot_lists): slot of every list entry, entering rows per step, load list of the entering rows
-    const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_src;   // slot_hi[s]: slots in use at step s are below it
+    const int32_t *act_slot, *slot_hi, *new_ptr, *new_pos, *ld_ptr, *ld_dst, *ld_csr;   // slot_hi[s]: slots in use at step s are below it
+    const int32_t *d0_csr;            // CSR indices of the first diagonal block
     bool slot;
-    // what the fill zeroes when the slot kernel factors (it reads the band through its load lists, except the first
-    // diagonal block and the KB entries of an entering row / column beside the block of its entering step): per column
-    // the rows [zlo_e, zlo_e + zcnt_e) (offsets inside the column), and ent_idx[new_ptr[s] .. new_ptr[s + 1]) = the rows
-    // entering at step s, zeroed in the columns of block s
-    const int32_t *zlo_e, *zcnt_e, *ent_idx;
     const int32_t *mlow, *mup; // [ceil(n/kb)] device: rows below / above block step s inside the envelope
     const int32_t *mlow_s, *mup_s;   // the same for the solves' block steps of band_block(bw) columns (= mlow, mup when kb is that)
     const int32_t *first;      // [n] device: first column of row i = first row of column i in the ordered pattern
@@ -129,16 +125,20 @@ void band_fill_lists(int n, const std::vector<int32_t> &rowptr, const std::vecto
 int band_active_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
                       int KB, std::vector<int32_t> &act_ptr, std::vector<int32_t> &act_idx, double *front_flop);
 void band_slot_lists(int n, const std::vector<int32_t> &rowptr, const std::vector<int32_t> &colidx, const std::vector<int32_t> &perm,
-                     int KB, int W, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
+                     int KB, int ldp, int ldw, const std::vector<int32_t> &act_ptr, const std::vector<int32_t> &act_idx, int na_max,
                      std::vector<int32_t> &act_slot, std::vector<int32_t> &slot_hi, std::vector<int32_t> &new_ptr, std::vector<int32_t> &new_pos,
-                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_src);
+                     std::vector<int32_t> &ld_ptr, std::vector<int32_t> &ld_dst, std::vector<int32_t> &ld_csr, std::vector<int32_t> &d0_csr);
 int band_front_ldw(int na_max);
+int band_front_ldp(int na_max);
 size_t band_slot_smem(int KB, int na_max);
 size_t band_front_smem(int KB, int na_max);     // dynamic shared memory of the front kernel
 cudaError_t launch_band_fill(const BandSpace &bs, int nb, int S, size_t vstride, size_t pstride, const double *vals, double *band,
                              cudaStream_t st);
 // pivots: nullptr or (min |pivot|, max |pivot|) of matrix (b, s) at pivots[2 (b pivS + s)]
-cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, double *band, double *pivots, int pivS, cudaStream_t st);
+// vals: this grid's CSR values of problem 0, species s of problem b at vals + b vstride + s nnz (read by the slot kernel)
+bool band_needs_fill(const BandSpace &bs);      // false: the factorisation reads the CSR values itself (slot kernel)
+cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstride, const double *vals, size_t vstride, double *band,
+                               double *pivots, int pivS, cudaStream_t st);
 // xg: nullptr, or scratch of nb * S * n doubles for the permuted vectors when band_solve_smem(n, bw) exceeds an SM
 size_t band_solve_smem(int n, int bw);
 cudaError_t launch_band_solve(const BandSpace &bs, int nb, int S, size_t xstride, size_t pstride, const double *band, const double *rhs,
