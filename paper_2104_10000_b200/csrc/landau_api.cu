@@ -260,11 +260,9 @@ int resolve_pair_path(const landau_ctx *ctx, int path) {
 
 constexpr double FRONT_MAX_WORK_RATIO = 0.5;     // LANDAU_BAND_AUTO: front kernel when its flops are at most half the hull's
 constexpr size_t FRONT_SMEM_MAX = size_t(225) * 1024;        // + 1 KB the driver reserves per block
-constexpr size_t SLOT_SMEM_TWO_PER_SM = size_t(112) * 1024;  // two blocks of the slot kernel on an SM
-
-// Columns per block step of the FACTORISATION.  band_block(bw) unless that is 32 and the envelope is so jagged that the
-// slot kernel with 16-column blocks keeps two matrices per SM (config 5: fill + factor 14.2 -> 10.8 ms; where its
-// window needs an SM for itself -- the ten-species 320-cell mesh -- 32-column blocks with look-ahead stay ahead).  The
+// Columns per block step of the FACTORISATION.  band_block(bw) unless that is 32 and the envelope is jagged enough for the
+// slot kernel with 16-column blocks: its window must fit the shared memory of an SM (two windows per SM: 256 threads per
+// matrix, config 5: fill + factor 14.2 -> 7.4 ms; one window: 512 threads, ten-species 320-cell mesh 20.8 -> 13.6 ms).  The
 // solves keep band_block(bw) in either case: L and U do not depend on the blocking, and a 16-column solve of a band
 // that wide takes twice as long (config 5: 5.9 against 3.45 ms).
 int band_factor_block(const HostSpace &hs, const std::vector<int32_t> &perm, int bw) {
@@ -275,7 +273,7 @@ int band_factor_block(const HostSpace &hs, const std::vector<int32_t> &perm, int
     const int na16 = band_active_lists(int(hs.n), hs.rowptr, hs.colidx, perm, 16, ap, ai, &f16);
     int bw2 = 0;
     const double hull16 = band_envelope(int(hs.n), hs.rowptr, hs.colidx, perm, bw2, nullptr, nullptr, 16);
-    return band_slot_smem(16, na16) <= SLOT_SMEM_TWO_PER_SM && na16 <= 160 && f16 <= FRONT_MAX_WORK_RATIO * hull16 ? 16 : kb;
+    return band_slot_smem(16, na16) <= FRONT_SMEM_MAX && na16 <= 160 && f16 <= FRONT_MAX_WORK_RATIO * hull16 ? 16 : kb;
 }
 
 // Small batches are launch-latency bound: both gathers then go in one launch (3-7 us per single build); large

@@ -772,6 +772,12 @@ k_front_factor(int n, int W, int LDP, int LDW, int na_max, size_t mat_doubles, s
 // Named barriers: 2 = warp 0 has the block out of the window, 3 / 4 / 5 = among the workers.
 // ------------------------------------------------------------------------------------------------
 constexpr int SLOT_NO_DST = INT32_MIN;
+#ifndef SLOT_NT2
+#define SLOT_NT2 256
+#endif
+#ifndef SLOT_NT2_MIN_KB
+#define SLOT_NT2_MIN_KB 56
+#endif
 constexpr int SLOT_LB = 8;                     // band loads a worker thread keeps in flight when it assembles entering rows
 template <int KB, int NT>
 __global__ void __launch_bounds__(NT)
@@ -1334,7 +1340,14 @@ cudaError_t launch_band_factor(const BandSpace &bs, int nmat, int S, size_t pstr
     // the front family: 16-column blocks take the slot kernel (measured: ten-species 80-cell 9.1 -> 7.4 ms, mesh 3A 5.6 -> 4.3),
     // 32-column blocks the gather / scatter kernel (config 5: 14.2 against 18.7 ms with slots -- its look-ahead of the next
     // diagonal block and the smaller tile sweep outweigh the round trip of the window there)
-    if (!band_needs_fill(bs)) return slot_t<16, 128>(bs, nmat, S, pstride, vals, vstride, band, pivots, pivS, st);
+    if (!band_needs_fill(bs)) {
+        // threads per matrix by the windows that fit an SM: one -> 512, two -> SLOT_NT2, more -> 128 (small fronts: the
+        // steps are chains of latencies, more matrices per SM hide them better than more threads per matrix)
+        const size_t smem = band_slot_smem(bs.kb, bs.na_max);
+        if (smem > size_t(112) * 1024) return slot_t<16, 512>(bs, nmat, S, pstride, vals, vstride, band, pivots, pivS, st);
+        if (smem > size_t(SLOT_NT2_MIN_KB) * 1024) return slot_t<16, SLOT_NT2>(bs, nmat, S, pstride, vals, vstride, band, pivots, pivS, st);
+        return slot_t<16, 128>(bs, nmat, S, pstride, vals, vstride, band, pivots, pivS, st);
+    }
     if (bs.front) {
         switch (bs.kb) {
             case 32: return front_t<32, 512>(bs, nmat, S, pstride, band, pivots, pivS, st);

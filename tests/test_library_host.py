@@ -165,19 +165,18 @@ def test_front_lists_of_the_envelope_factorisation(binding, cfg):
 
 
 def test_factor_block_width_in_the_32_column_range(binding):
-    """Half-bandwidths in (256, 384] mean 32-column blocks for the solves; the factorisation takes 16-column blocks there
-    when two of its fronts fit an SM (mesh 3B of config 5: 96 rows beside the block) and stays at 32 when they do not
-    (the ten-species 320-cell mesh: 108 rows at 32 columns).  Flop and front sizes are reported for the width chosen."""
-    for cfg, want in ((5, 16), (7, 32)):
+    """Half-bandwidths in (256, 384] mean 32-column blocks for the solves; the factorisation takes 16-column blocks (slot
+    kernel) there when the envelope is jagged and the window of its largest front fits an SM: mesh 3B of config 5 (96
+    rows beside the block: two windows per SM) and the ten-species 320-cell mesh (99 rows: one).  Flop and front sizes
+    are reported for the width chosen."""
+    for cfg, rows in ((5, 96), (7, 99)):
         wl = inputs.config(cfg)
         hs = binding.landau_setup_host(wl.mesh, wl.order)
         bo = binding.landau_band_order_host(wl.mesh, wl.order)
         fr = binding.landau_band_front_host(wl.mesh, wl.order)
-        assert 256 < bo["bw"] <= 384 and bo["block_columns"] == want
-        assert bo["flop"] == _envelope_work(hs["rowptr"], hs["colidx"], bo["perm"], want)
-        assert fr["fits"] and fr["flop"] < 0.3 * bo["flop"]
-        if want == 16:
-            assert fr["rows_max"] <= 100
+        assert 256 < bo["bw"] <= 384 and bo["block_columns"] == 16
+        assert bo["flop"] == _envelope_work(hs["rowptr"], hs["colidx"], bo["perm"], 16)
+        assert fr["fits"] and fr["flop"] < 0.3 * bo["flop"] and fr["rows_max"] == rows
 
 
 def test_multigrid_argument_checks_need_no_gpu(binding):
