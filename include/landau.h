@@ -217,8 +217,8 @@ int landau_implicit_operator_batched(landau_ctx *ctx, int nb, const double *f_de
  * use and the flop of its outer-product updates inside the envelope.  Any output may be NULL.
  * Block widths: 16 columns up to a half-bandwidth of 256, 32 up to 384, 16 up to 832, 8 beyond (the panels of a step
  * must fit shared memory); in the 32-column range the FACTORISATION takes 16-column blocks instead when the envelope is
- * jagged enough for two of its fronts to share an SM (the slot kernel below), while the solves keep 32: L and U do not
- * depend on the blocking. */
+ * jagged and the window of its largest front fits the shared memory of an SM (the slot kernel below), while the solves
+ * keep 32: L and U do not depend on the blocking. */
 int landau_band_order_host(const landau_mesh *mesh, int order, int32_t *perm_host, int32_t *half_bandwidth,
                            int32_t *block_columns, double *flop_per_factorization);
 int landau_band_sizes(const landau_ctx *ctx, int grid, int32_t *half_bandwidth, int64_t *doubles_per_matrix,
