@@ -258,7 +258,13 @@ int resolve_pair_path(const landau_ctx *ctx, int path) {
     return tensor_bytes(ctx->Ntot) <= free_b / 4 ? LANDAU_PAIR_SHARED : LANDAU_PAIR_PER_PROBLEM;
 }
 
-constexpr double FRONT_MAX_WORK_RATIO = 0.5;     // LANDAU_BAND_AUTO: front kernel when its flops are at most half the hull's
+// LANDAU_BAND_AUTO: the gather / scatter front kernel when its flops are at most half the hull's (it pays a gather and a
+// scatter of its window per block step); the slot kernel -- no fill, no gather, no scatter -- whenever it does not do more
+// flops than the hull kernel: measured ahead even on the uniform 8 x 16 Q3 mesh, where front = hull (5.18 against 5.63 ms)
+constexpr double FRONT_MAX_WORK_RATIO = 0.5, SLOT_MAX_WORK_RATIO = 1.0;
+static bool auto_front(bool front_fits, bool slot, double front_flop, double hull_flop) {
+    return front_fits && front_flop <= (slot ? SLOT_MAX_WORK_RATIO : FRONT_MAX_WORK_RATIO) * hull_flop;
+}
 constexpr size_t FRONT_SMEM_MAX = size_t(225) * 1024;        // + 1 KB the driver reserves per block
 // Columns per block step of the FACTORISATION.  band_block(bw) unless that is 32 and the envelope is jagged enough for the
 // slot kernel with 16-column blocks: its window must fit the shared memory of an SM (two windows per SM: 256 threads per
@@ -505,7 +511,7 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
             G.front_fits = band_front_smem(kb, G.bs.na_max) <= FRONT_SMEM_MAX && G.bs.na_max <= 160 && kb >= 16;   // FRONT_IR rows per lane
             // AUTO: the front kernel pays a gather and a scatter of its window per block step; it wins where the envelope
             // is jagged (refined meshes: a sixth of the hull's flops), not on uniform meshes (front = hull)
-            G.bs.front = G.front_fits && G.bs.front_flop <= FRONT_MAX_WORK_RATIO * G.bs.flop_per_matrix;
+            G.bs.front = auto_front(G.front_fits, G.bs.slot, G.bs.front_flop, G.bs.flop_per_matrix);
         }
         UPC(G.bs.perm, perm)
         G.boff = ctx->bstride;
@@ -858,7 +864,7 @@ int landau_band_set_method(landau_ctx *ctx, int method) {
     for (auto &g : ctx->grids) {
         if (method == LANDAU_BAND_FRONT && !g.front_fits) return LANDAU_EINVAL;
         g.bs.front = method == LANDAU_BAND_HULL ? false
-                     : (method == LANDAU_BAND_FRONT ? true : g.front_fits && g.bs.front_flop <= FRONT_MAX_WORK_RATIO * g.bs.flop_per_matrix);
+                     : (method == LANDAU_BAND_FRONT ? true : auto_front(g.front_fits, g.bs.slot, g.bs.front_flop, g.bs.flop_per_matrix));
     }
     return LANDAU_OK;
 }

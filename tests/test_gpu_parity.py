@@ -286,11 +286,12 @@ def test_band_lu_solve_parity(gpu, oracle, cfg, variant, method):
 
 def test_band_lu_front_and_hull_kernels_agree_and_auto_chooses(gpu):
     """The two factorisation kernels give the same solution up to rounding (they eliminate the same entries; only
-    the order inside a rank-KB update differs); LANDAU_BAND_AUTO takes the front kernel on the refined meshes (its
-    flops are a sixth of the hull's) and the hull kernel on the uniform Q3 mesh (front = hull there); forcing the front
-    kernel where the largest front cannot fit shared memory is refused; both are bitwise reproducible."""
+    the order inside a rank-KB update differs); LANDAU_BAND_AUTO takes the front family on the refined meshes (its
+    flops are a sixth of the hull's) and, since the slot kernel needs neither fill nor gather nor scatter, also on the
+    uniform Q3 mesh (front = hull there); the hull kernel where the largest front cannot fit shared memory, and forcing
+    the front kernel there is refused; both are bitwise reproducible."""
     import torch
-    for cfg, variant, want in ((3, "B", FRONT), (6, "B", FRONT), (2, "B", HULL)):
+    for cfg, variant, want in ((3, "B", FRONT), (6, "B", FRONT), (2, "B", FRONT)):
         wl = inputs.config(cfg, variant=variant)
         ctx = gpu.LandauContext(wl.mesh, wl.order, wl.species, 2)
         assert ctx.band_method()[0] == want, (wl.name, ctx.band_method())
