@@ -803,12 +803,15 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
     const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
     const int g = lane >> 2, k = lane & 3;
     double pmin = 1.79e308, pmax = 0.0;
+    const int NSL = NS > 1 ? 32 - __clz(NS - 1) : 0;
 
     // assembly of the rows entering at `step` by the threads t = 0 .. nt-1 (list and slots of that step in la / ls, the
     // positions of the entering rows in ln): slot rows / columns zeroed, (after the caller's barrier) original entries loaded
     auto zero_new = [&](int nnew, const int *ls, const int *ln, int t, int nt) {
-        for (int e = t; e < nnew * NS; e += nt) {
-            const int sn = ls[ln[e / NS]], o = e % NS;
+        for (int e = t; e < (nnew << NSL); e += nt) {          // (entering row, slot) pairs, NS rounded up to 2^NSL: no division
+            const int o = e & ((1 << NSL) - 1);
+            if (o >= NS) continue;
+            const int sn = ls[ln[e >> NSL]];
             sW[sn + (size_t)o * LDW] = 0.0;
             sW[o + (size_t)sn * LDW] = 0.0;
         }
@@ -893,8 +896,16 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
         const int nn0 = kbn > 0 ? new_ptr[step + 1] : 0, nnew = kbn > 0 ? new_ptr[step + 2] - nn0 : 0;
         const double *sDs = smem + cur * DSZ, *sDi = sDs + KB * KB;     // the eliminated diagonal block (rows), 1 / pivots
         __syncthreads();                        // this step's front is in place, its diagonal block eliminated
-        for (int i = tid; i < nan; i += NT) { sActN[i] = act_idx[a1 + i]; sSlotN[i] = act_slot[a1 + i]; }
-        for (int i = tid; i < nnew; i += NT) sNew[i] = new_pos[nn0 + i];
+        // the next step's lists: asked for now, parked in shared memory after the substitutions (their latency off the chain)
+        constexpr int LPT = (160 + NT - 1) / NT;          // list items per thread (fronts of at most 160 rows)
+        int rAct[LPT], rSlot[LPT], rNew[LPT];
+#pragma unroll
+        for (int q = 0; q < LPT; ++q) {
+            const int i = tid + q * NT;
+            rAct[q] = i < nan ? act_idx[a1 + i] : 0;
+            rSlot[q] = i < nan ? act_slot[a1 + i] : 0;
+            rNew[q] = i < nnew ? new_pos[nn0 + i] : 0;
+        }
         // panel substitutions, one chain per thread: items [0, na) are rows of the L panel (x U11 = a, right-looking),
         // items [na, 2 na) columns of the U panel (L11 y = a, left-looking); sums in ascending index order
         for (int it = tid; it < 2 * na; it += NT) {
@@ -946,6 +957,12 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
                     sU[(size_t)c * LDP + i] = x[c];
                 }
             }
+        }
+#pragma unroll
+        for (int q = 0; q < LPT; ++q) {
+            const int i = tid + q * NT;
+            if (i < nan) { sActN[i] = rAct[q]; sSlotN[i] = rSlot[q]; }
+            if (i < nnew) sNew[i] = rNew[q];
         }
         __syncthreads();
         // window update over all slots: sW += (-L)(U), warp tiles of 32 rows x 16 columns as in the band kernel
