@@ -447,6 +447,22 @@ static int create_impl(const landau_mesh *meshes, int ngrids, const int32_t *spe
         ds.r = ctx->r + ds.poff; ds.z = ctx->z + ds.poff; ds.invr = ctx->invr + ds.poff;
         UPC(ds.w_in, hs.w_in) UPC(ds.w_out, hs.w_out) UPC(ds.invJ, hs.invJ)
         UPC(ds.B, hs.B) UPC(ds.E0, hs.E0) UPC(ds.E1, hs.E1)
+        ds.Me = ds.Ae = nullptr;
+        if (hs.Nb == 16) {     // element mass and advection matrices of the implicit-step operator (k_element_q3<true>)
+            std::vector<double> Me(size_t(hs.Ne) * 256), Ae(size_t(hs.Ne) * 256);
+            for (int64_t e = 0; e < hs.Ne; ++e)
+                for (int a = 0; a < 16; ++a)
+                    for (int bb = 0; bb < 16; ++bb) {
+                        double m = 0.0, ad = 0.0;
+                        for (int q = 0; q < 16; ++q) {
+                            const double w = hs.w_out[e * 16 + q], Bqa = hs.B[q * 16 + a];
+                            m = std::fma(w * Bqa, hs.B[q * 16 + bb], m);
+                            ad = std::fma(w * hs.invJ[2 * e + 1] * Bqa, hs.E1[q * 16 + bb], ad);
+                        }
+                        Me[(e * 16 + a) * 16 + bb] = m; Ae[(e * 16 + a) * 16 + bb] = ad;
+                    }
+            UPC(ds.Me, Me) UPC(ds.Ae, Ae)
+        }
         UPC(ds.lptr, hs.lptr) UPC(ds.ldof, hs.ldof) UPC(ds.lw, hs.lw)
         UPC(ds.rowptr, hs.rowptr) UPC(ds.colidx, hs.colidx)
         UPC(ds.gptr, hs.gptr) UPC(ds.gidx, hs.gidx) UPC(ds.gw, hs.gw)

@@ -525,12 +525,26 @@ k_element_q3(DeviceSpace ds, int rounds, const double *__restrict__ Gsum, double
         // species-independent coefficients at this lane's four q: w J^-1 G_D J^-T (rr, rz, zz), w J^-1 G_K (r, z)
         // (summing the pair kernel's slabs here instead of in k_sum_partials was measured slower for every batch size)
         const double ir = in[ELQ3_IN_J], iz = in[ELQ3_IN_J + 1];
-        double g0[4], g1[4], g2[4], g3[4], g4[4], wq[4];
+        // FULL: the mass and E-field advection parts of the operator are, per cell, fixed matrices times a scalar --
+        // M_e[a][b] = sum_q w_q B_qa B_qb and A_e[a][b] = sum_q w_q (J^-1)_zz B_qa E1_qb (tabulated at landau_create) -- so
+        // they are added to the C fragment (this lane's 2 x 2 x 2 entries) instead of being multiplied out again for every
+        // problem and species: half the tensor-core work of the implicit-step operator.
+        double2 mF[2][2], aF[2][2];
+        if (FULL) {
+            const double *Mp = ds.Me + (size_t)e * 256 + 2 * k, *Ap = ds.Ae + (size_t)e * 256 + 2 * k;
+#pragma unroll
+            for (int mt = 0; mt < 2; ++mt)
+#pragma unroll
+                for (int nt = 0; nt < 2; ++nt) {
+                    mF[mt][nt] = *reinterpret_cast<const double2 *>(Mp + (8 * mt + g) * 16 + 8 * nt);
+                    aF[mt][nt] = *reinterpret_cast<const double2 *>(Ap + (8 * mt + g) * 16 + 8 * nt);
+                }
+        }
+        double g0[4], g1[4], g2[4], g3[4], g4[4];
 #pragma unroll
         for (int ks = 0; ks < 4; ++ks) {
             const int q = 4 * ks + k;
             const double w = in[ELQ3_IN_W + q];
-            wq[ks] = w;
             g0[ks] = ir * ir * w * in[q];
             g1[ks] = ir * iz * w * in[16 + q];
             g2[ks] = iz * iz * w * in[32 + q];
@@ -541,7 +555,6 @@ k_element_q3(DeviceSpace ds, int rounds, const double *__restrict__ Gsum, double
             const double u = in[ELQ3_IN_U + 16 * sp + (lane & 15)];
             const double kf = sgn * ds.kfac[sp], df = sgn * ds.dfac[sp];
             double acc[2][2][2] = {};       // [mt][nt][2]
-            double accM[2][2][2] = {};      // mass part (FULL), kept apart: the element vector excludes it
 #pragma unroll
             for (int ks = 0; ks < 4; ++ks) {
                 const double drr = df * g0[ks], drz = df * g1[ks], dzz = df * g2[ks], kr = kf * g3[ks], kz = kf * g4[ks];
@@ -558,16 +571,16 @@ k_element_q3(DeviceSpace ds, int rounds, const double *__restrict__ Gsum, double
                         dmma884(acc[mt][nt], tE0[ks][mt], X[nt]);
                         dmma884(acc[mt][nt], tE1[ks][mt], Y[nt]);
                     }
-                if (FULL) {
-                    const double ca = wq[ks] * (ds.qm[sp] * ezb) * iz, cm = wq[ks] * shift;
+            }
+            if (FULL) {     // + (e_s m0 / m_s) E_z x the cell's advection matrix (geometry only: tabulated, see above)
+                const double ca = ds.qm[sp] * ezb;
 #pragma unroll
-                    for (int mt = 0; mt < 2; ++mt)
+                for (int mt = 0; mt < 2; ++mt)
 #pragma unroll
-                        for (int nt = 0; nt < 2; ++nt) {
-                            dmma884(acc[mt][nt], tB[ks][mt], ca * tE1[ks][nt]);
-                            dmma884(accM[mt][nt], tB[ks][mt], cm * tB[ks][nt]);
-                        }
-                }
+                    for (int nt = 0; nt < 2; ++nt) {
+                        acc[mt][nt][0] = fma(ca, aF[mt][nt].x, acc[mt][nt][0]);
+                        acc[mt][nt][1] = fma(ca, aF[mt][nt].y, acc[mt][nt][1]);
+                    }
             }
             // C fragment: lane holds rows a = 8 mt + g, columns b = 8 nt + 2 k + {0, 1}
             const size_t mat = ((size_t)b * ds.S + sp) * ds.Ne + e;
@@ -580,8 +593,8 @@ k_element_q3(DeviceSpace ds, int rounds, const double *__restrict__ Gsum, double
                 for (int mt = 0; mt < 2; ++mt) {
                     part[mt] = fma(acc[mt][nt][0], u0, fma(acc[mt][nt][1], u1, part[mt]));
                     double2 v;
-                    v.x = FULL ? acc[mt][nt][0] + accM[mt][nt][0] : acc[mt][nt][0];
-                    v.y = FULL ? acc[mt][nt][1] + accM[mt][nt][1] : acc[mt][nt][1];
+                    v.x = FULL ? fma(shift, mF[mt][nt].x, acc[mt][nt][0]) : acc[mt][nt][0];      // the mass part is kept out of
+                    v.y = FULL ? fma(shift, mF[mt][nt].y, acc[mt][nt][1]) : acc[mt][nt][1];      // acc: the element vector excludes it
                     *reinterpret_cast<double2 *>(C + (8 * mt + g) * 16 + 8 * nt + 2 * k) = v;
                 }
             }

@@ -25,6 +25,7 @@ struct DeviceSpace {
     long long fstride;
     const double *r, *z, *invr, *w_in, *w_out;  // [N]
     const double *invJ;                          // [Ne][2]
+    const double *Me, *Ae;                       // Q3 only, [Ne][16][16]: sum_q w_q B_qa B_qb and sum_q w_q (2/hz) B_qa E1_qb (k_element_q3<true>)
     const double *B, *E0, *E1;                   // [Nq][Nb]
     const int32_t *lptr, *ldof; const double *lw;
     const int32_t *rowptr, *colidx;
