@@ -238,7 +238,9 @@ constexpr int BAND_THREADS = 512;
 #endif
 // threads per matrix in the solves (measured: bw = 339: 384 threads 4.2 ms, 256: 4.8, 512: 5.8; bw = 178: 64 threads 2.5 ms,
 // 256: 3.9, 512: 7.6 -- the solves are latency-bound, small blocks leave room for more matrices per SM)
-constexpr int SOLVE_NT32 = 384, SOLVE_NT16 = 64;
+// (after the solves were confined to the envelope and compiled for seven blocks per SM, bw = 278: 288 threads 2.45 ms,
+// 256: 2.47, 224: 2.69, 192: 2.91)
+constexpr int SOLVE_NT32 = 288, SOLVE_NT16 = 64;
 constexpr int WT = 32, WTJ = 16;   // warp tile of the window update: 32 rows x 16 columns = 4 x 2 mma tiles of 8 x 8
 
 // 1/x: MUFU seed and two Newton steps (full double precision up to rounding of the last step)
@@ -1049,8 +1051,11 @@ k_slot_factor(int n, int W, int LDP, int LDW, int NS, size_t mat_doubles, size_t
 
 // XG: the permuted vector of a matrix lives in global memory (xg + matrix * n) instead of shared memory -- for
 // orders n beyond the 227 KB of an SM (n > ~28,000); the block barriers order those accesses just the same.
+// The 32-column instantiation is compiled for seven blocks per SM (32 registers, 16 bytes of spill): the solves are chains
+// of short phases, what counts is how many matrices an SM holds -- config 5: 1,024 matrices were two waves on 148 x 5
+// places (3.54 ms), they are one on 148 x 7 (2.45 ms); 1,280 matrices of the ten-species 320-cell mesh 5.43 -> 4.76 ms.
 template <int KB, int NT, bool XG>
-__global__ void __launch_bounds__(NT)
+__global__ void __launch_bounds__(NT, KB == 32 ? 7 : 1)
 k_band_solve(int n, int W, size_t mat_doubles, size_t xstride, int S, const int32_t *__restrict__ perm,
              const int32_t *__restrict__ mlow, const int32_t *__restrict__ mup, const int32_t *__restrict__ first, size_t pstride,
              const double *__restrict__ band_all, const double *rhs, double *xout, double *xg) {     // xout may alias rhs (in-place solve): no __restrict__ on these two
